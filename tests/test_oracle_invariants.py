@@ -1,0 +1,220 @@
+"""Exact (bitwise) invariants of the oracle — SURVEY.md §8(c) "Exact invariants".
+
+Each one is a property the mathematics fixes, so a slip in the corresponding part of the
+oracle (a neighbour index, the back-bond J_d(i-e_d), the multi-hit counter, the colour
+rule) breaks it.
+"""
+import numpy as np
+import pytest
+
+import ising_workloads as W
+
+BETA_C = 0.4406868
+
+
+def state(o, r=0):
+    E, M = o.observables()
+    return int(E[r]), int(M[r]), o.hash(r)
+
+
+@pytest.mark.parametrize("dim,L", [(2, 2), (2, 4), (2, 16), (3, 2), (3, 4), (3, 8)])
+def test_ground_state_energy(orc, dim, L):
+    """E(all +1) = -dim·N for J = +1 (north_star: -2N in 2D, -3N in 3D); M = N."""
+    o = orc.Oracle(dim, L, seed=1)
+    o.set_spins(np.ones(L ** dim, dtype=np.int8))
+    E, M = o.observables()
+    assert (int(E[0]), int(M[0])) == (-dim * L ** dim, L ** dim)
+    # β = 40: every proposed flip costs ΔE > 0 and thr = 0 ⇒ nothing moves
+    o.sweep(40.0, 3, 2, 2)
+    assert state(o)[:2] == (-dim * L ** dim, L ** dim)
+
+
+def test_energy_definition_against_numpy(orc):
+    """E and M of a random state vs the definition written with numpy rolls (2D, 3D, ±J)."""
+    for dim, L in [(2, 12), (3, 6)]:
+        J = W.couplings(dim, L, 9)
+        o = orc.Oracle(dim, L, seed=5, J=J)
+        s = o.spins().astype(np.int64).reshape((L,) * dim)          # [z,]y,x
+        Jd = J.astype(np.int64).reshape((dim,) + (L,) * dim)
+        E = 0
+        for d in range(dim):
+            ax = dim - 1 - d                                       # e_0 = x is the last axis
+            E -= int((Jd[d] * s * np.roll(s, -1, axis=ax)).sum())
+        assert state(o)[:2] == (E, int(s.sum()))
+
+
+def test_parity_of_E_and_M(orc):
+    """Every flip changes E by a multiple of 4 and M by 2."""
+    o = orc.Oracle(2, 16, seed=3)
+    E0, M0, _ = state(o)
+    E, M = o.sweep_series(BETA_C, 50, 4, 2)
+    assert np.all((E[:, 0] - E0) % 4 == 0) and np.all((M[:, 0] - M0) % 2 == 0)
+    assert np.all((E[:, 0] + 2 * 256) % 4 == 0)   # E ≡ -dim·N (mod 4) for J = +1
+
+
+@pytest.mark.parametrize("dim,L,tile,k", [(2, 16, 4, 3), (2, 16, 16, 1), (3, 8, 4, 2)])
+def test_sweep_is_additive_and_reproducible(orc, dim, L, tile, k):
+    """sweep(a); sweep(b) ≡ sweep(a+b); same seed ⇒ same bits; the counter advances by n·k."""
+    beta = 0.3
+    a = orc.Oracle(dim, L, seed=77)
+    b = orc.Oracle(dim, L, seed=77)
+    a.sweep(beta, 3, tile, k)
+    a.sweep(beta, 4, tile, k)
+    b.sweep(beta, 7, tile, k)
+    assert state(a) == state(b)
+    assert a.counter == b.counter == 7 * k
+    c = orc.Oracle(dim, L, seed=78)
+    c.sweep(beta, 7, tile, k)
+    assert state(c)[2] != state(a)[2]
+    # resume from a checkpoint: spins + counter are the whole state (RNG is stateless)
+    d = orc.Oracle(dim, L, seed=77)
+    d.sweep(beta, 3, tile, k)
+    e = orc.Oracle(dim, L, seed=77)
+    e.set_spins(d.spins())
+    e.counter = d.counter
+    e.sweep(beta, 4, tile, k)
+    assert state(e) == state(a)
+
+
+def test_series_equals_observables_after_each_pass(orc):
+    a = orc.Oracle(2, 8, seed=5)
+    b = orc.Oracle(2, 8, seed=5)
+    E, M = a.sweep_series(BETA_C, 6, 4, 2)
+    for p in range(6):
+        b.sweep(BETA_C, 1, 4, 2)
+        assert state(b)[:2] == (int(E[p, 0]), int(M[p, 0]))
+
+
+@pytest.mark.parametrize("dim,L,tile,k", [(2, 16, 4, 2), (2, 24, 6, 1), (3, 8, 2, 2)])
+def test_tile_order_is_irrelevant(orc, dim, L, tile, k):
+    """Tiles of one coarse colour are independent: visiting them in reverse order
+    gives the same bits.  Fails if the coarse colouring lets two updated tiles touch."""
+    a = orc.Oracle(dim, L, seed=9)
+    b = orc.Oracle(dim, L, seed=9)
+    b.set_tile_order(True)
+    a.sweep(0.35, 5, tile, k)
+    b.sweep(0.35, 5, tile, k)
+    assert state(a) == state(b)
+
+
+def test_tile_size_changes_the_trajectory_but_k1_full_tile_is_plain(orc):
+    """SURVEY §8(c) reading 5: double checkerboard with k=1 is a different (valid) chain than
+    the plain checkerboard; tile = L and tile = 0 are the same thing."""
+    a = orc.Oracle(2, 16, seed=4); a.sweep(BETA_C, 3, 16, 1)
+    b = orc.Oracle(2, 16, seed=4); b.sweep(BETA_C, 3, 0, 1)
+    c = orc.Oracle(2, 16, seed=4); c.sweep(BETA_C, 3, 4, 1)
+    assert state(a) == state(b)
+    assert state(a)[2] != state(c)[2]
+
+
+def test_plain_checkerboard_against_lattice_synchronous_numpy(orc):
+    """tile = L, J = +1: one half-sweep is a synchronous update of one colour.  Restated with
+    whole-array numpy operations and random words fetched per site from the oracle's Philox
+    (so only the schedule/neighbour/acceptance logic is re-derived here, in a different shape)."""
+    L, seed, beta = 8, 13, 0.37
+    o = orc.Oracle(2, L, seed=seed)
+    s = o.spins().astype(np.int64).reshape(L, L)
+    thr = orc.thresholds(beta, 2)
+    y, x = np.mgrid[0:L, 0:L]
+    idx = x + L * y
+    for t in range(4):
+        for c in (0, 1):
+            H = 2 * t + c
+            r = np.zeros((L, L), dtype=np.uint64)
+            for i in range(L * L):
+                p = i >> 1
+                r.flat[i] = orc.philox4x32_10([p >> 2, 0, H & 0xFFFFFFFF, H >> 32], [seed, 0])[p & 3]
+            nb = np.roll(s, 1, 0) + np.roll(s, -1, 0) + np.roll(s, 1, 1) + np.roll(s, -1, 1)
+            a = s * nb
+            t_sel = np.where(a == 2, thr[0], np.where(a == 4, thr[1], 0)).astype(np.uint64)
+            flip = ((a <= 0) | (r < t_sel)) & (((x + y) & 1) == c)
+            s = np.where(flip, -s, s)
+    o.sweep(beta, 4, L, 1)
+    assert np.array_equal(o.spins().astype(np.int64).reshape(L, L), s)
+
+
+@pytest.mark.parametrize("dim,L,tile,k", [(2, 16, 4, 2), (3, 6, 6, 1)])
+def test_z2_symmetry(orc, dim, L, tile, k):
+    """Start from -s0 ⇒ trajectory -s_t: same E, opposite M (the update depends on s_i·field)."""
+    a = orc.Oracle(dim, L, seed=21)
+    b = orc.Oracle(dim, L, seed=21)
+    b.set_spins(-a.spins())
+    a.sweep(0.3, 6, tile, k)
+    b.sweep(0.3, 6, tile, k)
+    assert np.array_equal(a.spins(), -b.spins())
+    assert state(a)[0] == state(b)[0] and state(a)[1] == -state(b)[1]
+
+
+@pytest.mark.parametrize("dim,L,tile,k", [(2, 16, 4, 2), (2, 8, 8, 1), (3, 8, 4, 1)])
+def test_gauge_invariance_mattis(orc, dim, L, tile, k):
+    """J'_d(i) = ε_i ε_(i+e_d) J_d(i), start ε·s0 ⇒ trajectory ε·s_t and the same E series.
+    With J = +1 this is the Mattis model: exercises the whole coupling path (forward bond
+    J_d(i), back bond J_d(i-e_d), the d-major layout) against the ferromagnet."""
+    N = L ** dim
+    rng = np.random.default_rng(5)
+    eps = (1 - 2 * rng.integers(0, 2, N)).astype(np.int8)
+    e = eps.reshape((L,) * dim)
+    for J0 in (None, W.couplings(dim, L, 17)):
+        Jp = np.empty((dim,) + (L,) * dim, dtype=np.int8)
+        for d in range(dim):
+            base = 1 if J0 is None else J0.reshape((dim,) + (L,) * dim)[d]
+            Jp[d] = e * np.roll(e, -1, axis=dim - 1 - d) * base
+        a = orc.Oracle(dim, L, seed=33, J=J0)
+        b = orc.Oracle(dim, L, seed=33, J=Jp.reshape(-1))
+        b.set_spins(a.spins() * eps)
+        Ea, _ = a.sweep_series(0.5, 5, tile, k)
+        Eb, _ = b.sweep_series(0.5, 5, tile, k)
+        assert np.array_equal(Ea, Eb)
+        assert np.array_equal(a.spins() * eps, b.spins())
+
+
+def test_unit_couplings_equal_null(orc):
+    a = orc.Oracle(2, 16, seed=3)
+    b = orc.Oracle(2, 16, seed=3, J=np.ones(2 * 256, dtype=np.int8))
+    a.sweep(BETA_C, 4, 4, 2)
+    b.sweep(BETA_C, 4, 4, 2)
+    assert state(a) == state(b)
+
+
+def test_replicas_are_independent_runs_sharing_J(orc):
+    """A batched handle equals R single handles (realisations worked on concurrently)."""
+    J = W.couplings(2, 16, 5)
+    seeds = [100, 101, 102]
+    b = orc.Oracle(2, 16, seeds=seeds, J=J)
+    b.sweep(1.0, 5, 4, 4)
+    singles = []
+    for r, sd in enumerate(seeds):
+        o = orc.Oracle(2, 16, seed=sd, J=J)
+        o.sweep(1.0, 5, 4, 4)
+        assert state(o) == state(b, r)
+        singles.append(o.spins().astype(np.int64))
+    assert b.overlap(0, 2) == int((singles[0] * singles[2]).sum())
+    assert b.overlap(1, 1) == 256
+
+
+def test_argument_checks(orc):
+    o = orc.Oracle(2, 16, seed=1)
+    for tile in (3, 5, 16 // 1 + 2, 6):       # odd, not a divisor
+        with pytest.raises(ValueError):
+            o.sweep(0.4, 1, tile, 1)
+    o12 = orc.Oracle(2, 12, seed=1)
+    with pytest.raises(ValueError):
+        o12.sweep(0.4, 1, 4, 1)               # L/T = 3 odd: periodic coarse colouring impossible
+    with pytest.raises(ValueError):
+        o.sweep(0.4, 1, 4, 0)
+    with pytest.raises(ValueError):
+        o.sweep(-1.0, 1, 4, 1)
+    with pytest.raises(ValueError):
+        orc.Oracle(2, 7, seed=1)
+    with pytest.raises(ValueError):
+        orc.Oracle(4, 8, seed=1)
+
+
+def test_hot_start_is_unbiased_and_seeded(orc):
+    o = orc.Oracle(2, 256, seed=123456789012345)
+    s = o.spins().astype(np.int64)
+    assert abs(s.sum()) < 5 * 256
+    assert abs((s[:-1] * s[1:]).sum()) < 5 * 256
+    assert not np.array_equal(s, orc.Oracle(2, 256, seed=123456789012346).spins())
+    # hi word of the seed is part of the key
+    assert not np.array_equal(orc.Oracle(2, 8, seed=1).spins(), orc.Oracle(2, 8, seed=1 + 2 ** 32).spins())
