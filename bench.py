@@ -1,0 +1,272 @@
+#!/usr/bin/env python
+"""bench.py — spin flips per ns of the double-checkerboard Metropolis sweep (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--layout int8|bits] [--tile 32|64] [--k 1|4|16] [--L 16384] [--no-extras]
+
+One "step" = one outer pass of the whole hot path (colour-0 launch + colour-1 launch, k inner
+sweeps each) over the 2D L=16384 lattice of BASELINE.json config 3 (seed 3, beta = 0.4406868),
+spins resident in HBM.  `value` = attempted flips per ns = K * k * L^2 / t (time per attempted
+flip, measurement of E/M excluded).  Multi-GPU (`--gpus N` under torchrun): the path does not shard
+by contract (north_star: one GPU), so N ranks run N independent replicas ("replicas only", DESIGN.md
+§8) and `value` is the aggregate.  `--impl reference` times the CPU oracle (test infrastructure) on a
+bounded sample of the same workload; it is the only place besides `cpu_baseline` that touches oracle/.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+import numpy as np  # noqa: E402
+
+import ising_workloads as W  # noqa: E402
+
+METRIC = "spin flips/ns (2D Ising L=16384, beta_c)"
+UNIT = "flips/ns"
+
+
+def algorithmic_bytes_per_flip(tile: int, k: int, layout: str) -> float:
+    """read s(1 + 2*dim/T) + write s per site per pass, / k; s = 1 B int8, 1/8 B bits."""
+    s = 1.0 if layout == "int8" else 0.125
+    return s * (2.0 + 4.0 / tile) / k
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._pump, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [r for r in self.rows if t0 - 0.05 <= r[0] <= t1 + 0.15] or self.rows
+        for _, line in rows:
+            f = [x.strip() for x in line.split(",")]
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except Exception:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_flips_per_ns(L: int, tile: int, k: int, passes: int):
+    """Time the CPU oracle as it stands: `passes` outer passes on an L x L lattice, 1 core."""
+    from oracle import oracle as O
+    O.build()
+    o = O.Oracle(2, L, seed=3)
+    t0 = time.perf_counter()
+    o.sweep(W.BETA_C_2D, passes, tile, k)
+    dt = time.perf_counter() - t0
+    return passes * k * L * L / dt / 1e9, dt
+
+
+def run_reference(a, rank: int, world: int) -> None:
+    if rank != 0:
+        return
+    Ls = 4096                                   # bounded sample: 1/16 of the L=16384 sites per step
+    per_step = []
+    for i in range(a.warmup + a.steps):
+        v, dt = oracle_flips_per_ns(Ls, a.tile, a.k, 1)
+        if i >= a.warmup:
+            per_step.append(dt)
+    tot = sum(per_step)
+    val = a.steps * a.k * Ls * Ls / tot / 1e9
+    sample = f"each step = one outer pass (tile {a.tile}, k {a.k}, beta_c) of a {Ls}x{Ls} hot-start lattice, seed 3"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": a.gpus, "steps": a.steps,
+            "warmup": a.warmup, "ms_per_step": 1e3 * tot / a.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int8", "data": "synthetic",
+            "config": {"workload": f"BASELINE config 3: 2D Ising L=16384 {a.layout} tile={a.tile} k={a.k} (oracle on a bounded sample)"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line), flush=True)
+
+
+def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None):
+    """Device-timed throughput of one (layout, tile, k) variant; returns dict."""
+    g = P.Ising(2, L, seed=3)
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.sweep(W.BETA_C_2D, warmup, tile, k)
+    g.synchronize()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    n0 = P.ising_kernel_launches()
+    t0 = time.time()
+    if sampler:
+        sampler.start()
+        time.sleep(0.25)
+        t0 = time.time()
+    e0.record()
+    g.sweep(W.BETA_C_2D, steps, tile, k)        # K passes = 2K launches, no host sync in between
+    e1.record()
+    torch.cuda.synchronize()
+    t1 = time.time()
+    ms = e0.elapsed_time(e1)
+    clocks = sampler.stop(t0, t1) if sampler else None
+    launches = P.ising_kernel_launches() - n0
+    path = g.sweep_path()
+    g.destroy()
+    flips = steps * k * L * L
+    return {"ms": ms, "flips_per_ns": flips / (ms * 1e6), "launches": int(launches), "path": path, "clocks": clocks}
+
+
+def time_e2e(P, torch, L, layout, tile, k, steps):
+    """Same metric through the public API with HOST buffers: every step uploads the spins from
+    pinned host memory (ising_set_spins), runs one pass, and reads them back (ising_copy_spins)."""
+    g = P.Ising(2, L, seed=3)
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    host = torch.empty(L * L, dtype=torch.int8).pin_memory()
+    g.copy_spins(host)
+    g.sweep(W.BETA_C_2D, 1, tile, k)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        g.set_spins(host)
+        g.sweep(W.BETA_C_2D, 1, tile, k)
+        g.copy_spins(host)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    g.destroy()
+    return {"value": steps * k * L * L / (ms * 1e6), "unit": UNIT, "h2d_bytes_per_step": L * L,
+            "d2h_bytes_per_step": L * L, "steps": steps}
+
+
+def main() -> None:
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--layout", default="int8", choices=["int8", "bits"])
+    ap.add_argument("--tile", type=int, default=64)
+    ap.add_argument("--k", type=int, default=1)
+    ap.add_argument("--L", type=int, default=16384)
+    ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the k/tile table")
+    a = ap.parse_args()
+    a.warmup = max(a.warmup, 3) if a.impl == "ours" else a.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if a.impl == "reference":
+        run_reference(a, rank, world)
+        return
+
+    import torch
+    import paper_1006_3865_b200 as P
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device — the product has no CPU path")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    P.use_torch()
+    L = a.L
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    res = time_variant(P, torch, L, a.layout, a.tile, a.k, a.steps, a.warmup, sampler)
+    barrier()
+    ms = res["ms"]
+    if dist is not None:
+        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    flips = world * a.steps * a.k * L * L
+    value = flips / (ms * 1e6)
+
+    peak, peak_src, _ = measured_peaks()
+    bpf = algorithmic_bytes_per_flip(a.tile, a.k, a.layout)
+    launches_per_step = 2
+    bytes_per_launch = bpf * a.k * L * L / launches_per_step
+    launch_ms = res["ms"] / (a.steps * launches_per_step)
+    achieved = bytes_per_launch / (launch_ms * 1e6)            # GB/s
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+            "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u8" if a.layout == "int8" else "u32 bit-planes", "data": "synthetic",
+            "config": {"workload": f"BASELINE config 3: 2D Ising L={L} hot start seed 3 beta=0.4406868 layout={a.layout} "
+                                   f"tile={a.tile} k={a.k}; one step = one outer pass (2 launches)",
+                       "l2": "lattice (256 MiB int8) exceeds the 126 MB L2; no explicit flush" if a.layout == "int8"
+                             else "lattice (32 MiB bits) fits L2: bit-packed variant is ALU-bound, not an HBM claim",
+                       "kernel_path": res["path"], "parallelism": "replicas only" if world > 1 else "single GPU"},
+            "ns_per_flip": 1.0 / value, "gpu_launches": res["launches"], "clocks": res["clocks"],
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
+                         "algorithmic_bytes_per_flip": bpf, "kernel": f"k_tile_{'i8' if a.layout == 'int8' else 'bits'}<{a.tile}>",
+                         "avg_launch_ms": launch_ms}}
+    if rank == 0 and not a.no_extras and world == 1:
+        table = {}
+        for lay in ("int8",):
+            for T in (32, 64):
+                for k in (1, 4, 16):
+                    st = max(2, min(a.steps, 40 // k))
+                    r = time_variant(P, torch, L, lay, T, k, st, 3)
+                    table[f"{lay}_t{T}_k{k}"] = {"flips_per_ns": round(r["flips_per_ns"], 1), "steps": st,
+                                                "hbm_GBs": round(r["flips_per_ns"] * algorithmic_bytes_per_flip(T, k, lay), 1)}
+        line["variants"] = table
+        line["e2e"] = time_e2e(P, torch, L, a.layout, a.tile, a.k, 3)
+        ncores = 1
+        v, dt = oracle_flips_per_ns(L, a.tile, a.k, 2)
+        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": ncores, "kind": "oracle",
+                                "sample": f"2 outer passes of the full L={L} lattice (tile {a.tile}, k {a.k}), {dt:.1f} s, "
+                                          f"host has {os.cpu_count()} cores, oracle is sequential"}
+    elif rank == 0:
+        line["e2e"] = None
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -1,0 +1,138 @@
+/* ising.h — C ABI of libising_b200: the double-checkerboard Metropolis sweep of
+ * arXiv 1006.3865 (M. Weigel, "Simulating spin models on GPU") on one B200 (sm_100a).
+ *
+ * Citations: P:n = line n of the paper text; S8c.k = item k of the normative
+ * specification in SURVEY.md §8(c), restated with every reading in DESIGN.md §3.
+ *
+ * Model (eq. (1)): spins s_i = ±1 on a periodic square (dim 2) or simple cubic
+ * (dim 3) lattice of edge L, H = -Σ_<ij> J_ij s_i s_j.  A proposed flip is accepted with
+ * p = min[1, exp(-β ΔE)] (eq. (2)).  The update order is the double checkerboard of
+ * tiles of T^dim sites coloured even/odd, sites coloured even/odd, even first at
+ * both levels, k inner sweeps per tile visit ("multi-hit").
+ *
+ * Conventions common to every call
+ *   - Site index i = x + L*(y + L*z); canonical spin array = N = L^dim int8 values ±1 in
+ *     index order, replica-major when the handle holds R > 1 replicas (R*N bytes).
+ *   - Every pointer argument marked [host|device] may be either; the library asks the CUDA
+ *     runtime which it is.  Caller owns all argument buffers; the library owns the handle.
+ *   - Return value 0 = success, negative ISING_E* = failure (message: ising_last_error()).
+ *     ising_create* return NULL on failure.  No C++ exception crosses this boundary.
+ *   - All work is issued on the stream set by ising_set_device_hooks (default stream 0).
+ *     ising_sweep is asynchronous; calls that hand data back to the caller synchronise that
+ *     stream before returning.
+ *   - A handle is not thread-safe; distinct handles are independent.
+ *   - There is no CPU fallback: without a CUDA device every compute call fails with
+ *     ISING_ECUDA.
+ */
+#ifndef ISING_B200_H
+#define ISING_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct ising_ctx* ising_handle;
+
+enum {
+    ISING_OK = 0,
+    ISING_EINVAL = -1,       /* bad argument (message says which)                    */
+    ISING_ENOMEM = -2,       /* device allocation failed                              */
+    ISING_ECUDA = -3,        /* CUDA runtime / launch error, or no device            */
+    ISING_EUNSUPPORTED = -4  /* valid request this library has no kernel for         */
+};
+
+enum {
+    ISING_LAYOUT_I8 = 0,     /* one byte per spin in HBM (default)                    */
+    ISING_LAYOUT_BITS = 1    /* one bit per spin in HBM (synchronous multi-spin form) */
+};
+
+/* ising_create — P:53-57; S8c.1-3.
+ * dim ∈ {2,3}; L even, ≥ 2, N = L^dim ≤ 2^32.  coupling_or_null [host|device]: NULL ⇒
+ * J = +1 on every bond (eq. (1)); otherwise int8 J[dim][N], J[d][i] = bond between site i
+ * and i + e_d, every value ±1 (else NULL is returned); the array is copied.  seed = 64-bit
+ * Philox4x32-10 key: the hot start s_i = sign bit of Philox(ctr={i>>2,1,0,0})[i&3] and the
+ * sweep stream both derive from it.  The inner-sweep counter t starts at 0. */
+ising_handle ising_create(int dim, int L, const int8_t* coupling_or_null, uint64_t seed);
+
+/* ising_create_batch — P:100 ("many disorder realizations concurrently"); S8c item 12.
+ * n_replicas ≥ 1 independent spin systems (seeds[r], host pointer) sharing one coupling
+ * array, advanced together by every ising_sweep (one batched launch per phase). */
+ising_handle ising_create_batch(int dim, int L, const int8_t* coupling_or_null,
+                                const uint64_t* seeds, int n_replicas);
+
+void ising_destroy(ising_handle h);
+
+/* ising_sweep — P:64-74 (steps 1-7 and the k-fold multi-hit); S8c.4-6.
+ * n_sweeps ≥ 0 outer passes.  One pass = all tiles of coarse colour 0, then colour 1; each
+ * tile visit runs k_inner ≥ 1 times (even sites, then odd sites) with its halo frozen.
+ * tile = edge T: T even, T | L, and L/T even or T == L; 0 means T = L (the single
+ * checkerboard of P:62).  beta finite, ≥ 0.  Acceptance is the integer test
+ * r < floor(exp(-β ΔE)·2^32), table built in double on the host (S8c.4).  Half-sweep
+ * H = 2t + colour uses r = Philox(ctr={p>>2,0,lo32 H,hi32 H}, key=seed)[p&3], p = i>>1.
+ * Advances t by n_sweeps·k_inner.  Asynchronous. */
+int ising_sweep(ising_handle h, double beta, int n_sweeps, int tile, int k_inner);
+
+/* ising_sweep_series — same as ising_sweep, and after every outer pass writes
+ * E[pass*R + r], M[pass*R + r] (n_sweeps·R int64 each, [host|device], either may be NULL).
+ * Synchronises when an output is a host pointer. */
+int ising_sweep_series(ising_handle h, double beta, int n_sweeps, int tile, int k_inner,
+                       int64_t* E, int64_t* M);
+
+/* ising_observables — P:86 (E and M are measured but not timed); S8c.7.
+ * E[r] = -Σ_i Σ_{d<dim} J_d(i) s_i s_(i+e_d),  M[r] = Σ_i s_i, exact int64, r < R.
+ * E, M [host|device], either may be NULL.  Synchronises. */
+int ising_observables(ising_handle h, int64_t* E, int64_t* M);
+
+/* ising_overlap — replica overlap Q_ab = Σ_i s_i^a s_i^b (q = Q/N); S8c.7. */
+int ising_overlap(ising_handle h, int a, int b, int64_t* Q);
+
+/* ising_copy_spins — canonical int8 ±1 spins, R·N bytes, to dst [host|device]. Synchronises. */
+int ising_copy_spins(ising_handle h, int8_t* dst);
+
+/* ising_set_spins — overwrite the spins from canonical int8 ±1 (R·N bytes, [host|device]);
+ * any other value ⇒ ISING_EINVAL and the state is unchanged.  Does not touch t. */
+int ising_set_spins(ising_handle h, const int8_t* src);
+
+/* ising_set_layout — ISING_LAYOUT_I8 or ISING_LAYOUT_BITS: how spins are held in HBM between
+ * sweeps.  The trajectory does not depend on it (S8c: both layouts give the same bits). */
+int ising_set_layout(ising_handle h, int layout);
+
+/* The state of a run is (spins, t, seed): the random stream is stateless (S8c.3), so
+ * copy_spins + get_counter / set_spins + set_counter resume a run bit-exactly. */
+int ising_get_counter(ising_handle h, uint64_t* t);
+int ising_set_counter(ising_handle h, uint64_t t);
+
+/* ising_thresholds — the acceptance table of S8c.4 as the library builds it:
+ * out[m-1] = floor(exp(-β·4m)·2^32) for m = 1..dim, 0 beyond (host pointer, 3 entries). */
+int ising_thresholds(double beta, int dim, uint64_t* out);
+
+/* ising_set_device_hooks — process-wide.  alloc(bytes) returns a device pointer (or NULL),
+ * dealloc(ptr) releases it; cuda_stream is a cudaStream_t.  NULL alloc/dealloc restore
+ * cudaMalloc/cudaFree.  Existing handles keep (and later release through dealloc at the
+ * time of destroy) what they already hold, so set the hooks before creating handles. */
+int ising_set_device_hooks(void* (*alloc)(size_t), void (*dealloc)(void*), void* cuda_stream);
+
+/* ising_synchronize — wait for all work issued for this handle. */
+int ising_synchronize(ising_handle h);
+
+/* ising_kernel_launches — number of kernels this library has launched in this process
+ * (bench.py's gpu_launches). */
+uint64_t ising_kernel_launches(void);
+
+/* ising_sweep_path — name of the kernel family the last ising_sweep on h used
+ * ("generic", "tile_i8", "tile_bits", ...); static string, never NULL. */
+const char* ising_sweep_path(ising_handle h);
+
+/* ising_force_path — testing aid: 0 = automatic kernel choice, 1 = always the generic
+ * global-memory kernels. */
+int ising_force_path(ising_handle h, int generic_only);
+
+const char* ising_last_error(void); /* thread-local, never NULL */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ISING_B200_H */

@@ -1,0 +1,10 @@
+"""paper_1006_3865_b200 — B200-native double-checkerboard Metropolis sweep (arXiv 1006.3865).
+
+The product is the C-ABI library `libising_b200.so` (include/ising.h, csrc/*.cu, sm_100a);
+`binding` marshals arguments to it.  Nothing in this package imports `oracle/`.
+"""
+from .binding import (ISING_LAYOUT_BITS, ISING_LAYOUT_I8, SYMBOLS, Ising, IsingError,
+                      ising_kernel_launches, ising_thresholds, lib, use_torch)
+
+__all__ = ["Ising", "IsingError", "ISING_LAYOUT_I8", "ISING_LAYOUT_BITS", "SYMBOLS", "lib",
+           "use_torch", "ising_thresholds", "ising_kernel_launches"]

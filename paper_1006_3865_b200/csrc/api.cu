@@ -1,0 +1,417 @@
+// api.cu — the C ABI of include/ising.h: argument checking, the host-side acceptance table
+// (a2), storage-layout bookkeeping and kernel-path selection.  All compute is in the
+// kernels of generic.cu / tile_i8.cu / tile_bits.cu; there is no CPU path.
+#include <cmath>
+#include <cstdarg>
+#include <cstring>
+#include <atomic>
+#include <new>
+
+#include "kernels.h"
+
+namespace ising {
+
+static thread_local char g_err[512] = "";
+static std::atomic<uint64_t> g_launches{0};
+
+Hooks& hooks() {
+    static Hooks h;
+    return h;
+}
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof g_err, fmt, ap);
+    va_end(ap);
+}
+
+void count_launch(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+
+void* dev_alloc(size_t bytes) {
+    if (bytes == 0) bytes = 16;
+    void* p = nullptr;
+    if (hooks().alloc) {
+        p = hooks().alloc(bytes);
+        if (!p) set_error("device allocation hook returned NULL for %zu bytes", bytes);
+        return p;
+    }
+    cudaError_t e = cudaMalloc(&p, bytes);
+    if (e != cudaSuccess) {
+        set_error("cudaMalloc(%zu) failed: %s", bytes, cudaGetErrorString(e));
+        return nullptr;
+    }
+    return p;
+}
+
+void dev_free(void* p) {
+    if (!p) return;
+    if (hooks().dealloc) hooks().dealloc(p);
+    else cudaFree(p);
+}
+
+static bool is_device_ptr(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+static int have_device() {
+    int n = 0;
+    cudaError_t e = cudaGetDeviceCount(&n);
+    if (e != cudaSuccess || n < 1) {
+        cudaGetLastError();
+        set_error("no CUDA device: libising_b200 has no CPU path (%s)",
+                  e == cudaSuccess ? "device count 0" : cudaGetErrorString(e));
+        return ISING_ECUDA;
+    }
+    return 0;
+}
+
+// a2 / S8c.4: thr[m] = floor(exp(-β·4m)·2^32) in double, m = 1..dim.
+static void threshold_table(double beta, int dim, uint64_t thr[3]) {
+    for (int m = 1; m <= 3; ++m)
+        thr[m - 1] = (m <= dim) ? (uint64_t)std::floor(std::exp(-beta * 4.0 * (double)m) * 4294967296.0) : 0;
+}
+
+static Accept make_accept(double beta, int dim) {
+    uint64_t thr[3];
+    threshold_table(beta, dim, thr);
+    Accept a;
+    a.always = 0;
+    for (int m = 0; m < 3; ++m) {
+        a.thr_is_2p32[m] = (m < dim && thr[m] >= 4294967296ull) ? 1u : 0u;
+        a.thr[m] = a.thr_is_2p32[m] ? 0xffffffffu : (uint32_t)thr[m];
+        a.cneg[m] = 0;
+        if (m >= dim) continue;
+        if (thr[m] == 0) a.always += 1;                       // r >= 0 always
+        else if (!a.thr_is_2p32[m]) a.cneg[m] = (uint32_t)(4294967296ull - thr[m]);
+    }
+    return a;
+}
+
+static bool tile_valid(const ising_ctx* h, int T) {
+    if (T < 2 || (T & 1) || h->L % T) return false;
+    const int B = h->L / T;
+    return B == 1 || (B % 2 == 0);
+}
+
+// ---- storage bookkeeping --------------------------------------------------------------
+static int to_canon_scratch(ising_ctx* h) {   // tiles -> d_canon, store state unchanged
+    if (h->store == Store::TileI8) return launch_tile_i8_to_canon(h, h->store_tile, h->d_tiles, h->d_canon);
+    return 0;
+}
+
+static int ensure_canon(ising_ctx* h) {
+    if (h->store == Store::Canon) return 0;
+    const int rc = to_canon_scratch(h);
+    if (rc) return rc;
+    h->store = Store::Canon;
+    h->store_tile = 0;
+    return 0;
+}
+
+static int ensure_tile_i8(ising_ctx* h, int T) {
+    if (h->store == Store::TileI8 && h->store_tile == T) return 0;
+    int rc = ensure_canon(h);
+    if (rc) return rc;
+    const size_t need = tile_i8_bytes(h, T);
+    if (need > h->tiles_bytes) {
+        ISING_CUDA_OK(cudaStreamSynchronize(hooks().stream));
+        dev_free(h->d_tiles);
+        h->tiles_bytes = 0;
+        h->d_tiles = dev_alloc(need);
+        if (!h->d_tiles) return ISING_ENOMEM;
+        h->tiles_bytes = need;
+    }
+    rc = launch_canon_to_tile_i8(h, T, h->d_canon, h->d_tiles);
+    if (rc) return rc;
+    h->store = Store::TileI8;
+    h->store_tile = T;
+    return 0;
+}
+
+static const int8_t* canon_view(ising_ctx* h, int* rc) {
+    *rc = (h->store == Store::Canon) ? 0 : to_canon_scratch(h);
+    return h->d_canon;
+}
+
+static int copy_out(void* dst, const void* d_src, size_t bytes, bool* synced) {
+    cudaStream_t st = hooks().stream;
+    const bool dev = is_device_ptr(dst);
+    ISING_CUDA_OK(cudaMemcpyAsync(dst, d_src, bytes, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    ISING_CUDA_OK(cudaStreamSynchronize(st));
+    if (synced) *synced = true;
+    return 0;
+}
+
+}  // namespace ising
+
+using namespace ising;
+
+extern "C" {
+
+const char* ising_last_error(void) { return g_err; }
+uint64_t ising_kernel_launches(void) { return g_launches.load(); }
+
+int ising_set_device_hooks(void* (*alloc)(size_t), void (*dealloc)(void*), void* cuda_stream) {
+    if ((alloc == nullptr) != (dealloc == nullptr)) {
+        set_error("ising_set_device_hooks: alloc and dealloc must both be set or both be NULL");
+        return ISING_EINVAL;
+    }
+    hooks().alloc = alloc;
+    hooks().dealloc = dealloc;
+    hooks().stream = (cudaStream_t)cuda_stream;
+    return 0;
+}
+
+int ising_thresholds(double beta, int dim, uint64_t* out) {
+    if (!out || (dim != 2 && dim != 3) || !(beta >= 0.0) || !std::isfinite(beta)) {
+        set_error("ising_thresholds: need dim in {2,3}, finite beta >= 0, out != NULL");
+        return ISING_EINVAL;
+    }
+    threshold_table(beta, dim, out);
+    return 0;
+}
+
+void ising_destroy(ising_handle h) {
+    if (!h) return;
+    cudaStreamSynchronize(hooks().stream);
+    dev_free(h->d_J);
+    dev_free(h->d_seeds);
+    dev_free(h->d_canon);
+    dev_free(h->d_tiles);
+    dev_free(h->d_Jtiles);
+    dev_free(h->d_obs);
+    dev_free(h->d_flag);
+    delete h;
+}
+
+ising_handle ising_create_batch(int dim, int L, const int8_t* J, const uint64_t* seeds, int R) {
+    if ((dim != 2 && dim != 3) || L < 2 || (L & 1) || R < 1 || !seeds) {
+        set_error("ising_create: need dim in {2,3}, even L >= 2, n_replicas >= 1, seeds != NULL "
+                  "(got dim=%d L=%d R=%d)", dim, L, R);
+        return nullptr;
+    }
+    uint64_t N = 1;
+    for (int d = 0; d < dim; ++d) N *= (uint64_t)L;
+    if (N > (1ull << 32)) {
+        set_error("ising_create: N = L^dim = %llu exceeds 2^32", (unsigned long long)N);
+        return nullptr;
+    }
+    if (have_device()) return nullptr;
+    ising_ctx* h = new (std::nothrow) ising_ctx;
+    if (!h) return nullptr;
+    h->dim = dim; h->L = L; h->R = R; h->N = N;
+    h->seeds.assign(seeds, seeds + R);
+    cudaStream_t st = hooks().stream;
+    auto fail = [&](void) -> ising_handle { ising_destroy(h); return nullptr; };
+    h->d_seeds = (uint64_t*)dev_alloc(sizeof(uint64_t) * R);
+    h->d_canon = (int8_t*)dev_alloc((size_t)R * N);
+    h->d_obs = (long long*)dev_alloc(sizeof(long long) * (2 * (size_t)R + 2));
+    h->d_flag = (int*)dev_alloc(sizeof(int));
+    if (!h->d_seeds || !h->d_canon || !h->d_obs || !h->d_flag) return fail();
+    if (cudaMemcpyAsync(h->d_seeds, h->seeds.data(), sizeof(uint64_t) * R, cudaMemcpyHostToDevice, st) != cudaSuccess) {
+        set_error("ising_create: seed upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+        return fail();
+    }
+    if (J) {
+        const size_t jb = (size_t)dim * N;
+        h->d_J = (int8_t*)dev_alloc(jb);
+        if (!h->d_J) return fail();
+        const bool dev = is_device_ptr(J);
+        if (cudaMemcpyAsync(h->d_J, J, jb, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st) != cudaSuccess) {
+            set_error("ising_create: coupling upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+            return fail();
+        }
+        int bad = 0;
+        if (launch_validate_pm1(h->d_J, jb, h->d_flag, &bad)) return fail();
+        if (bad) {
+            set_error("ising_create: couplings must be +1 or -1");
+            return fail();
+        }
+        h->has_J = true;
+    }
+    if (launch_hot_start(h)) return fail();
+    if (cudaStreamSynchronize(st) != cudaSuccess) {   // seeds vector may go away; surface errors here
+        set_error("ising_create: %s", cudaGetErrorString(cudaGetLastError()));
+        return fail();
+    }
+    return h;
+}
+
+ising_handle ising_create(int dim, int L, const int8_t* J, uint64_t seed) {
+    return ising_create_batch(dim, L, J, &seed, 1);
+}
+
+}  // extern "C"
+
+// ---- sweeps ---------------------------------------------------------------------------
+static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64_t* E, int64_t* M) {
+    if (!h) { set_error("ising_sweep: NULL handle"); return ISING_EINVAL; }
+    const int T = (tile == 0) ? h->L : tile;
+    if (!tile_valid(h, T)) {
+        set_error("ising_sweep: tile=%d invalid for L=%d (need T even, T | L, L/T even or T == L)", tile, h->L);
+        return ISING_EINVAL;
+    }
+    if (k < 1 || n < 0 || !(beta >= 0.0) || !std::isfinite(beta)) {
+        set_error("ising_sweep: need k_inner >= 1, n_sweeps >= 0, finite beta >= 0");
+        return ISING_EINVAL;
+    }
+    const Accept acc = make_accept(beta, h->dim);
+    cudaStream_t st = hooks().stream;
+    const bool want_series = (E != nullptr) || (M != nullptr);
+    const size_t cnt = (size_t)n * h->R;
+    long long *d_E = nullptr, *d_M = nullptr, *tmp = nullptr;
+    const bool E_dev = E && is_device_ptr(E), M_dev = M && is_device_ptr(M);
+    if (want_series && cnt) {
+        const size_t need = ((E && !E_dev) ? cnt : 0) + ((M && !M_dev) ? cnt : 0);
+        if (need) {
+            tmp = (long long*)dev_alloc(need * sizeof(long long));
+            if (!tmp) return ISING_ENOMEM;
+        }
+        long long* q = tmp;
+        if (E) { d_E = E_dev ? (long long*)E : q; if (!E_dev) q += cnt; }
+        if (M) { d_M = M_dev ? (long long*)M : q; }
+    }
+    int rc = 0;
+    const bool thr_fits = !(acc.thr_is_2p32[0] || acc.thr_is_2p32[1] || acc.thr_is_2p32[2]);   // beta = 0 only
+    const bool use_tile_i8 = !h->force_generic && thr_fits && h->layout == ISING_LAYOUT_I8 && tile_i8_supported(h, T);
+    if (use_tile_i8) {
+        h->last_path = "tile_i8";
+        rc = ensure_tile_i8(h, T);
+        for (int pass = 0; pass < n && !rc; ++pass) {
+            rc = launch_tile_i8_pass(h, acc, T, k, h->t + (uint64_t)pass * (uint64_t)k);
+            if (!rc && want_series) {
+                rc = to_canon_scratch(h);
+                if (!rc) rc = launch_observables_canon(h, h->d_canon, d_E ? d_E + (size_t)pass * h->R : nullptr,
+                                                       d_M ? d_M + (size_t)pass * h->R : nullptr);
+            }
+        }
+    } else if (h->layout == ISING_LAYOUT_I8) {
+        h->last_path = "generic";
+        rc = ensure_canon(h);
+        if (!rc) rc = launch_generic_sweep(h, acc, n, T, k, d_E, d_M);
+    } else {
+        set_error("ising_sweep: no bit-packed kernel for dim=%d L=%d tile=%d", h->dim, h->L, T);
+        rc = ISING_EUNSUPPORTED;
+    }
+    if (!rc) h->t += (uint64_t)n * (uint64_t)k;
+    if (!rc && tmp) {
+        long long* q = tmp;
+        if (E && !E_dev) { rc = copy_out(E, q, cnt * sizeof(long long), nullptr); q += cnt; }
+        if (!rc && M && !M_dev) rc = copy_out(M, q, cnt * sizeof(long long), nullptr);
+    }
+    if (tmp) { cudaStreamSynchronize(st); dev_free(tmp); }
+    return rc;
+}
+
+extern "C" {
+
+int ising_sweep(ising_handle h, double beta, int n_sweeps, int tile, int k_inner) {
+    return sweep_impl(h, beta, n_sweeps, tile, k_inner, nullptr, nullptr);
+}
+
+int ising_sweep_series(ising_handle h, double beta, int n_sweeps, int tile, int k_inner, int64_t* E, int64_t* M) {
+    return sweep_impl(h, beta, n_sweeps, tile, k_inner, E, M);
+}
+
+int ising_observables(ising_handle h, int64_t* E, int64_t* M) {
+    if (!h) { set_error("ising_observables: NULL handle"); return ISING_EINVAL; }
+    int rc = 0;
+    const int8_t* s = canon_view(h, &rc);
+    if (rc) return rc;
+    rc = launch_observables_canon(h, s, h->d_obs, h->d_obs + h->R);
+    if (rc) return rc;
+    if (E) { rc = copy_out(E, h->d_obs, sizeof(long long) * h->R, nullptr); if (rc) return rc; }
+    if (M) { rc = copy_out(M, h->d_obs + h->R, sizeof(long long) * h->R, nullptr); if (rc) return rc; }
+    ISING_CUDA_OK(cudaStreamSynchronize(hooks().stream));
+    return 0;
+}
+
+int ising_overlap(ising_handle h, int a, int b, int64_t* Q) {
+    if (!h || !Q || a < 0 || b < 0 || a >= h->R || b >= h->R) {
+        set_error("ising_overlap: bad handle, NULL output or replica index out of range");
+        return ISING_EINVAL;
+    }
+    int rc = 0;
+    const int8_t* s = canon_view(h, &rc);
+    if (rc) return rc;
+    long long* d_Q = h->d_obs + 2 * h->R;
+    rc = launch_overlap_canon(h, s, a, b, d_Q);
+    if (rc) return rc;
+    return copy_out(Q, d_Q, sizeof(long long), nullptr);
+}
+
+int ising_copy_spins(ising_handle h, int8_t* dst) {
+    if (!h || !dst) { set_error("ising_copy_spins: NULL argument"); return ISING_EINVAL; }
+    int rc = 0;
+    const int8_t* s = canon_view(h, &rc);
+    if (rc) return rc;
+    return copy_out(dst, s, (size_t)h->R * h->N, nullptr);
+}
+
+int ising_set_spins(ising_handle h, const int8_t* src) {
+    if (!h || !src) { set_error("ising_set_spins: NULL argument"); return ISING_EINVAL; }
+    cudaStream_t st = hooks().stream;
+    const size_t bytes = (size_t)h->R * h->N;
+    int8_t* stage = (int8_t*)dev_alloc(bytes);
+    if (!stage) return ISING_ENOMEM;
+    const bool dev = is_device_ptr(src);
+    cudaError_t e = cudaMemcpyAsync(stage, src, bytes, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st);
+    int bad = 0;
+    int rc = (e == cudaSuccess) ? launch_validate_pm1(stage, bytes, h->d_flag, &bad) : ISING_ECUDA;
+    if (e != cudaSuccess) set_error("ising_set_spins: copy failed: %s", cudaGetErrorString(e));
+    if (!rc && bad) { set_error("ising_set_spins: spins must be +1 or -1"); rc = ISING_EINVAL; }
+    if (!rc) {
+        e = cudaMemcpyAsync(h->d_canon, stage, bytes, cudaMemcpyDeviceToDevice, st);
+        if (e != cudaSuccess) { set_error("ising_set_spins: %s", cudaGetErrorString(e)); rc = ISING_ECUDA; }
+        else { h->store = Store::Canon; h->store_tile = 0; }
+    }
+    cudaStreamSynchronize(st);
+    dev_free(stage);
+    return rc;
+}
+
+int ising_set_layout(ising_handle h, int layout) {
+    if (!h || (layout != ISING_LAYOUT_I8 && layout != ISING_LAYOUT_BITS)) {
+        set_error("ising_set_layout: layout must be ISING_LAYOUT_I8 or ISING_LAYOUT_BITS");
+        return ISING_EINVAL;
+    }
+    if (layout == h->layout) return 0;
+    const int rc = ensure_canon(h);
+    if (rc) return rc;
+    h->layout = layout;
+    return 0;
+}
+
+int ising_get_counter(ising_handle h, uint64_t* t) {
+    if (!h || !t) { set_error("ising_get_counter: NULL argument"); return ISING_EINVAL; }
+    *t = h->t;
+    return 0;
+}
+
+int ising_set_counter(ising_handle h, uint64_t t) {
+    if (!h) { set_error("ising_set_counter: NULL handle"); return ISING_EINVAL; }
+    h->t = t;
+    return 0;
+}
+
+int ising_synchronize(ising_handle h) {
+    (void)h;
+    ISING_CUDA_OK(cudaStreamSynchronize(hooks().stream));
+    return 0;
+}
+
+const char* ising_sweep_path(ising_handle h) { return h ? h->last_path : "none"; }
+
+int ising_force_path(ising_handle h, int generic_only) {
+    if (!h) { set_error("ising_force_path: NULL handle"); return ISING_EINVAL; }
+    h->force_generic = generic_only ? 1 : 0;
+    return 0;
+}
+
+}  // extern "C"

@@ -1,0 +1,87 @@
+// common.cuh — handle, error plumbing and launch helpers shared by the .cu files of
+// libising_b200.  Product code: nothing here (or anywhere under csrc/) includes oracle/.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+#include <cstdio>
+#include <string>
+#include <vector>
+
+#include "../../include/ising.h"
+
+namespace ising {
+
+// ---- process-wide hooks (ising_set_device_hooks) -------------------------------------
+struct Hooks {
+    void* (*alloc)(size_t) = nullptr;
+    void (*dealloc)(void*) = nullptr;
+    cudaStream_t stream = nullptr;
+};
+Hooks& hooks();
+void set_error(const char* fmt, ...);
+void count_launch(uint64_t n = 1);
+
+void* dev_alloc(size_t bytes);   // through the hooks; nullptr on failure (error set)
+void dev_free(void* p);
+
+#define ISING_CUDA_OK(expr)                                                              \
+    do {                                                                                 \
+        cudaError_t e__ = (expr);                                                        \
+        if (e__ != cudaSuccess) {                                                        \
+            ::ising::set_error("%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e__), \
+                               __FILE__, __LINE__);                                      \
+            return ISING_ECUDA;                                                          \
+        }                                                                                \
+    } while (0)
+
+// How the spins are currently held in HBM.
+enum class Store : int {
+    Canon = 0,   // int8 ±1, index order, R*N bytes (generic kernels, observables, I/O)
+    TileI8 = 1,  // tile records of 0/1 bytes, colour-split rows + edge columns (tile_i8.cu)
+    TileBits = 2 // tile records of bits (tile_bits.cu)
+};
+
+// Acceptance constants handed to every sweep kernel (S8c.4/5).
+// The device test is   flip  <=>  n_sat + #{m : r >= thr[m]} <= 2*dim,
+// which equals "a <= 0, or r < thr[a/2]" because thr[1] >= thr[2] >= thr[3]
+// (n_sat = number of satisfied bonds, a = 2*n_sat - 2*dim).
+// cneg[m-1] = 2^32 - thr[m] as a 32-bit addend whose carry-out is (r >= thr[m]);
+// thresholds equal to 2^32 (beta = 0) never carry (cneg = 0) and thresholds equal to 0
+// always count: those are folded into `always` instead (cneg = 0 as well).
+struct Accept {
+    uint32_t cneg[3];
+    uint32_t always;   // number of m in 1..dim with thr[m] == 0
+    uint32_t thr[3];   // thr[m] clipped to 32 bits (for kernels that compare directly)
+    uint32_t thr_is_2p32[3];
+};
+
+}  // namespace ising
+
+struct ising_ctx {
+    int dim = 2;
+    int L = 0;
+    int R = 1;
+    uint64_t N = 0;
+    bool has_J = false;
+    int8_t* d_J = nullptr;          // canonical ±1, dim*N bytes (nullptr if uniform)
+    uint64_t* d_seeds = nullptr;    // R Philox keys
+    std::vector<uint64_t> seeds;
+    uint64_t t = 0;                 // inner sweeps done (S8c.6)
+
+    int layout = ISING_LAYOUT_I8;   // requested HBM layout
+    ising::Store store = ising::Store::Canon;
+    int store_tile = 0;             // T of the tile records when store != Canon
+    int8_t* d_canon = nullptr;      // R*N bytes; valid iff store == Canon (else scratch)
+    void* d_tiles = nullptr;        // tile-record storage (TileI8 / TileBits)
+    size_t tiles_bytes = 0;
+    void* d_Jtiles = nullptr;       // couplings in tile-record form for store_tile
+    int Jtiles_tile = 0;
+    int Jtiles_kind = -1;
+    size_t Jtiles_bytes = 0;
+
+    long long* d_obs = nullptr;     // 2*R int64 accumulators (+1 for overlap)
+    int* d_flag = nullptr;          // validation flag
+    const char* last_path = "none";
+    int force_generic = 0;
+};

@@ -1,0 +1,240 @@
+// generic.cu — kernels on the canonical layout (int8 ±1, index order): hot start,
+// observables, overlap, validation, and the global-memory sweep that serves every
+// (dim, L, tile, couplings, replicas) combination the fast tile kernels do not.
+//
+// The generic sweep is the schedule of P:64-74 / S8c.6 issued as one launch per
+// (coarse colour C, inner sweep j, fine colour c): all sites of fine colour c inside tiles
+// of coarse colour C are independent, so one thread per site pair updates them in
+// place from the live array.  With tile == L this is the single checkerboard of P:62 (a8).
+#include "kernels.h"
+#include "philox.cuh"
+
+namespace ising {
+
+namespace {
+
+constexpr int kThreads = 256;
+
+__device__ __forceinline__ void key_of(uint64_t seed, uint32_t& k0, uint32_t& k1) {
+    k0 = (uint32_t)(seed & 0xffffffffull);
+    k1 = (uint32_t)(seed >> 32);
+}
+
+// a11 / S8c.3: s_i = (Philox(ctr = {i>>2, 1, 0, 0}, key = seed_r)[i & 3] >> 31) ? -1 : +1.
+__global__ void k_hot_start(int8_t* __restrict__ s, const uint64_t* __restrict__ seeds,
+                            uint64_t groups_per_replica, int R) {
+    const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= groups_per_replica * (uint64_t)R) return;
+    const uint64_t r = gid / groups_per_replica;
+    const uint64_t g = gid - r * groups_per_replica;
+    uint32_t k0, k1;
+    key_of(seeds[r], k0, k1);
+    const u32x4 o = philox4x32_10((uint32_t)g, kTagInit, 0u, 0u, k0, k1);
+    char4 v;
+    v.x = (o.x >> 31) ? -1 : 1;
+    v.y = (o.y >> 31) ? -1 : 1;
+    v.z = (o.z >> 31) ? -1 : 1;
+    v.w = (o.w >> 31) ? -1 : 1;
+    reinterpret_cast<char4*>(s)[r * groups_per_replica + g] = v;
+}
+
+struct GenericGeom {
+    int dim, L, T, R;
+    uint64_t N;
+};
+
+// One thread per site pair p = i >> 1 (S8c.3): the pair (2p, 2p+1) lies in one row because
+// L is even and holds exactly one site of each fine colour.
+__global__ void k_generic_halfsweep(int8_t* __restrict__ spins, const int8_t* __restrict__ J,
+                                    const uint64_t* __restrict__ seeds, GenericGeom g,
+                                    Accept acc, uint64_t H, int C, int c) {
+    const uint64_t pairs = g.N >> 1;
+    const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= pairs * (uint64_t)g.R) return;
+    const uint64_t r = gid / pairs;
+    const uint64_t p = gid - r * pairs;
+    const uint64_t L = (uint64_t)g.L;
+    const uint64_t i0 = p << 1;
+    const int x0 = (int)(i0 % L);
+    const int y = (int)((i0 / L) % L);
+    const int z = (int)(i0 / (L * L));
+    const int x = x0 + ((x0 + y + z + c) & 1);           // the site of fine colour c in the pair
+    if ((((x / g.T) + (y / g.T) + (z / g.T)) & 1) != C) return;   // S8c.1 coarse colour
+    const uint64_t i = i0 + (uint64_t)(x - x0);
+    int8_t* s = spins + r * g.N;
+    const int coord[3] = {x, y, z};
+    uint64_t stride = 1;
+    const int si = s[i];
+    int n_sat = 0;                                       // satisfied bonds J s_i s_j = +1
+    for (int d = 0; d < g.dim; ++d) {
+        const uint64_t ip = (coord[d] == g.L - 1) ? i - (L - 1) * stride : i + stride;
+        const uint64_t im = (coord[d] == 0) ? i + (L - 1) * stride : i - stride;
+        const int Jp = J ? (int)J[(uint64_t)d * g.N + i] : 1;
+        const int Jm = J ? (int)J[(uint64_t)d * g.N + im] : 1;
+        n_sat += (Jp * si * s[ip] > 0) + (Jm * si * s[im] > 0);
+        stride *= L;
+    }
+    const int a = 2 * n_sat - 2 * g.dim;                 // ΔE = 2a (S8c.5)
+    bool flip = true;
+    if (a > 0) {
+        uint32_t k0, k1;
+        key_of(seeds[r], k0, k1);
+        const u32x4 o = philox4x32_10((uint32_t)(p >> 2), kTagSweep, (uint32_t)(H & 0xffffffffull),
+                                      (uint32_t)(H >> 32), k0, k1);
+        const uint32_t w = (uint32_t)(p & 3);
+        const uint32_t rnd = w == 0 ? o.x : (w == 1 ? o.y : (w == 2 ? o.z : o.w));
+        const int m = a / 2 - 1;
+        flip = acc.thr_is_2p32[m] || (rnd < acc.thr[m]);
+    }
+    if (flip) s[i] = (int8_t)(-si);
+}
+
+__device__ __forceinline__ long long warp_sum(long long v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// a10 / S8c.7: E = -Σ_i Σ_d J_d(i) s_i s_(i+e_d), M = Σ_i s_i; blockIdx.y = replica.
+__global__ void k_observables(const int8_t* __restrict__ spins, const int8_t* __restrict__ J,
+                              GenericGeom g, long long* __restrict__ E, long long* __restrict__ M) {
+    const int r = blockIdx.y;
+    const int8_t* s = spins + (uint64_t)r * g.N;
+    const uint64_t L = (uint64_t)g.L;
+    long long e = 0, m = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < g.N;
+         i += (uint64_t)gridDim.x * blockDim.x) {
+        const int coord[3] = {(int)(i % L), (int)((i / L) % L), (int)(i / (L * L))};
+        const int si = s[i];
+        m += si;
+        uint64_t stride = 1;
+        for (int d = 0; d < g.dim; ++d) {
+            const uint64_t ip = (coord[d] == g.L - 1) ? i - (L - 1) * stride : i + stride;
+            const int Jp = J ? (int)J[(uint64_t)d * g.N + i] : 1;
+            e -= Jp * si * s[ip];
+            stride *= L;
+        }
+    }
+    __shared__ long long sh[2][kThreads / 32];
+    e = warp_sum(e);
+    m = warp_sum(m);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) { sh[0][w] = e; sh[1][w] = m; }
+    __syncthreads();
+    if (w == 0) {
+        e = lane < kThreads / 32 ? sh[0][lane] : 0;
+        m = lane < kThreads / 32 ? sh[1][lane] : 0;
+        e = warp_sum(e);
+        m = warp_sum(m);
+        if (lane == 0) {
+            if (E) atomicAdd((unsigned long long*)&E[r], (unsigned long long)e);
+            if (M) atomicAdd((unsigned long long*)&M[r], (unsigned long long)m);
+        }
+    }
+}
+
+__global__ void k_overlap(const int8_t* __restrict__ sa, const int8_t* __restrict__ sb, uint64_t N,
+                          long long* __restrict__ Q) {
+    long long q = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N;
+         i += (uint64_t)gridDim.x * blockDim.x)
+        q += (int)sa[i] * (int)sb[i];
+    __shared__ long long sh[kThreads / 32];
+    q = warp_sum(q);
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (lane == 0) sh[w] = q;
+    __syncthreads();
+    if (w == 0) {
+        q = lane < kThreads / 32 ? sh[lane] : 0;
+        q = warp_sum(q);
+        if (lane == 0) atomicAdd((unsigned long long*)Q, (unsigned long long)q);
+    }
+}
+
+__global__ void k_validate_pm1(const int8_t* __restrict__ d, uint64_t n, int* flag) {
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
+         i += (uint64_t)gridDim.x * blockDim.x)
+        if (d[i] != 1 && d[i] != -1) *flag = 1;
+}
+
+int reduce_grid(uint64_t n) {
+    uint64_t b = (n + kThreads - 1) / kThreads;
+    const uint64_t cap = 148ull * 16ull;
+    return (int)(b < cap ? (b ? b : 1) : cap);
+}
+
+}  // namespace
+
+int launch_hot_start(ising_ctx* h) {
+    const uint64_t groups = h->N / 4;
+    const uint64_t total = groups * (uint64_t)h->R;
+    const unsigned blocks = (unsigned)((total + kThreads - 1) / kThreads);
+    k_hot_start<<<blocks, kThreads, 0, hooks().stream>>>(h->d_canon, h->d_seeds, groups, h->R);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+int launch_observables_canon(ising_ctx* h, const int8_t* d_spins, long long* d_E, long long* d_M) {
+    cudaStream_t st = hooks().stream;
+    if (d_E) ISING_CUDA_OK(cudaMemsetAsync(d_E, 0, sizeof(long long) * h->R, st));
+    if (d_M) ISING_CUDA_OK(cudaMemsetAsync(d_M, 0, sizeof(long long) * h->R, st));
+    GenericGeom g{h->dim, h->L, h->L, h->R, h->N};
+    dim3 grid(reduce_grid(h->N), h->R);
+    k_observables<<<grid, kThreads, 0, st>>>(d_spins, h->d_J, g, d_E, d_M);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+int launch_overlap_canon(ising_ctx* h, const int8_t* d_spins, int a, int b, long long* d_Q) {
+    cudaStream_t st = hooks().stream;
+    ISING_CUDA_OK(cudaMemsetAsync(d_Q, 0, sizeof(long long), st));
+    k_overlap<<<reduce_grid(h->N), kThreads, 0, st>>>(d_spins + (uint64_t)a * h->N,
+                                                       d_spins + (uint64_t)b * h->N, h->N, d_Q);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+int launch_validate_pm1(const int8_t* d, uint64_t n, int* d_flag, int* host_bad) {
+    cudaStream_t st = hooks().stream;
+    ISING_CUDA_OK(cudaMemsetAsync(d_flag, 0, sizeof(int), st));
+    k_validate_pm1<<<reduce_grid(n), kThreads, 0, st>>>(d, n, d_flag);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    ISING_CUDA_OK(cudaMemcpyAsync(host_bad, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
+    ISING_CUDA_OK(cudaStreamSynchronize(st));
+    return 0;
+}
+
+// a1/a6/a8: the whole S8c.6 schedule, one launch per (C, j, c); optional E/M after each pass.
+int launch_generic_sweep(ising_ctx* h, const Accept& acc, int n, int T, int k, long long* d_E,
+                         long long* d_M) {
+    cudaStream_t st = hooks().stream;
+    GenericGeom g{h->dim, h->L, T, h->R, h->N};
+    const uint64_t total = (h->N >> 1) * (uint64_t)h->R;
+    const unsigned blocks = (unsigned)((total + kThreads - 1) / kThreads);
+    const int ncol = (T == h->L) ? 1 : 2;   // one tile: the odd coarse phase is empty
+    for (int pass = 0; pass < n; ++pass) {
+        for (int C = 0; C < ncol; ++C)
+            for (int j = 0; j < k; ++j) {
+                const uint64_t t = h->t + (uint64_t)pass * (uint64_t)k + (uint64_t)j;
+                for (int c = 0; c < 2; ++c) {
+                    k_generic_halfsweep<<<blocks, kThreads, 0, st>>>(h->d_canon, h->d_J, h->d_seeds,
+                                                                     g, acc, 2 * t + c, C, c);
+                    count_launch();
+                }
+            }
+        if (d_E || d_M) {
+            const int rc = launch_observables_canon(h, h->d_canon,
+                                                    d_E ? d_E + (size_t)pass * h->R : nullptr,
+                                                    d_M ? d_M + (size_t)pass * h->R : nullptr);
+            if (rc) return rc;
+        }
+    }
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+}  // namespace ising

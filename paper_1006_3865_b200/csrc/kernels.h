@@ -1,0 +1,23 @@
+// kernels.h — host-side launch functions implemented by the .cu files; called by api.cu.
+#pragma once
+#include "common.cuh"
+
+namespace ising {
+
+// ---- generic.cu: canonical int8 ±1 storage, any even L, any valid tile ---------------
+int launch_hot_start(ising_ctx* h);                                   // S8c.3 (a11)
+int launch_generic_sweep(ising_ctx* h, const Accept& acc, int n, int T, int k,
+                         long long* d_E, long long* d_M);             // a1,a4-a6,a8,a9
+int launch_observables_canon(ising_ctx* h, const int8_t* d_spins, long long* d_E,
+                             long long* d_M);                         // a10 (R values each)
+int launch_overlap_canon(ising_ctx* h, const int8_t* d_spins, int a, int b, long long* d_Q);
+int launch_validate_pm1(const int8_t* d, uint64_t n, int* d_flag, int* host_bad);
+
+// ---- tile_i8.cu: 2D tile records of 0/1 bytes, warp-per-tile staged kernel -----------
+bool tile_i8_supported(const ising_ctx* h, int T);
+size_t tile_i8_bytes(const ising_ctx* h, int T);
+int launch_canon_to_tile_i8(ising_ctx* h, int T, const int8_t* d_canon, void* d_tiles);
+int launch_tile_i8_to_canon(ising_ctx* h, int T, const void* d_tiles, int8_t* d_canon);
+int launch_tile_i8_pass(ising_ctx* h, const Accept& acc, int T, int k, uint64_t t_first);
+
+}  // namespace ising

@@ -1,0 +1,170 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, bit for bit, on the
+same seeded inputs.  Integer work only, so the bar is exact equality of every spin, E and M."""
+import numpy as np
+import pytest
+
+import ising_workloads as W
+
+pytestmark = pytest.mark.gpu
+
+BC2, BC3 = W.BETA_C_2D, W.BETA_C_3D
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1006_3865_b200 as pkg
+    pkg.use_torch()
+    return pkg
+
+
+def _both(P, orc, dim, L, seeds, J=None):
+    g = P.Ising(dim, L, coupling=J, seeds=seeds)
+    o = orc.Oracle(dim, L, seeds=seeds, J=J)
+    return g, o
+
+
+def _same_state(g, o):
+    sg = np.asarray(g.copy_spins()).reshape(-1)
+    so = np.asarray(o.spins()).reshape(-1)
+    bad = np.flatnonzero(sg != so)
+    assert bad.size == 0, f"{bad.size} spins differ, first at {bad[:8]}"
+    Eg, Mg = g.observables()
+    Eo, Mo = o.observables()
+    assert list(Eg) == list(Eo) and list(Mg) == list(Mo)
+
+
+@pytest.mark.parametrize("dim,L,seed", [(2, 2, 5), (2, 4, 3), (2, 64, 1), (2, 250, 8), (3, 2, 1), (3, 8, 4), (3, 30, 2)])
+def test_hot_start(P, orc, dim, L, seed):
+    g, o = _both(P, orc, dim, L, [seed])
+    _same_state(g, o)
+
+
+GENERIC = [
+    # dim, L, tile, k, n, beta, seeds, jseed
+    (2, 2, 2, 1, 5, BC2, [1], None),
+    (2, 4, 2, 3, 5, BC2, [3], None),
+    (2, 8, 4, 2, 3, BC2, [7], None),
+    (2, 64, 0, 1, 20, BC2, [1], None),          # config 1 shape: plain checkerboard
+    (2, 64, 8, 4, 6, BC2, [9], None),
+    (2, 96, 16, 2, 4, 0.6, [11], None),
+    (2, 36, 6, 2, 4, 0.3, [12], None),          # tile not a multiple of 8
+    (3, 2, 2, 1, 4, BC3, [2], None),
+    (3, 8, 4, 2, 5, BC3, [4], None),            # config 4 shape, small
+    (3, 16, 8, 4, 2, BC3, [4], None),
+    (3, 12, 6, 1, 3, 0.5, [6], None),
+    (2, 16, 4, 4, 10, 1.0, [100], 5),           # config 5 shape, small
+    (2, 64, 32, 4, 4, 1.0, [100, 101, 114], 5), # replicas sharing J
+    (3, 8, 4, 2, 3, 0.9, [1, 2], 17),
+    (2, 32, 8, 1, 3, 0.0, [4], None),           # beta = 0: thresholds are 2^32
+    (2, 32, 8, 2, 3, 30.0, [4], None),          # thresholds underflow to 0
+]
+
+
+@pytest.mark.parametrize("dim,L,tile,k,n,beta,seeds,jseed", GENERIC)
+def test_generic_path_matches_oracle(P, orc, dim, L, tile, k, n, beta, seeds, jseed):
+    J = W.couplings(dim, L, jseed) if jseed is not None else None
+    g, o = _both(P, orc, dim, L, seeds, J)
+    g.force_path(True)
+    Eg, Mg = g.sweep_series(beta, n, tile, k)
+    Eo, Mo = o.sweep_series(beta, n, tile, k)
+    assert g.sweep_path() == "generic"
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    assert g.counter == o.counter == n * k
+    if len(seeds) > 1:
+        assert g.overlap(0, 1) == o.overlap(0, 1)
+
+
+TILED = [
+    # L, tile, k, n, beta, seeds  — several tiles, both tile sizes, wrap-around in both directions
+    (64, 32, 1, 3, BC2, [3]),
+    (128, 32, 4, 3, BC2, [3]),
+    (128, 64, 1, 3, BC2, [5]),
+    (256, 64, 4, 2, 0.6, [6]),
+    (192, 32, 2, 3, 0.3, [7]),       # B = 6: ragged against the 2-tiles-per-warp job
+    (384, 64, 1, 2, BC2, [8]),       # B = 6
+    (256, 32, 16, 1, BC2, [3]),
+    (128, 32, 2, 2, 0.0, [2]),
+    (128, 64, 2, 2, 30.0, [2]),
+    (128, 32, 2, 3, BC2, [21, 22, 23]),   # replicas
+]
+
+
+@pytest.mark.parametrize("L,tile,k,n,beta,seeds", TILED)
+def test_tile_i8_path_matches_oracle(P, orc, L, tile, k, n, beta, seeds):
+    g, o = _both(P, orc, 2, L, seeds)
+    Eg, Mg = g.sweep_series(beta, n, tile, k)
+    assert g.sweep_path() == ("tile_i8" if beta > 0 else "generic")   # beta = 0: thr = 2^32, generic kernels
+    Eo, Mo = o.sweep_series(beta, n, tile, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+
+
+def test_paths_agree_and_sweeps_compose(P, orc):
+    """sweep(a); sweep(b) == sweep(a+b) across kernel paths and tile sizes (stateless RNG)."""
+    a = P.Ising(2, 256, seed=33)
+    b = P.Ising(2, 256, seed=33)
+    a.sweep(BC2, 2, 32, 4); a.sweep(BC2, 3, 64, 2); a.sweep(BC2, 1, 0, 1)
+    b.force_path(True)
+    b.sweep(BC2, 2, 32, 4); b.sweep(BC2, 3, 64, 2); b.sweep(BC2, 1, 0, 1)
+    assert np.array_equal(a.copy_spins(), b.copy_spins())
+    o = orc.Oracle(2, 256, seed=33)
+    o.sweep(BC2, 2, 32, 4); o.sweep(BC2, 3, 64, 2); o.sweep(BC2, 1, 0, 1)
+    _same_state(a, o)
+
+
+def test_set_spins_counter_resume_and_invariants(P, orc):
+    L = 128
+    g = P.Ising(2, L, seed=5)
+    up = np.ones(L * L, dtype=np.int8)
+    g.set_spins(up)
+    E, M = g.observables()
+    assert (int(E[0]), int(M[0])) == (-2 * L * L, L * L)          # E(all up) = -2N
+    g3 = P.Ising(3, 16, seed=5)
+    g3.set_spins(np.ones(16 ** 3, dtype=np.int8))
+    assert int(g3.observables()[0][0]) == -3 * 16 ** 3
+    with pytest.raises(P.IsingError):
+        g.set_spins(np.zeros(L * L, dtype=np.int8))
+    # resume: copy state + counter into a fresh handle
+    a = P.Ising(2, L, seed=9); a.sweep(BC2, 3, 32, 2)
+    b = P.Ising(2, L, seed=9); b.set_spins(a.copy_spins()); b.counter = a.counter
+    a.sweep(BC2, 2, 32, 2); b.sweep(BC2, 2, 32, 2)
+    assert np.array_equal(a.copy_spins(), b.copy_spins())
+    # Z2: start from -s0 gives -s_t
+    c = P.Ising(2, L, seed=9); s0 = c.copy_spins().copy()
+    d = P.Ising(2, L, seed=9); d.set_spins(-s0)
+    c.sweep(0.5, 3, 64, 2); d.sweep(0.5, 3, 64, 2)
+    assert np.array_equal(c.copy_spins(), -d.copy_spins())
+
+
+def test_device_pointer_outputs(P, orc):
+    import torch
+    g = P.Ising(2, 128, seed=4)
+    E = torch.zeros(5, dtype=torch.int64, device="cuda")
+    M = torch.zeros(5, dtype=torch.int64, device="cuda")
+    g.sweep_series(BC2, 5, 32, 1, E=E, M=M)
+    dst = torch.zeros(128 * 128, dtype=torch.int8, device="cuda")
+    g.copy_spins(dst)
+    o = orc.Oracle(2, 128, seed=4)
+    Eo, Mo = o.sweep_series(BC2, 5, 32, 1)
+    assert E.cpu().tolist() == Eo[:, 0].tolist() and M.cpu().tolist() == Mo[:, 0].tolist()
+    assert np.array_equal(dst.cpu().numpy(), o.spins())
+
+
+def test_argument_errors(P):
+    g = P.Ising(2, 64, seed=1)
+    for tile in (3, 5, 48, 128):
+        with pytest.raises(P.IsingError):
+            g.sweep(0.4, 1, tile, 1)
+    with pytest.raises(P.IsingError):
+        g.sweep(0.4, 1, 32, 0)
+    with pytest.raises(P.IsingError):
+        g.sweep(-0.1, 1, 32, 1)
+    with pytest.raises(P.IsingError):
+        g.sweep(float("nan"), 1, 32, 1)
+    with pytest.raises(P.IsingError):
+        P.Ising(2, 16, coupling=np.zeros(2 * 256, dtype=np.int8), seed=1)
+    g.sweep(0.4, 0, 32, 1)      # zero passes is a no-op
+    assert g.counter == 0
