@@ -32,6 +32,14 @@
 // Every exported function below is reached by at least one of those pins; none is
 // "parity unpinned".
 //
+// Two RNG->site mappings are implemented (DESIGN.md §3 reading R6; the paper is silent on
+// the generator, P:78/P:84 only say that a per-thread LCG was used and is unsafe):
+//   RNG_WORDS   S8c.3 verbatim: one full Philox output word per site.
+//   RNG_PLANES  multi-spin form: the 12 leading bits of r come from bit-planes shared by a
+//               block of 32 same-colour sites, the 20 trailing bits from a per-site call.
+// Both give every (site, half-sweep) its own uniform 32-bit r compared with the same
+// uint32 thresholds; they are different conventions, hence different trajectories.
+//
 // Build: g++ -O2 -std=c++17 -shared -fPIC ising_oracle.cpp -o liboracle_ising.so
 
 #include <cmath>
@@ -69,7 +77,11 @@ void philox4x32_10(const uint32_t ctr_in[4], const uint32_t key_in[2], uint32_t 
 }
 
 // Domain tags carried in ctr[1] (S8c.3).
-constexpr uint32_t TAG_SWEEP = 0, TAG_INIT = 1, TAG_COUPLING = 2;
+constexpr uint32_t TAG_SWEEP = 0, TAG_INIT = 1, TAG_COUPLING = 2, TAG_PLANES = 3, TAG_TAIL = 4;
+
+enum { RNG_WORDS = 0, RNG_PLANES = 1 };
+constexpr int HEAD_BITS = 12;                 // leading bits of r taken from bit-planes
+constexpr int TAIL_BITS = 32 - HEAD_BITS;     // trailing bits taken from the per-site call
 
 struct Oracle {
     int dim = 2;
@@ -82,6 +94,11 @@ struct Oracle {
     std::vector<int8_t> s;           // s[r*N + i], canonical order i = x + L*(y + L*z) (S8c.1)
     uint64_t t = 0;                  // inner sweeps done so far (S8c.6)
     int reverse_tiles = 0;           // test hook: visit the tiles of a colour in reverse order
+    int rng = RNG_PLANES;            // RNG->site mapping (see header); default = the product's
+    int use_memo = 1;                // test hook: 0 recomputes every Philox block (same values)
+    // RNG_PLANES memo: the HEAD_BITS planes of the last few blocks (direct-mapped cache)
+    struct PlaneMemo { uint64_t seed, H; uint32_t g; bool valid; uint32_t plane[HEAD_BITS]; };
+    std::vector<PlaneMemo> plane_memo;
     // one-entry memo of the last Philox block, so that the four same-colour sites that
     // share a counter do not recompute it.  Purely a cache: same values either way.
     uint32_t memo_ctr[4] = {0, 0, 0, 0};
@@ -103,7 +120,7 @@ uint32_t sweep_random(Oracle& o, uint64_t seed, uint64_t i, uint64_t H) {
                              (uint32_t)(H >> 32)};
     uint32_t key[2];
     seed_key(seed, key);
-    const bool hit = o.memo_valid && ctr[0] == o.memo_ctr[0] && ctr[1] == o.memo_ctr[1] &&
+    const bool hit = o.use_memo && o.memo_valid && ctr[0] == o.memo_ctr[0] && ctr[1] == o.memo_ctr[1] &&
                      ctr[2] == o.memo_ctr[2] && ctr[3] == o.memo_ctr[3] &&
                      key[0] == o.memo_key[0] && key[1] == o.memo_key[1];
     if (!hit) {
@@ -113,6 +130,61 @@ uint32_t sweep_random(Oracle& o, uint64_t seed, uint64_t i, uint64_t H) {
         o.memo_valid = true;
     }
     return o.memo_out[p & 3];
+}
+
+// RNG_PLANES geometry (DESIGN.md §3 R6).  Same-colour sites are addressed by their pair
+// p_x = x >> 1 inside row (y, z) (every aligned pair (2p_x, 2p_x+1) of a row holds one site of
+// each colour because L is even, S8c.3).  Rows and pairs are cut into blocks of BW pairs x
+// BH rows of y: (BW, BH) = (16, 2) in 2D, (4, 8) in 3D, so a block never straddles a tile
+// whose edge is a multiple of 32 (2D) or 8 (3D).  Inside a block
+//     bit   j = (y % BH) * BW + (p_x % BW)                       0 <= j < 32
+//     block g = ((z * GH + y / BH) * GW + p_x / BW),  GH = ceil(L / BH), GW = ceil((L/2) / BW)
+void plane_geometry(const Oracle& o, uint64_t i, uint32_t* g, int* j) {
+    const uint64_t L = (uint64_t)o.L;
+    const int x = (int)(i % L), y = (int)((i / L) % L), z = (int)(i / (L * L));
+    const int BW = (o.dim == 2) ? 16 : 4, BH = (o.dim == 2) ? 2 : 8;
+    const int px = x >> 1;
+    const int GW = ((o.L >> 1) + BW - 1) / BW, GH = (o.L + BH - 1) / BH;
+    *j = (y % BH) * BW + (px % BW);
+    *g = (uint32_t)(((uint64_t)z * GH + (uint64_t)(y / BH)) * GW + (uint64_t)(px / BW));
+}
+
+// RNG_PLANES, sweep stream of site i in half-sweep H = 2t + c(i):
+//   plane q (q = 0..HEAD_BITS-1) of block g  =  Philox(ctr = {g, TAG_PLANES + 256*(q>>2), lo32 H, hi32 H})[q & 3]
+//   head = sum_q ((plane_q >> j) & 1) << (HEAD_BITS-1-q)          (plane 0 is the most significant bit)
+//   tail = Philox(ctr = {i >> 1, TAG_TAIL, lo32 H, hi32 H})[0] >> HEAD_BITS
+//   r    = head << TAIL_BITS | tail
+uint32_t sweep_random_planes(Oracle& o, uint64_t seed, uint64_t i, uint64_t H) {
+    uint32_t g; int j;
+    plane_geometry(o, i, &g, &j);
+    uint32_t key[2];
+    seed_key(seed, key);
+    uint32_t local[HEAD_BITS];
+    const uint32_t* plane = local;
+    Oracle::PlaneMemo* m = nullptr;
+    if (o.use_memo) {
+        if (o.plane_memo.empty()) o.plane_memo.assign(4096, Oracle::PlaneMemo{0, 0, 0, false, {0}});
+        m = &o.plane_memo[g & 4095u];
+        if (m->valid && m->g == g && m->H == H && m->seed == seed) plane = m->plane;
+    }
+    if (plane == local) {
+        for (int n = 0; n < HEAD_BITS / 4; ++n) {
+            const uint32_t ctr[4] = {g, TAG_PLANES + 256u * (uint32_t)n, (uint32_t)(H & 0xffffffffu),
+                                     (uint32_t)(H >> 32)};
+            philox4x32_10(ctr, key, local + 4 * n);
+        }
+        if (m) {
+            m->seed = seed; m->H = H; m->g = g; m->valid = true;
+            std::memcpy(m->plane, local, sizeof local);
+            plane = m->plane;
+        }
+    }
+    uint32_t head = 0;
+    for (int q = 0; q < HEAD_BITS; ++q) head |= ((plane[q] >> j) & 1u) << (HEAD_BITS - 1 - q);
+    const uint32_t tctr[4] = {(uint32_t)(i >> 1), TAG_TAIL, (uint32_t)(H & 0xffffffffu), (uint32_t)(H >> 32)};
+    uint32_t tout[4];
+    philox4x32_10(tctr, key, tout);
+    return (head << TAIL_BITS) | (tout[0] >> HEAD_BITS);
 }
 
 // S8c.3, hot start: s_i = (Philox(ctr = {i >> 2, 1, 0, 0}, key = seed)[i & 3] >> 31) ? -1 : +1
@@ -163,7 +235,8 @@ void update_site(Oracle& o, int r, int x, int y, int z, uint64_t H, const uint64
     if (a <= 0) {
         flip = true;
     } else {
-        const uint64_t rnd = sweep_random(o, o.seeds[r], i, H);
+        const uint64_t rnd = (o.rng == RNG_PLANES) ? sweep_random_planes(o, o.seeds[r], i, H)
+                                                   : sweep_random(o, o.seeds[r], i, H);
         flip = rnd < thr[a / 2];
     }
     if (flip) s[i] = (int8_t)-s[i];
@@ -349,6 +422,19 @@ int oracle_set_spins(void* h, const int8_t* src) {
 
 int oracle_get_counter(void* h, uint64_t* t) { *t = ((Oracle*)h)->t; return 0; }
 int oracle_set_counter(void* h, uint64_t t) { ((Oracle*)h)->t = t; return 0; }
+// mode: 0 = RNG_WORDS (S8c.3), 1 = RNG_PLANES.  Does not touch spins or the counter.
+int oracle_set_rng(void* h, int mode) {
+    if (mode != RNG_WORDS && mode != RNG_PLANES) return -1;
+    ((Oracle*)h)->rng = mode;
+    return 0;
+}
+int oracle_get_rng(void* h) { return ((Oracle*)h)->rng; }
+int oracle_set_memo(void* h, int on) { ((Oracle*)h)->use_memo = on ? 1 : 0; return 0; }
+// the 32-bit random of (replica r, site i, half-sweep H) under the handle's current mapping
+uint32_t oracle_sweep_random(void* h, int r, uint64_t i, uint64_t H) {
+    Oracle& o = *(Oracle*)h;
+    return (o.rng == RNG_PLANES) ? sweep_random_planes(o, o.seeds[r], i, H) : sweep_random(o, o.seeds[r], i, H);
+}
 int oracle_set_tile_order(void* h, int reversed) { ((Oracle*)h)->reverse_tiles = reversed; return 0; }
 
 // S8c.8: FNV-1a-64 over the canonical bytes of replica r (0x01 for +1, 0xFF for -1).

@@ -53,6 +53,11 @@ def lib() -> C.CDLL:
         L.oracle_get_counter.argtypes = [C.c_void_p, u64p]
         L.oracle_set_counter.argtypes = [C.c_void_p, C.c_uint64]
         L.oracle_set_tile_order.argtypes = [C.c_void_p, C.c_int]
+        L.oracle_set_rng.argtypes = [C.c_void_p, C.c_int]
+        L.oracle_get_rng.argtypes = [C.c_void_p]
+        L.oracle_set_memo.argtypes = [C.c_void_p, C.c_int]
+        L.oracle_sweep_random.restype = C.c_uint32
+        L.oracle_sweep_random.argtypes = [C.c_void_p, C.c_int, C.c_uint64, C.c_uint64]
         L.oracle_hash.restype = C.c_uint64
         L.oracle_hash.argtypes = [C.c_void_p, C.c_int]
         L.oracle_hash_bytes.restype = C.c_uint64
@@ -90,10 +95,17 @@ def hash_bytes(a: np.ndarray) -> int:
     return int(lib().oracle_hash_bytes(a.ctypes.data, a.size))
 
 
-class Oracle:
-    """One lattice (or R replicas sharing one coupling array) advanced by the oracle."""
+RNG_MODES = {"words": 0, "planes": 1}
+DEFAULT_RNG = "planes"      # tests flip this to run one body under both mappings
 
-    def __init__(self, dim: int, L: int, seed=None, J: np.ndarray | None = None, seeds=None):
+
+class Oracle:
+    """One lattice (or R replicas sharing one coupling array) advanced by the oracle.
+
+    rng: "planes" (default, the product's default mapping) or "words" (SURVEY S8c.3 verbatim)."""
+
+    def __init__(self, dim: int, L: int, seed=None, J: np.ndarray | None = None, seeds=None,
+                 rng: str | None = None):
         if seeds is None:
             seeds = [seed]
         self.dim, self.L, self.N, self.R = dim, L, L ** dim, len(seeds)
@@ -106,6 +118,10 @@ class Oracle:
         self._h = lib().oracle_create_batch(dim, L, jp, _p(sd, C.c_uint64), self.R)
         if not self._h:
             raise ValueError("oracle_create_batch rejected its arguments")
+        rng = DEFAULT_RNG if rng is None else rng
+        self.rng = rng
+        if lib().oracle_set_rng(self._h, RNG_MODES[rng]) != 0:
+            raise ValueError("bad rng mode")
 
     def __del__(self):
         if getattr(self, "_h", None):
@@ -155,6 +171,13 @@ class Oracle:
     @counter.setter
     def counter(self, t: int) -> None:
         lib().oracle_set_counter(self._h, t)
+
+    def set_memo(self, on: bool) -> None:
+        lib().oracle_set_memo(self._h, int(on))
+
+    def sweep_random(self, i: int, H: int, r: int = 0) -> int:
+        """The 32-bit random of (replica r, site i, half-sweep H) under this handle's mapping."""
+        return int(lib().oracle_sweep_random(self._h, r, i, H))
 
     def set_tile_order(self, reverse: bool) -> None:
         lib().oracle_set_tile_order(self._h, int(reverse))

@@ -18,3 +18,12 @@ def orc():
     from oracle import oracle as O
     O.build()
     return O
+
+
+@pytest.fixture(params=["planes", "words"])
+def both_rngs(request, orc):
+    """Run the test body under both RNG->site mappings of the oracle (DESIGN.md §3 R6)."""
+    old = orc.DEFAULT_RNG
+    orc.DEFAULT_RNG = request.param
+    yield request.param
+    orc.DEFAULT_RNG = old

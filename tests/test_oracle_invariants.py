@@ -9,6 +9,8 @@ import pytest
 
 import ising_workloads as W
 
+pytestmark = pytest.mark.usefixtures("both_rngs")
+
 BETA_C = 0.4406868
 
 
@@ -107,30 +109,84 @@ def test_tile_size_changes_the_trajectory_but_k1_full_tile_is_plain(orc):
     assert state(a)[2] != state(c)[2]
 
 
-def test_plain_checkerboard_against_lattice_synchronous_numpy(orc):
+def _site_random(orc, rng, dim, L, i, H, seed):
+    """r(i, H) of DESIGN.md §3 R6, restated from the text on top of the KAT-pinned Philox."""
+    key, Hw = [seed & 0xFFFFFFFF, seed >> 32], [H & 0xFFFFFFFF, H >> 32]
+    if rng == "words":                       # S8c.3
+        p = i >> 1
+        return orc.philox4x32_10([p >> 2, 0] + Hw, key)[p & 3]
+    x, y, z = i % L, (i // L) % L, i // (L * L)
+    BW, BH = (16, 2) if dim == 2 else (4, 8)
+    px = x >> 1
+    GW, GH = -(-(L // 2) // BW), -(-L // BH)
+    j = (y % BH) * BW + px % BW
+    g = (z * GH + y // BH) * GW + px // BW
+    head = 0
+    for q in range(12):                      # plane 0 is the most significant bit
+        plane = orc.philox4x32_10([g, 3 + 256 * (q >> 2)] + Hw, key)[q & 3]
+        head = (head << 1) | ((plane >> j) & 1)
+    tail = orc.philox4x32_10([i >> 1, 4] + Hw, key)[0] >> 12
+    return (head << 20) | tail
+
+
+@pytest.mark.parametrize("dim,L", [(2, 8), (2, 36), (3, 4), (3, 10)])
+def test_plain_checkerboard_against_lattice_synchronous_numpy(orc, both_rngs, dim, L):
     """tile = L, J = +1: one half-sweep is a synchronous update of one colour.  Restated with
-    whole-array numpy operations and random words fetched per site from the oracle's Philox
-    (so only the schedule/neighbour/acceptance logic is re-derived here, in a different shape)."""
-    L, seed, beta = 8, 13, 0.37
-    o = orc.Oracle(2, L, seed=seed)
-    s = o.spins().astype(np.int64).reshape(L, L)
-    thr = orc.thresholds(beta, 2)
-    y, x = np.mgrid[0:L, 0:L]
-    idx = x + L * y
-    for t in range(4):
+    whole-array numpy operations; the random of every site is rebuilt here from the text of
+    the mapping (words: S8c.3; planes: block/bit geometry, 12 plane bits + 20 tail bits) using
+    only the oracle's Philox block function, which the KATs pin."""
+    seed, beta = 13 + (1 << 40), 0.37 if dim == 2 else 0.2
+    o = orc.Oracle(dim, L, seed=seed)
+    N = L ** dim
+    shape = (L,) * dim
+    s = o.spins().astype(np.int64).reshape(shape)        # index order: (z,) y, x
+    thr = list(orc.thresholds(beta, dim))
+    coords = np.indices(shape)
+    parity = coords.sum(axis=0) & 1
+    for t in range(2):
         for c in (0, 1):
             H = 2 * t + c
-            r = np.zeros((L, L), dtype=np.uint64)
-            for i in range(L * L):
-                p = i >> 1
-                r.flat[i] = orc.philox4x32_10([p >> 2, 0, H & 0xFFFFFFFF, H >> 32], [seed, 0])[p & 3]
-            nb = np.roll(s, 1, 0) + np.roll(s, -1, 0) + np.roll(s, 1, 1) + np.roll(s, -1, 1)
+            r = np.array([_site_random(orc, both_rngs, dim, L, i, H, seed) for i in range(N)],
+                         dtype=np.uint64).reshape(shape)
+            nb = sum(np.roll(s, sh, ax) for ax in range(dim) for sh in (1, -1))
             a = s * nb
-            t_sel = np.where(a == 2, thr[0], np.where(a == 4, thr[1], 0)).astype(np.uint64)
-            flip = ((a <= 0) | (r < t_sel)) & (((x + y) & 1) == c)
+            t_sel = np.zeros(shape, dtype=np.uint64)
+            for m in range(1, dim + 1):
+                t_sel = np.where(a == 2 * m, np.uint64(thr[m - 1]), t_sel)
+            flip = ((a <= 0) | (r < t_sel)) & (parity == c)
             s = np.where(flip, -s, s)
-    o.sweep(beta, 4, L, 1)
-    assert np.array_equal(o.spins().astype(np.int64).reshape(L, L), s)
+    o.sweep(beta, 2, L, 1)
+    assert np.array_equal(o.spins().astype(np.int64).reshape(shape), s)
+    # the exported per-site random agrees with the restatement, memo on or off
+    o.set_memo(False)
+    for i in (0, 1, N // 2 + 3, N - 1):
+        assert o.sweep_random(i, 5) == _site_random(orc, both_rngs, dim, L, i, 5, seed)
+
+
+def test_plane_randoms_are_distinct_bits(orc):
+    """Planes mapping: the 32 sites of a block take different bit positions of the same planes
+    and every active site of a half-sweep owns a distinct (block, bit) — no random bit is used
+    twice in a half-sweep.  Checked by brute force on small lattices, both dimensions."""
+    for dim, L in ((2, 6), (2, 34), (3, 4), (3, 10)):
+        N = L ** dim
+        BW, BH = (16, 2) if dim == 2 else (4, 8)
+        GW, GH = -(-(L // 2) // BW), -(-L // BH)
+        for c in (0, 1):
+            seen = set()
+            for i in range(N):
+                x, y, z = i % L, (i // L) % L, i // (L * L)
+                if (x + y + z) & 1 != c:
+                    continue
+                key = ((z * GH + y // BH) * GW + (x >> 1) // BW, (y % BH) * BW + (x >> 1) % BW)
+                assert key not in seen and 0 <= key[1] < 32
+                seen.add(key)
+
+
+def test_memo_is_only_a_cache(orc):
+    a = orc.Oracle(2, 16, seed=5); b = orc.Oracle(2, 16, seed=5)
+    b.set_memo(False)
+    a.sweep(BETA_C, 3, 4, 2); b.sweep(BETA_C, 3, 4, 2)
+    assert a.hash() == b.hash()
 
 
 @pytest.mark.parametrize("dim,L,tile,k", [(2, 16, 4, 2), (3, 6, 6, 1)])

@@ -11,6 +11,8 @@ import math
 import numpy as np
 import pytest
 
+pytestmark = pytest.mark.usefixtures("both_rngs")
+
 BETA_C = 0.4406868
 
 

@@ -105,7 +105,7 @@ def _run_case(orc, case, max_pass):
     J = None
     if "jseed" in case:
         J = W.couplings(case["dim"], case["L"], case["jseed"])
-    o = orc.Oracle(case["dim"], case["L"], seed=case["seed"], J=J)
+    o = orc.Oracle(case["dim"], case["L"], seed=case["seed"], J=J, rng="words")
     done = 0
     for p, E, M, h in case["checkpoints"]:
         if p > max_pass:
@@ -145,7 +145,7 @@ def test_survey_trajectories_medium(orc, case, max_pass):
 def test_survey_overlap_pass0(orc):
     """Q_ab of two hot starts sharing J (A.5): replica batching + overlap."""
     J = W.couplings(2, 4096, 5)
-    o = orc.Oracle(2, 4096, seeds=[100, 101, 114, 115], J=J)
+    o = orc.Oracle(2, 4096, seeds=[100, 101, 114, 115], J=J, rng="words")
     assert o.overlap(0, 1) == GOLD["config5_overlaps"]["100,101"]["0"]
     assert o.overlap(2, 3) == GOLD["config5_overlaps"]["114,115"]["0"]
     assert o.overlap(1, 1) == 4096 * 4096
