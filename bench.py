@@ -91,11 +91,11 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
-def oracle_flips_per_ns(L: int, tile: int, k: int, passes: int):
+def oracle_flips_per_ns(L: int, tile: int, k: int, passes: int, rng: str = "planes"):
     """Time the CPU oracle as it stands: `passes` outer passes on an L x L lattice, 1 core."""
     from oracle import oracle as O
     O.build()
-    o = O.Oracle(2, L, seed=3)
+    o = O.Oracle(2, L, seed=3, rng=rng)
     t0 = time.perf_counter()
     o.sweep(W.BETA_C_2D, passes, tile, k)
     dt = time.perf_counter() - t0
@@ -108,7 +108,7 @@ def run_reference(a, rank: int, world: int) -> None:
     Ls = 4096                                   # bounded sample: 1/16 of the L=16384 sites per step
     per_step = []
     for i in range(a.warmup + a.steps):
-        v, dt = oracle_flips_per_ns(Ls, a.tile, a.k, 1)
+        v, dt = oracle_flips_per_ns(Ls, a.tile, a.k, 1, a.rng)
         if i >= a.warmup:
             per_step.append(dt)
     tot = sum(per_step)
@@ -123,9 +123,9 @@ def run_reference(a, rank: int, world: int) -> None:
     print(json.dumps(line), flush=True)
 
 
-def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None):
-    """Device-timed throughput of one (layout, tile, k) variant; returns dict."""
-    g = P.Ising(2, L, seed=3)
+def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng="planes"):
+    """Device-timed throughput of one (rng, layout, tile, k) variant; returns dict."""
+    g = P.Ising(2, L, seed=3, rng=rng)
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
     g.sweep(W.BETA_C_2D, warmup, tile, k)
@@ -152,10 +152,10 @@ def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None):
     return {"ms": ms, "flips_per_ns": flips / (ms * 1e6), "launches": int(launches), "path": path, "clocks": clocks}
 
 
-def time_e2e(P, torch, L, layout, tile, k, steps):
+def time_e2e(P, torch, L, layout, tile, k, steps, rng="planes"):
     """Same metric through the public API with HOST buffers: every step uploads the spins from
     pinned host memory (ising_set_spins), runs one pass, and reads them back (ising_copy_spins)."""
-    g = P.Ising(2, L, seed=3)
+    g = P.Ising(2, L, seed=3, rng=rng)
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
     host = torch.empty(L * L, dtype=torch.int8).pin_memory()
@@ -185,6 +185,7 @@ def main() -> None:
     ap.add_argument("--layout", default="int8", choices=["int8", "bits"])
     ap.add_argument("--tile", type=int, default=64)
     ap.add_argument("--k", type=int, default=1)
+    ap.add_argument("--rng", default="planes", choices=["planes", "words"], help="RNG->site mapping (DESIGN.md R6)")
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the k/tile table")
     a = ap.parse_args()
@@ -215,7 +216,7 @@ def main() -> None:
 
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
-    res = time_variant(P, torch, L, a.layout, a.tile, a.k, a.steps, a.warmup, sampler)
+    res = time_variant(P, torch, L, a.layout, a.tile, a.k, a.steps, a.warmup, sampler, a.rng)
     barrier()
     ms = res["ms"]
     if dist is not None:
@@ -235,28 +236,28 @@ def main() -> None:
             "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "u8" if a.layout == "int8" else "u32 bit-planes", "data": "synthetic",
             "config": {"workload": f"BASELINE config 3: 2D Ising L={L} hot start seed 3 beta=0.4406868 layout={a.layout} "
-                                   f"tile={a.tile} k={a.k}; one step = one outer pass (2 launches)",
+                                   f"rng={a.rng} tile={a.tile} k={a.k}; one step = one outer pass (2 launches)",
                        "l2": "lattice (256 MiB int8) exceeds the 126 MB L2; no explicit flush" if a.layout == "int8"
                              else "lattice (32 MiB bits) fits L2: bit-packed variant is ALU-bound, not an HBM claim",
                        "kernel_path": res["path"], "parallelism": "replicas only" if world > 1 else "single GPU"},
             "ns_per_flip": 1.0 / value, "gpu_launches": res["launches"], "clocks": res["clocks"],
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": None, "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
-                         "algorithmic_bytes_per_flip": bpf, "kernel": f"k_tile_{'i8' if a.layout == 'int8' else 'bits'}<{a.tile}>",
+                         "algorithmic_bytes_per_flip": bpf, "kernel": f"{res['path']}<{a.tile}>",
                          "avg_launch_ms": launch_ms}}
     if rank == 0 and not a.no_extras and world == 1:
         table = {}
-        for lay in ("int8",):
+        for rng, lay in (("planes", "int8"), ("planes", "bits"), ("words", "int8")):
             for T in (32, 64):
                 for k in (1, 4, 16):
                     st = max(2, min(a.steps, 40 // k))
-                    r = time_variant(P, torch, L, lay, T, k, st, 3)
-                    table[f"{lay}_t{T}_k{k}"] = {"flips_per_ns": round(r["flips_per_ns"], 1), "steps": st,
+                    r = time_variant(P, torch, L, lay, T, k, st, 3, None, rng)
+                    table[f"{rng}_{lay}_t{T}_k{k}"] = {"flips_per_ns": round(r["flips_per_ns"], 1), "steps": st,
                                                 "hbm_GBs": round(r["flips_per_ns"] * algorithmic_bytes_per_flip(T, k, lay), 1)}
         line["variants"] = table
-        line["e2e"] = time_e2e(P, torch, L, a.layout, a.tile, a.k, 3)
+        line["e2e"] = time_e2e(P, torch, L, a.layout, a.tile, a.k, 3, a.rng)
         ncores = 1
-        v, dt = oracle_flips_per_ns(L, a.tile, a.k, 2)
+        v, dt = oracle_flips_per_ns(L, a.tile, a.k, 2, a.rng)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": ncores, "kind": "oracle",
                                 "sample": f"2 outer passes of the full L={L} lattice (tile {a.tile}, k {a.k}), {dt:.1f} s, "
                                           f"host has {os.cpu_count()} cores, oracle is sequential"}

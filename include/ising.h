@@ -49,6 +49,11 @@ enum {
     ISING_LAYOUT_BITS = 1    /* one bit per spin in HBM (synchronous multi-spin form) */
 };
 
+enum {
+    ISING_RNG_WORDS = 0,     /* one Philox4x32-10 output word per site          */
+    ISING_RNG_PLANES = 1     /* default: 12 bit-plane bits per 32-site block + 20 per-site bits */
+};
+
 /* ising_create — P:53-57; S8c.1-3.
  * dim ∈ {2,3}; L even, ≥ 2, N = L^dim ≤ 2^32.  coupling_or_null [host|device]: NULL ⇒
  * J = +1 on every bond (eq. (1)); otherwise int8 J[dim][N], J[d][i] = bond between site i
@@ -99,6 +104,18 @@ int ising_set_spins(ising_handle h, const int8_t* src);
 /* ising_set_layout — ISING_LAYOUT_I8 or ISING_LAYOUT_BITS: how spins are held in HBM between
  * sweeps.  The trajectory does not depend on it (S8c: both layouts give the same bits). */
 int ising_set_layout(ising_handle h, int layout);
+
+/* ising_set_rng — which RNG->site mapping the sweeps use (the paper names no generator, P:78,
+ * P:84; DESIGN.md §3 R6 defines both).  Every (site, half-sweep) gets its own uniform 32-bit r
+ * from Philox4x32-10 keyed by the seed, compared with the same uint32 thresholds:
+ *   ISING_RNG_WORDS   r = Philox(ctr={p>>2, 0, lo32 H, hi32 H})[p&3], p = i>>1 (S8c.3).
+ *   ISING_RNG_PLANES  (default) sites of one colour are cut into blocks of 32 (16 pairs x 2 rows
+ *     in 2D, 4 pairs x 8 rows in 3D); bit j of plane q = Philox(ctr={g, 3+256*(q>>2), lo32 H,
+ *     hi32 H})[q&3] is bit (11-q) of the 12-bit head of site j of block g; the 20-bit tail is
+ *     Philox(ctr={i>>1, 4, lo32 H, hi32 H})[0] >> 12; r = head<<20 | tail.
+ * The two mappings are different valid Markov chains (different trajectories).  May be called
+ * at any time; spins and t are untouched. */
+int ising_set_rng(ising_handle h, int mode);
 
 /* The state of a run is (spins, t, seed): the random stream is stateless (S8c.3), so
  * copy_spins + get_counter / set_spins + set_counter resume a run bit-exactly. */

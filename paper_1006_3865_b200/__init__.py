@@ -3,8 +3,8 @@
 The product is the C-ABI library `libising_b200.so` (include/ising.h, csrc/*.cu, sm_100a);
 `binding` marshals arguments to it.  Nothing in this package imports `oracle/`.
 """
-from .binding import (ISING_LAYOUT_BITS, ISING_LAYOUT_I8, SYMBOLS, Ising, IsingError,
+from .binding import (ISING_LAYOUT_BITS, ISING_LAYOUT_I8, ISING_RNG_PLANES, ISING_RNG_WORDS, SYMBOLS, Ising, IsingError,
                       ising_kernel_launches, ising_thresholds, lib, use_torch)
 
-__all__ = ["Ising", "IsingError", "ISING_LAYOUT_I8", "ISING_LAYOUT_BITS", "SYMBOLS", "lib",
+__all__ = ["Ising", "IsingError", "ISING_LAYOUT_I8", "ISING_LAYOUT_BITS", "ISING_RNG_WORDS", "ISING_RNG_PLANES", "SYMBOLS", "lib",
            "use_torch", "ising_thresholds", "ising_kernel_launches"]

@@ -17,10 +17,13 @@ from . import build as _build
 
 ISING_LAYOUT_I8 = 0
 ISING_LAYOUT_BITS = 1
+ISING_RNG_WORDS = 0
+ISING_RNG_PLANES = 1
+RNG_MODES = {"words": ISING_RNG_WORDS, "planes": ISING_RNG_PLANES}
 
 SYMBOLS = [
     "ising_create", "ising_create_batch", "ising_destroy", "ising_sweep", "ising_sweep_series",
-    "ising_observables", "ising_overlap", "ising_copy_spins", "ising_set_spins", "ising_set_layout",
+    "ising_observables", "ising_overlap", "ising_copy_spins", "ising_set_spins", "ising_set_layout", "ising_set_rng",
     "ising_get_counter", "ising_set_counter", "ising_thresholds", "ising_set_device_hooks",
     "ising_synchronize", "ising_kernel_launches", "ising_sweep_path", "ising_force_path",
     "ising_last_error",
@@ -61,6 +64,7 @@ def lib() -> C.CDLL:
     L.ising_copy_spins.argtypes = [vp, i8p]
     L.ising_set_spins.argtypes = [vp, i8p]
     L.ising_set_layout.argtypes = [vp, C.c_int]
+    L.ising_set_rng.argtypes = [vp, C.c_int]
     L.ising_get_counter.argtypes = [vp, u64p]
     L.ising_set_counter.argtypes = [vp, C.c_uint64]
     L.ising_thresholds.argtypes = [C.c_double, C.c_int, u64p]
@@ -129,7 +133,8 @@ def ising_kernel_launches() -> int:
 class Ising:
     """Owner of one `ising_handle`; methods are the C calls of include/ising.h minus the prefix."""
 
-    def __init__(self, dim: int, L: int, coupling=None, seed: int | None = None, seeds=None):
+    def __init__(self, dim: int, L: int, coupling=None, seed: int | None = None, seeds=None,
+                 rng: str | None = None):
         if seeds is None:
             seeds = [0 if seed is None else seed]
         sd = np.asarray(list(seeds), dtype=np.uint64)
@@ -139,6 +144,8 @@ class Ising:
         self._h = lib().ising_create_batch(dim, L, _ptr(coupling), _ptr(sd), self.R)
         if not self._h:
             raise IsingError(f"ising_create failed: {lib().ising_last_error().decode()}")
+        if rng is not None:
+            self.set_rng(rng)
 
     def destroy(self):
         if getattr(self, "_h", None):
@@ -182,6 +189,9 @@ class Ising:
             src = np.ascontiguousarray(src, dtype=np.int8).reshape(-1)
             assert src.size == self.R * self.N
         _check(lib().ising_set_spins(self._h, _ptr(src)))
+
+    def set_rng(self, mode) -> None:
+        _check(lib().ising_set_rng(self._h, RNG_MODES[mode] if isinstance(mode, str) else int(mode)))
 
     def set_layout(self, layout: int) -> None:
         _check(lib().ising_set_layout(self._h, int(layout)))

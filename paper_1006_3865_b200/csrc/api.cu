@@ -101,8 +101,12 @@ static bool tile_valid(const ising_ctx* h, int T) {
 
 // ---- storage bookkeeping --------------------------------------------------------------
 static int to_canon_scratch(ising_ctx* h) {   // tiles -> d_canon, store state unchanged
-    if (h->store == Store::TileI8) return launch_tile_i8_to_canon(h, h->store_tile, h->d_tiles, h->d_canon);
-    return 0;
+    switch (h->store) {
+        case Store::TileI8: return launch_tile_i8_to_canon(h, h->store_tile, h->d_tiles, h->d_canon);
+        case Store::PlaneI8: return launch_planes_to_canon(h, h->store_tile, false, h->d_tiles, h->d_canon);
+        case Store::PlaneBits: return launch_planes_to_canon(h, h->store_tile, true, h->d_tiles, h->d_canon);
+        default: return 0;
+    }
 }
 
 static int ensure_canon(ising_ctx* h) {
@@ -114,11 +118,12 @@ static int ensure_canon(ising_ctx* h) {
     return 0;
 }
 
-static int ensure_tile_i8(ising_ctx* h, int T) {
-    if (h->store == Store::TileI8 && h->store_tile == T) return 0;
+// Bring the spins into tile records of `kind` for tile edge T (re-laid out through the canonical array).
+static int ensure_store(ising_ctx* h, Store kind, int T) {
+    if (h->store == kind && h->store_tile == T) return 0;
     int rc = ensure_canon(h);
     if (rc) return rc;
-    const size_t need = tile_i8_bytes(h, T);
+    const size_t need = kind == Store::TileI8 ? tile_i8_bytes(h, T) : tile_planes_bytes(h, T, kind == Store::PlaneBits);
     if (need > h->tiles_bytes) {
         ISING_CUDA_OK(cudaStreamSynchronize(hooks().stream));
         dev_free(h->d_tiles);
@@ -127,9 +132,10 @@ static int ensure_tile_i8(ising_ctx* h, int T) {
         if (!h->d_tiles) return ISING_ENOMEM;
         h->tiles_bytes = need;
     }
-    rc = launch_canon_to_tile_i8(h, T, h->d_canon, h->d_tiles);
+    rc = kind == Store::TileI8 ? launch_canon_to_tile_i8(h, T, h->d_canon, h->d_tiles)
+                               : launch_canon_to_planes(h, T, kind == Store::PlaneBits, h->d_canon, h->d_tiles);
     if (rc) return rc;
-    h->store = Store::TileI8;
+    h->store = kind;
     h->store_tile = T;
     return 0;
 }
@@ -279,24 +285,28 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
     }
     int rc = 0;
     const bool thr_fits = !(acc.thr_is_2p32[0] || acc.thr_is_2p32[1] || acc.thr_is_2p32[2]);   // beta = 0 only
-    const bool use_tile_i8 = !h->force_generic && thr_fits && h->layout == ISING_LAYOUT_I8 && tile_i8_supported(h, T);
-    if (use_tile_i8) {
-        h->last_path = "tile_i8";
-        rc = ensure_tile_i8(h, T);
+    const bool use_tile_i8 = !h->force_generic && thr_fits && h->rng == ISING_RNG_WORDS &&
+                             h->layout == ISING_LAYOUT_I8 && tile_i8_supported(h, T);
+    const bool use_planes = !h->force_generic && h->rng == ISING_RNG_PLANES && tile_planes_supported(h, T);
+    if (use_tile_i8 || use_planes) {
+        const bool bits = h->layout == ISING_LAYOUT_BITS;
+        h->last_path = use_tile_i8 ? "tile_i8" : (bits ? "tile_planes_bits" : "tile_planes_i8");
+        rc = ensure_store(h, use_tile_i8 ? Store::TileI8 : (bits ? Store::PlaneBits : Store::PlaneI8), T);
         for (int pass = 0; pass < n && !rc; ++pass) {
-            rc = launch_tile_i8_pass(h, acc, T, k, h->t + (uint64_t)pass * (uint64_t)k);
+            const uint64_t t0 = h->t + (uint64_t)pass * (uint64_t)k;
+            rc = use_tile_i8 ? launch_tile_i8_pass(h, acc, T, k, t0) : launch_tile_planes_pass(h, acc, T, bits, k, t0);
             if (!rc && want_series) {
                 rc = to_canon_scratch(h);
                 if (!rc) rc = launch_observables_canon(h, h->d_canon, d_E ? d_E + (size_t)pass * h->R : nullptr,
                                                        d_M ? d_M + (size_t)pass * h->R : nullptr);
             }
         }
-    } else if (h->layout == ISING_LAYOUT_I8) {
+    } else if (h->layout == ISING_LAYOUT_I8 || h->force_generic) {
         h->last_path = "generic";
         rc = ensure_canon(h);
         if (!rc) rc = launch_generic_sweep(h, acc, n, T, k, d_E, d_M);
     } else {
-        set_error("ising_sweep: no bit-packed kernel for dim=%d L=%d tile=%d", h->dim, h->L, T);
+        set_error("ising_sweep: no bit-packed kernel for dim=%d L=%d tile=%d rng=%d", h->dim, h->L, T, h->rng);
         rc = ISING_EUNSUPPORTED;
     }
     if (!rc) h->t += (uint64_t)n * (uint64_t)k;
@@ -385,6 +395,15 @@ int ising_set_layout(ising_handle h, int layout) {
     const int rc = ensure_canon(h);
     if (rc) return rc;
     h->layout = layout;
+    return 0;
+}
+
+int ising_set_rng(ising_handle h, int mode) {
+    if (!h || (mode != ISING_RNG_WORDS && mode != ISING_RNG_PLANES)) {
+        set_error("ising_set_rng: mode must be ISING_RNG_WORDS or ISING_RNG_PLANES");
+        return ISING_EINVAL;
+    }
+    h->rng = mode;
     return 0;
 }
 

@@ -39,7 +39,8 @@ void dev_free(void* p);
 enum class Store : int {
     Canon = 0,   // int8 ±1, index order, R*N bytes (generic kernels, observables, I/O)
     TileI8 = 1,  // tile records of 0/1 bytes, colour-split rows + edge columns (tile_i8.cu)
-    TileBits = 2 // tile records of bits (tile_bits.cu)
+    PlaneI8 = 2, // piece-major tile records of 0/1 bytes (tile_planes.cu)
+    PlaneBits = 3 // tile records of bit words (tile_planes.cu)
 };
 
 // Acceptance constants handed to every sweep kernel (S8c.4/5).
@@ -69,11 +70,12 @@ struct ising_ctx {
     std::vector<uint64_t> seeds;
     uint64_t t = 0;                 // inner sweeps done (S8c.6)
 
+    int rng = ISING_RNG_PLANES;     // RNG->site mapping (DESIGN.md §3 R6)
     int layout = ISING_LAYOUT_I8;   // requested HBM layout
     ising::Store store = ising::Store::Canon;
     int store_tile = 0;             // T of the tile records when store != Canon
     int8_t* d_canon = nullptr;      // R*N bytes; valid iff store == Canon (else scratch)
-    void* d_tiles = nullptr;        // tile-record storage (TileI8 / TileBits)
+    void* d_tiles = nullptr;        // tile-record storage (TileI8 / PlaneI8 / PlaneBits)
     size_t tiles_bytes = 0;
     void* d_Jtiles = nullptr;       // couplings in tile-record form for store_tile
     int Jtiles_tile = 0;

@@ -89,6 +89,73 @@ __global__ void k_generic_halfsweep(int8_t* __restrict__ spins, const int8_t* __
     if (flip) s[i] = (int8_t)(-si);
 }
 
+// RNG mapping "planes" (DESIGN.md §3 R6): one thread per (replica, block g of 32 same-colour
+// sites).  The 12 head planes of the block come from three Philox calls; the thread then
+// walks its 32 bits.  The 20-bit tail of a site is drawn only when its head equals the head
+// of the threshold it is compared with (probability 2^-12).
+__global__ void k_generic_halfsweep_planes(int8_t* __restrict__ spins, const int8_t* __restrict__ J,
+                                           const uint64_t* __restrict__ seeds, GenericGeom g,
+                                           Accept acc, uint64_t H, int C, int c) {
+    const int BW = (g.dim == 2) ? 16 : 4, BH = (g.dim == 2) ? 2 : 8;
+    const int PW = g.L >> 1;
+    const int GW = (PW + BW - 1) / BW, GH = (g.L + BH - 1) / BH;
+    const int Lz = (g.dim == 3) ? g.L : 1;
+    const uint64_t blocks = (uint64_t)GW * GH * Lz;
+    const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= blocks * (uint64_t)g.R) return;
+    const uint64_t r = gid / blocks;
+    const uint32_t blk = (uint32_t)(gid - r * blocks);
+    const int pb = (int)(blk % GW), yb = (int)((blk / GW) % GH), z = (int)(blk / ((uint32_t)GW * GH));
+    uint32_t k0, k1;
+    key_of(seeds[r], k0, k1);
+    const uint32_t Hlo = (uint32_t)(H & 0xffffffffull), Hhi = (uint32_t)(H >> 32);
+    uint32_t plane[kHeadBits];
+#pragma unroll
+    for (int n = 0; n < kHeadBits / 4; ++n) {
+        const u32x4 o = philox4x32_10(blk, kTagPlanes + 256u * n, Hlo, Hhi, k0, k1);
+        plane[4 * n] = o.x; plane[4 * n + 1] = o.y; plane[4 * n + 2] = o.z; plane[4 * n + 3] = o.w;
+    }
+    int8_t* s = spins + r * g.N;
+    const uint64_t L = (uint64_t)g.L;
+    for (int j = 0; j < 32; ++j) {
+        const int y = yb * BH + j / BW, px = pb * BW + j % BW;
+        if (y >= g.L || px >= PW) continue;
+        const int x = 2 * px + ((y + z + c) & 1);
+        if ((((x / g.T) + (y / g.T) + (z / g.T)) & 1) != C) continue;
+        const uint64_t i = (uint64_t)x + L * ((uint64_t)y + L * (uint64_t)z);
+        const int coord[3] = {x, y, z};
+        uint64_t stride = 1;
+        const int si = s[i];
+        int n_sat = 0;
+        for (int d = 0; d < g.dim; ++d) {
+            const uint64_t ip = (coord[d] == g.L - 1) ? i - (L - 1) * stride : i + stride;
+            const uint64_t im = (coord[d] == 0) ? i + (L - 1) * stride : i - stride;
+            const int Jp = J ? (int)J[(uint64_t)d * g.N + i] : 1;
+            const int Jm = J ? (int)J[(uint64_t)d * g.N + im] : 1;
+            n_sat += (Jp * si * s[ip] > 0) + (Jm * si * s[im] > 0);
+            stride *= L;
+        }
+        const int a = 2 * n_sat - 2 * g.dim;
+        bool flip = true;
+        if (a > 0) {
+            const int m = a / 2 - 1;
+            if (!acc.thr_is_2p32[m]) {
+                uint32_t head = 0;
+#pragma unroll
+                for (int q = 0; q < kHeadBits; ++q) head |= ((plane[q] >> j) & 1u) << (kHeadBits - 1 - q);
+                const uint32_t th = acc.thr[m] >> kTailBits;
+                if (head != th) {
+                    flip = head < th;
+                } else {
+                    const u32x4 o = philox4x32_10((uint32_t)(i >> 1), kTagTail, Hlo, Hhi, k0, k1);
+                    flip = (o.x >> kHeadBits) < (acc.thr[m] & ((1u << kTailBits) - 1u));
+                }
+            }
+        }
+        if (flip) s[i] = (int8_t)(-si);
+    }
+}
+
 __device__ __forceinline__ long long warp_sum(long long v) {
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
@@ -215,14 +282,22 @@ int launch_generic_sweep(ising_ctx* h, const Accept& acc, int n, int T, int k, l
     GenericGeom g{h->dim, h->L, T, h->R, h->N};
     const uint64_t total = (h->N >> 1) * (uint64_t)h->R;
     const unsigned blocks = (unsigned)((total + kThreads - 1) / kThreads);
+    const int BW = (h->dim == 2) ? 16 : 4, BH = (h->dim == 2) ? 2 : 8;
+    const uint64_t nblk = (uint64_t)(((h->L >> 1) + BW - 1) / BW) * ((h->L + BH - 1) / BH) *
+                          (h->dim == 3 ? h->L : 1) * (uint64_t)h->R;
+    const unsigned pblocks = (unsigned)((nblk + kThreads - 1) / kThreads);
     const int ncol = (T == h->L) ? 1 : 2;   // one tile: the odd coarse phase is empty
     for (int pass = 0; pass < n; ++pass) {
         for (int C = 0; C < ncol; ++C)
             for (int j = 0; j < k; ++j) {
                 const uint64_t t = h->t + (uint64_t)pass * (uint64_t)k + (uint64_t)j;
                 for (int c = 0; c < 2; ++c) {
-                    k_generic_halfsweep<<<blocks, kThreads, 0, st>>>(h->d_canon, h->d_J, h->d_seeds,
-                                                                     g, acc, 2 * t + c, C, c);
+                    if (h->rng == ISING_RNG_PLANES)
+                        k_generic_halfsweep_planes<<<pblocks, kThreads, 0, st>>>(h->d_canon, h->d_J, h->d_seeds,
+                                                                                 g, acc, 2 * t + c, C, c);
+                    else
+                        k_generic_halfsweep<<<blocks, kThreads, 0, st>>>(h->d_canon, h->d_J, h->d_seeds,
+                                                                         g, acc, 2 * t + c, C, c);
                     count_launch();
                 }
             }

@@ -20,4 +20,11 @@ int launch_canon_to_tile_i8(ising_ctx* h, int T, const int8_t* d_canon, void* d_
 int launch_tile_i8_to_canon(ising_ctx* h, int T, const void* d_tiles, int8_t* d_canon);
 int launch_tile_i8_pass(ising_ctx* h, const Accept& acc, int T, int k, uint64_t t_first);
 
+// ---- tile_planes.cu: 2D multi-spin tile kernel (RNG mapping "planes"), int8 or bit records ----
+bool tile_planes_supported(const ising_ctx* h, int T);
+size_t tile_planes_bytes(const ising_ctx* h, int T, bool bits);
+int launch_canon_to_planes(ising_ctx* h, int T, bool bits, const int8_t* d_canon, void* d_tiles);
+int launch_planes_to_canon(ising_ctx* h, int T, bool bits, const void* d_tiles, int8_t* d_canon);
+int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, int k, uint64_t t_first);
+
 }  // namespace ising

@@ -14,6 +14,10 @@ constexpr uint32_t kPhiloxW1 = 0xBB67AE85u;
 // Stream tags carried in ctr[1] (S8c.3).
 constexpr uint32_t kTagSweep = 0u;
 constexpr uint32_t kTagInit = 1u;
+constexpr uint32_t kTagPlanes = 3u;   // RNG mapping "planes": head planes of a 32-site block, call n adds 256*n
+constexpr uint32_t kTagTail = 4u;     // RNG mapping "planes": per-site tail bits
+constexpr int kHeadBits = 12;         // leading bits of r taken from bit-planes (DESIGN.md §3 R6)
+constexpr int kTailBits = 32 - kHeadBits;
 
 struct u32x4 { uint32_t x, y, z, w; };
 

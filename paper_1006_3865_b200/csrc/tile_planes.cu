@@ -1,0 +1,447 @@
+// tile_planes.cu — the 2D double-checkerboard tile kernel in multi-spin (bit-plane) form,
+// RNG mapping "planes" (DESIGN.md §3 R6, §5, §6).  Steps a1, a3-a7 of SURVEY §8(a).
+//
+// Arithmetic form.  A 32-bit word holds the 32 same-colour sites of one RNG block: 16 pairs
+// p_x x 2 rows, bit j = (y & 1) * 16 + (p_x & 15).  For a half-sweep of colour c the four
+// neighbours of all 32 sites are four words of the other colour (same block; same block with
+// its halves swapped; the blocks above/below; the block shifted by one pair), so
+//   disagreement masks, a 4-input bit adder, and
+//   flip = [n_dis >= 2] | [n_dis >= 1] & R1 | R2,    R_m = [r < thr[m]] per site
+// cost ~10 LOP3 per 32 sites.  R_m comes from the 12 head planes of the block (3 Philox calls)
+// by a bit-serial borrow chain against the head bits of thr[m] (uniform operands), LSB plane
+// first; a site whose head equals the head of a threshold it needs (probability 2^-12) draws its
+// 20 tail bits from the per-site call.  Everything runs in registers: a warp owns 64 tile rows
+// (one 64x64 tile or two 32x32 tiles), lane = block row, vertical neighbours come by shuffle,
+// the k inner sweeps never touch memory.
+//
+// HBM layouts (tile records; a tile and every piece of its halo are contiguous 16-byte runs):
+//   int8  record = T*T body + 2T edge bytes, 0/1 per spin.  Body is piece-major: the 16 bytes
+//         (row 2Y+rp, colour cc, pairs 16gx..16gx+15) sit at ((rp*2+cc)*NW+gx)*LPT*16 + Y*16, so lane Y
+//         loads its 4*NW pieces with fully coalesced 128-bit accesses and no shared-memory staging.
+//         Then T bytes left edge column (x = 0) and T bytes right edge column (x = T-1) by row.
+//   bits  record = T*T/8 bytes: word (cc, Y, gx) at ((cc*NW+gx)*LPT + Y)*4.
+#include "kernels.h"
+#include "philox.cuh"
+
+namespace ising {
+
+namespace {
+
+template <int T>
+struct PG {
+    static constexpr int NW = T / 32;            // RNG blocks (words) per colour per lane
+    static constexpr int LPT = T / 2;            // lanes per tile = block rows
+    static constexpr int TPW = 64 / T;           // tiles per warp job
+    static constexpr int NCH = 4 * NW;           // 16-byte pieces per lane
+    static constexpr int BODY = T * T;
+    static constexpr int REC_I8 = T * T + 2 * T;
+    static constexpr int REC_BITS = T * T / 8;
+};
+
+struct PlaneArgs {
+    uint8_t* tiles;              // records, replica-major
+    const uint64_t* seeds;
+    int L, B, R;
+    int C;                       // coarse colour of this launch
+    int k;
+    uint64_t t_first;            // inner-sweep index of the first of the k sweeps
+    uint32_t njobs;
+    uint32_t u1[kHeadBits];      // plane q: all-ones if bit (31-q) of thr[1] is set, else 0
+    uint32_t u2[kHeadBits];      // same for thr[2]
+    uint32_t t1_tail, t2_tail;   // thr[m] & (2^20 - 1)
+    uint32_t force1, force2;     // all-ones if thr[m] = 2^32 (beta = 0: every r is below it), else 0
+};
+
+template <int LUT>
+__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
+    uint32_t r;
+    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(r) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+    return r;
+}
+// LOP3 immediates: value of f(a,b,c) at bit (a<<2 | b<<1 | c), a = 0xF0, b = 0xCC, c = 0xAA.
+constexpr int kLutChain = (~0xF0 & 0xAA) | (~(0xF0 ^ 0xAA) & 0xCC);    // (~p & u) | (~(p ^ u) & bw): p=a, bw=b, u=c
+constexpr int kLutNe = 0xF0 | (0xCC ^ 0xAA);                            // ne | (p ^ u): ne=a, p=b, u=c
+
+// Own-tile data is read once and written back by the same lane: plain (coherent) loads that
+// do not allocate in L1.  Halo data belongs to tiles of the other coarse colour, which this
+// launch never writes, so it may use the read-only path (__ldg).
+__device__ __forceinline__ uint4 ldg128(const void* p) {
+    uint4 v;
+    asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint32_t ldg32(const void* p) {
+    uint32_t v;
+    asm volatile("ld.global.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void stg128(void* p, uint4 v) {
+    asm volatile("st.global.v4.u32 [%4], {%0,%1,%2,%3};" ::"r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(p) : "memory");
+}
+
+// 4 bytes of 0/1 -> 4 bits in the top nibble: b0 -> bit 28, ..., b3 -> bit 31 (no carries collide).
+__device__ __forceinline__ uint32_t pack_step(uint32_t acc, uint32_t w) {
+    return __funnelshift_l(w * 0x10204080u, acc, 4);     // (acc << 4) | nibble
+}
+// 16 bytes (pairs 0..15) appended below acc: acc = (acc << 16) | bits, bit k = byte k.
+__device__ __forceinline__ uint32_t pack16(uint32_t acc, const uint4& v) {
+    acc = pack_step(acc, v.w);
+    acc = pack_step(acc, v.z);
+    acc = pack_step(acc, v.y);
+    return pack_step(acc, v.x);
+}
+
+template <int T>
+__device__ __forceinline__ void job_tile(const PlaneArgs& A, uint32_t job, int sub, int& r, int& tx, int& ty) {
+    // colour-C tiles enumerated row by row: q -> ty = q / (B/2), tx = 2*(q % (B/2)) + ((ty + C) & 1)
+    const uint32_t per_rep = (uint32_t)A.B * (uint32_t)A.B / 2u;
+    const uint32_t q = job * PG<T>::TPW + (uint32_t)sub;
+    r = (int)(q / per_rep);
+    const uint32_t qq = q - (uint32_t)r * per_rep;
+    const uint32_t hb = (uint32_t)A.B >> 1;
+    ty = (int)(qq / hb);
+    tx = (int)(2u * (qq - (uint32_t)ty * hb)) + ((ty + A.C) & 1);
+}
+
+// Everything a lane keeps of its job between load and store.
+template <int T>
+struct TileRegs {
+    uint32_t S[2][PG<T>::NW];     // S[cc][gx]: the lane's block row, colour cc
+    uint32_t up[2][PG<T>::NW];    // lane Y = 0: block row above (high half = halo row -1), by colour
+    uint32_t dn[2][PG<T>::NW];    // lane Y = LPT-1: block row below (low half = halo row T)
+    uint32_t hL0, hL1, hR0, hR1;  // halo column bits: x = -1 / x = T of rows 2Y (0) and 2Y+1 (1)
+};
+
+template <int T, bool BITS>
+__device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int ty, int Y, int lane_base, TileRegs<T>& t) {
+    using G = PG<T>;
+    constexpr int REC = BITS ? G::REC_BITS : G::REC_I8;
+    const int B = A.B;
+    const size_t rep = (size_t)r * B * B;
+    const uint8_t* rec = A.tiles + (rep + (size_t)ty * B + tx) * REC;
+    const uint8_t* recU = A.tiles + (rep + (size_t)(ty == 0 ? B - 1 : ty - 1) * B + tx) * REC;
+    const uint8_t* recD = A.tiles + (rep + (size_t)(ty == B - 1 ? 0 : ty + 1) * B + tx) * REC;
+    const uint8_t* recL = A.tiles + (rep + (size_t)ty * B + (tx == 0 ? B - 1 : tx - 1)) * REC;
+    const uint8_t* recR = A.tiles + (rep + (size_t)ty * B + (tx == B - 1 ? 0 : tx + 1)) * REC;
+    // halo rows: lane Y = idx < 4*NW fetches item idx = (which, cc, gx); which 0 = top, 1 = bottom
+    uint32_t item = 0;
+    {
+        const int which = Y / (2 * G::NW), rem = Y % (2 * G::NW), cc = rem / G::NW, gx = rem % G::NW;
+        if (Y < 4 * G::NW) {
+            if (BITS) {
+                const uint8_t* src = which == 0 ? recU + ((cc * G::NW + gx) * G::LPT + (G::LPT - 1)) * 4
+                                                : recD + ((cc * G::NW + gx) * G::LPT) * 4;
+                item = __ldg(reinterpret_cast<const uint32_t*>(src));
+            } else {
+                const int piece = ((which == 0 ? 2 : 0) + cc) * G::NW + gx;      // rp = 1 for the row above, 0 below
+                const uint8_t* src = (which == 0 ? recU + (piece * G::LPT + (G::LPT - 1)) * 16
+                                                 : recD + (piece * G::LPT) * 16);
+                const uint32_t b = pack16(0u, __ldg(reinterpret_cast<const uint4*>(src)));
+                item = which == 0 ? (b << 16) : b;
+            }
+        }
+    }
+    if (BITS) {
+#pragma unroll
+        for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+            for (int gx = 0; gx < G::NW; ++gx)
+                t.S[cc][gx] = ldg32(rec + ((cc * G::NW + gx) * G::LPT + Y) * 4);
+        const uint32_t l1 = __ldg(reinterpret_cast<const uint32_t*>(recL + ((1 * G::NW + G::NW - 1) * G::LPT + Y) * 4));
+        const uint32_t l0 = __ldg(reinterpret_cast<const uint32_t*>(recL + ((0 * G::NW + G::NW - 1) * G::LPT + Y) * 4));
+        const uint32_t r0 = __ldg(reinterpret_cast<const uint32_t*>(recR + ((0 * G::NW + 0) * G::LPT + Y) * 4));
+        const uint32_t r1 = __ldg(reinterpret_cast<const uint32_t*>(recR + ((1 * G::NW + 0) * G::LPT + Y) * 4));
+        t.hL0 = (l1 >> 15) & 1u;   // (x = T-1, even row) is colour 1, pair 15 of the last block
+        t.hL1 = l0 >> 31;          // (x = T-1, odd row) is colour 0
+        t.hR0 = r0 & 1u;           // (x = 0, even row) is colour 0
+        t.hR1 = (r1 >> 16) & 1u;   // (x = 0, odd row) is colour 1
+    } else {
+        uint4 v[G::NCH];
+#pragma unroll
+        for (int ch = 0; ch < G::NCH; ++ch) v[ch] = ldg128(rec + (ch * G::LPT + Y) * 16);
+        const uint32_t eL = __ldg(reinterpret_cast<const uint16_t*>(recL + G::BODY + T + 2 * Y));
+        const uint32_t eR = __ldg(reinterpret_cast<const uint16_t*>(recR + G::BODY + 2 * Y));
+#pragma unroll
+        for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+            for (int gx = 0; gx < G::NW; ++gx)
+                t.S[cc][gx] = pack16(pack16(0u, v[(2 + cc) * G::NW + gx]), v[cc * G::NW + gx]);
+        t.hL0 = eL & 1u; t.hL1 = (eL >> 8) & 1u;
+        t.hR0 = eR & 1u; t.hR1 = (eR >> 8) & 1u;
+    }
+#pragma unroll
+    for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+        for (int gx = 0; gx < G::NW; ++gx) {
+            t.up[cc][gx] = __shfl_sync(0xffffffffu, item, lane_base + cc * G::NW + gx);
+            t.dn[cc][gx] = __shfl_sync(0xffffffffu, item, lane_base + 2 * G::NW + cc * G::NW + gx);
+        }
+}
+
+// a7: write the lane's block row back (and, int8, the two edge-column bytes of its two rows).
+template <int T, bool BITS>
+__device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, int ty, int Y, const TileRegs<T>& t,
+                                           const uint2* lut) {
+    using G = PG<T>;
+    constexpr int REC = BITS ? G::REC_BITS : G::REC_I8;
+    uint8_t* rec = A.tiles + (((size_t)r * A.B + ty) * A.B + tx) * REC;
+    if (BITS) {
+#pragma unroll
+        for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+            for (int gx = 0; gx < G::NW; ++gx)
+                *reinterpret_cast<uint32_t*>(rec + ((cc * G::NW + gx) * G::LPT + Y) * 4) = t.S[cc][gx];
+    } else {
+#pragma unroll
+        for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+            for (int gx = 0; gx < G::NW; ++gx) {
+                const uint32_t w = t.S[cc][gx];
+#pragma unroll
+                for (int rp = 0; rp < 2; ++rp) {
+                    const uint2 a = lut[(w >> (16 * rp)) & 0xffu];          // bits 0..7  -> bytes 0..7
+                    const uint2 b = lut[(w >> (16 * rp + 8)) & 0xffu];      // bits 8..15 -> bytes 8..15
+                    stg128(rec + ((((rp * 2 + cc) * G::NW + gx) * G::LPT) + Y) * 16, make_uint4(a.x, a.y, b.x, b.y));
+                }
+            }
+        // x = 0: colour 0 on even rows (bit 0), colour 1 on odd rows (bit 16); x = T-1: colour 1 / colour 0, last pair
+        const uint32_t eL = (t.S[0][0] & 1u) | (((t.S[1][0] >> 16) & 1u) << 8);
+        const uint32_t eR = ((t.S[1][G::NW - 1] >> 15) & 1u) | ((t.S[0][G::NW - 1] >> 31) << 8);
+        *reinterpret_cast<uint16_t*>(rec + G::BODY + 2 * Y) = (uint16_t)eL;
+        *reinterpret_cast<uint16_t*>(rec + G::BODY + T + 2 * Y) = (uint16_t)eR;
+    }
+}
+
+// R_m = [r < thr[m]] for the 32 sites of block g in half-sweep H: head planes + borrow chains.
+// eq_m = sites whose 12 head bits equal the head of thr[m] (their tail decides).
+__device__ __forceinline__ void head_masks(const PlaneArgs& A, uint32_t g, uint32_t Hlo, uint32_t Hhi, uint32_t k0,
+                                           uint32_t k1, uint32_t& R1, uint32_t& R2, uint32_t& eq1, uint32_t& eq2) {
+    uint32_t bw1 = 0, bw2 = 0, ne1 = 0, ne2 = 0;
+#pragma unroll
+    for (int n = kHeadBits / 4 - 1; n >= 0; --n) {                  // least significant planes first
+        const u32x4 o = philox4x32_10(g, kTagPlanes + 256u * n, Hlo, Hhi, k0, k1);
+        const uint32_t p[4] = {o.x, o.y, o.z, o.w};
+#pragma unroll
+        for (int w = 3; w >= 0; --w) {
+            const int q = 4 * n + w;
+            bw1 = lop3<kLutChain>(p[w], bw1, A.u1[q]);
+            bw2 = lop3<kLutChain>(p[w], bw2, A.u2[q]);
+            ne1 = lop3<kLutNe>(ne1, p[w], A.u1[q]);
+            ne2 = lop3<kLutNe>(ne2, p[w], A.u2[q]);
+        }
+    }
+    R1 = bw1 | A.force1; R2 = bw2 | A.force2; eq1 = ~ne1; eq2 = ~ne2;
+}
+
+// a4-a5 for one block: S' = S ^ flip, neighbours V1, V2 (vertical), H1, H2 (horizontal) of the other colour.
+// und selects the (rare) sites whose tail must be drawn; p_base = pair index i>>1 of bit 0, row stride L/2.
+__device__ __forceinline__ uint32_t update_block(const PlaneArgs& A, uint32_t S, uint32_t V1, uint32_t V2, uint32_t H1,
+                                                 uint32_t H2, uint32_t g, uint32_t p_base, uint32_t Hlo, uint32_t Hhi,
+                                                 uint32_t k0, uint32_t k1) {
+    uint32_t R1, R2, eq1, eq2;
+    head_masks(A, g, Hlo, Hhi, k0, k1, R1, R2, eq1, eq2);
+    const uint32_t a = S ^ V1, b = S ^ V2, c = S ^ H1, d = S ^ H2;     // disagreeing neighbours
+    const uint32_t p1 = a | b, q1 = a & b, p2 = c | d, q2 = c & d;
+    const uint32_t ge1 = p1 | p2;                                     // n_dis >= 1
+    const uint32_t ge2 = (p1 & p2) | q1 | q2;                         // n_dis >= 2  <=>  dE <= 0: always flip (eq. (2))
+    uint32_t und = (eq1 & ge1 & ~ge2) | (eq2 & ~ge1);                 // n_dis == 1 needs thr[1], n_dis == 0 needs thr[2]
+    while (und) {                                                     // probability 2^-12 per site
+        const int j = __ffs(und) - 1;
+        und &= und - 1;
+        const uint32_t p = p_base + (uint32_t)(j >> 4) * (uint32_t)(A.L >> 1) + (uint32_t)(j & 15);
+        const u32x4 o = philox4x32_10(p, kTagTail, Hlo, Hhi, k0, k1);
+        const uint32_t tail = o.x >> kHeadBits;
+        if ((eq1 >> j) & 1u) R1 |= (uint32_t)(tail < A.t1_tail) << j;
+        if ((eq2 >> j) & 1u) R2 |= (uint32_t)(tail < A.t2_tail) << j;
+    }
+    const uint32_t flip = ge2 | (ge1 & R1) | R2;                      // thr[2] <= thr[1], so R2 is inside R1
+    return S ^ flip;
+}
+
+// a5-a6: one half-sweep of colour c on the lane's block row; o = 1 - c is read, c is written.
+template <int T>
+__device__ __forceinline__ void half_sweep(const PlaneArgs& A, TileRegs<T>& t, int c, int Y, uint32_t g0, uint32_t p0,
+                                           uint64_t H, uint32_t k0, uint32_t k1) {
+    using G = PG<T>;
+    const int o = 1 - c;
+    const uint32_t Hlo = (uint32_t)H, Hhi = (uint32_t)(H >> 32);
+    uint32_t O[G::NW], Snew[G::NW];
+#pragma unroll
+    for (int gx = 0; gx < G::NW; ++gx) O[gx] = t.S[o][gx];
+#pragma unroll
+    for (int gx = 0; gx < G::NW; ++gx) {
+        uint32_t Oup = __shfl_up_sync(0xffffffffu, O[gx], 1);
+        uint32_t Odn = __shfl_down_sync(0xffffffffu, O[gx], 1);
+        if (Y == 0) Oup = t.up[o][gx];
+        if (Y == G::LPT - 1) Odn = t.dn[o][gx];
+        const uint32_t V1 = __byte_perm(O[gx], O[gx], 0x1032);        // the other row of the same block
+        const uint32_t V2 = __byte_perm(Oup, Odn, 0x5432);            // row above the block | row below the block
+        // pair-shifted word: colour 0: even rows look at pair j-1 (carry from the left), odd rows at j+1;
+        // colour 1: even rows j+1, odd rows j-1.
+        uint32_t H2;
+        if (c == 0) {
+            const uint32_t cl = gx == 0 ? t.hL0 : ((O[gx > 0 ? gx - 1 : 0] >> 15) & 1u);
+            const uint32_t cr = gx == G::NW - 1 ? t.hR1 : ((O[gx < G::NW - 1 ? gx + 1 : gx] >> 16) & 1u);
+            H2 = ((O[gx] << 1) & 0x0000fffeu) | cl | ((O[gx] >> 1) & 0x7fff0000u) | (cr << 31);
+        } else {
+            const uint32_t cr = gx == G::NW - 1 ? t.hR0 : (O[gx < G::NW - 1 ? gx + 1 : gx] & 1u);
+            const uint32_t cl = gx == 0 ? t.hL1 : (O[gx > 0 ? gx - 1 : 0] >> 31);
+            H2 = ((O[gx] >> 1) & 0x00007fffu) | (cr << 15) | ((O[gx] << 1) & 0xfffe0000u) | (cl << 16);
+        }
+        Snew[gx] = update_block(A, t.S[c][gx], V1, V2, O[gx], H2, g0 + (uint32_t)gx, p0 + 16u * (uint32_t)gx, Hlo, Hhi, k0, k1);
+    }
+#pragma unroll
+    for (int gx = 0; gx < G::NW; ++gx) t.S[c][gx] = Snew[gx];
+}
+
+template <int T, bool BITS>
+__global__ void __launch_bounds__(128) k_tile_planes(PlaneArgs A) {
+    using G = PG<T>;
+    __shared__ uint2 lut[256];                  // int8 write-back: 8 bits -> 8 bytes of 0/1
+    if (!BITS) {
+        for (int i = threadIdx.x; i < 256; i += blockDim.x) {
+            uint32_t lo = 0, hi = 0;
+#pragma unroll
+            for (int b = 0; b < 4; ++b) {
+                lo |= ((i >> b) & 1u) << (8 * b);
+                hi |= ((i >> (4 + b)) & 1u) << (8 * b);
+            }
+            lut[i] = make_uint2(lo, hi);
+        }
+        __syncthreads();
+    }
+    const int lane = threadIdx.x & 31;
+    const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (job >= A.njobs) return;
+    const int sub = lane / G::LPT, Y = lane % G::LPT;
+    int r, tx, ty;
+    job_tile<T>(A, job, sub, r, tx, ty);
+    TileRegs<T> t;
+    load_tile<T, BITS>(A, r, tx, ty, Y, sub * G::LPT, t);
+    const uint64_t seed = A.seeds[r];
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);                         // global block row
+    const uint32_t g0 = Yg * (uint32_t)(A.L >> 5) + (uint32_t)(tx * G::NW);  // RNG block of gx = 0
+    const uint32_t p0 = 2u * Yg * (uint32_t)(A.L >> 1) + 16u * (uint32_t)(tx * G::NW);   // pair index of its bit 0
+    for (int j = 0; j < A.k; ++j) {
+        const uint64_t tt = A.t_first + (uint64_t)j;
+        half_sweep<T>(A, t, 0, Y, g0, p0, 2 * tt, k0, k1);
+        half_sweep<T>(A, t, 1, Y, g0, p0, 2 * tt + 1, k0, k1);
+    }
+    store_tile<T, BITS>(A, r, tx, ty, Y, t, lut);
+}
+
+// ---- layout converters (a11): canonical int8 +-1 <-> tile records; not on the timed path ----
+// One thread per site; MODE 0: canonical -> int8 records, 1: int8 records -> canonical,
+// 2: canonical -> bit records (atomicOr into zeroed storage), 3: bit records -> canonical.
+template <int MODE>
+__global__ void k_convert_planes(int8_t* __restrict__ canon, uint8_t* __restrict__ tiles, int L, int T, int R) {
+    const uint64_t N = (uint64_t)L * L;
+    const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (gid >= N * (uint64_t)R) return;
+    const int r = (int)(gid / N);
+    const uint64_t i = gid - (uint64_t)r * N;
+    const int x = (int)(i % L), y = (int)(i / L);
+    const int B = L / T, NW = T / 32, LPT = T / 2;
+    const int tx = x / T, ty = y / T, lx = x - tx * T, ly = y - ty * T;
+    const int cc = (lx + ly) & 1, px = lx >> 1, gx = px >> 4, kk = px & 15, rp = ly & 1, Y = ly >> 1;
+    const size_t tile = ((size_t)r * B + ty) * B + tx;
+    if (MODE < 2) {
+        uint8_t* rec = tiles + tile * (size_t)(T * T + 2 * T);
+        uint8_t* body = rec + ((((rp * 2 + cc) * NW + gx) * LPT) + Y) * 16 + kk;
+        if (MODE == 0) {
+            const uint8_t v = canon[gid] > 0 ? 1 : 0;
+            *body = v;
+            if (lx == 0) rec[T * T + ly] = v;
+            if (lx == T - 1) rec[T * T + T + ly] = v;
+        } else {
+            canon[gid] = *body ? 1 : -1;
+        }
+    } else {
+        uint32_t* w = reinterpret_cast<uint32_t*>(tiles + tile * (size_t)(T * T / 8)) + ((cc * NW + gx) * LPT + Y);
+        const int j = rp * 16 + kk;
+        if (MODE == 2) {
+            if (canon[gid] > 0) atomicOr(w, 1u << j);
+        } else {
+            canon[gid] = ((*w >> j) & 1u) ? 1 : -1;
+        }
+    }
+}
+
+template <int T, bool BITS>
+int launch_colour_planes(const PlaneArgs& A) {
+    const int warps = 4;
+    const uint32_t grid = (A.njobs + warps - 1) / warps;
+    k_tile_planes<T, BITS><<<grid, warps * 32, 0, hooks().stream>>>(A);
+    count_launch();
+    return 0;
+}
+
+}  // namespace
+
+bool tile_planes_supported(const ising_ctx* h, int T) {
+    if (h->dim != 2 || h->has_J) return false;
+    if (T != 32 && T != 64) return false;
+    if (h->L % T) return false;
+    const int B = h->L / T;
+    return B >= 2 && (B % 2 == 0);
+}
+
+size_t tile_planes_bytes(const ising_ctx* h, int T, bool bits) {
+    const size_t B = (size_t)(h->L / T);
+    return (size_t)h->R * B * B * (size_t)(bits ? T * T / 8 : T * T + 2 * T);
+}
+
+int launch_canon_to_planes(ising_ctx* h, int T, bool bits, const int8_t* d_canon, void* d_tiles) {
+    const uint64_t total = h->N * (uint64_t)h->R;
+    const unsigned blocks = (unsigned)((total + 255) / 256);
+    cudaStream_t st = hooks().stream;
+    if (bits) {
+        ISING_CUDA_OK(cudaMemsetAsync(d_tiles, 0, tile_planes_bytes(h, T, true), st));
+        k_convert_planes<2><<<blocks, 256, 0, st>>>(const_cast<int8_t*>(d_canon), (uint8_t*)d_tiles, h->L, T, h->R);
+    } else {
+        k_convert_planes<0><<<blocks, 256, 0, st>>>(const_cast<int8_t*>(d_canon), (uint8_t*)d_tiles, h->L, T, h->R);
+    }
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+int launch_planes_to_canon(ising_ctx* h, int T, bool bits, const void* d_tiles, int8_t* d_canon) {
+    const uint64_t total = h->N * (uint64_t)h->R;
+    const unsigned blocks = (unsigned)((total + 255) / 256);
+    cudaStream_t st = hooks().stream;
+    if (bits) k_convert_planes<3><<<blocks, 256, 0, st>>>(d_canon, (uint8_t*)const_cast<void*>(d_tiles), h->L, T, h->R);
+    else k_convert_planes<1><<<blocks, 256, 0, st>>>(d_canon, (uint8_t*)const_cast<void*>(d_tiles), h->L, T, h->R);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+// a1: one outer pass = colour-0 launch, colour-1 launch, k inner sweeps each.
+int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, int k, uint64_t t_first) {
+    PlaneArgs A;
+    A.tiles = (uint8_t*)h->d_tiles;
+    A.seeds = h->d_seeds;
+    A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first;
+    const uint32_t tiles_per_colour = (uint32_t)((size_t)h->R * A.B * A.B / 2);
+    A.njobs = tiles_per_colour / (uint32_t)(64 / T);
+    for (int q = 0; q < kHeadBits; ++q) {
+        A.u1[q] = ((acc.thr[0] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
+        A.u2[q] = ((acc.thr[1] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
+    }
+    A.force1 = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
+    A.force2 = acc.thr_is_2p32[1] ? 0xffffffffu : 0u;
+    A.t1_tail = acc.thr[0] & ((1u << kTailBits) - 1u);
+    A.t2_tail = acc.thr[1] & ((1u << kTailBits) - 1u);
+    for (int C = 0; C < 2; ++C) {
+        A.C = C;
+        if (T == 64) bits ? launch_colour_planes<64, true>(A) : launch_colour_planes<64, false>(A);
+        else bits ? launch_colour_planes<32, true>(A) : launch_colour_planes<32, false>(A);
+    }
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+}  // namespace ising

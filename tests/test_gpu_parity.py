@@ -19,9 +19,12 @@ def P():
     return pkg
 
 
-def _both(P, orc, dim, L, seeds, J=None):
-    g = P.Ising(dim, L, coupling=J, seeds=seeds)
-    o = orc.Oracle(dim, L, seeds=seeds, J=J)
+RNGS = ["planes", "words"]
+
+
+def _both(P, orc, dim, L, seeds, J=None, rng="planes"):
+    g = P.Ising(dim, L, coupling=J, seeds=seeds, rng=rng)
+    o = orc.Oracle(dim, L, seeds=seeds, J=J, rng=rng)
     return g, o
 
 
@@ -62,10 +65,11 @@ GENERIC = [
 ]
 
 
+@pytest.mark.parametrize("rng", RNGS)
 @pytest.mark.parametrize("dim,L,tile,k,n,beta,seeds,jseed", GENERIC)
-def test_generic_path_matches_oracle(P, orc, dim, L, tile, k, n, beta, seeds, jseed):
+def test_generic_path_matches_oracle(P, orc, dim, L, tile, k, n, beta, seeds, jseed, rng):
     J = W.couplings(dim, L, jseed) if jseed is not None else None
-    g, o = _both(P, orc, dim, L, seeds, J)
+    g, o = _both(P, orc, dim, L, seeds, J, rng)
     g.force_path(True)
     Eg, Mg = g.sweep_series(beta, n, tile, k)
     Eo, Mo = o.sweep_series(beta, n, tile, k)
@@ -92,9 +96,24 @@ TILED = [
 ]
 
 
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,tile,k,n,beta,seeds", TILED + [(512, 64, 3, 4, 1.0, [31]), (512, 32, 1, 6, 0.2, [32])])
+def test_tile_planes_path_matches_oracle(P, orc, L, tile, k, n, beta, seeds, layout):
+    """Multi-spin tile kernel (RNG mapping planes), both HBM layouts.  L >= 256 at beta_c draws
+    the per-site tail (head == threshold head, probability 2^-12 per site) several times."""
+    g, o = _both(P, orc, 2, L, seeds, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    Eg, Mg = g.sweep_series(beta, n, tile, k)
+    assert g.sweep_path() == f"tile_planes_{'i8' if layout == 'int8' else 'bits'}"
+    Eo, Mo = o.sweep_series(beta, n, tile, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+
+
 @pytest.mark.parametrize("L,tile,k,n,beta,seeds", TILED)
 def test_tile_i8_path_matches_oracle(P, orc, L, tile, k, n, beta, seeds):
-    g, o = _both(P, orc, 2, L, seeds)
+    g, o = _both(P, orc, 2, L, seeds, rng="words")
     Eg, Mg = g.sweep_series(beta, n, tile, k)
     assert g.sweep_path() == ("tile_i8" if beta > 0 else "generic")   # beta = 0: thr = 2^32, generic kernels
     Eo, Mo = o.sweep_series(beta, n, tile, k)
