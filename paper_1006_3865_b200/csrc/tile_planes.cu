@@ -46,6 +46,7 @@ struct PlaneArgs {
     int k;
     uint64_t t_first;            // inner-sweep index of the first of the k sweeps
     uint32_t njobs;
+    uint32_t magic_rep, magic_hb; // ceil(2^32 / d) for d = tiles per colour per replica, B/2 (0xffffffff for d = 1)
     uint32_t u1[kHeadBits];      // plane q: all-ones if bit (31-q) of thr[1] is set, else 0
     uint32_t u2[kHeadBits];      // same for thr[2]
     uint32_t t1_tail, t2_tail;   // thr[m] & (2^20 - 1)
@@ -97,10 +98,17 @@ __device__ __forceinline__ void job_tile(const PlaneArgs& A, uint32_t job, int s
     // colour-C tiles enumerated row by row: q -> ty = q / (B/2), tx = 2*(q % (B/2)) + ((ty + C) & 1)
     const uint32_t per_rep = (uint32_t)A.B * (uint32_t)A.B / 2u;
     const uint32_t q = job * PG<T>::TPW + (uint32_t)sub;
-    r = (int)(q / per_rep);
-    const uint32_t qq = q - (uint32_t)r * per_rep;
+    // q / per_rep and qq / hb by host-computed reciprocals ~2^32 / d, corrected by at most one either way
+    uint32_t rr = __umulhi(q, A.magic_rep);
+    if (rr * per_rep > q) --rr;
+    if ((rr + 1) * per_rep <= q) ++rr;
+    r = (int)rr;
+    const uint32_t qq = q - rr * per_rep;
     const uint32_t hb = (uint32_t)A.B >> 1;
-    ty = (int)(qq / hb);
+    uint32_t yy = __umulhi(qq, A.magic_hb);
+    if (yy * hb > qq) --yy;
+    if ((yy + 1) * hb <= qq) ++yy;
+    ty = (int)yy;
     tx = (int)(2u * (qq - (uint32_t)ty * hb)) + ((ty + A.C) & 1);
 }
 
@@ -301,13 +309,9 @@ __global__ void __launch_bounds__(128) k_tile_planes(PlaneArgs A) {
     __shared__ uint2 lut[256];                  // int8 write-back: 8 bits -> 8 bytes of 0/1
     if (!BITS) {
         for (int i = threadIdx.x; i < 256; i += blockDim.x) {
-            uint32_t lo = 0, hi = 0;
-#pragma unroll
-            for (int b = 0; b < 4; ++b) {
-                lo |= ((i >> b) & 1u) << (8 * b);
-                hi |= ((i >> (4 + b)) & 1u) << (8 * b);
-            }
-            lut[i] = make_uint2(lo, hi);
+            // 4 bits -> 4 bytes: n * 0x00204081 puts bit b at 8b (+ garbage elsewhere), no carries for n < 16
+            lut[i] = make_uint2(((uint32_t)(i & 15) * 0x00204081u) & 0x01010101u,
+                                ((uint32_t)(i >> 4) * 0x00204081u) & 0x01010101u);
         }
         __syncthreads();
     }
@@ -427,6 +431,9 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first;
     const uint32_t tiles_per_colour = (uint32_t)((size_t)h->R * A.B * A.B / 2);
     A.njobs = tiles_per_colour / (uint32_t)(64 / T);
+    auto magic = [](uint32_t d) { return d <= 1 ? 0xffffffffu : (uint32_t)((0x100000000ull + d - 1) / d); };
+    A.magic_rep = magic((uint32_t)A.B * (uint32_t)A.B / 2u);
+    A.magic_hb = magic((uint32_t)A.B / 2u);
     for (int q = 0; q < kHeadBits; ++q) {
         A.u1[q] = ((acc.thr[0] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
         A.u2[q] = ((acc.thr[1] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;

@@ -4,7 +4,8 @@ Expected values for the full-size parity tests of BASELINE.json configs 2-5, whe
 oracle inside the test would take too long.  Nothing here touches the CUDA path.  Each job is
 one oracle trajectory; checkpoints are [pass, E, M, FNV-1a-64 of the canonical spins]; for jobs
 with `series` the FNV-1a-64 of the little-endian int64 E series and M series (one value per
-outer pass) up to each checkpoint is stored too.
+outer pass) up to each checkpoint is stored too.  All jobs use the default RNG mapping "planes"
+(DESIGN.md §3.4); the words mapping is pinned by survey_appendix_a.json on the same configs.
 
     python tests/golden/make_goldens.py [--only SUBSTR] [--procs 8]
 
@@ -60,9 +61,10 @@ def run(job):
     import ising_workloads as W
     t0 = time.time()
     Jarr = W.couplings(job["dim"], job["L"], job["jseed"]) if "jseed" in job else None
-    o = O.Oracle(job["dim"], job["L"], seeds=job["seeds"], J=Jarr)
+    o = O.Oracle(job["dim"], job["L"], seeds=job["seeds"], J=Jarr, rng=job.get("rng", "planes"))
     R = len(job["seeds"])
     res = dict(job)
+    res["rng"] = job.get("rng", "planes")
     cps = []
     E0, M0 = o.observables()
     cps.append([0, [int(v) for v in E0], [int(v) for v in M0], ["%016x" % o.hash(r) for r in range(R)]])
