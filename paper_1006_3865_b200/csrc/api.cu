@@ -292,6 +292,14 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         const bool bits = h->layout == ISING_LAYOUT_BITS;
         h->last_path = use_tile_i8 ? "tile_i8" : (bits ? "tile_planes_bits" : "tile_planes_i8");
         rc = ensure_store(h, use_tile_i8 ? Store::TileI8 : (bits ? Store::PlaneBits : Store::PlaneI8), T);
+        if (!rc && use_planes && h->has_J && h->Jtiles_tile != T) {      // coupling records for this tile edge
+            if (!h->d_Jtiles) {
+                h->d_Jtiles = dev_alloc(coupling_record_bytes(h));
+                if (!h->d_Jtiles) rc = ISING_ENOMEM;
+            }
+            if (!rc) rc = launch_convert_couplings(h, T, h->d_Jtiles);
+            if (!rc) h->Jtiles_tile = T;
+        }
         for (int pass = 0; pass < n && !rc; ++pass) {
             const uint64_t t0 = h->t + (uint64_t)pass * (uint64_t)k;
             rc = use_tile_i8 ? launch_tile_i8_pass(h, acc, T, k, t0) : launch_tile_planes_pass(h, acc, T, bits, k, t0);

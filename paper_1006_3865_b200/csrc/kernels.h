@@ -25,6 +25,8 @@ bool tile_planes_supported(const ising_ctx* h, int T);
 size_t tile_planes_bytes(const ising_ctx* h, int T, bool bits);
 int launch_canon_to_planes(ising_ctx* h, int T, bool bits, const int8_t* d_canon, void* d_tiles);
 int launch_planes_to_canon(ising_ctx* h, int T, bool bits, const void* d_tiles, int8_t* d_canon);
+size_t coupling_record_bytes(const ising_ctx* h);
+int launch_convert_couplings(ising_ctx* h, int T, void* d_jrec);
 int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, int k, uint64_t t_first);
 
 }  // namespace ising

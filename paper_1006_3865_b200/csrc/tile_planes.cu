@@ -51,6 +51,9 @@ struct PlaneArgs {
     uint32_t u2[kHeadBits];      // same for thr[2]
     uint32_t t1_tail, t2_tail;   // thr[m] & (2^20 - 1)
     uint32_t force1, force2;     // all-ones if thr[m] = 2^32 (beta = 0: every r is below it), else 0
+    const uint4* jrec;           // coupling records (a9) or nullptr: per tile, uint4 (cc, gx, Y) =
+                                 // {V1, V2, H1, H2}: bit j set <=> the bond from site j of that block to its
+                                 // neighbour in the V1 / V2 / H1 / H2 word is J = -1.  Shared by all replicas.
 };
 
 template <int LUT>
@@ -244,12 +247,15 @@ __device__ __forceinline__ void head_masks(const PlaneArgs& A, uint32_t g, uint3
 
 // a4-a5 for one block: S' = S ^ flip, neighbours V1, V2 (vertical), H1, H2 (horizontal) of the other colour.
 // und selects the (rare) sites whose tail must be drawn; p_base = pair index i>>1 of bit 0, row stride L/2.
+template <bool HASJ>
 __device__ __forceinline__ uint32_t update_block(const PlaneArgs& A, uint32_t S, uint32_t V1, uint32_t V2, uint32_t H1,
-                                                 uint32_t H2, uint32_t g, uint32_t p_base, uint32_t Hlo, uint32_t Hhi,
-                                                 uint32_t k0, uint32_t k1) {
+                                                 uint32_t H2, const uint4& Jw, uint32_t g, uint32_t p_base, uint32_t Hlo,
+                                                 uint32_t Hhi, uint32_t k0, uint32_t k1) {
     uint32_t R1, R2, eq1, eq2;
     head_masks(A, g, Hlo, Hhi, k0, k1, R1, R2, eq1, eq2);
-    const uint32_t a = S ^ V1, b = S ^ V2, c = S ^ H1, d = S ^ H2;     // disagreeing neighbours
+    // unsatisfied bonds: J s_i s_j = -1  <=>  s_i != s_j for J = +1, s_i == s_j for J = -1 (eq. (1))
+    const uint32_t a = S ^ V1 ^ (HASJ ? Jw.x : 0u), b = S ^ V2 ^ (HASJ ? Jw.y : 0u);
+    const uint32_t c = S ^ H1 ^ (HASJ ? Jw.z : 0u), d = S ^ H2 ^ (HASJ ? Jw.w : 0u);
     const uint32_t p1 = a | b, q1 = a & b, p2 = c | d, q2 = c & d;
     const uint32_t ge1 = p1 | p2;                                     // n_dis >= 1
     const uint32_t ge2 = (p1 & p2) | q1 | q2;                         // n_dis >= 2  <=>  dE <= 0: always flip (eq. (2))
@@ -268,9 +274,9 @@ __device__ __forceinline__ uint32_t update_block(const PlaneArgs& A, uint32_t S,
 }
 
 // a5-a6: one half-sweep of colour c on the lane's block row; o = 1 - c is read, c is written.
-template <int T>
-__device__ __forceinline__ void half_sweep(const PlaneArgs& A, TileRegs<T>& t, int c, int Y, uint32_t g0, uint32_t p0,
-                                           uint64_t H, uint32_t k0, uint32_t k1) {
+template <int T, bool HASJ>
+__device__ __forceinline__ void half_sweep(const PlaneArgs& A, TileRegs<T>& t, const uint4 (&Jw)[2][PG<T>::NW], int c, int Y,
+                                           uint32_t g0, uint32_t p0, uint64_t H, uint32_t k0, uint32_t k1) {
     using G = PG<T>;
     const int o = 1 - c;
     const uint32_t Hlo = (uint32_t)H, Hhi = (uint32_t)(H >> 32);
@@ -297,13 +303,14 @@ __device__ __forceinline__ void half_sweep(const PlaneArgs& A, TileRegs<T>& t, i
             const uint32_t cl = gx == 0 ? t.hL1 : (O[gx > 0 ? gx - 1 : 0] >> 31);
             H2 = ((O[gx] >> 1) & 0x00007fffu) | (cr << 15) | ((O[gx] << 1) & 0xfffe0000u) | (cl << 16);
         }
-        Snew[gx] = update_block(A, t.S[c][gx], V1, V2, O[gx], H2, g0 + (uint32_t)gx, p0 + 16u * (uint32_t)gx, Hlo, Hhi, k0, k1);
+        Snew[gx] = update_block<HASJ>(A, t.S[c][gx], V1, V2, O[gx], H2, Jw[c][gx], g0 + (uint32_t)gx,
+                                      p0 + 16u * (uint32_t)gx, Hlo, Hhi, k0, k1);
     }
 #pragma unroll
     for (int gx = 0; gx < G::NW; ++gx) t.S[c][gx] = Snew[gx];
 }
 
-template <int T, bool BITS>
+template <int T, bool BITS, bool HASJ>
 __global__ void __launch_bounds__(128) k_tile_planes(PlaneArgs A) {
     using G = PG<T>;
     __shared__ uint2 lut[256];                  // int8 write-back: 8 bits -> 8 bytes of 0/1
@@ -323,6 +330,13 @@ __global__ void __launch_bounds__(128) k_tile_planes(PlaneArgs A) {
     job_tile<T>(A, job, sub, r, tx, ty);
     TileRegs<T> t;
     load_tile<T, BITS>(A, r, tx, ty, Y, sub * G::LPT, t);
+    uint4 Jw[2][G::NW];
+#pragma unroll
+    for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+        for (int gx = 0; gx < G::NW; ++gx)
+            Jw[cc][gx] = HASJ ? __ldg(A.jrec + ((size_t)ty * A.B + tx) * (2 * G::NW * G::LPT) + (cc * G::NW + gx) * G::LPT + Y)
+                              : make_uint4(0u, 0u, 0u, 0u);
     const uint64_t seed = A.seeds[r];
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);                         // global block row
@@ -330,8 +344,8 @@ __global__ void __launch_bounds__(128) k_tile_planes(PlaneArgs A) {
     const uint32_t p0 = 2u * Yg * (uint32_t)(A.L >> 1) + 16u * (uint32_t)(tx * G::NW);   // pair index of its bit 0
     for (int j = 0; j < A.k; ++j) {
         const uint64_t tt = A.t_first + (uint64_t)j;
-        half_sweep<T>(A, t, 0, Y, g0, p0, 2 * tt, k0, k1);
-        half_sweep<T>(A, t, 1, Y, g0, p0, 2 * tt + 1, k0, k1);
+        half_sweep<T, HASJ>(A, t, Jw, 0, Y, g0, p0, 2 * tt, k0, k1);
+        half_sweep<T, HASJ>(A, t, Jw, 1, Y, g0, p0, 2 * tt + 1, k0, k1);
     }
     store_tile<T, BITS>(A, r, tx, ty, Y, t, lut);
 }
@@ -373,11 +387,37 @@ __global__ void k_convert_planes(int8_t* __restrict__ canon, uint8_t* __restrict
     }
 }
 
+// Couplings, canonical J[d][i] (bond i -> i + e_d) -> coupling records (zeroed first).  One thread per site:
+// it owns the four bonds seen from that site, in the order of the neighbour words of update_block.
+__global__ void k_convert_couplings(const int8_t* __restrict__ J, uint32_t* __restrict__ jrec, int L, int T) {
+    const uint64_t N = (uint64_t)L * L;
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int x = (int)(i % L), y = (int)(i / L);
+    const int B = L / T, NW = T / 32, LPT = T / 2;
+    const int tx = x / T, ty = y / T, lx = x - tx * T, ly = y - ty * T;
+    const int cc = (lx + ly) & 1, px = lx >> 1, gx = px >> 4, kk = px & 15, rp = ly & 1, Y = ly >> 1;
+    const uint64_t iL = (uint64_t)(x == 0 ? L - 1 : x - 1) + (uint64_t)L * y;         // site to the left
+    const uint64_t iU = (uint64_t)x + (uint64_t)L * (y == 0 ? L - 1 : y - 1);         // site above (y - 1)
+    const bool right = J[i] < 0, left = J[iL] < 0, down = J[N + i] < 0, up = J[N + iU] < 0;
+    const bool v1 = rp == 0 ? down : up;          // V1 = the other row of the block
+    const bool v2 = rp == 0 ? up : down;          // V2 = the row outside the block
+    const bool h1 = (x & 1) == 0 ? right : left;  // H1 = the other site of the aligned pair (2p_x, 2p_x + 1)
+    const bool h2 = (x & 1) == 0 ? left : right;
+    uint32_t* w = jrec + (((size_t)ty * B + tx) * (2 * NW * LPT) + (cc * NW + gx) * LPT + Y) * 4;
+    const uint32_t bit = 1u << (rp * 16 + kk);
+    if (v1) atomicOr(w + 0, bit);
+    if (v2) atomicOr(w + 1, bit);
+    if (h1) atomicOr(w + 2, bit);
+    if (h2) atomicOr(w + 3, bit);
+}
+
 template <int T, bool BITS>
 int launch_colour_planes(const PlaneArgs& A) {
     const int warps = 4;
     const uint32_t grid = (A.njobs + warps - 1) / warps;
-    k_tile_planes<T, BITS><<<grid, warps * 32, 0, hooks().stream>>>(A);
+    if (A.jrec) k_tile_planes<T, BITS, true><<<grid, warps * 32, 0, hooks().stream>>>(A);
+    else k_tile_planes<T, BITS, false><<<grid, warps * 32, 0, hooks().stream>>>(A);
     count_launch();
     return 0;
 }
@@ -385,11 +425,22 @@ int launch_colour_planes(const PlaneArgs& A) {
 }  // namespace
 
 bool tile_planes_supported(const ising_ctx* h, int T) {
-    if (h->dim != 2 || h->has_J) return false;
+    if (h->dim != 2) return false;
     if (T != 32 && T != 64) return false;
     if (h->L % T) return false;
     const int B = h->L / T;
     return B >= 2 && (B % 2 == 0);
+}
+
+size_t coupling_record_bytes(const ising_ctx* h) { return (size_t)h->N / 2 * 4; }   // 4 bond bits per site
+
+int launch_convert_couplings(ising_ctx* h, int T, void* d_jrec) {
+    cudaStream_t st = hooks().stream;
+    ISING_CUDA_OK(cudaMemsetAsync(d_jrec, 0, coupling_record_bytes(h), st));
+    k_convert_couplings<<<(unsigned)((h->N + 255) / 256), 256, 0, st>>>(h->d_J, (uint32_t*)d_jrec, h->L, T);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
 }
 
 size_t tile_planes_bytes(const ising_ctx* h, int T, bool bits) {
@@ -429,6 +480,7 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_seeds;
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first;
+    A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
     const uint32_t tiles_per_colour = (uint32_t)((size_t)h->R * A.B * A.B / 2);
     A.njobs = tiles_per_colour / (uint32_t)(64 / T);
     auto magic = [](uint32_t d) { return d <= 1 ? 0xffffffffu : (uint32_t)((0x100000000ull + d - 1) / d); };

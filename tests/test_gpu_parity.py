@@ -111,6 +111,37 @@ def test_tile_planes_path_matches_oracle(P, orc, L, tile, k, n, beta, seeds, lay
     _same_state(g, o)
 
 
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,tile,k,n,beta,seeds,jseed", [
+    (128, 32, 4, 3, 1.0, [100, 101, 102], 5),      # config 5 shape: +-J glass, replicas share J
+    (256, 64, 2, 3, 0.8, [7], 11),
+    (192, 32, 1, 4, 0.5, [8, 9], 12),
+    (256, 32, 3, 2, 0.0, [3], 13),
+])
+def test_tile_planes_couplings_match_oracle(P, orc, L, tile, k, n, beta, seeds, jseed, layout):
+    """a9 on the multi-spin tile kernel: quenched +-J bonds as bit records shared by the replicas."""
+    J = W.couplings(2, L, jseed)
+    g, o = _both(P, orc, 2, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    Eg, Mg = g.sweep_series(beta, n, tile, k)
+    assert g.sweep_path() == f"tile_planes_{'i8' if layout == 'int8' else 'bits'}"
+    Eo, Mo = o.sweep_series(beta, n, tile, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    if len(seeds) > 1:
+        assert g.overlap(0, 1) == o.overlap(0, 1)
+    # gauge invariance on the GPU path alone: J' = eps_i eps_j J, s' = eps s gives the same E series
+    rng = np.random.default_rng(jseed)
+    eps = (1 - 2 * rng.integers(0, 2, size=(L, L))).astype(np.int8)
+    Jg = J.reshape(2, L, L) * eps[None] * np.stack([np.roll(eps, -1, 1), np.roll(eps, -1, 0)])
+    a = P.Ising(2, L, coupling=J, seeds=seeds[:1]); b = P.Ising(2, L, coupling=Jg.reshape(-1).astype(np.int8), seeds=seeds[:1])
+    b.set_spins((a.copy_spins().reshape(L, L) * eps).reshape(-1))
+    Ea, _ = a.sweep_series(beta, 2, tile, k); Eb, _ = b.sweep_series(beta, 2, tile, k)
+    assert np.array_equal(Ea, Eb)
+    assert np.array_equal(a.copy_spins().reshape(L, L) * eps, b.copy_spins().reshape(L, L))
+
+
 @pytest.mark.parametrize("L,tile,k,n,beta,seeds", TILED)
 def test_tile_i8_path_matches_oracle(P, orc, L, tile, k, n, beta, seeds):
     g, o = _both(P, orc, 2, L, seeds, rng="words")
