@@ -105,6 +105,8 @@ static int to_canon_scratch(ising_ctx* h) {   // tiles -> d_canon, store state u
         case Store::TileI8: return launch_tile_i8_to_canon(h, h->store_tile, h->d_tiles, h->d_canon);
         case Store::PlaneI8: return launch_planes_to_canon(h, h->store_tile, false, h->d_tiles, h->d_canon);
         case Store::PlaneBits: return launch_planes_to_canon(h, h->store_tile, true, h->d_tiles, h->d_canon);
+        case Store::Plane3I8: return launch_3d_to_canon(h, false, h->d_tiles, h->d_canon);
+        case Store::Plane3Bits: return launch_3d_to_canon(h, true, h->d_tiles, h->d_canon);
         default: return 0;
     }
 }
@@ -123,7 +125,10 @@ static int ensure_store(ising_ctx* h, Store kind, int T) {
     if (h->store == kind && h->store_tile == T) return 0;
     int rc = ensure_canon(h);
     if (rc) return rc;
-    const size_t need = kind == Store::TileI8 ? tile_i8_bytes(h, T) : tile_planes_bytes(h, T, kind == Store::PlaneBits);
+    const bool is3 = kind == Store::Plane3I8 || kind == Store::Plane3Bits;
+    const size_t need = kind == Store::TileI8 ? tile_i8_bytes(h, T)
+                        : is3 ? tile3d_bytes(h, kind == Store::Plane3Bits)
+                              : tile_planes_bytes(h, T, kind == Store::PlaneBits);
     if (need > h->tiles_bytes) {
         ISING_CUDA_OK(cudaStreamSynchronize(hooks().stream));
         dev_free(h->d_tiles);
@@ -133,7 +138,8 @@ static int ensure_store(ising_ctx* h, Store kind, int T) {
         h->tiles_bytes = need;
     }
     rc = kind == Store::TileI8 ? launch_canon_to_tile_i8(h, T, h->d_canon, h->d_tiles)
-                               : launch_canon_to_planes(h, T, kind == Store::PlaneBits, h->d_canon, h->d_tiles);
+         : is3 ? launch_canon_to_3d(h, kind == Store::Plane3Bits, h->d_canon, h->d_tiles)
+               : launch_canon_to_planes(h, T, kind == Store::PlaneBits, h->d_canon, h->d_tiles);
     if (rc) return rc;
     h->store = kind;
     h->store_tile = T;
@@ -288,10 +294,13 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
     const bool use_tile_i8 = !h->force_generic && thr_fits && h->rng == ISING_RNG_WORDS &&
                              h->layout == ISING_LAYOUT_I8 && tile_i8_supported(h, T);
     const bool use_planes = !h->force_generic && h->rng == ISING_RNG_PLANES && tile_planes_supported(h, T);
-    if (use_tile_i8 || use_planes) {
+    const bool use_3d = !h->force_generic && h->rng == ISING_RNG_PLANES && tile3d_supported(h, T);
+    if (use_tile_i8 || use_planes || use_3d) {
         const bool bits = h->layout == ISING_LAYOUT_BITS;
-        h->last_path = use_tile_i8 ? "tile_i8" : (bits ? "tile_planes_bits" : "tile_planes_i8");
-        rc = ensure_store(h, use_tile_i8 ? Store::TileI8 : (bits ? Store::PlaneBits : Store::PlaneI8), T);
+        h->last_path = use_tile_i8 ? "tile_i8" : use_3d ? (bits ? "tile3d_planes_bits" : "tile3d_planes_i8")
+                                                        : (bits ? "tile_planes_bits" : "tile_planes_i8");
+        rc = ensure_store(h, use_tile_i8 ? Store::TileI8 : use_3d ? (bits ? Store::Plane3Bits : Store::Plane3I8)
+                                                                  : (bits ? Store::PlaneBits : Store::PlaneI8), T);
         if (!rc && use_planes && h->has_J && h->Jtiles_tile != T) {      // coupling records for this tile edge
             if (!h->d_Jtiles) {
                 h->d_Jtiles = dev_alloc(coupling_record_bytes(h));
@@ -302,7 +311,9 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         }
         for (int pass = 0; pass < n && !rc; ++pass) {
             const uint64_t t0 = h->t + (uint64_t)pass * (uint64_t)k;
-            rc = use_tile_i8 ? launch_tile_i8_pass(h, acc, T, k, t0) : launch_tile_planes_pass(h, acc, T, bits, k, t0);
+            rc = use_tile_i8 ? launch_tile_i8_pass(h, acc, T, k, t0)
+                 : use_3d ? launch_tile3d_pass(h, acc, bits, k, t0)
+                          : launch_tile_planes_pass(h, acc, T, bits, k, t0);
             if (!rc && want_series) {
                 rc = to_canon_scratch(h);
                 if (!rc) rc = launch_observables_canon(h, h->d_canon, d_E ? d_E + (size_t)pass * h->R : nullptr,

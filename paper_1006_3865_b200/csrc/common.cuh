@@ -40,7 +40,9 @@ enum class Store : int {
     Canon = 0,   // int8 ±1, index order, R*N bytes (generic kernels, observables, I/O)
     TileI8 = 1,  // tile records of 0/1 bytes, colour-split rows + edge columns (tile_i8.cu)
     PlaneI8 = 2, // piece-major tile records of 0/1 bytes (tile_planes.cu)
-    PlaneBits = 3 // tile records of bit words (tile_planes.cu)
+    PlaneBits = 3, // tile records of bit words (tile_planes.cu)
+    Plane3I8 = 4,  // 3D 8^3 tile records, 0/1 bytes + bit-packed face copies (tile3d_planes.cu)
+    Plane3Bits = 5 // 3D 8^3 tile records, bit words + face copies
 };
 
 // Acceptance constants handed to every sweep kernel (S8c.4/5).

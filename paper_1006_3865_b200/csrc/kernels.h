@@ -29,4 +29,11 @@ size_t coupling_record_bytes(const ising_ctx* h);
 int launch_convert_couplings(ising_ctx* h, int T, void* d_jrec);
 int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, int k, uint64_t t_first);
 
+// ---- tile3d_planes.cu: 3D multi-spin tile kernel, 8x8x8 tiles (RNG mapping "planes") ----------
+bool tile3d_supported(const ising_ctx* h, int T);
+size_t tile3d_bytes(const ising_ctx* h, bool bits);
+int launch_canon_to_3d(ising_ctx* h, bool bits, const int8_t* d_canon, void* d_tiles);
+int launch_3d_to_canon(ising_ctx* h, bool bits, const void* d_tiles, int8_t* d_canon);
+int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64_t t_first);
+
 }  // namespace ising

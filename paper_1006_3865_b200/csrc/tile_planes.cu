@@ -21,7 +21,7 @@
 //         Then T bytes left edge column (x = 0) and T bytes right edge column (x = T-1) by row.
 //   bits  record = T*T/8 bytes: word (cc, Y, gx) at ((cc*NW+gx)*LPT + Y)*4.
 #include "kernels.h"
-#include "philox.cuh"
+#include "planes_common.cuh"
 
 namespace ising {
 
@@ -56,62 +56,16 @@ struct PlaneArgs {
                                  // neighbour in the V1 / V2 / H1 / H2 word is J = -1.  Shared by all replicas.
 };
 
-template <int LUT>
-__device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
-    uint32_t r;
-    asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(r) : "r"(a), "r"(b), "r"(c), "n"(LUT));
-    return r;
-}
-// LOP3 immediates: value of f(a,b,c) at bit (a<<2 | b<<1 | c), a = 0xF0, b = 0xCC, c = 0xAA.
-constexpr int kLutChain = (~0xF0 & 0xAA) | (~(0xF0 ^ 0xAA) & 0xCC);    // (~p & u) | (~(p ^ u) & bw): p=a, bw=b, u=c
-constexpr int kLutNe = 0xF0 | (0xCC ^ 0xAA);                            // ne | (p ^ u): ne=a, p=b, u=c
-
-// Own-tile data is read once and written back by the same lane: plain (coherent) loads that
-// do not allocate in L1.  Halo data belongs to tiles of the other coarse colour, which this
-// launch never writes, so it may use the read-only path (__ldg).
-__device__ __forceinline__ uint4 ldg128(const void* p) {
-    uint4 v;
-    asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
-                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ uint32_t ldg32(const void* p) {
-    uint32_t v;
-    asm volatile("ld.global.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
-    return v;
-}
-__device__ __forceinline__ void stg128(void* p, uint4 v) {
-    asm volatile("st.global.v4.u32 [%4], {%0,%1,%2,%3};" ::"r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(p) : "memory");
-}
-
-// 4 bytes of 0/1 -> 4 bits in the top nibble: b0 -> bit 28, ..., b3 -> bit 31 (no carries collide).
-__device__ __forceinline__ uint32_t pack_step(uint32_t acc, uint32_t w) {
-    return __funnelshift_l(w * 0x10204080u, acc, 4);     // (acc << 4) | nibble
-}
-// 16 bytes (pairs 0..15) appended below acc: acc = (acc << 16) | bits, bit k = byte k.
-__device__ __forceinline__ uint32_t pack16(uint32_t acc, const uint4& v) {
-    acc = pack_step(acc, v.w);
-    acc = pack_step(acc, v.z);
-    acc = pack_step(acc, v.y);
-    return pack_step(acc, v.x);
-}
-
 template <int T>
 __device__ __forceinline__ void job_tile(const PlaneArgs& A, uint32_t job, int sub, int& r, int& tx, int& ty) {
     // colour-C tiles enumerated row by row: q -> ty = q / (B/2), tx = 2*(q % (B/2)) + ((ty + C) & 1)
     const uint32_t per_rep = (uint32_t)A.B * (uint32_t)A.B / 2u;
     const uint32_t q = job * PG<T>::TPW + (uint32_t)sub;
-    // q / per_rep and qq / hb by host-computed reciprocals ~2^32 / d, corrected by at most one either way
-    uint32_t rr = __umulhi(q, A.magic_rep);
-    if (rr * per_rep > q) --rr;
-    if ((rr + 1) * per_rep <= q) ++rr;
+    const uint32_t rr = fastdiv(q, per_rep, A.magic_rep);
     r = (int)rr;
     const uint32_t qq = q - rr * per_rep;
     const uint32_t hb = (uint32_t)A.B >> 1;
-    uint32_t yy = __umulhi(qq, A.magic_hb);
-    if (yy * hb > qq) --yy;
-    if ((yy + 1) * hb <= qq) ++yy;
-    ty = (int)yy;
+    ty = (int)fastdiv(qq, hb, A.magic_hb);
     tx = (int)(2u * (qq - (uint32_t)ty * hb)) + ((ty + A.C) & 1);
 }
 
@@ -315,11 +269,7 @@ __global__ void __launch_bounds__(128) k_tile_planes(PlaneArgs A) {
     using G = PG<T>;
     __shared__ uint2 lut[256];                  // int8 write-back: 8 bits -> 8 bytes of 0/1
     if (!BITS) {
-        for (int i = threadIdx.x; i < 256; i += blockDim.x) {
-            // 4 bits -> 4 bytes: n * 0x00204081 puts bit b at 8b (+ garbage elsewhere), no carries for n < 16
-            lut[i] = make_uint2(((uint32_t)(i & 15) * 0x00204081u) & 0x01010101u,
-                                ((uint32_t)(i >> 4) * 0x00204081u) & 0x01010101u);
-        }
+        build_byte_lut(lut);
         __syncthreads();
     }
     const int lane = threadIdx.x & 31;
@@ -483,9 +433,8 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
     A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
     const uint32_t tiles_per_colour = (uint32_t)((size_t)h->R * A.B * A.B / 2);
     A.njobs = tiles_per_colour / (uint32_t)(64 / T);
-    auto magic = [](uint32_t d) { return d <= 1 ? 0xffffffffu : (uint32_t)((0x100000000ull + d - 1) / d); };
-    A.magic_rep = magic((uint32_t)A.B * (uint32_t)A.B / 2u);
-    A.magic_hb = magic((uint32_t)A.B / 2u);
+    A.magic_rep = fastdiv_magic((uint32_t)A.B * (uint32_t)A.B / 2u);
+    A.magic_hb = fastdiv_magic((uint32_t)A.B / 2u);
     for (int q = 0; q < kHeadBits; ++q) {
         A.u1[q] = ((acc.thr[0] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
         A.u2[q] = ((acc.thr[1] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;

@@ -142,6 +142,27 @@ def test_tile_planes_couplings_match_oracle(P, orc, L, tile, k, n, beta, seeds, 
     assert np.array_equal(a.copy_spins().reshape(L, L) * eps, b.copy_spins().reshape(L, L))
 
 
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,k,n,beta,seeds", [
+    (16, 1, 4, BC3, [4]),            # B = 2: every halo wraps onto the other tile
+    (32, 4, 3, BC3, [4]),            # config 4 shape
+    (48, 2, 3, 0.3, [5, 6]),         # B = 6, replicas
+    (64, 1, 3, BC3, [9]),            # 2^18 sites: the tail is drawn about 50 times per half-sweep
+    (32, 2, 2, 0.0, [2]),
+    (32, 2, 2, 9.0, [2]),
+])
+def test_tile3d_path_matches_oracle(P, orc, L, k, n, beta, seeds, layout):
+    """3D 8x8x8 tile kernel (config 4), both HBM layouts, against the oracle."""
+    g, o = _both(P, orc, 3, L, seeds, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    Eg, Mg = g.sweep_series(beta, n, 8, k)
+    assert g.sweep_path() == f"tile3d_planes_{'i8' if layout == 'int8' else 'bits'}"
+    Eo, Mo = o.sweep_series(beta, n, 8, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+
+
 @pytest.mark.parametrize("L,tile,k,n,beta,seeds", TILED)
 def test_tile_i8_path_matches_oracle(P, orc, L, tile, k, n, beta, seeds):
     g, o = _both(P, orc, 2, L, seeds, rng="words")
