@@ -294,8 +294,22 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
     const bool use_tile_i8 = !h->force_generic && thr_fits && h->rng == ISING_RNG_WORDS &&
                              h->layout == ISING_LAYOUT_I8 && tile_i8_supported(h, T);
     const bool use_planes = !h->force_generic && h->rng == ISING_RNG_PLANES && tile_planes_supported(h, T);
+    const bool use_plain64 = !h->force_generic && h->rng == ISING_RNG_PLANES && plain64_supported(h, T);
     const bool use_3d = !h->force_generic && h->rng == ISING_RNG_PLANES && tile3d_supported(h, T);
-    if (use_tile_i8 || use_planes || use_3d) {
+    if (use_plain64) {                       // a8: whole run in one launch, E/M measured in the kernel
+        const bool bits = h->layout == ISING_LAYOUT_BITS;
+        h->last_path = bits ? "plain64_planes_bits" : "plain64_planes_i8";
+        rc = ensure_store(h, bits ? Store::PlaneBits : Store::PlaneI8, T);
+        if (!rc && h->has_J && h->Jtiles_tile != T) {
+            if (!h->d_Jtiles) {
+                h->d_Jtiles = dev_alloc(coupling_record_bytes(h));
+                if (!h->d_Jtiles) rc = ISING_ENOMEM;
+            }
+            if (!rc) rc = launch_convert_couplings(h, T, h->d_Jtiles);
+            if (!rc) h->Jtiles_tile = T;
+        }
+        if (!rc && n > 0) rc = launch_plain64(h, acc, bits, n, k, h->t, d_E, d_M);
+    } else if (use_tile_i8 || use_planes || use_3d) {
         const bool bits = h->layout == ISING_LAYOUT_BITS;
         h->last_path = use_tile_i8 ? "tile_i8" : use_3d ? (bits ? "tile3d_planes_bits" : "tile3d_planes_i8")
                                                         : (bits ? "tile_planes_bits" : "tile_planes_i8");

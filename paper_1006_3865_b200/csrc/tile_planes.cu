@@ -228,7 +228,9 @@ __device__ __forceinline__ uint32_t update_block(const PlaneArgs& A, uint32_t S,
 }
 
 // a5-a6: one half-sweep of colour c on the lane's block row; o = 1 - c is read, c is written.
-template <int T, bool HASJ>
+// PERIODIC: the tile is the whole lattice (T = L, the plain checkerboard of P:62): "halos" are the tile's own,
+// live, opposite edges.
+template <int T, bool HASJ, bool PERIODIC = false>
 __device__ __forceinline__ void half_sweep(const PlaneArgs& A, TileRegs<T>& t, const uint4 (&Jw)[2][PG<T>::NW], int c, int Y,
                                            uint32_t g0, uint32_t p0, uint64_t H, uint32_t k0, uint32_t k1) {
     using G = PG<T>;
@@ -239,22 +241,28 @@ __device__ __forceinline__ void half_sweep(const PlaneArgs& A, TileRegs<T>& t, c
     for (int gx = 0; gx < G::NW; ++gx) O[gx] = t.S[o][gx];
 #pragma unroll
     for (int gx = 0; gx < G::NW; ++gx) {
-        uint32_t Oup = __shfl_up_sync(0xffffffffu, O[gx], 1);
-        uint32_t Odn = __shfl_down_sync(0xffffffffu, O[gx], 1);
-        if (Y == 0) Oup = t.up[o][gx];
-        if (Y == G::LPT - 1) Odn = t.dn[o][gx];
+        uint32_t Oup, Odn;
+        if (PERIODIC) {
+            Oup = __shfl_sync(0xffffffffu, O[gx], (Y + G::LPT - 1) % G::LPT);
+            Odn = __shfl_sync(0xffffffffu, O[gx], (Y + 1) % G::LPT);
+        } else {
+            Oup = __shfl_up_sync(0xffffffffu, O[gx], 1);
+            Odn = __shfl_down_sync(0xffffffffu, O[gx], 1);
+            if (Y == 0) Oup = t.up[o][gx];
+            if (Y == G::LPT - 1) Odn = t.dn[o][gx];
+        }
         const uint32_t V1 = __byte_perm(O[gx], O[gx], 0x1032);        // the other row of the same block
         const uint32_t V2 = __byte_perm(Oup, Odn, 0x5432);            // row above the block | row below the block
         // pair-shifted word: colour 0: even rows look at pair j-1 (carry from the left), odd rows at j+1;
         // colour 1: even rows j+1, odd rows j-1.
         uint32_t H2;
         if (c == 0) {
-            const uint32_t cl = gx == 0 ? t.hL0 : ((O[gx > 0 ? gx - 1 : 0] >> 15) & 1u);
-            const uint32_t cr = gx == G::NW - 1 ? t.hR1 : ((O[gx < G::NW - 1 ? gx + 1 : gx] >> 16) & 1u);
+            const uint32_t cl = (gx == 0 && !PERIODIC) ? t.hL0 : ((O[(gx + G::NW - 1) % G::NW] >> 15) & 1u);
+            const uint32_t cr = (gx == G::NW - 1 && !PERIODIC) ? t.hR1 : ((O[(gx + 1) % G::NW] >> 16) & 1u);
             H2 = ((O[gx] << 1) & 0x0000fffeu) | cl | ((O[gx] >> 1) & 0x7fff0000u) | (cr << 31);
         } else {
-            const uint32_t cr = gx == G::NW - 1 ? t.hR0 : (O[gx < G::NW - 1 ? gx + 1 : gx] & 1u);
-            const uint32_t cl = gx == 0 ? t.hL1 : (O[gx > 0 ? gx - 1 : 0] >> 31);
+            const uint32_t cr = (gx == G::NW - 1 && !PERIODIC) ? t.hR0 : (O[(gx + 1) % G::NW] & 1u);
+            const uint32_t cl = (gx == 0 && !PERIODIC) ? t.hL1 : (O[(gx + G::NW - 1) % G::NW] >> 31);
             H2 = ((O[gx] >> 1) & 0x00007fffu) | (cr << 15) | ((O[gx] << 1) & 0xfffe0000u) | (cl << 16);
         }
         Snew[gx] = update_block<HASJ>(A, t.S[c][gx], V1, V2, O[gx], H2, Jw[c][gx], g0 + (uint32_t)gx,
@@ -298,6 +306,64 @@ __global__ void __launch_bounds__(128) k_tile_planes(PlaneArgs A) {
         half_sweep<T, HASJ>(A, t, Jw, 1, Y, g0, p0, 2 * tt + 1, k0, k1);
     }
     store_tile<T, BITS>(A, r, tx, ty, Y, t, lut);
+}
+
+// a8: plain checkerboard of a 64x64 lattice (tile = L = 64, BASELINE config 1).  One warp holds a whole
+// replica in registers and runs all n passes of the call in one launch; E and M after every pass (a10) come
+// from popcounts: M = 2*#up - N, E = -(2N - 2*#unsatisfied bonds), every bond seen once from its colour-0 end.
+template <bool BITS, bool HASJ>
+__global__ void __launch_bounds__(32) k_plain64_planes(PlaneArgs A, int n, long long* __restrict__ E, long long* __restrict__ M) {
+    constexpr int T = 64;
+    using G = PG<T>;
+    __shared__ uint2 lut[BITS ? 1 : 256];
+    if (!BITS) {
+        build_byte_lut(lut);
+        __syncwarp();
+    }
+    const int Y = threadIdx.x, r = blockIdx.x;
+    TileRegs<T> t;
+    load_tile<T, BITS>(A, r, 0, 0, Y, 0, t);
+    uint4 Jw[2][G::NW];
+#pragma unroll
+    for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+        for (int gx = 0; gx < G::NW; ++gx)
+            Jw[cc][gx] = HASJ ? __ldg(A.jrec + (cc * G::NW + gx) * G::LPT + Y) : make_uint4(0u, 0u, 0u, 0u);
+    const uint64_t seed = A.seeds[r];
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    const uint32_t g0 = (uint32_t)Y * G::NW, p0 = 2u * (uint32_t)Y * (T / 2);
+    for (int pass = 0; pass < n; ++pass) {
+        for (int j = 0; j < A.k; ++j) {
+            const uint64_t tt = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
+            half_sweep<T, HASJ, true>(A, t, Jw, 0, Y, g0, p0, 2 * tt, k0, k1);
+            half_sweep<T, HASJ, true>(A, t, Jw, 1, Y, g0, p0, 2 * tt + 1, k0, k1);
+        }
+        if (E || M) {
+            int up = 0, unsat = 0;
+#pragma unroll
+            for (int gx = 0; gx < G::NW; ++gx) {
+                const uint32_t S = t.S[0][gx], O = t.S[1][gx];
+                const uint32_t Oup = __shfl_sync(0xffffffffu, O, (Y + G::LPT - 1) % G::LPT);
+                const uint32_t Odn = __shfl_sync(0xffffffffu, O, (Y + 1) % G::LPT);
+                const uint32_t V1 = __byte_perm(O, O, 0x1032), V2 = __byte_perm(Oup, Odn, 0x5432);
+                const uint32_t cl = (t.S[1][(gx + G::NW - 1) % G::NW] >> 15) & 1u, cr = (t.S[1][(gx + 1) % G::NW] >> 16) & 1u;
+                const uint32_t H2 = ((O << 1) & 0x0000fffeu) | cl | ((O >> 1) & 0x7fff0000u) | (cr << 31);
+                const uint4 Jc = Jw[0][gx];
+                unsat += __popc(S ^ V1 ^ Jc.x) + __popc(S ^ V2 ^ Jc.y) + __popc(S ^ O ^ Jc.z) + __popc(S ^ H2 ^ Jc.w);
+                up += __popc(S) + __popc(O);
+            }
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                up += __shfl_xor_sync(0xffffffffu, up, d);
+                unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+            }
+            if (Y == 0) {
+                if (M) M[(size_t)pass * A.R + r] = 2ll * up - (long long)(T * T);
+                if (E) E[(size_t)pass * A.R + r] = 2ll * unsat - 2ll * (T * T);
+            }
+        }
+    }
+    store_tile<T, BITS>(A, r, 0, 0, Y, t, lut);
 }
 
 // ---- layout converters (a11): canonical int8 +-1 <-> tile records; not on the timed path ----
@@ -424,6 +490,41 @@ int launch_planes_to_canon(ising_ctx* h, int T, bool bits, const void* d_tiles, 
     return 0;
 }
 
+bool plain64_supported(const ising_ctx* h, int T) { return h->dim == 2 && h->L == 64 && T == 64; }
+
+static void fill_accept(PlaneArgs& A, const Accept& acc) {
+    for (int q = 0; q < kHeadBits; ++q) {
+        A.u1[q] = ((acc.thr[0] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
+        A.u2[q] = ((acc.thr[1] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
+    }
+    A.force1 = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
+    A.force2 = acc.thr_is_2p32[1] ? 0xffffffffu : 0u;
+    A.t1_tail = acc.thr[0] & ((1u << kTailBits) - 1u);
+    A.t2_tail = acc.thr[1] & ((1u << kTailBits) - 1u);
+}
+
+// a8: all n passes of a 64x64 plain-checkerboard run in one launch, one warp per replica; d_E / d_M (n*R each) optional.
+int launch_plain64(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M) {
+    PlaneArgs A;
+    A.tiles = (uint8_t*)h->d_tiles;
+    A.seeds = h->d_seeds;
+    A.L = 64; A.B = 1; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0; A.njobs = (uint32_t)h->R;
+    A.magic_rep = A.magic_hb = 0;
+    A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
+    fill_accept(A, acc);
+    cudaStream_t st = hooks().stream;
+    if (bits) {
+        if (A.jrec) k_plain64_planes<true, true><<<h->R, 32, 0, st>>>(A, n, d_E, d_M);
+        else k_plain64_planes<true, false><<<h->R, 32, 0, st>>>(A, n, d_E, d_M);
+    } else {
+        if (A.jrec) k_plain64_planes<false, true><<<h->R, 32, 0, st>>>(A, n, d_E, d_M);
+        else k_plain64_planes<false, false><<<h->R, 32, 0, st>>>(A, n, d_E, d_M);
+    }
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
 // a1: one outer pass = colour-0 launch, colour-1 launch, k inner sweeps each.
 int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, int k, uint64_t t_first) {
     PlaneArgs A;
@@ -435,14 +536,7 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
     A.njobs = tiles_per_colour / (uint32_t)(64 / T);
     A.magic_rep = fastdiv_magic((uint32_t)A.B * (uint32_t)A.B / 2u);
     A.magic_hb = fastdiv_magic((uint32_t)A.B / 2u);
-    for (int q = 0; q < kHeadBits; ++q) {
-        A.u1[q] = ((acc.thr[0] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
-        A.u2[q] = ((acc.thr[1] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
-    }
-    A.force1 = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
-    A.force2 = acc.thr_is_2p32[1] ? 0xffffffffu : 0u;
-    A.t1_tail = acc.thr[0] & ((1u << kTailBits) - 1u);
-    A.t2_tail = acc.thr[1] & ((1u << kTailBits) - 1u);
+    fill_accept(A, acc);
     for (int C = 0; C < 2; ++C) {
         A.C = C;
         if (T == 64) bits ? launch_colour_planes<64, true>(A) : launch_colour_planes<64, false>(A);

@@ -163,6 +163,24 @@ def test_tile3d_path_matches_oracle(P, orc, L, k, n, beta, seeds, layout):
     _same_state(g, o)
 
 
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("k,n,beta,seeds,jseed", [(1, 50, BC2, [1], None), (3, 7, 0.6, [1, 2, 3], None), (2, 9, 1.0, [5, 6], 7),
+                                                    (1, 4, 0.0, [2], None)])
+def test_plain64_path_matches_oracle(P, orc, k, n, beta, seeds, jseed, layout):
+    """a8 / config 1 shape: 64x64 plain checkerboard, all passes in one launch, E and M measured in the kernel."""
+    J = W.couplings(2, 64, jseed) if jseed is not None else None
+    g, o = _both(P, orc, 2, 64, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    Eg, Mg = g.sweep_series(beta, n, 0, k)
+    assert g.sweep_path() == f"plain64_planes_{'i8' if layout == 'int8' else 'bits'}"
+    Eo, Mo = o.sweep_series(beta, n, 64, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    g.sweep(beta, 3, 64, k); o.sweep(beta, 3, 0, k)          # without the series, and composing with the counter
+    _same_state(g, o)
+
+
 @pytest.mark.parametrize("L,tile,k,n,beta,seeds", TILED)
 def test_tile_i8_path_matches_oracle(P, orc, L, tile, k, n, beta, seeds):
     g, o = _both(P, orc, 2, L, seeds, rng="words")
