@@ -48,8 +48,10 @@ __device__ __forceinline__ uint32_t pack16(uint32_t acc, const uint4& v) {
 }
 
 // int8 write-back table: 8 bits -> 8 bytes of 0/1 (256 entries, built once per CTA; caller syncs).
+template <int THREADS>
 __device__ __forceinline__ void build_byte_lut(uint2* lut) {
-    for (int i = threadIdx.x; i < 256; i += blockDim.x) {
+#pragma unroll
+    for (int i = threadIdx.x; i < 256; i += THREADS) {
         // 4 bits -> 4 bytes: n * 0x00204081 puts bit b at 8b (+ garbage elsewhere), no carries for n < 16
         lut[i] = make_uint2(((uint32_t)(i & 15) * 0x00204081u) & 0x01010101u,
                             ((uint32_t)(i >> 4) * 0x00204081u) & 0x01010101u);

@@ -212,7 +212,7 @@ template <bool BITS>
 __global__ void __launch_bounds__(128) k_tile3d_planes(Plane3Args A) {
     __shared__ uint2 lut[BITS ? 1 : 256];
     if (!BITS) {
-        build_byte_lut(lut);
+        build_byte_lut<128>(lut);
         __syncthreads();
     }
     const int lane = threadIdx.x & 31;

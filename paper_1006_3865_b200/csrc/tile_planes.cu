@@ -81,38 +81,27 @@ struct TileRegs {
 template <int T, bool BITS>
 __device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int ty, int Y, int lane_base, TileRegs<T>& t) {
     using G = PG<T>;
-    constexpr int REC = BITS ? G::REC_BITS : G::REC_I8;
-    const int B = A.B;
-    const size_t rep = (size_t)r * B * B;
-    const uint8_t* rec = A.tiles + (rep + (size_t)ty * B + tx) * REC;
-    const uint8_t* recU = A.tiles + (rep + (size_t)(ty == 0 ? B - 1 : ty - 1) * B + tx) * REC;
-    const uint8_t* recD = A.tiles + (rep + (size_t)(ty == B - 1 ? 0 : ty + 1) * B + tx) * REC;
-    const uint8_t* recL = A.tiles + (rep + (size_t)ty * B + (tx == 0 ? B - 1 : tx - 1)) * REC;
-    const uint8_t* recR = A.tiles + (rep + (size_t)ty * B + (tx == B - 1 ? 0 : tx + 1)) * REC;
-    // halo rows: lane Y = idx < 4*NW fetches item idx = (which, cc, gx); which 0 = top, 1 = bottom
+    constexpr uint32_t REC = BITS ? G::REC_BITS : G::REC_I8;
+    // tile indices in 32 bits, one widening multiply per record address
+    const uint32_t B = (uint32_t)A.B, utx = (uint32_t)tx, uty = (uint32_t)ty;
+    const uint32_t row0 = (uint32_t)r * B * B, rowc = row0 + uty * B;
+    const uint32_t tyU = uty == 0 ? B - 1 : uty - 1, tyD = uty == B - 1 ? 0 : uty + 1;
+    const uint32_t txL = utx == 0 ? B - 1 : utx - 1, txR = utx == B - 1 ? 0 : utx + 1;
+    auto rec_of = [&](uint32_t idx) { return A.tiles + (uint64_t)idx * REC; };
+    const uint8_t* rec = rec_of(rowc + utx);
+    const uint8_t* recL = rec_of(rowc + txL);
+    const uint8_t* recR = rec_of(rowc + txR);
+    // halo rows: lane Y = idx < 4*NW fetches item idx = (which, cc, gx); which 0 = row above, 1 = row below
+    const int which = Y / (2 * G::NW), idx = Y % (2 * G::NW);
+    const uint8_t* recV = rec_of(row0 + (which == 0 ? tyU : tyD) * B + utx);
     uint32_t item = 0;
-    {
-        const int which = Y / (2 * G::NW), rem = Y % (2 * G::NW), cc = rem / G::NW, gx = rem % G::NW;
-        if (Y < 4 * G::NW) {
-            if (BITS) {
-                const uint8_t* src = which == 0 ? recU + ((cc * G::NW + gx) * G::LPT + (G::LPT - 1)) * 4
-                                                : recD + ((cc * G::NW + gx) * G::LPT) * 4;
-                item = __ldg(reinterpret_cast<const uint32_t*>(src));
-            } else {
-                const int piece = ((which == 0 ? 2 : 0) + cc) * G::NW + gx;      // rp = 1 for the row above, 0 below
-                const uint8_t* src = (which == 0 ? recU + (piece * G::LPT + (G::LPT - 1)) * 16
-                                                 : recD + (piece * G::LPT) * 16);
-                const uint32_t b = pack16(0u, __ldg(reinterpret_cast<const uint4*>(src)));
-                item = which == 0 ? (b << 16) : b;
-            }
-        }
-    }
     if (BITS) {
+        if (Y < 4 * G::NW)
+            item = __ldg(reinterpret_cast<const uint32_t*>(recV + (idx * G::LPT + (which == 0 ? G::LPT - 1 : 0)) * 4));
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
-            for (int gx = 0; gx < G::NW; ++gx)
-                t.S[cc][gx] = ldg32(rec + ((cc * G::NW + gx) * G::LPT + Y) * 4);
+            for (int gx = 0; gx < G::NW; ++gx) t.S[cc][gx] = ldg32(rec + ((cc * G::NW + gx) * G::LPT + Y) * 4);
         const uint32_t l1 = __ldg(reinterpret_cast<const uint32_t*>(recL + ((1 * G::NW + G::NW - 1) * G::LPT + Y) * 4));
         const uint32_t l0 = __ldg(reinterpret_cast<const uint32_t*>(recL + ((0 * G::NW + G::NW - 1) * G::LPT + Y) * 4));
         const uint32_t r0 = __ldg(reinterpret_cast<const uint32_t*>(recR + ((0 * G::NW + 0) * G::LPT + Y) * 4));
@@ -125,13 +114,18 @@ __device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int
         uint4 v[G::NCH];
 #pragma unroll
         for (int ch = 0; ch < G::NCH; ++ch) v[ch] = ldg128(rec + (ch * G::LPT + Y) * 16);
-        const uint32_t eL = __ldg(reinterpret_cast<const uint16_t*>(recL + G::BODY + T + 2 * Y));
-        const uint32_t eR = __ldg(reinterpret_cast<const uint16_t*>(recR + G::BODY + 2 * Y));
+        uint4 hv = make_uint4(0u, 0u, 0u, 0u);
+        if (Y < 4 * G::NW)   // row above = row T-1 (rp = 1) of the tile above; row below = row 0 of the tile below
+            hv = __ldg(reinterpret_cast<const uint4*>(recV + (which == 0 ? ((2 * G::NW + idx) * G::LPT + G::LPT - 1) : idx * G::LPT) * 16));
+        const uint32_t eL = __ldg(reinterpret_cast<const uint16_t*>(recL + G::BODY + T + 2 * Y));   // neighbour's right edge
+        const uint32_t eR = __ldg(reinterpret_cast<const uint16_t*>(recR + G::BODY + 2 * Y));       // neighbour's left edge
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
             for (int gx = 0; gx < G::NW; ++gx)
                 t.S[cc][gx] = pack16(pack16(0u, v[(2 + cc) * G::NW + gx]), v[cc * G::NW + gx]);
+        const uint32_t b = pack16(0u, hv);
+        item = which == 0 ? (b << 16) : b;
         t.hL0 = eL & 1u; t.hL1 = (eL >> 8) & 1u;
         t.hR0 = eR & 1u; t.hR1 = (eR >> 8) & 1u;
     }
@@ -149,8 +143,8 @@ template <int T, bool BITS>
 __device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, int ty, int Y, const TileRegs<T>& t,
                                            const uint2* lut) {
     using G = PG<T>;
-    constexpr int REC = BITS ? G::REC_BITS : G::REC_I8;
-    uint8_t* rec = A.tiles + (((size_t)r * A.B + ty) * A.B + tx) * REC;
+    constexpr uint32_t REC = BITS ? G::REC_BITS : G::REC_I8;
+    uint8_t* rec = A.tiles + (uint64_t)(((uint32_t)r * (uint32_t)A.B + (uint32_t)ty) * (uint32_t)A.B + (uint32_t)tx) * REC;
     if (BITS) {
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
@@ -272,12 +266,14 @@ __device__ __forceinline__ void half_sweep(const PlaneArgs& A, TileRegs<T>& t, c
     for (int gx = 0; gx < G::NW; ++gx) t.S[c][gx] = Snew[gx];
 }
 
+constexpr int kPlaneThreads = 128;      // 4 warps = 4 jobs per CTA
+
 template <int T, bool BITS, bool HASJ>
-__global__ void __launch_bounds__(128) k_tile_planes(PlaneArgs A) {
+__global__ void __launch_bounds__(kPlaneThreads) k_tile_planes(PlaneArgs A) {
     using G = PG<T>;
     __shared__ uint2 lut[256];                  // int8 write-back: 8 bits -> 8 bytes of 0/1
     if (!BITS) {
-        build_byte_lut(lut);
+        build_byte_lut<kPlaneThreads>(lut);
         __syncthreads();
     }
     const int lane = threadIdx.x & 31;
@@ -317,7 +313,7 @@ __global__ void __launch_bounds__(32) k_plain64_planes(PlaneArgs A, int n, long 
     using G = PG<T>;
     __shared__ uint2 lut[BITS ? 1 : 256];
     if (!BITS) {
-        build_byte_lut(lut);
+        build_byte_lut<32>(lut);
         __syncwarp();
     }
     const int Y = threadIdx.x, r = blockIdx.x;
@@ -430,7 +426,7 @@ __global__ void k_convert_couplings(const int8_t* __restrict__ J, uint32_t* __re
 
 template <int T, bool BITS>
 int launch_colour_planes(const PlaneArgs& A) {
-    const int warps = 4;
+    const int warps = kPlaneThreads / 32;
     const uint32_t grid = (A.njobs + warps - 1) / warps;
     if (A.jrec) k_tile_planes<T, BITS, true><<<grid, warps * 32, 0, hooks().stream>>>(A);
     else k_tile_planes<T, BITS, false><<<grid, warps * 32, 0, hooks().stream>>>(A);
