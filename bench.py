@@ -47,6 +47,17 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
 
 
+# From the committed ncu captures (profiles/r01c_tile_planes_i8_t64.md), per launch of the kernel:
+# DRAM bytes read + written, and executed warp-instructions.  Keyed by (rng, layout, tile, k).
+NCU = {
+    ("planes", "int8", 64, 1): {"traffic": 171.99e6 + 82.06e6, "warp_instr": 37.42e6},
+    ("planes", "int8", 64, 16): {"traffic": 171.99e6 + 82.50e6, "warp_instr": 434.9e6},
+}
+# Issue ceiling of the path: 148 SMs x 4 SMSPs, one warp-instruction per 2 cycles at sm_max_mhz.
+def issue_peak_gips(sm_mhz: float) -> float:
+    return 148 * 4 * sm_mhz * 1e6 / 2 / 1e9
+
+
 class ClockSampler:
     """nvidia-smi clocks + throttle reasons during the timed region (B200_PROFILING.md recipe)."""
 
@@ -226,7 +237,8 @@ def main() -> None:
     flips = world * a.steps * a.k * L * L
     value = flips / (ms * 1e6)
 
-    peak, peak_src, _ = measured_peaks()
+    peak, peak_src, sm_max = measured_peaks()
+    ncu = NCU.get((a.rng, a.layout, a.tile, a.k)) if L == 16384 else None
     bpf = algorithmic_bytes_per_flip(a.tile, a.k, a.layout)
     launches_per_step = 2
     bytes_per_launch = bpf * a.k * L * L / launches_per_step
@@ -242,9 +254,15 @@ def main() -> None:
                        "kernel_path": res["path"], "parallelism": "replicas only" if world > 1 else "single GPU"},
             "ns_per_flip": 1.0 / value, "gpu_launches": res["launches"], "clocks": res["clocks"],
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": None, "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
+                         "traffic": ncu["traffic"] if ncu else None,
+                         "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01c_tile_planes_i8_t64.md" if ncu else None,
+                         "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
                          "algorithmic_bytes_per_flip": bpf, "kernel": f"{res['path']}<{a.tile}>",
-                         "avg_launch_ms": launch_ms}}
+                         "avg_launch_ms": launch_ms,
+                         "issue": ({"bound": "alu", "unit": "G warp-instr/s", "achieved": ncu["warp_instr"] / (launch_ms * 1e6),
+                                    "peak": issue_peak_gips(sm_max), "frac": ncu["warp_instr"] / (launch_ms * 1e6) / issue_peak_gips(sm_max),
+                                    "note": "DESIGN.md 7.3: IMAD.WIDE and LOP3 do not overlap on sm_100a, 2 SMSP-cycles per warp-instruction"}
+                                   if ncu else None)}}
     if rank == 0 and not a.no_extras and world == 1:
         table = {}
         for rng, lay in (("planes", "int8"), ("planes", "bits"), ("words", "int8")):

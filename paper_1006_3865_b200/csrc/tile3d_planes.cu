@@ -41,7 +41,7 @@ struct Plane3Args {
     uint32_t magic_rep, magic_z, magic_hb;
     uint32_t u[3][kHeadBits];    // plane q: all-ones if bit (31-q) of thr[m+1] is set
     uint32_t tail[3];            // thr[m+1] & (2^20 - 1)
-    uint32_t force[3];           // all-ones if thr[m+1] = 2^32
+    uint32_t force;              // all-ones if beta = 0 (every thr = 2^32: every proposal is accepted)
 };
 
 struct Tile3 {
@@ -167,7 +167,7 @@ __device__ __forceinline__ void head_masks3(const Plane3Args& A, uint32_t g, uin
         }
     }
 #pragma unroll
-    for (int m = 0; m < 3; ++m) { R[m] = bw[m] | A.force[m]; eq[m] = ~ne[m]; }
+    for (int m = 0; m < 3; ++m) { R[m] = bw[m]; eq[m] = ~ne[m]; }
 }
 
 // One half-sweep of colour c on the lane's slice (a4-a5, 6 neighbours).
@@ -192,7 +192,7 @@ __device__ __forceinline__ void half_sweep3(const Plane3Args& A, Slice& s, int c
     const uint32_t p1 = a | b, q1 = a & b, p2 = e | f, q2 = e & f, p3 = x | y, q3 = x & y;
     const uint32_t ge1 = p1 | p2 | p3;
     const uint32_t ge2 = q1 | q2 | q3 | (p1 & p2) | (p1 & p3) | (p2 & p3);
-    const uint32_t ge3 = (q1 & (p2 | p3)) | (q2 & (p1 | p3)) | (q3 & (p1 | p2)) | (p1 & p2 & p3);   // dE <= 0: always flip
+    const uint32_t ge3 = (q1 & (p2 | p3)) | (q2 & (p1 | p3)) | (q3 & (p1 | p2)) | (p1 & p2 & p3) | A.force;   // dE <= 0: always flip
     uint32_t und = (eq[0] & ge2 & ~ge3) | (eq[1] & ge1 & ~ge2) | (eq[2] & ~ge1);   // n_dis = 2, 1, 0 need thr[1], thr[2], thr[3]
     while (und) {                                                   // probability 2^-12 per site
         const int j = __ffs(und) - 1;
@@ -319,8 +319,8 @@ int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64
     for (int m = 0; m < 3; ++m) {
         for (int q = 0; q < kHeadBits; ++q) A.u[m][q] = ((acc.thr[m] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
         A.tail[m] = acc.thr[m] & ((1u << kTailBits) - 1u);
-        A.force[m] = acc.thr_is_2p32[m] ? 0xffffffffu : 0u;
     }
+    A.force = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
     const int warps = 4;
     const uint32_t grid = (A.njobs + warps - 1) / warps;
     for (int C = 0; C < 2; ++C) {

@@ -50,7 +50,7 @@ struct PlaneArgs {
     uint32_t u1[kHeadBits];      // plane q: all-ones if bit (31-q) of thr[1] is set, else 0
     uint32_t u2[kHeadBits];      // same for thr[2]
     uint32_t t1_tail, t2_tail;   // thr[m] & (2^20 - 1)
-    uint32_t force1, force2;     // all-ones if thr[m] = 2^32 (beta = 0: every r is below it), else 0
+    uint32_t force;              // all-ones if beta = 0 (every thr[m] = 2^32: every proposal is accepted), else 0
     const uint4* jrec;           // coupling records (a9) or nullptr: per tile, uint4 (cc, gx, Y) =
                                  // {V1, V2, H1, H2}: bit j set <=> the bond from site j of that block to its
                                  // neighbour in the V1 / V2 / H1 / H2 word is J = -1.  Shared by all replicas.
@@ -190,7 +190,7 @@ __device__ __forceinline__ void head_masks(const PlaneArgs& A, uint32_t g, uint3
             ne2 = lop3<kLutNe>(ne2, p[w], A.u2[q]);
         }
     }
-    R1 = bw1 | A.force1; R2 = bw2 | A.force2; eq1 = ~ne1; eq2 = ~ne2;
+    R1 = bw1; R2 = bw2; eq1 = ~ne1; eq2 = ~ne2;
 }
 
 // a4-a5 for one block: S' = S ^ flip, neighbours V1, V2 (vertical), H1, H2 (horizontal) of the other colour.
@@ -206,7 +206,7 @@ __device__ __forceinline__ uint32_t update_block(const PlaneArgs& A, uint32_t S,
     const uint32_t c = S ^ H1 ^ (HASJ ? Jw.z : 0u), d = S ^ H2 ^ (HASJ ? Jw.w : 0u);
     const uint32_t p1 = a | b, q1 = a & b, p2 = c | d, q2 = c & d;
     const uint32_t ge1 = p1 | p2;                                     // n_dis >= 1
-    const uint32_t ge2 = (p1 & p2) | q1 | q2;                         // n_dis >= 2  <=>  dE <= 0: always flip (eq. (2))
+    const uint32_t ge2 = (p1 & p2) | q1 | q2 | A.force;               // n_dis >= 2  <=>  dE <= 0: always flip (eq. (2))
     uint32_t und = (eq1 & ge1 & ~ge2) | (eq2 & ~ge1);                 // n_dis == 1 needs thr[1], n_dis == 0 needs thr[2]
     while (und) {                                                     // probability 2^-12 per site
         const int j = __ffs(und) - 1;
@@ -272,10 +272,12 @@ template <int T, bool BITS, bool HASJ>
 __global__ void __launch_bounds__(kPlaneThreads) k_tile_planes(PlaneArgs A) {
     using G = PG<T>;
     __shared__ uint2 lut[256];                  // int8 write-back: 8 bits -> 8 bytes of 0/1
-    if (!BITS) {
-        build_byte_lut<kPlaneThreads>(lut);
-        __syncthreads();
-    }
+    // Programmatic dependent launch: the next colour's grid may be scheduled while this one drains; it builds
+    // its table and then waits here until every store of the previous launch is visible.
+    asm volatile("griddepcontrol.launch_dependents;");
+    if (!BITS) build_byte_lut<kPlaneThreads>(lut);
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    if (!BITS) __syncthreads();
     const int lane = threadIdx.x & 31;
     const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (job >= A.njobs) return;
@@ -428,8 +430,14 @@ template <int T, bool BITS>
 int launch_colour_planes(const PlaneArgs& A) {
     const int warps = kPlaneThreads / 32;
     const uint32_t grid = (A.njobs + warps - 1) / warps;
-    if (A.jrec) k_tile_planes<T, BITS, true><<<grid, warps * 32, 0, hooks().stream>>>(A);
-    else k_tile_planes<T, BITS, false><<<grid, warps * 32, 0, hooks().stream>>>(A);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(warps * 32); cfg.dynamicSmemBytes = 0; cfg.stream = hooks().stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (A.jrec) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes<T, BITS, true>, A));
+    else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes<T, BITS, false>, A));
     count_launch();
     return 0;
 }
@@ -493,8 +501,7 @@ static void fill_accept(PlaneArgs& A, const Accept& acc) {
         A.u1[q] = ((acc.thr[0] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
         A.u2[q] = ((acc.thr[1] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
     }
-    A.force1 = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
-    A.force2 = acc.thr_is_2p32[1] ? 0xffffffffu : 0u;
+    A.force = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;       // thr[m] = 2^32 happens only at beta = 0, for every m at once
     A.t1_tail = acc.thr[0] & ((1u << kTailBits) - 1u);
     A.t2_tail = acc.thr[1] & ((1u << kTailBits) - 1u);
 }
