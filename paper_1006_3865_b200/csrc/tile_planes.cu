@@ -14,12 +14,13 @@
 // (one 64x64 tile or two 32x32 tiles), lane = block row, vertical neighbours come by shuffle,
 // the k inner sweeps never touch memory.
 //
-// HBM layouts (tile records; a tile and every piece of its halo are contiguous 16-byte runs):
-//   int8  record = T*T body + 2T edge bytes, 0/1 per spin.  Body is piece-major: the 16 bytes
+// HBM layouts (tile records; PG below):
+//   int8  record = T*T body + 64 edge bytes, 0/1 per spin.  Body is piece-major: the 16 bytes
 //         (row 2Y+rp, colour cc, pairs 16gx..16gx+15) sit at ((rp*2+cc)*NW+gx)*LPT*16 + Y*16, so lane Y
 //         loads its 4*NW pieces with fully coalesced 128-bit accesses and no shared-memory staging.
-//         Then T bytes left edge column (x = 0) and T bytes right edge column (x = T-1) by row.
-//   bits  record = T*T/8 bytes: word (cc, Y, gx) at ((cc*NW+gx)*LPT + Y)*4.
+//   bits  record = T*T/8 body + 64 edge bytes: word (cc, Y, gx) at ((cc*NW+gx)*LPT + Y)*4.
+//   edge  = bit-packed copies of the tile's own first / last block row and first / last column, written by
+//         the tile, so that every halo is one 16-byte run of ready-made words in the neighbour's record.
 #include "kernels.h"
 #include "planes_common.cuh"
 
@@ -34,8 +35,15 @@ struct PG {
     static constexpr int TPW = 64 / T;           // tiles per warp job
     static constexpr int NCH = 4 * NW;           // 16-byte pieces per lane
     static constexpr int BODY = T * T;
-    static constexpr int REC_I8 = T * T + 2 * T;
-    static constexpr int REC_BITS = T * T / 8;
+    // Every record ends with 64 bytes of bit-packed copies of the tile's own boundary, written by the tile, so
+    // that a neighbour reads each halo as one 16-byte run of ready-made words (no sector per row, no unpacking):
+    //   +0  TOP[cc][gx]: the words of block row 0 (low half = tile row 0)     -> the tile above reads them as "dn"
+    //   +16 COL[4]: bit Y of {L0, L1, R0, R1} = spin at x = 0 of row 2Y, x = 0 of row 2Y+1, x = T-1 of row 2Y, of row 2Y+1
+    //   +32 BOT[cc][gx]: the words of block row LPT-1 (high half = row T-1)   -> the tile below reads them as "up"
+    //   +48 zero padding, so that both 32-byte sectors are always written whole (no read-modify-write in L2 / HBM)
+    static constexpr int EDGE = 64, E_TOP = 0, E_COL = 16, E_BOT = 32;
+    static constexpr int REC_I8 = T * T + EDGE;
+    static constexpr int REC_BITS = T * T / 8 + EDGE;
 };
 
 struct PlaneArgs {
@@ -73,8 +81,8 @@ __device__ __forceinline__ void job_tile(const PlaneArgs& A, uint32_t job, int s
 template <int T>
 struct TileRegs {
     uint32_t S[2][PG<T>::NW];     // S[cc][gx]: the lane's block row, colour cc
-    uint32_t up[2][PG<T>::NW];    // lane Y = 0: block row above (high half = halo row -1), by colour
-    uint32_t dn[2][PG<T>::NW];    // lane Y = LPT-1: block row below (low half = halo row T)
+    uint32_t vrow[2][PG<T>::NW];  // lane Y = 0: block row above (high half = halo row -1), lane Y = LPT-1: block
+                                  // row below (low half = halo row T), by colour; unused on the other lanes
     uint32_t hL0, hL1, hR0, hR1;  // halo column bits: x = -1 / x = T of rows 2Y (0) and 2Y+1 (1)
 };
 
@@ -82,6 +90,7 @@ template <int T, bool BITS>
 __device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int ty, int Y, int lane_base, TileRegs<T>& t) {
     using G = PG<T>;
     constexpr uint32_t REC = BITS ? G::REC_BITS : G::REC_I8;
+    constexpr uint32_t BODY = REC - G::EDGE;
     // tile indices in 32 bits, one widening multiply per record address
     const uint32_t B = (uint32_t)A.B, utx = (uint32_t)tx, uty = (uint32_t)ty;
     const uint32_t row0 = (uint32_t)r * B * B, rowc = row0 + uty * B;
@@ -89,61 +98,43 @@ __device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int
     const uint32_t txL = utx == 0 ? B - 1 : utx - 1, txR = utx == B - 1 ? 0 : utx + 1;
     auto rec_of = [&](uint32_t idx) { return A.tiles + (uint64_t)idx * REC; };
     const uint8_t* rec = rec_of(rowc + utx);
-    const uint8_t* recL = rec_of(rowc + txL);
-    const uint8_t* recR = rec_of(rowc + txR);
-    // halo rows: lane Y = idx < 4*NW fetches item idx = (which, cc, gx); which 0 = row above, 1 = row below
-    const int which = Y / (2 * G::NW), idx = Y % (2 * G::NW);
-    const uint8_t* recV = rec_of(row0 + (which == 0 ? tyU : tyD) * B + utx);
-    uint32_t item = 0;
     if (BITS) {
-        if (Y < 4 * G::NW)
-            item = __ldg(reinterpret_cast<const uint32_t*>(recV + (idx * G::LPT + (which == 0 ? G::LPT - 1 : 0)) * 4));
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
             for (int gx = 0; gx < G::NW; ++gx) t.S[cc][gx] = ldg32(rec + ((cc * G::NW + gx) * G::LPT + Y) * 4);
-        const uint32_t l1 = __ldg(reinterpret_cast<const uint32_t*>(recL + ((1 * G::NW + G::NW - 1) * G::LPT + Y) * 4));
-        const uint32_t l0 = __ldg(reinterpret_cast<const uint32_t*>(recL + ((0 * G::NW + G::NW - 1) * G::LPT + Y) * 4));
-        const uint32_t r0 = __ldg(reinterpret_cast<const uint32_t*>(recR + ((0 * G::NW + 0) * G::LPT + Y) * 4));
-        const uint32_t r1 = __ldg(reinterpret_cast<const uint32_t*>(recR + ((1 * G::NW + 0) * G::LPT + Y) * 4));
-        t.hL0 = (l1 >> 15) & 1u;   // (x = T-1, even row) is colour 1, pair 15 of the last block
-        t.hL1 = l0 >> 31;          // (x = T-1, odd row) is colour 0
-        t.hR0 = r0 & 1u;           // (x = 0, even row) is colour 0
-        t.hR1 = (r1 >> 16) & 1u;   // (x = 0, odd row) is colour 1
     } else {
         uint4 v[G::NCH];
 #pragma unroll
         for (int ch = 0; ch < G::NCH; ++ch) v[ch] = ldg128(rec + (ch * G::LPT + Y) * 16);
-        uint4 hv = make_uint4(0u, 0u, 0u, 0u);
-        if (Y < 4 * G::NW)   // row above = row T-1 (rp = 1) of the tile above; row below = row 0 of the tile below
-            hv = __ldg(reinterpret_cast<const uint4*>(recV + (which == 0 ? ((2 * G::NW + idx) * G::LPT + G::LPT - 1) : idx * G::LPT) * 16));
-        const uint32_t eL = __ldg(reinterpret_cast<const uint16_t*>(recL + G::BODY + T + 2 * Y));   // neighbour's right edge
-        const uint32_t eR = __ldg(reinterpret_cast<const uint16_t*>(recR + G::BODY + 2 * Y));       // neighbour's left edge
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
             for (int gx = 0; gx < G::NW; ++gx)
                 t.S[cc][gx] = pack16(pack16(0u, v[(2 + cc) * G::NW + gx]), v[cc * G::NW + gx]);
-        const uint32_t b = pack16(0u, hv);
-        item = which == 0 ? (b << 16) : b;
-        t.hL0 = eL & 1u; t.hL1 = (eL >> 8) & 1u;
-        t.hR0 = eR & 1u; t.hR1 = (eR >> 8) & 1u;
     }
-#pragma unroll
-    for (int cc = 0; cc < 2; ++cc)
-#pragma unroll
-        for (int gx = 0; gx < G::NW; ++gx) {
-            t.up[cc][gx] = __shfl_sync(0xffffffffu, item, lane_base + cc * G::NW + gx);
-            t.dn[cc][gx] = __shfl_sync(0xffffffffu, item, lane_base + 2 * G::NW + cc * G::NW + gx);
-        }
+    // halo rows: the first lane of a tile takes BOT of the tile above, the last lane TOP of the tile below
+    uint4 hv = make_uint4(0u, 0u, 0u, 0u);
+    if (Y == 0 || Y == G::LPT - 1)
+        hv = __ldg(reinterpret_cast<const uint4*>(rec_of(row0 + (Y == 0 ? tyU : tyD) * B + utx) + BODY + (Y == 0 ? G::E_BOT : G::E_TOP)));
+    t.vrow[0][0] = hv.x;
+    if (G::NW == 2) { t.vrow[0][1] = hv.y; t.vrow[1][0] = hv.z; t.vrow[1][1] = hv.w; }
+    else t.vrow[1][0] = hv.y;
+    // halo columns: the left tile's right column, the right tile's left column (same address for every lane of a tile)
+    const uint2 cl = __ldg(reinterpret_cast<const uint2*>(rec_of(rowc + txL) + BODY + G::E_COL + 8));   // {R0, R1}
+    const uint2 cr = __ldg(reinterpret_cast<const uint2*>(rec_of(rowc + txR) + BODY + G::E_COL));       // {L0, L1}
+    t.hL0 = (cl.x >> Y) & 1u; t.hL1 = (cl.y >> Y) & 1u;
+    t.hR0 = (cr.x >> Y) & 1u; t.hR1 = (cr.y >> Y) & 1u;
+    (void)lane_base;
 }
 
-// a7: write the lane's block row back (and, int8, the two edge-column bytes of its two rows).
+// a7: write the lane's block row back, and the bit-packed copies of the tile's boundary (see PG).
 template <int T, bool BITS>
-__device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, int ty, int Y, const TileRegs<T>& t,
+__device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, int ty, int Y, int sub, const TileRegs<T>& t,
                                            const uint2* lut) {
     using G = PG<T>;
     constexpr uint32_t REC = BITS ? G::REC_BITS : G::REC_I8;
+    constexpr uint32_t BODY = REC - G::EDGE;
     uint8_t* rec = A.tiles + (uint64_t)(((uint32_t)r * (uint32_t)A.B + (uint32_t)ty) * (uint32_t)A.B + (uint32_t)tx) * REC;
     if (BITS) {
 #pragma unroll
@@ -164,11 +155,20 @@ __device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, in
                     stg128(rec + ((((rp * 2 + cc) * G::NW + gx) * G::LPT) + Y) * 16, make_uint4(a.x, a.y, b.x, b.y));
                 }
             }
-        // x = 0: colour 0 on even rows (bit 0), colour 1 on odd rows (bit 16); x = T-1: colour 1 / colour 0, last pair
-        const uint32_t eL = (t.S[0][0] & 1u) | (((t.S[1][0] >> 16) & 1u) << 8);
-        const uint32_t eR = ((t.S[1][G::NW - 1] >> 15) & 1u) | ((t.S[0][G::NW - 1] >> 31) << 8);
-        *reinterpret_cast<uint16_t*>(rec + G::BODY + 2 * Y) = (uint16_t)eL;
-        *reinterpret_cast<uint16_t*>(rec + G::BODY + T + 2 * Y) = (uint16_t)eR;
+    }
+    // boundary columns: x = 0 is colour 0 on even rows (bit 0) and colour 1 on odd rows (bit 16); x = T-1 is
+    // colour 1 / colour 0, last pair.  One ballot each; a warp holds 64 / T tiles, LPT bits per tile.
+    const uint32_t sh = (uint32_t)sub * G::LPT, m = G::LPT == 32 ? 0xffffffffu : ((1u << G::LPT) - 1u);
+    const uint32_t L0 = (__ballot_sync(0xffffffffu, t.S[0][0] & 1u) >> sh) & m;
+    const uint32_t L1 = (__ballot_sync(0xffffffffu, (t.S[1][0] >> 16) & 1u) >> sh) & m;
+    const uint32_t R0 = (__ballot_sync(0xffffffffu, (t.S[1][G::NW - 1] >> 15) & 1u) >> sh) & m;
+    const uint32_t R1 = (__ballot_sync(0xffffffffu, t.S[0][G::NW - 1] >> 31) >> sh) & m;
+    // first lane: TOP + COL (one sector), last lane: BOT + padding (the other sector)
+    if (Y == 0 || Y == G::LPT - 1) {
+        const uint4 w = G::NW == 2 ? make_uint4(t.S[0][0], t.S[0][1], t.S[1][0], t.S[1][1]) : make_uint4(t.S[0][0], t.S[1][0], 0u, 0u);
+        uint8_t* e = rec + BODY + (Y == 0 ? G::E_TOP : G::E_BOT);
+        stg128(e, w);
+        stg128(e + 16, Y == 0 ? make_uint4(L0, L1, R0, R1) : make_uint4(0u, 0u, 0u, 0u));
     }
 }
 
@@ -242,8 +242,8 @@ __device__ __forceinline__ void half_sweep(const PlaneArgs& A, TileRegs<T>& t, c
         } else {
             Oup = __shfl_up_sync(0xffffffffu, O[gx], 1);
             Odn = __shfl_down_sync(0xffffffffu, O[gx], 1);
-            if (Y == 0) Oup = t.up[o][gx];
-            if (Y == G::LPT - 1) Odn = t.dn[o][gx];
+            if (Y == 0) Oup = t.vrow[o][gx];
+            if (Y == G::LPT - 1) Odn = t.vrow[o][gx];
         }
         const uint32_t V1 = __byte_perm(O[gx], O[gx], 0x1032);        // the other row of the same block
         const uint32_t V2 = __byte_perm(Oup, Odn, 0x5432);            // row above the block | row below the block
@@ -303,7 +303,7 @@ __global__ void __launch_bounds__(kPlaneThreads) k_tile_planes(PlaneArgs A) {
         half_sweep<T, HASJ>(A, t, Jw, 0, Y, g0, p0, 2 * tt, k0, k1);
         half_sweep<T, HASJ>(A, t, Jw, 1, Y, g0, p0, 2 * tt + 1, k0, k1);
     }
-    store_tile<T, BITS>(A, r, tx, ty, Y, t, lut);
+    store_tile<T, BITS>(A, r, tx, ty, Y, sub, t, lut);
 }
 
 // a8: plain checkerboard of a 64x64 lattice (tile = L = 64, BASELINE config 1).  One warp holds a whole
@@ -361,12 +361,12 @@ __global__ void __launch_bounds__(32) k_plain64_planes(PlaneArgs A, int n, long 
             }
         }
     }
-    store_tile<T, BITS>(A, r, 0, 0, Y, t, lut);
+    store_tile<T, BITS>(A, r, 0, 0, Y, 0, t, lut);
 }
 
 // ---- layout converters (a11): canonical int8 +-1 <-> tile records; not on the timed path ----
 // One thread per site; MODE 0: canonical -> int8 records, 1: int8 records -> canonical,
-// 2: canonical -> bit records (atomicOr into zeroed storage), 3: bit records -> canonical.
+// 2: canonical -> bit records, 3: bit records -> canonical.  Bit fields are set by atomicOr into zeroed storage.
 template <int MODE>
 __global__ void k_convert_planes(int8_t* __restrict__ canon, uint8_t* __restrict__ tiles, int L, int T, int R) {
     const uint64_t N = (uint64_t)L * L;
@@ -379,26 +379,23 @@ __global__ void k_convert_planes(int8_t* __restrict__ canon, uint8_t* __restrict
     const int tx = x / T, ty = y / T, lx = x - tx * T, ly = y - ty * T;
     const int cc = (lx + ly) & 1, px = lx >> 1, gx = px >> 4, kk = px & 15, rp = ly & 1, Y = ly >> 1;
     const size_t tile = ((size_t)r * B + ty) * B + tx;
-    if (MODE < 2) {
-        uint8_t* rec = tiles + tile * (size_t)(T * T + 2 * T);
-        uint8_t* body = rec + ((((rp * 2 + cc) * NW + gx) * LPT) + Y) * 16 + kk;
-        if (MODE == 0) {
-            const uint8_t v = canon[gid] > 0 ? 1 : 0;
-            *body = v;
-            if (lx == 0) rec[T * T + ly] = v;
-            if (lx == T - 1) rec[T * T + T + ly] = v;
-        } else {
-            canon[gid] = *body ? 1 : -1;
-        }
-    } else {
-        uint32_t* w = reinterpret_cast<uint32_t*>(tiles + tile * (size_t)(T * T / 8)) + ((cc * NW + gx) * LPT + Y);
-        const int j = rp * 16 + kk;
-        if (MODE == 2) {
-            if (canon[gid] > 0) atomicOr(w, 1u << j);
-        } else {
-            canon[gid] = ((*w >> j) & 1u) ? 1 : -1;
-        }
-    }
+    constexpr bool BITS = MODE >= 2;
+    const size_t body_bytes = BITS ? (size_t)(T * T / 8) : (size_t)(T * T);
+    uint8_t* rec = tiles + tile * (body_bytes + 64);
+    uint8_t* body = rec + ((((rp * 2 + cc) * NW + gx) * LPT) + Y) * 16 + kk;
+    uint32_t* w = reinterpret_cast<uint32_t*>(rec) + ((cc * NW + gx) * LPT + Y);
+    const int j = rp * 16 + kk;
+    if (MODE == 1) { canon[gid] = *body ? 1 : -1; return; }
+    if (MODE == 3) { canon[gid] = ((*w >> j) & 1u) ? 1 : -1; return; }
+    const bool up = canon[gid] > 0;
+    if (!BITS) *body = up ? 1 : 0;
+    if (!up) return;
+    if (BITS) atomicOr(w, 1u << j);
+    uint32_t* e = reinterpret_cast<uint32_t*>(rec + body_bytes);          // boundary copies (zeroed first), see PG
+    if (Y == 0) atomicOr(e + 0 + cc * NW + gx, 1u << j);                  // TOP: words of block row 0
+    if (Y == LPT - 1) atomicOr(e + 8 + cc * NW + gx, 1u << j);            // BOT: words of block row LPT-1
+    if (lx == 0) atomicOr(e + 4 + rp, 1u << Y);                           // COL: L0, L1
+    if (lx == T - 1) atomicOr(e + 6 + rp, 1u << Y);                       //      R0, R1
 }
 
 // Couplings, canonical J[d][i] (bond i -> i + e_d) -> coupling records (zeroed first).  One thread per site:
@@ -465,15 +462,15 @@ int launch_convert_couplings(ising_ctx* h, int T, void* d_jrec) {
 
 size_t tile_planes_bytes(const ising_ctx* h, int T, bool bits) {
     const size_t B = (size_t)(h->L / T);
-    return (size_t)h->R * B * B * (size_t)(bits ? T * T / 8 : T * T + 2 * T);
+    return (size_t)h->R * B * B * (size_t)((bits ? T * T / 8 : T * T) + 64);
 }
 
 int launch_canon_to_planes(ising_ctx* h, int T, bool bits, const int8_t* d_canon, void* d_tiles) {
     const uint64_t total = h->N * (uint64_t)h->R;
     const unsigned blocks = (unsigned)((total + 255) / 256);
     cudaStream_t st = hooks().stream;
+    ISING_CUDA_OK(cudaMemsetAsync(d_tiles, 0, tile_planes_bytes(h, T, bits), st));
     if (bits) {
-        ISING_CUDA_OK(cudaMemsetAsync(d_tiles, 0, tile_planes_bytes(h, T, true), st));
         k_convert_planes<2><<<blocks, 256, 0, st>>>(const_cast<int8_t*>(d_canon), (uint8_t*)d_tiles, h->L, T, h->R);
     } else {
         k_convert_planes<0><<<blocks, 256, 0, st>>>(const_cast<int8_t*>(d_canon), (uint8_t*)d_tiles, h->L, T, h->R);
