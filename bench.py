@@ -134,6 +134,30 @@ def run_reference(a, rank: int, world: int) -> None:
     print(json.dumps(line), flush=True)
 
 
+def aggregate_replicas(ms_local: float, world: int, steps: int, k: int, L: int, dist=None, device="cpu"):
+    """'Replicas only': every rank ran the same independent workload; the job's time is the MAX
+    over ranks and the job's work is the sum.  Returns (ms, flips_per_ns)."""
+    ms = ms_local
+    if dist is not None:
+        import torch
+        t = torch.tensor([ms_local], device=device, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms = float(t.item())
+    return ms, world * steps * k * L * L / (ms * 1e6)
+
+
+def selftest_ranks(rank: int, world: int) -> None:
+    """CPU check of the multi-rank plumbing (gloo, no GPU): rank r pretends to have taken (1 + r) ms."""
+    import torch.distributed as dist
+    dist.init_process_group("gloo")
+    dist.barrier()
+    ms, value = aggregate_replicas(1.0 + rank, world, steps=2, k=1, L=1000, dist=dist)
+    assert ms == float(world), (ms, world)
+    if rank == 0:
+        print(json.dumps({"selftest": "ranks", "n_gpus": world, "ms": ms, "value": value, "scaling": "weak"}), flush=True)
+    dist.destroy_process_group()
+
+
 def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng="planes"):
     """Device-timed throughput of one (rng, layout, tile, k) variant; returns dict."""
     g = P.Ising(2, L, seed=3, rng=rng)
@@ -199,11 +223,15 @@ def main() -> None:
     ap.add_argument("--rng", default="planes", choices=["planes", "words"], help="RNG->site mapping (DESIGN.md R6)")
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the k/tile table")
+    ap.add_argument("--selftest-ranks", action="store_true", help="CPU/gloo check of the multi-rank aggregation, no GPU")
     a = ap.parse_args()
     a.warmup = max(a.warmup, 3) if a.impl == "ours" else a.warmup
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
+    if a.selftest_ranks:
+        selftest_ranks(rank, world)
+        return
     if a.impl == "reference":
         run_reference(a, rank, world)
         return
@@ -229,13 +257,7 @@ def main() -> None:
     sampler = ClockSampler(local) if rank == 0 else None
     res = time_variant(P, torch, L, a.layout, a.tile, a.k, a.steps, a.warmup, sampler, a.rng)
     barrier()
-    ms = res["ms"]
-    if dist is not None:
-        t = torch.tensor([ms], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms = float(t.item())
-    flips = world * a.steps * a.k * L * L
-    value = flips / (ms * 1e6)
+    ms, value = aggregate_replicas(res["ms"], world, a.steps, a.k, L, dist, "cuda")
 
     peak, peak_src, sm_max = measured_peaks()
     ncu = NCU.get((a.rng, a.layout, a.tile, a.k)) if L == 16384 else None
