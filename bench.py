@@ -211,10 +211,50 @@ def time_e2e(P, torch, L, layout, tile, k, steps, rng="planes"):
             "d2h_bytes_per_step": L * L, "steps": steps}
 
 
+def run_lscan(P, torch, a) -> None:
+    """flips/ns against L in the style of the paper's Fig. 3, planes mapping, int8 records."""
+    rows = []
+    for L in (64, 128, 256, 512, 1024, 2048, 4096, 8192, 16384):
+        for T in (32, 64):
+            if L % T or (L // T) % 2:
+                continue
+            for k in (1, 4, 16):
+                n = max(4, min(2000, int(2e10 / (k * L * L))))
+                r = time_variant(P, torch, L, "int8", T, k, n, 3, None, "planes")
+                rows.append({"L": L, "tile": T, "k": k, "passes": n, "flips_per_ns": round(r["flips_per_ns"], 2),
+                             "us_per_pass": round(1e3 * r["ms"] / n, 2), "path": r["path"]})
+    print(json.dumps({"study": "lscan", "unit": UNIT, "rows": rows}), flush=True)
+
+
+def run_autocorr(P, torch, a) -> None:
+    """what multi-hit costs in autocorrelation.  L=128 at beta_c, tile 32, 4e5 passes after
+    2e4 of thermalisation; tau_int of E and |M| in outer passes; independent samples per second of GPU time."""
+    from paper_1006_3865_b200.analysis import independent_samples_per_second, tau_int
+    L, T, n = 128, 32, 400000
+    rows = []
+    for k in (1, 2, 4, 8, 16):
+        g = P.Ising(2, L, seed=11)
+        g.sweep(W.BETA_C_2D, 20000, T, k)
+        E = torch.zeros(n, dtype=torch.int64, device="cuda")
+        M = torch.zeros(n, dtype=torch.int64, device="cuda")
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        g.sweep_series(W.BETA_C_2D, n, T, k, E=E, M=M)
+        torch.cuda.synchronize()
+        dt = time.perf_counter() - t0
+        tE, _ = tau_int(E.cpu().numpy())
+        tM, _ = tau_int(np.abs(M.cpu().numpy()))
+        rows.append({"k": k, "tau_E_passes": round(tE, 2), "tau_absM_passes": round(tM, 2),
+                     "tau_absM_inner_sweeps": round(tM * k, 2), "seconds": round(dt, 2),
+                     "indep_samples_per_s_absM": round(independent_samples_per_second(n, dt, tM), 1)})
+        g.destroy()
+    print(json.dumps({"study": "autocorr", "L": L, "tile": T, "beta": W.BETA_C_2D, "passes": n, "rows": rows}), flush=True)
+
+
 def main() -> None:
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=50)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--layout", default="int8", choices=["int8", "bits"])
@@ -223,6 +263,8 @@ def main() -> None:
     ap.add_argument("--rng", default="planes", choices=["planes", "words"], help="RNG->site mapping (DESIGN.md R6)")
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the k/tile table")
+    ap.add_argument("--lscan", action="store_true", help="study: flips/ns against L (SURVEY 8(f)-3)")
+    ap.add_argument("--autocorr", action="store_true", help="study: autocorrelation time against k (SURVEY 8(f)-2)")
     ap.add_argument("--selftest-ranks", action="store_true", help="CPU/gloo check of the multi-rank aggregation, no GPU")
     a = ap.parse_args()
     a.warmup = max(a.warmup, 3) if a.impl == "ours" else a.warmup
@@ -247,6 +289,9 @@ def main() -> None:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     P.use_torch()
     L = a.L
+    if a.lscan or a.autocorr:
+        (run_lscan if a.lscan else run_autocorr)(P, torch, a)
+        return
 
     def barrier():
         if dist is not None:
