@@ -146,6 +146,16 @@ static int ensure_store(ising_ctx* h, Store kind, int T) {
     return 0;
 }
 
+// a10 wherever the spins currently live: directly on 2D plane records, else on the canonical array.
+static int observables_now(ising_ctx* h, long long* d_E, long long* d_M) {
+    const bool planes2d = (h->store == Store::PlaneI8 || h->store == Store::PlaneBits) && h->L / h->store_tile >= 2 &&
+                          (!h->has_J || h->Jtiles_tile == h->store_tile);
+    if (planes2d) return launch_observables_planes(h, h->store_tile, h->store == Store::PlaneBits, d_E, d_M);
+    int rc = (h->store == Store::Canon) ? 0 : to_canon_scratch(h);
+    if (rc) return rc;
+    return launch_observables_canon(h, h->d_canon, d_E, d_M);
+}
+
 static const int8_t* canon_view(ising_ctx* h, int* rc) {
     *rc = (h->store == Store::Canon) ? 0 : to_canon_scratch(h);
     return h->d_canon;
@@ -328,11 +338,8 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             rc = use_tile_i8 ? launch_tile_i8_pass(h, acc, T, k, t0)
                  : use_3d ? launch_tile3d_pass(h, acc, bits, k, t0)
                           : launch_tile_planes_pass(h, acc, T, bits, k, t0);
-            if (!rc && want_series) {
-                rc = to_canon_scratch(h);
-                if (!rc) rc = launch_observables_canon(h, h->d_canon, d_E ? d_E + (size_t)pass * h->R : nullptr,
-                                                       d_M ? d_M + (size_t)pass * h->R : nullptr);
-            }
+            if (!rc && want_series)
+                rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);
         }
     } else if (h->layout == ISING_LAYOUT_I8 || h->force_generic) {
         h->last_path = "generic";
@@ -364,10 +371,7 @@ int ising_sweep_series(ising_handle h, double beta, int n_sweeps, int tile, int 
 
 int ising_observables(ising_handle h, int64_t* E, int64_t* M) {
     if (!h) { set_error("ising_observables: NULL handle"); return ISING_EINVAL; }
-    int rc = 0;
-    const int8_t* s = canon_view(h, &rc);
-    if (rc) return rc;
-    rc = launch_observables_canon(h, s, h->d_obs, h->d_obs + h->R);
+    int rc = observables_now(h, h->d_obs, h->d_obs + h->R);
     if (rc) return rc;
     if (E) { rc = copy_out(E, h->d_obs, sizeof(long long) * h->R, nullptr); if (rc) return rc; }
     if (M) { rc = copy_out(M, h->d_obs + h->R, sizeof(long long) * h->R, nullptr); if (rc) return rc; }

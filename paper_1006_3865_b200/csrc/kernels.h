@@ -29,6 +29,7 @@ size_t coupling_record_bytes(const ising_ctx* h);
 int launch_convert_couplings(ising_ctx* h, int T, void* d_jrec);
 bool plain64_supported(const ising_ctx* h, int T);
 int launch_plain64(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M);
+int launch_observables_planes(ising_ctx* h, int T, bool bits, long long* d_E, long long* d_M);
 int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, int k, uint64_t t_first);
 
 // ---- tile3d_planes.cu: 3D multi-spin tile kernel, 8x8x8 tiles (RNG mapping "planes") ----------

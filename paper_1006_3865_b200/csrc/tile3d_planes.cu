@@ -208,11 +208,13 @@ __device__ __forceinline__ void half_sweep3(const Plane3Args& A, Slice& s, int c
     s.S[c] = S ^ flip;
 }
 
+constexpr int kThreads3 = 64;        // 2 warps = 8 tiles per CTA: small CTAs so that config 4 (4096 warp jobs) fits one wave
+
 template <bool BITS>
-__global__ void __launch_bounds__(128) k_tile3d_planes(Plane3Args A) {
+__global__ void __launch_bounds__(kThreads3) k_tile3d_planes(Plane3Args A) {
     __shared__ uint2 lut[BITS ? 1 : 256];
     if (!BITS) {
-        build_byte_lut<128>(lut);
+        build_byte_lut<kThreads3>(lut);
         __syncthreads();
     }
     const int lane = threadIdx.x & 31;
@@ -321,7 +323,7 @@ int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64
         A.tail[m] = acc.thr[m] & ((1u << kTailBits) - 1u);
     }
     A.force = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
-    const int warps = 4;
+    const int warps = kThreads3 / 32;
     const uint32_t grid = (A.njobs + warps - 1) / warps;
     for (int C = 0; C < 2; ++C) {
         A.C = C;

@@ -222,48 +222,74 @@ __device__ __forceinline__ uint32_t update_block(const PlaneArgs& A, uint32_t S,
 }
 
 // a5-a6: one half-sweep of colour c on the lane's block row; o = 1 - c is read, c is written.
-// PERIODIC: the tile is the whole lattice (T = L, the plain checkerboard of P:62): "halos" are the tile's own,
-// live, opposite edges.
+// The four neighbour words of the lane's block (c, gx): V1 = other row of the block, V2 = the rows outside it
+// (shuffle; halo rows on the tile's first / last lane), H1 = same pairs, H2 = pairs shifted by one with carries
+// from the adjacent block or the halo column.  PERIODIC: the tile is the whole lattice (T = L, the plain
+// checkerboard of P:62): "halos" are the tile's own, live, opposite edges.
+template <int T, bool PERIODIC>
+__device__ __forceinline__ void neighbour_words(const TileRegs<T>& t, int c, int gx, int Y, uint32_t& V1, uint32_t& V2,
+                                                uint32_t& H1, uint32_t& H2) {
+    using G = PG<T>;
+    const int o = 1 - c;
+    const uint32_t O = t.S[o][gx], Ol = t.S[o][(gx + G::NW - 1) % G::NW], Or = t.S[o][(gx + 1) % G::NW];
+    uint32_t Oup, Odn;
+    if (PERIODIC) {
+        Oup = __shfl_sync(0xffffffffu, O, (Y + G::LPT - 1) % G::LPT);
+        Odn = __shfl_sync(0xffffffffu, O, (Y + 1) % G::LPT);
+    } else {
+        Oup = __shfl_up_sync(0xffffffffu, O, 1);
+        Odn = __shfl_down_sync(0xffffffffu, O, 1);
+        if (Y == 0) Oup = t.vrow[o][gx];
+        if (Y == G::LPT - 1) Odn = t.vrow[o][gx];
+    }
+    V1 = __byte_perm(O, O, 0x1032);               // the other row of the same block
+    V2 = __byte_perm(Oup, Odn, 0x5432);           // row above the block | row below the block
+    H1 = O;
+    // pair-shifted word: colour 0: even rows look at pair j-1 (carry from the left), odd rows at j+1;
+    // colour 1: even rows j+1, odd rows j-1.
+    if (c == 0) {
+        const uint32_t cl = (gx == 0 && !PERIODIC) ? t.hL0 : ((Ol >> 15) & 1u);
+        const uint32_t cr = (gx == G::NW - 1 && !PERIODIC) ? t.hR1 : ((Or >> 16) & 1u);
+        H2 = ((O << 1) & 0x0000fffeu) | cl | ((O >> 1) & 0x7fff0000u) | (cr << 31);
+    } else {
+        const uint32_t cr = (gx == G::NW - 1 && !PERIODIC) ? t.hR0 : (Or & 1u);
+        const uint32_t cl = (gx == 0 && !PERIODIC) ? t.hL1 : (Ol >> 31);
+        H2 = ((O >> 1) & 0x00007fffu) | (cr << 15) | ((O << 1) & 0xfffe0000u) | (cl << 16);
+    }
+}
+
+// a5-a6: one half-sweep of colour c on the lane's block row; o = 1 - c is read, c is written.
 template <int T, bool HASJ, bool PERIODIC = false>
 __device__ __forceinline__ void half_sweep(const PlaneArgs& A, TileRegs<T>& t, const uint4 (&Jw)[2][PG<T>::NW], int c, int Y,
                                            uint32_t g0, uint32_t p0, uint64_t H, uint32_t k0, uint32_t k1) {
     using G = PG<T>;
-    const int o = 1 - c;
     const uint32_t Hlo = (uint32_t)H, Hhi = (uint32_t)(H >> 32);
-    uint32_t O[G::NW], Snew[G::NW];
-#pragma unroll
-    for (int gx = 0; gx < G::NW; ++gx) O[gx] = t.S[o][gx];
+    uint32_t Snew[G::NW];
 #pragma unroll
     for (int gx = 0; gx < G::NW; ++gx) {
-        uint32_t Oup, Odn;
-        if (PERIODIC) {
-            Oup = __shfl_sync(0xffffffffu, O[gx], (Y + G::LPT - 1) % G::LPT);
-            Odn = __shfl_sync(0xffffffffu, O[gx], (Y + 1) % G::LPT);
-        } else {
-            Oup = __shfl_up_sync(0xffffffffu, O[gx], 1);
-            Odn = __shfl_down_sync(0xffffffffu, O[gx], 1);
-            if (Y == 0) Oup = t.vrow[o][gx];
-            if (Y == G::LPT - 1) Odn = t.vrow[o][gx];
-        }
-        const uint32_t V1 = __byte_perm(O[gx], O[gx], 0x1032);        // the other row of the same block
-        const uint32_t V2 = __byte_perm(Oup, Odn, 0x5432);            // row above the block | row below the block
-        // pair-shifted word: colour 0: even rows look at pair j-1 (carry from the left), odd rows at j+1;
-        // colour 1: even rows j+1, odd rows j-1.
-        uint32_t H2;
-        if (c == 0) {
-            const uint32_t cl = (gx == 0 && !PERIODIC) ? t.hL0 : ((O[(gx + G::NW - 1) % G::NW] >> 15) & 1u);
-            const uint32_t cr = (gx == G::NW - 1 && !PERIODIC) ? t.hR1 : ((O[(gx + 1) % G::NW] >> 16) & 1u);
-            H2 = ((O[gx] << 1) & 0x0000fffeu) | cl | ((O[gx] >> 1) & 0x7fff0000u) | (cr << 31);
-        } else {
-            const uint32_t cr = (gx == G::NW - 1 && !PERIODIC) ? t.hR0 : (O[(gx + 1) % G::NW] & 1u);
-            const uint32_t cl = (gx == 0 && !PERIODIC) ? t.hL1 : (O[(gx + G::NW - 1) % G::NW] >> 31);
-            H2 = ((O[gx] >> 1) & 0x00007fffu) | (cr << 15) | ((O[gx] << 1) & 0xfffe0000u) | (cl << 16);
-        }
-        Snew[gx] = update_block<HASJ>(A, t.S[c][gx], V1, V2, O[gx], H2, Jw[c][gx], g0 + (uint32_t)gx,
+        uint32_t V1, V2, H1, H2;
+        neighbour_words<T, PERIODIC>(t, c, gx, Y, V1, V2, H1, H2);
+        Snew[gx] = update_block<HASJ>(A, t.S[c][gx], V1, V2, H1, H2, Jw[c][gx], g0 + (uint32_t)gx,
                                       p0 + 16u * (uint32_t)gx, Hlo, Hhi, k0, k1);
     }
 #pragma unroll
     for (int gx = 0; gx < G::NW; ++gx) t.S[c][gx] = Snew[gx];
+}
+
+// a10 on a tile held in registers: #up spins and #unsatisfied bonds of the lane's block row, every bond of the
+// tile's colour-0 sites (each bond of the lattice has exactly one colour-0 end).  M = 2 #up - N, E = 2 #unsat - 2N.
+template <int T, bool PERIODIC>
+__device__ __forceinline__ void count_row(const TileRegs<T>& t, const uint4 (&Jw)[2][PG<T>::NW], int Y, int& up, int& unsat) {
+    using G = PG<T>;
+#pragma unroll
+    for (int gx = 0; gx < G::NW; ++gx) {
+        uint32_t V1, V2, H1, H2;
+        neighbour_words<T, PERIODIC>(t, 0, gx, Y, V1, V2, H1, H2);
+        const uint32_t S = t.S[0][gx];
+        const uint4 Jc = Jw[0][gx];
+        unsat += __popc(S ^ V1 ^ Jc.x) + __popc(S ^ V2 ^ Jc.y) + __popc(S ^ H1 ^ Jc.z) + __popc(S ^ H2 ^ Jc.w);
+        up += __popc(S) + __popc(t.S[1][gx]);
+    }
 }
 
 constexpr int kPlaneThreads = 128;      // 4 warps = 4 jobs per CTA
@@ -338,18 +364,7 @@ __global__ void __launch_bounds__(32) k_plain64_planes(PlaneArgs A, int n, long 
         }
         if (E || M) {
             int up = 0, unsat = 0;
-#pragma unroll
-            for (int gx = 0; gx < G::NW; ++gx) {
-                const uint32_t S = t.S[0][gx], O = t.S[1][gx];
-                const uint32_t Oup = __shfl_sync(0xffffffffu, O, (Y + G::LPT - 1) % G::LPT);
-                const uint32_t Odn = __shfl_sync(0xffffffffu, O, (Y + 1) % G::LPT);
-                const uint32_t V1 = __byte_perm(O, O, 0x1032), V2 = __byte_perm(Oup, Odn, 0x5432);
-                const uint32_t cl = (t.S[1][(gx + G::NW - 1) % G::NW] >> 15) & 1u, cr = (t.S[1][(gx + 1) % G::NW] >> 16) & 1u;
-                const uint32_t H2 = ((O << 1) & 0x0000fffeu) | cl | ((O >> 1) & 0x7fff0000u) | (cr << 31);
-                const uint4 Jc = Jw[0][gx];
-                unsat += __popc(S ^ V1 ^ Jc.x) + __popc(S ^ V2 ^ Jc.y) + __popc(S ^ O ^ Jc.z) + __popc(S ^ H2 ^ Jc.w);
-                up += __popc(S) + __popc(O);
-            }
+            count_row<T, true>(t, Jw, Y, up, unsat);
 #pragma unroll
             for (int d = 16; d > 0; d >>= 1) {
                 up += __shfl_xor_sync(0xffffffffu, up, d);
@@ -362,6 +377,39 @@ __global__ void __launch_bounds__(32) k_plain64_planes(PlaneArgs A, int n, long 
         }
     }
     store_tile<T, BITS>(A, r, 0, 0, Y, 0, t, lut);
+}
+
+// a10 directly on the tile records (no conversion to the canonical array): one launch per coarse colour C adds
+// the colour-C tiles' share to E[r], M[r] (zeroed by the caller): warp shuffle reduction, two 64-bit atomics per tile.
+template <int T, bool BITS, bool HASJ>
+__global__ void __launch_bounds__(kPlaneThreads) k_observables_planes(PlaneArgs A, long long* __restrict__ E, long long* __restrict__ M) {
+    using G = PG<T>;
+    const int lane = threadIdx.x & 31;
+    const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (job >= A.njobs) return;
+    const int sub = lane / G::LPT, Y = lane % G::LPT;
+    int r, tx, ty;
+    job_tile<T>(A, job, sub, r, tx, ty);
+    TileRegs<T> t;
+    load_tile<T, BITS>(A, r, tx, ty, Y, sub * G::LPT, t);
+    uint4 Jw[2][G::NW];
+#pragma unroll
+    for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+        for (int gx = 0; gx < G::NW; ++gx)
+            Jw[cc][gx] = HASJ ? __ldg(A.jrec + ((size_t)ty * A.B + tx) * (2 * G::NW * G::LPT) + (cc * G::NW + gx) * G::LPT + Y)
+                              : make_uint4(0u, 0u, 0u, 0u);
+    int up = 0, unsat = 0;
+    count_row<T, false>(t, Jw, Y, up, unsat);
+#pragma unroll
+    for (int d = G::LPT / 2; d > 0; d >>= 1) {           // reduce over the lanes of one tile
+        up += __shfl_xor_sync(0xffffffffu, up, d);
+        unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+    }
+    if (Y == 0) {
+        if (M) atomicAdd(reinterpret_cast<unsigned long long*>(M + r), (unsigned long long)(2ll * up - (long long)(T * T)));
+        if (E) atomicAdd(reinterpret_cast<unsigned long long*>(E + r), (unsigned long long)(2ll * unsat - 2ll * (T * T)));
+    }
 }
 
 // ---- layout converters (a11): canonical int8 +-1 <-> tile records; not on the timed path ----
@@ -521,6 +569,38 @@ int launch_plain64(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uin
         else k_plain64_planes<false, false><<<h->R, 32, 0, st>>>(A, n, d_E, d_M);
     }
     count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+// a10 on tile records: E[r], M[r] (R values each, either may be null) of the state held in plane records.
+int launch_observables_planes(ising_ctx* h, int T, bool bits, long long* d_E, long long* d_M) {
+    cudaStream_t st = hooks().stream;
+    if (d_E) ISING_CUDA_OK(cudaMemsetAsync(d_E, 0, sizeof(long long) * h->R, st));
+    if (d_M) ISING_CUDA_OK(cudaMemsetAsync(d_M, 0, sizeof(long long) * h->R, st));
+    PlaneArgs A = {};
+    A.tiles = (uint8_t*)h->d_tiles;
+    A.seeds = h->d_seeds;
+    A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = 0; A.t_first = 0;
+    A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
+    const uint32_t tiles_per_colour = (uint32_t)((size_t)h->R * A.B * A.B / 2);
+    A.njobs = tiles_per_colour / (uint32_t)(64 / T);
+    A.magic_rep = fastdiv_magic((uint32_t)A.B * (uint32_t)A.B / 2u);
+    A.magic_hb = fastdiv_magic((uint32_t)A.B / 2u);
+    const int warps = kPlaneThreads / 32;
+    const uint32_t grid = (A.njobs + warps - 1) / warps;
+    for (int C = 0; C < 2; ++C) {
+        A.C = C;
+#define ISING_OBS(TT, BB)                                                                                   \
+        do {                                                                                                \
+            if (A.jrec) k_observables_planes<TT, BB, true><<<grid, warps * 32, 0, st>>>(A, d_E, d_M);      \
+            else k_observables_planes<TT, BB, false><<<grid, warps * 32, 0, st>>>(A, d_E, d_M);            \
+        } while (0)
+        if (T == 64) { if (bits) ISING_OBS(64, true); else ISING_OBS(64, false); }
+        else { if (bits) ISING_OBS(32, true); else ISING_OBS(32, false); }
+#undef ISING_OBS
+        count_launch();
+    }
     ISING_CUDA_OK(cudaGetLastError());
     return 0;
 }
