@@ -479,7 +479,8 @@ int launch_colour_planes(const PlaneArgs& A) {
     cfg.gridDim = dim3(grid); cfg.blockDim = dim3(warps * 32); cfg.dynamicSmemBytes = 0; cfg.stream = hooks().stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    static const int pdl = getenv("ISING_NO_PDL") ? 0 : 1;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl;
     cfg.attrs = attr; cfg.numAttrs = 1;
     if (A.jrec) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes<T, BITS, true>, A));
     else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes<T, BITS, false>, A));
