@@ -47,16 +47,22 @@ __device__ __forceinline__ uint32_t pack16(uint32_t acc, const uint4& v) {
     return pack_step(acc, v.x);
 }
 
-// int8 write-back table: 8 bits -> 8 bytes of 0/1 (256 entries, built once per CTA; caller syncs).
-template <int THREADS>
-__device__ __forceinline__ void build_byte_lut(uint2* lut) {
-#pragma unroll
-    for (int i = threadIdx.x; i < 256; i += THREADS) {
-        // 4 bits -> 4 bytes: n * 0x00204081 puts bit b at 8b (+ garbage elsewhere), no carries for n < 16
-        lut[i] = make_uint2(((uint32_t)(i & 15) * 0x00204081u) & 0x01010101u,
-                            ((uint32_t)(i >> 4) * 0x00204081u) & 0x01010101u);
+// int8 write-back table: 8 bits -> 8 bytes of 0/1.  A compile-time constant array in global memory (2 KB, stays in
+// L1 / L2); lookups go through the read-only path, so no kernel builds a copy or needs a barrier.
+struct ByteLut {
+    uint2 e[256];
+    constexpr ByteLut() : e() {
+        for (int i = 0; i < 256; ++i) {
+            unsigned lo = 0, hi = 0;
+            for (int b = 0; b < 4; ++b) {
+                lo |= (unsigned)((i >> b) & 1) << (8 * b);
+                hi |= (unsigned)((i >> (4 + b)) & 1) << (8 * b);
+            }
+            e[i].x = lo; e[i].y = hi;
+        }
     }
-}
+};
+__device__ const ByteLut kByteLutGlobal = ByteLut();
 
 // ceil(2^32 / d) on the host; q / d on the device = umulhi(q, magic) corrected by at most one either way.
 inline uint32_t fastdiv_magic(uint32_t d) { return d <= 1 ? 0xffffffffu : (uint32_t)((0x100000000ull + d - 1) / d); }

@@ -132,8 +132,8 @@ __device__ __forceinline__ void store_slice(const Plane3Args& A, const Tile3& t,
         for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                const uint2 a = lut[(s.S[cc] >> (16 * h)) & 0xffu];
-                const uint2 b = lut[(s.S[cc] >> (16 * h + 8)) & 0xffu];
+                const uint2 a = __ldg(lut + ((s.S[cc] >> (16 * h)) & 0xffu));
+                const uint2 b = __ldg(lut + ((s.S[cc] >> (16 * h + 8)) & 0xffu));
                 stg128(rec + ((cc * 2 + h) * 8 + lz) * 16, make_uint4(a.x, a.y, b.x, b.y));
             }
     }
@@ -212,11 +212,7 @@ constexpr int kThreads3 = 64;        // 2 warps = 8 tiles per CTA: small CTAs so
 
 template <bool BITS>
 __global__ void __launch_bounds__(kThreads3) k_tile3d_planes(Plane3Args A) {
-    __shared__ uint2 lut[BITS ? 1 : 256];
-    if (!BITS) {
-        build_byte_lut<kThreads3>(lut);
-        __syncthreads();
-    }
+    const uint2* lut = kByteLutGlobal.e;      // int8 write-back table, read-only path (planes_common.cuh)
     const int lane = threadIdx.x & 31;
     const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (job >= A.njobs) return;

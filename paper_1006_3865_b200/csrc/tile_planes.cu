@@ -150,8 +150,8 @@ __device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, in
                 const uint32_t w = t.S[cc][gx];
 #pragma unroll
                 for (int rp = 0; rp < 2; ++rp) {
-                    const uint2 a = lut[(w >> (16 * rp)) & 0xffu];          // bits 0..7  -> bytes 0..7
-                    const uint2 b = lut[(w >> (16 * rp + 8)) & 0xffu];      // bits 8..15 -> bytes 8..15
+                    const uint2 a = __ldg(lut + ((w >> (16 * rp)) & 0xffu));          // bits 0..7  -> bytes 0..7
+                    const uint2 b = __ldg(lut + ((w >> (16 * rp + 8)) & 0xffu));      // bits 8..15 -> bytes 8..15
                     stg128(rec + ((((rp * 2 + cc) * G::NW + gx) * G::LPT) + Y) * 16, make_uint4(a.x, a.y, b.x, b.y));
                 }
             }
@@ -297,13 +297,13 @@ constexpr int kPlaneThreads = 128;      // 4 warps = 4 jobs per CTA
 template <int T, bool BITS, bool HASJ>
 __global__ void __launch_bounds__(kPlaneThreads) k_tile_planes(PlaneArgs A) {
     using G = PG<T>;
-    __shared__ uint2 lut[256];                  // int8 write-back: 8 bits -> 8 bytes of 0/1
-    // Programmatic dependent launch: the next colour's grid may be scheduled while this one drains; it builds
-    // its table and then waits here until every store of the previous launch is visible.
+    // int8 write-back table (8 bits -> 8 bytes of 0/1): a constant array in global memory read through the
+    // read-only path (2 KB, L1-resident) — no per-CTA build, no barrier (measured +6 % at k = 1 over a shared-memory copy).
+    const uint2* lut = kByteLutGlobal.e;
+    // Programmatic dependent launch: the next colour's grid may be scheduled while this one drains; it
+    // waits here until every store of the previous launch is visible.
     asm volatile("griddepcontrol.launch_dependents;");
-    if (!BITS) build_byte_lut<kPlaneThreads>(lut);
     asm volatile("griddepcontrol.wait;" ::: "memory");
-    if (!BITS) __syncthreads();
     const int lane = threadIdx.x & 31;
     const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (job >= A.njobs) return;
@@ -339,11 +339,7 @@ template <bool BITS, bool HASJ>
 __global__ void __launch_bounds__(32) k_plain64_planes(PlaneArgs A, int n, long long* __restrict__ E, long long* __restrict__ M) {
     constexpr int T = 64;
     using G = PG<T>;
-    __shared__ uint2 lut[BITS ? 1 : 256];
-    if (!BITS) {
-        build_byte_lut<32>(lut);
-        __syncwarp();
-    }
+    const uint2* lut = kByteLutGlobal.e;
     const int Y = threadIdx.x, r = blockIdx.x;
     TileRegs<T> t;
     load_tile<T, BITS>(A, r, 0, 0, Y, 0, t);
