@@ -35,16 +35,20 @@ __device__ __forceinline__ void stg128(void* p, uint4 v) {
     asm volatile("st.global.v4.u32 [%4], {%0,%1,%2,%3};" ::"r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(p) : "memory");
 }
 
-// 4 bytes of 0/1 -> 4 bits in the top nibble: b0 -> bit 28, ..., b3 -> bit 31 (no carries collide).
-__device__ __forceinline__ uint32_t pack_step(uint32_t acc, uint32_t w) {
-    return __funnelshift_l(w * 0x10204080u, acc, 4);     // (acc << 4) | nibble
+// int8 pieces.  A piece = 16 bytes of 0/1 = the 16 sites k = 0..15 of one half-word.  Site k lives at byte
+// piece_byte(k): sites 0..7 in words 0,1, sites 8..15 in words 2,3, inside a word pair even sites in the first
+// word, odd sites in the second.  That order makes packing two multiplies per 8 sites:
+//   c = w_even + 2 * w_odd has the site pair (2i, 2i+1) in bits (8i, 8i+1);  c * 0x01041040 moves them to bits
+//   24+2i, 25+2i (all other partial products land below bit 24 or overflow, none collide), i.e. 8 sites in the top byte.
+__host__ __device__ constexpr int piece_byte(int k) { return 8 * (k >> 3) + 4 * (k & 1) + ((k & 7) >> 1); }
+
+__device__ __forceinline__ uint32_t pack_step(uint32_t acc, uint32_t w_even, uint32_t w_odd) {
+    return __funnelshift_l((w_even + 2u * w_odd) * 0x01041040u, acc, 8);     // (acc << 8) | 8 site bits
 }
-// 16 bytes (pairs 0..15) appended below acc: acc = (acc << 16) | bits, bit k = byte k.
+// 16 bytes appended below acc: acc = (acc << 16) | bits, bit k = site k.
 __device__ __forceinline__ uint32_t pack16(uint32_t acc, const uint4& v) {
-    acc = pack_step(acc, v.w);
-    acc = pack_step(acc, v.z);
-    acc = pack_step(acc, v.y);
-    return pack_step(acc, v.x);
+    acc = pack_step(acc, v.z, v.w);
+    return pack_step(acc, v.x, v.y);
 }
 
 // int8 write-back table: 8 bits -> 8 bytes of 0/1.  A compile-time constant array in global memory (2 KB, stays in
@@ -54,9 +58,9 @@ struct ByteLut {
     constexpr ByteLut() : e() {
         for (int i = 0; i < 256; ++i) {
             unsigned lo = 0, hi = 0;
-            for (int b = 0; b < 4; ++b) {
-                lo |= (unsigned)((i >> b) & 1) << (8 * b);
-                hi |= (unsigned)((i >> (4 + b)) & 1) << (8 * b);
+            for (int b = 0; b < 4; ++b) {                    // piece_byte order: even sites, then odd sites
+                lo |= (unsigned)((i >> (2 * b)) & 1) << (8 * b);
+                hi |= (unsigned)((i >> (2 * b + 1)) & 1) << (8 * b);
             }
             e[i].x = lo; e[i].y = hi;
         }

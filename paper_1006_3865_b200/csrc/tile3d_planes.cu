@@ -12,7 +12,7 @@
 //
 // HBM tile record = body + 96 bytes of bit-packed face copies written by the tile itself, so that
 // a neighbour reads every halo as a few contiguous bytes and needs no unpacking:
-//   int8 body 512 B: the 16 bytes (slice lz, colour cc, rows 4h..4h+3) at ((cc*2+h)*8 + lz)*16, byte 4*(ly&3)+p_x
+//   int8 body 512 B: the 16 bytes (slice lz, colour cc, rows 4h..4h+3) at ((cc*2+h)*8 + lz)*16, byte piece_byte(4*(ly&3)+p_x)
 //   bits body  64 B: word (cc, lz) at (cc*8 + lz)*4
 //   faces: XL[8] words (sites x=0 of slice lz, row ly at bit 4ly+3), XR[8] words (x=7, bit 4ly),
 //          YL[8] bytes (row y=0: colour 0 pairs in bits 0-3, colour 1 in 4-7), YR[8] bytes (y=7),
@@ -250,7 +250,7 @@ __global__ void k_convert3d(int8_t* __restrict__ canon, uint8_t* __restrict__ ti
     constexpr int REC = BITS ? kRec3Bits : kRec3I8;
     constexpr int BODY = BITS ? kBody3Bits : kBody3I8;
     uint8_t* rec = tiles + ((size_t)r * B * B * B + ((size_t)tz * B + ty) * B + tx) * REC;
-    uint8_t* byte = rec + ((cc * 2 + (ly >> 2)) * 8 + lz) * 16 + 4 * (ly & 3) + px;
+    uint8_t* byte = rec + ((cc * 2 + (ly >> 2)) * 8 + lz) * 16 + piece_byte(4 * (ly & 3) + px);
     uint32_t* word = reinterpret_cast<uint32_t*>(rec) + cc * 8 + lz;
     if (MODE == 1) { canon[gid] = *byte ? 1 : -1; return; }
     if (MODE == 3) { canon[gid] = ((*word >> j) & 1u) ? 1 : -1; return; }

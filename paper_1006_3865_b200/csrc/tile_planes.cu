@@ -426,7 +426,7 @@ __global__ void k_convert_planes(int8_t* __restrict__ canon, uint8_t* __restrict
     constexpr bool BITS = MODE >= 2;
     const size_t body_bytes = BITS ? (size_t)(T * T / 8) : (size_t)(T * T);
     uint8_t* rec = tiles + tile * (body_bytes + 64);
-    uint8_t* body = rec + ((((rp * 2 + cc) * NW + gx) * LPT) + Y) * 16 + kk;
+    uint8_t* body = rec + ((((rp * 2 + cc) * NW + gx) * LPT) + Y) * 16 + piece_byte(kk);
     uint32_t* w = reinterpret_cast<uint32_t*>(rec) + ((cc * NW + gx) * LPT + Y);
     const int j = rp * 16 + kk;
     if (MODE == 1) { canon[gid] = *body ? 1 : -1; return; }
