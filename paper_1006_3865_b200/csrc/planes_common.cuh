@@ -17,13 +17,22 @@ __device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
 constexpr int kLutChain = (~0xF0 & 0xAA) | (~(0xF0 ^ 0xAA) & 0xCC);    // (~p & u) | (~(p ^ u) & bw): p=a, bw=b, u=c
 constexpr int kLutNe = 0xF0 | (0xCC ^ 0xAA);                            // ne | (p ^ u): ne=a, p=b, u=c
 
-// Own-tile data is read once and written back by the same lane: plain (coherent) loads that
-// do not allocate in L1.  Halo data belongs to tiles of the other coarse colour, which this
-// launch never writes, so it may use the read-only path (__ldg).
-__device__ __forceinline__ uint4 ldg128(const void* p) {
+// Own-tile data is read once and written back by the same lane: plain (coherent) loads that do not allocate in
+// L1.  Halo data belongs to tiles of the other coarse colour, which this launch never writes, so it may
+// use the read-only path (__ldg).
+// L2 policy for the tile bodies: when the records exceed L2 they are touched once per pass, so they are
+// streamed (evict-first) and the small edge copies the next launch needs stay resident (+5 % at L = 16384);
+// when the records fit L2 the normal policy keeps them there (streaming costs 7-10 % at L <= 8192).
+__device__ __forceinline__ uint64_t body_policy(bool stream) {
+    uint64_t first, normal;
+    asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(first));
+    asm("createpolicy.fractional.L2::evict_normal.b64 %0, 1.0;" : "=l"(normal));
+    return stream ? first : normal;
+}
+__device__ __forceinline__ uint4 ldg128(const void* p, uint64_t pol) {
     uint4 v;
-    asm volatile("ld.global.L1::no_allocate.v4.u32 {%0,%1,%2,%3}, [%4];"
-                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    asm volatile("ld.global.L1::no_allocate.L2::cache_hint.v4.u32 {%0,%1,%2,%3}, [%4], %5;"
+                 : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p), "l"(pol) : "memory");
     return v;
 }
 __device__ __forceinline__ uint32_t ldg32(const void* p) {
@@ -33,6 +42,9 @@ __device__ __forceinline__ uint32_t ldg32(const void* p) {
 }
 __device__ __forceinline__ void stg128(void* p, uint4 v) {
     asm volatile("st.global.v4.u32 [%4], {%0,%1,%2,%3};" ::"r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(p) : "memory");
+}
+__device__ __forceinline__ void stg128(void* p, uint4 v, uint64_t pol) {
+    asm volatile("st.global.L2::cache_hint.v4.u32 [%4], {%0,%1,%2,%3}, %5;" ::"r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(p), "l"(pol) : "memory");
 }
 
 // int8 pieces.  A piece = 16 bytes of 0/1 = the 16 sites k = 0..15 of one half-word.  Site k lives at byte

@@ -88,7 +88,7 @@ __device__ __forceinline__ void load_slice(const Plane3Args& A, const Tile3& t, 
     } else {
         uint4 v[4];
 #pragma unroll
-        for (int c = 0; c < 4; ++c) v[c] = ldg128(rec + (c * 8 + lz) * 16);
+        for (int c = 0; c < 4; ++c) v[c] = ldg128(rec + (c * 8 + lz) * 16, body_policy(false));
         s.S[0] = pack16(pack16(0u, v[1]), v[0]);
         s.S[1] = pack16(pack16(0u, v[3]), v[2]);
     }

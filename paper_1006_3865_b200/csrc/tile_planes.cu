@@ -59,6 +59,7 @@ struct PlaneArgs {
     uint32_t u2[kHeadBits];      // same for thr[2]
     uint32_t t1_tail, t2_tail;   // thr[m] & (2^20 - 1)
     uint32_t force;              // all-ones if beta = 0 (every thr[m] = 2^32: every proposal is accepted), else 0
+    uint32_t stream;             // 1: the records exceed L2, stream the tile bodies (planes_common.cuh: body_policy)
     const uint4* jrec;           // coupling records (a9) or nullptr: per tile, uint4 (cc, gx, Y) =
                                  // {V1, V2, H1, H2}: bit j set <=> the bond from site j of that block to its
                                  // neighbour in the V1 / V2 / H1 / H2 word is J = -1.  Shared by all replicas.
@@ -98,6 +99,7 @@ __device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int
     const uint32_t txL = utx == 0 ? B - 1 : utx - 1, txR = utx == B - 1 ? 0 : utx + 1;
     auto rec_of = [&](uint32_t idx) { return A.tiles + (uint64_t)idx * REC; };
     const uint8_t* rec = rec_of(rowc + utx);
+    const uint64_t pol = body_policy(A.stream != 0);
     if (BITS) {
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
@@ -106,7 +108,7 @@ __device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int
     } else {
         uint4 v[G::NCH];
 #pragma unroll
-        for (int ch = 0; ch < G::NCH; ++ch) v[ch] = ldg128(rec + (ch * G::LPT + Y) * 16);
+        for (int ch = 0; ch < G::NCH; ++ch) v[ch] = ldg128(rec + (ch * G::LPT + Y) * 16, pol);
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
@@ -136,6 +138,7 @@ __device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, in
     constexpr uint32_t REC = BITS ? G::REC_BITS : G::REC_I8;
     constexpr uint32_t BODY = REC - G::EDGE;
     uint8_t* rec = A.tiles + (uint64_t)(((uint32_t)r * (uint32_t)A.B + (uint32_t)ty) * (uint32_t)A.B + (uint32_t)tx) * REC;
+    const uint64_t pol = body_policy(A.stream != 0);
     if (BITS) {
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
@@ -152,7 +155,7 @@ __device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, in
                 for (int rp = 0; rp < 2; ++rp) {
                     const uint2 a = __ldg(lut + ((w >> (16 * rp)) & 0xffu));          // bits 0..7  -> bytes 0..7
                     const uint2 b = __ldg(lut + ((w >> (16 * rp + 8)) & 0xffu));      // bits 8..15 -> bytes 8..15
-                    stg128(rec + ((((rp * 2 + cc) * G::NW + gx) * G::LPT) + Y) * 16, make_uint4(a.x, a.y, b.x, b.y));
+                    stg128(rec + ((((rp * 2 + cc) * G::NW + gx) * G::LPT) + Y) * 16, make_uint4(a.x, a.y, b.x, b.y), pol);
                 }
             }
     }
@@ -536,6 +539,8 @@ int launch_planes_to_canon(ising_ctx* h, int T, bool bits, const void* d_tiles, 
     return 0;
 }
 
+constexpr size_t kL2StreamBytes = 96u << 20;    // records larger than this do not stay in the 126 MB L2 between passes
+
 bool plain64_supported(const ising_ctx* h, int T) { return h->dim == 2 && h->L == 64 && T == 64; }
 
 static void fill_accept(PlaneArgs& A, const Accept& acc) {
@@ -555,6 +560,7 @@ int launch_plain64(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uin
     A.seeds = h->d_seeds;
     A.L = 64; A.B = 1; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0; A.njobs = (uint32_t)h->R;
     A.magic_rep = A.magic_hb = 0;
+    A.stream = 0;
     A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
     fill_accept(A, acc);
     cudaStream_t st = hooks().stream;
@@ -609,6 +615,7 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
     A.seeds = h->d_seeds;
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first;
     A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
+    A.stream = tile_planes_bytes(h, T, bits) > kL2StreamBytes ? 1u : 0u;
     const uint32_t tiles_per_colour = (uint32_t)((size_t)h->R * A.B * A.B / 2);
     A.njobs = tiles_per_colour / (uint32_t)(64 / T);
     A.magic_rep = fastdiv_magic((uint32_t)A.B * (uint32_t)A.B / 2u);
