@@ -117,6 +117,21 @@ int ising_set_layout(ising_handle h, int layout);
  * at any time; spins and t are untouched. */
 int ising_set_rng(ising_handle h, int mode);
 
+enum {
+    ISING_JIT_AUTO = 0,      /* specialise on big calls only (>= 2^27 attempted flips per ising_sweep)   */
+    ISING_JIT_OFF = 1,       /* always the pre-compiled kernels                                          */
+    ISING_JIT_ON = 2         /* specialise whenever a specialisable kernel is used                       */
+};
+
+/* ising_set_jit — run-time specialisation of the 2D multi-spin tile kernel (a2 + a5).  The thresholds of
+ * S8c.4 depend on beta only; with their 12 head bits as compile-time constants the bit-serial compare of
+ * r with thr[a/2] needs half the instructions.  The library can compile its own kernel source for the
+ * current thresholds with NVRTC (first use of a beta: about a second; cached per process).  Results are
+ * bit-identical either way; if NVRTC is missing the pre-compiled kernel is used.
+ * ising_last_sweep_specialized returns 1 if the last ising_sweep on h ran a specialised kernel. */
+int ising_set_jit(ising_handle h, int mode);
+int ising_last_sweep_specialized(ising_handle h);
+
 /* The state of a run is (spins, t, seed): the random stream is stateless (S8c.3), so
  * copy_spins + get_counter / set_spins + set_counter resume a run bit-exactly. */
 int ising_get_counter(ising_handle h, uint64_t* t);

@@ -23,7 +23,7 @@ RNG_MODES = {"words": ISING_RNG_WORDS, "planes": ISING_RNG_PLANES}
 
 SYMBOLS = [
     "ising_create", "ising_create_batch", "ising_destroy", "ising_sweep", "ising_sweep_series",
-    "ising_observables", "ising_overlap", "ising_copy_spins", "ising_set_spins", "ising_set_layout", "ising_set_rng",
+    "ising_observables", "ising_overlap", "ising_copy_spins", "ising_set_spins", "ising_set_layout", "ising_set_rng", "ising_set_jit", "ising_last_sweep_specialized",
     "ising_get_counter", "ising_set_counter", "ising_thresholds", "ising_set_device_hooks",
     "ising_synchronize", "ising_kernel_launches", "ising_sweep_path", "ising_force_path",
     "ising_last_error",
@@ -65,6 +65,8 @@ def lib() -> C.CDLL:
     L.ising_set_spins.argtypes = [vp, i8p]
     L.ising_set_layout.argtypes = [vp, C.c_int]
     L.ising_set_rng.argtypes = [vp, C.c_int]
+    L.ising_set_jit.argtypes = [vp, C.c_int]
+    L.ising_last_sweep_specialized.argtypes = [vp]
     L.ising_get_counter.argtypes = [vp, u64p]
     L.ising_set_counter.argtypes = [vp, C.c_uint64]
     L.ising_thresholds.argtypes = [C.c_double, C.c_int, u64p]
@@ -192,6 +194,14 @@ class Ising:
 
     def set_rng(self, mode) -> None:
         _check(lib().ising_set_rng(self._h, RNG_MODES[mode] if isinstance(mode, str) else int(mode)))
+
+    def set_jit(self, mode) -> None:
+        """mode: "auto" (default), "off", "on" or the ISING_JIT_* value."""
+        m = {"auto": 0, "off": 1, "on": 2}.get(mode, mode)
+        _check(lib().ising_set_jit(self._h, int(m)))
+
+    def last_sweep_specialized(self) -> bool:
+        return bool(lib().ising_last_sweep_specialized(self._h))
 
     def set_layout(self, layout: int) -> None:
         _check(lib().ising_set_layout(self._h, int(layout)))

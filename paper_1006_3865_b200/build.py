@@ -14,7 +14,7 @@ CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libising_b200.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-         "-Xcompiler", "-fPIC", "-shared", "-cudart", "static"]
+         "-Xcompiler", "-fPIC", "-shared", "-cudart", "static", "-ldl"]
 
 
 def sources():
@@ -30,8 +30,29 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
+JIT_HEADERS = ["philox.cuh", "planes_common.cuh", "tile_planes_device.cuh"]   # in inclusion order
+JIT_INC = os.path.join(CSRC, "jit_source.inc")
+
+
+def write_jit_source() -> None:
+    """csrc/jit_source.inc = the device headers of the 2D multi-spin kernel as one C++ raw string literal: the
+    source planes_jit.cu hands to NVRTC at run time (local #include lines and #pragma once dropped)."""
+    parts = []
+    for name in JIT_HEADERS:
+        for line in open(os.path.join(CSRC, name)):
+            t = line.strip()
+            if t.startswith('#include "') or t == "#pragma once":
+                continue
+            parts.append(line)
+    text = 'R"ISINGJIT(\n' + "".join(parts) + ')ISINGJIT"\n'
+    if not os.path.exists(JIT_INC) or open(JIT_INC).read() != text:
+        with open(JIT_INC, "w") as f:
+            f.write(text)
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     """Compile every .cu under csrc/ into one shared library; returns its path."""
+    write_jit_source()
     if not force and not _stale():
         return LIB
     if not os.path.exists(NVCC):

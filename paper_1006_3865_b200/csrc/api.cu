@@ -333,11 +333,15 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             if (!rc) rc = launch_convert_couplings(h, T, h->d_Jtiles);
             if (!rc) h->Jtiles_tile = T;
         }
+        // run-time specialisation pays for its ~1 s of compilation only on big calls (AUTO: >= 2^27 attempted flips)
+        const bool use_jit = use_planes && (h->jit_mode == ISING_JIT_ON ||
+                             (h->jit_mode == ISING_JIT_AUTO && (double)n * k * (double)h->N * h->R >= 134217728.0));
+        h->last_jit = 0;
         for (int pass = 0; pass < n && !rc; ++pass) {
             const uint64_t t0 = h->t + (uint64_t)pass * (uint64_t)k;
             rc = use_tile_i8 ? launch_tile_i8_pass(h, acc, T, k, t0)
                  : use_3d ? launch_tile3d_pass(h, acc, bits, k, t0)
-                          : launch_tile_planes_pass(h, acc, T, bits, k, t0);
+                          : launch_tile_planes_pass(h, acc, T, bits, k, t0, use_jit);
             if (!rc && want_series)
                 rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);
         }
@@ -443,6 +447,17 @@ int ising_set_rng(ising_handle h, int mode) {
     h->rng = mode;
     return 0;
 }
+
+int ising_set_jit(ising_handle h, int mode) {
+    if (!h || (mode != ISING_JIT_AUTO && mode != ISING_JIT_OFF && mode != ISING_JIT_ON)) {
+        set_error("ising_set_jit: mode must be ISING_JIT_AUTO, ISING_JIT_OFF or ISING_JIT_ON");
+        return ISING_EINVAL;
+    }
+    h->jit_mode = mode;
+    return 0;
+}
+
+int ising_last_sweep_specialized(ising_handle h) { return h ? h->last_jit : 0; }
 
 int ising_get_counter(ising_handle h, uint64_t* t) {
     if (!h || !t) { set_error("ising_get_counter: NULL argument"); return ISING_EINVAL; }

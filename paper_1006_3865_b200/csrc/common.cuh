@@ -88,4 +88,6 @@ struct ising_ctx {
     int* d_flag = nullptr;          // validation flag
     const char* last_path = "none";
     int force_generic = 0;
+    int jit_mode = 0;               // ISING_JIT_AUTO / OFF / ON (ising_set_jit)
+    int last_jit = 0;               // 1 if the last tile launch used a run-time specialised kernel
 };

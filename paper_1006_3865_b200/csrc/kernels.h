@@ -30,7 +30,7 @@ int launch_convert_couplings(ising_ctx* h, int T, void* d_jrec);
 bool plain64_supported(const ising_ctx* h, int T);
 int launch_plain64(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M);
 int launch_observables_planes(ising_ctx* h, int T, bool bits, long long* d_E, long long* d_M);
-int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, int k, uint64_t t_first);
+int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, int k, uint64_t t_first, bool use_jit);
 
 // ---- tile3d_planes.cu: 3D multi-spin tile kernel, 8x8x8 tiles (RNG mapping "planes") ----------
 bool tile3d_supported(const ising_ctx* h, int T);
@@ -38,5 +38,10 @@ size_t tile3d_bytes(const ising_ctx* h, bool bits);
 int launch_canon_to_3d(ising_ctx* h, bool bits, const int8_t* d_canon, void* d_tiles);
 int launch_3d_to_canon(ising_ctx* h, bool bits, const void* d_tiles, int8_t* d_canon);
 int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64_t t_first);
+
+// ---- planes_jit.cu: run-time specialisation of k_tile_planes on the threshold head bits (NVRTC) ----
+cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp);   // nullptr: not available
+uint64_t planes_jit_compiled();
+const char* planes_jit_last_log();
 
 }  // namespace ising

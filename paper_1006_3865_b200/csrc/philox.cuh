@@ -2,7 +2,16 @@
 // S8c.2: multipliers 0xD2511F53 (on ctr[0]) and 0xCD9E8D57 (on ctr[2]); key increments
 // 0x9E3779B9 / 0xBB67AE85; ten rounds.  No RNG state ever lives in HBM (BASELINE north_star).
 #pragma once
+#ifdef __CUDACC_RTC__          // run-time compilation (planes_jit.cu): no host headers
+typedef unsigned char uint8_t;
+typedef signed char int8_t;
+typedef unsigned short uint16_t;
+typedef unsigned int uint32_t;
+typedef unsigned long long uint64_t;
+typedef unsigned long size_t;
+#else
 #include <cstdint>
+#endif
 
 namespace ising {
 

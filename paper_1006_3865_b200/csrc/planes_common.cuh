@@ -1,8 +1,6 @@
 // planes_common.cuh — device helpers shared by the multi-spin (bit-plane) tile kernels
 // (tile_planes.cu: 2D, tile3d_planes.cu: 3D).  DESIGN.md §6.1.
 #pragma once
-#include <cstdint>
-
 #include "philox.cuh"
 
 namespace ising {
@@ -67,7 +65,7 @@ __device__ __forceinline__ uint32_t pack16(uint32_t acc, const uint4& v) {
 // L1 / L2); lookups go through the read-only path, so no kernel builds a copy or needs a barrier.
 struct ByteLut {
     uint2 e[256];
-    constexpr ByteLut() : e() {
+    __host__ __device__ constexpr ByteLut() : e() {
         for (int i = 0; i < 256; ++i) {
             unsigned lo = 0, hi = 0;
             for (int b = 0; b < 4; ++b) {                    // piece_byte order: even sites, then odd sites
@@ -81,7 +79,9 @@ struct ByteLut {
 __device__ const ByteLut kByteLutGlobal = ByteLut();
 
 // ceil(2^32 / d) on the host; q / d on the device = umulhi(q, magic) corrected by at most one either way.
+#ifndef __CUDACC_RTC__
 inline uint32_t fastdiv_magic(uint32_t d) { return d <= 1 ? 0xffffffffu : (uint32_t)((0x100000000ull + d - 1) / d); }
+#endif
 __device__ __forceinline__ uint32_t fastdiv(uint32_t q, uint32_t d, uint32_t magic) {
     uint32_t r = __umulhi(q, magic);
     if (r * d > q) --r;

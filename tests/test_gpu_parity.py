@@ -181,6 +181,30 @@ def test_plain64_path_matches_oracle(P, orc, k, n, beta, seeds, jseed, layout):
     _same_state(g, o)
 
 
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,tile,k,n,beta,seeds,jseed", [
+    (256, 64, 2, 3, BC2, [3], None), (256, 32, 3, 2, 0.3, [4, 5], None), (128, 32, 2, 3, 1.0, [6, 7], 5),
+    (512, 64, 1, 4, 0.6, [8], None), (128, 64, 2, 2, 30.0, [2], None), (128, 32, 1, 2, 0.0, [2], None),
+])
+def test_specialised_kernel_matches_oracle(P, orc, L, tile, k, n, beta, seeds, jseed, layout):
+    """Run-time specialisation on the threshold head bits (ising_set_jit ON): same trajectory, bit for bit; and the
+    pre-compiled kernel (OFF) continues it identically."""
+    J = W.couplings(2, L, jseed) if jseed is not None else None
+    g, o = _both(P, orc, 2, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.set_jit("on")
+    Eg, Mg = g.sweep_series(beta, n, tile, k)
+    assert g.last_sweep_specialized() == (beta > 0), "NVRTC specialisation was not used (beta = 0 has no thresholds to fold)"
+    Eo, Mo = o.sweep_series(beta, n, tile, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    g.set_jit("off")
+    g.sweep(beta, 2, tile, k); o.sweep(beta, 2, tile, k)
+    assert not g.last_sweep_specialized()
+    _same_state(g, o)
+
+
 @pytest.mark.parametrize("L,tile,k,n,beta,seeds", TILED)
 def test_tile_i8_path_matches_oracle(P, orc, L, tile, k, n, beta, seeds):
     g, o = _both(P, orc, 2, L, seeds, rng="words")
