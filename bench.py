@@ -158,9 +158,13 @@ def selftest_ranks(rank: int, world: int) -> None:
     dist.destroy_process_group()
 
 
+JIT = "auto"     # --jit: run-time specialisation of the planes kernel (ising_set_jit)
+
+
 def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng="planes"):
     """Device-timed throughput of one (rng, layout, tile, k) variant; returns dict."""
     g = P.Ising(2, L, seed=3, rng=rng)
+    g.set_jit(JIT)
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
     g.sweep(W.BETA_C_2D, warmup, tile, k)
@@ -181,7 +185,7 @@ def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng=
     ms = e0.elapsed_time(e1)
     clocks = sampler.stop(t0, t1) if sampler else None
     launches = P.ising_kernel_launches() - n0
-    path = g.sweep_path()
+    path = g.sweep_path() + ("+jit" if g.last_sweep_specialized() else "")
     g.destroy()
     flips = steps * k * L * L
     return {"ms": ms, "flips_per_ns": flips / (ms * 1e6), "launches": int(launches), "path": path, "clocks": clocks}
@@ -191,6 +195,7 @@ def time_e2e(P, torch, L, layout, tile, k, steps, rng="planes"):
     """Same metric through the public API with HOST buffers: every step uploads the spins from
     pinned host memory (ising_set_spins), runs one pass, and reads them back (ising_copy_spins)."""
     g = P.Ising(2, L, seed=3, rng=rng)
+    g.set_jit(JIT)
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
     host = torch.empty(L * L, dtype=torch.int8).pin_memory()
@@ -263,10 +268,13 @@ def main() -> None:
     ap.add_argument("--rng", default="planes", choices=["planes", "words"], help="RNG->site mapping (DESIGN.md R6)")
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the k/tile table")
+    ap.add_argument("--jit", default="auto", choices=["auto", "on", "off"], help="run-time kernel specialisation (ising_set_jit)")
     ap.add_argument("--lscan", action="store_true", help="study: flips/ns against L (SURVEY 8(f)-3)")
     ap.add_argument("--autocorr", action="store_true", help="study: autocorrelation time against k (SURVEY 8(f)-2)")
     ap.add_argument("--selftest-ranks", action="store_true", help="CPU/gloo check of the multi-rank aggregation, no GPU")
     a = ap.parse_args()
+    global JIT
+    JIT = a.jit
     a.warmup = max(a.warmup, 3) if a.impl == "ours" else a.warmup
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

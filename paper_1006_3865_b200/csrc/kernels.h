@@ -40,7 +40,7 @@ int launch_3d_to_canon(ising_ctx* h, bool bits, const void* d_tiles, int8_t* d_c
 int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64_t t_first);
 
 // ---- planes_jit.cu: run-time specialisation of k_tile_planes on the threshold head bits (NVRTC) ----
-cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp);   // nullptr: not available
+cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R);   // nullptr: not available
 uint64_t planes_jit_compiled();
 const char* planes_jit_last_log();
 

@@ -61,7 +61,7 @@ struct Nvrtc {
 
 struct JitState {
     std::mutex mu;
-    std::map<std::tuple<int, int, int, uint32_t>, cudaKernel_t> cache;   // nullptr = tried and failed
+    std::map<std::tuple<int, int, int, uint32_t, int, int>, cudaKernel_t> cache;   // nullptr = tried and failed
     std::vector<cudaLibrary_t> libs;
     std::string last_log;
     uint64_t compiled = 0;
@@ -72,7 +72,7 @@ JitState& state() {
     return s;
 }
 
-cudaKernel_t compile_one(int T, bool bits, bool hasj, uint32_t hp, std::string& log) {
+cudaKernel_t compile_one(int T, bool bits, bool hasj, uint32_t hp, int B, int R, std::string& log) {
     static Nvrtc rt;
     if (!rt.ok) { log = "libnvrtc not available"; return nullptr; }
     char expr[160];
@@ -82,8 +82,11 @@ cudaKernel_t compile_one(int T, bool bits, bool hasj, uint32_t hp, std::string& 
     cudaKernel_t kernel = nullptr;
     do {
         if (rt.AddNameExpression(prog, expr) != 0) { log = "nvrtcAddNameExpression failed"; break; }
-        const char* opts[] = {"--gpu-architecture=sm_100a", "--std=c++17"};
-        const nvrtcResult_t rc = rt.CompileProgram(prog, 2, opts);
+        char defB[48], defR[48];                      // lattice geometry as constants: index arithmetic folds
+        snprintf(defB, sizeof defB, "-DISING_JIT_B=%uu", (unsigned)B);
+        snprintf(defR, sizeof defR, "-DISING_JIT_R=%uu", (unsigned)R);
+        const char* opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "--generate-line-info", defB, defR};
+        const nvrtcResult_t rc = rt.CompileProgram(prog, 5, opts);
         size_t n = 0;
         if (rt.GetProgramLogSize(prog, &n) == 0 && n > 1) { log.resize(n); rt.GetProgramLog(prog, &log[0]); }
         if (rc != 0) break;
@@ -112,15 +115,16 @@ cudaKernel_t compile_one(int T, bool bits, bool hasj, uint32_t hp, std::string& 
 
 }  // namespace
 
-// The specialised kernel for (T, BITS, HASJ, HP), compiled on first use; nullptr if it cannot be had.
-cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp) {
+// The kernel specialised for (T, BITS, HASJ, HP) and the geometry (B tiles per side, R replicas), compiled on
+// first use; nullptr if it cannot be had.
+cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R) {
     JitState& s = state();
     std::lock_guard<std::mutex> lock(s.mu);
-    const auto key = std::make_tuple(T, (int)bits, (int)hasj, hp);
+    const auto key = std::make_tuple(T, (int)bits, (int)hasj, hp, B, R);
     auto it = s.cache.find(key);
     if (it != s.cache.end()) return it->second;
     std::string log;
-    cudaKernel_t k = compile_one(T, bits, hasj, hp, log);
+    cudaKernel_t k = compile_one(T, bits, hasj, hp, B, R, log);
     if (k) ++s.compiled; else s.last_log = log;
     s.cache[key] = k;
     return k;

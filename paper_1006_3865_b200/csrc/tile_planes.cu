@@ -175,7 +175,7 @@ int launch_colour_planes(const PlaneArgs& A, bool use_jit, bool* used_jit) {
     attr[0].val.programmaticStreamSerializationAllowed = pdl;
     cfg.attrs = attr; cfg.numAttrs = 1;
     // specialised on the threshold head bits (planes_jit.cu) when asked for and available, else run-time operands
-    cudaKernel_t spec = (use_jit && !A.force) ? planes_jit_kernel(T, BITS, A.jrec != nullptr, A.hp) : nullptr;
+    cudaKernel_t spec = (use_jit && !A.force) ? planes_jit_kernel(T, BITS, A.jrec != nullptr, A.hp, A.B, A.R) : nullptr;
     if (spec) {
         void* args[] = {const_cast<PlaneArgs*>(&A)};
         ISING_CUDA_OK(cudaLaunchKernelExC(&cfg, (const void*)spec, args));

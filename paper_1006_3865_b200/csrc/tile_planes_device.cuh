@@ -54,17 +54,33 @@ struct PlaneArgs {
                                  // neighbour in the V1 / V2 / H1 / H2 word is J = -1.  Shared by all replicas.
 };
 
+// Lattice geometry: run-time fields of the arguments, or compile-time constants when the kernel is specialised at
+// run time (planes_jit.cu defines ISING_JIT_B = tiles per side and ISING_JIT_R = replicas).
+#ifdef ISING_JIT_B
+__device__ __forceinline__ uint32_t geom_B(const PlaneArgs&) { return ISING_JIT_B; }
+__device__ __forceinline__ uint32_t geom_R(const PlaneArgs&) { return ISING_JIT_R; }
+#else
+__device__ __forceinline__ uint32_t geom_B(const PlaneArgs& A) { return (uint32_t)A.B; }
+__device__ __forceinline__ uint32_t geom_R(const PlaneArgs& A) { return (uint32_t)A.R; }
+#endif
+
 template <int T>
 __device__ __forceinline__ void job_tile(const PlaneArgs& A, uint32_t job, int sub, int& r, int& tx, int& ty) {
     // colour-C tiles enumerated row by row: q -> ty = q / (B/2), tx = 2*(q % (B/2)) + ((ty + C) & 1)
-    const uint32_t per_rep = (uint32_t)A.B * (uint32_t)A.B / 2u;
+    const uint32_t B = geom_B(A), per_rep = B * B / 2u, hb = B >> 1;
     const uint32_t q = job * PG<T>::TPW + (uint32_t)sub;
-    const uint32_t rr = fastdiv(q, per_rep, A.magic_rep);
-    r = (int)rr;
+#ifdef ISING_JIT_B
+    const uint32_t rr = ISING_JIT_R == 1 ? 0u : q / per_rep;      // divisions by constants
     const uint32_t qq = q - rr * per_rep;
-    const uint32_t hb = (uint32_t)A.B >> 1;
-    ty = (int)fastdiv(qq, hb, A.magic_hb);
-    tx = (int)(2u * (qq - (uint32_t)ty * hb)) + ((ty + A.C) & 1);
+    const uint32_t yy = qq / hb;
+#else
+    const uint32_t rr = fastdiv(q, per_rep, A.magic_rep);
+    const uint32_t qq = q - rr * per_rep;
+    const uint32_t yy = fastdiv(qq, hb, A.magic_hb);
+#endif
+    r = (int)rr;
+    ty = (int)yy;
+    tx = (int)(2u * (qq - yy * hb)) + ((ty + A.C) & 1);
 }
 
 // Everything a lane keeps of its job between load and store.
@@ -82,7 +98,7 @@ __device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int
     constexpr uint32_t REC = BITS ? G::REC_BITS : G::REC_I8;
     constexpr uint32_t BODY = REC - G::EDGE;
     // tile indices in 32 bits, one widening multiply per record address
-    const uint32_t B = (uint32_t)A.B, utx = (uint32_t)tx, uty = (uint32_t)ty;
+    const uint32_t B = geom_B(A), utx = (uint32_t)tx, uty = (uint32_t)ty;
     const uint32_t row0 = (uint32_t)r * B * B, rowc = row0 + uty * B;
     const uint32_t tyU = uty == 0 ? B - 1 : uty - 1, tyD = uty == B - 1 ? 0 : uty + 1;
     const uint32_t txL = utx == 0 ? B - 1 : utx - 1, txR = utx == B - 1 ? 0 : utx + 1;
@@ -126,7 +142,7 @@ __device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, in
     using G = PG<T>;
     constexpr uint32_t REC = BITS ? G::REC_BITS : G::REC_I8;
     constexpr uint32_t BODY = REC - G::EDGE;
-    uint8_t* rec = A.tiles + (uint64_t)(((uint32_t)r * (uint32_t)A.B + (uint32_t)ty) * (uint32_t)A.B + (uint32_t)tx) * REC;
+    uint8_t* rec = A.tiles + (uint64_t)(((uint32_t)r * geom_B(A) + (uint32_t)ty) * geom_B(A) + (uint32_t)tx) * REC;
     const uint64_t pol = body_policy(A.stream != 0);
     if (BITS) {
 #pragma unroll
@@ -231,8 +247,8 @@ __device__ __forceinline__ void head_masks_sel(uint32_t g, uint32_t Hlo, uint32_
 // und selects the (rare) sites whose tail must be drawn; p_base = pair index i>>1 of bit 0, row stride L/2.
 template <bool HASJ, uint32_t HP>
 __device__ __forceinline__ uint32_t update_block(const PlaneArgs& A, uint32_t S, uint32_t V1, uint32_t V2, uint32_t H1,
-                                                 uint32_t H2, const uint4& Jw, uint32_t g, uint32_t p_base, uint32_t Hlo,
-                                                 uint32_t Hhi, uint32_t k0, uint32_t k1) {
+                                                 uint32_t H2, const uint4& Jw, uint32_t g, uint32_t p_base, uint32_t prow,
+                                                 uint32_t Hlo, uint32_t Hhi, uint32_t k0, uint32_t k1) {
     // unsatisfied bonds: J s_i s_j = -1  <=>  s_i != s_j for J = +1, s_i == s_j for J = -1 (eq. (1))
     const uint32_t a = S ^ V1 ^ (HASJ ? Jw.x : 0u), b = S ^ V2 ^ (HASJ ? Jw.y : 0u);
     const uint32_t c = S ^ H1 ^ (HASJ ? Jw.z : 0u), d = S ^ H2 ^ (HASJ ? Jw.w : 0u);
@@ -247,7 +263,7 @@ __device__ __forceinline__ uint32_t update_block(const PlaneArgs& A, uint32_t S,
         while (und) {                                                 // probability 2^-12 per site
             const int j = __ffs(und) - 1;
             und &= und - 1;
-            const uint32_t p = p_base + (uint32_t)(j >> 4) * (uint32_t)(A.L >> 1) + (uint32_t)(j & 15);
+            const uint32_t p = p_base + (uint32_t)(j >> 4) * prow + (uint32_t)(j & 15);
             const u32x4 o = philox4x32_10(p, kTagTail, Hlo, Hhi, k0, k1);
             R |= (uint32_t)((o.x >> kHeadBits) < (((sel >> j) & 1u) ? A.t2_tail : A.t1_tail)) << j;
         }
@@ -259,7 +275,7 @@ __device__ __forceinline__ uint32_t update_block(const PlaneArgs& A, uint32_t S,
     while (und) {                                                     // probability 2^-12 per site
         const int j = __ffs(und) - 1;
         und &= und - 1;
-        const uint32_t p = p_base + (uint32_t)(j >> 4) * (uint32_t)(A.L >> 1) + (uint32_t)(j & 15);
+        const uint32_t p = p_base + (uint32_t)(j >> 4) * prow + (uint32_t)(j & 15);
         const u32x4 o = philox4x32_10(p, kTagTail, Hlo, Hhi, k0, k1);
         const uint32_t tail = o.x >> kHeadBits;
         if ((eq1 >> j) & 1u) R1 |= (uint32_t)(tail < A.t1_tail) << j;
@@ -318,7 +334,7 @@ __device__ __forceinline__ void half_sweep(const PlaneArgs& A, TileRegs<T>& t, c
         uint32_t V1, V2, H1, H2;
         neighbour_words<T, PERIODIC>(t, c, gx, Y, V1, V2, H1, H2);
         Snew[gx] = update_block<HASJ, HP>(A, t.S[c][gx], V1, V2, H1, H2, Jw[c][gx], g0 + (uint32_t)gx,
-                                      p0 + 16u * (uint32_t)gx, Hlo, Hhi, k0, k1);
+                                          p0 + 16u * (uint32_t)gx, geom_B(A) * (uint32_t)(T / 2), Hlo, Hhi, k0, k1);
     }
 #pragma unroll
     for (int gx = 0; gx < G::NW; ++gx) t.S[c][gx] = Snew[gx];
@@ -365,13 +381,13 @@ __global__ void __launch_bounds__(kPlaneThreads) k_tile_planes(PlaneArgs A) {
     for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
         for (int gx = 0; gx < G::NW; ++gx)
-            Jw[cc][gx] = HASJ ? __ldg(A.jrec + ((size_t)ty * A.B + tx) * (2 * G::NW * G::LPT) + (cc * G::NW + gx) * G::LPT + Y)
+            Jw[cc][gx] = HASJ ? __ldg(A.jrec + ((size_t)ty * geom_B(A) + tx) * (2 * G::NW * G::LPT) + (cc * G::NW + gx) * G::LPT + Y)
                               : make_uint4(0u, 0u, 0u, 0u);
     const uint64_t seed = A.seeds[r];
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);                         // global block row
-    const uint32_t g0 = Yg * (uint32_t)(A.L >> 5) + (uint32_t)(tx * G::NW);  // RNG block of gx = 0
-    const uint32_t p0 = 2u * Yg * (uint32_t)(A.L >> 1) + 16u * (uint32_t)(tx * G::NW);   // pair index of its bit 0
+    const uint32_t g0 = Yg * (geom_B(A) * G::NW) + (uint32_t)(tx * G::NW);   // RNG block of gx = 0 (L / 32 blocks per row)
+    const uint32_t p0 = 2u * Yg * (geom_B(A) * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);   // pair index of its bit 0
     for (int j = 0; j < A.k; ++j) {
         const uint64_t tt = A.t_first + (uint64_t)j;
         half_sweep<T, HASJ, false, HP>(A, t, Jw, 0, Y, g0, p0, 2 * tt, k0, k1);
