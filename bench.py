@@ -47,11 +47,11 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
 
 
-# From the committed ncu captures (profiles/r01c_tile_planes_i8_t64.md), per launch of the kernel:
-# DRAM bytes read + written, and executed warp-instructions.  Keyed by (rng, layout, tile, k).
+# From the committed ncu captures (profiles/r01d_tile_planes_jit_i8_t64.md), per launch of the kernel:
+# DRAM bytes read + written, and executed warp-instructions.  Keyed by (rng, layout, tile, k, jit).
 NCU = {
-    ("planes", "int8", 64, 1): {"traffic": 171.99e6 + 82.06e6, "warp_instr": 37.42e6},
-    ("planes", "int8", 64, 16): {"traffic": 171.99e6 + 82.50e6, "warp_instr": 434.9e6},
+    ("planes", "int8", 64, 1, True): {"traffic": 138.44e6 + 79.40e6, "warp_instr": 33.78e6},
+    ("planes", "int8", 64, 16, True): {"traffic": 138.44e6 + 79.33e6, "warp_instr": 391.3e6},
 }
 # Issue ceiling of the path: 148 SMs x 4 SMSPs, one warp-instruction per 2 cycles at sm_max_mhz.
 def issue_peak_gips(sm_mhz: float) -> float:
@@ -313,7 +313,7 @@ def main() -> None:
     ms, value = aggregate_replicas(res["ms"], world, a.steps, a.k, L, dist, "cuda")
 
     peak, peak_src, sm_max = measured_peaks()
-    ncu = NCU.get((a.rng, a.layout, a.tile, a.k)) if L == 16384 else None
+    ncu = NCU.get((a.rng, a.layout, a.tile, a.k, res["path"].endswith("+jit"))) if L == 16384 else None
     bpf = algorithmic_bytes_per_flip(a.tile, a.k, a.layout)
     launches_per_step = 2
     bytes_per_launch = bpf * a.k * L * L / launches_per_step
@@ -330,7 +330,7 @@ def main() -> None:
             "ns_per_flip": 1.0 / value, "gpu_launches": res["launches"], "clocks": res["clocks"],
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": ncu["traffic"] if ncu else None,
-                         "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01c_tile_planes_i8_t64.md" if ncu else None,
+                         "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01d_tile_planes_jit_i8_t64.md" if ncu else None,
                          "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
                          "algorithmic_bytes_per_flip": bpf, "kernel": f"{res['path']}<{a.tile}>",
                          "avg_launch_ms": launch_ms,
