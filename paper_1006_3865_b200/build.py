@@ -30,24 +30,28 @@ def _stale() -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-JIT_HEADERS = ["philox.cuh", "planes_common.cuh", "tile_planes_device.cuh"]   # in inclusion order
-JIT_INC = os.path.join(CSRC, "jit_source.inc")
+JIT_SOURCES = {   # generated file -> device headers in inclusion order
+    "jit_source.inc": ["philox.cuh", "planes_common.cuh", "tile_planes_device.cuh"],
+    "jit_source3d.inc": ["philox.cuh", "planes_common.cuh", "tile3d_planes_device.cuh"],
+}
 
 
 def write_jit_source() -> None:
-    """csrc/jit_source.inc = the device headers of the 2D multi-spin kernel as one C++ raw string literal: the
-    source planes_jit.cu hands to NVRTC at run time (local #include lines and #pragma once dropped)."""
-    parts = []
-    for name in JIT_HEADERS:
-        for line in open(os.path.join(CSRC, name)):
-            t = line.strip()
-            if t.startswith('#include "') or t == "#pragma once":
-                continue
-            parts.append(line)
-    text = 'R"ISINGJIT(\n' + "".join(parts) + ')ISINGJIT"\n'
-    if not os.path.exists(JIT_INC) or open(JIT_INC).read() != text:
-        with open(JIT_INC, "w") as f:
-            f.write(text)
+    """csrc/jit_source*.inc = the device headers of the multi-spin kernels as one C++ raw string literal each: the
+    sources planes_jit.cu hands to NVRTC at run time (local #include lines and #pragma once dropped)."""
+    for inc, headers in JIT_SOURCES.items():
+        parts = []
+        for name in headers:
+            for line in open(os.path.join(CSRC, name)):
+                t = line.strip()
+                if t.startswith('#include "') or t == "#pragma once":
+                    continue
+                parts.append(line)
+        text = 'R"ISINGJIT(\n' + "".join(parts) + ')ISINGJIT"\n'
+        path = os.path.join(CSRC, inc)
+        if not os.path.exists(path) or open(path).read() != text:
+            with open(path, "w") as f:
+                f.write(text)
 
 
 def build(force: bool = False, verbose: bool = False) -> str:

@@ -334,13 +334,13 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             if (!rc) h->Jtiles_tile = T;
         }
         // run-time specialisation pays for its ~1 s of compilation only on big calls (AUTO: >= 2^27 attempted flips)
-        const bool use_jit = use_planes && (h->jit_mode == ISING_JIT_ON ||
+        const bool use_jit = (use_planes || use_3d) && (h->jit_mode == ISING_JIT_ON ||
                              (h->jit_mode == ISING_JIT_AUTO && (double)n * k * (double)h->N * h->R >= 134217728.0));
         h->last_jit = 0;
         for (int pass = 0; pass < n && !rc; ++pass) {
             const uint64_t t0 = h->t + (uint64_t)pass * (uint64_t)k;
             rc = use_tile_i8 ? launch_tile_i8_pass(h, acc, T, k, t0)
-                 : use_3d ? launch_tile3d_pass(h, acc, bits, k, t0)
+                 : use_3d ? launch_tile3d_pass(h, acc, bits, k, t0, use_jit)
                           : launch_tile_planes_pass(h, acc, T, bits, k, t0, use_jit);
             if (!rc && want_series)
                 rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);

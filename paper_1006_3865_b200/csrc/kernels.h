@@ -37,10 +37,11 @@ bool tile3d_supported(const ising_ctx* h, int T);
 size_t tile3d_bytes(const ising_ctx* h, bool bits);
 int launch_canon_to_3d(ising_ctx* h, bool bits, const int8_t* d_canon, void* d_tiles);
 int launch_3d_to_canon(ising_ctx* h, bool bits, const void* d_tiles, int8_t* d_canon);
-int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64_t t_first);
+int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64_t t_first, bool use_jit);
 
 // ---- planes_jit.cu: run-time specialisation of k_tile_planes on the threshold head bits (NVRTC) ----
-cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R);   // nullptr: not available
+cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R);
+cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3);   // nullptr: not available
 uint64_t planes_jit_compiled();
 const char* planes_jit_last_log();
 

@@ -10,6 +10,7 @@
 // for the life of the process.  libnvrtc is loaded with dlopen: when it is missing, or anything fails, the
 // caller falls back to the pre-compiled kernel with run-time threshold operands (same results, slower).
 #include <dlfcn.h>
+#include <stdlib.h>
 
 #include <map>
 #include <mutex>
@@ -23,9 +24,13 @@ namespace ising {
 
 namespace {
 
-// The device source, concatenated by build.py (philox.cuh + planes_common.cuh + tile_planes_device.cuh).
+// The device sources, concatenated by build.py: philox.cuh + planes_common.cuh + tile_planes_device.cuh (2D) and
+// philox.cuh + planes_common.cuh + tile3d_planes_device.cuh (3D).
 const char* const kJitSource =
 #include "jit_source.inc"
+    ;
+const char* const kJitSource3d =
+#include "jit_source3d.inc"
     ;
 
 typedef int nvrtcResult_t;
@@ -45,6 +50,7 @@ struct Nvrtc {
     bool ok = false;
 
     Nvrtc() {
+        if (getenv("ISING_NO_NVRTC")) return;          // testing aid: behave as if libnvrtc were not installed
         const char* names[] = {"libnvrtc.so.12", "libnvrtc.so", "/usr/local/cuda/lib64/libnvrtc.so.12", "/usr/local/cuda/lib64/libnvrtc.so"};
         for (const char* n : names) {
             lib = dlopen(n, RTLD_NOW | RTLD_LOCAL);
@@ -61,7 +67,7 @@ struct Nvrtc {
 
 struct JitState {
     std::mutex mu;
-    std::map<std::tuple<int, int, int, uint32_t, int, int>, cudaKernel_t> cache;   // nullptr = tried and failed
+    std::map<std::string, cudaKernel_t> cache;   // name expression + macros -> kernel; nullptr = tried and failed
     std::vector<cudaLibrary_t> libs;
     std::string last_log;
     uint64_t compiled = 0;
@@ -72,26 +78,22 @@ JitState& state() {
     return s;
 }
 
-cudaKernel_t compile_one(int T, bool bits, bool hasj, uint32_t hp, int B, int R, std::string& log) {
+cudaKernel_t compile_one(const char* source, const std::string& expr, const std::vector<std::string>& defs, std::string& log) {
     static Nvrtc rt;
     if (!rt.ok) { log = "libnvrtc not available"; return nullptr; }
-    char expr[160];
-    snprintf(expr, sizeof expr, "ising::jit::k_tile_planes<%d, %s, %s, %uu>", T, bits ? "true" : "false", hasj ? "true" : "false", hp);
     nvrtcProgram_t prog = nullptr;
-    if (rt.CreateProgram(&prog, kJitSource, "tile_planes_jit.cu", 0, nullptr, nullptr) != 0) { log = "nvrtcCreateProgram failed"; return nullptr; }
+    if (rt.CreateProgram(&prog, source, "ising_jit.cu", 0, nullptr, nullptr) != 0) { log = "nvrtcCreateProgram failed"; return nullptr; }
     cudaKernel_t kernel = nullptr;
     do {
-        if (rt.AddNameExpression(prog, expr) != 0) { log = "nvrtcAddNameExpression failed"; break; }
-        char defB[48], defR[48];                      // lattice geometry as constants: index arithmetic folds
-        snprintf(defB, sizeof defB, "-DISING_JIT_B=%uu", (unsigned)B);
-        snprintf(defR, sizeof defR, "-DISING_JIT_R=%uu", (unsigned)R);
-        const char* opts[] = {"--gpu-architecture=sm_100a", "--std=c++17", "--generate-line-info", defB, defR};
-        const nvrtcResult_t rc = rt.CompileProgram(prog, 5, opts);
+        if (rt.AddNameExpression(prog, expr.c_str()) != 0) { log = "nvrtcAddNameExpression failed"; break; }
+        std::vector<const char*> opts = {"--gpu-architecture=sm_100a", "--std=c++17", "--generate-line-info"};
+        for (const std::string& d : defs) opts.push_back(d.c_str());
+        const nvrtcResult_t rc = rt.CompileProgram(prog, (int)opts.size(), opts.data());
         size_t n = 0;
         if (rt.GetProgramLogSize(prog, &n) == 0 && n > 1) { log.resize(n); rt.GetProgramLog(prog, &log[0]); }
         if (rc != 0) break;
         const char* lowered = nullptr;
-        if (rt.GetLoweredName(prog, expr, &lowered) != 0 || !lowered) { log += " nvrtcGetLoweredName failed"; break; }
+        if (rt.GetLoweredName(prog, expr.c_str(), &lowered) != 0 || !lowered) { log += " nvrtcGetLoweredName failed"; break; }
         size_t sz = 0;
         if (rt.GetCUBINSize(prog, &sz) != 0 || sz == 0) { log += " no cubin"; break; }
         std::vector<char> cubin(sz);
@@ -113,21 +115,35 @@ cudaKernel_t compile_one(int T, bool bits, bool hasj, uint32_t hp, int B, int R,
     return kernel;
 }
 
-}  // namespace
-
-// The kernel specialised for (T, BITS, HASJ, HP) and the geometry (B tiles per side, R replicas), compiled on
-// first use; nullptr if it cannot be had.
-cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R) {
+cudaKernel_t cached(const char* source, const std::string& expr, const std::vector<std::string>& defs) {
     JitState& s = state();
     std::lock_guard<std::mutex> lock(s.mu);
-    const auto key = std::make_tuple(T, (int)bits, (int)hasj, hp, B, R);
+    std::string key = expr;
+    for (const std::string& d : defs) key += " " + d;
     auto it = s.cache.find(key);
     if (it != s.cache.end()) return it->second;
     std::string log;
-    cudaKernel_t k = compile_one(T, bits, hasj, hp, B, R, log);
+    cudaKernel_t k = compile_one(source, expr, defs, log);
     if (k) ++s.compiled; else s.last_log = log;
     s.cache[key] = k;
     return k;
+}
+
+}  // namespace
+
+// The 2D kernel specialised for (T, BITS, HASJ, HP) and the geometry (B tiles per side, R replicas), compiled on
+// first use; nullptr if it cannot be had.
+cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R) {
+    char expr[160];
+    snprintf(expr, sizeof expr, "ising::jit::k_tile_planes<%d, %s, %s, %uu>", T, bits ? "true" : "false", hasj ? "true" : "false", hp);
+    return cached(kJitSource, expr, {"-DISING_JIT_B=" + std::to_string(B) + "u", "-DISING_JIT_R=" + std::to_string(R) + "u"});
+}
+
+// The 3D kernel specialised for (BITS, HP3 = the three threshold heads).
+cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3) {
+    char expr[160];
+    snprintf(expr, sizeof expr, "ising::jit::k_tile3d_planes<%s, %lluull>", bits ? "true" : "false", hp3);
+    return cached(kJitSource3d, expr, {});
 }
 
 uint64_t planes_jit_compiled() { return state().compiled; }

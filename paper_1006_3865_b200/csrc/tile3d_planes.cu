@@ -18,220 +18,11 @@
 //          YL[8] bytes (row y=0: colour 0 pairs in bits 0-3, colour 1 in 4-7), YR[8] bytes (y=7),
 //          ZL 2 words (slice 0, colour 0 and 1), ZR 2 words (slice 7).
 #include "kernels.h"
-#include "planes_common.cuh"
+#include "tile3d_planes_device.cuh"
 
 namespace ising {
 
 namespace {
-
-constexpr int kT3 = 8;
-constexpr int kBody3I8 = 512, kBody3Bits = 64, kFaces3 = 96;
-constexpr int kRec3I8 = 640, kRec3Bits = 160;        // padded to multiples of 128 / 32 bytes
-constexpr int kXL = 0, kXR = 32, kYL = 64, kYR = 72, kZL = 80, kZR = 88;   // offsets inside the face area
-
-struct Plane3Args {
-    uint8_t* tiles;              // records, replica-major; tile (tz, ty, tx) at ((tz*B + ty)*B + tx)
-    const uint64_t* seeds;
-    int L, B, R;
-    int C;                       // coarse colour of this launch
-    int k;
-    uint64_t t_first;
-    uint32_t njobs;              // 4 tiles per job
-    uint32_t per_rep, per_z, hb; // tiles of one colour per replica (B^3/2), per tz (B*B/2), per ty (B/2)
-    uint32_t magic_rep, magic_z, magic_hb;
-    uint32_t u[3][kHeadBits];    // plane q: all-ones if bit (31-q) of thr[m+1] is set
-    uint32_t tail[3];            // thr[m+1] & (2^20 - 1)
-    uint32_t force;              // all-ones if beta = 0 (every thr = 2^32: every proposal is accepted)
-};
-
-struct Tile3 {
-    int r, tx, ty, tz;
-};
-
-__device__ __forceinline__ Tile3 job_tile3(const Plane3Args& A, uint32_t q) {
-    // colour-C tiles enumerated (tz, ty, txh): tx = 2*txh + ((ty + tz + C) & 1)
-    Tile3 t;
-    const uint32_t rr = fastdiv(q, A.per_rep, A.magic_rep);
-    uint32_t rem = q - rr * A.per_rep;
-    const uint32_t zz = fastdiv(rem, A.per_z, A.magic_z);
-    rem -= zz * A.per_z;
-    const uint32_t yy = fastdiv(rem, A.hb, A.magic_hb);
-    rem -= yy * A.hb;
-    t.r = (int)rr; t.tz = (int)zz; t.ty = (int)yy;
-    t.tx = (int)(2u * rem) + (((int)yy + (int)zz + A.C) & 1);
-    return t;
-}
-
-// What a lane keeps of its slice.
-struct Slice {
-    uint32_t S[2];        // the slice's two colour words
-    uint32_t xl, xr;      // halo bits x = -1 (at 4ly) and x = 8 (at 4ly+3), every row, either colour
-    uint32_t ym, yp;      // halo row y = -1 and y = 8: colour 0 pairs in bits 0-3, colour 1 in bits 4-7
-    uint32_t zm[2], zp[2];// lanes lz = 0 / 7: the slice below / above, by colour
-};
-
-template <bool BITS>
-__device__ __forceinline__ void load_slice(const Plane3Args& A, const Tile3& t, int lz, Slice& s) {
-    constexpr int REC = BITS ? kRec3Bits : kRec3I8;
-    constexpr int BODY = BITS ? kBody3Bits : kBody3I8;
-    const int B = A.B;
-    const uint8_t* rep = A.tiles + (size_t)t.r * B * B * B * REC;
-    auto rec_of = [&](int tz, int ty, int tx) { return rep + (((size_t)tz * B + ty) * B + tx) * REC; };
-    const uint8_t* rec = rec_of(t.tz, t.ty, t.tx);
-    const uint8_t* fXm = rec_of(t.tz, t.ty, t.tx == 0 ? B - 1 : t.tx - 1) + BODY;
-    const uint8_t* fXp = rec_of(t.tz, t.ty, t.tx == B - 1 ? 0 : t.tx + 1) + BODY;
-    const uint8_t* fYm = rec_of(t.tz, t.ty == 0 ? B - 1 : t.ty - 1, t.tx) + BODY;
-    const uint8_t* fYp = rec_of(t.tz, t.ty == B - 1 ? 0 : t.ty + 1, t.tx) + BODY;
-    if (BITS) {
-        s.S[0] = ldg32(rec + lz * 4);
-        s.S[1] = ldg32(rec + (8 + lz) * 4);
-    } else {
-        uint4 v[4];
-#pragma unroll
-        for (int c = 0; c < 4; ++c) v[c] = ldg128(rec + (c * 8 + lz) * 16, body_policy(false));
-        s.S[0] = pack16(pack16(0u, v[1]), v[0]);
-        s.S[1] = pack16(pack16(0u, v[3]), v[2]);
-    }
-    s.xl = __ldg(reinterpret_cast<const uint32_t*>(fXm + kXR) + lz);     // left tile's x = 7 sites, bit 4ly
-    s.xr = __ldg(reinterpret_cast<const uint32_t*>(fXp + kXL) + lz);     // right tile's x = 0 sites, bit 4ly+3
-    s.ym = __ldg(fYm + kYR + lz);                                        // tile in front: its row y = 7
-    s.yp = __ldg(fYp + kYL + lz);                                        // tile behind: its row y = 0
-    s.zm[0] = s.zm[1] = s.zp[0] = s.zp[1] = 0u;
-    if (lz == 0) {
-        const uint2 w = __ldg(reinterpret_cast<const uint2*>(rec_of(t.tz == 0 ? B - 1 : t.tz - 1, t.ty, t.tx) + BODY + kZR));
-        s.zm[0] = w.x; s.zm[1] = w.y;
-    }
-    if (lz == 7) {
-        const uint2 w = __ldg(reinterpret_cast<const uint2*>(rec_of(t.tz == B - 1 ? 0 : t.tz + 1, t.ty, t.tx) + BODY + kZL));
-        s.zp[0] = w.x; s.zp[1] = w.y;
-    }
-}
-
-// The slice's own face copies: the four words / bytes its x- and y-neighbours will read.
-__device__ __forceinline__ void face_words(const uint32_t (&S)[2], int lz, uint32_t& XL, uint32_t& XR, uint32_t& YL, uint32_t& YR) {
-    // x = 0 is pair 0 (bit 4ly) of colour (ly+lz)&1; x = 7 is pair 3 (bit 4ly+3) of colour (ly+lz+1)&1
-    const uint32_t ev = (lz & 1) ? 0x10101010u : 0x01010101u;            // bit 4ly of the rows with (ly+lz) even
-    const uint32_t od = (lz & 1) ? 0x08080808u : 0x80808080u;            // bit 4ly+3 of the rows with (ly+lz) odd
-    XL = ((S[0] & ev) | (S[1] & (0x11111111u ^ ev))) << 3;
-    XR = ((S[0] & od) | (S[1] & (0x88888888u ^ od))) >> 3;
-    YL = (S[0] & 0xfu) | ((S[1] & 0xfu) << 4);
-    YR = (S[0] >> 28) | ((S[1] >> 28) << 4);
-}
-
-template <bool BITS>
-__device__ __forceinline__ void store_slice(const Plane3Args& A, const Tile3& t, int lz, const Slice& s, const uint2* lut) {
-    constexpr int REC = BITS ? kRec3Bits : kRec3I8;
-    constexpr int BODY = BITS ? kBody3Bits : kBody3I8;
-    const int B = A.B;
-    uint8_t* rec = A.tiles + ((size_t)t.r * B * B * B + ((size_t)t.tz * B + t.ty) * B + t.tx) * REC;
-    if (BITS) {
-        *reinterpret_cast<uint32_t*>(rec + lz * 4) = s.S[0];
-        *reinterpret_cast<uint32_t*>(rec + (8 + lz) * 4) = s.S[1];
-    } else {
-#pragma unroll
-        for (int cc = 0; cc < 2; ++cc)
-#pragma unroll
-            for (int h = 0; h < 2; ++h) {
-                const uint2 a = __ldg(lut + ((s.S[cc] >> (16 * h)) & 0xffu));
-                const uint2 b = __ldg(lut + ((s.S[cc] >> (16 * h + 8)) & 0xffu));
-                stg128(rec + ((cc * 2 + h) * 8 + lz) * 16, make_uint4(a.x, a.y, b.x, b.y));
-            }
-    }
-    uint32_t XL, XR, YL, YR;
-    face_words(s.S, lz, XL, XR, YL, YR);
-    uint8_t* f = rec + BODY;
-    reinterpret_cast<uint32_t*>(f + kXL)[lz] = XL;
-    reinterpret_cast<uint32_t*>(f + kXR)[lz] = XR;
-    f[kYL + lz] = (uint8_t)YL;
-    f[kYR + lz] = (uint8_t)YR;
-    if (lz == 0) *reinterpret_cast<uint2*>(f + kZL) = make_uint2(s.S[0], s.S[1]);
-    if (lz == 7) *reinterpret_cast<uint2*>(f + kZR) = make_uint2(s.S[0], s.S[1]);
-}
-
-// R_m = [r < thr[m]], m = 1..3, and tie masks, for the 32 sites of block g (12 head planes).
-__device__ __forceinline__ void head_masks3(const Plane3Args& A, uint32_t g, uint32_t Hlo, uint32_t Hhi, uint32_t k0,
-                                            uint32_t k1, uint32_t (&R)[3], uint32_t (&eq)[3]) {
-    uint32_t bw[3] = {0u, 0u, 0u}, ne[3] = {0u, 0u, 0u};
-#pragma unroll
-    for (int n = kHeadBits / 4 - 1; n >= 0; --n) {                  // least significant planes first
-        const u32x4 o = philox4x32_10(g, kTagPlanes + 256u * n, Hlo, Hhi, k0, k1);
-        const uint32_t p[4] = {o.x, o.y, o.z, o.w};
-#pragma unroll
-        for (int w = 3; w >= 0; --w) {
-            const int q = 4 * n + w;
-#pragma unroll
-            for (int m = 0; m < 3; ++m) {
-                bw[m] = lop3<kLutChain>(p[w], bw[m], A.u[m][q]);
-                ne[m] = lop3<kLutNe>(ne[m], p[w], A.u[m][q]);
-            }
-        }
-    }
-#pragma unroll
-    for (int m = 0; m < 3; ++m) { R[m] = bw[m]; eq[m] = ~ne[m]; }
-}
-
-// One half-sweep of colour c on the lane's slice (a4-a5, 6 neighbours).
-__device__ __forceinline__ void half_sweep3(const Plane3Args& A, Slice& s, int c, int lz, uint32_t g, uint32_t p_base,
-                                            uint64_t H, uint32_t k0, uint32_t k1) {
-    const int o = 1 - c;
-    const uint32_t Hlo = (uint32_t)H, Hhi = (uint32_t)(H >> 32);
-    const uint32_t O = s.S[o], S = s.S[c];
-    uint32_t Zm = __shfl_up_sync(0xffffffffu, O, 1), Zp = __shfl_down_sync(0xffffffffu, O, 1);
-    if (lz == 0) Zm = s.zm[o];
-    if (lz == 7) Zp = s.zp[o];
-    const uint32_t Ym = (O << 4) | ((s.ym >> (4 * o)) & 0xfu);
-    const uint32_t Yp = (O >> 4) | (((s.yp >> (4 * o)) & 0xfu) << 28);
-    // rows where the active site is the left one of its pair (x = 2 p_x): ly = lz + c (mod 2); their second
-    // x-neighbour is pair p_x - 1, the other rows' is pair p_x + 1
-    const uint32_t m = ((lz + c) & 1) ? 0xf0f0f0f0u : 0x0f0f0f0fu;
-    const uint32_t X2 = ((((O << 1) & 0xeeeeeeeeu) | s.xl) & m) | ((((O >> 1) & 0x77777777u) | s.xr) & ~m);
-    uint32_t R[3], eq[3];
-    head_masks3(A, g, Hlo, Hhi, k0, k1, R, eq);
-    // disagreeing neighbours, pairwise counts, then thresholds of the sum of six
-    const uint32_t a = S ^ Zm, b = S ^ Zp, e = S ^ Ym, f = S ^ Yp, x = S ^ O, y = S ^ X2;
-    const uint32_t p1 = a | b, q1 = a & b, p2 = e | f, q2 = e & f, p3 = x | y, q3 = x & y;
-    const uint32_t ge1 = p1 | p2 | p3;
-    const uint32_t ge2 = q1 | q2 | q3 | (p1 & p2) | (p1 & p3) | (p2 & p3);
-    const uint32_t ge3 = (q1 & (p2 | p3)) | (q2 & (p1 | p3)) | (q3 & (p1 | p2)) | (p1 & p2 & p3) | A.force;   // dE <= 0: always flip
-    uint32_t und = (eq[0] & ge2 & ~ge3) | (eq[1] & ge1 & ~ge2) | (eq[2] & ~ge1);   // n_dis = 2, 1, 0 need thr[1], thr[2], thr[3]
-    while (und) {                                                   // probability 2^-12 per site
-        const int j = __ffs(und) - 1;
-        und &= und - 1;
-        const uint32_t p = p_base + (uint32_t)(j >> 2) * (uint32_t)(A.L >> 1) + (uint32_t)(j & 3);
-        const u32x4 t = philox4x32_10(p, kTagTail, Hlo, Hhi, k0, k1);
-        const uint32_t tail = t.x >> kHeadBits;
-#pragma unroll
-        for (int mm = 0; mm < 3; ++mm)
-            if ((eq[mm] >> j) & 1u) R[mm] |= (uint32_t)(tail < A.tail[mm]) << j;
-    }
-    const uint32_t flip = ge3 | (ge2 & R[0]) | (ge1 & R[1]) | R[2];   // thr[3] <= thr[2] <= thr[1]
-    s.S[c] = S ^ flip;
-}
-
-constexpr int kThreads3 = 64;        // 2 warps = 8 tiles per CTA: small CTAs so that config 4 (4096 warp jobs) fits one wave
-
-template <bool BITS>
-__global__ void __launch_bounds__(kThreads3) k_tile3d_planes(Plane3Args A) {
-    const uint2* lut = kByteLutGlobal.e;      // int8 write-back table, read-only path (planes_common.cuh)
-    const int lane = threadIdx.x & 31;
-    const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (job >= A.njobs) return;
-    const int sub = lane >> 3, lz = lane & 7;
-    const Tile3 t = job_tile3(A, job * 4u + (uint32_t)sub);
-    Slice s;
-    load_slice<BITS>(A, t, lz, s);
-    const uint64_t seed = A.seeds[t.r];
-    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
-    const uint32_t z = (uint32_t)(t.tz * kT3 + lz);
-    const uint32_t g = (z * (uint32_t)A.B + (uint32_t)t.ty) * (uint32_t)A.B + (uint32_t)t.tx;     // RNG block (S3.4)
-    const uint32_t p_base = (uint32_t)(t.tx * 4) + (uint32_t)(A.L >> 1) * ((uint32_t)(t.ty * kT3) + (uint32_t)A.L * z);
-    for (int j = 0; j < A.k; ++j) {
-        const uint64_t tt = A.t_first + (uint64_t)j;
-        half_sweep3(A, s, 0, lz, g, p_base, 2 * tt, k0, k1);
-        half_sweep3(A, s, 1, lz, g, p_base, 2 * tt + 1, k0, k1);
-    }
-    store_slice<BITS>(A, t, lz, s, lut);
-}
 
 // ---- layout converters (a11).  MODE 0/2: canonical -> int8 / bit records (face copies included; bit
 // fields by atomicOr into zeroed storage), MODE 1/3: records -> canonical.  One thread per site.
@@ -305,7 +96,7 @@ int launch_3d_to_canon(ising_ctx* h, bool bits, const void* d_tiles, int8_t* d_c
 }
 
 // a1: one outer pass = colour-0 launch, colour-1 launch, k inner sweeps each.
-int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64_t t_first) {
+int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64_t t_first, bool use_jit) {
     Plane3Args A;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_seeds;
@@ -321,10 +112,23 @@ int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64
     A.force = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
     const int warps = kThreads3 / 32;
     const uint32_t grid = (A.njobs + warps - 1) / warps;
+    // specialised on the three threshold heads (planes_jit.cu) when asked for and available
+    const unsigned long long hp3 = ((unsigned long long)(acc.thr[0] >> kTailBits) << 24) |
+                                   ((unsigned long long)(acc.thr[1] >> kTailBits) << 12) | (unsigned long long)(acc.thr[2] >> kTailBits);
+    cudaKernel_t spec = (use_jit && !A.force) ? planes3d_jit_kernel(bits, hp3) : nullptr;
+    h->last_jit = spec ? 1 : 0;
     for (int C = 0; C < 2; ++C) {
         A.C = C;
-        if (bits) k_tile3d_planes<true><<<grid, warps * 32, 0, hooks().stream>>>(A);
-        else k_tile3d_planes<false><<<grid, warps * 32, 0, hooks().stream>>>(A);
+        if (spec) {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(grid); cfg.blockDim = dim3(warps * 32); cfg.stream = hooks().stream;
+            void* args[] = {&A};
+            ISING_CUDA_OK(cudaLaunchKernelExC(&cfg, (const void*)spec, args));
+        } else if (bits) {
+            k_tile3d_planes<true><<<grid, warps * 32, 0, hooks().stream>>>(A);
+        } else {
+            k_tile3d_planes<false><<<grid, warps * 32, 0, hooks().stream>>>(A);
+        }
         count_launch();
     }
     ISING_CUDA_OK(cudaGetLastError());

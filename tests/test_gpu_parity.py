@@ -205,6 +205,40 @@ def test_specialised_kernel_matches_oracle(P, orc, L, tile, k, n, beta, seeds, j
     _same_state(g, o)
 
 
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,k,n,beta,seeds", [(32, 2, 3, BC3, [4]), (48, 1, 3, 0.3, [5, 6]), (64, 1, 2, BC3, [9]), (32, 2, 2, 9.0, [2])])
+def test_specialised_3d_kernel_matches_oracle(P, orc, L, k, n, beta, seeds, layout):
+    """The 3D kernel specialised at run time on its three threshold heads, against the oracle."""
+    g, o = _both(P, orc, 3, L, seeds, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.set_jit("on")
+    Eg, Mg = g.sweep_series(beta, n, 8, k)
+    assert g.last_sweep_specialized()
+    Eo, Mo = o.sweep_series(beta, n, 8, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+
+
+def test_missing_nvrtc_falls_back_to_the_precompiled_kernel():
+    """With libnvrtc unavailable (simulated by ISING_NO_NVRTC in a fresh process) ising_set_jit(ON) still sweeps, on the
+    pre-compiled kernel, and still matches the oracle: the fallback is another CUDA kernel, never a CPU path."""
+    import os, subprocess, sys
+    code = (
+        "import numpy as np, paper_1006_3865_b200 as P\n"
+        "from oracle import oracle as O\n"
+        "P.use_torch()\n"
+        "g = P.Ising(2, 128, seed=5); o = O.Oracle(2, 128, seed=5)\n"
+        "g.set_jit('on'); g.sweep(0.44, 3, 32, 2); o.sweep(0.44, 3, 32, 2)\n"
+        "assert not g.last_sweep_specialized() and g.sweep_path() == 'tile_planes_i8'\n"
+        "assert np.array_equal(g.copy_spins(), o.spins())\n"
+        "print('fallback ok')\n")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, ISING_NO_NVRTC="1"),
+                         capture_output=True, text=True, timeout=600)
+    assert out.returncode == 0 and "fallback ok" in out.stdout, out.stderr[-2000:]
+
+
 @pytest.mark.parametrize("L,tile,k,n,beta,seeds", TILED)
 def test_tile_i8_path_matches_oracle(P, orc, L, tile, k, n, beta, seeds):
     g, o = _both(P, orc, 2, L, seeds, rng="words")
