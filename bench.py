@@ -216,6 +216,39 @@ def time_e2e(P, torch, L, layout, tile, k, steps, rng="planes"):
             "d2h_bytes_per_step": L * L, "steps": steps}
 
 
+def run_config(P, torch, a) -> None:
+    """Device-timed flips/ns of another BASELINE.json config (1, 2, 4, 5; config 3 is the default run), planes
+    mapping, int8 records unless --layout bits.  One JSON line per (k or beta) variant of the config."""
+    c = W.CONFIGS[a.config]
+    dim, L = c["dim"], c["L"]
+    seeds = list(c.get("seeds", [c.get("seed")]))
+    J = W.couplings(dim, L, c["jseed"]) if "jseed" in c else None
+    variants = [(c["beta"], k) for k in c.get("ks", [c.get("k")])] if "beta" in c else [(b, c["k"]) for b in c["betas"]]
+    for beta, k in variants:
+        g = P.Ising(dim, L, coupling=J, seeds=seeds, rng=a.rng)
+        g.set_jit(JIT)
+        if a.layout == "bits":
+            g.set_layout(P.ISING_LAYOUT_BITS)
+        n = max(4, min(c["n"], a.steps if a.steps != 50 else c["n"], int(4e10 / (k * len(seeds) * L ** dim))))
+        g.sweep(beta, max(a.warmup, min(n, -(-(1 << 27) // (k * len(seeds) * L ** dim)))), c["tile"], k)   # warm-up also compiles
+        g.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n0 = P.ising_kernel_launches()
+        e0.record()
+        g.sweep(beta, n, c["tile"], k)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        flips = n * k * len(seeds) * L ** dim
+        print(json.dumps({"metric": f"spin flips/ns (BASELINE config {a.config})", "value": flips / (ms * 1e6), "unit": UNIT,
+                          "n_gpus": 1, "steps": n, "ms_per_step": ms / n, "higher_is_better": True, "dtype": "u8" if a.layout == "int8" else "u32 bit-planes",
+                          "data": "synthetic", "gpu_launches": int(P.ising_kernel_launches() - n0),
+                          "config": {"workload": f"BASELINE config {a.config}: dim={dim} L={L} replicas={len(seeds)} J={'+-1 (jseed %d)' % c['jseed'] if J is not None else '+1'} "
+                                                 f"beta={beta} tile={c['tile']} k={k} layout={a.layout} rng={a.rng}",
+                                     "kernel_path": g.sweep_path() + ("+jit" if g.last_sweep_specialized() else "")}}), flush=True)
+        g.destroy()
+
+
 def run_lscan(P, torch, a) -> None:
     """flips/ns against L in the style of the paper's Fig. 3, planes mapping, int8 records."""
     rows = []
@@ -269,6 +302,7 @@ def main() -> None:
     ap.add_argument("--L", type=int, default=16384)
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the k/tile table")
     ap.add_argument("--jit", default="auto", choices=["auto", "on", "off"], help="run-time kernel specialisation (ising_set_jit)")
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5], help="time another BASELINE config (default 3 = the headline run)")
     ap.add_argument("--lscan", action="store_true", help="study: flips/ns against L (SURVEY 8(f)-3)")
     ap.add_argument("--autocorr", action="store_true", help="study: autocorrelation time against k (SURVEY 8(f)-2)")
     ap.add_argument("--selftest-ranks", action="store_true", help="CPU/gloo check of the multi-rank aggregation, no GPU")
@@ -299,6 +333,9 @@ def main() -> None:
     L = a.L
     if a.lscan or a.autocorr:
         (run_lscan if a.lscan else run_autocorr)(P, torch, a)
+        return
+    if a.config != 3:
+        run_config(P, torch, a)
         return
 
     def barrier():
