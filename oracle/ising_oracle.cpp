@@ -91,6 +91,12 @@ struct Oracle {
     bool has_J = false;
     std::vector<int8_t> J;           // J[d*N + i] = bond from site i to i + e_d (S8b)
     std::vector<uint64_t> seeds;     // one Philox key per replica
+    // Asynchronous multi-spin coding batch (DESIGN.md §3.6 R17): every replica is its own disorder
+    // realisation (own couplings J[r][d][i], own hot start from seeds[r]) but all draw the SAME sweep random
+    // r(i, H), keyed by sweep_seed.  Each replica is then an ordinary run whose random stream happens to be shared.
+    bool J_per_replica = false;
+    bool shared_sweep = false;
+    uint64_t sweep_seed = 0;
     std::vector<int8_t> s;           // s[r*N + i], canonical order i = x + L*(y + L*z) (S8c.1)
     uint64_t t = 0;                  // inner sweeps done so far (S8c.6)
     int reverse_tiles = 0;           // test hook: visit the tiles of a colour in reverse order
@@ -219,14 +225,15 @@ void update_site(Oracle& o, int r, int x, int y, int z, uint64_t H, const uint64
     int8_t* s = o.s.data() + (uint64_t)r * o.N;
     const uint64_t i = site_index(o, x, y, z);
     const int coord[3] = {x, y, z};
+    const int8_t* Jr = o.J.data() + (o.J_per_replica ? (uint64_t)r * o.dim * o.N : 0);
     uint64_t stride = 1;  // index distance of one step along e_d: 1, L, L^2 (S8c.1)
     int field = 0;
     for (int d = 0; d < o.dim; ++d) {
         // periodic neighbours i + e_d and i - e_d
         const uint64_t ip = (coord[d] == o.L - 1) ? i - (uint64_t)(o.L - 1) * stride : i + stride;
         const uint64_t im = (coord[d] == 0) ? i + (uint64_t)(o.L - 1) * stride : i - stride;
-        const int Jp = o.has_J ? o.J[(uint64_t)d * o.N + i] : 1;    // bond i -> i+e_d
-        const int Jm = o.has_J ? o.J[(uint64_t)d * o.N + im] : 1;   // bond (i-e_d) -> i
+        const int Jp = o.has_J ? Jr[(uint64_t)d * o.N + i] : 1;     // bond i -> i+e_d
+        const int Jm = o.has_J ? Jr[(uint64_t)d * o.N + im] : 1;    // bond (i-e_d) -> i
         field += Jp * s[ip] + Jm * s[im];
         stride *= (uint64_t)o.L;
     }
@@ -235,8 +242,8 @@ void update_site(Oracle& o, int r, int x, int y, int z, uint64_t H, const uint64
     if (a <= 0) {
         flip = true;
     } else {
-        const uint64_t rnd = (o.rng == RNG_PLANES) ? sweep_random_planes(o, o.seeds[r], i, H)
-                                                   : sweep_random(o, o.seeds[r], i, H);
+        const uint64_t key = o.shared_sweep ? o.sweep_seed : o.seeds[r];
+        const uint64_t rnd = (o.rng == RNG_PLANES) ? sweep_random_planes(o, key, i, H) : sweep_random(o, key, i, H);
         flip = rnd < thr[a / 2];
     }
     if (flip) s[i] = (int8_t)-s[i];
@@ -267,7 +274,7 @@ void observables(const Oracle& o, int r, int64_t* E, int64_t* M) {
                     int cp[3] = {x, y, z};
                     cp[d] = wrap(c[d] + 1, o.L);
                     const uint64_t ip = site_index(o, cp[0], cp[1], cp[2]);
-                    const int Jp = o.has_J ? o.J[(uint64_t)d * o.N + i] : 1;
+                    const int Jp = o.has_J ? o.J[(o.J_per_replica ? (uint64_t)r * o.dim * o.N : 0) + (uint64_t)d * o.N + i] : 1;
                     e -= Jp * s[i] * s[ip];
                 }
             }
@@ -374,6 +381,23 @@ void* oracle_create_batch(int dim, int L, const int8_t* J, const uint64_t* seeds
     return o;
 }
 
+// Multi-realisation batch with shared sweep randoms (asynchronous multi-spin coding; R17): J = R*dim*N
+// couplings (realisation-major), init_seeds[r] = hot start of realisation r, sweep_seed = key of the shared r(i, H).
+void* oracle_create_multi(int dim, int L, const int8_t* J, const uint64_t* init_seeds, int R, uint64_t sweep_seed) {
+    if ((dim != 2 && dim != 3) || L < 2 || (L & 1) || R < 1 || !J) return nullptr;
+    Oracle* o = new Oracle;
+    o->dim = dim; o->L = L; o->R = R;
+    o->N = 1;
+    for (int d = 0; d < dim; ++d) o->N *= (uint64_t)L;
+    o->has_J = true; o->J_per_replica = true; o->shared_sweep = true; o->sweep_seed = sweep_seed;
+    o->J.assign(J, J + (uint64_t)R * dim * o->N);
+    for (int8_t v : o->J) if (v != 1 && v != -1) { delete o; return nullptr; }
+    o->seeds.assign(init_seeds, init_seeds + R);
+    o->s.resize((uint64_t)R * o->N);
+    for (int r = 0; r < R; ++r) hot_start(o->s.data() + (uint64_t)r * o->N, o->N, init_seeds[r]);
+    return o;
+}
+
 void* oracle_create(int dim, int L, const int8_t* J, uint64_t seed) {
     return oracle_create_batch(dim, L, J, &seed, 1);
 }
@@ -433,7 +457,8 @@ int oracle_set_memo(void* h, int on) { ((Oracle*)h)->use_memo = on ? 1 : 0; retu
 // the 32-bit random of (replica r, site i, half-sweep H) under the handle's current mapping
 uint32_t oracle_sweep_random(void* h, int r, uint64_t i, uint64_t H) {
     Oracle& o = *(Oracle*)h;
-    return (o.rng == RNG_PLANES) ? sweep_random_planes(o, o.seeds[r], i, H) : sweep_random(o, o.seeds[r], i, H);
+    const uint64_t key = o.shared_sweep ? o.sweep_seed : o.seeds[r];
+    return (o.rng == RNG_PLANES) ? sweep_random_planes(o, key, i, H) : sweep_random(o, key, i, H);
 }
 int oracle_set_tile_order(void* h, int reversed) { ((Oracle*)h)->reverse_tiles = reversed; return 0; }
 

@@ -43,6 +43,8 @@ def lib() -> C.CDLL:
         L.oracle_create.argtypes = [C.c_int, C.c_int, i8p, C.c_uint64]
         L.oracle_create_batch.restype = C.c_void_p
         L.oracle_create_batch.argtypes = [C.c_int, C.c_int, i8p, u64p, C.c_int]
+        L.oracle_create_multi.restype = C.c_void_p
+        L.oracle_create_multi.argtypes = [C.c_int, C.c_int, i8p, u64p, C.c_int, C.c_uint64]
         L.oracle_destroy.argtypes = [C.c_void_p]
         L.oracle_sweep.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_int, C.c_int]
         L.oracle_sweep_series.argtypes = [C.c_void_p, C.c_double, C.c_int, C.c_int, C.c_int, i64p, i64p]
@@ -105,7 +107,7 @@ class Oracle:
     rng: "planes" (default, the product's default mapping) or "words" (SURVEY S8c.3 verbatim)."""
 
     def __init__(self, dim: int, L: int, seed=None, J: np.ndarray | None = None, seeds=None,
-                 rng: str | None = None):
+                 rng: str | None = None, sweep_seed: int | None = None):
         if seeds is None:
             seeds = [seed]
         self.dim, self.L, self.N, self.R = dim, L, L ** dim, len(seeds)
@@ -113,9 +115,14 @@ class Oracle:
         jp = None
         if J is not None:
             J = np.ascontiguousarray(J, dtype=np.int8).reshape(-1)
-            assert J.size == dim * self.N
+            assert J.size == dim * self.N or (sweep_seed is not None and J.size == self.R * dim * self.N)
             jp = _p(J, C.c_int8)
-        self._h = lib().oracle_create_batch(dim, L, jp, _p(sd, C.c_uint64), self.R)
+        if sweep_seed is not None:      # multi-realisation batch: J holds R coupling arrays, sweep randoms shared (R17)
+            J = np.ascontiguousarray(J, dtype=np.int8).reshape(-1)
+            assert J.size == self.R * dim * self.N
+            self._h = lib().oracle_create_multi(dim, L, _p(J, C.c_int8), _p(sd, C.c_uint64), self.R, sweep_seed)
+        else:
+            self._h = lib().oracle_create_batch(dim, L, jp, _p(sd, C.c_uint64), self.R)
         if not self._h:
             raise ValueError("oracle_create_batch rejected its arguments")
         rng = DEFAULT_RNG if rng is None else rng

@@ -274,3 +274,22 @@ def test_hot_start_is_unbiased_and_seeded(orc):
     assert not np.array_equal(s, orc.Oracle(2, 256, seed=123456789012346).spins())
     # hi word of the seed is part of the key
     assert not np.array_equal(orc.Oracle(2, 8, seed=1).spins(), orc.Oracle(2, 8, seed=1 + 2 ** 32).spins())
+
+
+def test_multi_realisation_batch_is_R_ordinary_runs_with_a_shared_random_stream(orc, both_rngs):
+    """Asynchronous multi-spin coding batch (R17): realisation r of a multi batch = an ordinary
+    single run with couplings J[r], started from the hot start of seeds[r], whose sweep key is the shared one."""
+    dim, L, R, K = 2, 16, 3, 777
+    Js = np.stack([W.couplings(dim, L, 50 + r) for r in range(R)])
+    seeds = [11, 12, 13]
+    m = orc.Oracle(dim, L, seeds=seeds, J=Js, sweep_seed=K)
+    m.sweep(0.9, 4, 4, 2)
+    for r in range(R):
+        start = orc.Oracle(dim, L, seed=seeds[r]).spins()                 # hot start of seeds[r]
+        single = orc.Oracle(dim, L, seed=K, J=Js[r])                      # sweep key K, couplings J[r]
+        single.set_spins(start)
+        single.sweep(0.9, 4, 4, 2)
+        assert np.array_equal(m.spins()[r], single.spins())
+        assert int(m.observables()[0][r]) == int(single.observables()[0][0])
+    # shared randoms: the same site of two realisations sees the same r(i, H)
+    assert m.sweep_random(5, 3, r=0) == m.sweep_random(5, 3, r=2)
