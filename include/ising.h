@@ -68,6 +68,17 @@ ising_handle ising_create(int dim, int L, const int8_t* coupling_or_null, uint64
 ising_handle ising_create_batch(int dim, int L, const int8_t* coupling_or_null,
                                 const uint64_t* seeds, int n_replicas);
 
+/* ising_create_multi — P:100 ("asynchronous multi-spin coding", many disorder realisations at once); DESIGN.md
+ * §3.6 R17.  R >= 1 realisations of the +-J model, each with its own couplings (couplings = int8 J[R][dim][N],
+ * [host|device]) and its own hot start (init_seeds[r], host pointer), all driven by ONE sweep random stream
+ * r(i, H) keyed by sweep_seed: realisation r is exactly an ordinary run with couplings J[r] whose random stream
+ * happens to be shared with the others.  Everything else (sweep, observables per realisation, copy_spins R*N bytes,
+ * overlap) is as for ising_create_batch.  The RNG mapping of a multi handle starts as ISING_RNG_WORDS (one random
+ * word per site serves all realisations); with it, dim 2, n_realisations <= 32 and tile 32 / 64 the sweep runs on
+ * the multi-spin-coded kernel (32 realisations per machine word). */
+ising_handle ising_create_multi(int dim, int L, const int8_t* couplings, const uint64_t* init_seeds, int n_realisations,
+                                uint64_t sweep_seed);
+
 void ising_destroy(ising_handle h);
 
 /* ising_sweep — P:64-74 (steps 1-7 and the k-fold multi-hit); S8c.4-6.

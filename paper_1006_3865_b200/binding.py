@@ -22,7 +22,7 @@ ISING_RNG_PLANES = 1
 RNG_MODES = {"words": ISING_RNG_WORDS, "planes": ISING_RNG_PLANES}
 
 SYMBOLS = [
-    "ising_create", "ising_create_batch", "ising_destroy", "ising_sweep", "ising_sweep_series",
+    "ising_create", "ising_create_batch", "ising_create_multi", "ising_destroy", "ising_sweep", "ising_sweep_series",
     "ising_observables", "ising_overlap", "ising_copy_spins", "ising_set_spins", "ising_set_layout", "ising_set_rng", "ising_set_jit", "ising_last_sweep_specialized",
     "ising_get_counter", "ising_set_counter", "ising_thresholds", "ising_set_device_hooks",
     "ising_synchronize", "ising_kernel_launches", "ising_sweep_path", "ising_force_path",
@@ -55,6 +55,8 @@ def lib() -> C.CDLL:
     L.ising_create.argtypes = [C.c_int, C.c_int, i8p, C.c_uint64]
     L.ising_create_batch.restype = vp
     L.ising_create_batch.argtypes = [C.c_int, C.c_int, i8p, u64p, C.c_int]
+    L.ising_create_multi.restype = vp
+    L.ising_create_multi.argtypes = [C.c_int, C.c_int, i8p, u64p, C.c_int, C.c_uint64]
     L.ising_destroy.restype = None
     L.ising_destroy.argtypes = [vp]
     L.ising_sweep.argtypes = [vp, C.c_double, C.c_int, C.c_int, C.c_int]
@@ -136,14 +138,17 @@ class Ising:
     """Owner of one `ising_handle`; methods are the C calls of include/ising.h minus the prefix."""
 
     def __init__(self, dim: int, L: int, coupling=None, seed: int | None = None, seeds=None,
-                 rng: str | None = None):
+                 rng: str | None = None, sweep_seed: int | None = None):
         if seeds is None:
             seeds = [0 if seed is None else seed]
         sd = np.asarray(list(seeds), dtype=np.uint64)
         self.dim, self.L, self.N, self.R = dim, L, L ** dim, len(sd)
         if coupling is not None and isinstance(coupling, np.ndarray):
             coupling = np.ascontiguousarray(coupling, dtype=np.int8).reshape(-1)
-        self._h = lib().ising_create_batch(dim, L, _ptr(coupling), _ptr(sd), self.R)
+        if sweep_seed is not None:      # ising_create_multi: coupling holds R arrays, sweep randoms shared
+            self._h = lib().ising_create_multi(dim, L, _ptr(coupling), _ptr(sd), self.R, int(sweep_seed))
+        else:
+            self._h = lib().ising_create_batch(dim, L, _ptr(coupling), _ptr(sd), self.R)
         if not self._h:
             raise IsingError(f"ising_create failed: {lib().ising_last_error().decode()}")
         if rng is not None:

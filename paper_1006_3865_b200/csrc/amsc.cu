@@ -1,0 +1,190 @@
+// amsc.cu — asynchronous multi-spin coding for the 2D +-J model (DESIGN.md §3.6 R17, §6.5).
+//
+// Up to 32 disorder realisations are simulated at once: bit r of the 32-bit word at site i is the spin of
+// realisation r, bit r of JX[i] / JY[i] says that realisation r's bond i -> i+e_x / i+e_y is J = -1.  A site is
+// updated for all realisations with a dozen bitwise operations, and — the point of the method — with ONE random
+// number r(i, H) (RNG mapping "words": one Philox4x32-10 output word per site, S8c.3), so the cost of the random
+// numbers, which dominates everything else in this library, is shared 32 ways.  Each realisation is exactly an
+// ordinary run of the oracle with its own couplings and the shared random stream (R17).
+//
+// Schedule: the double checkerboard of P:62-74 unchanged.  One CTA per tile: the tile, its halo and the bonds that
+// touch it are staged in shared memory (coalesced row loads), k x {even sites, barrier, odd sites, barrier}, write
+// back.  A thread owns 8 consecutive columns of one row, i.e. the 4 same-colour sites that share one Philox call.
+#include "kernels.h"
+#include "philox.cuh"
+
+namespace ising {
+
+namespace {
+
+struct AmscArgs {
+    uint32_t* spins;             // word lattice, site order i = x + L*y
+    const uint32_t* jx;          // bond i -> i+e_x, bit r set <=> J = -1 for realisation r
+    const uint32_t* jy;          // bond i -> i+e_y
+    int L, B;
+    int C;                       // coarse colour of this launch
+    int k;
+    uint64_t t_first;
+    uint32_t k0, k1;             // the shared sweep key
+    uint32_t thr1, thr2;         // thresholds for dE = 4, 8
+    uint32_t all1, all2;         // all-ones if the threshold is 2^32 (beta = 0)
+    uint32_t rmask;              // bits of the realisations in use
+};
+
+template <int T>
+__global__ void __launch_bounds__(T * T / 8) k_amsc(AmscArgs A) {
+    constexpr int P = T + 2;                       // pitch of the spin image (halo all round)
+    extern __shared__ uint32_t smem[];
+    uint32_t* S = smem;                            // (T+2)^2 spin words
+    uint32_t* JX = S + P * P;                      // column -1 .. T-1 of every tile row: JX[y][x+1]
+    uint32_t* JY = JX + T * (T + 1);               // row -1 .. T-1: JY[y+1][x]
+    const int L = A.L, B = A.B;
+    // colour-C tiles row by row: q -> ty = q / (B/2), tx = 2*(q % (B/2)) + ((ty + C) & 1)
+    const int hb = B >> 1;
+    const int ty = blockIdx.x / hb, tx = 2 * (blockIdx.x % hb) + ((ty + A.C) & 1);
+    const int x0 = tx * T, y0 = ty * T;
+    const int tid = threadIdx.x, nthr = T * T / 8;
+    // a3: stage.  Rows -1 .. T of the spins (T + 2 words each, periodic), bonds of the tile and of its left / upper rim.
+    for (int idx = tid; idx < P * P; idx += nthr) {
+        const int yy = idx / P - 1, xx = idx % P - 1;
+        const int gy = (y0 + yy + L) % L, gx = (x0 + xx + L) % L;
+        S[idx] = A.spins[(size_t)gy * L + gx];
+    }
+    for (int idx = tid; idx < T * (T + 1); idx += nthr) {
+        const int yy = idx / (T + 1), xx = idx % (T + 1) - 1;
+        JX[idx] = A.jx[(size_t)(y0 + yy) * L + (x0 + xx + L) % L];
+    }
+    for (int idx = tid; idx < (T + 1) * T; idx += nthr) {
+        const int yy = idx / T - 1, xx = idx % T;
+        JY[idx] = A.jy[(size_t)((y0 + yy + L) % L) * L + (x0 + xx)];
+    }
+    __syncthreads();
+    const int y = tid / (T / 8), g = tid % (T / 8);                  // row and 8-column group of this thread
+    // Philox group of the thread's 4 same-colour sites: p = i >> 1 = Y*(L/2) + X/2, group = p >> 2 (S8c.3)
+    const uint32_t grp = (uint32_t)(((size_t)(y0 + y) * (L >> 1) + (x0 >> 1)) >> 2) + (uint32_t)g;
+    for (int j = 0; j < A.k; ++j) {
+        const uint64_t tt = A.t_first + (uint64_t)j;
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            const uint64_t H = 2 * tt + (uint64_t)c;
+            const u32x4 rnd = philox4x32_10(grp, kTagSweep, (uint32_t)H, (uint32_t)(H >> 32), A.k0, A.k1);
+            const uint32_t r4[4] = {rnd.x, rnd.y, rnd.z, rnd.w};
+            const int par = (y + c) & 1;                               // y0 and x0 are even: local parity = global parity
+#pragma unroll
+            for (int m = 0; m < 4; ++m) {
+                const int x = 8 * g + 2 * m + par;
+                const uint32_t s = S[(y + 1) * P + x + 1];
+                const uint32_t a = s ^ S[y * P + x + 1] ^ JY[y * T + x];               // up: bond (y-1) -> y
+                const uint32_t b = s ^ S[(y + 2) * P + x + 1] ^ JY[(y + 1) * T + x];   // down: bond y -> y+1
+                const uint32_t cc = s ^ S[(y + 1) * P + x] ^ JX[y * (T + 1) + x];      // left: bond (x-1) -> x
+                const uint32_t d = s ^ S[(y + 1) * P + x + 2] ^ JX[y * (T + 1) + x + 1];   // right
+                const uint32_t p1 = a | b, q1 = a & b, p2 = cc | d, q2 = cc & d;
+                const uint32_t ge1 = p1 | p2, ge2 = (p1 & p2) | q1 | q2;               // unsatisfied bonds >= 1, >= 2
+                const uint32_t R1 = (r4[m] < A.thr1 ? 0xffffffffu : 0u) | A.all1;      // the same r for every realisation
+                const uint32_t R2 = (r4[m] < A.thr2 ? 0xffffffffu : 0u) | A.all2;
+                const uint32_t flip = (ge2 | (ge1 & R1) | R2) & A.rmask;               // dE <= 0, dE = 4, dE = 8 (eq. (2))
+                S[(y + 1) * P + x + 1] = s ^ flip;
+            }
+            __syncthreads();
+        }
+    }
+    // a7: write the interior back, coalesced rows
+    for (int idx = tid; idx < T * T; idx += nthr) {
+        const int yy = idx / T, xx = idx % T;
+        A.spins[(size_t)(y0 + yy) * L + (x0 + xx)] = S[(yy + 1) * P + xx + 1];
+    }
+}
+
+// canonical int8 +-1 (R*N, realisation-major) <-> word lattice; couplings J[R][2][N] -> JX, JY words.
+__global__ void k_amsc_pack(const int8_t* __restrict__ canon, uint32_t* __restrict__ words, uint64_t N, int R, int negative) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    uint32_t w = 0;
+    for (int r = 0; r < R; ++r) {
+        const int8_t v = canon[(uint64_t)r * N + i];
+        w |= (uint32_t)(negative ? v < 0 : v > 0) << r;
+    }
+    words[i] = w;
+}
+__global__ void k_amsc_pack_J(const int8_t* __restrict__ J, uint32_t* __restrict__ jx, uint32_t* __restrict__ jy, uint64_t N, int R) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    uint32_t wx = 0, wy = 0;
+    for (int r = 0; r < R; ++r) {
+        wx |= (uint32_t)(J[((uint64_t)r * 2 + 0) * N + i] < 0) << r;
+        wy |= (uint32_t)(J[((uint64_t)r * 2 + 1) * N + i] < 0) << r;
+    }
+    jx[i] = wx; jy[i] = wy;
+}
+__global__ void k_amsc_unpack(const uint32_t* __restrict__ words, int8_t* __restrict__ canon, uint64_t N, int R) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const uint32_t w = words[i];
+    for (int r = 0; r < R; ++r) canon[(uint64_t)r * N + i] = ((w >> r) & 1u) ? 1 : -1;
+}
+
+}  // namespace
+
+bool amsc_supported(const ising_ctx* h, int T) {
+    if (h->dim != 2 || !h->J_per_replica || !h->shared_sweep || h->rng != ISING_RNG_WORDS || h->R > 32) return false;
+    if (T != 32 && T != 64) return false;
+    if (h->L % T) return false;
+    const int B = h->L / T;
+    return B >= 2 && (B % 2 == 0);
+}
+
+size_t amsc_spin_bytes(const ising_ctx* h) { return (size_t)h->N * 4; }
+
+// J word lattices (2 * N words), built once per handle.
+int launch_amsc_pack_J(ising_ctx* h, void* d_jwords) {
+    uint32_t* jx = (uint32_t*)d_jwords;
+    k_amsc_pack_J<<<(unsigned)((h->N + 255) / 256), 256, 0, hooks().stream>>>(h->d_J, jx, jx + h->N, h->N, h->R);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+int launch_canon_to_amsc(ising_ctx* h, const int8_t* d_canon, void* d_words) {
+    k_amsc_pack<<<(unsigned)((h->N + 255) / 256), 256, 0, hooks().stream>>>(d_canon, (uint32_t*)d_words, h->N, h->R, 0);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+int launch_amsc_to_canon(ising_ctx* h, const void* d_words, int8_t* d_canon) {
+    k_amsc_unpack<<<(unsigned)((h->N + 255) / 256), 256, 0, hooks().stream>>>((const uint32_t*)d_words, d_canon, h->N, h->R);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+// a1: one outer pass = colour-0 launch, colour-1 launch, k inner sweeps each.
+int launch_amsc_pass(ising_ctx* h, const Accept& acc, int T, int k, uint64_t t_first, const void* d_jwords) {
+    AmscArgs A;
+    A.spins = (uint32_t*)h->d_tiles;
+    A.jx = (const uint32_t*)d_jwords;
+    A.jy = A.jx + h->N;
+    A.L = h->L; A.B = h->L / T; A.k = k; A.t_first = t_first;
+    A.k0 = (uint32_t)h->sweep_seed; A.k1 = (uint32_t)(h->sweep_seed >> 32);
+    A.thr1 = acc.thr[0]; A.thr2 = acc.thr[1];
+    A.all1 = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
+    A.all2 = acc.thr_is_2p32[1] ? 0xffffffffu : 0u;
+    A.rmask = h->R >= 32 ? 0xffffffffu : ((1u << h->R) - 1u);
+    const unsigned grid = (unsigned)(A.B * A.B / 2);
+    const size_t smem = sizeof(uint32_t) * (size_t)((T + 2) * (T + 2) + 2 * T * (T + 1));   // 13 KB (T = 32), 50.7 KB (T = 64)
+    static bool attr_set = false;
+    if (!attr_set) {
+        ISING_CUDA_OK(cudaFuncSetAttribute(k_amsc<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
+        attr_set = true;
+    }
+    for (int C = 0; C < 2; ++C) {
+        A.C = C;
+        if (T == 64) k_amsc<64><<<grid, 64 * 64 / 8, smem, hooks().stream>>>(A);
+        else k_amsc<32><<<grid, 32 * 32 / 8, smem, hooks().stream>>>(A);
+        count_launch();
+    }
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+}  // namespace ising

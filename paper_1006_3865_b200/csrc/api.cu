@@ -107,6 +107,7 @@ static int to_canon_scratch(ising_ctx* h) {   // tiles -> d_canon, store state u
         case Store::PlaneBits: return launch_planes_to_canon(h, h->store_tile, true, h->d_tiles, h->d_canon);
         case Store::Plane3I8: return launch_3d_to_canon(h, false, h->d_tiles, h->d_canon);
         case Store::Plane3Bits: return launch_3d_to_canon(h, true, h->d_tiles, h->d_canon);
+        case Store::Amsc: return launch_amsc_to_canon(h, h->d_tiles, h->d_canon);
         default: return 0;
     }
 }
@@ -126,7 +127,8 @@ static int ensure_store(ising_ctx* h, Store kind, int T) {
     int rc = ensure_canon(h);
     if (rc) return rc;
     const bool is3 = kind == Store::Plane3I8 || kind == Store::Plane3Bits;
-    const size_t need = kind == Store::TileI8 ? tile_i8_bytes(h, T)
+    const size_t need = kind == Store::Amsc ? amsc_spin_bytes(h)
+                        : kind == Store::TileI8 ? tile_i8_bytes(h, T)
                         : is3 ? tile3d_bytes(h, kind == Store::Plane3Bits)
                               : tile_planes_bytes(h, T, kind == Store::PlaneBits);
     if (need > h->tiles_bytes) {
@@ -137,7 +139,8 @@ static int ensure_store(ising_ctx* h, Store kind, int T) {
         if (!h->d_tiles) return ISING_ENOMEM;
         h->tiles_bytes = need;
     }
-    rc = kind == Store::TileI8 ? launch_canon_to_tile_i8(h, T, h->d_canon, h->d_tiles)
+    rc = kind == Store::Amsc ? launch_canon_to_amsc(h, h->d_canon, h->d_tiles)
+         : kind == Store::TileI8 ? launch_canon_to_tile_i8(h, T, h->d_canon, h->d_tiles)
          : is3 ? launch_canon_to_3d(h, kind == Store::Plane3Bits, h->d_canon, h->d_tiles)
                : launch_canon_to_planes(h, T, kind == Store::PlaneBits, h->d_canon, h->d_tiles);
     if (rc) return rc;
@@ -203,16 +206,18 @@ void ising_destroy(ising_handle h) {
     if (!h) return;
     cudaStreamSynchronize(hooks().stream);
     dev_free(h->d_J);
+    if (h->d_sweep_seeds != h->d_seeds) dev_free(h->d_sweep_seeds);
     dev_free(h->d_seeds);
     dev_free(h->d_canon);
     dev_free(h->d_tiles);
     dev_free(h->d_Jtiles);
+    dev_free(h->d_amsc_J);
     dev_free(h->d_obs);
     dev_free(h->d_flag);
     delete h;
 }
 
-ising_handle ising_create_batch(int dim, int L, const int8_t* J, const uint64_t* seeds, int R) {
+static ising_handle create_impl(int dim, int L, const int8_t* J, const uint64_t* seeds, int R, bool multi, uint64_t sweep_seed) {
     if ((dim != 2 && dim != 3) || L < 2 || (L & 1) || R < 1 || !seeds) {
         set_error("ising_create: need dim in {2,3}, even L >= 2, n_replicas >= 1, seeds != NULL "
                   "(got dim=%d L=%d R=%d)", dim, L, R);
@@ -229,6 +234,8 @@ ising_handle ising_create_batch(int dim, int L, const int8_t* J, const uint64_t*
     if (!h) return nullptr;
     h->dim = dim; h->L = L; h->R = R; h->N = N;
     h->seeds.assign(seeds, seeds + R);
+    h->J_per_replica = multi; h->shared_sweep = multi; h->sweep_seed = sweep_seed;
+    if (multi) h->rng = ISING_RNG_WORDS;     // one random word per site serves every realisation (ising.h)
     cudaStream_t st = hooks().stream;
     auto fail = [&](void) -> ising_handle { ising_destroy(h); return nullptr; };
     h->d_seeds = (uint64_t*)dev_alloc(sizeof(uint64_t) * R);
@@ -240,8 +247,19 @@ ising_handle ising_create_batch(int dim, int L, const int8_t* J, const uint64_t*
         set_error("ising_create: seed upload failed: %s", cudaGetErrorString(cudaGetLastError()));
         return fail();
     }
+    h->d_sweep_seeds = h->d_seeds;
+    if (multi) {                                       // R copies of the shared sweep key (R17)
+        h->d_sweep_seeds = (uint64_t*)dev_alloc(sizeof(uint64_t) * R);
+        if (!h->d_sweep_seeds) return fail();
+        std::vector<uint64_t> ks((size_t)R, sweep_seed);
+        if (cudaMemcpyAsync(h->d_sweep_seeds, ks.data(), sizeof(uint64_t) * R, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+            cudaStreamSynchronize(st) != cudaSuccess) {
+            set_error("ising_create_multi: seed upload failed: %s", cudaGetErrorString(cudaGetLastError()));
+            return fail();
+        }
+    }
     if (J) {
-        const size_t jb = (size_t)dim * N;
+        const size_t jb = (size_t)dim * N * (multi ? (size_t)R : 1);
         h->d_J = (int8_t*)dev_alloc(jb);
         if (!h->d_J) return fail();
         const bool dev = is_device_ptr(J);
@@ -265,6 +283,18 @@ ising_handle ising_create_batch(int dim, int L, const int8_t* J, const uint64_t*
     return h;
 }
 
+ising_handle ising_create_batch(int dim, int L, const int8_t* J, const uint64_t* seeds, int R) {
+    return create_impl(dim, L, J, seeds, R, false, 0);
+}
+
+ising_handle ising_create_multi(int dim, int L, const int8_t* couplings, const uint64_t* init_seeds, int R, uint64_t sweep_seed) {
+    if (!couplings) {
+        set_error("ising_create_multi: couplings must not be NULL (R*dim*N values)");
+        return nullptr;
+    }
+    return create_impl(dim, L, couplings, init_seeds, R, true, sweep_seed);
+}
+
 ising_handle ising_create(int dim, int L, const int8_t* J, uint64_t seed) {
     return ising_create_batch(dim, L, J, &seed, 1);
 }
@@ -272,6 +302,8 @@ ising_handle ising_create(int dim, int L, const int8_t* J, uint64_t seed) {
 }  // extern "C"
 
 // ---- sweeps ---------------------------------------------------------------------------
+static bool thr_fits_or_zero(const Accept&) { return true; }   // amsc.cu handles thr = 2^32 with all-ones masks
+
 static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64_t* E, int64_t* M) {
     if (!h) { set_error("ising_sweep: NULL handle"); return ISING_EINVAL; }
     const int T = (tile == 0) ? h->L : tile;
@@ -306,7 +338,21 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
     const bool use_planes = !h->force_generic && h->rng == ISING_RNG_PLANES && tile_planes_supported(h, T);
     const bool use_plain64 = !h->force_generic && h->rng == ISING_RNG_PLANES && plain64_supported(h, T);
     const bool use_3d = !h->force_generic && h->rng == ISING_RNG_PLANES && tile3d_supported(h, T);
-    if (use_plain64) {                       // a8: whole run in one launch, E/M measured in the kernel
+    const bool use_amsc = !h->force_generic && thr_fits_or_zero(acc) && amsc_supported(h, T);
+    if (use_amsc) {                          // f1: 32 realisations per word, one random number per site
+        h->last_path = "amsc";
+        if (!h->d_amsc_J) {
+            h->d_amsc_J = dev_alloc((size_t)h->N * 8);
+            if (!h->d_amsc_J) rc = ISING_ENOMEM;
+            if (!rc) rc = launch_amsc_pack_J(h, h->d_amsc_J);
+        }
+        if (!rc) rc = ensure_store(h, Store::Amsc, 0);
+        for (int pass = 0; pass < n && !rc; ++pass) {
+            rc = launch_amsc_pass(h, acc, T, k, h->t + (uint64_t)pass * (uint64_t)k, h->d_amsc_J);
+            if (!rc && want_series)
+                rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);
+        }
+    } else if (use_plain64) {                // a8: whole run in one launch, E/M measured in the kernel
         const bool bits = h->layout == ISING_LAYOUT_BITS;
         h->last_path = bits ? "plain64_planes_bits" : "plain64_planes_i8";
         rc = ensure_store(h, bits ? Store::PlaneBits : Store::PlaneI8, T);

@@ -42,7 +42,8 @@ enum class Store : int {
     PlaneI8 = 2, // piece-major tile records of 0/1 bytes (tile_planes.cu)
     PlaneBits = 3, // tile records of bit words (tile_planes.cu)
     Plane3I8 = 4,  // 3D 8^3 tile records, 0/1 bytes + bit-packed face copies (tile3d_planes.cu)
-    Plane3Bits = 5 // 3D 8^3 tile records, bit words + face copies
+    Plane3Bits = 5, // 3D 8^3 tile records, bit words + face copies
+    Amsc = 6       // one 32-bit word per site, bit r = realisation r (amsc.cu)
 };
 
 // Acceptance constants handed to every sweep kernel (S8c.4/5).
@@ -68,7 +69,11 @@ struct ising_ctx {
     uint64_t N = 0;
     bool has_J = false;
     int8_t* d_J = nullptr;          // canonical ±1, dim*N bytes (nullptr if uniform)
-    uint64_t* d_seeds = nullptr;    // R Philox keys
+    uint64_t* d_seeds = nullptr;    // R Philox keys (hot start; and sweeps unless shared_sweep)
+    uint64_t* d_sweep_seeds = nullptr;   // keys of the sweep stream: d_seeds, or R copies of sweep_seed (R17)
+    bool J_per_replica = false;     // d_J holds R coupling arrays (multi-realisation batch, R17)
+    bool shared_sweep = false;
+    uint64_t sweep_seed = 0;
     std::vector<uint64_t> seeds;
     uint64_t t = 0;                 // inner sweeps done (S8c.6)
 
@@ -79,6 +84,7 @@ struct ising_ctx {
     int8_t* d_canon = nullptr;      // R*N bytes; valid iff store == Canon (else scratch)
     void* d_tiles = nullptr;        // tile-record storage (TileI8 / PlaneI8 / PlaneBits)
     size_t tiles_bytes = 0;
+    void* d_amsc_J = nullptr;       // JX, JY word lattices of a multi handle (2*N words), built on first use
     void* d_Jtiles = nullptr;       // couplings in tile-record form for store_tile
     int Jtiles_tile = 0;
     int Jtiles_kind = -1;

@@ -41,6 +41,7 @@ __global__ void k_hot_start(int8_t* __restrict__ s, const uint64_t* __restrict__
 struct GenericGeom {
     int dim, L, T, R;
     uint64_t N;
+    uint64_t Jrep;     // distance between the coupling arrays of consecutive replicas: 0 (shared J) or dim*N (R17)
 };
 
 // One thread per site pair p = i >> 1 (S8c.3): the pair (2p, 2p+1) lies in one row because
@@ -69,8 +70,8 @@ __global__ void k_generic_halfsweep(int8_t* __restrict__ spins, const int8_t* __
     for (int d = 0; d < g.dim; ++d) {
         const uint64_t ip = (coord[d] == g.L - 1) ? i - (L - 1) * stride : i + stride;
         const uint64_t im = (coord[d] == 0) ? i + (L - 1) * stride : i - stride;
-        const int Jp = J ? (int)J[(uint64_t)d * g.N + i] : 1;
-        const int Jm = J ? (int)J[(uint64_t)d * g.N + im] : 1;
+        const int Jp = J ? (int)J[r * g.Jrep + (uint64_t)d * g.N + i] : 1;
+        const int Jm = J ? (int)J[r * g.Jrep + (uint64_t)d * g.N + im] : 1;
         n_sat += (Jp * si * s[ip] > 0) + (Jm * si * s[im] > 0);
         stride *= L;
     }
@@ -130,8 +131,8 @@ __global__ void k_generic_halfsweep_planes(int8_t* __restrict__ spins, const int
         for (int d = 0; d < g.dim; ++d) {
             const uint64_t ip = (coord[d] == g.L - 1) ? i - (L - 1) * stride : i + stride;
             const uint64_t im = (coord[d] == 0) ? i + (L - 1) * stride : i - stride;
-            const int Jp = J ? (int)J[(uint64_t)d * g.N + i] : 1;
-            const int Jm = J ? (int)J[(uint64_t)d * g.N + im] : 1;
+            const int Jp = J ? (int)J[r * g.Jrep + (uint64_t)d * g.N + i] : 1;
+            const int Jm = J ? (int)J[r * g.Jrep + (uint64_t)d * g.N + im] : 1;
             n_sat += (Jp * si * s[ip] > 0) + (Jm * si * s[im] > 0);
             stride *= L;
         }
@@ -177,7 +178,7 @@ __global__ void k_observables(const int8_t* __restrict__ spins, const int8_t* __
         uint64_t stride = 1;
         for (int d = 0; d < g.dim; ++d) {
             const uint64_t ip = (coord[d] == g.L - 1) ? i - (L - 1) * stride : i + stride;
-            const int Jp = J ? (int)J[(uint64_t)d * g.N + i] : 1;
+            const int Jp = J ? (int)J[(uint64_t)r * g.Jrep + (uint64_t)d * g.N + i] : 1;
             e -= Jp * si * s[ip];
             stride *= L;
         }
@@ -246,7 +247,7 @@ int launch_observables_canon(ising_ctx* h, const int8_t* d_spins, long long* d_E
     cudaStream_t st = hooks().stream;
     if (d_E) ISING_CUDA_OK(cudaMemsetAsync(d_E, 0, sizeof(long long) * h->R, st));
     if (d_M) ISING_CUDA_OK(cudaMemsetAsync(d_M, 0, sizeof(long long) * h->R, st));
-    GenericGeom g{h->dim, h->L, h->L, h->R, h->N};
+    GenericGeom g{h->dim, h->L, h->L, h->R, h->N, h->J_per_replica ? (uint64_t)h->dim * h->N : 0};
     dim3 grid(reduce_grid(h->N), h->R);
     k_observables<<<grid, kThreads, 0, st>>>(d_spins, h->d_J, g, d_E, d_M);
     count_launch();
@@ -279,7 +280,7 @@ int launch_validate_pm1(const int8_t* d, uint64_t n, int* d_flag, int* host_bad)
 int launch_generic_sweep(ising_ctx* h, const Accept& acc, int n, int T, int k, long long* d_E,
                          long long* d_M) {
     cudaStream_t st = hooks().stream;
-    GenericGeom g{h->dim, h->L, T, h->R, h->N};
+    GenericGeom g{h->dim, h->L, T, h->R, h->N, h->J_per_replica ? (uint64_t)h->dim * h->N : 0};
     const uint64_t total = (h->N >> 1) * (uint64_t)h->R;
     const unsigned blocks = (unsigned)((total + kThreads - 1) / kThreads);
     const int BW = (h->dim == 2) ? 16 : 4, BH = (h->dim == 2) ? 2 : 8;
@@ -293,10 +294,10 @@ int launch_generic_sweep(ising_ctx* h, const Accept& acc, int n, int T, int k, l
                 const uint64_t t = h->t + (uint64_t)pass * (uint64_t)k + (uint64_t)j;
                 for (int c = 0; c < 2; ++c) {
                     if (h->rng == ISING_RNG_PLANES)
-                        k_generic_halfsweep_planes<<<pblocks, kThreads, 0, st>>>(h->d_canon, h->d_J, h->d_seeds,
+                        k_generic_halfsweep_planes<<<pblocks, kThreads, 0, st>>>(h->d_canon, h->d_J, h->d_sweep_seeds,
                                                                                  g, acc, 2 * t + c, C, c);
                     else
-                        k_generic_halfsweep<<<blocks, kThreads, 0, st>>>(h->d_canon, h->d_J, h->d_seeds,
+                        k_generic_halfsweep<<<blocks, kThreads, 0, st>>>(h->d_canon, h->d_J, h->d_sweep_seeds,
                                                                          g, acc, 2 * t + c, C, c);
                     count_launch();
                 }

@@ -39,6 +39,14 @@ int launch_canon_to_3d(ising_ctx* h, bool bits, const int8_t* d_canon, void* d_t
 int launch_3d_to_canon(ising_ctx* h, bool bits, const void* d_tiles, int8_t* d_canon);
 int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64_t t_first, bool use_jit);
 
+// ---- amsc.cu: asynchronous multi-spin coding, 32 disorder realisations per word (multi handles, R17) ----
+bool amsc_supported(const ising_ctx* h, int T);
+size_t amsc_spin_bytes(const ising_ctx* h);
+int launch_amsc_pack_J(ising_ctx* h, void* d_jwords);
+int launch_canon_to_amsc(ising_ctx* h, const int8_t* d_canon, void* d_words);
+int launch_amsc_to_canon(ising_ctx* h, const void* d_words, int8_t* d_canon);
+int launch_amsc_pass(ising_ctx* h, const Accept& acc, int T, int k, uint64_t t_first, const void* d_jwords);
+
 // ---- planes_jit.cu: run-time specialisation of k_tile_planes on the threshold head bits (NVRTC) ----
 cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R);
 cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3);   // nullptr: not available

@@ -99,7 +99,7 @@ int launch_3d_to_canon(ising_ctx* h, bool bits, const void* d_tiles, int8_t* d_c
 int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64_t t_first, bool use_jit) {
     Plane3Args A;
     A.tiles = (uint8_t*)h->d_tiles;
-    A.seeds = h->d_seeds;
+    A.seeds = h->d_sweep_seeds;
     A.L = h->L; A.B = h->L / kT3; A.R = h->R; A.k = k; A.t_first = t_first;
     const uint32_t B = (uint32_t)A.B;
     A.per_rep = B * B * B / 2u; A.per_z = B * B / 2u; A.hb = B / 2u;

@@ -384,7 +384,7 @@ int launch_tile_i8_to_canon(ising_ctx* h, int T, const void* d_tiles, int8_t* d_
 int launch_tile_i8_pass(ising_ctx* h, const Accept& acc, int T, int k, uint64_t t_first) {
     TileArgs A;
     A.tiles = (uint8_t*)h->d_tiles;
-    A.seeds = h->d_seeds;
+    A.seeds = h->d_sweep_seeds;
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first;
     const uint32_t tiles_per_colour = (uint32_t)((size_t)h->R * A.B * A.B / 2);
     A.njobs = tiles_per_colour / (uint32_t)(64 / T);

@@ -192,7 +192,7 @@ int launch_colour_planes(const PlaneArgs& A, bool use_jit, bool* used_jit) {
 }  // namespace
 
 bool tile_planes_supported(const ising_ctx* h, int T) {
-    if (h->dim != 2) return false;
+    if (h->dim != 2 || h->J_per_replica) return false;     // coupling records are shared by the replicas
     if (T != 32 && T != 64) return false;
     if (h->L % T) return false;
     const int B = h->L / T;
@@ -243,7 +243,7 @@ int launch_planes_to_canon(ising_ctx* h, int T, bool bits, const void* d_tiles, 
 
 constexpr size_t kL2StreamBytes = 96u << 20;    // records larger than this do not stay in the 126 MB L2 between passes
 
-bool plain64_supported(const ising_ctx* h, int T) { return h->dim == 2 && h->L == 64 && T == 64; }
+bool plain64_supported(const ising_ctx* h, int T) { return h->dim == 2 && h->L == 64 && T == 64 && !h->J_per_replica; }
 
 static void fill_accept(PlaneArgs& A, const Accept& acc) {
     for (int q = 0; q < kHeadBits; ++q) {
@@ -260,7 +260,7 @@ static void fill_accept(PlaneArgs& A, const Accept& acc) {
 int launch_plain64(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M) {
     PlaneArgs A;
     A.tiles = (uint8_t*)h->d_tiles;
-    A.seeds = h->d_seeds;
+    A.seeds = h->d_sweep_seeds;
     A.L = 64; A.B = 1; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0; A.njobs = (uint32_t)h->R;
     A.magic_rep = A.magic_hb = 0;
     A.stream = 0;
@@ -286,7 +286,7 @@ int launch_observables_planes(ising_ctx* h, int T, bool bits, long long* d_E, lo
     if (d_M) ISING_CUDA_OK(cudaMemsetAsync(d_M, 0, sizeof(long long) * h->R, st));
     PlaneArgs A = {};
     A.tiles = (uint8_t*)h->d_tiles;
-    A.seeds = h->d_seeds;
+    A.seeds = h->d_sweep_seeds;
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = 0; A.t_first = 0;
     A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
     const uint32_t tiles_per_colour = (uint32_t)((size_t)h->R * A.B * A.B / 2);
@@ -315,7 +315,7 @@ int launch_observables_planes(ising_ctx* h, int T, bool bits, long long* d_E, lo
 int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, int k, uint64_t t_first, bool use_jit) {
     PlaneArgs A;
     A.tiles = (uint8_t*)h->d_tiles;
-    A.seeds = h->d_seeds;
+    A.seeds = h->d_sweep_seeds;
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first;
     A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
     A.stream = tile_planes_bytes(h, T, bits) > kL2StreamBytes ? 1u : 0u;

@@ -220,6 +220,34 @@ def test_specialised_3d_kernel_matches_oracle(P, orc, L, k, n, beta, seeds, layo
     _same_state(g, o)
 
 
+@pytest.mark.parametrize("L,tile,k,n,beta,R", [(64, 32, 1, 3, 1.0, 32), (128, 32, 4, 2, 0.8, 16), (128, 64, 2, 3, 1.2, 5),
+                                                 (192, 32, 2, 2, 0.5, 32), (128, 64, 1, 2, 0.0, 3), (64, 32, 2, 2, 30.0, 2)])
+def test_multi_realisation_batch_matches_oracle(P, orc, L, tile, k, n, beta, R):
+    """SURVEY 8(f)-1, asynchronous multi-spin coding (R17): R disorder realisations in one word lattice driven by
+    one random stream; every realisation against the oracle's multi batch; and the generic path on the same handle."""
+    Js = np.stack([W.couplings(2, L, 900 + r) for r in range(R)])
+    seeds = [2000 + r for r in range(R)]
+    g = P.Ising(2, L, coupling=Js, seeds=seeds, sweep_seed=4242)
+    o = orc.Oracle(2, L, J=Js, seeds=seeds, sweep_seed=4242, rng="words")
+    _same_state(g, o)
+    Eg, Mg = g.sweep_series(beta, n, tile, k)
+    assert g.sweep_path() == "amsc"
+    Eo, Mo = o.sweep_series(beta, n, tile, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    assert g.overlap(0, R - 1) == o.overlap(0, R - 1)
+    g.force_path(True)                                        # the generic kernels continue the same trajectories
+    g.sweep(beta, 1, tile, k); o.sweep(beta, 1, tile, k)
+    assert g.sweep_path() == "generic"
+    _same_state(g, o)
+    g.force_path(False); g.set_rng("planes"); o2 = None       # planes mapping on a multi handle: generic path, still exact
+    op = orc.Oracle(2, L, J=Js, seeds=seeds, sweep_seed=4242, rng="planes")
+    op.set_spins(o.spins()); op.counter = o.counter
+    g.sweep(beta, 1, tile, k); op.sweep(beta, 1, tile, k)
+    assert g.sweep_path() == "generic"
+    _same_state(g, op)
+
+
 def test_missing_nvrtc_falls_back_to_the_precompiled_kernel():
     """With libnvrtc unavailable (simulated by ISING_NO_NVRTC in a fresh process) ising_set_jit(ON) still sweeps, on the
     pre-compiled kernel, and still matches the oracle: the fallback is another CUDA kernel, never a CPU path."""
