@@ -249,6 +249,32 @@ def run_config(P, torch, a) -> None:
         g.destroy()
 
 
+def run_amsc(P, torch, a) -> None:
+    """asynchronous multi-spin coding ("0.15 ps per spin flip").  32 disorder realisations of the
+    2D +-J model per word, one random number per site; attempted flips per ns summed over the realisations."""
+    rows = []
+    R = 32
+    for L in (1024, 2048, 4096):
+        J = W.realisations(2, L, R, 5)
+        for T in (32, 64):
+            for k in (1, 4, 16):
+                g = P.Ising(2, L, coupling=J, seeds=list(range(100, 100 + R)), sweep_seed=77)
+                n = max(4, min(400, int(4e11 / (k * R * L * L))))
+                g.sweep(1.0, 3, T, k)
+                g.synchronize()
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                g.sweep(1.0, n, T, k)
+                e1.record()
+                torch.cuda.synchronize()
+                ms = e0.elapsed_time(e1)
+                rows.append({"L": L, "tile": T, "k": k, "realisations": R, "passes": n, "path": g.sweep_path(),
+                             "flips_per_ns": round(n * k * R * L * L / (ms * 1e6), 1),
+                             "ps_per_flip": round(ms * 1e9 / (n * k * R * L * L), 4)})
+                g.destroy()
+    print(json.dumps({"study": "amsc", "beta": 1.0, "unit": UNIT, "rows": rows}), flush=True)
+
+
 def run_lscan(P, torch, a) -> None:
     """flips/ns against L in the style of the paper's Fig. 3, planes mapping, int8 records."""
     rows = []
@@ -303,6 +329,7 @@ def main() -> None:
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the k/tile table")
     ap.add_argument("--jit", default="auto", choices=["auto", "on", "off"], help="run-time kernel specialisation (ising_set_jit)")
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5], help="time another BASELINE config (default 3 = the headline run)")
+    ap.add_argument("--amsc", action="store_true", help="study: asynchronous multi-spin coding throughput (SURVEY 8(f)-1)")
     ap.add_argument("--lscan", action="store_true", help="study: flips/ns against L (SURVEY 8(f)-3)")
     ap.add_argument("--autocorr", action="store_true", help="study: autocorrelation time against k (SURVEY 8(f)-2)")
     ap.add_argument("--selftest-ranks", action="store_true", help="CPU/gloo check of the multi-rank aggregation, no GPU")
@@ -331,8 +358,8 @@ def main() -> None:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     P.use_torch()
     L = a.L
-    if a.lscan or a.autocorr:
-        (run_lscan if a.lscan else run_autocorr)(P, torch, a)
+    if a.lscan or a.autocorr or a.amsc:
+        (run_lscan if a.lscan else run_autocorr if a.autocorr else run_amsc)(P, torch, a)
         return
     if a.config != 3:
         run_config(P, torch, a)

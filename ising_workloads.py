@@ -68,3 +68,14 @@ def couplings(dim: int, L: int, jseed: int) -> np.ndarray:
             hi = min(lo + bits.size, N)
             out[d, lo:hi] = 1 - 2 * bits[: hi - lo].astype(np.int8)
     return out.reshape(-1)
+
+
+def realisations(dim: int, L: int, R: int, jseed: int) -> np.ndarray:
+    """R independent +-J coupling arrays (p = 1/2), int8 [R][dim][N], for multi-realisation batches
+    (ising_create_multi).  numpy's PCG64 seeded with (jseed, r): fast enough for R = 32 at L = 4096."""
+    N = L ** dim
+    out = np.empty((R, dim * N), dtype=np.int8)
+    for r in range(R):
+        bits = np.random.default_rng([jseed, r]).integers(0, 2, size=dim * N, dtype=np.int8)
+        out[r] = 1 - 2 * bits
+    return out
