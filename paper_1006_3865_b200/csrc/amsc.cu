@@ -44,19 +44,39 @@ __global__ void __launch_bounds__(T * T / 8) k_amsc(AmscArgs A) {
     const int ty = blockIdx.x / hb, tx = 2 * (blockIdx.x % hb) + ((ty + A.C) & 1);
     const int x0 = tx * T, y0 = ty * T;
     const int tid = threadIdx.x, nthr = T * T / 8;
-    // a3: stage.  Rows -1 .. T of the spins (T + 2 words each, periodic), bonds of the tile and of its left / upper rim.
-    for (int idx = tid; idx < P * P; idx += nthr) {
-        const int yy = idx / P - 1, xx = idx % P - 1;
-        const int gy = (y0 + yy + L) % L, gx = (x0 + xx + L) % L;
-        S[idx] = A.spins[(size_t)gy * L + gx];
+    // a3: stage, row by row with 128-bit loads (no per-element wrap arithmetic): spin rows -1 .. T, bond rows, then the
+    // two halo columns and the left rim of JX.
+    constexpr int V = T / 4;                                          // 16-byte chunks per tile row
+    for (int idx = tid; idx < (T + 2) * V; idx += nthr) {             // spins: rows -1 .. T
+        const int rr = idx / V, v = idx - rr * V;
+        int gy = y0 + rr - 1;
+        gy = gy < 0 ? gy + L : (gy >= L ? gy - L : gy);
+        const uint4 w = *reinterpret_cast<const uint4*>(A.spins + (size_t)gy * L + x0 + 4 * v);
+        uint32_t* d = S + rr * P + 1 + 4 * v;
+        d[0] = w.x; d[1] = w.y; d[2] = w.z; d[3] = w.w;
     }
-    for (int idx = tid; idx < T * (T + 1); idx += nthr) {
-        const int yy = idx / (T + 1), xx = idx % (T + 1) - 1;
-        JX[idx] = A.jx[(size_t)(y0 + yy) * L + (x0 + xx + L) % L];
+    for (int idx = tid; idx < T * V; idx += nthr) {                   // JX: rows 0 .. T-1, columns 0 .. T-1
+        const int rr = idx / V, v = idx - rr * V;
+        const uint4 w = *reinterpret_cast<const uint4*>(A.jx + (size_t)(y0 + rr) * L + x0 + 4 * v);
+        uint32_t* d = JX + rr * (T + 1) + 1 + 4 * v;
+        d[0] = w.x; d[1] = w.y; d[2] = w.z; d[3] = w.w;
     }
-    for (int idx = tid; idx < (T + 1) * T; idx += nthr) {
-        const int yy = idx / T - 1, xx = idx % T;
-        JY[idx] = A.jy[(size_t)((y0 + yy + L) % L) * L + (x0 + xx)];
+    for (int idx = tid; idx < (T + 1) * V; idx += nthr) {             // JY: rows -1 .. T-1
+        const int rr = idx / V, v = idx - rr * V;
+        const int gy = y0 + rr - 1 < 0 ? y0 + rr - 1 + L : y0 + rr - 1;
+        const uint4 w = *reinterpret_cast<const uint4*>(A.jy + (size_t)gy * L + x0 + 4 * v);
+        uint32_t* d = JY + rr * T + 4 * v;
+        d[0] = w.x; d[1] = w.y; d[2] = w.z; d[3] = w.w;
+    }
+    {
+        const int xl = x0 == 0 ? L - 1 : x0 - 1, xr = x0 + T == L ? 0 : x0 + T;
+        for (int idx = tid; idx < 3 * T; idx += nthr) {                // halo columns x = -1, x = T; JX of column -1
+            const int rr = idx % T, which = idx / T;
+            const size_t row = (size_t)(y0 + rr) * L;
+            if (which == 0) S[(rr + 1) * P] = A.spins[row + xl];
+            else if (which == 1) S[(rr + 1) * P + T + 1] = A.spins[row + xr];
+            else JX[rr * (T + 1)] = A.jx[row + xl];
+        }
     }
     __syncthreads();
     const int y = tid / (T / 8), g = tid % (T / 8);                  // row and 8-column group of this thread
@@ -88,10 +108,11 @@ __global__ void __launch_bounds__(T * T / 8) k_amsc(AmscArgs A) {
             __syncthreads();
         }
     }
-    // a7: write the interior back, coalesced rows
-    for (int idx = tid; idx < T * T; idx += nthr) {
-        const int yy = idx / T, xx = idx % T;
-        A.spins[(size_t)(y0 + yy) * L + (x0 + xx)] = S[(yy + 1) * P + xx + 1];
+    // a7: write the interior back, 128-bit stores, coalesced rows
+    for (int idx = tid; idx < T * V; idx += nthr) {
+        const int rr = idx / V, v = idx - rr * V;
+        const uint32_t* d = S + (rr + 1) * P + 1 + 4 * v;
+        *reinterpret_cast<uint4*>(A.spins + (size_t)(y0 + rr) * L + x0 + 4 * v) = make_uint4(d[0], d[1], d[2], d[3]);
     }
 }
 
