@@ -254,10 +254,11 @@ def run_amsc(P, torch, a) -> None:
     2D +-J model per word, one random number per site; attempted flips per ns summed over the realisations."""
     rows = []
     R = 32
-    for L in (1024, 2048, 4096):
+    single = a.L != 16384                      # --L given: one variant (--L, --tile, --k), e.g. for an ncu capture
+    for L in ((a.L,) if single else (1024, 2048, 4096)):
         J = W.realisations(2, L, R, 5)
-        for T in (32, 64):
-            for k in (1, 4, 16):
+        for T in ((a.tile,) if single else (32, 64)):
+            for k in ((a.k,) if single else (1, 4, 16)):
                 g = P.Ising(2, L, coupling=J, seeds=list(range(100, 100 + R)), sweep_seed=77)
                 n = max(4, min(400, int(4e11 / (k * R * L * L))))
                 g.sweep(1.0, 3, T, k)
