@@ -166,7 +166,8 @@ int ising_synchronize(ising_handle h);
 uint64_t ising_kernel_launches(void);
 
 /* ising_sweep_path — name of the kernel family the last ising_sweep on h used
- * ("generic", "tile_i8", "tile_bits", ...); static string, never NULL. */
+ * ("generic", "tile_i8", "tile_planes_i8", "tile_planes_bits", "tile3d_planes_i8", "tile3d_planes_bits",
+ * "plain64_planes_i8", "plain64_planes_bits", "amsc"); static string, never NULL. */
 const char* ising_sweep_path(ising_handle h);
 
 /* ising_force_path — testing aid: 0 = automatic kernel choice, 1 = always the generic

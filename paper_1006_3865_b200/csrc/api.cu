@@ -1,6 +1,6 @@
 // api.cu — the C ABI of include/ising.h: argument checking, the host-side acceptance table
 // (a2), storage-layout bookkeeping and kernel-path selection.  All compute is in the
-// kernels of generic.cu / tile_i8.cu / tile_bits.cu; there is no CPU path.
+// kernels of generic.cu / tile_i8.cu / tile_planes.cu / tile3d_planes.cu / amsc.cu; there is no CPU path.
 #include <cmath>
 #include <cstdarg>
 #include <cstring>
