@@ -28,6 +28,10 @@ SYMBOLS = [
     "ising_synchronize", "ising_kernel_launches", "ising_sweep_path", "ising_force_path",
     "ising_last_error",
 ]
+HEIS_SYMBOLS = [     # include/heisenberg.h
+    "heis_create", "heis_destroy", "heis_sweep", "heis_observables", "heis_copy_spins", "heis_set_spins",
+    "heis_get_counter", "heis_set_counter", "heis_sweep_path", "heis_force_generic",
+]
 
 
 class IsingError(RuntimeError):
@@ -79,6 +83,19 @@ def lib() -> C.CDLL:
     L.ising_sweep_path.argtypes = [vp]
     L.ising_force_path.argtypes = [vp, C.c_int]
     L.ising_last_error.restype = C.c_char_p
+    L.heis_create.restype = vp
+    L.heis_create.argtypes = [C.c_int, C.c_int, C.c_uint64]
+    L.heis_destroy.restype = None
+    L.heis_destroy.argtypes = [vp]
+    L.heis_sweep.argtypes = [vp, C.c_double, C.c_int, C.c_int, C.c_int]
+    L.heis_observables.argtypes = [vp, vp, vp]
+    L.heis_copy_spins.argtypes = [vp, vp]
+    L.heis_set_spins.argtypes = [vp, vp]
+    L.heis_get_counter.argtypes = [vp, u64p]
+    L.heis_set_counter.argtypes = [vp, C.c_uint64]
+    L.heis_sweep_path.restype = C.c_char_p
+    L.heis_sweep_path.argtypes = [vp]
+    L.heis_force_generic.argtypes = [vp, C.c_int]
     _lib = L
     return L
 
@@ -229,3 +246,58 @@ class Ising:
 
     def force_path(self, generic_only: bool) -> None:
         _check(lib().ising_force_path(self._h, int(bool(generic_only))))
+
+
+class Heisenberg:
+    """Owner of one `heis_handle`; methods are the C calls of include/heisenberg.h minus the prefix."""
+
+    def __init__(self, dim: int, L: int, seed: int = 0):
+        self.dim, self.L, self.N = dim, L, L ** dim
+        self._h = lib().heis_create(dim, L, int(seed))
+        if not self._h:
+            raise IsingError(f"heis_create failed: {lib().ising_last_error().decode()}")
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().heis_destroy(self._h)
+            self._h = None
+
+    __del__ = destroy
+
+    def sweep(self, beta: float, n_sweeps: int, tile: int = 0, k_inner: int = 1) -> None:
+        _check(lib().heis_sweep(self._h, float(beta), int(n_sweeps), int(tile), int(k_inner)))
+
+    def observables(self):
+        E = np.zeros(1, dtype=np.float64)
+        M = np.zeros(3, dtype=np.float64)
+        _check(lib().heis_observables(self._h, _ptr(E), _ptr(M)))
+        return float(E[0]), M
+
+    def copy_spins(self, dst=None):
+        """(3, N) float32, component-major; dst may be a numpy array or a torch tensor (host or device)."""
+        if dst is None:
+            dst = np.zeros((3, self.N), dtype=np.float32)
+        _check(lib().heis_copy_spins(self._h, _ptr(dst)))
+        return dst
+
+    def set_spins(self, src) -> None:
+        if isinstance(src, np.ndarray):
+            src = np.ascontiguousarray(src, dtype=np.float32).reshape(-1)
+            assert src.size == 3 * self.N
+        _check(lib().heis_set_spins(self._h, _ptr(src)))
+
+    @property
+    def counter(self) -> int:
+        t = np.zeros(1, dtype=np.uint64)
+        _check(lib().heis_get_counter(self._h, _ptr(t)))
+        return int(t[0])
+
+    @counter.setter
+    def counter(self, t: int) -> None:
+        _check(lib().heis_set_counter(self._h, int(t)))
+
+    def sweep_path(self) -> str:
+        return lib().heis_sweep_path(self._h).decode()
+
+    def force_generic(self, on: bool) -> None:
+        _check(lib().heis_force_generic(self._h, int(bool(on))))

@@ -26,7 +26,7 @@ def _stale() -> bool:
         return True
     t = os.path.getmtime(LIB)
     deps = sources() + glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h"))
-    deps.append(os.path.join(HERE, "..", "include", "ising.h"))
+    deps += [os.path.join(HERE, "..", "include", n) for n in ("ising.h", "heisenberg.h")]
     return any(os.path.getmtime(d) > t for d in deps)
 
 

@@ -1,0 +1,503 @@
+// heis.cu — classical Heisenberg (O(3)) double-checkerboard Metropolis, include/heisenberg.h (SURVEY.md
+// §8(f) item 4; readings H1-H8 of DESIGN.md §3.7).  Single precision, every operation stated: the device code
+// below uses the round-to-nearest intrinsics (__fmaf_rn, __fmul_rn, __fadd_rn, __fsub_rn, __fsqrt_rn), which the
+// compiler neither contracts nor re-associates, so the trajectory is a pure function of (seed, schedule).
+//
+// Storage: three float planes s[c][i] (c = x, y, z) in index order.  Two kernel families:
+//   k_heis_tile<DIM, T>   one CTA per tile of the launch's coarse colour: tile + halo faces staged in shared memory
+//                         (128-bit loads of the rows), k inner sweeps of both fine colours on chip, interior written
+//                         back with 128-bit stores (steps a3, a5-a7 of the Ising path, same schedule);
+//   k_heis_generic        one launch per half-sweep on the live array (any valid tile, T = L included).
+#include <algorithm>
+#include <cmath>
+#include <new>
+
+#include "kernels.h"
+#include "philox.cuh"
+#include "../../include/heisenberg.h"
+
+struct heis_ctx {
+    int dim = 2;
+    int L = 0;
+    uint64_t N = 0;
+    uint64_t seed = 0;
+    uint64_t t = 0;
+    float* d_s = nullptr;       // 3*N floats
+    double* d_obs = nullptr;    // E, Mx, My, Mz
+    const char* last_path = "none";
+    int force_generic = 0;
+};
+
+namespace ising {
+
+namespace {
+
+constexpr uint32_t kTagHeisSweep = 5u;   // H4
+constexpr uint32_t kTagHeisInit = 6u;    // H3
+
+struct f3 { float x, y, z; };
+
+// H2: two random words -> a uniform direction.
+__device__ __forceinline__ f3 heis_direction(uint32_t w0, uint32_t w1) {
+    constexpr float PI_4 = (float)0.78539816339744830962;
+    constexpr float S3 = (float)(-1.0 / 6.0), S5 = (float)(1.0 / 120.0), S7 = (float)(-1.0 / 5040.0), S9 = (float)(1.0 / 362880.0);
+    constexpr float C2 = (float)(-1.0 / 2.0), C4 = (float)(1.0 / 24.0), C6 = (float)(-1.0 / 720.0), C8 = (float)(1.0 / 40320.0),
+                    C10 = (float)(-1.0 / 3628800.0);
+    const float z = __fmaf_rn(__uint2float_rn(w0 >> 8), 0x1p-23f, -1.0f);
+    const float rho = __fsqrt_rn(__fmaf_rn(-z, z, 1.0f));
+    const uint32_t q = w1 >> 29;
+    float t = __fmul_rn(__uint2float_rn((w1 >> 5) & 0xffffffu), 0x1p-24f);
+    if (q & 1u) t = __fsub_rn(t, 1.0f);
+    const float x = __fmul_rn(t, PI_4);
+    const float x2 = __fmul_rn(x, x);
+    const float x3 = __fmul_rn(x2, x);
+    float ps = __fmaf_rn(x2, S9, S7);
+    ps = __fmaf_rn(x2, ps, S5);
+    ps = __fmaf_rn(x2, ps, S3);
+    const float sn = __fmaf_rn(x3, ps, x);
+    float pc = __fmaf_rn(x2, C10, C8);
+    pc = __fmaf_rn(x2, pc, C6);
+    pc = __fmaf_rn(x2, pc, C4);
+    pc = __fmaf_rn(x2, pc, C2);
+    const float cs = __fmaf_rn(x2, pc, 1.0f);
+    const uint32_t Q = ((q + 1u) >> 1) & 3u;
+    float c = (Q & 1u) ? sn : cs;          // Q: 0 (cs, sn)  1 (-sn, cs)  2 (-cs, -sn)  3 (sn, -cs)
+    float s = (Q & 1u) ? cs : sn;
+    if (Q == 1u || Q == 2u) c = -c;
+    if (Q >= 2u) s = -s;
+    return f3{__fmul_rn(rho, c), __fmul_rn(rho, s), z};
+}
+
+// H6: acceptance probability for a < 0.
+__device__ __forceinline__ float heis_accept_probability(float a) {
+    constexpr float LOG2E = (float)1.4426950408889634074, LN2 = (float)0.69314718055994530942;
+    constexpr float E2 = (float)(1.0 / 2.0), E3 = (float)(1.0 / 6.0), E4 = (float)(1.0 / 24.0), E5 = (float)(1.0 / 120.0),
+                    E6 = (float)(1.0 / 720.0), E7 = (float)(1.0 / 5040.0);
+    const float tt = __fmul_rn(a, LOG2E);
+    if (tt < -64.0f) return 0.0f;
+    const float n = rintf(tt);
+    const float f = __fsub_rn(tt, n);
+    const float g = __fmul_rn(f, LN2);
+    float p = __fmaf_rn(g, E7, E6);
+    p = __fmaf_rn(g, p, E5);
+    p = __fmaf_rn(g, p, E4);
+    p = __fmaf_rn(g, p, E3);
+    p = __fmaf_rn(g, p, E2);
+    p = __fmaf_rn(g, p, 1.0f);
+    p = __fmaf_rn(g, p, 1.0f);
+    return __fmul_rn(p, __uint_as_float((uint32_t)(__float2int_rn(n) + 127) << 23));
+}
+
+// H5 given the old spin and the local field; returns true and the new spin if the move is accepted.
+__device__ __forceinline__ bool heis_update(uint32_t pair, uint64_t H, uint32_t k0, uint32_t k1, float betaf,
+                                            const f3& s, const f3& h, f3& sp) {
+    const u32x4 w = philox4x32_10(pair, kTagHeisSweep, (uint32_t)H, (uint32_t)(H >> 32), k0, k1);
+    sp = heis_direction(w.x, w.y);
+    const float dx = __fsub_rn(sp.x, s.x), dy = __fsub_rn(sp.y, s.y), dz = __fsub_rn(sp.z, s.z);
+    float e = __fmul_rn(dx, h.x);
+    e = __fmaf_rn(dy, h.y, e);
+    e = __fmaf_rn(dz, h.z, e);
+    if (e >= 0.0f) return true;
+    const float u = __fmul_rn(__uint2float_rn(w.z >> 8), 0x1p-24f);
+    return u < heis_accept_probability(__fmul_rn(betaf, e));
+}
+
+// ---- H3 ----------------------------------------------------------------------------------------------
+__global__ void k_heis_hot_start(float* __restrict__ s, uint64_t N, uint32_t k0, uint32_t k1) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const u32x4 w = philox4x32_10((uint32_t)i, kTagHeisInit, 0u, 0u, k0, k1);
+    const f3 v = heis_direction(w.x, w.y);
+    s[i] = v.x; s[N + i] = v.y; s[2 * N + i] = v.z;
+}
+
+// ---- generic half-sweep: one thread per aligned pair, live neighbours ------------------------------------
+struct GenArgs {
+    float* s;
+    uint64_t N, H;
+    int L, dim, T, C, c;     // T == L: one tile (phase C = 1 is never launched)
+    uint32_t k0, k1;
+    float betaf;
+};
+
+__global__ void k_heis_generic(GenArgs A) {
+    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= A.N / 2) return;
+    const int L = A.L;
+    const uint64_t i0 = 2 * p;
+    const int y = A.dim > 1 ? (int)((i0 / L) % L) : 0;
+    const int z = A.dim > 2 ? (int)(i0 / ((uint64_t)L * L)) : 0;
+    const int x = (int)(i0 % L) + ((y + z + A.c) & 1);
+    if (A.T != L && ((x / A.T + y / A.T + z / A.T) & 1) != A.C) return;
+    const uint64_t i = i0 - (i0 % L) + x;
+    const uint64_t N = A.N;
+    const float* sx = A.s;
+    const float* sy = A.s + N;
+    const float* sz = A.s + 2 * N;
+    const uint64_t xm = i - x + (x == 0 ? L - 1 : x - 1), xp = i - x + (x == L - 1 ? 0 : x + 1);
+    f3 h{__fadd_rn(sx[xm], sx[xp]), __fadd_rn(sy[xm], sy[xp]), __fadd_rn(sz[xm], sz[xp])};
+    if (A.dim > 1) {
+        const uint64_t row = (uint64_t)L;
+        const uint64_t ym = y == 0 ? i + row * (L - 1) : i - row, yp = y == L - 1 ? i - row * (L - 1) : i + row;
+        h.x = __fadd_rn(h.x, sx[ym]); h.y = __fadd_rn(h.y, sy[ym]); h.z = __fadd_rn(h.z, sz[ym]);
+        h.x = __fadd_rn(h.x, sx[yp]); h.y = __fadd_rn(h.y, sy[yp]); h.z = __fadd_rn(h.z, sz[yp]);
+    }
+    if (A.dim > 2) {
+        const uint64_t pl = (uint64_t)L * L;
+        const uint64_t zm = z == 0 ? i + pl * (L - 1) : i - pl, zp = z == L - 1 ? i - pl * (L - 1) : i + pl;
+        h.x = __fadd_rn(h.x, sx[zm]); h.y = __fadd_rn(h.y, sy[zm]); h.z = __fadd_rn(h.z, sz[zm]);
+        h.x = __fadd_rn(h.x, sx[zp]); h.y = __fadd_rn(h.y, sy[zp]); h.z = __fadd_rn(h.z, sz[zp]);
+    }
+    const f3 s{sx[i], sy[i], sz[i]};
+    f3 sp;
+    if (heis_update((uint32_t)p, A.H, A.k0, A.k1, A.betaf, s, h, sp)) {
+        A.s[i] = sp.x; A.s[N + i] = sp.y; A.s[2 * N + i] = sp.z;
+    }
+}
+
+// ---- tile kernel -------------------------------------------------------------------------------------------
+// Shared-memory tile of one component: [ZP][YP][XP] floats, interior site (lx, ly, lz) at (lz+1, ly+1, lx+4) (2D:
+// ZP = 1, no z offset): column 3 and column T+4 are the x halos, and the interior rows start 16-byte aligned.
+// XP = T + 8 is even, so that the 16 (T = 32) active sites of a row and the 16 of the next row, which have the
+// other parity, fall into different banks.
+template <int DIM, int T>
+struct HG {
+    static constexpr int XP = T + 8;
+    static constexpr int YP = T + 2;
+    static constexpr int ZP = DIM == 3 ? T + 2 : 1;
+    static constexpr int COMP = XP * YP * ZP;                   // floats per component
+    static constexpr int SITES = DIM == 3 ? T * T * T : T * T;
+    static constexpr int THREADS = SITES / 4 < 64 ? 64 : (SITES / 4 > 512 ? 512 : SITES / 4);
+    static constexpr size_t SMEM = (size_t)3 * COMP * sizeof(float);
+    __device__ static constexpr int at(int lx, int ly, int lz) {
+        return ((DIM == 3 ? lz + 1 : 0) * YP + (ly + 1)) * XP + lx + 4;
+    }
+};
+
+struct TileArgs {
+    float* s;
+    uint64_t N, t_first;
+    int L, B, C, k;
+    uint32_t k0, k1;
+    float betaf;
+};
+
+template <int DIM, int T>
+__global__ void __launch_bounds__(HG<DIM, T>::THREADS) k_heis_tile(TileArgs A) {
+    using G = HG<DIM, T>;
+    extern __shared__ __align__(16) float sm[];
+    const int tid = threadIdx.x;
+    const int L = A.L, B = A.B;
+    // tile of coarse colour C: blockIdx -> (tx/2, ty, tz)
+    const int hb = B / 2;
+    const int txh = blockIdx.x % hb;
+    const int ty = (blockIdx.x / hb) % B;
+    const int tz = DIM == 3 ? blockIdx.x / (hb * B) : 0;
+    const int tx = 2 * txh + ((ty + tz + A.C) & 1);
+    const int x0 = tx * T, y0 = ty * T, z0 = tz * T;
+    const uint64_t N = A.N;
+    const uint64_t row = (uint64_t)L, plane = (uint64_t)L * L;
+
+    // a3: interior rows and the y / z faces as 128-bit loads, the x faces as scalars
+    constexpr int Q = T / 4;
+    for (int c = 0; c < 3; ++c) {
+        const float* g = A.s + (uint64_t)c * N;
+        float* d = sm + c * G::COMP;
+        for (int idx = tid; idx < G::SITES / 4; idx += G::THREADS) {
+            const int q = idx % Q, ly = (idx / Q) % T, lz = idx / (Q * T);
+            const float4 v = *reinterpret_cast<const float4*>(g + (uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)(y0 + ly) * row + x0 + 4 * q);
+            *reinterpret_cast<float4*>(d + G::at(4 * q, ly, lz)) = v;
+        }
+        constexpr int FACE = G::SITES / T;      // sites of one face
+        // y faces
+        for (int idx = tid; idx < 2 * FACE / 4; idx += G::THREADS) {
+            const int side = idx / (FACE / 4), r = idx % (FACE / 4);
+            const int q = r % Q, lz = r / Q;
+            const int y = side ? (y0 + T == L ? 0 : y0 + T) : (y0 == 0 ? L - 1 : y0 - 1);
+            const float4 v = *reinterpret_cast<const float4*>(g + (uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)y * row + x0 + 4 * q);
+            *reinterpret_cast<float4*>(d + G::at(4 * q, side ? T : -1, lz)) = v;
+        }
+        if (DIM == 3) {
+            for (int idx = tid; idx < 2 * FACE / 4; idx += G::THREADS) {
+                const int side = idx / (FACE / 4), r = idx % (FACE / 4);
+                const int q = r % Q, ly = r / Q;
+                const int z = side ? (z0 + T == L ? 0 : z0 + T) : (z0 == 0 ? L - 1 : z0 - 1);
+                const float4 v = *reinterpret_cast<const float4*>(g + (uint64_t)z * plane + (uint64_t)(y0 + ly) * row + x0 + 4 * q);
+                *reinterpret_cast<float4*>(d + G::at(4 * q, ly, side ? T : -1)) = v;
+            }
+        }
+        for (int idx = tid; idx < 2 * FACE; idx += G::THREADS) {
+            const int side = idx / FACE, r = idx % FACE;
+            const int ly = r % T, lz = r / T;
+            const int x = side ? (x0 + T == L ? 0 : x0 + T) : (x0 == 0 ? L - 1 : x0 - 1);
+            d[G::at(side ? T : -1, ly, lz)] = g[(uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)(y0 + ly) * row + x];
+        }
+    }
+    __syncthreads();
+
+    // a5/a6: k inner sweeps, fine colour 0 then 1; the halo stays as loaded
+    float* const SX = sm;
+    float* const SY = sm + G::COMP;
+    float* const SZ = sm + 2 * G::COMP;
+    constexpr int HALF = T / 2;
+    for (int j = 0; j < A.k; ++j) {
+        for (int c = 0; c < 2; ++c) {
+            const uint64_t H = 2 * (A.t_first + (uint64_t)j) + (uint64_t)c;
+#pragma unroll 2
+            for (int idx = tid; idx < G::SITES / 2; idx += G::THREADS) {
+                const int px = idx % HALF, ly = (idx / HALF) % T, lz = idx / (HALF * T);
+                const int lx = 2 * px + ((ly + lz + c) & 1);      // x0, y0, z0 are even
+                const int o = G::at(lx, ly, lz);
+                f3 h{__fadd_rn(SX[o - 1], SX[o + 1]), __fadd_rn(SY[o - 1], SY[o + 1]), __fadd_rn(SZ[o - 1], SZ[o + 1])};
+                h.x = __fadd_rn(h.x, SX[o - G::XP]); h.y = __fadd_rn(h.y, SY[o - G::XP]); h.z = __fadd_rn(h.z, SZ[o - G::XP]);
+                h.x = __fadd_rn(h.x, SX[o + G::XP]); h.y = __fadd_rn(h.y, SY[o + G::XP]); h.z = __fadd_rn(h.z, SZ[o + G::XP]);
+                if (DIM == 3) {
+                    constexpr int ZS = G::XP * G::YP;
+                    h.x = __fadd_rn(h.x, SX[o - ZS]); h.y = __fadd_rn(h.y, SY[o - ZS]); h.z = __fadd_rn(h.z, SZ[o - ZS]);
+                    h.x = __fadd_rn(h.x, SX[o + ZS]); h.y = __fadd_rn(h.y, SY[o + ZS]); h.z = __fadd_rn(h.z, SZ[o + ZS]);
+                }
+                const f3 s{SX[o], SY[o], SZ[o]};
+                const uint64_t i = (uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)(y0 + ly) * row + (uint64_t)(x0 + lx);
+                f3 sp;
+                if (heis_update((uint32_t)(i >> 1), H, A.k0, A.k1, A.betaf, s, h, sp)) {
+                    SX[o] = sp.x; SY[o] = sp.y; SZ[o] = sp.z;
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    // a7: interior back to HBM
+    for (int c = 0; c < 3; ++c) {
+        float* g = A.s + (uint64_t)c * N;
+        const float* d = sm + c * G::COMP;
+        for (int idx = tid; idx < G::SITES / 4; idx += G::THREADS) {
+            const int q = idx % Q, ly = (idx / Q) % T, lz = idx / (Q * T);
+            *reinterpret_cast<float4*>(g + (uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)(y0 + ly) * row + x0 + 4 * q) =
+                *reinterpret_cast<const float4*>(d + G::at(4 * q, ly, lz));
+        }
+    }
+}
+
+// ---- H8 ----------------------------------------------------------------------------------------------
+__global__ void k_heis_observables(const float* __restrict__ s, uint64_t N, int L, int dim, double* __restrict__ out) {
+    double acc[4] = {0.0, 0.0, 0.0, 0.0};
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < N; i += (uint64_t)gridDim.x * blockDim.x) {
+        const int x = (int)(i % L);
+        const int y = dim > 1 ? (int)((i / L) % L) : 0;
+        const int z = dim > 2 ? (int)(i / ((uint64_t)L * L)) : 0;
+        const uint64_t xp = x == L - 1 ? i - (L - 1) : i + 1;
+        const uint64_t yp = y == L - 1 ? i - (uint64_t)L * (L - 1) : i + L;
+        const uint64_t zp = z == L - 1 ? i - (uint64_t)L * L * (L - 1) : i + (uint64_t)L * L;
+        for (int c = 0; c < 3; ++c) {
+            const float* p = s + (uint64_t)c * N;
+            const double v = (double)p[i];
+            double nb = (double)p[xp];
+            if (dim > 1) nb += (double)p[yp];
+            if (dim > 2) nb += (double)p[zp];
+            acc[0] -= v * nb;
+            acc[1 + c] += v;
+        }
+    }
+    __shared__ double red[4][8];
+    for (int q = 0; q < 4; ++q) {
+        double v = acc[q];
+        for (int o = 16; o > 0; o >>= 1) v += __shfl_down_sync(0xffffffffu, v, o);
+        if ((threadIdx.x & 31) == 0) red[q][threadIdx.x >> 5] = v;
+    }
+    __syncthreads();
+    if (threadIdx.x < 4) {
+        double v = 0.0;
+        for (int w = 0; w < (int)(blockDim.x >> 5); ++w) v += red[threadIdx.x][w];
+        atomicAdd(out + threadIdx.x, v);
+    }
+}
+
+bool is_device_ptr(const void* p) {
+    cudaPointerAttributes a;
+    if (cudaPointerGetAttributes(&a, p) != cudaSuccess) {
+        cudaGetLastError();
+        return false;
+    }
+    return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+bool tile_valid(const heis_ctx* h, int T) {
+    if (T < 2 || (T & 1) || h->L % T) return false;
+    const int B = h->L / T;
+    return B == 1 || (B % 2 == 0);
+}
+
+template <int DIM, int T>
+int launch_tile(heis_ctx* h, TileArgs A) {
+    using G = HG<DIM, T>;
+    static bool attr_set = false;
+    if (!attr_set) {
+        ISING_CUDA_OK(cudaFuncSetAttribute(k_heis_tile<DIM, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
+        attr_set = true;
+    }
+    unsigned tiles = (unsigned)(A.B / 2) * A.B * (DIM == 3 ? A.B : 1);
+    for (int C = 0; C < 2; ++C) {
+        A.C = C;
+        k_heis_tile<DIM, T><<<tiles, G::THREADS, G::SMEM, hooks().stream>>>(A);
+        count_launch();
+    }
+    ISING_CUDA_OK(cudaGetLastError());
+    (void)h;
+    return 0;
+}
+
+// 0: launched; 1: no tile kernel for this (dim, T)
+int tile_pass(heis_ctx* h, const TileArgs& A, int T) {
+    if (h->L % 4 || h->L / T < 2) return 1;
+    if (h->dim == 2) {
+        switch (T) {
+            case 16: return launch_tile<2, 16>(h, A);
+            case 32: return launch_tile<2, 32>(h, A);
+            case 64: return launch_tile<2, 64>(h, A);
+            default: return 1;
+        }
+    }
+    switch (T) {
+        case 4: return launch_tile<3, 4>(h, A);
+        case 8: return launch_tile<3, 8>(h, A);
+        case 16: return launch_tile<3, 16>(h, A);
+        default: return 1;
+    }
+}
+
+}  // namespace
+}  // namespace ising
+
+using namespace ising;
+
+extern "C" {
+
+heis_handle heis_create(int dim, int L, uint64_t seed) {
+    if (dim < 2 || dim > 3 || L < 2 || (L & 1)) {
+        set_error("heis_create: need dim in {2,3} and even L >= 2 (got dim=%d L=%d)", dim, L);
+        return nullptr;
+    }
+    double n = 1.0;
+    for (int d = 0; d < dim; ++d) n *= (double)L;
+    if (n > 4294967296.0) {
+        set_error("heis_create: N = L^dim must not exceed 2^32");
+        return nullptr;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        set_error("no CUDA device: libising_b200 has no CPU path");
+        return nullptr;
+    }
+    heis_ctx* h = new (std::nothrow) heis_ctx;
+    if (!h) { set_error("out of host memory"); return nullptr; }
+    h->dim = dim; h->L = L; h->seed = seed; h->N = (uint64_t)n;
+    h->d_s = (float*)dev_alloc(3 * h->N * sizeof(float));
+    h->d_obs = (double*)dev_alloc(4 * sizeof(double));
+    if (!h->d_s || !h->d_obs) { heis_destroy(h); return nullptr; }
+    const unsigned blocks = (unsigned)((h->N + 255) / 256);
+    k_heis_hot_start<<<blocks, 256, 0, hooks().stream>>>(h->d_s, h->N, (uint32_t)seed, (uint32_t)(seed >> 32));
+    count_launch();
+    if (cudaGetLastError() != cudaSuccess) { set_error("hot-start launch failed"); heis_destroy(h); return nullptr; }
+    return h;
+}
+
+void heis_destroy(heis_handle h) {
+    if (!h) return;
+    cudaStreamSynchronize(hooks().stream);
+    dev_free(h->d_s);
+    dev_free(h->d_obs);
+    delete h;
+}
+
+int heis_sweep(heis_handle h, double beta, int n_sweeps, int tile, int k_inner) {
+    if (!h) { set_error("heis_sweep: NULL handle"); return ISING_EINVAL; }
+    if (!(beta >= 0.0) || !std::isfinite(beta) || n_sweeps < 0 || k_inner < 1) {
+        set_error("heis_sweep: need finite beta >= 0, n_sweeps >= 0, k_inner >= 1");
+        return ISING_EINVAL;
+    }
+    const int T = tile == 0 ? h->L : tile;
+    if (!tile_valid(h, T)) {
+        set_error("heis_sweep: tile %d invalid for L=%d (T even, T | L, L/T even or T == L)", T, h->L);
+        return ISING_EINVAL;
+    }
+    const float betaf = (float)beta;
+    const uint32_t k0 = (uint32_t)h->seed, k1 = (uint32_t)(h->seed >> 32);
+    for (int pass = 0; pass < n_sweeps; ++pass) {
+        const uint64_t t_first = h->t + (uint64_t)pass * k_inner;
+        int rc = 1;
+        if (!h->force_generic) {
+            TileArgs A{h->d_s, h->N, t_first, h->L, h->L / T, 0, k_inner, k0, k1, betaf};
+            rc = tile_pass(h, A, T);
+            if (rc < 0) return rc;
+            if (rc == 0) h->last_path = "heis_tile";
+        }
+        if (rc == 1) {
+            h->last_path = "heis_generic";
+            const unsigned blocks = (unsigned)((h->N / 2 + 255) / 256);
+            for (int C = 0; C < (T == h->L ? 1 : 2); ++C)
+                for (int j = 0; j < k_inner; ++j)
+                    for (int c = 0; c < 2; ++c) {
+                        GenArgs G{h->d_s, h->N, 2 * (t_first + (uint64_t)j) + (uint64_t)c, h->L, h->dim, T, C, c, k0, k1, betaf};
+                        k_heis_generic<<<blocks, 256, 0, hooks().stream>>>(G);
+                        count_launch();
+                    }
+            ISING_CUDA_OK(cudaGetLastError());
+        }
+    }
+    h->t += (uint64_t)n_sweeps * k_inner;
+    return 0;
+}
+
+int heis_observables(heis_handle h, double* E, double* M) {
+    if (!h) { set_error("heis_observables: NULL handle"); return ISING_EINVAL; }
+    cudaStream_t st = hooks().stream;
+    ISING_CUDA_OK(cudaMemsetAsync(h->d_obs, 0, 4 * sizeof(double), st));
+    const unsigned blocks = (unsigned)std::min<uint64_t>((h->N + 255) / 256, 148 * 8);
+    k_heis_observables<<<blocks, 256, 0, st>>>(h->d_s, h->N, h->L, h->dim, h->d_obs);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    if (E) ISING_CUDA_OK(cudaMemcpyAsync(E, h->d_obs, sizeof(double), is_device_ptr(E) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    if (M) ISING_CUDA_OK(cudaMemcpyAsync(M, h->d_obs + 1, 3 * sizeof(double), is_device_ptr(M) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    ISING_CUDA_OK(cudaStreamSynchronize(st));
+    return 0;
+}
+
+int heis_copy_spins(heis_handle h, float* dst) {
+    if (!h || !dst) { set_error("heis_copy_spins: NULL argument"); return ISING_EINVAL; }
+    cudaStream_t st = hooks().stream;
+    ISING_CUDA_OK(cudaMemcpyAsync(dst, h->d_s, 3 * h->N * sizeof(float), is_device_ptr(dst) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st));
+    ISING_CUDA_OK(cudaStreamSynchronize(st));
+    return 0;
+}
+
+int heis_set_spins(heis_handle h, const float* src) {
+    if (!h || !src) { set_error("heis_set_spins: NULL argument"); return ISING_EINVAL; }
+    cudaStream_t st = hooks().stream;
+    ISING_CUDA_OK(cudaMemcpyAsync(h->d_s, src, 3 * h->N * sizeof(float), is_device_ptr(src) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
+    ISING_CUDA_OK(cudaStreamSynchronize(st));
+    return 0;
+}
+
+int heis_get_counter(heis_handle h, uint64_t* t) {
+    if (!h || !t) { set_error("heis_get_counter: NULL argument"); return ISING_EINVAL; }
+    *t = h->t;
+    return 0;
+}
+
+int heis_set_counter(heis_handle h, uint64_t t) {
+    if (!h) { set_error("heis_set_counter: NULL handle"); return ISING_EINVAL; }
+    h->t = t;
+    return 0;
+}
+
+const char* heis_sweep_path(heis_handle h) { return h ? h->last_path : "none"; }
+
+int heis_force_generic(heis_handle h, int on) {
+    if (!h) { set_error("heis_force_generic: NULL handle"); return ISING_EINVAL; }
+    h->force_generic = on ? 1 : 0;
+    return 0;
+}
+
+}  // extern "C"

@@ -28,6 +28,18 @@ def test_every_declared_symbol_is_exported(pkg):
         assert hasattr(L, name), name
 
 
+def test_every_declared_heisenberg_symbol_is_exported(pkg):
+    hdr = open(os.path.join(ROOT, "include", "heisenberg.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(heis_[a-z_]+)\s*\(", hdr))
+    assert declared and declared == set(pkg.HEIS_SYMBOLS)
+    L = pkg.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    assert not L.heis_create(1, 8, 0) and not L.heis_create(2, 7, 0) and not L.heis_create(3, 2048, 0)
+    assert L.heis_sweep(None, 0.5, 1, 0, 1) < 0 and L.heis_observables(None, None, None) < 0
+
+
 def test_thresholds_host_table_matches_oracle(pkg, orc):
     # S8c.4: both sides call the host exp(); the tables must be identical
     for beta in (0.0, 0.30, 0.40, 0.4406868, 0.50, 0.60, 1.0, 0.2216546, 3.0, 7.0):
