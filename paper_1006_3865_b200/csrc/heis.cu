@@ -74,7 +74,6 @@ __device__ __forceinline__ float heis_accept_probability(float a) {
     constexpr float E2 = (float)(1.0 / 2.0), E3 = (float)(1.0 / 6.0), E4 = (float)(1.0 / 24.0), E5 = (float)(1.0 / 120.0),
                     E6 = (float)(1.0 / 720.0), E7 = (float)(1.0 / 5040.0);
     const float tt = __fmul_rn(a, LOG2E);
-    if (tt < -64.0f) return 0.0f;
     const float n = rintf(tt);
     const float f = __fsub_rn(tt, n);
     const float g = __fmul_rn(f, LN2);
@@ -85,7 +84,8 @@ __device__ __forceinline__ float heis_accept_probability(float a) {
     p = __fmaf_rn(g, p, E2);
     p = __fmaf_rn(g, p, 1.0f);
     p = __fmaf_rn(g, p, 1.0f);
-    return __fmul_rn(p, __uint_as_float((uint32_t)(__float2int_rn(n) + 127) << 23));
+    const float P = __fmul_rn(p, __uint_as_float((uint32_t)(__float2int_rn(n) + 127) << 23));
+    return tt < -64.0f ? 0.0f : P;        // (for tt outside [-64, 0] P is meaningless and not used)
 }
 
 // H5 given the old spin and the local field; returns true and the new spin if the move is accepted.
@@ -97,9 +97,11 @@ __device__ __forceinline__ bool heis_update(uint32_t pair, uint64_t H, uint32_t 
     float e = __fmul_rn(dx, h.x);
     e = __fmaf_rn(dy, h.y, e);
     e = __fmaf_rn(dz, h.z, e);
-    if (e >= 0.0f) return true;
+    // both sides of "e >= 0 or u < P" are evaluated (a warp nearly always holds both cases): for e >= 0 the value
+    // of P is not used
     const float u = __fmul_rn(__uint2float_rn(w.z >> 8), 0x1p-24f);
-    return u < heis_accept_probability(__fmul_rn(betaf, e));
+    const float P = heis_accept_probability(__fmul_rn(betaf, e));
+    return (e >= 0.0f) | (u < P);
 }
 
 // ---- H3 ----------------------------------------------------------------------------------------------
@@ -158,16 +160,25 @@ __global__ void k_heis_generic(GenArgs A) {
 // ---- tile kernel -------------------------------------------------------------------------------------------
 // Shared-memory tile of one component: [ZP][YP][XP] floats, interior site (lx, ly, lz) at (lz+1, ly+1, lx+4) (2D:
 // ZP = 1, no z offset): column 3 and column T+4 are the x halos, and the interior rows start 16-byte aligned.
-// XP = T + 8 is even, so that the 16 (T = 32) active sites of a row and the 16 of the next row, which have the
-// other parity, fall into different banks.
+// XP is even, so that the active sites of a row and those of the next row, which have the other parity, fall
+// into different banks; T + 8 (T + 4 for T = 8: row offsets 12r mod 32) also keeps the rows of equal parity that one
+// warp touches apart.
 template <int DIM, int T>
 struct HG {
-    static constexpr int XP = T + 8;
+    static constexpr int XP = T <= 8 ? T + 4 : T + 8;          // T + 4: the right halo of a row sits in the unused column 0 of the next
     static constexpr int YP = T + 2;
     static constexpr int ZP = DIM == 3 ? T + 2 : 1;
-    static constexpr int COMP = XP * YP * ZP;                   // floats per component
+    static constexpr int COMP = XP * YP * ZP + 4;               // floats per component
     static constexpr int SITES = DIM == 3 ? T * T * T : T * T;
-    static constexpr int THREADS = SITES / 4 < 64 ? 64 : (SITES / 4 > 512 ? 512 : SITES / 4);
+    static constexpr int THREADS = SITES / 4 < 32 ? 32 : (SITES / 4 > 512 ? 512 : SITES / 4);
+    // update loop: thread = (pair column px, row r); per half-sweep it updates UPT sites RS rows apart.  RS rows are an
+    // even number of rows (2D) / of z layers (3D), so the column parity of a thread's active sites is fixed.
+    static constexpr int HALF = T / 2;
+    static constexpr int RS = THREADS / HALF;
+    static constexpr int UPT = SITES / 2 / THREADS;
+    static constexpr int OSTEP = DIM == 3 ? (RS / T) * XP * YP : RS * XP;
+    static_assert(THREADS % HALF == 0 && UPT * THREADS * 2 == SITES, "thread mapping");
+    static_assert(UPT == 1 || (DIM == 3 ? (RS % T == 0 && (RS / T) % 2 == 0) : RS % 2 == 0), "fixed parity per thread");
     static constexpr size_t SMEM = (size_t)3 * COMP * sizeof(float);
     __device__ static constexpr int at(int lx, int ly, int lz) {
         return ((DIM == 3 ? lz + 1 : 0) * YP + (ly + 1)) * XP + lx + 4;
@@ -239,15 +250,19 @@ __global__ void __launch_bounds__(HG<DIM, T>::THREADS) k_heis_tile(TileArgs A) {
     float* const SX = sm;
     float* const SY = sm + G::COMP;
     float* const SZ = sm + 2 * G::COMP;
-    constexpr int HALF = T / 2;
+    const int px = tid % G::HALF, r = tid / G::HALF;
+    const int ly = r % T, lz = r / T;
+    const int par = (ly + lz) & 1;                                    // x0, y0, z0 are even
+    const int o_row = G::at(2 * px, ly, lz);
+    const uint32_t p_base = (uint32_t)(((uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)(y0 + ly) * row + (uint64_t)x0) >> 1) + (uint32_t)px;
+    const uint32_t p_step = DIM == 3 ? (uint32_t)(G::RS / T) * (uint32_t)(plane >> 1) : (uint32_t)G::RS * (uint32_t)(L >> 1);
     for (int j = 0; j < A.k; ++j) {
         for (int c = 0; c < 2; ++c) {
             const uint64_t H = 2 * (A.t_first + (uint64_t)j) + (uint64_t)c;
-#pragma unroll 2
-            for (int idx = tid; idx < G::SITES / 2; idx += G::THREADS) {
-                const int px = idx % HALF, ly = (idx / HALF) % T, lz = idx / (HALF * T);
-                const int lx = 2 * px + ((ly + lz + c) & 1);      // x0, y0, z0 are even
-                const int o = G::at(lx, ly, lz);
+            const int o0 = o_row + ((par + c) & 1);
+#pragma unroll
+            for (int u = 0; u < G::UPT; ++u) {
+                const int o = o0 + u * G::OSTEP;
                 f3 h{__fadd_rn(SX[o - 1], SX[o + 1]), __fadd_rn(SY[o - 1], SY[o + 1]), __fadd_rn(SZ[o - 1], SZ[o + 1])};
                 h.x = __fadd_rn(h.x, SX[o - G::XP]); h.y = __fadd_rn(h.y, SY[o - G::XP]); h.z = __fadd_rn(h.z, SZ[o - G::XP]);
                 h.x = __fadd_rn(h.x, SX[o + G::XP]); h.y = __fadd_rn(h.y, SY[o + G::XP]); h.z = __fadd_rn(h.z, SZ[o + G::XP]);
@@ -257,9 +272,8 @@ __global__ void __launch_bounds__(HG<DIM, T>::THREADS) k_heis_tile(TileArgs A) {
                     h.x = __fadd_rn(h.x, SX[o + ZS]); h.y = __fadd_rn(h.y, SY[o + ZS]); h.z = __fadd_rn(h.z, SZ[o + ZS]);
                 }
                 const f3 s{SX[o], SY[o], SZ[o]};
-                const uint64_t i = (uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)(y0 + ly) * row + (uint64_t)(x0 + lx);
                 f3 sp;
-                if (heis_update((uint32_t)(i >> 1), H, A.k0, A.k1, A.betaf, s, h, sp)) {
+                if (heis_update(p_base + (uint32_t)u * p_step, H, A.k0, A.k1, A.betaf, s, h, sp)) {
                     SX[o] = sp.x; SY[o] = sp.y; SZ[o] = sp.z;
                 }
             }
