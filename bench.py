@@ -276,6 +276,70 @@ def run_amsc(P, torch, a) -> None:
     print(json.dumps({"study": "amsc", "beta": 1.0, "unit": UNIT, "rows": rows}), flush=True)
 
 
+def heis_alu_peak(dim: int, sm_mhz: float = 1965.0) -> dict:
+    """Issue ceiling of one Heisenberg update on B200: the operations H2-H6 state, costed with the
+    pipe rates measured in profiles/r01_microbench.md.  Per warp-update, in SMSP-cycles: Philox4x32-10 84.6 (measured),
+    every stated float / convert / select operation and every shared-memory access one issue slot."""
+    fp = 34 + (3 + 6 * (dim - 1)) + 3 + 3 + 2 + 16 + 3       # direction, field adds, d, e, u, P(beta*e), decision
+    lsu = 3 * (2 * dim + 1) + 3                              # neighbour + own loads, store of an accepted spin
+    cycles = 84.6 + fp + lsu
+    return {"cycles_per_warp_update": cycles, "peak": 148 * 4 * sm_mhz * 1e6 / cycles * 32 / 1e9}
+
+
+def run_heisenberg(P, torch, a) -> None:
+    """the continuous-spin (classical Heisenberg) sweep of P:100 in single precision, include/heisenberg.h.
+    Spin updates per ns, device-timed; lattices larger than L2 (three float planes: 805 MB at 2D L=8192, 201 MB at 3D
+    L=256).  One JSON line per (dim, L, tile, k); the first carries the CPU oracle timed on a small lattice."""
+    single = a.L != 16384
+    variants = [(a.dim, a.L, a.tile, a.k)] if single else \
+        [(2, 8192, 32, 1), (2, 8192, 32, 4), (2, 8192, 32, 16), (2, 8192, 16, 16), (2, 8192, 64, 16),
+         (3, 256, 8, 1), (3, 256, 8, 4), (3, 256, 16, 4)]
+    hbm_gbs, _, sm_mhz = measured_peaks()
+    first = True
+    for dim, L, T, k in variants:
+        beta = 0.7 if dim == 2 else 0.693            # 3D: near the critical coupling 0.6930 of the model
+        g = P.Heisenberg(dim, L, seed=3)
+        n = max(4, min(a.steps, int(6e9 / (k * L ** dim))))
+        g.sweep(beta, max(3, a.warmup), T, k)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n0 = P.ising_kernel_launches()
+        e0.record()
+        g.sweep(beta, n, T, k)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        upd = n * k * L ** dim / (ms * 1e6)
+        alu = heis_alu_peak(dim, sm_mhz)
+        bytes_per_update = (12.0 * (1 + 2 * dim / T) + 12.0) / k
+        line = {"metric": "spin updates/ns (Heisenberg, single precision)", "value": upd, "unit": "updates/ns", "n_gpus": 1,
+                "steps": n, "warmup": max(3, a.warmup), "ms_per_step": ms / n, "higher_is_better": True, "scaling": "weak",
+                "vs_baseline": None, "dtype": "f32", "data": "synthetic", "gpu_launches": int(P.ising_kernel_launches() - n0),
+                "config": {"workload": f"Heisenberg dim={dim} L={L} seed=3 beta={beta} tile={T} k={k}; {3 * 4 * L ** dim / 1e6:.0f} MB of spins (> L2)",
+                           "kernel_path": g.sweep_path()},
+                "roofline": {"bound": "alu", "achieved": upd, "peak": alu["peak"], "unit": "updates/ns", "frac": upd / alu["peak"],
+                             "traffic": None, "cycles_per_warp_update": alu["cycles_per_warp_update"],
+                             "hbm_algorithmic_gbs": upd * bytes_per_update, "bytes_per_update": bytes_per_update,
+                             "hbm_frac": upd * bytes_per_update / hbm_gbs,
+                             "note": "peak = issue ceiling of the stated operations (DESIGN.md 7.4); HBM is not the bound for k >= 2"}}
+        g.destroy()
+        if first and not a.no_extras:
+            from oracle import heisenberg as HO
+            Lo = 256 if dim == 2 else 40
+            o = HO.HeisenbergOracle(dim, Lo, seed=3)
+            o.sweep(beta, 1, T if Lo % (2 * T) == 0 else 0, 1)
+            t0 = time.perf_counter()
+            passes = 0
+            while time.perf_counter() - t0 < 10.0:
+                o.sweep(beta, 4, T if Lo % (2 * T) == 0 else 0, k)
+                passes += 4
+            dt = time.perf_counter() - t0
+            line["cpu_baseline"] = {"value": passes * k * Lo ** dim / (dt * 1e9), "unit": "updates/ns", "cores": 1, "kind": "oracle",
+                                    "sample": f"{passes} passes of dim={dim} L={Lo} tile={T} k={k} (same update rule, smaller lattice)"}
+        first = False
+        print(json.dumps(line), flush=True)
+
+
 def run_lscan(P, torch, a) -> None:
     """flips/ns against L in the style of the paper's Fig. 3, planes mapping, int8 records."""
     rows = []
@@ -331,6 +395,8 @@ def main() -> None:
     ap.add_argument("--jit", default="auto", choices=["auto", "on", "off"], help="run-time kernel specialisation (ising_set_jit)")
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5], help="time another BASELINE config (default 3 = the headline run)")
     ap.add_argument("--amsc", action="store_true", help="study: asynchronous multi-spin coding throughput (SURVEY 8(f)-1)")
+    ap.add_argument("--heisenberg", action="store_true", help="study: the continuous-spin (Heisenberg) sweep, include/heisenberg.h (SURVEY 8(f)-4)")
+    ap.add_argument("--dim", type=int, default=2, choices=[2, 3], help="with --heisenberg --L: lattice dimension")
     ap.add_argument("--lscan", action="store_true", help="study: flips/ns against L (SURVEY 8(f)-3)")
     ap.add_argument("--autocorr", action="store_true", help="study: autocorrelation time against k (SURVEY 8(f)-2)")
     ap.add_argument("--selftest-ranks", action="store_true", help="CPU/gloo check of the multi-rank aggregation, no GPU")
@@ -359,8 +425,8 @@ def main() -> None:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     P.use_torch()
     L = a.L
-    if a.lscan or a.autocorr or a.amsc:
-        (run_lscan if a.lscan else run_autocorr if a.autocorr else run_amsc)(P, torch, a)
+    if a.lscan or a.autocorr or a.amsc or a.heisenberg:
+        (run_lscan if a.lscan else run_autocorr if a.autocorr else run_amsc if a.amsc else run_heisenberg)(P, torch, a)
         return
     if a.config != 3:
         run_config(P, torch, a)

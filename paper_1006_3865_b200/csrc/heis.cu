@@ -24,6 +24,9 @@ struct heis_ctx {
     uint64_t t = 0;
     float* d_s = nullptr;       // 3*N floats
     double* d_obs = nullptr;    // E, Mx, My, Mz
+    float* d_xface = nullptr;   // x-face copies of the tile kernel, valid for tile size xface_T (0: stale)
+    size_t xface_bytes = 0;
+    int xface_T = 0;
     const char* last_path = "none";
     int force_generic = 0;
 };
@@ -179,7 +182,9 @@ struct HG {
     static constexpr int OSTEP = DIM == 3 ? (RS / T) * XP * YP : RS * XP;
     static_assert(THREADS % HALF == 0 && UPT * THREADS * 2 == SITES, "thread mapping");
     static_assert(UPT == 1 || (DIM == 3 ? (RS % T == 0 && (RS / T) % 2 == 0) : RS % 2 == 0), "fixed parity per thread");
-    static constexpr size_t SMEM = (size_t)3 * COMP * sizeof(float);
+    static constexpr int FACE = SITES / T;                       // sites of one face
+    // shared memory: three components of the tile + halo, then the staged x faces XF[c][side][FACE]
+    static constexpr size_t SMEM = (size_t)(3 * COMP + 6 * FACE) * sizeof(float);
     __device__ static constexpr int at(int lx, int ly, int lz) {
         return ((DIM == 3 ? lz + 1 : 0) * YP + (ly + 1)) * XP + lx + 4;
     }
@@ -187,19 +192,47 @@ struct HG {
 
 struct TileArgs {
     float* s;
+    float* xface;        // x-face copies, see below
     uint64_t N, t_first;
     int L, B, C, k;
+    uint32_t ntiles;     // all tiles, both colours
     uint32_t k0, k1;
     float betaf;
 };
 
+// x-face copies.  The x halos of a tile are single floats T apart in a row: read from the spin planes each would
+// cost a whole 64-byte DRAM access.  So every tile also keeps copies of its own two x faces (the columns lx = 0 and
+// lx = T-1, FACE = T^(dim-1) floats each, ordered (lz, ly)) in a side array
+//     xface[((c * ntiles + tile) * 2 + side) * FACE + lz * T + ly],   tile = (tz * B + ty) * B + tx,
+// written with the tile's write-back and read by the two x neighbours as contiguous 16-byte copies.  The spin planes
+// stay complete and current; the host rebuilds the copies (k_heis_build_xface) when something else wrote the spins.
+__device__ __forceinline__ void cp_async16(float* smem, const float* gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+template <int DIM, int T>
+__global__ void k_heis_build_xface(const float* __restrict__ s, float* __restrict__ xface, uint64_t N, int L, int B, uint32_t ntiles) {
+    constexpr int FACE = HG<DIM, T>::FACE;
+    const uint64_t e = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;     // entry of xface
+    if (e >= (uint64_t)3 * ntiles * 2 * FACE) return;
+    const int f = (int)(e % FACE), side = (int)((e / FACE) & 1);
+    const uint32_t tile = (uint32_t)((e / (2 * FACE)) % ntiles);
+    const int c = (int)(e / ((uint64_t)2 * FACE * ntiles));
+    const int tx = tile % B, ty = (tile / B) % B, tz = DIM == 3 ? tile / (B * B) : 0;
+    const int ly = f % T, lz = f / T;
+    const uint64_t i = (uint64_t)(tz * T + lz) * L * L * (DIM == 3) + (uint64_t)(ty * T + ly) * L + (uint64_t)(tx * T + (side ? T - 1 : 0));
+    xface[e] = s[(uint64_t)c * N + i];
+}
+
+// One CTA per tile of the launch's coarse colour (job -> (tx/2, ty, tz) row-major).
 template <int DIM, int T>
 __global__ void __launch_bounds__(HG<DIM, T>::THREADS) k_heis_tile(TileArgs A) {
     using G = HG<DIM, T>;
     extern __shared__ __align__(16) float sm[];
     const int tid = threadIdx.x;
     const int L = A.L, B = A.B;
-    // tile of coarse colour C: blockIdx -> (tx/2, ty, tz)
     const int hb = B / 2;
     const int txh = blockIdx.x % hb;
     const int ty = (blockIdx.x / hb) % B;
@@ -208,41 +241,47 @@ __global__ void __launch_bounds__(HG<DIM, T>::THREADS) k_heis_tile(TileArgs A) {
     const int x0 = tx * T, y0 = ty * T, z0 = tz * T;
     const uint64_t N = A.N;
     const uint64_t row = (uint64_t)L, plane = (uint64_t)L * L;
-
-    // a3: interior rows and the y / z faces as 128-bit loads, the x faces as scalars
     constexpr int Q = T / 4;
+    constexpr int FACE = G::FACE;
+    const uint32_t tile_row = (uint32_t)(tz * B + ty) * (uint32_t)B;
+    const uint32_t t_self = tile_row + tx, t_left = tile_row + (tx == 0 ? B - 1 : tx - 1), t_right = tile_row + (tx == B - 1 ? 0 : tx + 1);
+    float* const XF = sm + 3 * G::COMP;
+
+    // a3: interior rows, the y / z faces and the x-face copies as 16-byte asynchronous copies
     for (int c = 0; c < 3; ++c) {
-        const float* g = A.s + (uint64_t)c * N;
+        const float* g = A.s + (uint64_t)c * N + (DIM == 3 ? (uint64_t)z0 * plane : 0) + (uint64_t)y0 * row + x0;
         float* d = sm + c * G::COMP;
         for (int idx = tid; idx < G::SITES / 4; idx += G::THREADS) {
             const int q = idx % Q, ly = (idx / Q) % T, lz = idx / (Q * T);
-            const float4 v = *reinterpret_cast<const float4*>(g + (uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)(y0 + ly) * row + x0 + 4 * q);
-            *reinterpret_cast<float4*>(d + G::at(4 * q, ly, lz)) = v;
+            cp_async16(d + G::at(4 * q, ly, lz), g + (DIM == 3 ? (uint64_t)lz * plane : 0) + (uint64_t)ly * row + 4 * q);
         }
-        constexpr int FACE = G::SITES / T;      // sites of one face
-        // y faces
         for (int idx = tid; idx < 2 * FACE / 4; idx += G::THREADS) {
             const int side = idx / (FACE / 4), r = idx % (FACE / 4);
             const int q = r % Q, lz = r / Q;
-            const int y = side ? (y0 + T == L ? 0 : y0 + T) : (y0 == 0 ? L - 1 : y0 - 1);
-            const float4 v = *reinterpret_cast<const float4*>(g + (uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)y * row + x0 + 4 * q);
-            *reinterpret_cast<float4*>(d + G::at(4 * q, side ? T : -1, lz)) = v;
+            const int64_t dy = side ? (y0 + T == L ? -(int64_t)y0 : T) : (y0 == 0 ? L - 1 : -1);
+            cp_async16(d + G::at(4 * q, side ? T : -1, lz), g + (DIM == 3 ? (uint64_t)lz * plane : 0) + dy * (int64_t)row + 4 * q);
         }
         if (DIM == 3) {
             for (int idx = tid; idx < 2 * FACE / 4; idx += G::THREADS) {
                 const int side = idx / (FACE / 4), r = idx % (FACE / 4);
                 const int q = r % Q, ly = r / Q;
-                const int z = side ? (z0 + T == L ? 0 : z0 + T) : (z0 == 0 ? L - 1 : z0 - 1);
-                const float4 v = *reinterpret_cast<const float4*>(g + (uint64_t)z * plane + (uint64_t)(y0 + ly) * row + x0 + 4 * q);
-                *reinterpret_cast<float4*>(d + G::at(4 * q, ly, side ? T : -1)) = v;
+                const int64_t dz = side ? (z0 + T == L ? -(int64_t)z0 : T) : (z0 == 0 ? L - 1 : -1);
+                cp_async16(d + G::at(4 * q, ly, side ? T : -1), g + dz * (int64_t)plane + (uint64_t)ly * row + 4 * q);
             }
         }
-        for (int idx = tid; idx < 2 * FACE; idx += G::THREADS) {
-            const int side = idx / FACE, r = idx % FACE;
-            const int ly = r % T, lz = r / T;
-            const int x = side ? (x0 + T == L ? 0 : x0 + T) : (x0 == 0 ? L - 1 : x0 - 1);
-            d[G::at(side ? T : -1, ly, lz)] = g[(uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)(y0 + ly) * row + x];
+        // left halo = right face (side 1) of the left neighbour, right halo = left face (side 0) of the right one
+        for (int idx = tid; idx < 2 * FACE / 4; idx += G::THREADS) {
+            const int side = idx / (FACE / 4), r = idx % (FACE / 4);
+            const float* src = A.xface + (((uint64_t)c * A.ntiles + (side ? t_right : t_left)) * 2 + (side ? 0 : 1)) * FACE + 4 * r;
+            cp_async16(XF + (c * 2 + side) * FACE + 4 * r, src);
         }
+    }
+    cp_async_commit();
+    cp_async_wait_all();
+    __syncthreads();
+    for (int idx = tid; idx < 6 * FACE; idx += G::THREADS) {          // staged x faces -> halo columns
+        const int f = idx % FACE, side = (idx / FACE) & 1, c = idx / (2 * FACE);
+        sm[c * G::COMP + G::at(side ? T : -1, f % T, f / T)] = XF[idx];
     }
     __syncthreads();
 
@@ -281,15 +320,19 @@ __global__ void __launch_bounds__(HG<DIM, T>::THREADS) k_heis_tile(TileArgs A) {
         }
     }
 
-    // a7: interior back to HBM
+    // a7: interior back to HBM, and the tile's own x faces into the side array
     for (int c = 0; c < 3; ++c) {
-        float* g = A.s + (uint64_t)c * N;
+        float* g = A.s + (uint64_t)c * N + (DIM == 3 ? (uint64_t)z0 * plane : 0) + (uint64_t)y0 * row + x0;
         const float* d = sm + c * G::COMP;
         for (int idx = tid; idx < G::SITES / 4; idx += G::THREADS) {
-            const int q = idx % Q, ly = (idx / Q) % T, lz = idx / (Q * T);
-            *reinterpret_cast<float4*>(g + (uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)(y0 + ly) * row + x0 + 4 * q) =
-                *reinterpret_cast<const float4*>(d + G::at(4 * q, ly, lz));
+            const int q = idx % Q, yy = (idx / Q) % T, zz = idx / (Q * T);
+            *reinterpret_cast<float4*>(g + (DIM == 3 ? (uint64_t)zz * plane : 0) + (uint64_t)yy * row + 4 * q) =
+                *reinterpret_cast<const float4*>(d + G::at(4 * q, yy, zz));
         }
+    }
+    for (int idx = tid; idx < 6 * FACE; idx += G::THREADS) {
+        const int f = idx % FACE, side = (idx / FACE) & 1, c = idx / (2 * FACE);
+        A.xface[(((uint64_t)c * A.ntiles + t_self) * 2 + side) * FACE + f] = sm[c * G::COMP + G::at(side ? T - 1 : 0, f % T, f / T)];
     }
 }
 
@@ -350,14 +393,27 @@ int launch_tile(heis_ctx* h, TileArgs A) {
         ISING_CUDA_OK(cudaFuncSetAttribute(k_heis_tile<DIM, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
         attr_set = true;
     }
-    unsigned tiles = (unsigned)(A.B / 2) * A.B * (DIM == 3 ? A.B : 1);
+    A.ntiles = (uint32_t)A.B * A.B * (DIM == 3 ? A.B : 1);
+    const size_t entries = (size_t)3 * A.ntiles * 2 * G::FACE;
+    if (h->xface_T != T) {                       // (re)build the x-face copies from the spin planes
+        if (h->xface_bytes < entries * sizeof(float)) {
+            dev_free(h->d_xface);
+            h->xface_bytes = 0;
+            h->d_xface = (float*)dev_alloc(entries * sizeof(float));
+            if (!h->d_xface) return ISING_ENOMEM;
+            h->xface_bytes = entries * sizeof(float);
+        }
+        k_heis_build_xface<DIM, T><<<(unsigned)((entries + 255) / 256), 256, 0, hooks().stream>>>(h->d_s, h->d_xface, h->N, h->L, A.B, A.ntiles);
+        count_launch();
+        h->xface_T = T;
+    }
+    A.xface = h->d_xface;
     for (int C = 0; C < 2; ++C) {
         A.C = C;
-        k_heis_tile<DIM, T><<<tiles, G::THREADS, G::SMEM, hooks().stream>>>(A);
+        k_heis_tile<DIM, T><<<A.ntiles / 2, G::THREADS, G::SMEM, hooks().stream>>>(A);
         count_launch();
     }
     ISING_CUDA_OK(cudaGetLastError());
-    (void)h;
     return 0;
 }
 
@@ -422,6 +478,7 @@ void heis_destroy(heis_handle h) {
     cudaStreamSynchronize(hooks().stream);
     dev_free(h->d_s);
     dev_free(h->d_obs);
+    dev_free(h->d_xface);
     delete h;
 }
 
@@ -442,13 +499,14 @@ int heis_sweep(heis_handle h, double beta, int n_sweeps, int tile, int k_inner) 
         const uint64_t t_first = h->t + (uint64_t)pass * k_inner;
         int rc = 1;
         if (!h->force_generic) {
-            TileArgs A{h->d_s, h->N, t_first, h->L, h->L / T, 0, k_inner, k0, k1, betaf};
+            TileArgs A{h->d_s, nullptr, h->N, t_first, h->L, h->L / T, 0, k_inner, 0u, k0, k1, betaf};
             rc = tile_pass(h, A, T);
             if (rc < 0) return rc;
             if (rc == 0) h->last_path = "heis_tile";
         }
         if (rc == 1) {
             h->last_path = "heis_generic";
+            h->xface_T = 0;
             const unsigned blocks = (unsigned)((h->N / 2 + 255) / 256);
             for (int C = 0; C < (T == h->L ? 1 : 2); ++C)
                 for (int j = 0; j < k_inner; ++j)
@@ -489,6 +547,7 @@ int heis_copy_spins(heis_handle h, float* dst) {
 int heis_set_spins(heis_handle h, const float* src) {
     if (!h || !src) { set_error("heis_set_spins: NULL argument"); return ISING_EINVAL; }
     cudaStream_t st = hooks().stream;
+    h->xface_T = 0;
     ISING_CUDA_OK(cudaMemcpyAsync(h->d_s, src, 3 * h->N * sizeof(float), is_device_ptr(src) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st));
     ISING_CUDA_OK(cudaStreamSynchronize(st));
     return 0;
