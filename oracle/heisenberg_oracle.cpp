@@ -19,24 +19,27 @@
 //
 // H1 model, storage   H = -Σ_<ij> s_i·s_j; s[c][i], c = 0,1,2 = x,y,z, float; site index, fine and
 //                     coarse colours as S8c.1.
-// H2 direction D(w0,w1)  uniform point of the sphere from two 32-bit words (Archimedes: z uniform,
-//                     azimuth uniform):
-//                       z   = fma(float(w0 >> 8), 2^-23, -1)                       (exact, in [-1, 1))
+// H2 direction D(wa,wb)  uniform point of the sphere from 40 bits of two 32-bit words (Archimedes: z uniform,
+//                     azimuth uniform): z20 = wa >> 12, phi20 = ((wa & 0xfff) << 8) | (wb >> 24)
+//                       z   = fma(float(z20), 2^-19, -1)                           (exact, in [-1, 1))
 //                       rho = sqrt(fma(-z, z, 1))
-//                       q = w1 >> 29 (octant), t = float((w1 >> 5) & 0xffffff) * 2^-24 (exact); if q odd: t = t - 1
+//                       q = phi20 >> 17 (octant), t = float(phi20 & 0x1ffff) * 2^-17 (exact); if q odd: t = t - 1
 //                       x = t * PI_4;  x2 = x*x;  x3 = x2*x                       (azimuth - Q*pi/2, |x| <= pi/4)
 //                       sn = fma(x3, S(x2), x),  S = ((S9*x2 + S7)*x2 + S5)*x2 + S3    by fma, S_n = ±1/n!
 //                       cs = fma(x2, C(x2), 1),  C = (((C10*x2 + C8)*x2 + C6)*x2 + C4)*x2 + C2 by fma
 //                       Q = ((q + 1) >> 1) & 3:  (c, s) = (cs, sn), (-sn, cs), (-cs, -sn), (sn, -cs)
 //                       D = (rho*c, rho*s, z)
 //                     (Taylor polynomials: remainders x^11/11! and x^12/12! are below 2e-9 on |x| <= pi/4.)
-// H3 hot start        s_i = D(w0, w1), (w0, w1, ., .) = Philox(ctr = {i, 6, 0, 0}, key = seed).
-// H4 sweep randoms    site i in half-sweep H = 2t + c(i):  (w0, w1, w2, .) = Philox(ctr = {i >> 1, 5, lo32 H, hi32 H}).
-//                     (L even: the aligned pair (2j, 2j+1) holds one site of each colour, S8c.3.)
-// H5 update           proposal s' = D(w0, w1) (uniform, independent of s: symmetric).  Local field
+//                     The remaining 24 bits, wb & 0xffffff, are the uniform number of the acceptance test (H5).
+// H3 hot start        s_i = D(wa, wb), (wa, wb) = words (2h, 2h+1), h = i & 1, of Philox(ctr = {i >> 1, 6, 0, 0}, key = seed).
+// H4 sweep randoms    one call serves the two sites that are active in a 2x2 block of the xy plane: site (x, y, z) in
+//                     half-sweep H = 2t + c(i) takes (wa, wb) = words (2h, 2h+1), h = y & 1, of
+//                     Philox(ctr = {g, 5, lo32 H, hi32 H}),  g = (z*(L/2) + (y >> 1))*(L/2) + (x >> 1)
+//                     (L even: of the four sites of a block, one per row has the active colour).
+// H5 update           proposal s' = D(wa, wb) (uniform, independent of s: symmetric).  Local field
 //                     h = ((((s(i-e0) + s(i+e0)) + s(i-e1)) + s(i+e1)) + s(i-e2)) + s(i+e2), per component, in this order.
 //                     d = s' - s;  e = d_x*h_x;  e = fma(d_y, h_y, e);  e = fma(d_z, h_z, e)      (ΔE = -e)
-//                     accept if e >= 0; else u = float(w2 >> 8) * 2^-24 and accept iff u < P(float(β) * e).
+//                     accept if e >= 0; else u = float(wb & 0xffffff) * 2^-24 and accept iff u < P(float(β) * e).
 // H6 P(a), a < 0      (e^a to about 1e-6 relative)  tt = a * LOG2E; if tt < -64: P = 0; n = rint(tt) (ties to even);
 //                     f = tt - n (exact); g = f * LN2; p = 1 + g(1 + g(1/2 + g(1/6 + g(1/24 + g(1/120 + g(1/720 + g/5040))))))
 //                     by fma (Horner); P = p * 2^n (exact scaling).
@@ -81,11 +84,13 @@ const float S3 = (float)(-1.0 / 6.0), S5 = (float)(1.0 / 120.0), S7 = (float)(-1
 const float C2 = (float)(-1.0 / 2.0), C4 = (float)(1.0 / 24.0), C6 = (float)(-1.0 / 720.0), C8 = (float)(1.0 / 40320.0),
             C10 = (float)(-1.0 / 3628800.0);
 
-void direction(uint32_t w0, uint32_t w1, float out[3]) {
-    const float z = fmaf((float)(w0 >> 8), 0x1p-23f, -1.0f);
+void direction(uint32_t wa, uint32_t wb, float out[3]) {
+    const uint32_t z20 = wa >> 12;
+    const uint32_t phi20 = ((wa & 0xfffu) << 8) | (wb >> 24);
+    const float z = fmaf((float)z20, 0x1p-19f, -1.0f);
     const float rho = sqrtf(fmaf(-z, z, 1.0f));
-    const uint32_t q = w1 >> 29;
-    float t = (float)((w1 >> 5) & 0xffffffu) * 0x1p-24f;
+    const uint32_t q = phi20 >> 17;
+    float t = (float)(phi20 & 0x1ffffu) * 0x1p-17f;
     if (q & 1u) t = t - 1.0f;
     const float x = t * PI_4;
     const float x2 = x * x;
@@ -163,12 +168,18 @@ inline uint64_t neighbour(const Heis* h, uint64_t i, int d, int sign) {
 
 // H5: one Metropolis update of site i in half-sweep H.
 void update(Heis* h, uint64_t i, uint64_t H, float betaf) {
-    const uint32_t ctr[4] = {(uint32_t)(i >> 1), TAG_HSWEEP, (uint32_t)H, (uint32_t)(H >> 32)};
+    int xyz[3];
+    coords(h, i, xyz);
+    const uint64_t half_L = (uint64_t)(h->L / 2);
+    const uint64_t g = ((uint64_t)xyz[2] * half_L + (uint64_t)(xyz[1] >> 1)) * half_L + (uint64_t)(xyz[0] >> 1);
+    const int hw = xyz[1] & 1;
+    const uint32_t ctr[4] = {(uint32_t)g, TAG_HSWEEP, (uint32_t)H, (uint32_t)(H >> 32)};
     const uint32_t key[2] = {(uint32_t)h->seed, (uint32_t)(h->seed >> 32)};
     uint32_t w[4];
     philox(ctr, key, w);
+    const uint32_t wa = w[2 * hw], wb = w[2 * hw + 1];
     float sp[3];
-    direction(w[0], w[1], sp);
+    direction(wa, wb, sp);
     const uint64_t N = h->N;
     float hf[3];
     for (int c = 0; c < 3; ++c) {
@@ -185,7 +196,7 @@ void update(Heis* h, uint64_t i, uint64_t H, float betaf) {
     e = fmaf(dz, hf[2], e);
     bool acc = e >= 0.0f;
     if (!acc) {
-        const float u = (float)(w[2] >> 8) * 0x1p-24f;
+        const float u = (float)(wb & 0xffffffu) * 0x1p-24f;
         acc = u < accept_probability(betaf * e);
     }
     h->attempted++;
@@ -212,11 +223,11 @@ void* horacle_create(int dim, int L, uint64_t seed) {
     h->s.resize(3 * h->N);
     const uint32_t key[2] = {(uint32_t)seed, (uint32_t)(seed >> 32)};
     for (uint64_t i = 0; i < h->N; ++i) {   // H3
-        const uint32_t ctr[4] = {(uint32_t)i, TAG_HINIT, 0u, 0u};
+        const uint32_t ctr[4] = {(uint32_t)(i >> 1), TAG_HINIT, 0u, 0u};
         uint32_t w[4];
         philox(ctr, key, w);
         float v[3];
-        direction(w[0], w[1], v);
+        direction(w[2 * (i & 1)], w[2 * (i & 1) + 1], v);
         for (int c = 0; c < 3; ++c) h->s[c * h->N + i] = v[c];
     }
     return h;

@@ -9,9 +9,10 @@ from oracle import heisenberg as H
 
 
 # ---- H2: the direction map against its closed form in double precision -------------------------------
-def closed_form_direction(w0, w1):
-    z = (w0 >> 8) * 2.0 ** -23 - 1.0
-    phi = ((w1 >> 29) + ((w1 >> 5) & 0xFFFFFF) * 2.0 ** -24) * (math.pi / 4)
+def closed_form_direction(wa, wb):
+    z = (wa >> 12) * 2.0 ** -19 - 1.0
+    phi20 = ((wa & 0xFFF) << 8) | (wb >> 24)
+    phi = phi20 * 2.0 ** -17 * (math.pi / 4)          # octant + fraction, in units of pi/4
     rho = math.sqrt(max(0.0, 1.0 - z * z))
     return np.array([rho * math.cos(phi), rho * math.sin(phi), z])
 
@@ -21,9 +22,10 @@ def test_direction_matches_closed_form():
     words = [(int(a), int(b)) for a, b in rs.randint(0, 2 ** 32, size=(20000, 2), dtype=np.uint64)]
     # octant boundaries and extreme heights
     for q in range(8):
-        for frac in (0, 1, 0xFFFFFF, 0x800000):
-            words.append((0x80000000, (q << 29) | (frac << 5)))
-    words += [(0, 0), (0xFFFFFFFF, 0xFFFFFFFF), (0xFF, 0x1F), (0x100, 0x20)]
+        for frac in (0, 1, 0x1FFFF, 0x10000):
+            phi20 = (q << 17) | frac
+            words.append((0x80000000 | (phi20 >> 8), (phi20 & 0xFF) << 24))
+    words += [(0, 0), (0xFFFFFFFF, 0xFFFFFFFF), (0xFFF, 0xFF000000), (0x1000, 0x00FFFFFF)]
     worst = 0.0
     for w0, w1 in words:
         d = H.direction(w0, w1).astype(np.float64)
@@ -33,11 +35,12 @@ def test_direction_matches_closed_form():
 
 
 def test_direction_is_a_pure_function_of_the_stated_bits():
-    # H2 uses bits 31..8 of w0 and 31..5 of w1 only
-    a = H.direction(0x12345600, 0x89ABCDE0)
-    assert np.array_equal(a, H.direction(0x123456FF, 0x89ABCDFF))
-    assert not np.array_equal(a, H.direction(0x12345700, 0x89ABCDE0))
-    assert not np.array_equal(a, H.direction(0x12345600, 0x89ABCE00))
+    # H2 uses all of wa and bits 31..24 of wb only (the low 24 bits of wb are the acceptance number)
+    a = H.direction(0x12345678, 0x89ABCDEF)
+    assert np.array_equal(a, H.direction(0x12345678, 0x89000000))
+    assert not np.array_equal(a, H.direction(0x12345679, 0x89ABCDEF))
+    assert not np.array_equal(a, H.direction(0x12345678, 0x8AABCDEF))
+    assert not np.array_equal(a, H.direction(0x12346678, 0x89ABCDEF))
 
 
 # ---- H6: the acceptance probability against exp ---------------------------------------------------
@@ -79,8 +82,9 @@ def test_hot_start_moments_of_the_uniform_sphere():
     # the first site follows H3 literally
     w = H.philox([0, 6, 0, 0], [11, 0])
     assert np.array_equal(o.spins()[:, 0], H.direction(w[0], w[1]))
-    w = H.philox([77, 6, 0, 0], [11, 0])
-    assert np.array_equal(o.spins()[:, 77], H.direction(w[0], w[1]))
+    assert np.array_equal(o.spins()[:, 1], H.direction(w[2], w[3]))
+    w = H.philox([77 >> 1, 6, 0, 0], [11, 0])
+    assert np.array_equal(o.spins()[:, 77], H.direction(w[2], w[3]))
 
 
 # ---- H8: energy of spin spirals (closed form), pins the neighbour indexing of E in 1D/2D/3D ----------
@@ -132,8 +136,12 @@ def test_beta_zero_accepts_everything():
     # and the last proposal of site 0 (colour 0, inner sweep t = 5, H = 10) is what H4/H2 say
     w = H.philox([0, 5, 10, 0], [3, 0])
     assert np.array_equal(o.spins()[:, 0], H.direction(w[0], w[1]))
-    w = H.philox([1 >> 1, 5, 11, 0], [3, 0])       # site 1: colour 1, H = 11, pair index 0
+    assert np.array_equal(o.spins()[:, 8 + 1], H.direction(w[2], w[3]))     # (1, 1): same block, row 1, colour 0
+    w = H.philox([0, 5, 11, 0], [3, 0])            # colour 1, H = 11: sites (1, 0) and (0, 1) of block 0
     assert np.array_equal(o.spins()[:, 1], H.direction(w[0], w[1]))
+    assert np.array_equal(o.spins()[:, 8], H.direction(w[2], w[3]))
+    w = H.philox([(5 >> 1) * 4 + (6 >> 1), 5, 10, 0], [3, 0])              # site (6, 4): block row 2, block column 3
+    assert np.array_equal(o.spins()[:, 4 * 8 + 6], H.direction(w[0], w[1]))
 
 
 # ---- exact finite systems: Joyce (1967), ring of N classical Heisenberg spins -------------------------
