@@ -40,16 +40,17 @@ constexpr uint32_t kTagHeisInit = 6u;    // H3
 
 struct f3 { float x, y, z; };
 
-// H2: two random words -> a uniform direction.
-__device__ __forceinline__ f3 heis_direction(uint32_t w0, uint32_t w1) {
+// H2: 40 bits of two random words -> a uniform direction (the low 24 bits of wb are the acceptance number).
+__device__ __forceinline__ f3 heis_direction(uint32_t wa, uint32_t wb) {
     constexpr float PI_4 = (float)0.78539816339744830962;
     constexpr float S3 = (float)(-1.0 / 6.0), S5 = (float)(1.0 / 120.0), S7 = (float)(-1.0 / 5040.0), S9 = (float)(1.0 / 362880.0);
     constexpr float C2 = (float)(-1.0 / 2.0), C4 = (float)(1.0 / 24.0), C6 = (float)(-1.0 / 720.0), C8 = (float)(1.0 / 40320.0),
                     C10 = (float)(-1.0 / 3628800.0);
-    const float z = __fmaf_rn(__uint2float_rn(w0 >> 8), 0x1p-23f, -1.0f);
+    const uint32_t phi20 = __funnelshift_l(wb, wa, 8) & 0xfffffu;       // ((wa & 0xfff) << 8) | (wb >> 24)
+    const float z = __fmaf_rn(__uint2float_rn(wa >> 12), 0x1p-19f, -1.0f);
     const float rho = __fsqrt_rn(__fmaf_rn(-z, z, 1.0f));
-    const uint32_t q = w1 >> 29;
-    float t = __fmul_rn(__uint2float_rn((w1 >> 5) & 0xffffffu), 0x1p-24f);
+    const uint32_t q = phi20 >> 17;
+    float t = __fmul_rn(__uint2float_rn(phi20 & 0x1ffffu), 0x1p-17f);
     if (q & 1u) t = __fsub_rn(t, 1.0f);
     const float x = __fmul_rn(t, PI_4);
     const float x2 = __fmul_rn(x, x);
@@ -91,18 +92,16 @@ __device__ __forceinline__ float heis_accept_probability(float a) {
     return tt < -64.0f ? 0.0f : P;        // (for tt outside [-64, 0] P is meaningless and not used)
 }
 
-// H5 given the old spin and the local field; returns true and the new spin if the move is accepted.
-__device__ __forceinline__ bool heis_update(uint32_t pair, uint64_t H, uint32_t k0, uint32_t k1, float betaf,
-                                            const f3& s, const f3& h, f3& sp) {
-    const u32x4 w = philox4x32_10(pair, kTagHeisSweep, (uint32_t)H, (uint32_t)(H >> 32), k0, k1);
-    sp = heis_direction(w.x, w.y);
+// H5 given the two random words, the old spin and the local field; returns true and the new spin if the move is accepted.
+__device__ __forceinline__ bool heis_update(uint32_t wa, uint32_t wb, float betaf, const f3& s, const f3& h, f3& sp) {
+    sp = heis_direction(wa, wb);
     const float dx = __fsub_rn(sp.x, s.x), dy = __fsub_rn(sp.y, s.y), dz = __fsub_rn(sp.z, s.z);
     float e = __fmul_rn(dx, h.x);
     e = __fmaf_rn(dy, h.y, e);
     e = __fmaf_rn(dz, h.z, e);
     // both sides of "e >= 0 or u < P" are evaluated (a warp nearly always holds both cases): for e >= 0 the value
     // of P is not used
-    const float u = __fmul_rn(__uint2float_rn(w.z >> 8), 0x1p-24f);
+    const float u = __fmul_rn(__uint2float_rn(wb & 0xffffffu), 0x1p-24f);
     const float P = heis_accept_probability(__fmul_rn(betaf, e));
     return (e >= 0.0f) | (u < P);
 }
@@ -111,12 +110,12 @@ __device__ __forceinline__ bool heis_update(uint32_t pair, uint64_t H, uint32_t 
 __global__ void k_heis_hot_start(float* __restrict__ s, uint64_t N, uint32_t k0, uint32_t k1) {
     const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
-    const u32x4 w = philox4x32_10((uint32_t)i, kTagHeisInit, 0u, 0u, k0, k1);
-    const f3 v = heis_direction(w.x, w.y);
+    const u32x4 w = philox4x32_10((uint32_t)(i >> 1), kTagHeisInit, 0u, 0u, k0, k1);
+    const f3 v = (i & 1) ? heis_direction(w.z, w.w) : heis_direction(w.x, w.y);
     s[i] = v.x; s[N + i] = v.y; s[2 * N + i] = v.z;
 }
 
-// ---- generic half-sweep: one thread per aligned pair, live neighbours ------------------------------------
+// ---- generic half-sweep: one thread per 2x2 block of the xy plane (= one Philox call, H4), live neighbours --------
 struct GenArgs {
     float* s;
     uint64_t N, H;
@@ -126,37 +125,38 @@ struct GenArgs {
 };
 
 __global__ void k_heis_generic(GenArgs A) {
-    const uint64_t p = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= A.N / 2) return;
-    const int L = A.L;
-    const uint64_t i0 = 2 * p;
-    const int y = A.dim > 1 ? (int)((i0 / L) % L) : 0;
-    const int z = A.dim > 2 ? (int)(i0 / ((uint64_t)L * L)) : 0;
-    const int x = (int)(i0 % L) + ((y + z + A.c) & 1);
-    if (A.T != L && ((x / A.T + y / A.T + z / A.T) & 1) != A.C) return;
-    const uint64_t i = i0 - (i0 % L) + x;
+    const uint64_t g = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (g >= A.N / 4) return;
+    const int L = A.L, hl = L / 2;
+    const int bx = (int)(g % hl), by = (int)((g / hl) % hl), z = (int)(g / ((uint64_t)hl * hl));
+    // T is even: the block lies in one tile
+    if (A.T != L && (((2 * bx) / A.T + (2 * by) / A.T + z / A.T) & 1) != A.C) return;
+    const u32x4 w = philox4x32_10((uint32_t)g, kTagHeisSweep, (uint32_t)A.H, (uint32_t)(A.H >> 32), A.k0, A.k1);
     const uint64_t N = A.N;
     const float* sx = A.s;
     const float* sy = A.s + N;
     const float* sz = A.s + 2 * N;
-    const uint64_t xm = i - x + (x == 0 ? L - 1 : x - 1), xp = i - x + (x == L - 1 ? 0 : x + 1);
-    f3 h{__fadd_rn(sx[xm], sx[xp]), __fadd_rn(sy[xm], sy[xp]), __fadd_rn(sz[xm], sz[xp])};
-    if (A.dim > 1) {
+    for (int hw = 0; hw < 2; ++hw) {         // the two rows of the block; their active sites are not neighbours
+        const int y = 2 * by + hw;
+        const int x = 2 * bx + ((y + z + A.c) & 1);
+        const uint64_t i = ((uint64_t)z * L + y) * L + x;
+        const uint64_t xm = i - x + (x == 0 ? L - 1 : x - 1), xp = i - x + (x == L - 1 ? 0 : x + 1);
+        f3 h{__fadd_rn(sx[xm], sx[xp]), __fadd_rn(sy[xm], sy[xp]), __fadd_rn(sz[xm], sz[xp])};
         const uint64_t row = (uint64_t)L;
         const uint64_t ym = y == 0 ? i + row * (L - 1) : i - row, yp = y == L - 1 ? i - row * (L - 1) : i + row;
         h.x = __fadd_rn(h.x, sx[ym]); h.y = __fadd_rn(h.y, sy[ym]); h.z = __fadd_rn(h.z, sz[ym]);
         h.x = __fadd_rn(h.x, sx[yp]); h.y = __fadd_rn(h.y, sy[yp]); h.z = __fadd_rn(h.z, sz[yp]);
-    }
-    if (A.dim > 2) {
-        const uint64_t pl = (uint64_t)L * L;
-        const uint64_t zm = z == 0 ? i + pl * (L - 1) : i - pl, zp = z == L - 1 ? i - pl * (L - 1) : i + pl;
-        h.x = __fadd_rn(h.x, sx[zm]); h.y = __fadd_rn(h.y, sy[zm]); h.z = __fadd_rn(h.z, sz[zm]);
-        h.x = __fadd_rn(h.x, sx[zp]); h.y = __fadd_rn(h.y, sy[zp]); h.z = __fadd_rn(h.z, sz[zp]);
-    }
-    const f3 s{sx[i], sy[i], sz[i]};
-    f3 sp;
-    if (heis_update((uint32_t)p, A.H, A.k0, A.k1, A.betaf, s, h, sp)) {
-        A.s[i] = sp.x; A.s[N + i] = sp.y; A.s[2 * N + i] = sp.z;
+        if (A.dim > 2) {
+            const uint64_t pl = (uint64_t)L * L;
+            const uint64_t zm = z == 0 ? i + pl * (L - 1) : i - pl, zp = z == L - 1 ? i - pl * (L - 1) : i + pl;
+            h.x = __fadd_rn(h.x, sx[zm]); h.y = __fadd_rn(h.y, sy[zm]); h.z = __fadd_rn(h.z, sz[zm]);
+            h.x = __fadd_rn(h.x, sx[zp]); h.y = __fadd_rn(h.y, sy[zp]); h.z = __fadd_rn(h.z, sz[zp]);
+        }
+        const f3 s{sx[i], sy[i], sz[i]};
+        f3 sp;
+        if (heis_update(hw ? w.z : w.x, hw ? w.w : w.y, A.betaf, s, h, sp)) {
+            A.s[i] = sp.x; A.s[N + i] = sp.y; A.s[2 * N + i] = sp.z;
+        }
     }
 }
 
@@ -164,29 +164,36 @@ __global__ void k_heis_generic(GenArgs A) {
 // Shared-memory tile of one component: [ZP][YP][XP] floats, interior site (lx, ly, lz) at (lz+1, ly+1, lx+4) (2D:
 // ZP = 1, no z offset): column 3 and column T+4 are the x halos, and the interior rows start 16-byte aligned.
 // XP is even, so that the active sites of a row and those of the next row, which have the other parity, fall
-// into different banks; T + 8 (T + 4 for T = 8: row offsets 12r mod 32) also keeps the rows of equal parity that one
-// warp touches apart.
+// into different banks; the pitches and the order in which a thread takes the two rows of its block (swap_rows) were
+// chosen by enumerating the banks a warp touches: no conflicts in the update loop for any supported (dim, T).
 template <int DIM, int T>
 struct HG {
-    static constexpr int XP = T <= 8 ? T + 4 : T + 8;          // T + 4: the right halo of a row sits in the unused column 0 of the next
+    static constexpr int XP = T <= 16 ? T + 4 : T + 8;          // T + 4: the right halo of a row sits in the unused column 0 of the next
     static constexpr int YP = T + 2;
     static constexpr int ZP = DIM == 3 ? T + 2 : 1;
-    static constexpr int COMP = XP * YP * ZP + 4;               // floats per component
+    static constexpr int ZS = XP * YP + (DIM == 3 && T == 4 ? 4 : 0);   // layer pitch
+    static constexpr int COMP = ZS * ZP + 4;                    // floats per component
     static constexpr int SITES = DIM == 3 ? T * T * T : T * T;
     static constexpr int THREADS = SITES / 4 < 32 ? 32 : (SITES / 4 > 512 ? 512 : SITES / 4);
-    // update loop: thread = (pair column px, row r); per half-sweep it updates UPT sites RS rows apart.  RS rows are an
-    // even number of rows (2D) / of z layers (3D), so the column parity of a thread's active sites is fixed.
+    // update loop: an item = a 2x2 block of the xy plane (one Philox call, two active sites per half-sweep, H4);
+    // thread = (pair column px, row pair rp[, layer lz]) takes IPT items, THREADS / (T/2) row pairs (2D) or
+    // THREADS / (T*T/4) layers (3D) apart; both are even, so the parities a thread sees are fixed.
     static constexpr int HALF = T / 2;
-    static constexpr int RS = THREADS / HALF;
-    static constexpr int UPT = SITES / 2 / THREADS;
-    static constexpr int OSTEP = DIM == 3 ? (RS / T) * XP * YP : RS * XP;
-    static_assert(THREADS % HALF == 0 && UPT * THREADS * 2 == SITES, "thread mapping");
-    static_assert(UPT == 1 || (DIM == 3 ? (RS % T == 0 && (RS / T) % 2 == 0) : RS % 2 == 0), "fixed parity per thread");
+    static constexpr int ITEMS = SITES / 4;
+    static constexpr int IPT = ITEMS / THREADS > 0 ? ITEMS / THREADS : 1;
+    static constexpr int RSTEP = THREADS / HALF;                       // row pairs per round of THREADS items
+    static constexpr int OSTEP = DIM == 3 ? (RSTEP / HALF) * ZS : 2 * RSTEP * XP;
+    // 1: the thread takes row 2rp+1 of its block first
+    __device__ static constexpr int swap_rows(int px, int rp) {
+        return DIM == 2 && T == 64 ? (px >> 4) & 1 : (DIM == 3 && T == 8 ? 0 : rp & 1);
+    }
+    static_assert(THREADS % HALF == 0 && (ITEMS < THREADS || IPT * THREADS == ITEMS), "thread mapping");
+    static_assert(IPT == 1 || (DIM == 3 ? (RSTEP % HALF == 0 && (RSTEP / HALF) % 2 == 0) : RSTEP % 2 == 0), "fixed parity per thread");
     static constexpr int FACE = SITES / T;                       // sites of one face
     // shared memory: three components of the tile + halo, then the staged x faces XF[c][side][FACE]
     static constexpr size_t SMEM = (size_t)(3 * COMP + 6 * FACE) * sizeof(float);
     __device__ static constexpr int at(int lx, int ly, int lz) {
-        return ((DIM == 3 ? lz + 1 : 0) * YP + (ly + 1)) * XP + lx + 4;
+        return (DIM == 3 ? lz + 1 : 0) * ZS + (ly + 1) * XP + lx + 4;
     }
 };
 
@@ -289,31 +296,43 @@ __global__ void __launch_bounds__(HG<DIM, T>::THREADS) k_heis_tile(TileArgs A) {
     float* const SX = sm;
     float* const SY = sm + G::COMP;
     float* const SZ = sm + 2 * G::COMP;
-    const int px = tid % G::HALF, r = tid / G::HALF;
-    const int ly = r % T, lz = r / T;
-    const int par = (ly + lz) & 1;                                    // x0, y0, z0 are even
-    const int o_row = G::at(2 * px, ly, lz);
-    const uint32_t p_base = (uint32_t)(((uint64_t)(z0 + lz) * plane * (DIM == 3) + (uint64_t)(y0 + ly) * row + (uint64_t)x0) >> 1) + (uint32_t)px;
-    const uint32_t p_step = DIM == 3 ? (uint32_t)(G::RS / T) * (uint32_t)(plane >> 1) : (uint32_t)G::RS * (uint32_t)(L >> 1);
+    // thread -> block (px, rp, lz); some threads take their two rows in the order (2rp+1, 2rp), so that the lanes of a
+    // warp touch rows of both parities at the same time (different banks)
+    const int px = tid % G::HALF, rp = (tid / G::HALF) % G::HALF, lz = tid / (G::HALF * G::HALF);
+    const int sw = G::swap_rows(px, rp);
+    const int rowA = 2 * rp + sw, rowB = 2 * rp + 1 - sw;
+    const int parA = (rowA + lz) & 1;                                  // x0, y0, z0 are even
+    const int oA_row = G::at(2 * px, rowA, lz), oB_row = G::at(2 * px, rowB, lz);
+    const uint32_t hl = (uint32_t)(L >> 1);
+    const uint32_t g_base = ((uint32_t)(z0 + lz) * hl * (DIM == 3) + (uint32_t)(y0 >> 1) + (uint32_t)rp) * hl + (uint32_t)(x0 >> 1) + (uint32_t)px;
+    const uint32_t g_step = DIM == 3 ? (uint32_t)(G::RSTEP / G::HALF) * hl * hl : (uint32_t)G::RSTEP * hl;
+    const bool live = G::ITEMS >= G::THREADS || tid < G::ITEMS;
     for (int j = 0; j < A.k; ++j) {
         for (int c = 0; c < 2; ++c) {
             const uint64_t H = 2 * (A.t_first + (uint64_t)j) + (uint64_t)c;
-            const int o0 = o_row + ((par + c) & 1);
+            const int aA = (parA + c) & 1;
+            if (live) {
 #pragma unroll
-            for (int u = 0; u < G::UPT; ++u) {
-                const int o = o0 + u * G::OSTEP;
-                f3 h{__fadd_rn(SX[o - 1], SX[o + 1]), __fadd_rn(SY[o - 1], SY[o + 1]), __fadd_rn(SZ[o - 1], SZ[o + 1])};
-                h.x = __fadd_rn(h.x, SX[o - G::XP]); h.y = __fadd_rn(h.y, SY[o - G::XP]); h.z = __fadd_rn(h.z, SZ[o - G::XP]);
-                h.x = __fadd_rn(h.x, SX[o + G::XP]); h.y = __fadd_rn(h.y, SY[o + G::XP]); h.z = __fadd_rn(h.z, SZ[o + G::XP]);
-                if (DIM == 3) {
-                    constexpr int ZS = G::XP * G::YP;
-                    h.x = __fadd_rn(h.x, SX[o - ZS]); h.y = __fadd_rn(h.y, SY[o - ZS]); h.z = __fadd_rn(h.z, SZ[o - ZS]);
-                    h.x = __fadd_rn(h.x, SX[o + ZS]); h.y = __fadd_rn(h.y, SY[o + ZS]); h.z = __fadd_rn(h.z, SZ[o + ZS]);
-                }
-                const f3 s{SX[o], SY[o], SZ[o]};
-                f3 sp;
-                if (heis_update(p_base + (uint32_t)u * p_step, H, A.k0, A.k1, A.betaf, s, h, sp)) {
-                    SX[o] = sp.x; SY[o] = sp.y; SZ[o] = sp.z;
+                for (int n = 0; n < G::IPT; ++n) {
+                    const u32x4 w = philox4x32_10(g_base + (uint32_t)n * g_step, kTagHeisSweep, (uint32_t)H, (uint32_t)(H >> 32), A.k0, A.k1);
+#pragma unroll
+                    for (int second = 0; second < 2; ++second) {
+                        const int o = (second ? oB_row + 1 - aA : oA_row + aA) + n * G::OSTEP;
+                        const bool odd_row = (second != 0) != (sw != 0);            // row 2rp+1 takes words 2, 3
+                        f3 h{__fadd_rn(SX[o - 1], SX[o + 1]), __fadd_rn(SY[o - 1], SY[o + 1]), __fadd_rn(SZ[o - 1], SZ[o + 1])};
+                        h.x = __fadd_rn(h.x, SX[o - G::XP]); h.y = __fadd_rn(h.y, SY[o - G::XP]); h.z = __fadd_rn(h.z, SZ[o - G::XP]);
+                        h.x = __fadd_rn(h.x, SX[o + G::XP]); h.y = __fadd_rn(h.y, SY[o + G::XP]); h.z = __fadd_rn(h.z, SZ[o + G::XP]);
+                        if (DIM == 3) {
+                            constexpr int ZS = G::ZS;
+                            h.x = __fadd_rn(h.x, SX[o - ZS]); h.y = __fadd_rn(h.y, SY[o - ZS]); h.z = __fadd_rn(h.z, SZ[o - ZS]);
+                            h.x = __fadd_rn(h.x, SX[o + ZS]); h.y = __fadd_rn(h.y, SY[o + ZS]); h.z = __fadd_rn(h.z, SZ[o + ZS]);
+                        }
+                        const f3 s{SX[o], SY[o], SZ[o]};
+                        f3 sp;
+                        if (heis_update(odd_row ? w.z : w.x, odd_row ? w.w : w.y, A.betaf, s, h, sp)) {
+                            SX[o] = sp.x; SY[o] = sp.y; SZ[o] = sp.z;
+                        }
+                    }
                 }
             }
             __syncthreads();
@@ -507,7 +526,7 @@ int heis_sweep(heis_handle h, double beta, int n_sweeps, int tile, int k_inner) 
         if (rc == 1) {
             h->last_path = "heis_generic";
             h->xface_T = 0;
-            const unsigned blocks = (unsigned)((h->N / 2 + 255) / 256);
+            const unsigned blocks = (unsigned)((h->N / 4 + 255) / 256);
             for (int C = 0; C < (T == h->L ? 1 : 2); ++C)
                 for (int j = 0; j < k_inner; ++j)
                     for (int c = 0; c < 2; ++c) {
