@@ -278,11 +278,12 @@ def run_amsc(P, torch, a) -> None:
 
 def heis_alu_peak(dim: int, sm_mhz: float = 1965.0) -> dict:
     """Issue ceiling of one Heisenberg update on B200: the operations H2-H6 state, costed with the
-    pipe rates measured in profiles/r01_microbench.md.  Per warp-update, in SMSP-cycles: Philox4x32-10 84.6 (measured),
-    every stated float / convert / select operation and every shared-memory access one issue slot."""
-    fp = 34 + (3 + 6 * (dim - 1)) + 3 + 3 + 2 + 16 + 3       # direction, field adds, d, e, u, P(beta*e), decision
+    pipe rates measured in profiles/r01_microbench.md.  Per warp-update, in SMSP-cycles: half a Philox4x32-10 call
+    (84.6 measured per call, one call serves two updates), every stated float / convert / bit-field / select operation
+    and every shared-memory access one issue slot."""
+    fp = 35 + (3 + 6 * (dim - 1)) + 3 + 3 + 3 + 16 + 3       # direction, field adds, d, e, u, P(beta*e), decision
     lsu = 3 * (2 * dim + 1) + 3                              # neighbour + own loads, store of an accepted spin
-    cycles = 84.6 + fp + lsu
+    cycles = 84.6 / 2 + fp + lsu
     return {"cycles_per_warp_update": cycles, "peak": 148 * 4 * sm_mhz * 1e6 / cycles * 32 / 1e9}
 
 
@@ -292,8 +293,8 @@ def run_heisenberg(P, torch, a) -> None:
     L=256).  One JSON line per (dim, L, tile, k); the first carries the CPU oracle timed on a small lattice."""
     single = a.L != 16384
     variants = [(a.dim, a.L, a.tile, a.k)] if single else \
-        [(2, 8192, 32, 1), (2, 8192, 32, 4), (2, 8192, 32, 16), (2, 8192, 16, 16), (2, 8192, 64, 16),
-         (3, 256, 8, 1), (3, 256, 8, 4), (3, 256, 16, 4)]
+        [(2, 8192, 32, 1), (2, 8192, 32, 4), (2, 8192, 32, 16), (2, 8192, 64, 1), (2, 8192, 64, 4), (2, 8192, 64, 16),
+         (3, 256, 8, 1), (3, 256, 8, 4), (3, 256, 8, 16), (3, 256, 16, 4)]
     hbm_gbs, _, sm_mhz = measured_peaks()
     first = True
     for dim, L, T, k in variants:
@@ -317,11 +318,14 @@ def run_heisenberg(P, torch, a) -> None:
                 "vs_baseline": None, "dtype": "f32", "data": "synthetic", "gpu_launches": int(P.ising_kernel_launches() - n0),
                 "config": {"workload": f"Heisenberg dim={dim} L={L} seed=3 beta={beta} tile={T} k={k}; {3 * 4 * L ** dim / 1e6:.0f} MB of spins (> L2)",
                            "kernel_path": g.sweep_path()},
-                "roofline": {"bound": "alu", "achieved": upd, "peak": alu["peak"], "unit": "updates/ns", "frac": upd / alu["peak"],
-                             "traffic": None, "cycles_per_warp_update": alu["cycles_per_warp_update"],
-                             "hbm_algorithmic_gbs": upd * bytes_per_update, "bytes_per_update": bytes_per_update,
-                             "hbm_frac": upd * bytes_per_update / hbm_gbs,
-                             "note": "peak = issue ceiling of the stated operations (DESIGN.md 7.4); HBM is not the bound for k >= 2"}}
+                "roofline": ({"bound": "alu", "achieved": upd, "peak": alu["peak"], "unit": "updates/ns", "frac": upd / alu["peak"]}
+                             if alu["peak"] * bytes_per_update < hbm_gbs else
+                             {"bound": "hbm", "achieved": upd * bytes_per_update, "peak": hbm_gbs, "unit": "GB/s",
+                              "frac": upd * bytes_per_update / hbm_gbs})}
+        line["roofline"].update({"traffic": None, "alu_peak_updates_per_ns": alu["peak"], "alu_frac": upd / alu["peak"],
+                                 "cycles_per_warp_update": alu["cycles_per_warp_update"], "bytes_per_update": bytes_per_update,
+                                 "hbm_algorithmic_gbs": upd * bytes_per_update, "hbm_frac": upd * bytes_per_update / hbm_gbs,
+                                 "note": "bound = the lower of the HBM roofline (algorithmic bytes) and the issue ceiling of the stated operations (DESIGN.md 7.4)"})
         g.destroy()
         if first and not a.no_extras:
             from oracle import heisenberg as HO

@@ -189,6 +189,8 @@ struct HG {
     }
     static_assert(THREADS % HALF == 0 && (ITEMS < THREADS || IPT * THREADS == ITEMS), "thread mapping");
     static_assert(IPT == 1 || (DIM == 3 ? (RSTEP % HALF == 0 && (RSTEP / HALF) % 2 == 0) : RSTEP % 2 == 0), "fixed parity per thread");
+    // 2D T=64: 42 registers for a third 512-thread CTA per SM (+15 % at k=1, -3 % at k=16); 0 = the compiler's own choice
+    static constexpr int MIN_CTAS = DIM == 2 && T == 64 ? 3 : 0;
     static constexpr int FACE = SITES / T;                       // sites of one face
     // shared memory: three components of the tile + halo, then the staged x faces XF[c][side][FACE]
     static constexpr size_t SMEM = (size_t)(3 * COMP + 6 * FACE) * sizeof(float);
@@ -235,7 +237,7 @@ __global__ void k_heis_build_xface(const float* __restrict__ s, float* __restric
 
 // One CTA per tile of the launch's coarse colour (job -> (tx/2, ty, tz) row-major).
 template <int DIM, int T>
-__global__ void __launch_bounds__(HG<DIM, T>::THREADS) k_heis_tile(TileArgs A) {
+__global__ void __launch_bounds__(HG<DIM, T>::THREADS, HG<DIM, T>::MIN_CTAS) k_heis_tile(TileArgs A) {
     using G = HG<DIM, T>;
     extern __shared__ __align__(16) float sm[];
     const int tid = threadIdx.x;
