@@ -215,8 +215,8 @@ struct TileArgs {
 //     xface[((c * ntiles + tile) * 2 + side) * FACE + lz * T + ly],   tile = (tz * B + ty) * B + tx,
 // written with the tile's write-back and read by the two x neighbours as contiguous 16-byte copies.  The spin planes
 // stay complete and current; the host rebuilds the copies (k_heis_build_xface) when something else wrote the spins.
-__device__ __forceinline__ void cp_async16(float* smem, const float* gmem) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((uint32_t)__cvta_generic_to_shared(smem)), "l"(gmem) : "memory");
+__device__ __forceinline__ void cp_async16_addr(uint32_t smem_addr, const float* gmem) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr), "l"(gmem) : "memory");
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
@@ -256,41 +256,72 @@ __global__ void __launch_bounds__(HG<DIM, T>::THREADS, HG<DIM, T>::MIN_CTAS) k_h
     const uint32_t t_self = tile_row + tx, t_left = tile_row + (tx == 0 ? B - 1 : tx - 1), t_right = tile_row + (tx == B - 1 ? 0 : tx + 1);
     float* const XF = sm + 3 * G::COMP;
 
-    // a3: interior rows, the y / z faces and the x-face copies as 16-byte asynchronous copies
-    for (int c = 0; c < 3; ++c) {
-        const float* g = A.s + (uint64_t)c * N + (DIM == 3 ? (uint64_t)z0 * plane : 0) + (uint64_t)y0 * row + x0;
-        float* d = sm + c * G::COMP;
-        for (int idx = tid; idx < G::SITES / 4; idx += G::THREADS) {
-            const int q = idx % Q, ly = (idx / Q) % T, lz = idx / (Q * T);
-            cp_async16(d + G::at(4 * q, ly, lz), g + (DIM == 3 ? (uint64_t)lz * plane : 0) + (uint64_t)ly * row + 4 * q);
-        }
-        for (int idx = tid; idx < 2 * FACE / 4; idx += G::THREADS) {
-            const int side = idx / (FACE / 4), r = idx % (FACE / 4);
-            const int q = r % Q, lz = r / Q;
-            const int64_t dy = side ? (y0 + T == L ? -(int64_t)y0 : T) : (y0 == 0 ? L - 1 : -1);
-            cp_async16(d + G::at(4 * q, side ? T : -1, lz), g + (DIM == 3 ? (uint64_t)lz * plane : 0) + dy * (int64_t)row + 4 * q);
-        }
-        if (DIM == 3) {
-            for (int idx = tid; idx < 2 * FACE / 4; idx += G::THREADS) {
-                const int side = idx / (FACE / 4), r = idx % (FACE / 4);
-                const int q = r % Q, ly = r / Q;
-                const int64_t dz = side ? (z0 + T == L ? -(int64_t)z0 : T) : (z0 == 0 ? L - 1 : -1);
-                cp_async16(d + G::at(4 * q, ly, side ? T : -1), g + dz * (int64_t)plane + (uint64_t)ly * row + 4 * q);
+    // a3: interior rows, the y / z faces and the x-face copies as 16-byte asynchronous copies.  Every offset is worked
+    // out once per thread, the loop over the three components is innermost.  Float offsets inside one component are
+    // below N <= 2^32.
+    const uint32_t sm_addr = (uint32_t)__cvta_generic_to_shared(sm);
+    const uint32_t origin = (uint32_t)((DIM == 3 ? (uint64_t)z0 * plane : 0) + (uint64_t)y0 * row + (uint64_t)x0);
+    constexpr int INT_ROUNDS = (G::SITES / 4 + G::THREADS - 1) / G::THREADS;
+    uint32_t int_g[INT_ROUNDS], int_s[INT_ROUNDS];                    // interior 16-byte pieces of this thread (write-back too)
+#pragma unroll
+    for (int n = 0; n < INT_ROUNDS; ++n) {
+        const int idx = tid + n * G::THREADS;
+        const int q = idx % Q, yy = (idx / Q) % T, zz = idx / (Q * T);
+        int_g[n] = origin + (uint32_t)(DIM == 3 ? zz : 0) * (uint32_t)plane + (uint32_t)yy * (uint32_t)L + 4u * q;
+        int_s[n] = (uint32_t)G::at(4 * q, yy, zz);
+    }
+    const bool int_live = G::SITES / 4 >= G::THREADS || tid < G::SITES / 4;
+    if (int_live) {
+#pragma unroll
+        for (int n = 0; n < INT_ROUNDS; ++n)
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+                cp_async16_addr(sm_addr + 4u * (c * G::COMP + int_s[n]), A.s + (uint64_t)c * N + int_g[n]);
+    }
+    // faces: FQ = FACE/4 pieces per face; kinds 0,1 = y faces, 2,3 = x-face copies, 4,5 = z faces (3D): one per thread
+    constexpr int FQ = FACE / 4;
+    constexpr int NFACE = (DIM == 3 ? 6 : 4) * FQ;
+    static_assert(NFACE <= G::THREADS, "one face piece per thread");
+    if (tid < NFACE) {
+        const int kind = tid / FQ, r = tid % FQ, side = kind & 1;
+        const float* src;
+        uint64_t cstride;                                             // floats between the components at the source
+        uint32_t dst;
+        if ((kind >> 1) == 1) {
+            // left halo = right face (side 1) of the left neighbour, right halo = left face (side 0) of the right one
+            src = A.xface + ((uint64_t)(side ? t_right : t_left) * 2 + (side ? 0 : 1)) * FACE + 4 * r;
+            cstride = (uint64_t)A.ntiles * 2 * FACE;
+            dst = (uint32_t)(3 * G::COMP + side * FACE + 4 * r);     // XF[c][side][.]: component stride 2*FACE, see below
+        } else {
+            const int q = r % Q, w = r / Q;                          // w = lz for a y face, ly for a z face
+            uint32_t off;
+            if (kind < 2) {
+                const uint32_t y = side ? (y0 + T == L ? 0u : (uint32_t)(y0 + T)) : (y0 == 0 ? (uint32_t)(L - 1) : (uint32_t)(y0 - 1));
+                off = (uint32_t)(DIM == 3 ? z0 + w : 0) * (uint32_t)plane + y * (uint32_t)L + (uint32_t)x0 + 4u * q;
+                dst = (uint32_t)G::at(4 * q, side ? T : -1, w);
+            } else {
+                const uint32_t z = side ? (z0 + T == L ? 0u : (uint32_t)(z0 + T)) : (z0 == 0 ? (uint32_t)(L - 1) : (uint32_t)(z0 - 1));
+                off = z * (uint32_t)plane + (uint32_t)(y0 + w) * (uint32_t)L + (uint32_t)x0 + 4u * q;
+                dst = (uint32_t)G::at(4 * q, w, side ? T : -1);
             }
+            src = A.s + off;
+            cstride = N;
         }
-        // left halo = right face (side 1) of the left neighbour, right halo = left face (side 0) of the right one
-        for (int idx = tid; idx < 2 * FACE / 4; idx += G::THREADS) {
-            const int side = idx / (FACE / 4), r = idx % (FACE / 4);
-            const float* src = A.xface + (((uint64_t)c * A.ntiles + (side ? t_right : t_left)) * 2 + (side ? 0 : 1)) * FACE + 4 * r;
-            cp_async16(XF + (c * 2 + side) * FACE + 4 * r, src);
-        }
+        const uint32_t dstride = (kind >> 1) == 1 ? 2u * FACE : (uint32_t)G::COMP;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) cp_async16_addr(sm_addr + 4u * (dst + c * dstride), src + c * cstride);
     }
     cp_async_commit();
     cp_async_wait_all();
     __syncthreads();
-    for (int idx = tid; idx < 6 * FACE; idx += G::THREADS) {          // staged x faces -> halo columns
-        const int f = idx % FACE, side = (idx / FACE) & 1, c = idx / (2 * FACE);
-        sm[c * G::COMP + G::at(side ? T : -1, f % T, f / T)] = XF[idx];
+    static_assert(2 * FACE <= G::THREADS, "one x-halo site per thread");
+    uint32_t halo_s = 0, edge_s = 0;                                  // this thread's x-halo site and own edge site
+    if (tid < 2 * FACE) {                                             // staged x faces -> halo columns
+        const int f = tid % FACE, side = tid / FACE;
+        halo_s = (uint32_t)G::at(side ? T : -1, f % T, f / T);
+        edge_s = (uint32_t)G::at(side ? T - 1 : 0, f % T, f / T);
+#pragma unroll
+        for (int c = 0; c < 3; ++c) sm[c * G::COMP + halo_s] = XF[c * 2 * FACE + tid];
     }
     __syncthreads();
 
@@ -342,18 +373,17 @@ __global__ void __launch_bounds__(HG<DIM, T>::THREADS, HG<DIM, T>::MIN_CTAS) k_h
     }
 
     // a7: interior back to HBM, and the tile's own x faces into the side array
-    for (int c = 0; c < 3; ++c) {
-        float* g = A.s + (uint64_t)c * N + (DIM == 3 ? (uint64_t)z0 * plane : 0) + (uint64_t)y0 * row + x0;
-        const float* d = sm + c * G::COMP;
-        for (int idx = tid; idx < G::SITES / 4; idx += G::THREADS) {
-            const int q = idx % Q, yy = (idx / Q) % T, zz = idx / (Q * T);
-            *reinterpret_cast<float4*>(g + (DIM == 3 ? (uint64_t)zz * plane : 0) + (uint64_t)yy * row + 4 * q) =
-                *reinterpret_cast<const float4*>(d + G::at(4 * q, yy, zz));
-        }
+    if (int_live) {
+#pragma unroll
+        for (int n = 0; n < INT_ROUNDS; ++n)
+#pragma unroll
+            for (int c = 0; c < 3; ++c)
+                *reinterpret_cast<float4*>(A.s + (uint64_t)c * N + int_g[n]) = *reinterpret_cast<const float4*>(sm + c * G::COMP + int_s[n]);
     }
-    for (int idx = tid; idx < 6 * FACE; idx += G::THREADS) {
-        const int f = idx % FACE, side = (idx / FACE) & 1, c = idx / (2 * FACE);
-        A.xface[(((uint64_t)c * A.ntiles + t_self) * 2 + side) * FACE + f] = sm[c * G::COMP + G::at(side ? T - 1 : 0, f % T, f / T)];
+    if (tid < 2 * FACE) {
+        float* dst = A.xface + (uint64_t)t_self * 2 * FACE + tid;
+#pragma unroll
+        for (int c = 0; c < 3; ++c) dst[(uint64_t)c * A.ntiles * 2 * FACE] = sm[c * G::COMP + edge_s];
     }
 }
 
