@@ -25,15 +25,18 @@ extern "C" {
 
 typedef struct heis_ctx* heis_handle; /* opaque, owned by the library */
 
-/* Hot start (H3): s_i = D(w0, w1) with (w0, w1, ., .) = Philox(ctr = {i, 6, 0, 0}, key = seed), D the direction
- * map H2.  dim in {2, 3}; L even, L % 4 == 0, N = L^dim <= 2^32.  Spins live in HBM as three float planes
- * s[c][i], c = x, y, z, i = x + L*(y + L*z).  Returns NULL on failure. */
+/* Hot start (H3): s_i = D(wa, wb) with (wa, wb) = words (2h, 2h+1), h = i & 1, of Philox(ctr = {i >> 1, 6, 0, 0},
+ * key = seed), D the direction map H2.  dim in {2, 3}; L even, N = L^dim <= 2^32.  Spins live in HBM as three float
+ * planes s[c][i], c = x, y, z, i = x + L*(y + L*z).  The shared-memory tile kernels serve L % 4 == 0 with tile in
+ * {16, 32, 64} (2D) / {4, 8, 16} (3D) and L/tile even; every other valid combination runs on the generic kernels.
+ * Returns NULL on failure. */
 heis_handle heis_create(int dim, int L, uint64_t seed);
 void heis_destroy(heis_handle h);
 
 /* n_sweeps outer passes of the double checkerboard (H7): per pass the tiles of coarse colour 0, then
  * colour 1; per tile k_inner inner sweeps, each = fine colour 0 then fine colour 1; update H5
- * with the acceptance probability H6; beta is rounded to float once.  tile: edge T, even, T | L, L/T even or
+ * with the acceptance probability H6 and the random numbers H4 (one Philox call per 2x2 block of the xy plane and
+ * half-sweep); beta is rounded to float once.  tile: edge T, even, T | L, L/T even or
  * T == L (0 means L: plain checkerboard).  One pass attempts k_inner*N updates; the handle's counter of inner
  * sweeps advances by n_sweeps*k_inner.  Asynchronous on the hooked stream. */
 int heis_sweep(heis_handle h, double beta, int n_sweeps, int tile, int k_inner);
