@@ -191,15 +191,21 @@ def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng=
     return {"ms": ms, "flips_per_ns": flips / (ms * 1e6), "launches": int(launches), "path": path, "clocks": clocks}
 
 
-def time_e2e(P, torch, L, layout, tile, k, steps, rng="planes"):
+def time_e2e(P, torch, L, layout, tile, k, steps, rng="planes", packed=False):
     """Same metric through the public API with HOST buffers: every step uploads the spins from
-    pinned host memory (ising_set_spins), runs one pass, and reads them back (ising_copy_spins)."""
+    pinned host memory (ising_set_spins), runs one pass, and reads them back (ising_copy_spins).
+    packed: the one-bit-per-site host format (ising_set_spins_bits / ising_copy_spins_bits)."""
     g = P.Ising(2, L, seed=3, rng=rng)
     g.set_jit(JIT)
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
-    host = torch.empty(L * L, dtype=torch.int8).pin_memory()
-    g.copy_spins(host)
+    if packed:
+        host = torch.empty(L * L // 32, dtype=torch.int32).pin_memory()
+        g.copy_spins_bits(host)
+        g.set_spins, g.copy_spins = g.set_spins_bits, g.copy_spins_bits
+    else:
+        host = torch.empty(L * L, dtype=torch.int8).pin_memory()
+        g.copy_spins(host)
     g.sweep(W.BETA_C_2D, 1, tile, k)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -212,8 +218,10 @@ def time_e2e(P, torch, L, layout, tile, k, steps, rng="planes"):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
     g.destroy()
-    return {"value": steps * k * L * L / (ms * 1e6), "unit": UNIT, "h2d_bytes_per_step": L * L,
-            "d2h_bytes_per_step": L * L, "steps": steps}
+    nbytes = host.numel() * host.element_size()
+    return {"value": steps * k * L * L / (ms * 1e6), "unit": UNIT, "h2d_bytes_per_step": nbytes,
+            "d2h_bytes_per_step": nbytes, "steps": steps,
+            "host_format": "one bit per site (ising_set_spins_bits / ising_copy_spins_bits)" if packed else "int8 +-1 (ising_set_spins / ising_copy_spins)"}
 
 
 def run_config(P, torch, a) -> None:
@@ -484,6 +492,7 @@ def main() -> None:
                                                 "hbm_GBs": round(r["flips_per_ns"] * algorithmic_bytes_per_flip(T, k, lay), 1)}
         line["variants"] = table
         line["e2e"] = time_e2e(P, torch, L, a.layout, a.tile, a.k, 3, a.rng)
+        line["e2e_bits"] = time_e2e(P, torch, L, a.layout, a.tile, a.k, 3, a.rng, packed=True)
         ncores = 1
         v, dt = oracle_flips_per_ns(L, a.tile, a.k, 2, a.rng)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": ncores, "kind": "oracle",

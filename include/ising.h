@@ -112,6 +112,13 @@ int ising_copy_spins(ising_handle h, int8_t* dst);
  * any other value ⇒ ISING_EINVAL and the state is unchanged.  Does not touch t. */
 int ising_set_spins(ising_handle h, const int8_t* src);
 
+/* ising_copy_spins_bits / ising_set_spins_bits — the same state as one bit per site (eight times fewer bytes over
+ * PCIe; the spin is all the model has): word (r·N + i) >> 5, bit i & 31, set ⇔ s_i = +1; R·N/32 uint32
+ * words [host|device].  Needs N % 32 == 0 (else ISING_EUNSUPPORTED).  Every bit pattern is a valid state.
+ * Synchronise; do not touch t. */
+int ising_copy_spins_bits(ising_handle h, uint32_t* dst);
+int ising_set_spins_bits(ising_handle h, const uint32_t* src);
+
 /* ising_set_layout — ISING_LAYOUT_I8 or ISING_LAYOUT_BITS: how spins are held in HBM between
  * sweeps.  The trajectory does not depend on it (S8c: both layouts give the same bits). */
 int ising_set_layout(ising_handle h, int layout);

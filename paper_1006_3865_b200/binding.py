@@ -23,7 +23,7 @@ RNG_MODES = {"words": ISING_RNG_WORDS, "planes": ISING_RNG_PLANES}
 
 SYMBOLS = [
     "ising_create", "ising_create_batch", "ising_create_multi", "ising_destroy", "ising_sweep", "ising_sweep_series",
-    "ising_observables", "ising_overlap", "ising_copy_spins", "ising_set_spins", "ising_set_layout", "ising_set_rng", "ising_set_jit", "ising_last_sweep_specialized",
+    "ising_observables", "ising_overlap", "ising_copy_spins", "ising_set_spins", "ising_copy_spins_bits", "ising_set_spins_bits", "ising_set_layout", "ising_set_rng", "ising_set_jit", "ising_last_sweep_specialized",
     "ising_get_counter", "ising_set_counter", "ising_thresholds", "ising_set_device_hooks",
     "ising_synchronize", "ising_kernel_launches", "ising_sweep_path", "ising_force_path",
     "ising_last_error",
@@ -69,6 +69,8 @@ def lib() -> C.CDLL:
     L.ising_overlap.argtypes = [vp, C.c_int, C.c_int, i64p]
     L.ising_copy_spins.argtypes = [vp, i8p]
     L.ising_set_spins.argtypes = [vp, i8p]
+    L.ising_copy_spins_bits.argtypes = [vp, vp]
+    L.ising_set_spins_bits.argtypes = [vp, vp]
     L.ising_set_layout.argtypes = [vp, C.c_int]
     L.ising_set_rng.argtypes = [vp, C.c_int]
     L.ising_set_jit.argtypes = [vp, C.c_int]
@@ -213,6 +215,19 @@ class Ising:
             src = np.ascontiguousarray(src, dtype=np.int8).reshape(-1)
             assert src.size == self.R * self.N
         _check(lib().ising_set_spins(self._h, _ptr(src)))
+
+    def copy_spins_bits(self, dst=None):
+        """One bit per site (set = +1): R*N/32 uint32 words; dst numpy or torch (host or device)."""
+        if dst is None:
+            dst = np.zeros(self.R * self.N // 32, dtype=np.uint32)
+        _check(lib().ising_copy_spins_bits(self._h, _ptr(dst)))
+        return dst
+
+    def set_spins_bits(self, src) -> None:
+        if isinstance(src, np.ndarray):
+            src = np.ascontiguousarray(src, dtype=np.uint32).reshape(-1)
+            assert src.size == self.R * self.N // 32
+        _check(lib().ising_set_spins_bits(self._h, _ptr(src)))
 
     def set_rng(self, mode) -> None:
         _check(lib().ising_set_rng(self._h, RNG_MODES[mode] if isinstance(mode, str) else int(mode)))

@@ -455,19 +455,55 @@ int ising_set_spins(ising_handle h, const int8_t* src) {
     if (!h || !src) { set_error("ising_set_spins: NULL argument"); return ISING_EINVAL; }
     cudaStream_t st = hooks().stream;
     const size_t bytes = (size_t)h->R * h->N;
-    int8_t* stage = (int8_t*)dev_alloc(bytes);
-    if (!stage) return ISING_ENOMEM;
+    // While the state lives in tile records, d_canon is scratch: land there, check, and only then switch over.
+    // Otherwise d_canon is the state and must survive a rejected input: land in a staging buffer.
+    const bool scratch = h->store != Store::Canon;
+    int8_t* land = scratch ? h->d_canon : (int8_t*)dev_alloc(bytes);
+    if (!land) return ISING_ENOMEM;
     const bool dev = is_device_ptr(src);
-    cudaError_t e = cudaMemcpyAsync(stage, src, bytes, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st);
+    cudaError_t e = cudaMemcpyAsync(land, src, bytes, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st);
     int bad = 0;
-    int rc = (e == cudaSuccess) ? launch_validate_pm1(stage, bytes, h->d_flag, &bad) : ISING_ECUDA;
+    int rc = (e == cudaSuccess) ? launch_validate_pm1(land, bytes, h->d_flag, &bad) : ISING_ECUDA;
     if (e != cudaSuccess) set_error("ising_set_spins: copy failed: %s", cudaGetErrorString(e));
     if (!rc && bad) { set_error("ising_set_spins: spins must be +1 or -1"); rc = ISING_EINVAL; }
-    if (!rc) {
-        e = cudaMemcpyAsync(h->d_canon, stage, bytes, cudaMemcpyDeviceToDevice, st);
+    if (!rc && !scratch) {
+        e = cudaMemcpyAsync(h->d_canon, land, bytes, cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) { set_error("ising_set_spins: %s", cudaGetErrorString(e)); rc = ISING_ECUDA; }
-        else { h->store = Store::Canon; h->store_tile = 0; }
     }
+    if (!rc) { h->store = Store::Canon; h->store_tile = 0; }
+    cudaStreamSynchronize(st);
+    if (!scratch) dev_free(land);
+    return rc;
+}
+
+int ising_copy_spins_bits(ising_handle h, uint32_t* dst) {
+    if (!h || !dst) { set_error("ising_copy_spins_bits: NULL argument"); return ISING_EINVAL; }
+    if (h->N % 32) { set_error("ising_copy_spins_bits: N = %llu is not a multiple of 32", (unsigned long long)h->N); return ISING_EUNSUPPORTED; }
+    int rc = 0;
+    const int8_t* s = canon_view(h, &rc);
+    if (rc) return rc;
+    const uint64_t nwords = (uint64_t)h->R * h->N / 32;
+    uint32_t* stage = (uint32_t*)dev_alloc(nwords * 4);
+    if (!stage) return ISING_ENOMEM;
+    rc = launch_pack_bits(s, stage, nwords);
+    if (!rc) rc = copy_out(dst, stage, nwords * 4, nullptr);
+    cudaStreamSynchronize(hooks().stream);
+    dev_free(stage);
+    return rc;
+}
+
+int ising_set_spins_bits(ising_handle h, const uint32_t* src) {
+    if (!h || !src) { set_error("ising_set_spins_bits: NULL argument"); return ISING_EINVAL; }
+    if (h->N % 32) { set_error("ising_set_spins_bits: N = %llu is not a multiple of 32", (unsigned long long)h->N); return ISING_EUNSUPPORTED; }
+    cudaStream_t st = hooks().stream;
+    const uint64_t nwords = (uint64_t)h->R * h->N / 32;
+    uint32_t* stage = (uint32_t*)dev_alloc(nwords * 4);
+    if (!stage) return ISING_ENOMEM;
+    int rc = 0;
+    cudaError_t e = cudaMemcpyAsync(stage, src, nwords * 4, is_device_ptr(src) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { set_error("ising_set_spins_bits: copy failed: %s", cudaGetErrorString(e)); rc = ISING_ECUDA; }
+    if (!rc) rc = launch_unpack_bits(stage, h->d_canon, nwords);      // every bit pattern is a valid state
+    if (!rc) { h->store = Store::Canon; h->store_tile = 0; }
     cudaStreamSynchronize(st);
     dev_free(stage);
     return rc;

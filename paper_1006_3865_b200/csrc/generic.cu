@@ -219,10 +219,51 @@ __global__ void k_overlap(const int8_t* __restrict__ sa, const int8_t* __restric
     }
 }
 
+// every byte must be +1 (0x01) or -1 (0xff); 16 bytes per thread and step, the tail byte-wise
 __global__ void k_validate_pm1(const int8_t* __restrict__ d, uint64_t n, int* flag) {
-    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n;
-         i += (uint64_t)gridDim.x * blockDim.x)
-        if (d[i] != 1 && d[i] != -1) *flag = 1;
+    const uint64_t n16 = n / 16;
+    const uint4* v = reinterpret_cast<const uint4*>(d);
+    bool bad = false;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (uint64_t)gridDim.x * blockDim.x) {
+        const uint4 w = v[i];
+        const uint32_t ok = (__vcmpeq4(w.x, 0x01010101u) | __vcmpeq4(w.x, 0xffffffffu)) & (__vcmpeq4(w.y, 0x01010101u) | __vcmpeq4(w.y, 0xffffffffu)) &
+                            (__vcmpeq4(w.z, 0x01010101u) | __vcmpeq4(w.z, 0xffffffffu)) & (__vcmpeq4(w.w, 0x01010101u) | __vcmpeq4(w.w, 0xffffffffu));
+        bad |= ok != 0xffffffffu;
+    }
+    if (blockIdx.x == 0)
+        for (uint64_t i = 16 * n16 + threadIdx.x; i < n; i += blockDim.x) bad |= d[i] != 1 && d[i] != -1;
+    if (bad) *flag = 1;
+}
+
+// canonical +-1 bytes <-> one bit per site (bit i & 31 of word i >> 5 set = spin up); one thread per word
+__global__ void k_pack_bits(const int8_t* __restrict__ canon, uint32_t* __restrict__ words, uint64_t nwords) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nwords) return;
+    const uint4* v = reinterpret_cast<const uint4*>(canon) + 2 * i;
+    const uint4 a = v[0], b = v[1];
+    const uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+    uint32_t out = 0;
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const uint32_t up = ~(w[q] >> 1) & 0x01010101u;          // 0x01 -> 1, 0xff -> 0, per byte
+        out |= ((up * 0x01020408u) >> 24) << (4 * q);             // the four byte flags -> four adjacent bits
+    }
+    words[i] = out;
+}
+
+__global__ void k_unpack_bits(const uint32_t* __restrict__ words, int8_t* __restrict__ canon, uint64_t nwords) {
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= nwords) return;
+    const uint32_t in = words[i];
+    uint32_t w[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) {
+        const uint32_t up = (((in >> (4 * q)) & 0xfu) * 0x00204081u) & 0x01010101u;   // four bits -> four byte flags
+        w[q] = ((up ^ 0x01010101u) * 255u) | up;                  // 1 -> 0x01, 0 -> 0xff
+    }
+    uint4* v = reinterpret_cast<uint4*>(canon) + 2 * i;
+    v[0] = make_uint4(w[0], w[1], w[2], w[3]);
+    v[1] = make_uint4(w[4], w[5], w[6], w[7]);
 }
 
 int reduce_grid(uint64_t n) {
@@ -273,6 +314,20 @@ int launch_validate_pm1(const int8_t* d, uint64_t n, int* d_flag, int* host_bad)
     ISING_CUDA_OK(cudaGetLastError());
     ISING_CUDA_OK(cudaMemcpyAsync(host_bad, d_flag, sizeof(int), cudaMemcpyDeviceToHost, st));
     ISING_CUDA_OK(cudaStreamSynchronize(st));
+    return 0;
+}
+
+int launch_pack_bits(const int8_t* d_canon, uint32_t* d_words, uint64_t nwords) {
+    k_pack_bits<<<(unsigned)((nwords + kThreads - 1) / kThreads), kThreads, 0, hooks().stream>>>(d_canon, d_words, nwords);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+int launch_unpack_bits(const uint32_t* d_words, int8_t* d_canon, uint64_t nwords) {
+    k_unpack_bits<<<(unsigned)((nwords + kThreads - 1) / kThreads), kThreads, 0, hooks().stream>>>(d_words, d_canon, nwords);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
     return 0;
 }
 

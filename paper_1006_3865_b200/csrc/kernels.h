@@ -12,6 +12,8 @@ int launch_observables_canon(ising_ctx* h, const int8_t* d_spins, long long* d_E
                              long long* d_M);                         // a10 (R values each)
 int launch_overlap_canon(ising_ctx* h, const int8_t* d_spins, int a, int b, long long* d_Q);
 int launch_validate_pm1(const int8_t* d, uint64_t n, int* d_flag, int* host_bad);
+int launch_pack_bits(const int8_t* d_canon, uint32_t* d_words, uint64_t nwords);     // +-1 bytes -> one bit per site
+int launch_unpack_bits(const uint32_t* d_words, int8_t* d_canon, uint64_t nwords);
 
 // ---- tile_i8.cu: 2D tile records of 0/1 bytes, warp-per-tile staged kernel -----------
 bool tile_i8_supported(const ising_ctx* h, int T);

@@ -138,6 +138,130 @@ __global__ void k_convert_planes(int8_t* __restrict__ canon, uint8_t* __restrict
     if (lx == T - 1) atomicOr(e + 6 + rp, 1u << Y);                       //      R0, R1
 }
 
+// ---- fast converters for the int8 records (the layout behind ising_set_spins / ising_copy_spins on the headline
+// path).  Lane = block row Y of a tile (T = 64: a warp per tile; T = 32: two tiles per warp): it owns the rows 2Y and
+// 2Y+1, i.e. one 16-byte piece per (rp, cc, gx).  Canonical side: 32-byte runs of a row (whole sectors); record side:
+// the 32 (16) lanes of a tile touch consecutive pieces.  A 32-byte run of row ly holds the 16 sites of both colours
+// of one RNG block row: site k of colour cc at byte 2k + a, a = (cc + ly) & 1, and piece_byte() wants words
+// {k even of 0..7, k odd of 0..7, k even of 8..15, k odd of 8..15}: two byte permutations per word.
+template <int T>
+__global__ void __launch_bounds__(256) k_canon_to_planes_i8(const int8_t* __restrict__ canon, uint8_t* __restrict__ tiles,
+                                                            int L, int B, uint32_t ntiles) {
+    using G = PG<T>;
+    const int lane = threadIdx.x & 31;
+    const uint32_t warp = (uint32_t)((blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+    const uint32_t tile = warp * G::TPW + (uint32_t)(lane / G::LPT);
+    const int Y = lane % G::LPT;
+    const bool live = tile < ntiles;
+    const uint32_t tc = live ? tile : 0;
+    const uint32_t per_rep = (uint32_t)B * B;
+    const uint32_t r = tc / per_rep, t2 = tc - r * per_rep;
+    const int ty = (int)(t2 / B), tx = (int)(t2 - (uint32_t)ty * B);
+    uint8_t* rec = tiles + (size_t)tc * G::REC_I8;
+    uint32_t words[2 * G::NW];                         // this lane's bit words [cc * NW + gx]: TOP for Y = 0, BOT for Y = LPT-1
+#pragma unroll
+    for (int i = 0; i < 2 * G::NW; ++i) words[i] = 0;
+    uint32_t col[4];                                    // L0, L1, R0, R1 ballots
+#pragma unroll
+    for (int rp = 1; rp >= 0; --rp) {                   // row 2Y+1 first: pack16 shifts the earlier half up
+        const int8_t* rowp = canon + (size_t)r * L * L + (size_t)(ty * T + 2 * Y + rp) * L + (size_t)tx * T;
+        bool left = false, right = false;
+#pragma unroll
+        for (int gx = 0; gx < G::NW; ++gx) {
+            uint4 a = make_uint4(0, 0, 0, 0), b = a;
+            if (live) {
+                a = __ldg(reinterpret_cast<const uint4*>(rowp + 32 * gx));
+                b = __ldg(reinterpret_cast<const uint4*>(rowp + 32 * gx + 16));
+            }
+            uint32_t w[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+#pragma unroll
+            for (int i = 0; i < 8; ++i) w[i] = ~(w[i] >> 1) & 0x01010101u;         // +1 (0x01) -> 1, -1 (0xff) -> 0
+            if (gx == 0) left = (w[0] & 1u) != 0;
+            if (gx == G::NW - 1) right = (w[7] >> 24) != 0;
+            uint4 pe, po;                                // even bytes (a = 0) and odd bytes (a = 1) of the run
+            {
+                const uint32_t e01 = __byte_perm(w[0], w[1], 0x6240), e23 = __byte_perm(w[2], w[3], 0x6240);
+                const uint32_t e45 = __byte_perm(w[4], w[5], 0x6240), e67 = __byte_perm(w[6], w[7], 0x6240);
+                pe = make_uint4(__byte_perm(e01, e23, 0x5410), __byte_perm(e01, e23, 0x7632), __byte_perm(e45, e67, 0x5410), __byte_perm(e45, e67, 0x7632));
+                const uint32_t o01 = __byte_perm(w[0], w[1], 0x7351), o23 = __byte_perm(w[2], w[3], 0x7351);
+                const uint32_t o45 = __byte_perm(w[4], w[5], 0x7351), o67 = __byte_perm(w[6], w[7], 0x7351);
+                po = make_uint4(__byte_perm(o01, o23, 0x5410), __byte_perm(o01, o23, 0x7632), __byte_perm(o45, o67, 0x5410), __byte_perm(o45, o67, 0x7632));
+            }
+            // a = (cc + ly) & 1 and ly = 2Y + rp: the even bytes are colour rp, the odd bytes colour 1 - rp
+#pragma unroll
+            for (int odd = 0; odd < 2; ++odd) {
+                const int cc = odd ? 1 - rp : rp;
+                const uint4 piece = odd ? po : pe;
+                if (live) *reinterpret_cast<uint4*>(rec + ((((rp * 2 + cc) * G::NW + gx) * G::LPT) + Y) * 16) = piece;
+                words[cc * G::NW + gx] = pack16(words[cc * G::NW + gx], piece);
+            }
+        }
+        col[0 + rp] = __ballot_sync(0xffffffffu, left);
+        col[2 + rp] = __ballot_sync(0xffffffffu, right);
+    }
+    if (!live) return;
+    const int sh = (lane / G::LPT) * G::LPT;                                       // T = 32: this tile's half of the ballot
+    const uint32_t mask = G::LPT == 32 ? 0xffffffffu : ((1u << G::LPT) - 1u);
+    uint32_t* e = reinterpret_cast<uint32_t*>(rec + G::BODY);
+    if (Y == 0) {
+        uint32_t top[4] = {0, 0, 0, 0};
+#pragma unroll
+        for (int i = 0; i < 2 * G::NW; ++i) top[i] = words[i];
+        *reinterpret_cast<uint4*>(e + 0) = make_uint4(top[0], top[1], top[2], top[3]);
+        *reinterpret_cast<uint4*>(e + 4) = make_uint4((col[0] >> sh) & mask, (col[1] >> sh) & mask, (col[2] >> sh) & mask, (col[3] >> sh) & mask);
+        *reinterpret_cast<uint4*>(e + 12) = make_uint4(0, 0, 0, 0);
+    }
+    if (Y == G::LPT - 1) {
+        uint32_t bot[4] = {0, 0, 0, 0};
+#pragma unroll
+        for (int i = 0; i < 2 * G::NW; ++i) bot[i] = words[i];
+        *reinterpret_cast<uint4*>(e + 8) = make_uint4(bot[0], bot[1], bot[2], bot[3]);
+    }
+}
+
+template <int T>
+__global__ void __launch_bounds__(256) k_planes_i8_to_canon(int8_t* __restrict__ canon, const uint8_t* __restrict__ tiles,
+                                                            int L, int B, uint32_t ntiles) {
+    using G = PG<T>;
+    const int lane = threadIdx.x & 31;
+    const uint32_t warp = (uint32_t)((blockIdx.x * blockDim.x + threadIdx.x) >> 5);
+    const uint32_t tile = warp * G::TPW + (uint32_t)(lane / G::LPT);
+    const int Y = lane % G::LPT;
+    if (tile >= ntiles) return;
+    const uint32_t per_rep = (uint32_t)B * B;
+    const uint32_t r = tile / per_rep, t2 = tile - r * per_rep;
+    const int ty = (int)(t2 / B), tx = (int)(t2 - (uint32_t)ty * B);
+    const uint8_t* rec = tiles + (size_t)tile * G::REC_I8;
+#pragma unroll
+    for (int rp = 0; rp < 2; ++rp) {
+        int8_t* rowp = canon + (size_t)r * L * L + (size_t)(ty * T + 2 * Y + rp) * L + (size_t)tx * T;
+#pragma unroll
+        for (int gx = 0; gx < G::NW; ++gx) {
+            // even bytes of the run = colour rp, odd bytes = colour 1 - rp
+            const uint4 pe = __ldg(reinterpret_cast<const uint4*>(rec + ((((rp * 2 + rp) * G::NW + gx) * G::LPT) + Y) * 16));
+            const uint4 po = __ldg(reinterpret_cast<const uint4*>(rec + ((((rp * 2 + 1 - rp) * G::NW + gx) * G::LPT) + Y) * 16));
+            uint32_t w[8];
+            // word m of the run = sites k = 2m (piece word 0/2, byte m & 3) and 2m+1 (piece word 1/3) of both colours:
+            // bytes {pe[k=2m], po[k=2m], pe[k=2m+1], po[k=2m+1]}
+#pragma unroll
+            for (int half = 0; half < 2; ++half) {
+                const uint32_t ee = half ? pe.z : pe.x, eo = half ? pe.w : pe.y;      // colour "even byte": k even, k odd
+                const uint32_t oe = half ? po.z : po.x, oo = half ? po.w : po.y;
+                const uint32_t lo_e = __byte_perm(ee, oe, 0x5140), hi_e = __byte_perm(ee, oe, 0x7362);   // (ee.b0, oe.b0, ee.b1, oe.b1), (.b2, .b3)
+                const uint32_t lo_o = __byte_perm(eo, oo, 0x5140), hi_o = __byte_perm(eo, oo, 0x7362);
+                w[4 * half + 0] = __byte_perm(lo_e, lo_o, 0x5410);        // k = 0 (both colours), k = 1 (both colours)
+                w[4 * half + 1] = __byte_perm(lo_e, lo_o, 0x7632);        // k = 2, 3
+                w[4 * half + 2] = __byte_perm(hi_e, hi_o, 0x5410);        // k = 4, 5
+                w[4 * half + 3] = __byte_perm(hi_e, hi_o, 0x7632);        // k = 6, 7
+            }
+#pragma unroll
+            for (int i = 0; i < 8; ++i) w[i] = ((w[i] ^ 0x01010101u) * 255u) | w[i];   // 1 -> 0x01, 0 -> 0xff
+            *reinterpret_cast<uint4*>(rowp + 32 * gx) = make_uint4(w[0], w[1], w[2], w[3]);
+            *reinterpret_cast<uint4*>(rowp + 32 * gx + 16) = make_uint4(w[4], w[5], w[6], w[7]);
+        }
+    }
+}
+
 // Couplings, canonical J[d][i] (bond i -> i + e_d) -> coupling records (zeroed first).  One thread per site:
 // it owns the four bonds seen from that site, in the order of the neighbour words of update_block.
 __global__ void k_convert_couplings(const int8_t* __restrict__ J, uint32_t* __restrict__ jrec, int L, int T) {
@@ -219,6 +343,16 @@ int launch_canon_to_planes(ising_ctx* h, int T, bool bits, const int8_t* d_canon
     const uint64_t total = h->N * (uint64_t)h->R;
     const unsigned blocks = (unsigned)((total + 255) / 256);
     cudaStream_t st = hooks().stream;
+    if (!bits) {                                  // fast path: a warp per tile, whole sectors on both sides
+        const uint32_t ntiles = (uint32_t)h->R * (uint32_t)(h->L / T) * (uint32_t)(h->L / T);
+        const uint32_t warps = (ntiles + (64 / T) - 1) / (64 / T);
+        const unsigned grid = (warps + 7) / 8;
+        if (T == 64) k_canon_to_planes_i8<64><<<grid, 256, 0, st>>>(d_canon, (uint8_t*)d_tiles, h->L, h->L / T, ntiles);
+        else k_canon_to_planes_i8<32><<<grid, 256, 0, st>>>(d_canon, (uint8_t*)d_tiles, h->L, h->L / T, ntiles);
+        count_launch();
+        ISING_CUDA_OK(cudaGetLastError());
+        return 0;
+    }
     ISING_CUDA_OK(cudaMemsetAsync(d_tiles, 0, tile_planes_bytes(h, T, bits), st));
     if (bits) {
         k_convert_planes<2><<<blocks, 256, 0, st>>>(const_cast<int8_t*>(d_canon), (uint8_t*)d_tiles, h->L, T, h->R);
@@ -234,6 +368,16 @@ int launch_planes_to_canon(ising_ctx* h, int T, bool bits, const void* d_tiles, 
     const uint64_t total = h->N * (uint64_t)h->R;
     const unsigned blocks = (unsigned)((total + 255) / 256);
     cudaStream_t st = hooks().stream;
+    if (!bits) {
+        const uint32_t ntiles = (uint32_t)h->R * (uint32_t)(h->L / T) * (uint32_t)(h->L / T);
+        const uint32_t warps = (ntiles + (64 / T) - 1) / (64 / T);
+        const unsigned grid = (warps + 7) / 8;
+        if (T == 64) k_planes_i8_to_canon<64><<<grid, 256, 0, st>>>(d_canon, (const uint8_t*)d_tiles, h->L, h->L / T, ntiles);
+        else k_planes_i8_to_canon<32><<<grid, 256, 0, st>>>(d_canon, (const uint8_t*)d_tiles, h->L, h->L / T, ntiles);
+        count_launch();
+        ISING_CUDA_OK(cudaGetLastError());
+        return 0;
+    }
     if (bits) k_convert_planes<3><<<blocks, 256, 0, st>>>(d_canon, (uint8_t*)const_cast<void*>(d_tiles), h->L, T, h->R);
     else k_convert_planes<1><<<blocks, 256, 0, st>>>(d_canon, (uint8_t*)const_cast<void*>(d_tiles), h->L, T, h->R);
     count_launch();

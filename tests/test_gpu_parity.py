@@ -343,3 +343,54 @@ def test_argument_errors(P):
         P.Ising(2, 16, coupling=np.zeros(2 * 256, dtype=np.int8), seed=1)
     g.sweep(0.4, 0, 32, 1)      # zero passes is a no-op
     assert g.counter == 0
+
+
+@pytest.mark.parametrize("dim,L,T,seeds,layout", [(2, 64, 32, [1], "int8"), (2, 128, 64, [2, 3], "int8"), (2, 128, 64, [4], "bits"),
+                                                   (3, 16, 8, [5], "int8"), (2, 8, 4, [6], "int8"), (2, 192, 32, [7], "int8")])
+def test_bit_packed_host_io(P, orc, dim, L, T, seeds, layout):
+    """ising_copy_spins_bits / ising_set_spins_bits: bit i & 31 of word i >> 5 set <=> s_i = +1, against numpy's packing of
+    the oracle's spins; a state set from bits continues like the oracle's."""
+    g, o = _both(P, orc, dim, L, seeds)
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.sweep(BC2, 2, T, 2); o.sweep(BC2, 2, T, 2)
+    want = np.packbits((np.asarray(o.spins()).reshape(-1) > 0).astype(np.uint8), bitorder="little").view(np.uint32)
+    got = g.copy_spins_bits()
+    assert np.array_equal(got, want)
+    # round trip through a fresh handle, then both continue
+    h = P.Ising(dim, L, seeds=seeds)
+    if layout == "bits":
+        h.set_layout(P.ISING_LAYOUT_BITS)
+    h.set_spins_bits(got); h.counter = g.counter
+    h.sweep(BC2, 2, T, 1); o.sweep(BC2, 2, T, 1)
+    _same_state(h, o)
+    import torch
+    d = torch.zeros(len(seeds) * L ** dim // 32, dtype=torch.int32, device="cuda")
+    h.copy_spins_bits(d)
+    want = np.packbits((np.asarray(o.spins()).reshape(-1) > 0).astype(np.uint8), bitorder="little").view(np.uint32)
+    assert np.array_equal(d.cpu().numpy().view(np.uint32), want)
+
+
+def test_bit_packed_io_needs_whole_words(P):
+    g = P.Ising(2, 6, seed=1)          # N = 36
+    with pytest.raises(P.IsingError):
+        g.copy_spins_bits(np.zeros(2, dtype=np.uint32))
+
+
+def test_set_spins_rejects_bad_values_and_keeps_the_state(P, orc):
+    """in both situations: state in the canonical array (fresh handle) and state in tile records (after a sweep)"""
+    for swept in (False, True):
+        g, o = _both(P, orc, 2, 64, [9])
+        if swept:
+            g.sweep(BC2, 1, 32, 1); o.sweep(BC2, 1, 32, 1)
+        bad = np.asarray(o.spins()).reshape(-1).copy()
+        bad[1234] = 0
+        with pytest.raises(P.IsingError):
+            g.set_spins(bad)
+        bad[1234] = 3
+        bad[-1] = 1
+        with pytest.raises(P.IsingError):
+            g.set_spins(bad)
+        _same_state(g, o)
+        g.sweep(BC2, 1, 32, 1); o.sweep(BC2, 1, 32, 1)
+        _same_state(g, o)
