@@ -198,11 +198,7 @@ int launch_amsc_pass(ising_ctx* h, const Accept& acc, int T, int k, uint64_t t_f
     A.rmask = h->R >= 32 ? 0xffffffffu : ((1u << h->R) - 1u);
     const unsigned grid = (unsigned)(A.B * A.B / 2);
     const size_t smem = sizeof(uint32_t) * (size_t)((T + 2) * (T == 32 ? T + 9 : T + 2) + T * (T + 1) + (T + 1) * (T == 32 ? T + 1 : T));
-    static bool attr_set = false;
-    if (!attr_set) {
-        ISING_CUDA_OK(cudaFuncSetAttribute(k_amsc<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
-        attr_set = true;
-    }
+    if (int rc = set_max_dynamic_smem<k_amsc<64>>(64 * 1024)) return rc;
     for (int C = 0; C < 2; ++C) {
         A.C = C;
         if (T == 64) k_amsc<64><<<grid, 64 * 64 / 8, smem, hooks().stream>>>(A);

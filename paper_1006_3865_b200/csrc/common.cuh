@@ -3,6 +3,7 @@
 #pragma once
 #include <cuda_runtime.h>
 
+#include <atomic>
 #include <cstdint>
 #include <cstdio>
 #include <string>
@@ -34,6 +35,20 @@ void dev_free(void* p);
             return ISING_ECUDA;                                                          \
         }                                                                                \
     } while (0)
+
+// Opt a kernel in to more than 48 KB of dynamic shared memory, once per (kernel, device): the attribute is per
+// device, and one process may drive several.
+template <auto Kernel>
+int set_max_dynamic_smem(int bytes) {
+    static std::atomic<uint64_t> done{0};        // one bit per device ordinal (mod 64)
+    int dev = 0;
+    ISING_CUDA_OK(cudaGetDevice(&dev));
+    const uint64_t bit = 1ull << (dev & 63);
+    if (done.load(std::memory_order_acquire) & bit) return 0;
+    ISING_CUDA_OK(cudaFuncSetAttribute(Kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes));
+    done.fetch_or(bit, std::memory_order_release);
+    return 0;
+}
 
 // How the spins are currently held in HBM.
 enum class Store : int {

@@ -439,11 +439,7 @@ bool tile_valid(const heis_ctx* h, int T) {
 template <int DIM, int T>
 int launch_tile(heis_ctx* h, TileArgs A) {
     using G = HG<DIM, T>;
-    static bool attr_set = false;
-    if (!attr_set) {
-        ISING_CUDA_OK(cudaFuncSetAttribute(k_heis_tile<DIM, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)G::SMEM));
-        attr_set = true;
-    }
+    if (int rc = set_max_dynamic_smem<k_heis_tile<DIM, T>>((int)G::SMEM)) return rc;
     A.ntiles = (uint32_t)A.B * A.B * (DIM == 3 ? A.B : 1);
     const size_t entries = (size_t)3 * A.ntiles * 2 * G::FACE;
     if (h->xface_T != T) {                       // (re)build the x-face copies from the spin planes

@@ -329,11 +329,7 @@ template <int T, int S>
 int launch_colour(ising_ctx* h, TileArgs& A, int warps, int ctas_per_sm) {
     using G = TG<T>;
     const size_t smem = (size_t)warps * S * G::NT * G::IMG;
-    static bool attr_set = false;
-    if (!attr_set) {
-        ISING_CUDA_OK(cudaFuncSetAttribute(k_tile_i8<T, S>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_set = true;
-    }
+    if (int rc = set_max_dynamic_smem<k_tile_i8<T, S>>(200 * 1024)) return rc;
     const uint32_t need = (A.njobs + warps - 1) / warps;
     uint32_t grid = 148u * (uint32_t)ctas_per_sm;
     if (grid > need) grid = need;
