@@ -259,8 +259,9 @@ class Ising:
     def sweep_path(self) -> str:
         return lib().ising_sweep_path(self._h).decode()
 
-    def force_path(self, generic_only: bool) -> None:
-        _check(lib().ising_force_path(self._h, int(bool(generic_only))))
+    def force_path(self, mode) -> None:
+        """0 / False: automatic; 1 / True: generic kernels only; 2: automatic but never the cluster-resident kernel."""
+        _check(lib().ising_force_path(self._h, int(mode)))
 
 
 class Heisenberg:

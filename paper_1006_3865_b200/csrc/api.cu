@@ -383,7 +383,14 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         const bool use_jit = (use_planes || use_3d) && (h->jit_mode == ISING_JIT_ON ||
                              (h->jit_mode == ISING_JIT_AUTO && (double)n * k * (double)h->N * h->R >= 134217728.0));
         h->last_jit = 0;
-        for (int pass = 0; pass < n && !rc; ++pass) {
+        // small lattices, several passes, nothing to measure in between: the whole call in one cluster launch
+        const bool use_resident = use_planes && !want_series && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->has_J && !h->no_resident &&
+                                  resident_planes_supported(h, T);
+        if (use_resident && !rc) {
+            h->last_path = bits ? "resident_planes_bits" : "resident_planes_i8";
+            rc = launch_resident_planes(h, acc, T, bits, n, k, h->t);
+        }
+        for (int pass = 0; pass < n && !rc && !use_resident; ++pass) {
             const uint64_t t0 = h->t + (uint64_t)pass * (uint64_t)k;
             rc = use_tile_i8 ? launch_tile_i8_pass(h, acc, T, k, t0)
                  : use_3d ? launch_tile3d_pass(h, acc, bits, k, t0, use_jit)
@@ -563,7 +570,8 @@ const char* ising_sweep_path(ising_handle h) { return h ? h->last_path : "none";
 
 int ising_force_path(ising_handle h, int generic_only) {
     if (!h) { set_error("ising_force_path: NULL handle"); return ISING_EINVAL; }
-    h->force_generic = generic_only ? 1 : 0;
+    h->force_generic = generic_only == 1 ? 1 : 0;
+    h->no_resident = generic_only == 2 ? 1 : 0;
     return 0;
 }
 

@@ -109,6 +109,7 @@ struct ising_ctx {
     int* d_flag = nullptr;          // validation flag
     const char* last_path = "none";
     int force_generic = 0;
+    int no_resident = 0;            // ising_force_path(h, 2): per-pass launches even where the cluster-resident kernel applies
     int jit_mode = 0;               // ISING_JIT_AUTO / OFF / ON (ising_set_jit)
     int last_jit = 0;               // 1 if the last tile launch used a run-time specialised kernel
 };

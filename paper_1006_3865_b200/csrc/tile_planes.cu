@@ -21,6 +21,8 @@
 //   bits  record = T*T/8 body + 64 edge bytes: word (cc, Y, gx) at ((cc*NW+gx)*LPT + Y)*4.
 //   edge  = bit-packed copies of the tile's own first / last block row and first / last column, written by
 //         the tile, so that every halo is one 16-byte run of ready-made words in the neighbour's record.
+#include <cooperative_groups.h>
+
 #include "kernels.h"
 #include "tile_planes_device.cuh"
 
@@ -476,6 +478,172 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
         if (rc) return rc;
         h->last_jit = used ? 1 : 0;
     }
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+// ---- whole lattice on chip ("a persistent whole-lattice-on-chip kernel for small L") ----------------
+// For L <= 1024 a pass of the tile kernel is two launches whose duration is launch latency + one L2 round trip, not
+// work.  Here one thread-block cluster per replica keeps every tile in registers for the whole call: warp w of the
+// cluster owns the jobs w, w + W, ... of each coarse colour (a job = 64 / T tiles, lane = block row, exactly as in
+// k_tile_planes), a tile publishes its boundary words (TOP / COL / BOT of PG) in the shared memory of its CTA after
+// every phase, its neighbours — of the other colour, so idle in that phase — read them through distributed shared
+// memory at the start of theirs, and the two coarse-colour phases of a pass are separated by cluster barriers
+// instead of kernel boundaries.  HBM is touched twice: records in at the start, records out at the end.
+constexpr int kResWarps = 4;       // warps per CTA: one per SM sub-partition
+constexpr int kResMaxJobs = 4;     // jobs per warp and colour (registers)
+constexpr int kResMaxCluster = 16;
+
+struct ResArgs {
+    PlaneArgs P;
+    int n;                         // outer passes
+    uint32_t jobs_per_colour;      // per replica
+};
+
+template <int T, bool BITS>
+__global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
+    using G = PG<T>;
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    const uint32_t CL = cluster.num_blocks(), rank = cluster.block_rank();
+    const PlaneArgs& A = R.P;
+    const int r = (int)(blockIdx.x / CL);                              // one cluster per replica
+    const int lane = threadIdx.x & 31, wic = threadIdx.x >> 5;
+    const uint32_t wg = rank * kResWarps + (uint32_t)wic, W = CL * kResWarps;
+    const int sub = lane / G::LPT, Y = lane % G::LPT;
+    const uint32_t B = (uint32_t)A.B, hb = B >> 1, JC = R.jobs_per_colour;
+    const uint2* lut = kByteLutGlobal.e;
+    __shared__ __align__(16) uint32_t edges[2][kResMaxJobs][kResWarps][G::TPW][12];
+
+    auto tile_of = [&](int C, uint32_t job, int& tx, int& ty) {
+        const uint32_t qq = job * G::TPW + (uint32_t)sub;
+        ty = (int)(qq / hb);
+        tx = (int)(2u * (qq - (uint32_t)ty * hb)) + ((ty + C) & 1);
+    };
+    auto edge_of = [&](uint32_t tx, uint32_t ty) -> const uint32_t* {   // published words of tile (tx, ty), anywhere in the cluster
+        const uint32_t C = (tx + ty) & 1u, qq = ty * hb + (tx >> 1);
+        const uint32_t job = qq / G::TPW, sb = qq % G::TPW, w = job % W, m = job / W;
+        return cluster.map_shared_rank(&edges[C][m][w % kResWarps][sb][0], w / kResWarps);
+    };
+    auto publish = [&](int C, int m, const TileRegs<T>& t) {
+        const uint32_t sh = (uint32_t)sub * G::LPT, msk = G::LPT == 32 ? 0xffffffffu : ((1u << G::LPT) - 1u);
+        const uint32_t L0 = (__ballot_sync(0xffffffffu, t.S[0][0] & 1u) >> sh) & msk;
+        const uint32_t L1 = (__ballot_sync(0xffffffffu, (t.S[1][0] >> 16) & 1u) >> sh) & msk;
+        const uint32_t R0 = (__ballot_sync(0xffffffffu, (t.S[1][G::NW - 1] >> 15) & 1u) >> sh) & msk;
+        const uint32_t R1 = (__ballot_sync(0xffffffffu, t.S[0][G::NW - 1] >> 31) >> sh) & msk;
+        uint32_t* e = &edges[C][m][wic][sub][0];
+        const uint4 w = G::NW == 2 ? make_uint4(t.S[0][0], t.S[0][1], t.S[1][0], t.S[1][1]) : make_uint4(t.S[0][0], t.S[1][0], 0u, 0u);
+        if (Y == 0) {
+            *reinterpret_cast<uint4*>(e + G::E_TOP / 4) = w;
+            *reinterpret_cast<uint4*>(e + G::E_COL / 4) = make_uint4(L0, L1, R0, R1);
+        }
+        if (Y == G::LPT - 1) *reinterpret_cast<uint4*>(e + G::E_BOT / 4) = w;
+    };
+    auto refresh = [&](int tx, int ty, TileRegs<T>& t) {               // halos from the neighbours' published words
+        const uint32_t utx = (uint32_t)tx, uty = (uint32_t)ty;
+        const uint32_t tyU = uty == 0 ? B - 1 : uty - 1, tyD = uty == B - 1 ? 0 : uty + 1;
+        const uint32_t txL = utx == 0 ? B - 1 : utx - 1, txR = utx == B - 1 ? 0 : utx + 1;
+        uint4 hv = make_uint4(0u, 0u, 0u, 0u);
+        if (Y == 0) hv = *reinterpret_cast<const uint4*>(edge_of(utx, tyU) + G::E_BOT / 4);
+        else if (Y == G::LPT - 1) hv = *reinterpret_cast<const uint4*>(edge_of(utx, tyD) + G::E_TOP / 4);
+        t.vrow[0][0] = hv.x;
+        if (G::NW == 2) { t.vrow[0][1] = hv.y; t.vrow[1][0] = hv.z; t.vrow[1][1] = hv.w; }
+        else t.vrow[1][0] = hv.y;
+        const uint2 cl = *reinterpret_cast<const uint2*>(edge_of(txL, uty) + G::E_COL / 4 + 2);   // {R0, R1}
+        const uint2 cr = *reinterpret_cast<const uint2*>(edge_of(txR, uty) + G::E_COL / 4);       // {L0, L1}
+        t.hL0 = (cl.x >> Y) & 1u; t.hL1 = (cl.y >> Y) & 1u;
+        t.hR0 = (cr.x >> Y) & 1u; t.hR1 = (cr.y >> Y) & 1u;
+    };
+
+    TileRegs<T> t[2][kResMaxJobs];
+    int txs[2][kResMaxJobs], tys[2][kResMaxJobs];
+#pragma unroll
+    for (int C = 0; C < 2; ++C)
+#pragma unroll
+        for (int m = 0; m < kResMaxJobs; ++m) {
+            const uint32_t job = wg + (uint32_t)m * W;
+            if (job < JC) {
+                tile_of(C, job, txs[C][m], tys[C][m]);
+                load_tile<T, BITS>(A, r, txs[C][m], tys[C][m], Y, sub * G::LPT, t[C][m]);
+                publish(C, m, t[C][m]);
+            }
+        }
+    cluster.sync();
+
+    const uint64_t seed = A.seeds[r];
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    const uint4 Jw[2][G::NW] = {};
+    for (int pass = 0; pass < R.n; ++pass) {
+#pragma unroll
+        for (int C = 0; C < 2; ++C) {
+#pragma unroll
+            for (int m = 0; m < kResMaxJobs; ++m) {
+                const uint32_t job = wg + (uint32_t)m * W;
+                if (job < JC) {
+                    const int tx = txs[C][m], ty = tys[C][m];
+                    refresh(tx, ty, t[C][m]);
+                    const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);
+                    const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(tx * G::NW);
+                    const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);
+                    for (int j = 0; j < A.k; ++j) {
+                        const uint64_t tt = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
+                        half_sweep<T, false, false, kNoSpec>(A, t[C][m], Jw, 0, Y, g0, p0, 2 * tt, k0, k1);
+                        half_sweep<T, false, false, kNoSpec>(A, t[C][m], Jw, 1, Y, g0, p0, 2 * tt + 1, k0, k1);
+                    }
+                    publish(C, m, t[C][m]);
+                }
+            }
+            cluster.sync();
+        }
+    }
+#pragma unroll
+    for (int C = 0; C < 2; ++C)
+#pragma unroll
+        for (int m = 0; m < kResMaxJobs; ++m) {
+            const uint32_t job = wg + (uint32_t)m * W;
+            if (job < JC) store_tile<T, BITS>(A, r, txs[C][m], tys[C][m], Y, sub, t[C][m], lut);
+        }
+}
+
+bool resident_planes_supported(const ising_ctx* h, int T) {
+    if (!tile_planes_supported(h, T) || h->has_J) return false;
+    const uint32_t B = (uint32_t)(h->L / T);
+    return B * B / 2u / (uint32_t)(64 / T) <= (uint32_t)(kResMaxCluster * kResWarps * kResMaxJobs);
+}
+
+template <int T, bool BITS>
+static int launch_resident(const ResArgs& R, int replicas) {
+    const uint32_t want = (R.jobs_per_colour + kResWarps - 1) / kResWarps;
+    unsigned cl = 1;
+    while (cl < want && cl < (unsigned)kResMaxCluster) cl *= 2;
+    if (cl > 8) ISING_CUDA_OK(cudaFuncSetAttribute(k_resident_planes<T, BITS>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(cl * (unsigned)replicas); cfg.blockDim = dim3(kResWarps * 32); cfg.dynamicSmemBytes = 0; cfg.stream = hooks().stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_resident_planes<T, BITS>, R));
+    count_launch();
+    return 0;
+}
+
+// n passes in one launch; the records must hold the state (ensure_store) and are current again afterwards.
+int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first) {
+    ResArgs R;
+    PlaneArgs& A = R.P;
+    A.tiles = (uint8_t*)h->d_tiles;
+    A.seeds = h->d_sweep_seeds;
+    A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0;
+    A.jrec = nullptr;
+    A.stream = 0;
+    A.njobs = 0; A.magic_rep = A.magic_hb = 0;
+    fill_accept(A, acc);
+    R.n = n;
+    R.jobs_per_colour = (uint32_t)A.B * (uint32_t)A.B / 2u / (uint32_t)(64 / T);
+    const int rc = T == 64 ? (bits ? launch_resident<64, true>(R, h->R) : launch_resident<64, false>(R, h->R))
+                           : (bits ? launch_resident<32, true>(R, h->R) : launch_resident<32, false>(R, h->R));
+    if (rc) return rc;
     ISING_CUDA_OK(cudaGetLastError());
     return 0;
 }

@@ -394,3 +394,41 @@ def test_set_spins_rejects_bad_values_and_keeps_the_state(P, orc):
         _same_state(g, o)
         g.sweep(BC2, 1, 32, 1); o.sweep(BC2, 1, 32, 1)
         _same_state(g, o)
+
+
+RESIDENT = [
+    # L, tile, k, n, beta, seeds: 1 .. 256 warp jobs per colour, cluster sizes 1 .. 16, 1 .. 4 jobs per warp
+    (64, 32, 1, 3, BC2, [3]),
+    (128, 64, 2, 4, BC2, [5]),
+    (128, 32, 3, 2, 0.6, [4]),
+    (192, 32, 2, 3, 0.3, [7]),
+    (384, 64, 1, 5, BC2, [8]),
+    (256, 32, 2, 4, BC2, [21, 22, 23]),    # one cluster per replica
+    (512, 32, 1, 6, 0.2, [32]),
+    (512, 64, 3, 2, 1.0, [31]),
+    (128, 32, 2, 2, 0.0, [2]),
+    (128, 64, 2, 2, 30.0, [2]),
+    (1024, 32, 1, 3, BC2, [9]),            # 256 jobs per colour: 4 per warp of a 16-CTA cluster
+    (1024, 64, 2, 2, BC2, [10]),
+]
+
+
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,tile,k,n,beta,seeds", RESIDENT)
+def test_cluster_resident_kernel_matches_oracle(P, orc, L, tile, k, n, beta, seeds, layout):
+    """Small lattices, n >= 2 passes, no series: one launch of one cluster per replica, tiles in registers, boundaries
+    through distributed shared memory.  Same trajectory as everything else."""
+    g, o = _both(P, orc, 2, L, seeds, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.sweep(beta, n, tile, k); o.sweep(beta, n, tile, k)
+    assert g.sweep_path() == f"resident_planes_{'i8' if layout == 'int8' else 'bits'}"
+    _same_state(g, o)
+    g.sweep(beta, 1, tile, k); o.sweep(beta, 1, tile, k)          # a single pass goes through the per-pass kernel and composes
+    assert g.sweep_path().startswith("tile_planes")
+    g.sweep(beta, 2, tile, k); o.sweep(beta, 2, tile, k)
+    _same_state(g, o)
+    g.force_path(2)
+    g.sweep(beta, 2, tile, k); o.sweep(beta, 2, tile, k)
+    assert g.sweep_path().startswith("tile_planes")
+    _same_state(g, o)
