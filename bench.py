@@ -164,7 +164,14 @@ JIT = "auto"     # --jit: run-time specialisation of the planes kernel (ising_se
 def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng="planes"):
     """Device-timed throughput of one (rng, layout, tile, k) variant; returns dict."""
     g = P.Ising(2, L, seed=3, rng=rng)
-    g.set_jit(JIT)
+    # the library's AUTO rule (specialise calls of >= 2^27 attempted flips), decided here for the timed call so that
+    # the warm-up call, which is shorter, already compiles the kernel the timed call will use
+    # (lattices small enough for the cluster-resident kernel, <= 64 warp jobs per colour, stay on AUTO: it serves them)
+    resident = (L // tile) ** 2 // 2 // (64 // tile) <= 64 and steps >= 2
+    if not resident:
+        g.set_jit("on" if JIT == "on" or (JIT == "auto" and steps * k * L * L >= 2 ** 27) else "off")
+    else:
+        g.set_jit(JIT)
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
     g.sweep(W.BETA_C_2D, warmup, tile, k)

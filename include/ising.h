@@ -175,7 +175,7 @@ uint64_t ising_kernel_launches(void);
 /* ising_sweep_path — name of the kernel family the last ising_sweep on h used
  * ("generic", "tile_i8", "tile_planes_i8", "tile_planes_bits", "tile3d_planes_i8", "tile3d_planes_bits",
  * "plain64_planes_i8", "plain64_planes_bits", "resident_planes_i8", "resident_planes_bits", "amsc"); static string,
- * never NULL.  "resident_planes_*": 2D, J = +1, at most 256 warp jobs per coarse colour (L <= 1024 at tile 32),
+ * never NULL.  "resident_planes_*": 2D, J = +1, at most 64 warp jobs per coarse colour (L <= 512 at tile 32 or 64),
  * n_sweeps >= 2: the whole call runs in one launch of one thread-block cluster per replica with the lattice held
  * in registers and the tile boundaries exchanged through distributed shared memory (same trajectory). */
 const char* ising_sweep_path(ising_handle h);

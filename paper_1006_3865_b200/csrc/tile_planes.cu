@@ -483,7 +483,7 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
 }
 
 // ---- whole lattice on chip ("a persistent whole-lattice-on-chip kernel for small L") ----------------
-// For L <= 1024 a pass of the tile kernel is two launches whose duration is launch latency + one L2 round trip, not
+// For L <= 512 a pass of the tile kernel is two launches whose duration is launch latency + one L2 round trip, not
 // work.  Here one thread-block cluster per replica keeps every tile in registers for the whole call: warp w of the
 // cluster owns the jobs w, w + W, ... of each coarse colour (a job = 64 / T tiles, lane = block row, exactly as in
 // k_tile_planes), a tile publishes its boundary words (TOP / COL / BOT of PG) in the shared memory of its CTA after
@@ -491,7 +491,7 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
 // memory at the start of theirs, and the two coarse-colour phases of a pass are separated by cluster barriers
 // instead of kernel boundaries.  HBM is touched twice: records in at the start, records out at the end.
 constexpr int kResWarps = 4;       // warps per CTA: one per SM sub-partition
-constexpr int kResMaxJobs = 4;     // jobs per warp and colour (registers)
+constexpr int kResMaxJobs = 1;     // jobs per warp and colour: with more, 16 SMs are slower than per-pass launches on 148 (measured at L = 1024)
 constexpr int kResMaxCluster = 16;
 
 struct ResArgs {
@@ -539,24 +539,29 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
         }
         if (Y == G::LPT - 1) *reinterpret_cast<uint4*>(e + G::E_BOT / 4) = w;
     };
-    auto refresh = [&](int tx, int ty, TileRegs<T>& t) {               // halos from the neighbours' published words
+    struct Nb { const uint32_t *up, *dn, *lf, *rt; };                  // the four neighbours' published words (fixed for the run)
+    auto neighbours = [&](int tx, int ty) {
         const uint32_t utx = (uint32_t)tx, uty = (uint32_t)ty;
         const uint32_t tyU = uty == 0 ? B - 1 : uty - 1, tyD = uty == B - 1 ? 0 : uty + 1;
         const uint32_t txL = utx == 0 ? B - 1 : utx - 1, txR = utx == B - 1 ? 0 : utx + 1;
+        return Nb{edge_of(utx, tyU), edge_of(utx, tyD), edge_of(txL, uty), edge_of(txR, uty)};
+    };
+    auto refresh = [&](const Nb& nb, TileRegs<T>& t) {                 // halos from the neighbours' published words
         uint4 hv = make_uint4(0u, 0u, 0u, 0u);
-        if (Y == 0) hv = *reinterpret_cast<const uint4*>(edge_of(utx, tyU) + G::E_BOT / 4);
-        else if (Y == G::LPT - 1) hv = *reinterpret_cast<const uint4*>(edge_of(utx, tyD) + G::E_TOP / 4);
+        if (Y == 0) hv = *reinterpret_cast<const uint4*>(nb.up + G::E_BOT / 4);
+        else if (Y == G::LPT - 1) hv = *reinterpret_cast<const uint4*>(nb.dn + G::E_TOP / 4);
         t.vrow[0][0] = hv.x;
         if (G::NW == 2) { t.vrow[0][1] = hv.y; t.vrow[1][0] = hv.z; t.vrow[1][1] = hv.w; }
         else t.vrow[1][0] = hv.y;
-        const uint2 cl = *reinterpret_cast<const uint2*>(edge_of(txL, uty) + G::E_COL / 4 + 2);   // {R0, R1}
-        const uint2 cr = *reinterpret_cast<const uint2*>(edge_of(txR, uty) + G::E_COL / 4);       // {L0, L1}
+        const uint2 cl = *reinterpret_cast<const uint2*>(nb.lf + G::E_COL / 4 + 2);   // {R0, R1}
+        const uint2 cr = *reinterpret_cast<const uint2*>(nb.rt + G::E_COL / 4);       // {L0, L1}
         t.hL0 = (cl.x >> Y) & 1u; t.hL1 = (cl.y >> Y) & 1u;
         t.hR0 = (cr.x >> Y) & 1u; t.hR1 = (cr.y >> Y) & 1u;
     };
 
     TileRegs<T> t[2][kResMaxJobs];
     int txs[2][kResMaxJobs], tys[2][kResMaxJobs];
+    Nb nbs[2][kResMaxJobs];
 #pragma unroll
     for (int C = 0; C < 2; ++C)
 #pragma unroll
@@ -564,6 +569,7 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
             const uint32_t job = wg + (uint32_t)m * W;
             if (job < JC) {
                 tile_of(C, job, txs[C][m], tys[C][m]);
+                nbs[C][m] = neighbours(txs[C][m], tys[C][m]);
                 load_tile<T, BITS>(A, r, txs[C][m], tys[C][m], Y, sub * G::LPT, t[C][m]);
                 publish(C, m, t[C][m]);
             }
@@ -581,7 +587,7 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
                 const uint32_t job = wg + (uint32_t)m * W;
                 if (job < JC) {
                     const int tx = txs[C][m], ty = tys[C][m];
-                    refresh(tx, ty, t[C][m]);
+                    refresh(nbs[C][m], t[C][m]);
                     const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);
                     const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(tx * G::NW);
                     const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);
