@@ -469,13 +469,16 @@ def main() -> None:
     bytes_per_launch = bpf * a.k * L * L / launches_per_step
     launch_ms = res["ms"] / (a.steps * launches_per_step)
     achieved = bytes_per_launch / (launch_ms * 1e6)            # GB/s
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
+    lat_bytes = L * L if a.layout == "int8" else L * L // 8
+    line = {"metric": METRIC if L == 16384 else f"spin flips/ns (2D Ising L={L}, beta_c)", "value": value, "unit": UNIT,
+            "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
             "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "u8" if a.layout == "int8" else "u32 bit-planes", "data": "synthetic",
-            "config": {"workload": f"BASELINE config 3: 2D Ising L={L} hot start seed 3 beta=0.4406868 layout={a.layout} "
-                                   f"rng={a.rng} tile={a.tile} k={a.k}; one step = one outer pass (2 launches)",
-                       "l2": "lattice (256 MiB int8) exceeds the 126 MB L2; no explicit flush" if a.layout == "int8"
-                             else "lattice (32 MiB bits) fits L2: bit-packed variant is ALU-bound, not an HBM claim",
+            "config": {"workload": f"{'BASELINE config 3' if L == 16384 else 'config 3 at another size'}: 2D Ising L={L} hot start seed 3 "
+                                   f"beta=0.4406868 layout={a.layout} rng={a.rng} tile={a.tile} k={a.k}; one step = one outer pass "
+                                   + ("(2 launches)" if not res["path"].startswith("resident") else "(all steps in one cluster launch)"),
+                       "l2": f"lattice ({lat_bytes / 2 ** 20:g} MiB {a.layout}) exceeds the 126 MB L2; no explicit flush" if lat_bytes > 126e6
+                             else f"lattice ({lat_bytes / 2 ** 20:g} MiB {a.layout}) fits L2: not an HBM claim",
                        "kernel_path": res["path"], "parallelism": "replicas only" if world > 1 else "single GPU"},
             "ns_per_flip": 1.0 / value, "gpu_launches": res["launches"], "clocks": res["clocks"],
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
