@@ -386,11 +386,16 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         // small lattices, several passes, nothing to measure in between: the whole call in one cluster launch
         const bool use_resident = use_planes && !want_series && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->has_J && !h->no_resident &&
                                   resident_planes_supported(h, T);
+        bool resident_done = false;
         if (use_resident && !rc) {
-            h->last_path = bits ? "resident_planes_bits" : "resident_planes_i8";
-            rc = launch_resident_planes(h, acc, T, bits, n, k, h->t);
+            if (launch_resident_planes(h, acc, T, bits, n, k, h->t) == 0) {
+                h->last_path = bits ? "resident_planes_bits" : "resident_planes_i8";
+                resident_done = true;
+            } else {
+                cudaGetLastError();      // the cluster did not fit (shared or partitioned GPU): a launch per colour instead
+            }
         }
-        for (int pass = 0; pass < n && !rc && !use_resident; ++pass) {
+        for (int pass = 0; pass < n && !rc && !resident_done; ++pass) {
             const uint64_t t0 = h->t + (uint64_t)pass * (uint64_t)k;
             rc = use_tile_i8 ? launch_tile_i8_pass(h, acc, T, k, t0)
                  : use_3d ? launch_tile3d_pass(h, acc, bits, k, t0, use_jit)
