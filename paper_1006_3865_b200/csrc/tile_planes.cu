@@ -106,11 +106,12 @@ __global__ void __launch_bounds__(kPlaneThreads) k_observables_planes(PlaneArgs 
     }
 }
 
-// ---- layout converters (a11): canonical int8 +-1 <-> tile records; not on the timed path ----
-// One thread per site; MODE 0: canonical -> int8 records, 1: int8 records -> canonical,
-// 2: canonical -> bit records, 3: bit records -> canonical.  Bit fields are set by atomicOr into zeroed storage.
+// ---- layout converters (a11): canonical int8 +-1 <-> bit records; not on the timed path ----
+// One thread per site; MODE 2: canonical -> bit records, 3: bit records -> canonical.  Bit fields are set by atomicOr
+// into zeroed storage.  (The int8 records have their own converters below.)
 template <int MODE>
 __global__ void k_convert_planes(int8_t* __restrict__ canon, uint8_t* __restrict__ tiles, int L, int T, int R) {
+    static_assert(MODE == 2 || MODE == 3, "bit records only");
     const uint64_t N = (uint64_t)L * L;
     const uint64_t gid = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (gid >= N * (uint64_t)R) return;
@@ -121,18 +122,13 @@ __global__ void k_convert_planes(int8_t* __restrict__ canon, uint8_t* __restrict
     const int tx = x / T, ty = y / T, lx = x - tx * T, ly = y - ty * T;
     const int cc = (lx + ly) & 1, px = lx >> 1, gx = px >> 4, kk = px & 15, rp = ly & 1, Y = ly >> 1;
     const size_t tile = ((size_t)r * B + ty) * B + tx;
-    constexpr bool BITS = MODE >= 2;
-    const size_t body_bytes = BITS ? (size_t)(T * T / 8) : (size_t)(T * T);
+    const size_t body_bytes = (size_t)(T * T / 8);
     uint8_t* rec = tiles + tile * (body_bytes + 64);
-    uint8_t* body = rec + ((((rp * 2 + cc) * NW + gx) * LPT) + Y) * 16 + piece_byte(kk);
     uint32_t* w = reinterpret_cast<uint32_t*>(rec) + ((cc * NW + gx) * LPT + Y);
     const int j = rp * 16 + kk;
-    if (MODE == 1) { canon[gid] = *body ? 1 : -1; return; }
     if (MODE == 3) { canon[gid] = ((*w >> j) & 1u) ? 1 : -1; return; }
-    const bool up = canon[gid] > 0;
-    if (!BITS) *body = up ? 1 : 0;
-    if (!up) return;
-    if (BITS) atomicOr(w, 1u << j);
+    if (canon[gid] <= 0) return;
+    atomicOr(w, 1u << j);
     uint32_t* e = reinterpret_cast<uint32_t*>(rec + body_bytes);          // boundary copies (zeroed first), see PG
     if (Y == 0) atomicOr(e + 0 + cc * NW + gx, 1u << j);                  // TOP: words of block row 0
     if (Y == LPT - 1) atomicOr(e + 8 + cc * NW + gx, 1u << j);            // BOT: words of block row LPT-1
@@ -356,11 +352,7 @@ int launch_canon_to_planes(ising_ctx* h, int T, bool bits, const int8_t* d_canon
         return 0;
     }
     ISING_CUDA_OK(cudaMemsetAsync(d_tiles, 0, tile_planes_bytes(h, T, bits), st));
-    if (bits) {
-        k_convert_planes<2><<<blocks, 256, 0, st>>>(const_cast<int8_t*>(d_canon), (uint8_t*)d_tiles, h->L, T, h->R);
-    } else {
-        k_convert_planes<0><<<blocks, 256, 0, st>>>(const_cast<int8_t*>(d_canon), (uint8_t*)d_tiles, h->L, T, h->R);
-    }
+    k_convert_planes<2><<<blocks, 256, 0, st>>>(const_cast<int8_t*>(d_canon), (uint8_t*)d_tiles, h->L, T, h->R);
     count_launch();
     ISING_CUDA_OK(cudaGetLastError());
     return 0;
@@ -380,8 +372,7 @@ int launch_planes_to_canon(ising_ctx* h, int T, bool bits, const void* d_tiles, 
         ISING_CUDA_OK(cudaGetLastError());
         return 0;
     }
-    if (bits) k_convert_planes<3><<<blocks, 256, 0, st>>>(d_canon, (uint8_t*)const_cast<void*>(d_tiles), h->L, T, h->R);
-    else k_convert_planes<1><<<blocks, 256, 0, st>>>(d_canon, (uint8_t*)const_cast<void*>(d_tiles), h->L, T, h->R);
+    k_convert_planes<3><<<blocks, 256, 0, st>>>(d_canon, (uint8_t*)const_cast<void*>(d_tiles), h->L, T, h->R);
     count_launch();
     ISING_CUDA_OK(cudaGetLastError());
     return 0;
