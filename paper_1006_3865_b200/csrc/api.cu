@@ -384,11 +384,11 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
                              (h->jit_mode == ISING_JIT_AUTO && (double)n * k * (double)h->N * h->R >= 134217728.0));
         h->last_jit = 0;
         // small lattices, several passes, nothing to measure in between: the whole call in one cluster launch
-        const bool use_resident = use_planes && !want_series && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->has_J && !h->no_resident &&
+        const bool use_resident = use_planes && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->has_J && !h->no_resident &&
                                   resident_planes_supported(h, T);
         bool resident_done = false;
         if (use_resident && !rc) {
-            if (launch_resident_planes(h, acc, T, bits, n, k, h->t) == 0) {
+            if (launch_resident_planes(h, acc, T, bits, n, k, h->t, d_E, d_M) == 0) {
                 h->last_path = bits ? "resident_planes_bits" : "resident_planes_i8";
                 resident_done = true;
             } else {

@@ -489,6 +489,8 @@ struct ResArgs {
     PlaneArgs P;
     int n;                         // outer passes
     uint32_t jobs_per_colour;      // per replica
+    long long* E;                  // optional series (a10 after every pass): E[pass * R + r], M[pass * R + r]
+    long long* M;
 };
 
 template <int T, bool BITS>
@@ -505,6 +507,19 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
     const uint32_t B = (uint32_t)A.B, hb = B >> 1, JC = R.jobs_per_colour;
     const uint2* lut = kByteLutGlobal.e;
     __shared__ __align__(16) uint32_t edges[2][kResMaxJobs][kResWarps][G::TPW][12];
+    __shared__ int acc[2][2];          // rank 0 only: {#up, #unsatisfied bonds} of the replica, for even / odd passes
+    if (threadIdx.x < 4) (&acc[0][0])[threadIdx.x] = 0;
+    int* const acc0 = cluster.map_shared_rank(&acc[0][0], 0);
+    const bool series = R.E != nullptr || R.M != nullptr;
+    const long long nsites = (long long)A.L * A.L;
+    auto write_series = [&](int pass) {                                // by one thread of the cluster, a barrier after the atomics
+        if (rank == 0 && threadIdx.x == 0) {
+            int* a = &acc[pass & 1][0];
+            if (R.M) R.M[(size_t)pass * A.R + r] = 2ll * a[0] - nsites;
+            if (R.E) R.E[(size_t)pass * A.R + r] = 2ll * a[1] - 2ll * nsites;
+            a[0] = 0; a[1] = 0;
+        }
+    };
 
     auto tile_of = [&](int C, uint32_t job, int& tx, int& ty) {
         const uint32_t qq = job * G::TPW + (uint32_t)sub;
@@ -573,6 +588,8 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
     for (int pass = 0; pass < R.n; ++pass) {
 #pragma unroll
         for (int C = 0; C < 2; ++C) {
+            // the previous pass's sums were added after its last barrier and are complete since the barrier just passed
+            if (series && C == 1 && pass > 0) write_series(pass - 1);
 #pragma unroll
             for (int m = 0; m < kResMaxJobs; ++m) {
                 const uint32_t job = wg + (uint32_t)m * W;
@@ -592,6 +609,35 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
             }
             cluster.sync();
         }
+        if (series) {
+            // a10 on the registers: every bond has one end of fine colour 0; the colour-0 tiles' halos are one phase
+            // old, the colour-1 tiles' are current.  Sums go to rank 0 (alternating slots, so that the thread that
+            // writes pass p out, one barrier later, never meets the atomics of pass p + 1).
+            int up = 0, unsat = 0;
+#pragma unroll
+            for (int C = 0; C < 2; ++C)
+#pragma unroll
+                for (int m = 0; m < kResMaxJobs; ++m) {
+                    const uint32_t job = wg + (uint32_t)m * W;
+                    if (job < JC) {
+                        if (C == 0) refresh(nbs[C][m], t[C][m]);
+                        count_row<T, false>(t[C][m], Jw, Y, up, unsat);
+                    }
+                }
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                up += __shfl_xor_sync(0xffffffffu, up, d);
+                unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+            }
+            if (lane == 0) {
+                atomicAdd(acc0 + 2 * (pass & 1), up);
+                atomicAdd(acc0 + 2 * (pass & 1) + 1, unsat);
+            }
+        }
+    }
+    if (series && R.n > 0) {
+        cluster.sync();
+        write_series(R.n - 1);
     }
 #pragma unroll
     for (int C = 0; C < 2; ++C)
@@ -600,6 +646,7 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
             const uint32_t job = wg + (uint32_t)m * W;
             if (job < JC) store_tile<T, BITS>(A, r, txs[C][m], tys[C][m], Y, sub, t[C][m], lut);
         }
+    cluster.sync();            // no CTA leaves while its shared memory may still be read or added to
 }
 
 bool resident_planes_supported(const ising_ctx* h, int T) {
@@ -626,8 +673,10 @@ static int launch_resident(const ResArgs& R, int replicas) {
 }
 
 // n passes in one launch; the records must hold the state (ensure_store) and are current again afterwards.
-int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first) {
+int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first,
+                           long long* d_E, long long* d_M) {
     ResArgs R;
+    R.E = d_E; R.M = d_M;
     PlaneArgs& A = R.P;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;

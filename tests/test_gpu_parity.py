@@ -104,6 +104,7 @@ def test_tile_planes_path_matches_oracle(P, orc, L, tile, k, n, beta, seeds, lay
     g, o = _both(P, orc, 2, L, seeds, rng="planes")
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
+    g.force_path(2)            # a launch per coarse colour also where the cluster-resident kernel would serve
     Eg, Mg = g.sweep_series(beta, n, tile, k)
     assert g.sweep_path() == f"tile_planes_{'i8' if layout == 'int8' else 'bits'}"
     Eo, Mo = o.sweep_series(beta, n, tile, k)
@@ -436,3 +437,14 @@ def test_cluster_resident_kernel_matches_oracle(P, orc, L, tile, k, n, beta, see
     g.sweep(beta, 2, tile, k); o.sweep(beta, 2, tile, k)
     assert g.sweep_path().startswith("tile_planes")
     _same_state(g, o)
+    g.force_path(0)
+    Eg, Mg = g.sweep_series(beta, n + 1, tile, k)                 # E and M after every pass, measured on the registers
+    assert g.sweep_path().startswith("resident_planes")
+    Eo, Mo = o.sweep_series(beta, n + 1, tile, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    import torch
+    Ed = torch.zeros((2, len(seeds)), dtype=torch.int64, device="cuda")   # device buffers, E only
+    g.sweep_series(beta, 2, tile, k, E=Ed, M=None)
+    Eo, _ = o.sweep_series(beta, 2, tile, k)
+    assert np.array_equal(Ed.cpu().numpy(), Eo)
