@@ -387,6 +387,16 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         const bool use_resident = use_planes && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->has_J && !h->no_resident &&
                                   resident_planes_supported(h, T);
         bool resident_done = false;
+        const bool use_resident3 = use_3d && !want_series && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident &&
+                                   resident3d_supported(h, T);
+        if (use_resident3 && !rc) {
+            if (launch_resident3d(h, acc, bits, n, k, h->t) == 0) {
+                h->last_path = bits ? "resident3d_planes_bits" : "resident3d_planes_i8";
+                resident_done = true;
+            } else {
+                cudaGetLastError();
+            }
+        }
         if (use_resident && !rc) {
             if (launch_resident_planes(h, acc, T, bits, n, k, h->t, d_E, d_M) == 0) {
                 h->last_path = bits ? "resident_planes_bits" : "resident_planes_i8";

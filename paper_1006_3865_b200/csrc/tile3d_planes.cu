@@ -17,6 +17,8 @@
 //   faces: XL[8] words (sites x=0 of slice lz, row ly at bit 4ly+3), XR[8] words (x=7, bit 4ly),
 //          YL[8] bytes (row y=0: colour 0 pairs in bits 0-3, colour 1 in 4-7), YR[8] bytes (y=7),
 //          ZL 2 words (slice 0, colour 0 and 1), ZR 2 words (slice 7).
+#include <cooperative_groups.h>
+
 #include "kernels.h"
 #include "tile3d_planes_device.cuh"
 
@@ -131,6 +133,154 @@ int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64
         }
         count_launch();
     }
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+// ---- whole lattice on chip, 3D (L <= 64): one thread-block cluster per replica, slices in registers, the 96-byte face
+// areas of the tiles in shared memory, read by the neighbours through distributed shared memory; the design of
+// k_resident_planes (tile_planes.cu) carried over.
+constexpr int kRes3Warps = 4;
+constexpr int kRes3MaxCluster = 16;
+
+struct Res3Args {
+    Plane3Args P;
+    int n;
+    uint32_t jobs_per_colour;      // per replica, 4 tiles per job
+};
+
+template <bool BITS>
+__global__ void __launch_bounds__(kRes3Warps * 32) k_resident3d(Res3Args R) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    const uint32_t CL = cluster.num_blocks(), rank = cluster.block_rank();
+    const Plane3Args& A = R.P;
+    const int r = (int)(blockIdx.x / CL);
+    const int lane = threadIdx.x & 31, wic = threadIdx.x >> 5;
+    const uint32_t wg = rank * kRes3Warps + (uint32_t)wic;            // one job per warp and colour
+    const int sub = lane >> 3, lz = lane & 7;
+    const uint32_t B = (uint32_t)A.B, hb = B >> 1, JC = R.jobs_per_colour;
+    const uint2* lut = kByteLutGlobal.e;
+    __shared__ __align__(16) uint8_t faces[2][kRes3Warps][4][kFaces3];
+
+    auto tile_of = [&](int C, uint32_t job) {
+        uint32_t q = job * 4u + (uint32_t)sub;                        // colour-C tiles of the replica, (tz, ty, tx/2) row-major
+        Tile3 t;
+        t.r = r;
+        t.tz = (int)(q / (B * hb)); q -= (uint32_t)t.tz * B * hb;
+        t.ty = (int)(q / hb); q -= (uint32_t)t.ty * hb;
+        t.tx = (int)(2u * q) + ((t.ty + t.tz + C) & 1);
+        return t;
+    };
+    auto faces_of = [&](uint32_t tx, uint32_t ty, uint32_t tz) -> const uint8_t* {
+        const uint32_t C = (tx + ty + tz) & 1u, q = (tz * B + ty) * hb + (tx >> 1);
+        const uint32_t job = q >> 2, sb = q & 3u;                      // job < W: one job per warp and colour
+        return cluster.map_shared_rank(&faces[C][job % kRes3Warps][sb][0], job / kRes3Warps);
+    };
+    struct Nb { const uint8_t *xm, *xp, *ym, *yp, *zm, *zp; };
+    auto neighbours = [&](const Tile3& t) {
+        const uint32_t tx = (uint32_t)t.tx, ty = (uint32_t)t.ty, tz = (uint32_t)t.tz;
+        return Nb{faces_of(tx == 0 ? B - 1 : tx - 1, ty, tz), faces_of(tx == B - 1 ? 0 : tx + 1, ty, tz),
+                  faces_of(tx, ty == 0 ? B - 1 : ty - 1, tz), faces_of(tx, ty == B - 1 ? 0 : ty + 1, tz),
+                  faces_of(tx, ty, tz == 0 ? B - 1 : tz - 1), faces_of(tx, ty, tz == B - 1 ? 0 : tz + 1)};
+    };
+    auto publish = [&](int C, const Slice& s) {
+        uint32_t XL, XR, YL, YR;
+        face_words(s.S, lz, XL, XR, YL, YR);
+        uint8_t* f = &faces[C][wic][sub][0];
+        reinterpret_cast<uint32_t*>(f + kXL)[lz] = XL;
+        reinterpret_cast<uint32_t*>(f + kXR)[lz] = XR;
+        f[kYL + lz] = (uint8_t)YL;
+        f[kYR + lz] = (uint8_t)YR;
+        if (lz == 0) *reinterpret_cast<uint2*>(f + kZL) = make_uint2(s.S[0], s.S[1]);
+        if (lz == 7) *reinterpret_cast<uint2*>(f + kZR) = make_uint2(s.S[0], s.S[1]);
+    };
+    auto refresh = [&](const Nb& nb, Slice& s) {
+        s.xl = reinterpret_cast<const uint32_t*>(nb.xm + kXR)[lz];
+        s.xr = reinterpret_cast<const uint32_t*>(nb.xp + kXL)[lz];
+        s.ym = nb.ym[kYR + lz];
+        s.yp = nb.yp[kYL + lz];
+        if (lz == 0) { const uint2 w = *reinterpret_cast<const uint2*>(nb.zm + kZR); s.zm[0] = w.x; s.zm[1] = w.y; }
+        if (lz == 7) { const uint2 w = *reinterpret_cast<const uint2*>(nb.zp + kZL); s.zp[0] = w.x; s.zp[1] = w.y; }
+    };
+
+    const bool mine = wg < JC;
+    Slice s[2];
+    Tile3 t[2];
+    Nb nb[2];
+#pragma unroll
+    for (int C = 0; C < 2; ++C)
+        if (mine) {
+            t[C] = tile_of(C, wg);
+            nb[C] = neighbours(t[C]);
+            load_slice<BITS>(A, t[C], lz, s[C]);
+            publish(C, s[C]);
+        }
+    cluster.sync();
+
+    const uint64_t seed = A.seeds[r];
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    for (int pass = 0; pass < R.n; ++pass) {
+#pragma unroll
+        for (int C = 0; C < 2; ++C) {
+            if (mine) {
+                refresh(nb[C], s[C]);
+                const uint32_t z = (uint32_t)(t[C].tz * kT3 + lz);
+                const uint32_t g = (z * B + (uint32_t)t[C].ty) * B + (uint32_t)t[C].tx;
+                const uint32_t p_base = (uint32_t)(t[C].tx * 4) + (uint32_t)(A.L >> 1) * ((uint32_t)(t[C].ty * kT3) + (uint32_t)A.L * z);
+                for (int j = 0; j < A.k; ++j) {
+                    const uint64_t tt = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
+                    half_sweep3<kNoSpec3>(A, s[C], 0, lz, g, p_base, 2 * tt, k0, k1);
+                    half_sweep3<kNoSpec3>(A, s[C], 1, lz, g, p_base, 2 * tt + 1, k0, k1);
+                }
+                publish(C, s[C]);
+            }
+            cluster.sync();
+        }
+    }
+#pragma unroll
+    for (int C = 0; C < 2; ++C)
+        if (mine) store_slice<BITS>(A, t[C], lz, s[C], lut);
+}
+
+bool resident3d_supported(const ising_ctx* h, int T) {
+    if (!tile3d_supported(h, T)) return false;
+    const uint32_t B = (uint32_t)(h->L / kT3);
+    return B * B * B / 2u / 4u <= (uint32_t)(kRes3MaxCluster * kRes3Warps) && (B * B * B / 2u) % 4u == 0;
+}
+
+int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first) {
+    Res3Args R;
+    Plane3Args& A = R.P;
+    A.tiles = (uint8_t*)h->d_tiles;
+    A.seeds = h->d_sweep_seeds;
+    A.L = h->L; A.B = h->L / kT3; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0;
+    A.njobs = 0; A.per_rep = A.per_z = A.hb = 0; A.magic_rep = A.magic_z = A.magic_hb = 0;
+    for (int m = 0; m < 3; ++m) {
+        for (int q = 0; q < kHeadBits; ++q) A.u[m][q] = ((acc.thr[m] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
+        A.tail[m] = acc.thr[m] & ((1u << kTailBits) - 1u);
+    }
+    A.force = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
+    R.n = n;
+    const uint32_t B = (uint32_t)A.B;
+    R.jobs_per_colour = B * B * B / 2u / 4u;
+    const uint32_t want = (R.jobs_per_colour + kRes3Warps - 1) / kRes3Warps;
+    unsigned cl = 1;
+    while (cl < want && cl < (unsigned)kRes3MaxCluster) cl *= 2;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(cl * (unsigned)h->R); cfg.blockDim = dim3(kRes3Warps * 32); cfg.dynamicSmemBytes = 0; cfg.stream = hooks().stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (bits) {
+        if (cl > 8) ISING_CUDA_OK(cudaFuncSetAttribute(k_resident3d<true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_resident3d<true>, R));
+    } else {
+        if (cl > 8) ISING_CUDA_OK(cudaFuncSetAttribute(k_resident3d<false>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_resident3d<false>, R));
+    }
+    count_launch();
     ISING_CUDA_OK(cudaGetLastError());
     return 0;
 }

@@ -448,3 +448,30 @@ def test_cluster_resident_kernel_matches_oracle(P, orc, L, tile, k, n, beta, see
     g.sweep_series(beta, 2, tile, k, E=Ed, M=None)
     Eo, _ = o.sweep_series(beta, 2, tile, k)
     assert np.array_equal(Ed.cpu().numpy(), Eo)
+
+
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,k,n,beta,seeds", [
+    (16, 1, 4, BC3, [4]),            # one job per colour, a cluster of one CTA; every halo wraps onto the other tile
+    (32, 4, 3, BC3, [4]),
+    (48, 2, 3, 0.3, [5, 6]),         # 27 jobs per colour, two clusters
+    (64, 1, 5, BC3, [9]),            # 64 jobs per colour: all 64 warps of a 16-CTA cluster
+    (32, 2, 2, 0.0, [2]),
+    (32, 2, 2, 9.0, [2]),
+])
+def test_cluster_resident_3d_kernel_matches_oracle(P, orc, L, k, n, beta, seeds, layout):
+    """3D, L <= 64, n >= 2 passes: one launch of one cluster per replica, slices in registers, faces through DSMEM."""
+    g, o = _both(P, orc, 3, L, seeds, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.sweep(beta, n, 8, k); o.sweep(beta, n, 8, k)
+    assert g.sweep_path() == f"resident3d_planes_{'i8' if layout == 'int8' else 'bits'}"
+    _same_state(g, o)
+    g.sweep(beta, 1, 8, k); o.sweep(beta, 1, 8, k)
+    assert g.sweep_path().startswith("tile3d_planes")
+    g.sweep(beta, 2, 8, k); o.sweep(beta, 2, 8, k)
+    _same_state(g, o)
+    if L == 64 and layout == "int8":
+        big = P.Ising(3, 128, seed=1)
+        big.sweep(beta, 2, 8, 1)
+        assert big.sweep_path() == "tile3d_planes_i8"
