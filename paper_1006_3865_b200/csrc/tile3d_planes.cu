@@ -19,6 +19,8 @@
 //          ZL 2 words (slice 0, colour 0 and 1), ZR 2 words (slice 7).
 #include <cooperative_groups.h>
 
+#include <cstdlib>
+
 #include "kernels.h"
 #include "tile3d_planes_device.cuh"
 
@@ -119,17 +121,22 @@ int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64
                                    ((unsigned long long)(acc.thr[1] >> kTailBits) << 12) | (unsigned long long)(acc.thr[2] >> kTailBits);
     cudaKernel_t spec = (use_jit && !A.force) ? planes3d_jit_kernel(bits, hp3) : nullptr;
     h->last_jit = spec ? 1 : 0;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(warps * 32); cfg.stream = hooks().stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    static const int pdl = getenv("ISING_NO_PDL") ? 0 : 1;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl;
+    cfg.attrs = attr; cfg.numAttrs = 1;
     for (int C = 0; C < 2; ++C) {
         A.C = C;
         if (spec) {
-            cudaLaunchConfig_t cfg = {};
-            cfg.gridDim = dim3(grid); cfg.blockDim = dim3(warps * 32); cfg.stream = hooks().stream;
             void* args[] = {&A};
             ISING_CUDA_OK(cudaLaunchKernelExC(&cfg, (const void*)spec, args));
         } else if (bits) {
-            k_tile3d_planes<true><<<grid, warps * 32, 0, hooks().stream>>>(A);
+            ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_planes<true>, A));
         } else {
-            k_tile3d_planes<false><<<grid, warps * 32, 0, hooks().stream>>>(A);
+            ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_planes<false>, A));
         }
         count_launch();
     }

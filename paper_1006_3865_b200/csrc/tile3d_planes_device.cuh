@@ -255,6 +255,10 @@ constexpr int kThreads3 = 64;        // 2 warps = 8 tiles per CTA: small CTAs so
 template <bool BITS, unsigned long long HP3 = kNoSpec3>
 __global__ void __launch_bounds__(kThreads3) k_tile3d_planes(Plane3Args A) {
     const uint2* lut = kByteLutGlobal.e;      // int8 write-back table, read-only path (planes_common.cuh)
+    // Programmatic dependent launch, as in k_tile_planes: the next colour's grid may be scheduled while this one
+    // drains; it waits here until every store of the previous launch is visible.
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
     const int lane = threadIdx.x & 31;
     const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (job >= A.njobs) return;
