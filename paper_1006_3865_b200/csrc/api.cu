@@ -384,7 +384,7 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
                              (h->jit_mode == ISING_JIT_AUTO && (double)n * k * (double)h->N * h->R >= 134217728.0));
         h->last_jit = 0;
         // small lattices, several passes, nothing to measure in between: the whole call in one cluster launch
-        const bool use_resident = use_planes && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->has_J && !h->no_resident &&
+        const bool use_resident = use_planes && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident &&
                                   resident_planes_supported(h, T);
         bool resident_done = false;
         const bool use_resident3 = use_3d && !want_series && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident &&

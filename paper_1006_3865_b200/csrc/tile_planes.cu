@@ -493,7 +493,7 @@ struct ResArgs {
     long long* M;
 };
 
-template <int T, bool BITS>
+template <int T, bool BITS, bool HASJ>
 __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
     using G = PG<T>;
     namespace cg = cooperative_groups;
@@ -568,6 +568,7 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
     TileRegs<T> t[2][kResMaxJobs];
     int txs[2][kResMaxJobs], tys[2][kResMaxJobs];
     Nb nbs[2][kResMaxJobs];
+    uint4 Jws[2][kResMaxJobs][2][G::NW];                               // coupling words of the tiles (a9), zero for J = +1
 #pragma unroll
     for (int C = 0; C < 2; ++C)
 #pragma unroll
@@ -576,6 +577,12 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
             if (job < JC) {
                 tile_of(C, job, txs[C][m], tys[C][m]);
                 nbs[C][m] = neighbours(txs[C][m], tys[C][m]);
+#pragma unroll
+                for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+                    for (int gx = 0; gx < G::NW; ++gx)
+                        Jws[C][m][cc][gx] = HASJ ? __ldg(A.jrec + ((size_t)tys[C][m] * B + txs[C][m]) * (2 * G::NW * G::LPT) + (cc * G::NW + gx) * G::LPT + Y)
+                                                 : make_uint4(0u, 0u, 0u, 0u);
                 load_tile<T, BITS>(A, r, txs[C][m], tys[C][m], Y, sub * G::LPT, t[C][m]);
                 publish(C, m, t[C][m]);
             }
@@ -584,7 +591,6 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
 
     const uint64_t seed = A.seeds[r];
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
-    const uint4 Jw[2][G::NW] = {};
     for (int pass = 0; pass < R.n; ++pass) {
 #pragma unroll
         for (int C = 0; C < 2; ++C) {
@@ -601,8 +607,8 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
                     const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);
                     for (int j = 0; j < A.k; ++j) {
                         const uint64_t tt = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
-                        half_sweep<T, false, false, kNoSpec>(A, t[C][m], Jw, 0, Y, g0, p0, 2 * tt, k0, k1);
-                        half_sweep<T, false, false, kNoSpec>(A, t[C][m], Jw, 1, Y, g0, p0, 2 * tt + 1, k0, k1);
+                        half_sweep<T, HASJ, false, kNoSpec>(A, t[C][m], Jws[C][m], 0, Y, g0, p0, 2 * tt, k0, k1);
+                        half_sweep<T, HASJ, false, kNoSpec>(A, t[C][m], Jws[C][m], 1, Y, g0, p0, 2 * tt + 1, k0, k1);
                     }
                     publish(C, m, t[C][m]);
                 }
@@ -621,7 +627,7 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
                     const uint32_t job = wg + (uint32_t)m * W;
                     if (job < JC) {
                         if (C == 0) refresh(nbs[C][m], t[C][m]);
-                        count_row<T, false>(t[C][m], Jw, Y, up, unsat);
+                        count_row<T, false>(t[C][m], Jws[C][m], Y, up, unsat);
                     }
                 }
 #pragma unroll
@@ -650,24 +656,24 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
 }
 
 bool resident_planes_supported(const ising_ctx* h, int T) {
-    if (!tile_planes_supported(h, T) || h->has_J) return false;
+    if (!tile_planes_supported(h, T)) return false;
     const uint32_t B = (uint32_t)(h->L / T);
     return B * B / 2u / (uint32_t)(64 / T) <= (uint32_t)(kResMaxCluster * kResWarps * kResMaxJobs);
 }
 
-template <int T, bool BITS>
+template <int T, bool BITS, bool HASJ>
 static int launch_resident(const ResArgs& R, int replicas) {
     const uint32_t want = (R.jobs_per_colour + kResWarps - 1) / kResWarps;
     unsigned cl = 1;
     while (cl < want && cl < (unsigned)kResMaxCluster) cl *= 2;
-    if (cl > 8) ISING_CUDA_OK(cudaFuncSetAttribute(k_resident_planes<T, BITS>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    if (cl > 8) ISING_CUDA_OK(cudaFuncSetAttribute(k_resident_planes<T, BITS, HASJ>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(cl * (unsigned)replicas); cfg.blockDim = dim3(kResWarps * 32); cfg.dynamicSmemBytes = 0; cfg.stream = hooks().stream;
     cudaLaunchAttribute attr[1];
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_resident_planes<T, BITS>, R));
+    ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_resident_planes<T, BITS, HASJ>, R));
     count_launch();
     return 0;
 }
@@ -681,14 +687,17 @@ int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, in
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0;
-    A.jrec = nullptr;
+    A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;        // shared by the replicas
     A.stream = 0;
     A.njobs = 0; A.magic_rep = A.magic_hb = 0;
     fill_accept(A, acc);
     R.n = n;
     R.jobs_per_colour = (uint32_t)A.B * (uint32_t)A.B / 2u / (uint32_t)(64 / T);
-    const int rc = T == 64 ? (bits ? launch_resident<64, true>(R, h->R) : launch_resident<64, false>(R, h->R))
-                           : (bits ? launch_resident<32, true>(R, h->R) : launch_resident<32, false>(R, h->R));
+    int rc;
+    if (A.jrec) rc = T == 64 ? (bits ? launch_resident<64, true, true>(R, h->R) : launch_resident<64, false, true>(R, h->R))
+                             : (bits ? launch_resident<32, true, true>(R, h->R) : launch_resident<32, false, true>(R, h->R));
+    else rc = T == 64 ? (bits ? launch_resident<64, true, false>(R, h->R) : launch_resident<64, false, false>(R, h->R))
+                      : (bits ? launch_resident<32, true, false>(R, h->R) : launch_resident<32, false, false>(R, h->R));
     if (rc) return rc;
     ISING_CUDA_OK(cudaGetLastError());
     return 0;

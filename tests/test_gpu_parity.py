@@ -125,6 +125,7 @@ def test_tile_planes_couplings_match_oracle(P, orc, L, tile, k, n, beta, seeds, 
     g, o = _both(P, orc, 2, L, seeds, J, rng="planes")
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
+    g.force_path(2)            # a launch per coarse colour (the cluster-resident kernel has its own test)
     Eg, Mg = g.sweep_series(beta, n, tile, k)
     assert g.sweep_path() == f"tile_planes_{'i8' if layout == 'int8' else 'bits'}"
     Eo, Mo = o.sweep_series(beta, n, tile, k)
@@ -475,3 +476,29 @@ def test_cluster_resident_3d_kernel_matches_oracle(P, orc, L, k, n, beta, seeds,
         big = P.Ising(3, 128, seed=1)
         big.sweep(beta, 2, 8, 1)
         assert big.sweep_path() == "tile3d_planes_i8"
+
+
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,tile,k,n,beta,seeds,jseed", [
+    (64, 32, 2, 4, 1.0, [100, 101, 102], 5),       # small +-J glass, three replicas = three clusters sharing J
+    (128, 64, 1, 3, 0.8, [7], 11),
+    (192, 32, 3, 2, 0.5, [8, 9], 12),
+    (512, 32, 1, 3, 1.2, [3], 13),
+])
+def test_cluster_resident_kernel_with_couplings(P, orc, L, tile, k, n, beta, seeds, jseed, layout):
+    """a9 on the cluster-resident kernel: the tiles' coupling words stay in registers with the spins."""
+    J = W.couplings(2, L, jseed)
+    g, o = _both(P, orc, 2, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.sweep(beta, n, tile, k); o.sweep(beta, n, tile, k)
+    assert g.sweep_path() == f"resident_planes_{'i8' if layout == 'int8' else 'bits'}"
+    _same_state(g, o)
+    Eg, Mg = g.sweep_series(beta, n, tile, k)
+    assert g.sweep_path().startswith("resident_planes")
+    Eo, Mo = o.sweep_series(beta, n, tile, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    for a in range(len(seeds)):
+        for b in range(a + 1, len(seeds)):
+            assert g.overlap(a, b) == o.overlap(a, b)
