@@ -371,12 +371,12 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
                                                         : (bits ? "tile_planes_bits" : "tile_planes_i8");
         rc = ensure_store(h, use_tile_i8 ? Store::TileI8 : use_3d ? (bits ? Store::Plane3Bits : Store::Plane3I8)
                                                                   : (bits ? Store::PlaneBits : Store::PlaneI8), T);
-        if (!rc && use_planes && h->has_J && h->Jtiles_tile != T) {      // coupling records for this tile edge
+        if (!rc && (use_planes || use_3d) && h->has_J && h->Jtiles_tile != T) {      // coupling records for this tile edge
             if (!h->d_Jtiles) {
-                h->d_Jtiles = dev_alloc(coupling_record_bytes(h));
+                h->d_Jtiles = dev_alloc(use_3d ? coupling_record3d_bytes(h) : coupling_record_bytes(h));
                 if (!h->d_Jtiles) rc = ISING_ENOMEM;
             }
-            if (!rc) rc = launch_convert_couplings(h, T, h->d_Jtiles);
+            if (!rc) rc = use_3d ? launch_convert_couplings3d(h, h->d_Jtiles) : launch_convert_couplings(h, T, h->d_Jtiles);
             if (!rc) h->Jtiles_tile = T;
         }
         // run-time specialisation pays for its ~1 s of compilation only on big calls (AUTO: >= 2^27 attempted flips)

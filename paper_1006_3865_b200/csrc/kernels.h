@@ -43,6 +43,8 @@ size_t tile3d_bytes(const ising_ctx* h, bool bits);
 int launch_canon_to_3d(ising_ctx* h, bool bits, const int8_t* d_canon, void* d_tiles);
 int launch_3d_to_canon(ising_ctx* h, bool bits, const void* d_tiles, int8_t* d_canon);
 int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64_t t_first, bool use_jit);
+size_t coupling_record3d_bytes(const ising_ctx* h);
+int launch_convert_couplings3d(ising_ctx* h, void* d_jrec);
 bool resident3d_supported(const ising_ctx* h, int T);            // L <= 64: the whole call in one cluster launch
 int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first);
 

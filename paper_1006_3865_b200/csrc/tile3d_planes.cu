@@ -63,10 +63,46 @@ __global__ void k_convert3d(int8_t* __restrict__ canon, uint8_t* __restrict__ ti
     if (lz == 7) atomicOr(reinterpret_cast<uint32_t*>(f + kZR) + cc, 1u << j);
 }
 
+// Couplings, canonical J[d][i] (bond i -> i + e_d) -> coupling records (zeroed first).  One thread per site: it owns
+// the six bonds seen from that site, in the order of the neighbour words of half_sweep3 (Zm, Zp, Ym, Yp, O, X2).
+__global__ void k_convert_couplings3d(const int8_t* __restrict__ J, uint32_t* __restrict__ jrec, int L) {
+    const uint64_t N = (uint64_t)L * L * L;
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const int x = (int)(i % L), y = (int)((i / L) % L), z = (int)(i / ((uint64_t)L * L));
+    const int B = L / kT3;
+    const int tx = x >> 3, ty = y >> 3, tz = z >> 3, lx = x & 7, ly = y & 7, lz = z & 7;
+    const int cc = (lx + ly + lz) & 1, px = lx >> 1, j = 4 * ly + px;
+    const uint64_t ixm = i - x + (x == 0 ? L - 1 : x - 1);
+    const uint64_t iym = y == 0 ? i + (uint64_t)L * (L - 1) : i - L;
+    const uint64_t izm = z == 0 ? i + (uint64_t)L * L * (L - 1) : i - (uint64_t)L * L;
+    const bool xp = J[i] < 0, xm = J[ixm] < 0, yp = J[N + i] < 0, ym = J[N + iym] < 0, zp = J[2 * N + i] < 0, zm = J[2 * N + izm] < 0;
+    const bool left = (lx & 1) == 0;              // the other site of the aligned pair is x + 1 for a left site
+    const bool b[6] = {zm, zp, ym, yp, left ? xp : xm, left ? xm : xp};
+    uint32_t* w = jrec + ((((size_t)tz * B + ty) * B + tx) * 32 + (size_t)(cc * 8 + lz) * 2) * 4;
+#pragma unroll
+    for (int n = 0; n < 6; ++n)
+        if (b[n]) atomicOr(w + n, 1u << j);
+}
+
 }  // namespace
 
+size_t coupling_record3d_bytes(const ising_ctx* h) {
+    const size_t B = (size_t)(h->L / kT3);
+    return B * B * B * 32 * sizeof(uint4);
+}
+
+int launch_convert_couplings3d(ising_ctx* h, void* d_jrec) {
+    cudaStream_t st = hooks().stream;
+    ISING_CUDA_OK(cudaMemsetAsync(d_jrec, 0, coupling_record3d_bytes(h), st));
+    k_convert_couplings3d<<<(unsigned)((h->N + 255) / 256), 256, 0, st>>>(h->d_J, (uint32_t*)d_jrec, h->L);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
 bool tile3d_supported(const ising_ctx* h, int T) {
-    if (h->dim != 3 || h->has_J || T != kT3 || h->L % kT3) return false;
+    if (h->dim != 3 || h->J_per_replica || T != kT3 || h->L % kT3) return false;
     const int B = h->L / kT3;
     return B >= 2 && (B % 2 == 0);
 }
@@ -114,12 +150,13 @@ int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64
         A.tail[m] = acc.thr[m] & ((1u << kTailBits) - 1u);
     }
     A.force = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
+    A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
     const int warps = kThreads3 / 32;
     const uint32_t grid = (A.njobs + warps - 1) / warps;
     // specialised on the three threshold heads (planes_jit.cu) when asked for and available
     const unsigned long long hp3 = ((unsigned long long)(acc.thr[0] >> kTailBits) << 24) |
                                    ((unsigned long long)(acc.thr[1] >> kTailBits) << 12) | (unsigned long long)(acc.thr[2] >> kTailBits);
-    cudaKernel_t spec = (use_jit && !A.force) ? planes3d_jit_kernel(bits, hp3) : nullptr;
+    cudaKernel_t spec = (use_jit && !A.force && !A.jrec) ? planes3d_jit_kernel(bits, hp3) : nullptr;
     h->last_jit = spec ? 1 : 0;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid); cfg.blockDim = dim3(warps * 32); cfg.stream = hooks().stream;
@@ -133,6 +170,9 @@ int launch_tile3d_pass(ising_ctx* h, const Accept& acc, bool bits, int k, uint64
         if (spec) {
             void* args[] = {&A};
             ISING_CUDA_OK(cudaLaunchKernelExC(&cfg, (const void*)spec, args));
+        } else if (A.jrec) {
+            if (bits) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_planes<true, kNoSpec3, true>, A));
+            else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_planes<false, kNoSpec3, true>, A));
         } else if (bits) {
             ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_planes<true>, A));
         } else {
@@ -156,7 +196,7 @@ struct Res3Args {
     uint32_t jobs_per_colour;      // per replica, 4 tiles per job
 };
 
-template <bool BITS>
+template <bool BITS, bool HASJ>
 __global__ void __launch_bounds__(kRes3Warps * 32) k_resident3d(Res3Args R) {
     namespace cg = cooperative_groups;
     cg::cluster_group cluster = cg::this_cluster();
@@ -221,6 +261,7 @@ __global__ void __launch_bounds__(kRes3Warps * 32) k_resident3d(Res3Args R) {
             t[C] = tile_of(C, wg);
             nb[C] = neighbours(t[C]);
             load_slice<BITS>(A, t[C], lz, s[C]);
+            load_couplings<HASJ>(A, t[C], lz, s[C]);
             publish(C, s[C]);
         }
     cluster.sync();
@@ -237,8 +278,8 @@ __global__ void __launch_bounds__(kRes3Warps * 32) k_resident3d(Res3Args R) {
                 const uint32_t p_base = (uint32_t)(t[C].tx * 4) + (uint32_t)(A.L >> 1) * ((uint32_t)(t[C].ty * kT3) + (uint32_t)A.L * z);
                 for (int j = 0; j < A.k; ++j) {
                     const uint64_t tt = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
-                    half_sweep3<kNoSpec3>(A, s[C], 0, lz, g, p_base, 2 * tt, k0, k1);
-                    half_sweep3<kNoSpec3>(A, s[C], 1, lz, g, p_base, 2 * tt + 1, k0, k1);
+                    half_sweep3<kNoSpec3, HASJ>(A, s[C], 0, lz, g, p_base, 2 * tt, k0, k1);
+                    half_sweep3<kNoSpec3, HASJ>(A, s[C], 1, lz, g, p_base, 2 * tt + 1, k0, k1);
                 }
                 publish(C, s[C]);
             }
@@ -268,6 +309,7 @@ int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, 
         A.tail[m] = acc.thr[m] & ((1u << kTailBits) - 1u);
     }
     A.force = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
+    A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
     R.n = n;
     const uint32_t B = (uint32_t)A.B;
     R.jobs_per_colour = B * B * B / 2u / 4u;
@@ -280,13 +322,14 @@ int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, 
     attr[0].id = cudaLaunchAttributeClusterDimension;
     attr[0].val.clusterDim.x = cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    if (bits) {
-        if (cl > 8) ISING_CUDA_OK(cudaFuncSetAttribute(k_resident3d<true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_resident3d<true>, R));
-    } else {
-        if (cl > 8) ISING_CUDA_OK(cudaFuncSetAttribute(k_resident3d<false>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
-        ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_resident3d<false>, R));
-    }
+    auto go = [&](auto kernel) -> int {
+        if (cl > 8) ISING_CUDA_OK(cudaFuncSetAttribute(kernel, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+        ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, kernel, R));
+        return 0;
+    };
+    const int rc = A.jrec ? (bits ? go(k_resident3d<true, true>) : go(k_resident3d<false, true>))
+                          : (bits ? go(k_resident3d<true, false>) : go(k_resident3d<false, false>));
+    if (rc) return rc;
     count_launch();
     ISING_CUDA_OK(cudaGetLastError());
     return 0;

@@ -32,6 +32,9 @@ struct Plane3Args {
     uint32_t u[3][kHeadBits];    // plane q: all-ones if bit (31-q) of thr[m+1] is set
     uint32_t tail[3];            // thr[m+1] & (2^20 - 1)
     uint32_t force;              // all-ones if beta = 0 (every thr = 2^32: every proposal is accepted)
+    const uint4* jrec;           // coupling records (a9) or nullptr: per tile 2 x 8 x 2 uint4, (cc, lz) -> {Zm, Zp, Ym, Yp},
+                                 // {X1, X2, 0, 0}: bit j set <=> the bond from site j of that word to its neighbour in the
+                                 // Zm / Zp / Ym / Yp / O / X2 word of half_sweep3 is J = -1.  Shared by the replicas.
 };
 
 struct Tile3 {
@@ -58,7 +61,19 @@ struct Slice {
     uint32_t xl, xr;      // halo bits x = -1 (at 4ly) and x = 8 (at 4ly+3), every row, either colour
     uint32_t ym, yp;      // halo row y = -1 and y = 8: colour 0 pairs in bits 0-3, colour 1 in bits 4-7
     uint32_t zm[2], zp[2];// lanes lz = 0 / 7: the slice below / above, by colour
+    uint32_t J[2][6];     // coupling words of the slice's two colours (kernels with HASJ only)
 };
+
+template <bool HASJ>
+__device__ __forceinline__ void load_couplings(const Plane3Args& A, const Tile3& t, int lz, Slice& s) {
+    if (!HASJ) return;
+    const uint4* rec = A.jrec + (((size_t)t.tz * A.B + t.ty) * A.B + t.tx) * 32;
+#pragma unroll
+    for (int cc = 0; cc < 2; ++cc) {
+        const uint4 a = __ldg(rec + (cc * 8 + lz) * 2), b = __ldg(rec + (cc * 8 + lz) * 2 + 1);
+        s.J[cc][0] = a.x; s.J[cc][1] = a.y; s.J[cc][2] = a.z; s.J[cc][3] = a.w; s.J[cc][4] = b.x; s.J[cc][5] = b.y;
+    }
+}
 
 template <bool BITS>
 __device__ __forceinline__ void load_slice(const Plane3Args& A, const Tile3& t, int lz, Slice& s) {
@@ -196,7 +211,7 @@ __device__ __forceinline__ void head_masks3_sel(uint32_t g, uint32_t Hlo, uint32
 }
 
 // One half-sweep of colour c on the lane's slice (a4-a5, 6 neighbours).
-template <unsigned long long HP3 = kNoSpec3>
+template <unsigned long long HP3 = kNoSpec3, bool HASJ = false>
 __device__ __forceinline__ void half_sweep3(const Plane3Args& A, Slice& s, int c, int lz, uint32_t g, uint32_t p_base,
                                             uint64_t H, uint32_t k0, uint32_t k1) {
     const int o = 1 - c;
@@ -212,7 +227,10 @@ __device__ __forceinline__ void half_sweep3(const Plane3Args& A, Slice& s, int c
     const uint32_t m = ((lz + c) & 1) ? 0xf0f0f0f0u : 0x0f0f0f0fu;
     const uint32_t X2 = ((((O << 1) & 0xeeeeeeeeu) | s.xl) & m) | ((((O >> 1) & 0x77777777u) | s.xr) & ~m);
     // disagreeing neighbours, pairwise counts, then thresholds of the sum of six
-    const uint32_t a = S ^ Zm, b = S ^ Zp, e = S ^ Ym, f = S ^ Yp, x = S ^ O, y = S ^ X2;
+    // unsatisfied bonds: J s_i s_j = -1  <=>  s_i != s_j for J = +1, s_i == s_j for J = -1 (eq. (1))
+    const uint32_t a = S ^ Zm ^ (HASJ ? s.J[c][0] : 0u), b = S ^ Zp ^ (HASJ ? s.J[c][1] : 0u);
+    const uint32_t e = S ^ Ym ^ (HASJ ? s.J[c][2] : 0u), f = S ^ Yp ^ (HASJ ? s.J[c][3] : 0u);
+    const uint32_t x = S ^ O ^ (HASJ ? s.J[c][4] : 0u), y = S ^ X2 ^ (HASJ ? s.J[c][5] : 0u);
     const uint32_t p1 = a | b, q1 = a & b, p2 = e | f, q2 = e & f, p3 = x | y, q3 = x & y;
     const uint32_t ge1 = p1 | p2 | p3;
     const uint32_t ge2 = q1 | q2 | q3 | (p1 & p2) | (p1 & p3) | (p2 & p3);
@@ -252,7 +270,7 @@ __device__ __forceinline__ void half_sweep3(const Plane3Args& A, Slice& s, int c
 
 constexpr int kThreads3 = 64;        // 2 warps = 8 tiles per CTA: small CTAs so that config 4 (4096 warp jobs) fits one wave
 
-template <bool BITS, unsigned long long HP3 = kNoSpec3>
+template <bool BITS, unsigned long long HP3 = kNoSpec3, bool HASJ = false>
 __global__ void __launch_bounds__(kThreads3) k_tile3d_planes(Plane3Args A) {
     const uint2* lut = kByteLutGlobal.e;      // int8 write-back table, read-only path (planes_common.cuh)
     // Programmatic dependent launch, as in k_tile_planes: the next colour's grid may be scheduled while this one
@@ -266,6 +284,7 @@ __global__ void __launch_bounds__(kThreads3) k_tile3d_planes(Plane3Args A) {
     const Tile3 t = job_tile3(A, job * 4u + (uint32_t)sub);
     Slice s;
     load_slice<BITS>(A, t, lz, s);
+    load_couplings<HASJ>(A, t, lz, s);
     const uint64_t seed = A.seeds[t.r];
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     const uint32_t z = (uint32_t)(t.tz * kT3 + lz);
@@ -273,8 +292,8 @@ __global__ void __launch_bounds__(kThreads3) k_tile3d_planes(Plane3Args A) {
     const uint32_t p_base = (uint32_t)(t.tx * 4) + (uint32_t)(A.L >> 1) * ((uint32_t)(t.ty * kT3) + (uint32_t)A.L * z);
     for (int j = 0; j < A.k; ++j) {
         const uint64_t tt = A.t_first + (uint64_t)j;
-        half_sweep3<HP3>(A, s, 0, lz, g, p_base, 2 * tt, k0, k1);
-        half_sweep3<HP3>(A, s, 1, lz, g, p_base, 2 * tt + 1, k0, k1);
+        half_sweep3<HP3, HASJ>(A, s, 0, lz, g, p_base, 2 * tt, k0, k1);
+        half_sweep3<HP3, HASJ>(A, s, 1, lz, g, p_base, 2 * tt + 1, k0, k1);
     }
     store_slice<BITS>(A, t, lz, s, lut);
 }

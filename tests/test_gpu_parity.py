@@ -502,3 +502,30 @@ def test_cluster_resident_kernel_with_couplings(P, orc, L, tile, k, n, beta, see
     for a in range(len(seeds)):
         for b in range(a + 1, len(seeds)):
             assert g.overlap(a, b) == o.overlap(a, b)
+
+
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,k,n,beta,seeds,jseed", [
+    (16, 2, 3, 0.9, [1], 3),                 # B = 2
+    (32, 1, 3, 1.1, [4, 5, 6], 7),           # 3D Edwards-Anderson glass, replicas share J
+    (48, 3, 2, 0.5, [8], 9),
+    (96, 1, 2, 0.9, [2], 10),                # B = 12: too large for the resident kernel
+    (32, 2, 2, 0.0, [2], 11),
+])
+def test_tile3d_couplings_match_oracle(P, orc, L, k, n, beta, seeds, jseed, layout):
+    """a9 in 3D: quenched +-J bonds as bit records (six words per slice and colour), per-pass and cluster-resident kernels."""
+    J = W.couplings(3, L, jseed)
+    g, o = _both(P, orc, 3, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    Eg, Mg = g.sweep_series(beta, n, 8, k)          # series: a launch per colour
+    assert g.sweep_path() == f"tile3d_planes_{'i8' if layout == 'int8' else 'bits'}"
+    Eo, Mo = o.sweep_series(beta, n, 8, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    g.sweep(beta, n, 8, k); o.sweep(beta, n, 8, k)
+    assert g.sweep_path().startswith("resident3d_planes" if L <= 64 else "tile3d_planes")
+    _same_state(g, o)
+    for a in range(len(seeds)):
+        for b in range(a + 1, len(seeds)):
+            assert g.overlap(a, b) == o.overlap(a, b)
