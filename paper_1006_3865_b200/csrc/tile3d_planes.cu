@@ -1,5 +1,5 @@
 // tile3d_planes.cu — the 3D double-checkerboard tile kernel (8x8x8 tiles, "completely
-// analogous"; BASELINE config 4) in multi-spin form, RNG mapping "planes" (DESIGN.md §3.4, §6.4).
+// analogous"; BASELINE config 4) in multi-spin form, RNG mapping "planes" (DESIGN.md §3.4, §6.1b, §6.1d).
 //
 // A 32-bit word holds the 32 same-colour sites of one z-slice of a tile = one RNG block of the 3D
 // planes mapping (4 pairs p_x x 8 rows y): bit j = 4*ly + p_x.  A tile is 8 slices x 2 colours =
