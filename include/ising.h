@@ -179,7 +179,7 @@ uint64_t ising_kernel_launches(void);
  * never NULL.  "resident_planes_*": 2D, J = +1 or +-J, at most 64 warp jobs per coarse colour (L <= 512 at tile 32 or 64),
  * n_sweeps >= 2: the whole call runs in one launch of one thread-block cluster per replica with the lattice held
  * in registers and the tile boundaries exchanged through distributed shared memory (same trajectory).
- * "resident3d_planes_*": the same for 3D, J = +1 or +-J, L <= 64 (without E/M series). */
+ * "resident3d_planes_*": the same for 3D, J = +1 or +-J, L <= 64. */
 const char* ising_sweep_path(ising_handle h);
 
 /* ising_force_path — testing aid: 0 = automatic kernel choice, 1 = always the generic

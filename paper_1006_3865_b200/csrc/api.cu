@@ -154,6 +154,8 @@ static int observables_now(ising_ctx* h, long long* d_E, long long* d_M) {
     const bool planes2d = (h->store == Store::PlaneI8 || h->store == Store::PlaneBits) && h->L / h->store_tile >= 2 &&
                           (!h->has_J || h->Jtiles_tile == h->store_tile);
     if (planes2d) return launch_observables_planes(h, h->store_tile, h->store == Store::PlaneBits, d_E, d_M);
+    const bool planes3d = (h->store == Store::Plane3I8 || h->store == Store::Plane3Bits) && (!h->has_J || h->Jtiles_tile == h->store_tile);
+    if (planes3d) return launch_observables3d(h, h->store == Store::Plane3Bits, d_E, d_M);
     int rc = (h->store == Store::Canon) ? 0 : to_canon_scratch(h);
     if (rc) return rc;
     return launch_observables_canon(h, h->d_canon, d_E, d_M);
@@ -387,10 +389,10 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         const bool use_resident = use_planes && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident &&
                                   resident_planes_supported(h, T);
         bool resident_done = false;
-        const bool use_resident3 = use_3d && !want_series && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident &&
+        const bool use_resident3 = use_3d && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident &&
                                    resident3d_supported(h, T);
         if (use_resident3 && !rc) {
-            if (launch_resident3d(h, acc, bits, n, k, h->t) == 0) {
+            if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M) == 0) {
                 h->last_path = bits ? "resident3d_planes_bits" : "resident3d_planes_i8";
                 resident_done = true;
             } else {

@@ -85,7 +85,68 @@ __global__ void k_convert_couplings3d(const int8_t* __restrict__ J, uint32_t* __
         if (b[n]) atomicOr(w + n, 1u << j);
 }
 
+// a10 directly on the 3D tile records: one launch per coarse colour C adds the colour-C tiles' share to E[r], M[r]
+// (zeroed by the caller); the four tiles of a warp job belong to one replica (B^3/2 is a multiple of 4).
+template <bool BITS, bool HASJ>
+__global__ void __launch_bounds__(kThreads3) k_observables3d(Plane3Args A, long long* __restrict__ E, long long* __restrict__ M) {
+    const int lane = threadIdx.x & 31;
+    const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (job >= A.njobs) return;
+    const int sub = lane >> 3, lz = lane & 7;
+    const Tile3 t = job_tile3(A, job * 4u + (uint32_t)sub);
+    Slice s;
+    load_slice<BITS>(A, t, lz, s);
+    load_couplings<HASJ>(A, t, lz, s);
+    int up = 0, unsat = 0;
+    count_slice<HASJ>(s, lz, up, unsat);
+#pragma unroll
+    for (int d = 16; d > 0; d >>= 1) {
+        up += __shfl_xor_sync(0xffffffffu, up, d);
+        unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+    }
+    if (lane == 0) {
+        const long long sites = 4ll * kT3 * kT3 * kT3;
+        if (M) atomicAdd(reinterpret_cast<unsigned long long*>(M + t.r), (unsigned long long)(2ll * up - sites));
+        if (E) atomicAdd(reinterpret_cast<unsigned long long*>(E + t.r), (unsigned long long)(2ll * unsat - 3ll * sites));
+    }
+}
+
 }  // namespace
+
+static void fill_geometry3(Plane3Args& A, const ising_ctx* h) {
+    A.tiles = (uint8_t*)h->d_tiles;
+    A.seeds = h->d_sweep_seeds;
+    A.L = h->L; A.B = h->L / kT3; A.R = h->R;
+    const uint32_t B = (uint32_t)A.B;
+    A.per_rep = B * B * B / 2u; A.per_z = B * B / 2u; A.hb = B / 2u;
+    A.magic_rep = fastdiv_magic(A.per_rep); A.magic_z = fastdiv_magic(A.per_z); A.magic_hb = fastdiv_magic(A.hb);
+    A.njobs = (uint32_t)((size_t)h->R * A.per_rep / 4u);
+    A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
+}
+
+// a10 on 3D tile records: E[r], M[r] (R values each, either may be null).
+int launch_observables3d(ising_ctx* h, bool bits, long long* d_E, long long* d_M) {
+    cudaStream_t st = hooks().stream;
+    if (d_E) ISING_CUDA_OK(cudaMemsetAsync(d_E, 0, sizeof(long long) * h->R, st));
+    if (d_M) ISING_CUDA_OK(cudaMemsetAsync(d_M, 0, sizeof(long long) * h->R, st));
+    Plane3Args A = {};
+    fill_geometry3(A, h);
+    const int warps = kThreads3 / 32;
+    const uint32_t grid = (A.njobs + warps - 1) / warps;
+    for (int C = 0; C < 2; ++C) {
+        A.C = C;
+        if (A.jrec) {
+            if (bits) k_observables3d<true, true><<<grid, warps * 32, 0, st>>>(A, d_E, d_M);
+            else k_observables3d<false, true><<<grid, warps * 32, 0, st>>>(A, d_E, d_M);
+        } else {
+            if (bits) k_observables3d<true, false><<<grid, warps * 32, 0, st>>>(A, d_E, d_M);
+            else k_observables3d<false, false><<<grid, warps * 32, 0, st>>>(A, d_E, d_M);
+        }
+        count_launch();
+    }
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
 
 size_t coupling_record3d_bytes(const ising_ctx* h) {
     const size_t B = (size_t)(h->L / kT3);
@@ -194,6 +255,8 @@ struct Res3Args {
     Plane3Args P;
     int n;
     uint32_t jobs_per_colour;      // per replica, 4 tiles per job
+    long long* E;                  // optional series (a10 after every pass): E[pass * R + r], M[pass * R + r]
+    long long* M;
 };
 
 template <bool BITS, bool HASJ>
@@ -209,6 +272,19 @@ __global__ void __launch_bounds__(kRes3Warps * 32) k_resident3d(Res3Args R) {
     const uint32_t B = (uint32_t)A.B, hb = B >> 1, JC = R.jobs_per_colour;
     const uint2* lut = kByteLutGlobal.e;
     __shared__ __align__(16) uint8_t faces[2][kRes3Warps][4][kFaces3];
+    __shared__ int acc[2][2];          // rank 0 only: {#up, #unsatisfied bonds} of the replica, for even / odd passes
+    if (threadIdx.x < 4) (&acc[0][0])[threadIdx.x] = 0;
+    int* const acc0 = cluster.map_shared_rank(&acc[0][0], 0);
+    const bool series = R.E != nullptr || R.M != nullptr;
+    const long long nsites = (long long)A.L * A.L * A.L;
+    auto write_series = [&](int pass) {                                // one thread of the cluster, a barrier after the atomics
+        if (rank == 0 && threadIdx.x == 0) {
+            int* a = &acc[pass & 1][0];
+            if (R.M) R.M[(size_t)pass * A.R + r] = 2ll * a[0] - nsites;
+            if (R.E) R.E[(size_t)pass * A.R + r] = 2ll * a[1] - 3ll * nsites;
+            a[0] = 0; a[1] = 0;
+        }
+    };
 
     auto tile_of = [&](int C, uint32_t job) {
         uint32_t q = job * 4u + (uint32_t)sub;                        // colour-C tiles of the replica, (tz, ty, tx/2) row-major
@@ -271,6 +347,7 @@ __global__ void __launch_bounds__(kRes3Warps * 32) k_resident3d(Res3Args R) {
     for (int pass = 0; pass < R.n; ++pass) {
 #pragma unroll
         for (int C = 0; C < 2; ++C) {
+            if (series && C == 1 && pass > 0) write_series(pass - 1);    // complete since the barrier just passed
             if (mine) {
                 refresh(nb[C], s[C]);
                 const uint32_t z = (uint32_t)(t[C].tz * kT3 + lz);
@@ -285,10 +362,32 @@ __global__ void __launch_bounds__(kRes3Warps * 32) k_resident3d(Res3Args R) {
             }
             cluster.sync();
         }
+        if (series) {                       // as in k_resident_planes: count on the registers, sums to rank 0
+            int up = 0, unsat = 0;
+            if (mine) {
+                refresh(nb[0], s[0]);       // the colour-0 tiles' halos are one phase old
+                count_slice<HASJ>(s[0], lz, up, unsat);
+                count_slice<HASJ>(s[1], lz, up, unsat);
+            }
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                up += __shfl_xor_sync(0xffffffffu, up, d);
+                unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+            }
+            if (lane == 0 && mine) {
+                atomicAdd(acc0 + 2 * (pass & 1), up);
+                atomicAdd(acc0 + 2 * (pass & 1) + 1, unsat);
+            }
+        }
+    }
+    if (series && R.n > 0) {
+        cluster.sync();
+        write_series(R.n - 1);
     }
 #pragma unroll
     for (int C = 0; C < 2; ++C)
         if (mine) store_slice<BITS>(A, t[C], lz, s[C], lut);
+    cluster.sync();            // no CTA leaves while its shared memory may still be read or added to
 }
 
 bool resident3d_supported(const ising_ctx* h, int T) {
@@ -297,8 +396,9 @@ bool resident3d_supported(const ising_ctx* h, int T) {
     return B * B * B / 2u / 4u <= (uint32_t)(kRes3MaxCluster * kRes3Warps) && (B * B * B / 2u) % 4u == 0;
 }
 
-int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first) {
+int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M) {
     Res3Args R;
+    R.E = d_E; R.M = d_M;
     Plane3Args& A = R.P;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;

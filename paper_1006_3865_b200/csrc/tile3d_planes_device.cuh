@@ -210,22 +210,44 @@ __device__ __forceinline__ void head_masks3_sel(uint32_t g, uint32_t Hlo, uint32
     R = bw; eq = ~ne;
 }
 
+// The six neighbour words of the lane's slice for the sites of colour c (o = 1 - c is read): z-1 / z+1 by shuffle (halo
+// words at the tile faces), y-1 / y+1 by 4-bit shifts, the other site of the aligned pair (O) and the pair-shifted word (X2).
+__device__ __forceinline__ void neighbour_words3(const Slice& s, int c, int lz, uint32_t& Zm, uint32_t& Zp, uint32_t& Ym,
+                                                 uint32_t& Yp, uint32_t& O, uint32_t& X2) {
+    const int o = 1 - c;
+    O = s.S[o];
+    Zm = __shfl_up_sync(0xffffffffu, O, 1);
+    Zp = __shfl_down_sync(0xffffffffu, O, 1);
+    if (lz == 0) Zm = s.zm[o];
+    if (lz == 7) Zp = s.zp[o];
+    Ym = (O << 4) | ((s.ym >> (4 * o)) & 0xfu);
+    Yp = (O >> 4) | (((s.yp >> (4 * o)) & 0xfu) << 28);
+    // rows where the active site is the left one of its pair (x = 2 p_x): ly = lz + c (mod 2); their second
+    // x-neighbour is pair p_x - 1, the other rows' is pair p_x + 1
+    const uint32_t m = ((lz + c) & 1) ? 0xf0f0f0f0u : 0x0f0f0f0fu;
+    X2 = ((((O << 1) & 0xeeeeeeeeu) | s.xl) & m) | ((((O >> 1) & 0x77777777u) | s.xr) & ~m);
+}
+
+// a10 on a slice held in registers: #up spins of both colours and #unsatisfied bonds seen from the colour-0 sites (every
+// bond of the lattice has exactly one colour-0 end).  M = 2 #up - N, E = 2 #unsat - 3N.
+template <bool HASJ>
+__device__ __forceinline__ void count_slice(const Slice& s, int lz, int& up, int& unsat) {
+    uint32_t Zm, Zp, Ym, Yp, O, X2;
+    neighbour_words3(s, 0, lz, Zm, Zp, Ym, Yp, O, X2);
+    const uint32_t S = s.S[0];
+    unsat += __popc(S ^ Zm ^ (HASJ ? s.J[0][0] : 0u)) + __popc(S ^ Zp ^ (HASJ ? s.J[0][1] : 0u)) + __popc(S ^ Ym ^ (HASJ ? s.J[0][2] : 0u)) +
+             __popc(S ^ Yp ^ (HASJ ? s.J[0][3] : 0u)) + __popc(S ^ O ^ (HASJ ? s.J[0][4] : 0u)) + __popc(S ^ X2 ^ (HASJ ? s.J[0][5] : 0u));
+    up += __popc(s.S[0]) + __popc(s.S[1]);
+}
+
 // One half-sweep of colour c on the lane's slice (a4-a5, 6 neighbours).
 template <unsigned long long HP3 = kNoSpec3, bool HASJ = false>
 __device__ __forceinline__ void half_sweep3(const Plane3Args& A, Slice& s, int c, int lz, uint32_t g, uint32_t p_base,
                                             uint64_t H, uint32_t k0, uint32_t k1) {
-    const int o = 1 - c;
     const uint32_t Hlo = (uint32_t)H, Hhi = (uint32_t)(H >> 32);
-    const uint32_t O = s.S[o], S = s.S[c];
-    uint32_t Zm = __shfl_up_sync(0xffffffffu, O, 1), Zp = __shfl_down_sync(0xffffffffu, O, 1);
-    if (lz == 0) Zm = s.zm[o];
-    if (lz == 7) Zp = s.zp[o];
-    const uint32_t Ym = (O << 4) | ((s.ym >> (4 * o)) & 0xfu);
-    const uint32_t Yp = (O >> 4) | (((s.yp >> (4 * o)) & 0xfu) << 28);
-    // rows where the active site is the left one of its pair (x = 2 p_x): ly = lz + c (mod 2); their second
-    // x-neighbour is pair p_x - 1, the other rows' is pair p_x + 1
-    const uint32_t m = ((lz + c) & 1) ? 0xf0f0f0f0u : 0x0f0f0f0fu;
-    const uint32_t X2 = ((((O << 1) & 0xeeeeeeeeu) | s.xl) & m) | ((((O >> 1) & 0x77777777u) | s.xr) & ~m);
+    const uint32_t S = s.S[c];
+    uint32_t Zm, Zp, Ym, Yp, O, X2;
+    neighbour_words3(s, c, lz, Zm, Zp, Ym, Yp, O, X2);
     // disagreeing neighbours, pairwise counts, then thresholds of the sum of six
     // unsatisfied bonds: J s_i s_j = -1  <=>  s_i != s_j for J = +1, s_i == s_j for J = -1 (eq. (1))
     const uint32_t a = S ^ Zm ^ (HASJ ? s.J[c][0] : 0u), b = S ^ Zp ^ (HASJ ? s.J[c][1] : 0u);

@@ -158,6 +158,7 @@ def test_tile3d_path_matches_oracle(P, orc, L, k, n, beta, seeds, layout):
     g, o = _both(P, orc, 3, L, seeds, rng="planes")
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
+    g.force_path(2)            # a launch per colour; E and M by k_observables3d on the records
     Eg, Mg = g.sweep_series(beta, n, 8, k)
     assert g.sweep_path() == f"tile3d_planes_{'i8' if layout == 'int8' else 'bits'}"
     Eo, Mo = o.sweep_series(beta, n, 8, k)
@@ -468,6 +469,10 @@ def test_cluster_resident_3d_kernel_matches_oracle(P, orc, L, k, n, beta, seeds,
     g.sweep(beta, n, 8, k); o.sweep(beta, n, 8, k)
     assert g.sweep_path() == f"resident3d_planes_{'i8' if layout == 'int8' else 'bits'}"
     _same_state(g, o)
+    Eg, Mg = g.sweep_series(beta, n, 8, k)          # E and M after every pass, counted on the registers
+    assert g.sweep_path().startswith("resident3d_planes")
+    Eo, Mo = o.sweep_series(beta, n, 8, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
     g.sweep(beta, 1, 8, k); o.sweep(beta, 1, 8, k)
     assert g.sweep_path().startswith("tile3d_planes")
     g.sweep(beta, 2, 8, k); o.sweep(beta, 2, 8, k)
@@ -518,13 +523,19 @@ def test_tile3d_couplings_match_oracle(P, orc, L, k, n, beta, seeds, jseed, layo
     g, o = _both(P, orc, 3, L, seeds, J, rng="planes")
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
-    Eg, Mg = g.sweep_series(beta, n, 8, k)          # series: a launch per colour
+    g.force_path(2)
+    Eg, Mg = g.sweep_series(beta, n, 8, k)          # a launch per colour, E and M on the records
     assert g.sweep_path() == f"tile3d_planes_{'i8' if layout == 'int8' else 'bits'}"
     Eo, Mo = o.sweep_series(beta, n, 8, k)
     assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
     _same_state(g, o)
+    g.force_path(0)
     g.sweep(beta, n, 8, k); o.sweep(beta, n, 8, k)
     assert g.sweep_path().startswith("resident3d_planes" if L <= 64 else "tile3d_planes")
+    _same_state(g, o)
+    Eg, Mg = g.sweep_series(beta, n, 8, k)          # L <= 64: measured on the registers of the resident kernel
+    Eo, Mo = o.sweep_series(beta, n, 8, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
     _same_state(g, o)
     for a in range(len(seeds)):
         for b in range(a + 1, len(seeds)):
