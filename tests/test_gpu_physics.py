@@ -97,3 +97,24 @@ def test_heisenberg_high_temperature_series_3d(P):
     lang = 1 / math.tanh(beta) - 1 / beta
     assert abs(mean + (lang + 4 * lang ** 3)) < 4 * err + 2e-4, (mean, lang + 4 * lang ** 3, err)
     assert err < 1e-4
+
+
+def test_3d_equilibrium_is_the_same_for_both_schedules(P):
+    """3D Ising L = 16 at the critical coupling: the double checkerboard with 8^3 tiles (cluster-resident kernel, E counted
+    on the registers) and the plain checkerboard (tile = L, generic kernels) are different chains with the same
+    equilibrium; no exact finite-lattice value exists in 3D, so the two are compared with each other."""
+    import torch
+    L, beta = 16, W.BETA_C_3D
+    means = []
+    for tile, k, n, path in ((8, 1, 200000, "resident3d_planes_i8"), (8, 2, 100000, "resident3d_planes_i8"), (16, 1, 60000, "generic")):
+        g = P.Ising(3, L, seed=31 + tile + k)
+        g.sweep(beta, 3000, tile, k)
+        E = torch.zeros(n, dtype=torch.int64, device="cuda")
+        M = torch.zeros(n, dtype=torch.int64, device="cuda")
+        g.sweep_series(beta, n, tile, k, E=E, M=M)
+        assert g.sweep_path() == path
+        means.append(binned(E.cpu().numpy().astype(np.float64) / L ** 3, nbins=40))
+    (m0, e0), (m1, e1), (m2, e2) = means
+    assert abs(m0 - m2) < 4 * math.hypot(e0, e2), means
+    assert abs(m1 - m2) < 4 * math.hypot(e1, e2), means
+    assert max(e0, e1, e2) < 4e-3 and -1.1 < m0 < -0.9          # u_c = -0.99 in the infinite lattice
