@@ -46,6 +46,11 @@ int heis_sweep(heis_handle h, double beta, int n_sweeps, int tile, int k_inner);
  * either may be NULL.  Synchronises. */
 int heis_observables(heis_handle h, double* E, double* M);
 
+/* heis_sweep with E and M after every outer pass: E[n_sweeps] and M[3 * n_sweeps] (pass-major: Mx, My, Mz of pass p
+ * at M + 3p), caller-owned, host or device, either may be NULL.  Nothing is copied or synchronised between the passes
+ * (the sums are accumulated on the device); synchronises at the end. */
+int heis_sweep_series(heis_handle h, double beta, int n_sweeps, int tile, int k_inner, double* E, double* M);
+
 /* dst / src: 3*N floats, component-major (x plane, y plane, z plane), host or device.  Synchronise.
  * heis_set_spins does not normalise or check the lengths. */
 int heis_copy_spins(heis_handle h, float* dst);

@@ -29,7 +29,7 @@ SYMBOLS = [
     "ising_last_error",
 ]
 HEIS_SYMBOLS = [     # include/heisenberg.h
-    "heis_create", "heis_destroy", "heis_sweep", "heis_observables", "heis_copy_spins", "heis_set_spins",
+    "heis_create", "heis_destroy", "heis_sweep", "heis_sweep_series", "heis_observables", "heis_copy_spins", "heis_set_spins",
     "heis_get_counter", "heis_set_counter", "heis_sweep_path", "heis_force_generic",
 ]
 
@@ -91,6 +91,7 @@ def lib() -> C.CDLL:
     L.heis_destroy.argtypes = [vp]
     L.heis_sweep.argtypes = [vp, C.c_double, C.c_int, C.c_int, C.c_int]
     L.heis_observables.argtypes = [vp, vp, vp]
+    L.heis_sweep_series.argtypes = [vp, C.c_double, C.c_int, C.c_int, C.c_int, vp, vp]
     L.heis_copy_spins.argtypes = [vp, vp]
     L.heis_set_spins.argtypes = [vp, vp]
     L.heis_get_counter.argtypes = [vp, u64p]
@@ -282,6 +283,15 @@ class Heisenberg:
 
     def sweep(self, beta: float, n_sweeps: int, tile: int = 0, k_inner: int = 1) -> None:
         _check(lib().heis_sweep(self._h, float(beta), int(n_sweeps), int(tile), int(k_inner)))
+
+    def sweep_series(self, beta: float, n_sweeps: int, tile: int = 0, k_inner: int = 1, E=None, M=None):
+        """E (n_sweeps) and M (n_sweeps, 3) after every pass; optional caller buffers (numpy or torch float64)."""
+        if E is None:
+            E = np.zeros(n_sweeps, dtype=np.float64)
+        if M is None:
+            M = np.zeros((n_sweeps, 3), dtype=np.float64)
+        _check(lib().heis_sweep_series(self._h, float(beta), int(n_sweeps), int(tile), int(k_inner), _ptr(E), _ptr(M)))
+        return E, M
 
     def observables(self):
         E = np.zeros(1, dtype=np.float64)

@@ -529,7 +529,7 @@ void heis_destroy(heis_handle h) {
     delete h;
 }
 
-int heis_sweep(heis_handle h, double beta, int n_sweeps, int tile, int k_inner) {
+static int heis_sweep_impl(heis_handle h, double beta, int n_sweeps, int tile, int k_inner, double* d_series) {
     if (!h) { set_error("heis_sweep: NULL handle"); return ISING_EINVAL; }
     if (!(beta >= 0.0) || !std::isfinite(beta) || n_sweeps < 0 || k_inner < 1) {
         set_error("heis_sweep: need finite beta >= 0, n_sweeps >= 0, k_inner >= 1");
@@ -564,9 +564,37 @@ int heis_sweep(heis_handle h, double beta, int n_sweeps, int tile, int k_inner) 
                     }
             ISING_CUDA_OK(cudaGetLastError());
         }
+        if (d_series) {
+            const unsigned blocks = (unsigned)std::min<uint64_t>((h->N + 255) / 256, 148 * 8);
+            k_heis_observables<<<blocks, 256, 0, hooks().stream>>>(h->d_s, h->N, h->L, h->dim, d_series + (size_t)pass * 4);
+            count_launch();
+        }
     }
     h->t += (uint64_t)n_sweeps * k_inner;
     return 0;
+}
+
+int heis_sweep(heis_handle h, double beta, int n_sweeps, int tile, int k_inner) {
+    return heis_sweep_impl(h, beta, n_sweeps, tile, k_inner, nullptr);
+}
+
+int heis_sweep_series(heis_handle h, double beta, int n_sweeps, int tile, int k_inner, double* E, double* M) {
+    if (!h) { set_error("heis_sweep_series: NULL handle"); return ISING_EINVAL; }
+    if (n_sweeps <= 0 || (!E && !M)) return heis_sweep_impl(h, beta, n_sweeps, tile, k_inner, nullptr);
+    cudaStream_t st = hooks().stream;
+    double* d_series = (double*)dev_alloc((size_t)n_sweeps * 4 * sizeof(double));      // {E, Mx, My, Mz} per pass
+    if (!d_series) return ISING_ENOMEM;
+    int rc = 0;
+    if (cudaMemsetAsync(d_series, 0, (size_t)n_sweeps * 4 * sizeof(double), st) != cudaSuccess) { set_error("heis_sweep_series: memset failed"); rc = ISING_ECUDA; }
+    if (!rc) rc = heis_sweep_impl(h, beta, n_sweeps, tile, k_inner, d_series);
+    if (!rc && E && cudaMemcpy2DAsync(E, sizeof(double), d_series, 4 * sizeof(double), sizeof(double), (size_t)n_sweeps,
+                                      is_device_ptr(E) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = ISING_ECUDA;
+    if (!rc && M && cudaMemcpy2DAsync(M, 3 * sizeof(double), d_series + 1, 4 * sizeof(double), 3 * sizeof(double), (size_t)n_sweeps,
+                                      is_device_ptr(M) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, st) != cudaSuccess) rc = ISING_ECUDA;
+    if (rc == ISING_ECUDA) { set_error("heis_sweep_series: copy of the series failed: %s", cudaGetErrorString(cudaGetLastError())); }
+    cudaStreamSynchronize(st);
+    dev_free(d_series);
+    return rc;
 }
 
 int heis_observables(heis_handle h, double* E, double* M) {

@@ -93,6 +93,25 @@ def test_sweeps_compose_and_counter_resume(P):
     assert np.array_equal(np.asarray(a.copy_spins()), np.asarray(c.copy_spins()))
 
 
+@pytest.mark.parametrize("dim,L,T,k,n", [(2, 64, 32, 2, 5), (3, 16, 8, 1, 4), (2, 24, 12, 1, 3)])
+def test_sweep_series(P, dim, L, T, k, n):
+    """heis_sweep_series: E and M after every pass equal the oracle's observables after the same passes."""
+    import torch
+    g, o = P.Heisenberg(dim, L, seed=13), HO.HeisenbergOracle(dim, L, seed=13)
+    Eg, Mg = g.sweep_series(0.8, n, T, k)
+    tol = 1e-9 * dim * L ** dim
+    for p in range(n):
+        o.sweep(0.8, 1, T, k)
+        Eo, Mo = o.observables()
+        assert abs(Eg[p] - Eo) <= tol and np.all(np.abs(Mg[p] - Mo) <= tol)
+    _same(g, o)
+    Ed = torch.zeros(n, dtype=torch.float64, device="cuda")          # device buffer, E only
+    g.sweep_series(0.8, n, T, k, E=Ed, M=None)
+    o.sweep(0.8, n, T, k)
+    assert abs(float(Ed[-1].item()) - o.observables()[0]) <= tol
+    _same(g, o)
+
+
 def test_set_spins_then_sweep_matches_oracle(P):
     rs = np.random.RandomState(3)
     v = rs.normal(size=(3, 64 * 64)).astype(np.float32)

@@ -88,10 +88,7 @@ def test_heisenberg_high_temperature_series_3d(P):
     g = P.Heisenberg(3, L, seed=9)
     g.sweep(beta, 500, 8, 1)
     assert g.sweep_path() == "heis_tile"
-    Es = []
-    for _ in range(6000):
-        g.sweep(beta, 2, 8, 1)
-        Es.append(g.observables()[0])
+    Es, _ = g.sweep_series(beta, 12000, 8, 1)
     nb = 3 * L ** 3
     mean, err = binned(np.asarray(Es) / nb, nbins=40)
     lang = 1 / math.tanh(beta) - 1 / beta
