@@ -341,7 +341,35 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
     const bool use_plain64 = !h->force_generic && h->rng == ISING_RNG_PLANES && plain64_supported(h, T);
     const bool use_3d = !h->force_generic && h->rng == ISING_RNG_PLANES && tile3d_supported(h, T);
     const bool use_amsc = !h->force_generic && thr_fits_or_zero(acc) && amsc_supported(h, T);
-    if (use_amsc) {                          // f1: 32 realisations per word, one random number per site
+    // a8 beyond L = 64: the plain checkerboard (tile == L) on the cluster-resident kernel; the register tiling Tp is
+    // invisible in the result
+    int Tp = 0;
+    if (!h->force_generic && !h->no_resident && !use_plain64 && !use_amsc && h->rng == ISING_RNG_PLANES && T == h->L && h->dim == 2 && n > 0)
+        Tp = resident_planes_supported(h, 32) ? 32 : (resident_planes_supported(h, 64) ? 64 : 0);
+    bool plain_done = false;
+    if (Tp) {
+        const bool bits = h->layout == ISING_LAYOUT_BITS;
+        rc = ensure_store(h, bits ? Store::PlaneBits : Store::PlaneI8, Tp);
+        if (!rc && h->has_J && h->Jtiles_tile != Tp) {
+            if (!h->d_Jtiles) {
+                h->d_Jtiles = dev_alloc(coupling_record_bytes(h));
+                if (!h->d_Jtiles) rc = ISING_ENOMEM;
+            }
+            if (!rc) rc = launch_convert_couplings(h, Tp, h->d_Jtiles);
+            if (!rc) h->Jtiles_tile = Tp;
+        }
+        if (!rc) {
+            if (launch_resident_planes(h, acc, Tp, bits, n, k, h->t, d_E, d_M, true) == 0) {
+                h->last_path = bits ? "resident_plain_bits" : "resident_plain_i8";
+                plain_done = true;
+            } else {
+                cudaGetLastError();          // the cluster did not fit: the generic kernels below
+            }
+        }
+    }
+    if (plain_done || rc) {
+        // nothing more to launch
+    } else if (use_amsc) {                          // f1: 32 realisations per word, one random number per site
         h->last_path = "amsc";
         if (!h->d_amsc_J) {
             h->d_amsc_J = dev_alloc((size_t)h->N * 8);
@@ -400,7 +428,7 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             }
         }
         if (use_resident && !rc) {
-            if (launch_resident_planes(h, acc, T, bits, n, k, h->t, d_E, d_M) == 0) {
+            if (launch_resident_planes(h, acc, T, bits, n, k, h->t, d_E, d_M, false) == 0) {
                 h->last_path = bits ? "resident_planes_bits" : "resident_planes_i8";
                 resident_done = true;
             } else {

@@ -491,6 +491,8 @@ struct ResArgs {
     uint32_t jobs_per_colour;      // per replica
     long long* E;                  // optional series (a10 after every pass): E[pass * R + r], M[pass * R + r]
     long long* M;
+    int plain;                     // 1: the plain checkerboard of the whole lattice (tile == L, a8): every tile takes part in
+                                   // every half-sweep, a barrier after each; T is then only how the lattice is cut into registers
 };
 
 template <int T, bool BITS, bool HASJ>
@@ -591,7 +593,54 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
 
     const uint64_t seed = A.seeds[r];
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
-    for (int pass = 0; pass < R.n; ++pass) {
+    for (int pass = 0; pass < R.n && R.plain; ++pass) {                 // a8: fine colour 0 of every tile, barrier, fine colour 1, barrier
+        for (int j = 0; j < A.k; ++j) {
+            const uint64_t tt = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+                if (series && j == 0 && c == 1 && pass > 0) write_series(pass - 1);
+#pragma unroll
+                for (int C = 0; C < 2; ++C)
+#pragma unroll
+                    for (int m = 0; m < kResMaxJobs; ++m) {
+                        const uint32_t job = wg + (uint32_t)m * W;
+                        if (job < JC) {
+                            const int tx = txs[C][m], ty = tys[C][m];
+                            refresh(nbs[C][m], t[C][m]);
+                            const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);
+                            const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(tx * G::NW);
+                            const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);
+                            half_sweep<T, HASJ, false, kNoSpec>(A, t[C][m], Jws[C][m], c, Y, g0, p0, 2 * tt + (uint64_t)c, k0, k1);
+                            publish(C, m, t[C][m]);
+                        }
+                    }
+                cluster.sync();
+            }
+        }
+        if (series) {
+            int up = 0, unsat = 0;
+#pragma unroll
+            for (int C = 0; C < 2; ++C)
+#pragma unroll
+                for (int m = 0; m < kResMaxJobs; ++m) {
+                    const uint32_t job = wg + (uint32_t)m * W;
+                    if (job < JC) {
+                        refresh(nbs[C][m], t[C][m]);
+                        count_row<T, false>(t[C][m], Jws[C][m], Y, up, unsat);
+                    }
+                }
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                up += __shfl_xor_sync(0xffffffffu, up, d);
+                unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+            }
+            if (lane == 0) {
+                atomicAdd(acc0 + 2 * (pass & 1), up);
+                atomicAdd(acc0 + 2 * (pass & 1) + 1, unsat);
+            }
+        }
+    }
+    for (int pass = 0; pass < R.n && !R.plain; ++pass) {
 #pragma unroll
         for (int C = 0; C < 2; ++C) {
             // the previous pass's sums were added after its last barrier and are complete since the barrier just passed
@@ -680,9 +729,10 @@ static int launch_resident(const ResArgs& R, int replicas) {
 
 // n passes in one launch; the records must hold the state (ensure_store) and are current again afterwards.
 int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first,
-                           long long* d_E, long long* d_M) {
+                           long long* d_E, long long* d_M, bool plain) {
     ResArgs R;
     R.E = d_E; R.M = d_M;
+    R.plain = plain ? 1 : 0;
     PlaneArgs& A = R.P;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;

@@ -540,3 +540,35 @@ def test_tile3d_couplings_match_oracle(P, orc, L, k, n, beta, seeds, jseed, layo
     for a in range(len(seeds)):
         for b in range(a + 1, len(seeds)):
             assert g.overlap(a, b) == o.overlap(a, b)
+
+
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,k,n,beta,seeds,jseed", [
+    (128, 1, 4, BC2, [3], None),
+    (192, 2, 3, 0.3, [7], None),             # 6 x 6 register tiles of 32
+    (256, 1, 3, BC2, [21, 22], None),        # replicas
+    (512, 2, 2, BC2, [32], None),
+    (640, 1, 2, 0.6, [5], None),             # L/32 = 20 tiles: too many jobs at 32, cut into 64 x 64 tiles instead
+    (128, 2, 3, 1.0, [100, 101], 5),         # +-J
+    (128, 1, 1, BC2, [4], None),             # a single pass too
+])
+def test_plain_checkerboard_on_the_resident_kernel(P, orc, L, k, n, beta, seeds, jseed, layout):
+    """a8 beyond L = 64: tile == L, the whole lattice's even sites, barrier, odd sites, on the cluster-resident kernel."""
+    J = W.couplings(2, L, jseed) if jseed is not None else None
+    g, o = _both(P, orc, 2, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.sweep(beta, n, 0, k); o.sweep(beta, n, 0, k)
+    assert g.sweep_path() == f"resident_plain_{'i8' if layout == 'int8' else 'bits'}"
+    _same_state(g, o)
+    Eg, Mg = g.sweep_series(beta, n + 1, L, k)
+    assert g.sweep_path().startswith("resident_plain")
+    Eo, Mo = o.sweep_series(beta, n + 1, L, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    g.sweep(beta, 2, 32, 1); o.sweep(beta, 2, 32, 1)      # and back to tiles
+    _same_state(g, o)
+    g.force_path(True)
+    g.sweep(beta, 1, 0, k); o.sweep(beta, 1, 0, k)
+    assert g.sweep_path() == "generic"
+    _same_state(g, o)
