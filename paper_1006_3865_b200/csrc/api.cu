@@ -344,8 +344,12 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
     // a8 beyond L = 64: the plain checkerboard (tile == L) on the cluster-resident kernel; the register tiling Tp is
     // invisible in the result
     int Tp = 0;
-    if (!h->force_generic && !h->no_resident && !use_plain64 && !use_amsc && h->rng == ISING_RNG_PLANES && T == h->L && h->dim == 2 && n > 0)
-        Tp = resident_planes_supported(h, 32) ? 32 : (resident_planes_supported(h, 64) ? 64 : 0);
+    bool Tp_resident = false;
+    if (!h->force_generic && !use_plain64 && !use_amsc && h->rng == ISING_RNG_PLANES && T == h->L && h->dim == 2 && n > 0) {
+        if (!h->no_resident) Tp = resident_planes_supported(h, 32) ? 32 : (resident_planes_supported(h, 64) ? 64 : 0);
+        Tp_resident = Tp != 0;
+        if (!Tp) Tp = tile_planes_supported(h, 64) ? 64 : (tile_planes_supported(h, 32) ? 32 : 0);   // large L: a launch per half-sweep
+    }
     bool plain_done = false;
     if (Tp) {
         const bool bits = h->layout == ISING_LAYOUT_BITS;
@@ -358,13 +362,22 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             if (!rc) rc = launch_convert_couplings(h, Tp, h->d_Jtiles);
             if (!rc) h->Jtiles_tile = Tp;
         }
-        if (!rc) {
+        if (!rc && Tp_resident) {
             if (launch_resident_planes(h, acc, Tp, bits, n, k, h->t, d_E, d_M, true) == 0) {
                 h->last_path = bits ? "resident_plain_bits" : "resident_plain_i8";
                 plain_done = true;
             } else {
-                cudaGetLastError();          // the cluster did not fit: the generic kernels below
+                cudaGetLastError();          // the cluster did not fit: a launch per half-sweep
             }
+        }
+        if (!rc && !plain_done) {
+            h->last_path = bits ? "tile_plain_bits" : "tile_plain_i8";
+            for (int pass = 0; pass < n && !rc; ++pass) {
+                rc = launch_tile_planes_plain(h, acc, Tp, bits, 1, k, h->t + (uint64_t)pass * (uint64_t)k);
+                if (!rc && want_series)
+                    rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);
+            }
+            plain_done = !rc;
         }
     }
     if (plain_done || rc) {

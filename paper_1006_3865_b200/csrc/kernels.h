@@ -33,6 +33,7 @@ bool plain64_supported(const ising_ctx* h, int T);
 int launch_plain64(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M);
 int launch_observables_planes(ising_ctx* h, int T, bool bits, long long* d_E, long long* d_M);
 int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, int k, uint64_t t_first, bool use_jit);
+int launch_tile_planes_plain(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first);   // a8, large L
 bool resident_planes_supported(const ising_ctx* h, int T);      // small lattices: the whole call in one cluster launch
 int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first,
                            long long* d_E, long long* d_M, bool plain);   // d_E / d_M: optional series, n * R values each;

@@ -473,6 +473,78 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
     return 0;
 }
 
+// ---- a8 for large lattices: the plain checkerboard (tile == L) with a launch per half-sweep.  Every tile of the
+// register tiling T takes part: load (neighbours' boundary copies of the other fine colour are not being changed by
+// this launch), one half-sweep of fine colour c, store.  The scheme the paper starts from: the whole lattice
+// crosses HBM twice per sweep, which is what the double checkerboard's k inner sweeps per load avoid.
+template <int T, bool BITS, bool HASJ>
+__global__ void __launch_bounds__(kPlaneThreads) k_tile_planes_plain(PlaneArgs A, int c, uint64_t tt) {
+    using G = PG<T>;
+    const uint2* lut = kByteLutGlobal.e;
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const int lane = threadIdx.x & 31;
+    const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (job >= A.njobs) return;
+    const int sub = lane / G::LPT, Y = lane % G::LPT;
+    const uint32_t B = (uint32_t)A.B, q = job * G::TPW + (uint32_t)sub;        // all tiles, replica-major, row-major
+    const int r = (int)(q / (B * B));
+    const uint32_t qq = q - (uint32_t)r * B * B;
+    const int ty = (int)(qq / B), tx = (int)(qq - (uint32_t)ty * B);
+    TileRegs<T> t;
+    load_tile<T, BITS>(A, r, tx, ty, Y, sub * G::LPT, t);
+    uint4 Jw[2][G::NW];
+#pragma unroll
+    for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+        for (int gx = 0; gx < G::NW; ++gx)
+            Jw[cc][gx] = HASJ ? __ldg(A.jrec + ((size_t)ty * B + tx) * (2 * G::NW * G::LPT) + (cc * G::NW + gx) * G::LPT + Y)
+                              : make_uint4(0u, 0u, 0u, 0u);
+    const uint64_t seed = A.seeds[r];
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);
+    const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(tx * G::NW);
+    const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);
+    half_sweep<T, HASJ, false, kNoSpec>(A, t, Jw, c, Y, g0, p0, 2 * tt + (uint64_t)c, k0, k1);
+    store_tile<T, BITS>(A, r, tx, ty, Y, sub, t, lut);
+}
+
+// n passes of k plain-checkerboard sweeps: 2 n k launches.
+int launch_tile_planes_plain(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first) {
+    PlaneArgs A;
+    A.tiles = (uint8_t*)h->d_tiles;
+    A.seeds = h->d_sweep_seeds;
+    A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0;
+    A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
+    A.stream = tile_planes_bytes(h, T, bits) > kL2StreamBytes ? 1u : 0u;
+    A.njobs = (uint32_t)((size_t)h->R * A.B * A.B / (size_t)(64 / T));
+    A.magic_rep = A.magic_hb = 0;
+    fill_accept(A, acc);
+    const int warps = kPlaneThreads / 32;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((A.njobs + warps - 1) / warps); cfg.blockDim = dim3(warps * 32); cfg.dynamicSmemBytes = 0; cfg.stream = hooks().stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    static const int pdl = getenv("ISING_NO_PDL") ? 0 : 1;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    for (uint64_t s = 0; s < (uint64_t)n * (uint64_t)k; ++s)
+        for (int c = 0; c < 2; ++c) {
+            const uint64_t tt = t_first + s;
+#define ISING_PLAIN(TT, BB)                                                                                          \
+            do {                                                                                                     \
+                if (A.jrec) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes_plain<TT, BB, true>, A, c, tt));    \
+                else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes_plain<TT, BB, false>, A, c, tt));          \
+            } while (0)
+            if (T == 64) { if (bits) ISING_PLAIN(64, true); else ISING_PLAIN(64, false); }
+            else { if (bits) ISING_PLAIN(32, true); else ISING_PLAIN(32, false); }
+#undef ISING_PLAIN
+            count_launch();
+        }
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
 // ---- whole lattice on chip ("a persistent whole-lattice-on-chip kernel for small L") ----------------
 // For L <= 512 a pass of the tile kernel is two launches whose duration is launch latency + one L2 round trip, not
 // work.  Here one thread-block cluster per replica keeps every tile in registers for the whole call: warp w of the

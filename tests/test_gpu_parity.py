@@ -572,3 +572,24 @@ def test_plain_checkerboard_on_the_resident_kernel(P, orc, L, k, n, beta, seeds,
     g.sweep(beta, 1, 0, k); o.sweep(beta, 1, 0, k)
     assert g.sweep_path() == "generic"
     _same_state(g, o)
+
+
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,k,n,beta,seeds,jseed", [
+    (1024, 1, 3, BC2, [3], None),
+    (704, 2, 2, 0.3, [7, 8], None),          # 22 x 22 tiles of 32 (11 x 11 of 64 would be odd)
+    (768, 1, 2, 1.0, [100], 5),              # +-J
+])
+def test_plain_checkerboard_large_lattices(P, orc, L, k, n, beta, seeds, jseed, layout):
+    """a8 for L > 512: the tile kernel with a launch per half-sweep over all tiles."""
+    J = W.couplings(2, L, jseed) if jseed is not None else None
+    g, o = _both(P, orc, 2, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    Eg, Mg = g.sweep_series(beta, n, 0, k)
+    assert g.sweep_path() == f"tile_plain_{'i8' if layout == 'int8' else 'bits'}"
+    Eo, Mo = o.sweep_series(beta, n, 0, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    g.sweep(beta, 2, L, 1); o.sweep(beta, 2, L, 1)
+    _same_state(g, o)
