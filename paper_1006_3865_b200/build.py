@@ -55,16 +55,30 @@ def write_jit_source() -> None:
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
-    """Compile every .cu under csrc/ into one shared library; returns its path."""
+    """Compile every .cu under csrc/ (one nvcc process per file, in parallel) and link them into one shared library;
+    returns its path."""
     write_jit_source()
     if not force and not _stale():
         return LIB
     if not os.path.exists(NVCC):
         raise RuntimeError(f"nvcc not found at {NVCC}: cannot build libising_b200.so")
-    tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [NVCC, *FLAGS, *( ["-Xptxas", "-v"] if verbose else []), "-o", tmp, *sources()]
-    subprocess.check_call(cmd)
-    os.replace(tmp, LIB)
+    import shutil
+    import tempfile
+    from concurrent.futures import ThreadPoolExecutor
+    compile_flags = [f for f in FLAGS if f not in ("-shared", "-ldl")]
+    tmpdir = tempfile.mkdtemp(prefix="ising_b200_build_")
+    try:
+        def compile_one(src):
+            obj = os.path.join(tmpdir, os.path.basename(src) + ".o")
+            subprocess.check_call([NVCC, *compile_flags, *(["-Xptxas", "-v"] if verbose else []), "-c", src, "-o", obj])
+            return obj
+        with ThreadPoolExecutor(max_workers=min(8, os.cpu_count() or 1)) as pool:
+            objs = list(pool.map(compile_one, sources()))
+        tmp = LIB + f".tmp{os.getpid()}"
+        subprocess.check_call([NVCC, *FLAGS, "-o", tmp, *objs])
+        os.replace(tmp, LIB)
+    finally:
+        shutil.rmtree(tmpdir, ignore_errors=True)
     return LIB
 
 
