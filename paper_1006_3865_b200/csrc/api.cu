@@ -380,6 +380,37 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             plain_done = !rc;
         }
     }
+    // the same in 3D: 8^3 register tiles, cluster-resident up to L = 64, else a launch per half-sweep
+    if (!Tp && !rc && !h->force_generic && !use_amsc && h->rng == ISING_RNG_PLANES && T == h->L && h->dim == 3 && n > 0 &&
+        tile3d_supported(h, 8)) {
+        const bool bits = h->layout == ISING_LAYOUT_BITS;
+        rc = ensure_store(h, bits ? Store::Plane3Bits : Store::Plane3I8, 8);
+        if (!rc && h->has_J && h->Jtiles_tile != 8) {
+            if (!h->d_Jtiles) {
+                h->d_Jtiles = dev_alloc(coupling_record3d_bytes(h));
+                if (!h->d_Jtiles) rc = ISING_ENOMEM;
+            }
+            if (!rc) rc = launch_convert_couplings3d(h, h->d_Jtiles);
+            if (!rc) h->Jtiles_tile = 8;
+        }
+        if (!rc && !h->no_resident && resident3d_supported(h, 8)) {
+            if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M, true) == 0) {
+                h->last_path = bits ? "resident3d_plain_bits" : "resident3d_plain_i8";
+                plain_done = true;
+            } else {
+                cudaGetLastError();
+            }
+        }
+        if (!rc && !plain_done) {
+            h->last_path = bits ? "tile3d_plain_bits" : "tile3d_plain_i8";
+            for (int pass = 0; pass < n && !rc; ++pass) {
+                rc = launch_tile3d_plain(h, acc, bits, 1, k, h->t + (uint64_t)pass * (uint64_t)k);
+                if (!rc && want_series)
+                    rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);
+            }
+            plain_done = !rc;
+        }
+    }
     if (plain_done || rc) {
         // nothing more to launch
     } else if (use_amsc) {                          // f1: 32 realisations per word, one random number per site
@@ -433,7 +464,7 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         const bool use_resident3 = use_3d && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident &&
                                    resident3d_supported(h, T);
         if (use_resident3 && !rc) {
-            if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M) == 0) {
+            if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M, false) == 0) {
                 h->last_path = bits ? "resident3d_planes_bits" : "resident3d_planes_i8";
                 resident_done = true;
             } else {

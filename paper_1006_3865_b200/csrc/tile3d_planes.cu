@@ -111,6 +111,36 @@ __global__ void __launch_bounds__(kThreads3) k_observables3d(Plane3Args A, long 
     }
 }
 
+// a8 in 3D for L > 64: the plain checkerboard (tile == L) with a launch per half-sweep over all tiles.  Face words mix
+// the two fine colours, but a word is written whole and the bits a neighbour uses in this launch (the other fine
+// colour) are the same before and after.
+template <bool BITS, bool HASJ>
+__global__ void __launch_bounds__(kThreads3) k_tile3d_plain(Plane3Args A, int c, uint64_t tt) {
+    const uint2* lut = kByteLutGlobal.e;
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+    const int lane = threadIdx.x & 31;
+    const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    if (job >= A.njobs) return;
+    const int sub = lane >> 3, lz = lane & 7;
+    const uint32_t B = (uint32_t)A.B;
+    uint32_t q = job * 4u + (uint32_t)sub;                      // all tiles, replica-major, (tz, ty, tx) row-major
+    Tile3 t;
+    t.r = (int)(q / (B * B * B)); q -= (uint32_t)t.r * B * B * B;
+    t.tz = (int)(q / (B * B)); q -= (uint32_t)t.tz * B * B;
+    t.ty = (int)(q / B); t.tx = (int)(q - (uint32_t)t.ty * B);
+    Slice s;
+    load_slice<BITS>(A, t, lz, s);
+    load_couplings<HASJ>(A, t, lz, s);
+    const uint64_t seed = A.seeds[t.r];
+    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+    const uint32_t z = (uint32_t)(t.tz * kT3 + lz);
+    const uint32_t g = (z * B + (uint32_t)t.ty) * B + (uint32_t)t.tx;
+    const uint32_t p_base = (uint32_t)(t.tx * 4) + (uint32_t)(A.L >> 1) * ((uint32_t)(t.ty * kT3) + (uint32_t)A.L * z);
+    half_sweep3<kNoSpec3, HASJ>(A, s, c, lz, g, p_base, 2 * tt + (uint64_t)c, k0, k1);
+    store_slice<BITS>(A, t, lz, s, lut);
+}
+
 }  // namespace
 
 static void fill_geometry3(Plane3Args& A, const ising_ctx* h) {
@@ -122,6 +152,45 @@ static void fill_geometry3(Plane3Args& A, const ising_ctx* h) {
     A.magic_rep = fastdiv_magic(A.per_rep); A.magic_z = fastdiv_magic(A.per_z); A.magic_hb = fastdiv_magic(A.hb);
     A.njobs = (uint32_t)((size_t)h->R * A.per_rep / 4u);
     A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
+}
+
+static void fill_accept3(Plane3Args& A, const Accept& acc) {
+    for (int m = 0; m < 3; ++m) {
+        for (int q = 0; q < kHeadBits; ++q) A.u[m][q] = ((acc.thr[m] >> (31 - q)) & 1u) ? 0xffffffffu : 0u;
+        A.tail[m] = acc.thr[m] & ((1u << kTailBits) - 1u);
+    }
+    A.force = acc.thr_is_2p32[0] ? 0xffffffffu : 0u;
+}
+
+// n passes of k plain-checkerboard sweeps in 3D: 2 n k launches.
+int launch_tile3d_plain(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first) {
+    Plane3Args A = {};
+    fill_geometry3(A, h);
+    fill_accept3(A, acc);
+    A.k = k; A.t_first = t_first; A.C = 0;
+    A.njobs = (uint32_t)((size_t)h->R * A.B * A.B * A.B / 4u);
+    const int warps = kThreads3 / 32;
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((A.njobs + warps - 1) / warps); cfg.blockDim = dim3(warps * 32); cfg.stream = hooks().stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    static const int pdl = getenv("ISING_NO_PDL") ? 0 : 1;
+    attr[0].val.programmaticStreamSerializationAllowed = pdl;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    for (uint64_t s = 0; s < (uint64_t)n * (uint64_t)k; ++s)
+        for (int c = 0; c < 2; ++c) {
+            const uint64_t tt = t_first + s;
+            if (A.jrec) {
+                if (bits) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<true, true>, A, c, tt));
+                else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<false, true>, A, c, tt));
+            } else {
+                if (bits) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<true, false>, A, c, tt));
+                else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<false, false>, A, c, tt));
+            }
+            count_launch();
+        }
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
 }
 
 // a10 on 3D tile records: E[r], M[r] (R values each, either may be null).
@@ -257,6 +326,7 @@ struct Res3Args {
     uint32_t jobs_per_colour;      // per replica, 4 tiles per job
     long long* E;                  // optional series (a10 after every pass): E[pass * R + r], M[pass * R + r]
     long long* M;
+    int plain;                     // 1: plain checkerboard of the whole lattice (tile == L), a barrier after every half-sweep
 };
 
 template <bool BITS, bool HASJ>
@@ -344,7 +414,45 @@ __global__ void __launch_bounds__(kRes3Warps * 32) k_resident3d(Res3Args R) {
 
     const uint64_t seed = A.seeds[r];
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
-    for (int pass = 0; pass < R.n; ++pass) {
+    for (int pass = 0; pass < R.n && R.plain; ++pass) {        // a8: fine colour 0 of every tile, barrier, fine colour 1, barrier
+        for (int j = 0; j < A.k; ++j) {
+            const uint64_t tt = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+                if (series && j == 0 && c == 1 && pass > 0) write_series(pass - 1);
+#pragma unroll
+                for (int C = 0; C < 2; ++C)
+                    if (mine) {
+                        refresh(nb[C], s[C]);
+                        const uint32_t z = (uint32_t)(t[C].tz * kT3 + lz);
+                        const uint32_t g = (z * B + (uint32_t)t[C].ty) * B + (uint32_t)t[C].tx;
+                        const uint32_t p_base = (uint32_t)(t[C].tx * 4) + (uint32_t)(A.L >> 1) * ((uint32_t)(t[C].ty * kT3) + (uint32_t)A.L * z);
+                        half_sweep3<kNoSpec3, HASJ>(A, s[C], c, lz, g, p_base, 2 * tt + (uint64_t)c, k0, k1);
+                        publish(C, s[C]);
+                    }
+                cluster.sync();
+            }
+        }
+        if (series) {
+            int up = 0, unsat = 0;
+            if (mine) {
+                refresh(nb[0], s[0]);
+                refresh(nb[1], s[1]);
+                count_slice<HASJ>(s[0], lz, up, unsat);
+                count_slice<HASJ>(s[1], lz, up, unsat);
+            }
+#pragma unroll
+            for (int d = 16; d > 0; d >>= 1) {
+                up += __shfl_xor_sync(0xffffffffu, up, d);
+                unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+            }
+            if (lane == 0 && mine) {
+                atomicAdd(acc0 + 2 * (pass & 1), up);
+                atomicAdd(acc0 + 2 * (pass & 1) + 1, unsat);
+            }
+        }
+    }
+    for (int pass = 0; pass < R.n && !R.plain; ++pass) {
 #pragma unroll
         for (int C = 0; C < 2; ++C) {
             if (series && C == 1 && pass > 0) write_series(pass - 1);    // complete since the barrier just passed
@@ -396,9 +504,11 @@ bool resident3d_supported(const ising_ctx* h, int T) {
     return B * B * B / 2u / 4u <= (uint32_t)(kRes3MaxCluster * kRes3Warps) && (B * B * B / 2u) % 4u == 0;
 }
 
-int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M) {
+int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M,
+                      bool plain) {
     Res3Args R;
     R.E = d_E; R.M = d_M;
+    R.plain = plain ? 1 : 0;
     Plane3Args& A = R.P;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;

@@ -593,3 +593,29 @@ def test_plain_checkerboard_large_lattices(P, orc, L, k, n, beta, seeds, jseed, 
     _same_state(g, o)
     g.sweep(beta, 2, L, 1); o.sweep(beta, 2, L, 1)
     _same_state(g, o)
+
+
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,k,n,beta,seeds,jseed,path", [
+    (16, 1, 4, BC3, [4], None, "resident3d_plain"),
+    (32, 2, 3, BC3, [4, 5], None, "resident3d_plain"),
+    (64, 1, 2, 0.3, [9], None, "resident3d_plain"),
+    (32, 1, 3, 0.9, [1, 2], 7, "resident3d_plain"),        # 3D +-J
+    (96, 1, 2, BC3, [2], None, "tile3d_plain"),             # L > 64: a launch per half-sweep
+    (80, 2, 2, 0.9, [3], 11, "tile3d_plain"),
+])
+def test_plain_checkerboard_3d(P, orc, L, k, n, beta, seeds, jseed, path, layout):
+    """a8 in 3D: tile == L on the 8^3 register tiling, cluster-resident (L <= 64) or a launch per half-sweep."""
+    J = W.couplings(3, L, jseed) if jseed is not None else None
+    g, o = _both(P, orc, 3, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.sweep(beta, n, 0, k); o.sweep(beta, n, 0, k)
+    assert g.sweep_path() == f"{path}_{'i8' if layout == 'int8' else 'bits'}"
+    _same_state(g, o)
+    Eg, Mg = g.sweep_series(beta, n, L, k)
+    Eo, Mo = o.sweep_series(beta, n, L, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    g.sweep(beta, 2, 8, 1); o.sweep(beta, 2, 8, 1)          # and back to the double checkerboard
+    _same_state(g, o)
