@@ -345,7 +345,9 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
     // invisible in the result
     int Tp = 0;
     bool Tp_resident = false;
-    if (!h->force_generic && !use_plain64 && !use_amsc && h->rng == ISING_RNG_PLANES && T == h->L && h->dim == 2 && n > 0) {
+    // ... and the double checkerboard of the paper's small tiles (T = 2, 4, 8, 16 < 32) as masked half-sweeps on the same tiling
+    const int Tc = (T == 2 || T == 4 || T == 8 || T == 16) && T != h->L ? T : 0;
+    if (!h->force_generic && !use_plain64 && !use_amsc && h->rng == ISING_RNG_PLANES && (T == h->L || Tc) && h->dim == 2 && n > 0) {
         if (!h->no_resident) Tp = resident_planes_supported(h, 32) ? 32 : (resident_planes_supported(h, 64) ? 64 : 0);
         Tp_resident = Tp != 0;
         if (!Tp) Tp = tile_planes_supported(h, 64) ? 64 : (tile_planes_supported(h, 32) ? 32 : 0);   // large L: a launch per half-sweep
@@ -363,17 +365,17 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             if (!rc) h->Jtiles_tile = Tp;
         }
         if (!rc && Tp_resident) {
-            if (launch_resident_planes(h, acc, Tp, bits, n, k, h->t, d_E, d_M, true) == 0) {
-                h->last_path = bits ? "resident_plain_bits" : "resident_plain_i8";
+            if (launch_resident_planes(h, acc, Tp, bits, n, k, h->t, d_E, d_M, true, Tc) == 0) {
+                h->last_path = Tc ? (bits ? "resident_masked_bits" : "resident_masked_i8") : (bits ? "resident_plain_bits" : "resident_plain_i8");
                 plain_done = true;
             } else {
                 cudaGetLastError();          // the cluster did not fit: a launch per half-sweep
             }
         }
         if (!rc && !plain_done) {
-            h->last_path = bits ? "tile_plain_bits" : "tile_plain_i8";
+            h->last_path = Tc ? (bits ? "tile_masked_bits" : "tile_masked_i8") : (bits ? "tile_plain_bits" : "tile_plain_i8");
             for (int pass = 0; pass < n && !rc; ++pass) {
-                rc = launch_tile_planes_plain(h, acc, Tp, bits, 1, k, h->t + (uint64_t)pass * (uint64_t)k);
+                rc = launch_tile_planes_plain(h, acc, Tp, bits, 1, k, h->t + (uint64_t)pass * (uint64_t)k, Tc);
                 if (!rc && want_series)
                     rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);
             }
@@ -472,7 +474,7 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             }
         }
         if (use_resident && !rc) {
-            if (launch_resident_planes(h, acc, T, bits, n, k, h->t, d_E, d_M, false) == 0) {
+            if (launch_resident_planes(h, acc, T, bits, n, k, h->t, d_E, d_M, false, 0) == 0) {
                 h->last_path = bits ? "resident_planes_bits" : "resident_planes_i8";
                 resident_done = true;
             } else {

@@ -33,10 +33,10 @@ bool plain64_supported(const ising_ctx* h, int T);
 int launch_plain64(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M);
 int launch_observables_planes(ising_ctx* h, int T, bool bits, long long* d_E, long long* d_M);
 int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, int k, uint64_t t_first, bool use_jit);
-int launch_tile_planes_plain(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first);   // a8, large L
+int launch_tile_planes_plain(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, int Tc);   // a8, large L; Tc: coarse tiles 2..16 or 0
 bool resident_planes_supported(const ising_ctx* h, int T);      // small lattices: the whole call in one cluster launch
 int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first,
-                           long long* d_E, long long* d_M, bool plain);   // d_E / d_M: optional series, n * R values each;
+                           long long* d_E, long long* d_M, bool plain, int Tc);   // d_E / d_M: optional series, n * R values each;
                                                                            // plain: the tile == L schedule, T = register tiling only
 
 // ---- tile3d_planes.cu: 3D multi-spin tile kernel, 8x8x8 tiles (RNG mapping "planes") ----------

@@ -473,12 +473,35 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
     return 0;
 }
 
+// ---- coarse tiles smaller than a register tile (the paper's own T = 4, 8, 16): the double checkerboard of
+// coarse tiles Tc in {2, 4, 8, 16} on the register tiling T in {32, 64}.  A phase (coarse colour Cc, inner sweep, fine
+// colour c) is a half-sweep of the whole lattice in which only the sites of the colour-Cc coarse tiles may flip: the
+// flip word is masked.  Bit j = 16 rp + kk of a block word is the site x = 32 gx + 2 kk + a, y = 2 Yg + rp, so the parity
+// of x / Tc is a fixed bit pattern and that of y / Tc depends on the block row only.
+__device__ __forceinline__ uint32_t coarse_mask(int Tc, uint32_t Yg, int Cc) {
+    if (Tc == 0) return 0xffffffffu;
+    const uint32_t even_x = Tc == 16 ? 0x00ff00ffu : Tc == 8 ? 0x0f0f0f0fu : Tc == 4 ? 0x33333333u : 0x55555555u;
+    const uint32_t typ = ((2u * Yg) / (uint32_t)Tc) & 1u;
+    return ((typ ^ (uint32_t)Cc) & 1u) ? ~even_x : even_x;
+}
+
+template <int T, bool HASJ>
+__device__ __forceinline__ void half_sweep_masked(const PlaneArgs& A, TileRegs<T>& t, const uint4 (&Jw)[2][PG<T>::NW], int c, int Y,
+                                                  uint32_t g0, uint32_t p0, uint64_t H, uint32_t k0, uint32_t k1, uint32_t mask) {
+    uint32_t old[PG<T>::NW];
+#pragma unroll
+    for (int gx = 0; gx < PG<T>::NW; ++gx) old[gx] = t.S[c][gx];
+    half_sweep<T, HASJ, false, kNoSpec>(A, t, Jw, c, Y, g0, p0, H, k0, k1);
+#pragma unroll
+    for (int gx = 0; gx < PG<T>::NW; ++gx) t.S[c][gx] = (t.S[c][gx] & mask) | (old[gx] & ~mask);
+}
+
 // ---- a8 for large lattices: the plain checkerboard (tile == L) with a launch per half-sweep.  Every tile of the
 // register tiling T takes part: load (neighbours' boundary copies of the other fine colour are not being changed by
 // this launch), one half-sweep of fine colour c, store.  The scheme the paper starts from: the whole lattice
 // crosses HBM twice per sweep, which is what the double checkerboard's k inner sweeps per load avoid.
 template <int T, bool BITS, bool HASJ>
-__global__ void __launch_bounds__(kPlaneThreads) k_tile_planes_plain(PlaneArgs A, int c, uint64_t tt) {
+__global__ void __launch_bounds__(kPlaneThreads) k_tile_planes_plain(PlaneArgs A, int c, uint64_t tt, int Tc, int Cc) {
     using G = PG<T>;
     const uint2* lut = kByteLutGlobal.e;
     asm volatile("griddepcontrol.launch_dependents;");
@@ -505,12 +528,13 @@ __global__ void __launch_bounds__(kPlaneThreads) k_tile_planes_plain(PlaneArgs A
     const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);
     const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(tx * G::NW);
     const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);
-    half_sweep<T, HASJ, false, kNoSpec>(A, t, Jw, c, Y, g0, p0, 2 * tt + (uint64_t)c, k0, k1);
+    half_sweep_masked<T, HASJ>(A, t, Jw, c, Y, g0, p0, 2 * tt + (uint64_t)c, k0, k1, coarse_mask(Tc, Yg, Cc));
     store_tile<T, BITS>(A, r, tx, ty, Y, sub, t, lut);
 }
 
-// n passes of k plain-checkerboard sweeps: 2 n k launches.
-int launch_tile_planes_plain(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first) {
+// n passes of k plain-checkerboard sweeps: 2 n k launches; with coarse tiles Tc (0: none) n passes of the double
+// checkerboard of Tc-tiles: 4 n k launches.
+int launch_tile_planes_plain(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, int Tc) {
     PlaneArgs A;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;
@@ -528,19 +552,21 @@ int launch_tile_planes_plain(ising_ctx* h, const Accept& acc, int T, bool bits, 
     static const int pdl = getenv("ISING_NO_PDL") ? 0 : 1;
     attr[0].val.programmaticStreamSerializationAllowed = pdl;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    for (uint64_t s = 0; s < (uint64_t)n * (uint64_t)k; ++s)
-        for (int c = 0; c < 2; ++c) {
-            const uint64_t tt = t_first + s;
-#define ISING_PLAIN(TT, BB)                                                                                          \
-            do {                                                                                                     \
-                if (A.jrec) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes_plain<TT, BB, true>, A, c, tt));    \
-                else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes_plain<TT, BB, false>, A, c, tt));          \
-            } while (0)
-            if (T == 64) { if (bits) ISING_PLAIN(64, true); else ISING_PLAIN(64, false); }
-            else { if (bits) ISING_PLAIN(32, true); else ISING_PLAIN(32, false); }
+    for (int pass = 0; pass < n; ++pass)
+        for (int Cc = 0; Cc < (Tc ? 2 : 1); ++Cc)
+            for (int j = 0; j < k; ++j)
+                for (int c = 0; c < 2; ++c) {
+                    const uint64_t tt = t_first + (uint64_t)pass * (uint64_t)k + (uint64_t)j;
+#define ISING_PLAIN(TT, BB)                                                                                                  \
+                    do {                                                                                                     \
+                        if (A.jrec) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes_plain<TT, BB, true>, A, c, tt, Tc, Cc));    \
+                        else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes_plain<TT, BB, false>, A, c, tt, Tc, Cc));          \
+                    } while (0)
+                    if (T == 64) { if (bits) ISING_PLAIN(64, true); else ISING_PLAIN(64, false); }
+                    else { if (bits) ISING_PLAIN(32, true); else ISING_PLAIN(32, false); }
 #undef ISING_PLAIN
-            count_launch();
-        }
+                    count_launch();
+                }
     ISING_CUDA_OK(cudaGetLastError());
     return 0;
 }
@@ -565,6 +591,7 @@ struct ResArgs {
     long long* M;
     int plain;                     // 1: the plain checkerboard of the whole lattice (tile == L, a8): every tile takes part in
                                    // every half-sweep, a barrier after each; T is then only how the lattice is cut into registers
+    int coarse;                    // with plain: coarse tile edge Tc in {2, 4, 8, 16} of a masked double checkerboard, or 0
 };
 
 template <int T, bool BITS, bool HASJ>
@@ -666,11 +693,12 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
     const uint64_t seed = A.seeds[r];
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     for (int pass = 0; pass < R.n && R.plain; ++pass) {                 // a8: fine colour 0 of every tile, barrier, fine colour 1, barrier
+      for (int Cc = 0; Cc < (R.coarse ? 2 : 1); ++Cc)                   // (masked double checkerboard: both coarse colours in turn)
         for (int j = 0; j < A.k; ++j) {
             const uint64_t tt = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
-                if (series && j == 0 && c == 1 && pass > 0) write_series(pass - 1);
+                if (series && Cc == 0 && j == 0 && c == 1 && pass > 0) write_series(pass - 1);
 #pragma unroll
                 for (int C = 0; C < 2; ++C)
 #pragma unroll
@@ -682,7 +710,7 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
                             const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);
                             const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(tx * G::NW);
                             const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);
-                            half_sweep<T, HASJ, false, kNoSpec>(A, t[C][m], Jws[C][m], c, Y, g0, p0, 2 * tt + (uint64_t)c, k0, k1);
+                            half_sweep_masked<T, HASJ>(A, t[C][m], Jws[C][m], c, Y, g0, p0, 2 * tt + (uint64_t)c, k0, k1, coarse_mask(R.coarse, Yg, Cc));
                             publish(C, m, t[C][m]);
                         }
                     }
@@ -801,10 +829,11 @@ static int launch_resident(const ResArgs& R, int replicas) {
 
 // n passes in one launch; the records must hold the state (ensure_store) and are current again afterwards.
 int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first,
-                           long long* d_E, long long* d_M, bool plain) {
+                           long long* d_E, long long* d_M, bool plain, int Tc) {
     ResArgs R;
     R.E = d_E; R.M = d_M;
     R.plain = plain ? 1 : 0;
+    R.coarse = plain ? Tc : 0;
     PlaneArgs& A = R.P;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;

@@ -619,3 +619,30 @@ def test_plain_checkerboard_3d(P, orc, L, k, n, beta, seeds, jseed, path, layout
     _same_state(g, o)
     g.sweep(beta, 2, 8, 1); o.sweep(beta, 2, 8, 1)          # and back to the double checkerboard
     _same_state(g, o)
+
+
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,tile,k,n,beta,seeds,jseed,path", [
+    (64, 16, 1, 4, BC2, [3], None, "resident_masked"),       # the paper's tile sizes 4, 8, 16
+    (128, 8, 2, 3, BC2, [5], None, "resident_masked"),
+    (128, 4, 1, 3, 0.6, [6, 7], None, "resident_masked"),
+    (64, 2, 3, 2, 0.3, [8], None, "resident_masked"),
+    (256, 16, 4, 2, 1.0, [100, 101], 5, "resident_masked"),  # +-J
+    (1024, 16, 1, 2, BC2, [9], None, "tile_masked"),
+    (704, 8, 2, 1, 0.5, [10], None, "tile_masked"),
+])
+def test_small_coarse_tiles_on_the_fast_kernels(P, orc, L, tile, k, n, beta, seeds, jseed, path, layout):
+    """Double checkerboard with coarse tiles smaller than a register tile: masked half-sweeps, same trajectory as the oracle's."""
+    J = W.couplings(2, L, jseed) if jseed is not None else None
+    g, o = _both(P, orc, 2, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.sweep(beta, n, tile, k); o.sweep(beta, n, tile, k)
+    assert g.sweep_path() == f"{path}_{'i8' if layout == 'int8' else 'bits'}"
+    _same_state(g, o)
+    Eg, Mg = g.sweep_series(beta, n, tile, k)
+    Eo, Mo = o.sweep_series(beta, n, tile, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    g.sweep(beta, 2, 32, 1); o.sweep(beta, 2, 32, 1)
+    _same_state(g, o)
