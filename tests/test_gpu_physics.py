@@ -98,12 +98,12 @@ def test_heisenberg_high_temperature_series_3d(P):
 
 def test_3d_equilibrium_is_the_same_for_both_schedules(P):
     """3D Ising L = 16 at the critical coupling: the double checkerboard with 8^3 tiles (cluster-resident kernel, E counted
-    on the registers) and the plain checkerboard (tile = L, generic kernels) are different chains with the same
+    on the registers) and the plain checkerboard (tile = L, the same kernel in plain mode) are different chains with the same
     equilibrium; no exact finite-lattice value exists in 3D, so the two are compared with each other."""
     import torch
     L, beta = 16, W.BETA_C_3D
     means = []
-    for tile, k, n, path in ((8, 1, 200000, "resident3d_planes_i8"), (8, 2, 100000, "resident3d_planes_i8"), (16, 1, 60000, "generic")):
+    for tile, k, n, path in ((8, 1, 200000, "resident3d_planes_i8"), (8, 2, 100000, "resident3d_planes_i8"), (16, 1, 100000, "resident3d_plain_i8")):
         g = P.Ising(3, L, seed=31 + tile + k)
         g.sweep(beta, 3000, tile, k)
         E = torch.zeros(n, dtype=torch.int64, device="cuda")
