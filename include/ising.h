@@ -184,7 +184,7 @@ uint64_t ising_kernel_launches(void);
  * of a 2D lattice with 64 < L <= 512 on the same kernel (one barrier per half-sweep); "tile_plain_*": the plain
  * checkerboard of larger 2D lattices (L a multiple of 64 with L/64 even, or of 32 with L/32 even), a launch per half-sweep.
  * "resident3d_plain_*" / "tile3d_plain_*": the plain checkerboard in 3D (L a multiple of 8 with L/8 even; L <= 64 / larger).
- * "resident_masked_*" / "tile_masked_*": 2D double checkerboard with tiles of 2, 4, 8 or 16 (the paper's sizes) as masked
+ * "resident_masked_*" / "tile_masked_*": 2D double checkerboard with tiles of 2, 4, 8, 16 (the paper's sizes), 128, 256, ... as masked
  * half-sweeps on the same kernels. */
 const char* ising_sweep_path(ising_handle h);
 

@@ -346,7 +346,8 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
     int Tp = 0;
     bool Tp_resident = false;
     // ... and the double checkerboard of the paper's small tiles (T = 2, 4, 8, 16 < 32) as masked half-sweeps on the same tiling
-    const int Tc = (T == 2 || T == 4 || T == 8 || T == 16) && T != h->L ? T : 0;
+    // (and tiles of 128, 256, ...: whole register tiles switched on and off)
+    const int Tc = (T >= 2 && (T & (T - 1)) == 0 && T != 32 && T != 64 && T != h->L) ? T : 0;
     if (!h->force_generic && !use_plain64 && !use_amsc && h->rng == ISING_RNG_PLANES && (T == h->L || Tc) && h->dim == 2 && n > 0) {
         if (!h->no_resident) Tp = resident_planes_supported(h, 32) ? 32 : (resident_planes_supported(h, 64) ? 64 : 0);
         Tp_resident = Tp != 0;

@@ -474,26 +474,36 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
 }
 
 // ---- coarse tiles smaller than a register tile (the paper's own T = 4, 8, 16): the double checkerboard of
-// coarse tiles Tc in {2, 4, 8, 16} on the register tiling T in {32, 64}.  A phase (coarse colour Cc, inner sweep, fine
+// coarse tiles Tc = 2, 4, 8, 16 (and of the powers of two above 64, where a mask is all or nothing) on the register tiling
+// T in {32, 64}.  A phase (coarse colour Cc, inner sweep, fine
 // colour c) is a half-sweep of the whole lattice in which only the sites of the colour-Cc coarse tiles may flip: the
 // flip word is masked.  Bit j = 16 rp + kk of a block word is the site x = 32 gx + 2 kk + a, y = 2 Yg + rp, so the parity
 // of x / Tc is a fixed bit pattern and that of y / Tc depends on the block row only.
-__device__ __forceinline__ uint32_t coarse_mask(int Tc, uint32_t Yg, int Cc) {
+__device__ __forceinline__ uint32_t coarse_mask(int Tc, uint32_t Yg, uint32_t gxg, int Cc) {
     if (Tc == 0) return 0xffffffffu;
-    const uint32_t even_x = Tc == 16 ? 0x00ff00ffu : Tc == 8 ? 0x0f0f0f0fu : Tc == 4 ? 0x33333333u : 0x55555555u;
     const uint32_t typ = ((2u * Yg) / (uint32_t)Tc) & 1u;
+    if (Tc >= 32) {                                        // the 32 columns of the block lie in one coarse tile: all or nothing
+        const uint32_t txp = ((32u * gxg) / (uint32_t)Tc) & 1u;
+        return ((txp ^ typ ^ (uint32_t)Cc) & 1u) ? 0u : 0xffffffffu;
+    }
+    const uint32_t even_x = Tc == 16 ? 0x00ff00ffu : Tc == 8 ? 0x0f0f0f0fu : Tc == 4 ? 0x33333333u : 0x55555555u;
     return ((typ ^ (uint32_t)Cc) & 1u) ? ~even_x : even_x;
 }
 
+// gxg0: global block column of the lane's word gx = 0
 template <int T, bool HASJ>
 __device__ __forceinline__ void half_sweep_masked(const PlaneArgs& A, TileRegs<T>& t, const uint4 (&Jw)[2][PG<T>::NW], int c, int Y,
-                                                  uint32_t g0, uint32_t p0, uint64_t H, uint32_t k0, uint32_t k1, uint32_t mask) {
+                                                  uint32_t g0, uint32_t p0, uint64_t H, uint32_t k0, uint32_t k1, int Tc, uint32_t Yg,
+                                                  uint32_t gxg0, int Cc) {
     uint32_t old[PG<T>::NW];
 #pragma unroll
     for (int gx = 0; gx < PG<T>::NW; ++gx) old[gx] = t.S[c][gx];
     half_sweep<T, HASJ, false, kNoSpec>(A, t, Jw, c, Y, g0, p0, H, k0, k1);
 #pragma unroll
-    for (int gx = 0; gx < PG<T>::NW; ++gx) t.S[c][gx] = (t.S[c][gx] & mask) | (old[gx] & ~mask);
+    for (int gx = 0; gx < PG<T>::NW; ++gx) {
+        const uint32_t mask = coarse_mask(Tc, Yg, gxg0 + (uint32_t)gx, Cc);
+        t.S[c][gx] = (t.S[c][gx] & mask) | (old[gx] & ~mask);
+    }
 }
 
 // ---- a8 for large lattices: the plain checkerboard (tile == L) with a launch per half-sweep.  Every tile of the
@@ -528,7 +538,7 @@ __global__ void __launch_bounds__(kPlaneThreads) k_tile_planes_plain(PlaneArgs A
     const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);
     const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(tx * G::NW);
     const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);
-    half_sweep_masked<T, HASJ>(A, t, Jw, c, Y, g0, p0, 2 * tt + (uint64_t)c, k0, k1, coarse_mask(Tc, Yg, Cc));
+    half_sweep_masked<T, HASJ>(A, t, Jw, c, Y, g0, p0, 2 * tt + (uint64_t)c, k0, k1, Tc, Yg, (uint32_t)(tx * G::NW), Cc);
     store_tile<T, BITS>(A, r, tx, ty, Y, sub, t, lut);
 }
 
@@ -710,7 +720,7 @@ __global__ void __launch_bounds__(kResWarps * 32) k_resident_planes(ResArgs R) {
                             const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);
                             const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(tx * G::NW);
                             const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);
-                            half_sweep_masked<T, HASJ>(A, t[C][m], Jws[C][m], c, Y, g0, p0, 2 * tt + (uint64_t)c, k0, k1, coarse_mask(R.coarse, Yg, Cc));
+                            half_sweep_masked<T, HASJ>(A, t[C][m], Jws[C][m], c, Y, g0, p0, 2 * tt + (uint64_t)c, k0, k1, R.coarse, Yg, (uint32_t)(tx * G::NW), Cc);
                             publish(C, m, t[C][m]);
                         }
                     }

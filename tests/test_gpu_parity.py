@@ -628,6 +628,9 @@ def test_plain_checkerboard_3d(P, orc, L, k, n, beta, seeds, jseed, path, layout
     (128, 4, 1, 3, 0.6, [6, 7], None, "resident_masked"),
     (64, 2, 3, 2, 0.3, [8], None, "resident_masked"),
     (256, 16, 4, 2, 1.0, [100, 101], 5, "resident_masked"),  # +-J
+    (512, 128, 2, 2, BC2, [11], None, "resident_masked"),    # tiles above 64: whole register tiles switched on and off
+    (1024, 256, 1, 2, 0.5, [12], None, "tile_masked"),
+    (1024, 128, 2, 1, BC2, [13], None, "tile_masked"),
     (1024, 16, 1, 2, BC2, [9], None, "tile_masked"),
     (704, 8, 2, 1, 0.5, [10], None, "tile_masked"),
 ])
