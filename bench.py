@@ -167,7 +167,7 @@ def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng=
     # the library's AUTO rule (specialise calls of >= 2^27 attempted flips), decided here for the timed call so that
     # the warm-up call, which is shorter, already compiles the kernel the timed call will use
     # (lattices small enough for the cluster-resident kernel, <= 64 warp jobs per colour, stay on AUTO: it serves them)
-    resident = (L // tile) ** 2 // 2 // (64 // tile) <= 64 and steps >= 2
+    resident = tile in (32, 64) and (L // tile) ** 2 // 2 // (64 // tile) <= 64 and steps >= 2
     if not resident:
         g.set_jit("on" if JIT == "on" or (JIT == "auto" and steps * k * L * L >= 2 ** 27) else "off")
     else:
@@ -360,14 +360,18 @@ def run_heisenberg(P, torch, a) -> None:
 
 
 def run_lscan(P, torch, a) -> None:
-    """flips/ns against L in the style of the paper's Fig. 3, planes mapping, int8 records."""
+    """flips/ns against L in the style of the paper's Fig. 3 and its tile tuning, planes mapping, int8
+    records: tiles 32 and 64 (the native register tiles) at k = 1, 4, 16; tiles 8, 16, 128 (masked half-sweeps) and the plain
+    checkerboard (tile 0 = L) at k = 1."""
     rows = []
     for L in (64, 128, 256, 512, 1024, 2048, 4096, 8192, 16384):
-        for T in (32, 64):
-            if L % T or (L // T) % 2:
+        for T in (8, 16, 32, 64, 128, 0):
+            if T and (L % T or (L // T) % 2):
                 continue
-            for k in (1, 4, 16):
+            for k in ((1, 4, 16) if T in (32, 64) else (1,)):
                 n = max(4, min(2000, int(2e10 / (k * L * L))))
+                if T not in (32, 64):
+                    n = max(4, n // 4)
                 r = time_variant(P, torch, L, "int8", T, k, n, 3, None, "planes")
                 rows.append({"L": L, "tile": T, "k": k, "passes": n, "flips_per_ns": round(r["flips_per_ns"], 2),
                              "us_per_pass": round(1e3 * r["ms"] / n, 2), "path": r["path"]})
