@@ -175,7 +175,7 @@ uint64_t ising_kernel_launches(void);
 /* ising_sweep_path — name of the kernel family the last ising_sweep on h used
  * ("generic", "tile_i8", "tile_planes_i8", "tile_planes_bits", "tile3d_planes_i8", "tile3d_planes_bits",
  * "plain64_planes_i8", "plain64_planes_bits", "resident_planes_i8", "resident_planes_bits", "resident3d_planes_i8",
- * "resident3d_planes_bits", "resident_plain_i8", "resident_plain_bits", "tile_plain_i8", "tile_plain_bits", "resident3d_plain_i8/_bits", "tile3d_plain_i8/_bits", "resident_masked_i8/_bits", "tile_masked_i8/_bits", "amsc");
+ * "resident3d_planes_bits", "resident_plain_i8", "resident_plain_bits", "tile_plain_i8", "tile_plain_bits", "resident3d_plain_i8/_bits", "tile3d_plain_i8/_bits", "resident_masked_i8/_bits", "tile_masked_i8/_bits", "resident3d_masked_i8/_bits", "tile3d_masked_i8/_bits", "amsc");
  * static string,
  * never NULL.  "resident_planes_*": 2D, J = +1 or +-J, at most 64 warp jobs per coarse colour (L <= 512 at tile 32 or 64),
  * n_sweeps >= 2: the whole call runs in one launch of one thread-block cluster per replica with the lattice held
@@ -185,7 +185,7 @@ uint64_t ising_kernel_launches(void);
  * checkerboard of larger 2D lattices (L a multiple of 64 with L/64 even, or of 32 with L/32 even), a launch per half-sweep.
  * "resident3d_plain_*" / "tile3d_plain_*": the plain checkerboard in 3D (L a multiple of 8 with L/8 even; L <= 64 / larger).
  * "resident_masked_*" / "tile_masked_*": 2D double checkerboard with tiles of 2, 4, 8, 16 (the paper's sizes), 128, 256, ... as masked
- * half-sweeps on the same kernels. */
+ * half-sweeps on the same kernels; "resident3d_masked_*" / "tile3d_masked_*": 3D tiles of 2, 4, 16, 32, ... likewise. */
 const char* ising_sweep_path(ising_handle h);
 
 /* ising_force_path — testing aid: 0 = automatic kernel choice, 1 = always the generic

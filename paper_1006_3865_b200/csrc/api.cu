@@ -384,7 +384,8 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         }
     }
     // the same in 3D: 8^3 register tiles, cluster-resident up to L = 64, else a launch per half-sweep
-    if (!Tp && !rc && !h->force_generic && !use_amsc && h->rng == ISING_RNG_PLANES && T == h->L && h->dim == 3 && n > 0 &&
+    const int Tc3 = (h->dim == 3 && T >= 2 && (T & (T - 1)) == 0 && T != 8 && T != h->L) ? T : 0;      // masked coarse tiles in 3D
+    if (!Tp && !rc && !h->force_generic && !use_amsc && h->rng == ISING_RNG_PLANES && (T == h->L || Tc3) && h->dim == 3 && n > 0 &&
         tile3d_supported(h, 8)) {
         const bool bits = h->layout == ISING_LAYOUT_BITS;
         rc = ensure_store(h, bits ? Store::Plane3Bits : Store::Plane3I8, 8);
@@ -397,17 +398,17 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             if (!rc) h->Jtiles_tile = 8;
         }
         if (!rc && !h->no_resident && resident3d_supported(h, 8)) {
-            if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M, true) == 0) {
-                h->last_path = bits ? "resident3d_plain_bits" : "resident3d_plain_i8";
+            if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M, true, Tc3) == 0) {
+                h->last_path = Tc3 ? (bits ? "resident3d_masked_bits" : "resident3d_masked_i8") : (bits ? "resident3d_plain_bits" : "resident3d_plain_i8");
                 plain_done = true;
             } else {
                 cudaGetLastError();
             }
         }
         if (!rc && !plain_done) {
-            h->last_path = bits ? "tile3d_plain_bits" : "tile3d_plain_i8";
+            h->last_path = Tc3 ? (bits ? "tile3d_masked_bits" : "tile3d_masked_i8") : (bits ? "tile3d_plain_bits" : "tile3d_plain_i8");
             for (int pass = 0; pass < n && !rc; ++pass) {
-                rc = launch_tile3d_plain(h, acc, bits, 1, k, h->t + (uint64_t)pass * (uint64_t)k);
+                rc = launch_tile3d_plain(h, acc, bits, 1, k, h->t + (uint64_t)pass * (uint64_t)k, Tc3);
                 if (!rc && want_series)
                     rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);
             }
@@ -467,7 +468,7 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         const bool use_resident3 = use_3d && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident &&
                                    resident3d_supported(h, T);
         if (use_resident3 && !rc) {
-            if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M, false) == 0) {
+            if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M, false, 0) == 0) {
                 h->last_path = bits ? "resident3d_planes_bits" : "resident3d_planes_i8";
                 resident_done = true;
             } else {

@@ -49,8 +49,8 @@ size_t coupling_record3d_bytes(const ising_ctx* h);
 int launch_convert_couplings3d(ising_ctx* h, void* d_jrec);
 bool resident3d_supported(const ising_ctx* h, int T);            // L <= 64: the whole call in one cluster launch
 int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M,
-                      bool plain);                                // plain: the tile == L schedule
-int launch_tile3d_plain(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first);   // a8 in 3D, L > 64
+                      bool plain, int Tc);                        // plain: the tile == L schedule; Tc: masked coarse tiles or 0
+int launch_tile3d_plain(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, int Tc);   // a8 in 3D, L > 64
 int launch_observables3d(ising_ctx* h, bool bits, long long* d_E, long long* d_M);   // a10 on 3D tile records
 
 // ---- amsc.cu: asynchronous multi-spin coding, 32 disorder realisations per word (multi handles, R17) ----

@@ -111,11 +111,34 @@ __global__ void __launch_bounds__(kThreads3) k_observables3d(Plane3Args A, long 
     }
 }
 
+// ---- coarse tiles other than the 8^3 register tile (Tc = 2, 4, or a power of two above 8) as masked half-sweeps, as in
+// tile_planes.cu: bit j = 4 ly + px of a slice word is the site x = 8 tx + 2 px + a, y = 8 ty + ly, z = 8 tz + lz.
+__device__ __forceinline__ uint32_t coarse_mask3(int Tc, const Tile3& t, int lz, int Cc) {
+    if (Tc == 0) return 0xffffffffu;
+    if (Tc >= kT3) {                                       // a register tile lies in one coarse tile: all or nothing
+        const uint32_t par = ((uint32_t)(kT3 * t.tx) / (uint32_t)Tc + (uint32_t)(kT3 * t.ty) / (uint32_t)Tc +
+                              (uint32_t)(kT3 * t.tz + lz) / (uint32_t)Tc) & 1u;
+        return par == (uint32_t)Cc ? 0xffffffffu : 0u;
+    }
+    const uint32_t X1 = Tc == 4 ? 0xccccccccu : 0xaaaaaaaau;       // sites with odd x / Tc
+    const uint32_t Y1 = Tc == 4 ? 0xffff0000u : 0xff00ff00u;       // sites with odd y / Tc
+    const uint32_t tzp = ((uint32_t)lz / (uint32_t)Tc) & 1u;       // 8 / Tc is even: tz does not matter
+    return ((uint32_t)Cc ^ tzp) ? (X1 ^ Y1) : ~(X1 ^ Y1);
+}
+
+template <bool HASJ>
+__device__ __forceinline__ void half_sweep3_masked(const Plane3Args& A, Slice& s, int c, int lz, uint32_t g, uint32_t p_base,
+                                                   uint64_t H, uint32_t k0, uint32_t k1, uint32_t mask) {
+    const uint32_t old = s.S[c];
+    half_sweep3<kNoSpec3, HASJ>(A, s, c, lz, g, p_base, H, k0, k1);
+    s.S[c] = (s.S[c] & mask) | (old & ~mask);
+}
+
 // a8 in 3D for L > 64: the plain checkerboard (tile == L) with a launch per half-sweep over all tiles.  Face words mix
 // the two fine colours, but a word is written whole and the bits a neighbour uses in this launch (the other fine
 // colour) are the same before and after.
 template <bool BITS, bool HASJ>
-__global__ void __launch_bounds__(kThreads3) k_tile3d_plain(Plane3Args A, int c, uint64_t tt) {
+__global__ void __launch_bounds__(kThreads3) k_tile3d_plain(Plane3Args A, int c, uint64_t tt, int Tc, int Cc) {
     const uint2* lut = kByteLutGlobal.e;
     asm volatile("griddepcontrol.launch_dependents;");
     asm volatile("griddepcontrol.wait;" ::: "memory");
@@ -137,7 +160,7 @@ __global__ void __launch_bounds__(kThreads3) k_tile3d_plain(Plane3Args A, int c,
     const uint32_t z = (uint32_t)(t.tz * kT3 + lz);
     const uint32_t g = (z * B + (uint32_t)t.ty) * B + (uint32_t)t.tx;
     const uint32_t p_base = (uint32_t)(t.tx * 4) + (uint32_t)(A.L >> 1) * ((uint32_t)(t.ty * kT3) + (uint32_t)A.L * z);
-    half_sweep3<kNoSpec3, HASJ>(A, s, c, lz, g, p_base, 2 * tt + (uint64_t)c, k0, k1);
+    half_sweep3_masked<HASJ>(A, s, c, lz, g, p_base, 2 * tt + (uint64_t)c, k0, k1, coarse_mask3(Tc, t, lz, Cc));
     store_slice<BITS>(A, t, lz, s, lut);
 }
 
@@ -163,7 +186,7 @@ static void fill_accept3(Plane3Args& A, const Accept& acc) {
 }
 
 // n passes of k plain-checkerboard sweeps in 3D: 2 n k launches.
-int launch_tile3d_plain(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first) {
+int launch_tile3d_plain(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, int Tc) {
     Plane3Args A = {};
     fill_geometry3(A, h);
     fill_accept3(A, acc);
@@ -177,18 +200,20 @@ int launch_tile3d_plain(ising_ctx* h, const Accept& acc, bool bits, int n, int k
     static const int pdl = getenv("ISING_NO_PDL") ? 0 : 1;
     attr[0].val.programmaticStreamSerializationAllowed = pdl;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    for (uint64_t s = 0; s < (uint64_t)n * (uint64_t)k; ++s)
-        for (int c = 0; c < 2; ++c) {
-            const uint64_t tt = t_first + s;
-            if (A.jrec) {
-                if (bits) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<true, true>, A, c, tt));
-                else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<false, true>, A, c, tt));
-            } else {
-                if (bits) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<true, false>, A, c, tt));
-                else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<false, false>, A, c, tt));
-            }
-            count_launch();
-        }
+    for (int pass = 0; pass < n; ++pass)
+        for (int Cc = 0; Cc < (Tc ? 2 : 1); ++Cc)
+            for (int j = 0; j < k; ++j)
+                for (int c = 0; c < 2; ++c) {
+                    const uint64_t tt = t_first + (uint64_t)pass * (uint64_t)k + (uint64_t)j;
+                    if (A.jrec) {
+                        if (bits) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<true, true>, A, c, tt, Tc, Cc));
+                        else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<false, true>, A, c, tt, Tc, Cc));
+                    } else {
+                        if (bits) ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<true, false>, A, c, tt, Tc, Cc));
+                        else ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile3d_plain<false, false>, A, c, tt, Tc, Cc));
+                    }
+                    count_launch();
+                }
     ISING_CUDA_OK(cudaGetLastError());
     return 0;
 }
@@ -327,6 +352,7 @@ struct Res3Args {
     long long* E;                  // optional series (a10 after every pass): E[pass * R + r], M[pass * R + r]
     long long* M;
     int plain;                     // 1: plain checkerboard of the whole lattice (tile == L), a barrier after every half-sweep
+    int coarse;                    // with plain: coarse tile edge of a masked double checkerboard, or 0
 };
 
 template <bool BITS, bool HASJ>
@@ -415,11 +441,12 @@ __global__ void __launch_bounds__(kRes3Warps * 32) k_resident3d(Res3Args R) {
     const uint64_t seed = A.seeds[r];
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     for (int pass = 0; pass < R.n && R.plain; ++pass) {        // a8: fine colour 0 of every tile, barrier, fine colour 1, barrier
+      for (int Cc = 0; Cc < (R.coarse ? 2 : 1); ++Cc)          // (masked double checkerboard: both coarse colours in turn)
         for (int j = 0; j < A.k; ++j) {
             const uint64_t tt = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
 #pragma unroll
             for (int c = 0; c < 2; ++c) {
-                if (series && j == 0 && c == 1 && pass > 0) write_series(pass - 1);
+                if (series && Cc == 0 && j == 0 && c == 1 && pass > 0) write_series(pass - 1);
 #pragma unroll
                 for (int C = 0; C < 2; ++C)
                     if (mine) {
@@ -427,7 +454,7 @@ __global__ void __launch_bounds__(kRes3Warps * 32) k_resident3d(Res3Args R) {
                         const uint32_t z = (uint32_t)(t[C].tz * kT3 + lz);
                         const uint32_t g = (z * B + (uint32_t)t[C].ty) * B + (uint32_t)t[C].tx;
                         const uint32_t p_base = (uint32_t)(t[C].tx * 4) + (uint32_t)(A.L >> 1) * ((uint32_t)(t[C].ty * kT3) + (uint32_t)A.L * z);
-                        half_sweep3<kNoSpec3, HASJ>(A, s[C], c, lz, g, p_base, 2 * tt + (uint64_t)c, k0, k1);
+                        half_sweep3_masked<HASJ>(A, s[C], c, lz, g, p_base, 2 * tt + (uint64_t)c, k0, k1, coarse_mask3(R.coarse, t[C], lz, Cc));
                         publish(C, s[C]);
                     }
                 cluster.sync();
@@ -505,10 +532,11 @@ bool resident3d_supported(const ising_ctx* h, int T) {
 }
 
 int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M,
-                      bool plain) {
+                      bool plain, int Tc) {
     Res3Args R;
     R.E = d_E; R.M = d_M;
     R.plain = plain ? 1 : 0;
+    R.coarse = plain ? Tc : 0;
     Plane3Args& A = R.P;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;

@@ -649,3 +649,27 @@ def test_small_coarse_tiles_on_the_fast_kernels(P, orc, L, tile, k, n, beta, see
     _same_state(g, o)
     g.sweep(beta, 2, 32, 1); o.sweep(beta, 2, 32, 1)
     _same_state(g, o)
+
+
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,tile,k,n,beta,seeds,jseed,path", [
+    (16, 4, 1, 4, BC3, [4], None, "resident3d_masked"),
+    (32, 2, 2, 2, BC3, [5], None, "resident3d_masked"),
+    (32, 16, 1, 3, 0.3, [6, 7], None, "resident3d_masked"),     # coarse tiles of 2 x 2 x 2 register tiles
+    (64, 4, 1, 2, 0.9, [1, 2], 7, "resident3d_masked"),         # +-J
+    (96, 4, 1, 2, BC3, [2], None, "tile3d_masked"),
+    (128, 32, 2, 1, BC3, [3], None, "tile3d_masked"),
+])
+def test_other_coarse_tiles_3d(P, orc, L, tile, k, n, beta, seeds, jseed, path, layout):
+    """3D double checkerboard with coarse tiles other than 8 on the 8^3 register tiling (masked half-sweeps)."""
+    J = W.couplings(3, L, jseed) if jseed is not None else None
+    g, o = _both(P, orc, 3, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.sweep(beta, n, tile, k); o.sweep(beta, n, tile, k)
+    assert g.sweep_path() == f"{path}_{'i8' if layout == 'int8' else 'bits'}"
+    _same_state(g, o)
+    Eg, Mg = g.sweep_series(beta, n, tile, k)
+    Eo, Mo = o.sweep_series(beta, n, tile, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
