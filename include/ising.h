@@ -172,20 +172,26 @@ int ising_synchronize(ising_handle h);
  * (bench.py's gpu_launches). */
 uint64_t ising_kernel_launches(void);
 
-/* ising_sweep_path — name of the kernel family the last ising_sweep on h used
- * ("generic", "tile_i8", "tile_planes_i8", "tile_planes_bits", "tile3d_planes_i8", "tile3d_planes_bits",
- * "plain64_planes_i8", "plain64_planes_bits", "resident_planes_i8", "resident_planes_bits", "resident3d_planes_i8",
- * "resident3d_planes_bits", "resident_plain_i8", "resident_plain_bits", "tile_plain_i8", "tile_plain_bits", "resident3d_plain_i8/_bits", "tile3d_plain_i8/_bits", "resident_masked_i8/_bits", "tile_masked_i8/_bits", "resident3d_masked_i8/_bits", "tile3d_masked_i8/_bits", "amsc");
- * static string,
- * never NULL.  "resident_planes_*": 2D, J = +1 or +-J, at most 64 warp jobs per coarse colour (L <= 512 at tile 32 or 64),
- * n_sweeps >= 2: the whole call runs in one launch of one thread-block cluster per replica with the lattice held
- * in registers and the tile boundaries exchanged through distributed shared memory (same trajectory).
- * "resident3d_planes_*": the same for 3D, J = +1 or +-J, L <= 64.  "resident_plain_*": the plain checkerboard (tile == L)
- * of a 2D lattice with 64 < L <= 512 on the same kernel (one barrier per half-sweep); "tile_plain_*": the plain
- * checkerboard of larger 2D lattices (L a multiple of 64 with L/64 even, or of 32 with L/32 even), a launch per half-sweep.
- * "resident3d_plain_*" / "tile3d_plain_*": the plain checkerboard in 3D (L a multiple of 8 with L/8 even; L <= 64 / larger).
- * "resident_masked_*" / "tile_masked_*": 2D double checkerboard with tiles of 2, 4, 8, 16 (the paper's sizes), 128, 256, ... as masked
- * half-sweeps on the same kernels; "resident3d_masked_*" / "tile3d_masked_*": 3D tiles of 2, 4, 16, 32, ... likewise. */
+/* ising_sweep_path — name of the kernel family the last ising_sweep on h used; static string, never NULL.  Every
+ * family computes the same trajectory; names end in _i8 or _bits (the HBM layout) where both exist.
+ *   generic                 global-memory kernels, one launch per half-sweep: any valid (dim, L, tile, J)
+ *   tile_i8                 2D tiles 32 / 64, RNG mapping "words"
+ *   tile_planes_*           2D tiles 32 / 64, J = +1 or +-J, replicas: a launch per coarse colour (the headline kernel)
+ *   tile3d_planes_*         3D tiles 8, J = +1 or +-J, replicas
+ *   plain64_planes_*        L = 64 plain checkerboard, the whole call in one launch of one warp per replica
+ *   resident_planes_*       2D, at most 64 warp jobs per coarse colour (L <= 512), n_sweeps >= 2: the whole call in one
+ *                           launch of one thread-block cluster per replica, lattice in registers, tile boundaries through
+ *                           distributed shared memory, E / M of ising_sweep_series counted on the registers
+ *   resident3d_planes_*     the same in 3D, L <= 64
+ *   resident_plain_*, tile_plain_*, resident3d_plain_*, tile3d_plain_*
+ *                           the plain checkerboard (tile == L) on the cluster-resident kernels (2D 64 < L <= 512, 3D L <= 64)
+ *                           or, for larger lattices, with a launch per half-sweep
+ *   resident_masked_*, tile_masked_*, resident3d_masked_*, tile3d_masked_*
+ *                           double checkerboard with power-of-two tiles other than the register tiles (2D: 2, 4, 8, 16 —
+ *                           the paper's sizes, P:86 — and 128, 256, ...; 3D: 2, 4, 16, 32, ...) as masked half-sweeps
+ *   amsc                    asynchronous multi-spin coding of a multi-realisation batch (ising_create_multi)
+ * The fast 2D families need L % 32 == 0 (L % 64 for tile 64) and an even number of register tiles per side, the 3D ones
+ * L % 8 == 0 and L / 8 even. */
 const char* ising_sweep_path(ising_handle h);
 
 /* ising_force_path — testing aid: 0 = automatic kernel choice, 1 = always the generic
