@@ -39,6 +39,8 @@ def _energy_series(P, L, seed, beta, tile, k, n, therm, layout="int8", rng="plan
     (128, 64, 1, "int8", "planes", 300000),
     (64, 32, 1, "int8", "words", 300000),
     (64, 64, 1, "int8", "planes", 300000),       # plain checkerboard (config 1 shape)
+    (128, 128, 1, "int8", "planes", 200000),     # plain checkerboard on the cluster-resident kernel
+    (128, 16, 1, "int8", "planes", 200000),      # the paper's tile size: masked half-sweeps
 ])
 def test_energy_at_the_critical_point_matches_kaufman(P, L, tile, k, layout, rng, n):
     """<E>/N at beta_c on the periodic L x L lattice against Kaufman's exact finite-lattice value."""
