@@ -506,6 +506,43 @@ __device__ __forceinline__ void half_sweep_masked(const PlaneArgs& A, TileRegs<T
     }
 }
 
+// store_tile for a half-sweep that changed only fine colour c: that colour's pieces and the boundary copies (a plain-
+// checkerboard half-sweep then writes half the lattice, 1.5 N bytes of traffic instead of 2 N).
+template <int T, bool BITS>
+__device__ __forceinline__ void store_tile_colour(const PlaneArgs& A, int r, int tx, int ty, int Y, int sub, const TileRegs<T>& t,
+                                                  const uint2* lut, int c) {
+    using G = PG<T>;
+    constexpr uint32_t REC = BITS ? G::REC_BITS : G::REC_I8;
+    constexpr uint32_t BODY = REC - G::EDGE;
+    uint8_t* rec = A.tiles + (uint64_t)(((uint32_t)r * (uint32_t)A.B + (uint32_t)ty) * (uint32_t)A.B + (uint32_t)tx) * REC;
+    const uint64_t pol = body_policy(A.stream != 0);
+#pragma unroll
+    for (int gx = 0; gx < G::NW; ++gx) {
+        const uint32_t w = c ? t.S[1][gx] : t.S[0][gx];
+        if (BITS) {
+            *reinterpret_cast<uint32_t*>(rec + ((c * G::NW + gx) * G::LPT + Y) * 4) = w;
+        } else {
+#pragma unroll
+            for (int rp = 0; rp < 2; ++rp) {
+                const uint2 a = __ldg(lut + ((w >> (16 * rp)) & 0xffu));
+                const uint2 b = __ldg(lut + ((w >> (16 * rp + 8)) & 0xffu));
+                stg128(rec + ((((rp * 2 + c) * G::NW + gx) * G::LPT) + Y) * 16, make_uint4(a.x, a.y, b.x, b.y), pol);
+            }
+        }
+    }
+    const uint32_t sh = (uint32_t)sub * G::LPT, m = G::LPT == 32 ? 0xffffffffu : ((1u << G::LPT) - 1u);
+    const uint32_t L0 = (__ballot_sync(0xffffffffu, t.S[0][0] & 1u) >> sh) & m;
+    const uint32_t L1 = (__ballot_sync(0xffffffffu, (t.S[1][0] >> 16) & 1u) >> sh) & m;
+    const uint32_t R0 = (__ballot_sync(0xffffffffu, (t.S[1][G::NW - 1] >> 15) & 1u) >> sh) & m;
+    const uint32_t R1 = (__ballot_sync(0xffffffffu, t.S[0][G::NW - 1] >> 31) >> sh) & m;
+    if (Y == 0 || Y == G::LPT - 1) {
+        const uint4 w = G::NW == 2 ? make_uint4(t.S[0][0], t.S[0][1], t.S[1][0], t.S[1][1]) : make_uint4(t.S[0][0], t.S[1][0], 0u, 0u);
+        uint8_t* e = rec + BODY + (Y == 0 ? G::E_TOP : G::E_BOT);
+        stg128(e, w);
+        stg128(e + 16, Y == 0 ? make_uint4(L0, L1, R0, R1) : make_uint4(0u, 0u, 0u, 0u));
+    }
+}
+
 // ---- a8 for large lattices: the plain checkerboard (tile == L) with a launch per half-sweep.  Every tile of the
 // register tiling T takes part: load (neighbours' boundary copies of the other fine colour are not being changed by
 // this launch), one half-sweep of fine colour c, store.  The scheme the paper starts from: the whole lattice
@@ -539,7 +576,7 @@ __global__ void __launch_bounds__(kPlaneThreads) k_tile_planes_plain(PlaneArgs A
     const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(tx * G::NW);
     const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);
     half_sweep_masked<T, HASJ>(A, t, Jw, c, Y, g0, p0, 2 * tt + (uint64_t)c, k0, k1, Tc, Yg, (uint32_t)(tx * G::NW), Cc);
-    store_tile<T, BITS>(A, r, tx, ty, Y, sub, t, lut);
+    store_tile_colour<T, BITS>(A, r, tx, ty, Y, sub, t, lut, c);
 }
 
 // n passes of k plain-checkerboard sweeps: 2 n k launches; with coarse tiles Tc (0: none) n passes of the double
