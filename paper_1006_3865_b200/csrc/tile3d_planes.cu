@@ -134,6 +134,35 @@ __device__ __forceinline__ void half_sweep3_masked(const Plane3Args& A, Slice& s
     s.S[c] = (s.S[c] & mask) | (old & ~mask);
 }
 
+// store_slice for a half-sweep that changed only fine colour c: that colour's pieces and the face copies.
+template <bool BITS>
+__device__ __forceinline__ void store_slice_colour(const Plane3Args& A, const Tile3& t, int lz, const Slice& s, const uint2* lut, int c) {
+    constexpr int REC = BITS ? kRec3Bits : kRec3I8;
+    constexpr int BODY = BITS ? kBody3Bits : kBody3I8;
+    const int B = A.B;
+    uint8_t* rec = A.tiles + ((size_t)t.r * B * B * B + ((size_t)t.tz * B + t.ty) * B + t.tx) * REC;
+    const uint32_t w = c ? s.S[1] : s.S[0];
+    if (BITS) {
+        *reinterpret_cast<uint32_t*>(rec + (c * 8 + lz) * 4) = w;
+    } else {
+#pragma unroll
+        for (int h = 0; h < 2; ++h) {
+            const uint2 a = __ldg(lut + ((w >> (16 * h)) & 0xffu));
+            const uint2 b = __ldg(lut + ((w >> (16 * h + 8)) & 0xffu));
+            stg128(rec + ((c * 2 + h) * 8 + lz) * 16, make_uint4(a.x, a.y, b.x, b.y));
+        }
+    }
+    uint32_t XL, XR, YL, YR;
+    face_words(s.S, lz, XL, XR, YL, YR);
+    uint8_t* f = rec + BODY;
+    reinterpret_cast<uint32_t*>(f + kXL)[lz] = XL;
+    reinterpret_cast<uint32_t*>(f + kXR)[lz] = XR;
+    f[kYL + lz] = (uint8_t)YL;
+    f[kYR + lz] = (uint8_t)YR;
+    if (lz == 0) *reinterpret_cast<uint2*>(f + kZL) = make_uint2(s.S[0], s.S[1]);
+    if (lz == 7) *reinterpret_cast<uint2*>(f + kZR) = make_uint2(s.S[0], s.S[1]);
+}
+
 // a8 in 3D for L > 64: the plain checkerboard (tile == L) with a launch per half-sweep over all tiles.  Face words mix
 // the two fine colours, but a word is written whole and the bits a neighbour uses in this launch (the other fine
 // colour) are the same before and after.
@@ -161,7 +190,7 @@ __global__ void __launch_bounds__(kThreads3) k_tile3d_plain(Plane3Args A, int c,
     const uint32_t g = (z * B + (uint32_t)t.ty) * B + (uint32_t)t.tx;
     const uint32_t p_base = (uint32_t)(t.tx * 4) + (uint32_t)(A.L >> 1) * ((uint32_t)(t.ty * kT3) + (uint32_t)A.L * z);
     half_sweep3_masked<HASJ>(A, s, c, lz, g, p_base, 2 * tt + (uint64_t)c, k0, k1, coarse_mask3(Tc, t, lz, Cc));
-    store_slice<BITS>(A, t, lz, s, lut);
+    store_slice_colour<BITS>(A, t, lz, s, lut, c);
 }
 
 }  // namespace
