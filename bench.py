@@ -33,9 +33,12 @@ METRIC = "spin flips/ns (2D Ising L=16384, beta_c)"
 UNIT = "flips/ns"
 
 
-def algorithmic_bytes_per_flip(tile: int, k: int, layout: str) -> float:
-    """read s(1 + 2*dim/T) + write s per site per pass, / k; s = 1 B int8, 1/8 B bits."""
+def algorithmic_bytes_per_flip(tile: int, k: int, layout: str, L: int = 0) -> float:
+    """read s(1 + 2*dim/T) + write s per site per pass, / k; s = 1 B int8, 1/8 B bits.
+    Plain checkerboard (tile == L, row a8): each half-sweep reads every site and writes the updated half: 3 s per flip."""
     s = 1.0 if layout == "int8" else 0.125
+    if tile in (0, L):
+        return 3.0 * s
     return s * (2.0 + 4.0 / tile) / k
 
 
@@ -52,6 +55,9 @@ def measured_peaks():
 NCU = {
     ("planes", "int8", 64, 1, True): {"traffic": 138.44e6 + 79.40e6, "warp_instr": 33.78e6},
     ("planes", "int8", 64, 16, True): {"traffic": 138.44e6 + 79.33e6, "warp_instr": 391.3e6},
+    # plain checkerboard, one launch = one half-sweep of the whole lattice (profiles/r01g_tile_planes_plain_i8.md)
+    ("planes", "int8", 16384, 1, False): {"traffic": 272.66e6 + 97.58e6, "warp_instr": 52.12e6,
+                                          "source": "profiles/r01g_tile_planes_plain_i8.md"},
 }
 # Issue ceiling of the path: 148 SMs x 4 SMSPs, one warp-instruction per 2 cycles at sm_max_mhz.
 def issue_peak_gips(sm_mhz: float) -> float:
@@ -468,7 +474,7 @@ def main() -> None:
 
     peak, peak_src, sm_max = measured_peaks()
     ncu = NCU.get((a.rng, a.layout, a.tile, a.k, res["path"].endswith("+jit"))) if L == 16384 else None
-    bpf = algorithmic_bytes_per_flip(a.tile, a.k, a.layout)
+    bpf = algorithmic_bytes_per_flip(a.tile, a.k, a.layout, L)
     launches_per_step = 2
     bytes_per_launch = bpf * a.k * L * L / launches_per_step
     launch_ms = res["ms"] / (a.steps * launches_per_step)
@@ -487,7 +493,8 @@ def main() -> None:
             "ns_per_flip": 1.0 / value, "gpu_launches": res["launches"], "clocks": res["clocks"],
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": ncu["traffic"] if ncu else None,
-                         "traffic_source": "ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, profiles/r01d_tile_planes_jit_i8_t64.md" if ncu else None,
+                         "traffic_source": ("ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, "
+                                            + ncu.get("source", "profiles/r01d_tile_planes_jit_i8_t64.md")) if ncu else None,
                          "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
                          "algorithmic_bytes_per_flip": bpf, "kernel": f"{res['path']}<{a.tile}>",
                          "avg_launch_ms": launch_ms,
