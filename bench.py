@@ -511,6 +511,12 @@ def main() -> None:
                     r = time_variant(P, torch, L, lay, T, k, st, 3, None, rng)
                     table[f"{rng}_{lay}_t{T}_k{k}"] = {"flips_per_ns": round(r["flips_per_ns"], 1), "steps": st,
                                                 "hbm_GBs": round(r["flips_per_ns"] * algorithmic_bytes_per_flip(T, k, lay), 1)}
+        # the scheme the paper starts from (row a8): plain checkerboard, tile == L, a launch per half-sweep
+        for lay in ("int8", "bits"):
+            st = max(2, min(a.steps, 40))
+            r = time_variant(P, torch, L, lay, L, 1, st, 3, None, "planes")
+            table[f"planes_{lay}_plain"] = {"flips_per_ns": round(r["flips_per_ns"], 1), "steps": st, "kernel_path": r["path"],
+                                            "hbm_GBs": round(r["flips_per_ns"] * algorithmic_bytes_per_flip(L, 1, lay, L), 1)}
         line["variants"] = table
         line["e2e"] = time_e2e(P, torch, L, a.layout, a.tile, a.k, 3, a.rng)
         line["e2e_bits"] = time_e2e(P, torch, L, a.layout, a.tile, a.k, 3, a.rng, packed=True)
