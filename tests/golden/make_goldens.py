@@ -43,6 +43,9 @@ def jobs():
                           checkpoints=[1, 2]))
             J.append(dict(name=f"c3_L2048_t{T}_k{k}", dim=2, L=2048, seeds=[3], beta=BC, tile=T, k=k,
                           checkpoints=[1, 2, 50, 200]))
+    # row a8 at the bench size: plain checkerboard (tile == L) on the config-3 and config-4 lattices, two sweeps
+    J.append(dict(name="c3_L16384_plain", dim=2, L=16384, seeds=[3], beta=BC, tile=16384, k=1, checkpoints=[1, 2]))
+    J.append(dict(name="c4_plain", dim=3, L=256, seeds=[4], beta=0.2216546, tile=256, k=1, checkpoints=[1, 2]))
     # config 4: 3D L=256, tile 8
     for k in (1, 4):
         J.append(dict(name=f"c4_k{k}", dim=3, L=256, seeds=[4], beta=0.2216546, tile=8, k=k,

@@ -55,7 +55,7 @@ def test_survey_appendix_a_words(P, orc, case):
 
 PLANES_JOBS = ["c2_beta0.3", "c2_beta0.4", "c2_beta0.4406868", "c2_beta0.5", "c2_beta0.6"] + \
     [f"c3_L{L}_t{T}_k{k}" for L in (16384, 2048) for T in (32, 64) for k in (1, 4, 16)] + \
-    ["c4_k1", "c4_k4", "c5_all16", "c5_seed100", "c5_seed101", "c5_seed114", "c5_seed115"]
+    ["c3_L16384_plain", "c4_plain", "c4_k1", "c4_k4", "c5_all16", "c5_seed100", "c5_seed101", "c5_seed114", "c5_seed115"]
 
 
 @pytest.mark.parametrize("layout", ["int8", "bits"])
@@ -95,7 +95,9 @@ def test_oracle_goldens_planes(P, orc, name, layout):
                 assert g.overlap(a, b) == q
     if job["dim"] == 2 and job["tile"] in (32, 64) and job["L"] > 64:
         assert g.sweep_path() in (f"tile_planes_{'i8' if layout == 'int8' else 'bits'}", f"resident_planes_{'i8' if layout == 'int8' else 'bits'}")
-    if job["dim"] == 3:
+    if job["tile"] == job["L"]:
+        assert g.sweep_path() == ("tile_plain_" if job["dim"] == 2 else "tile3d_plain_") + ("i8" if layout == "int8" else "bits")
+    elif job["dim"] == 3:
         assert g.sweep_path() in (f"tile3d_planes_{'i8' if layout == 'int8' else 'bits'}", f"resident3d_planes_{'i8' if layout == 'int8' else 'bits'}")
     g.destroy()
 
