@@ -74,35 +74,59 @@ __global__ void __launch_bounds__(32) k_plain64_planes(PlaneArgs A, int n, long 
 }
 
 // a10 directly on the tile records (no conversion to the canonical array): one launch per coarse colour C adds
-// the colour-C tiles' share to E[r], M[r] (zeroed by the caller): warp shuffle reduction, two 64-bit atomics per tile.
+// the colour-C tiles' share to E[r], M[r] (zeroed by the caller): warp shuffle reduction over the lanes of a tile,
+// then the (up to 8) tiles of the CTA meet in shared memory and one thread adds them per replica: all CTAs add to the
+// same two words, and at L = 16384 the 65536 same-address atomics of a tile-level add cost more than reading the tiles.
 template <int T, bool BITS, bool HASJ>
 __global__ void __launch_bounds__(kPlaneThreads) k_observables_planes(PlaneArgs A, long long* __restrict__ E, long long* __restrict__ M) {
     using G = PG<T>;
+    constexpr int NT = kPlaneThreads / 32 * G::TPW;        // tiles per CTA
+    __shared__ int s_r[NT], s_up[NT], s_unsat[NT];
     const int lane = threadIdx.x & 31;
     const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (job >= A.njobs) return;
     const int sub = lane / G::LPT, Y = lane % G::LPT;
-    int r, tx, ty;
-    job_tile<T>(A, job, sub, r, tx, ty);
-    TileRegs<T> t;
-    load_tile<T, BITS>(A, r, tx, ty, Y, sub * G::LPT, t);
-    uint4 Jw[2][G::NW];
+    int r = -1, up = 0, unsat = 0;
+    if (job < A.njobs) {                                   // warp-uniform
+        int tx, ty;
+        job_tile<T>(A, job, sub, r, tx, ty);
+        TileRegs<T> t;
+        load_tile<T, BITS>(A, r, tx, ty, Y, sub * G::LPT, t);
+        uint4 Jw[2][G::NW];
 #pragma unroll
-    for (int cc = 0; cc < 2; ++cc)
+        for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
-        for (int gx = 0; gx < G::NW; ++gx)
-            Jw[cc][gx] = HASJ ? __ldg(A.jrec + ((size_t)ty * A.B + tx) * (2 * G::NW * G::LPT) + (cc * G::NW + gx) * G::LPT + Y)
-                              : make_uint4(0u, 0u, 0u, 0u);
-    int up = 0, unsat = 0;
-    count_row<T, false>(t, Jw, Y, up, unsat);
+            for (int gx = 0; gx < G::NW; ++gx)
+                Jw[cc][gx] = HASJ ? __ldg(A.jrec + ((size_t)ty * A.B + tx) * (2 * G::NW * G::LPT) + (cc * G::NW + gx) * G::LPT + Y)
+                                  : make_uint4(0u, 0u, 0u, 0u);
+        count_row<T, false>(t, Jw, Y, up, unsat);
 #pragma unroll
-    for (int d = G::LPT / 2; d > 0; d >>= 1) {           // reduce over the lanes of one tile
-        up += __shfl_xor_sync(0xffffffffu, up, d);
-        unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+        for (int d = G::LPT / 2; d > 0; d >>= 1) {           // reduce over the lanes of one tile
+            up += __shfl_xor_sync(0xffffffffu, up, d);
+            unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+        }
     }
     if (Y == 0) {
-        if (M) atomicAdd(reinterpret_cast<unsigned long long*>(M + r), (unsigned long long)(2ll * up - (long long)(T * T)));
-        if (E) atomicAdd(reinterpret_cast<unsigned long long*>(E + r), (unsigned long long)(2ll * unsat - 2ll * (T * T)));
+        const int i = (threadIdx.x >> 5) * G::TPW + sub;
+        s_r[i] = r; s_up[i] = up; s_unsat[i] = unsat;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int cr = -1;
+        long long m = 0, e = 0;
+        for (int i = 0; i <= NT; ++i) {
+            const int ri = i < NT ? s_r[i] : -1;
+            if (ri != cr) {                                 // tiles of a CTA are consecutive jobs: runs of equal r
+                if (cr >= 0) {
+                    if (M) atomicAdd(reinterpret_cast<unsigned long long*>(M + cr), (unsigned long long)m);
+                    if (E) atomicAdd(reinterpret_cast<unsigned long long*>(E + cr), (unsigned long long)e);
+                }
+                cr = ri; m = 0; e = 0;
+            }
+            if (ri >= 0) {
+                m += 2ll * s_up[i] - (long long)(T * T);
+                e += 2ll * s_unsat[i] - 2ll * (T * T);
+            }
+        }
     }
 }
 
