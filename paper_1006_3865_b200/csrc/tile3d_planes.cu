@@ -86,28 +86,49 @@ __global__ void k_convert_couplings3d(const int8_t* __restrict__ J, uint32_t* __
 }
 
 // a10 directly on the 3D tile records: one launch per coarse colour C adds the colour-C tiles' share to E[r], M[r]
-// (zeroed by the caller); the four tiles of a warp job belong to one replica (B^3/2 is a multiple of 4).
+// (zeroed by the caller); the four tiles of a warp job belong to one replica (B^3/2 is a multiple of 4).  The warps of a
+// CTA meet in shared memory and one thread adds per replica (every CTA adds to the same two words: fewer, larger adds).
+constexpr int kObs3Warps = 8;
 template <bool BITS, bool HASJ>
-__global__ void __launch_bounds__(kThreads3) k_observables3d(Plane3Args A, long long* __restrict__ E, long long* __restrict__ M) {
-    const int lane = threadIdx.x & 31;
-    const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-    if (job >= A.njobs) return;
-    const int sub = lane >> 3, lz = lane & 7;
-    const Tile3 t = job_tile3(A, job * 4u + (uint32_t)sub);
-    Slice s;
-    load_slice<BITS>(A, t, lz, s);
-    load_couplings<HASJ>(A, t, lz, s);
-    int up = 0, unsat = 0;
-    count_slice<HASJ>(s, lz, up, unsat);
+__global__ void __launch_bounds__(kObs3Warps * 32) k_observables3d(Plane3Args A, long long* __restrict__ E, long long* __restrict__ M) {
+    __shared__ int s_r[kObs3Warps], s_up[kObs3Warps], s_unsat[kObs3Warps];
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (uint32_t)w;
+    int r = -1, up = 0, unsat = 0;
+    if (job < A.njobs) {                                   // warp-uniform
+        const int sub = lane >> 3, lz = lane & 7;
+        const Tile3 t = job_tile3(A, job * 4u + (uint32_t)sub);
+        Slice s;
+        load_slice<BITS>(A, t, lz, s);
+        load_couplings<HASJ>(A, t, lz, s);
+        count_slice<HASJ>(s, lz, up, unsat);
 #pragma unroll
-    for (int d = 16; d > 0; d >>= 1) {
-        up += __shfl_xor_sync(0xffffffffu, up, d);
-        unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+        for (int d = 16; d > 0; d >>= 1) {
+            up += __shfl_xor_sync(0xffffffffu, up, d);
+            unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+        }
+        r = __shfl_sync(0xffffffffu, t.r, 0);
     }
-    if (lane == 0) {
+    if (lane == 0) { s_r[w] = r; s_up[w] = up; s_unsat[w] = unsat; }
+    __syncthreads();
+    if (threadIdx.x == 0) {
         const long long sites = 4ll * kT3 * kT3 * kT3;
-        if (M) atomicAdd(reinterpret_cast<unsigned long long*>(M + t.r), (unsigned long long)(2ll * up - sites));
-        if (E) atomicAdd(reinterpret_cast<unsigned long long*>(E + t.r), (unsigned long long)(2ll * unsat - 3ll * sites));
+        int cr = -1;
+        long long m = 0, e = 0;
+        for (int i = 0; i <= kObs3Warps; ++i) {
+            const int ri = i < kObs3Warps ? s_r[i] : -1;
+            if (ri != cr) {                                 // consecutive jobs: runs of equal r
+                if (cr >= 0) {
+                    if (M) atomicAdd(reinterpret_cast<unsigned long long*>(M + cr), (unsigned long long)m);
+                    if (E) atomicAdd(reinterpret_cast<unsigned long long*>(E + cr), (unsigned long long)e);
+                }
+                cr = ri; m = 0; e = 0;
+            }
+            if (ri >= 0) {
+                m += 2ll * s_up[i] - sites;
+                e += 2ll * s_unsat[i] - 3ll * sites;
+            }
+        }
     }
 }
 
@@ -254,7 +275,7 @@ int launch_observables3d(ising_ctx* h, bool bits, long long* d_E, long long* d_M
     if (d_M) ISING_CUDA_OK(cudaMemsetAsync(d_M, 0, sizeof(long long) * h->R, st));
     Plane3Args A = {};
     fill_geometry3(A, h);
-    const int warps = kThreads3 / 32;
+    const int warps = kObs3Warps;
     const uint32_t grid = (A.njobs + warps - 1) / warps;
     for (int C = 0; C < 2; ++C) {
         A.C = C;
