@@ -50,10 +50,14 @@ def jobs():
     for k in (1, 4):
         J.append(dict(name=f"c4_k{k}", dim=3, L=256, seeds=[4], beta=0.2216546, tile=8, k=k,
                       checkpoints=[1, 10, 100, 500]))
-    # config 5: ±J glass L=4096, 16 replicas to 10 passes, 4 replicas to 100
+    # config 5: ±J glass L=4096 at the depth SURVEY §8(d) lists: all 16 replicas (with the 120 overlaps) to 100 passes,
+    # two replicas in full (1000 passes), two more to 100
     J.append(dict(name="c5_all16", dim=2, L=4096, seeds=list(range(100, 116)), jseed=5, beta=1.0, tile=32, k=4,
-                  checkpoints=[1, 10], overlaps=True))
-    for sd in (100, 101, 114, 115):
+                  checkpoints=[1, 10, 100], overlaps=True))
+    for sd in (100, 101):
+        J.append(dict(name=f"c5_seed{sd}", dim=2, L=4096, seeds=[sd], jseed=5, beta=1.0, tile=32, k=4,
+                      checkpoints=[1, 10, 100, 1000]))
+    for sd in (114, 115):
         J.append(dict(name=f"c5_seed{sd}", dim=2, L=4096, seeds=[sd], jseed=5, beta=1.0, tile=32, k=4,
                       checkpoints=[1, 10, 100]))
     return J
