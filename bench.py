@@ -50,8 +50,19 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
 
 
-# From the committed ncu captures (profiles/r01d_tile_planes_jit_i8_t64.md), per launch of the kernel:
-# DRAM bytes read + written, and executed warp-instructions.  Keyed by (rng, layout, tile, k, jit).
+def kernel_fingerprint() -> str:
+    """sha1 (12 hex digits) over the sources of the headline kernel: an ncu figure quoted below is only printed while the
+    kernel it was captured from is the kernel being timed."""
+    import hashlib
+    h = hashlib.sha1()
+    for n in ("philox.cuh", "planes_common.cuh", "tile_planes_device.cuh", "tile_planes.cu"):
+        h.update(open(os.path.join(ROOT, "paper_1006_3865_b200", "csrc", n), "rb").read())
+    return h.hexdigest()[:12]
+
+
+# From the committed ncu captures, per launch of the kernel: DRAM bytes read + written, and executed warp-instructions.
+# Keyed by (rng, layout, tile, k, jit); "fingerprint" = kernel_fingerprint() of the sources the capture was taken from.
+NCU_FINGERPRINT = "335e7167c47f"
 NCU = {
     ("planes", "int8", 64, 1, True): {"traffic": 138.44e6 + 79.40e6, "warp_instr": 33.78e6},
     ("planes", "int8", 64, 16, True): {"traffic": 138.44e6 + 79.33e6, "warp_instr": 391.3e6},
@@ -87,6 +98,12 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.rows.append((time.time(), line.strip()))
 
+    def wait_first_row(self, timeout: float) -> None:
+        """nvidia-smi needs a few hundred ms before its first row: do not start the timed region without one."""
+        t = time.time()
+        while self.proc is not None and not self.rows and time.time() - t < timeout:
+            time.sleep(0.02)
+
     def stop(self, t0: float, t1: float):
         if self.proc is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
@@ -94,7 +111,9 @@ class ClockSampler:
         self.proc.terminate()
         sm, mx, reasons = [], None, set()
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        rows = [r for r in self.rows if t0 - 0.05 <= r[0] <= t1 + 0.15] or self.rows
+        rows = [r for r in self.rows if t0 - 0.05 <= r[0] <= t1 + 0.15]
+        if len(rows) < 2:            # a timed region shorter than the sampling period: the rows around it
+            rows = [r for r in self.rows if t0 - 0.3 <= r[0] <= t1 + 0.3] or self.rows
         for _, line in rows:
             f = [x.strip() for x in line.split(",")]
             try:
@@ -167,12 +186,18 @@ def selftest_ranks(rank: int, world: int) -> None:
 JIT = "auto"     # --jit: run-time specialisation of the planes kernel (ising_set_jit)
 
 
-def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng="planes"):
-    """Device-timed throughput of one (rng, layout, tile, k) variant; returns dict."""
+def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng="planes", min_seconds=0.0, max_reps=1):
+    """Device-timed throughput of one (rng, layout, tile, k) variant; returns dict.
+
+    One repetition = one `ising_sweep(steps)` call = exactly `steps` outer passes (2 launches each, no host sync inside),
+    bracketed by CUDA events on the library's stream.  The repetition is repeated back to back until `min_seconds` of GPU
+    time have elapsed (at most `max_reps` times): `ms` is the MEDIAN repetition, `ms_min` / `ms_max` the spread.  The
+    clock sampler (if any) runs from before the warm-up to after the last repetition, so that it has rows however short a
+    repetition is (20 steps are 2.4 ms)."""
     g = P.Ising(2, L, seed=3, rng=rng)
     # the library's AUTO rule (specialise calls of >= 2^27 attempted flips), decided here for the timed call so that
     # the warm-up call, which is shorter, already compiles the kernel the timed call will use
-    # (lattices small enough for the cluster-resident kernel, <= 64 warp jobs per colour, stay on AUTO: it serves them)
+    # (lattices small enough for the resident kernels stay on AUTO: they serve them)
     resident = tile in (32, 64) and (L // tile) ** 2 // 2 // (64 // tile) <= 64 and steps >= 2
     if not resident:
         g.set_jit("on" if JIT == "on" or (JIT == "auto" and steps * k * L * L >= 2 ** 27) else "off")
@@ -180,28 +205,40 @@ def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng=
         g.set_jit(JIT)
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
+    if sampler:
+        sampler.start()
     g.sweep(W.BETA_C_2D, warmup, tile, k)
     g.synchronize()
     torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if sampler:
+        sampler.wait_first_row(3.0)
     n0 = P.ising_kernel_launches()
     t0 = time.time()
-    if sampler:
-        sampler.start()
-        time.sleep(0.25)
-        t0 = time.time()
-    e0.record()
-    g.sweep(W.BETA_C_2D, steps, tile, k)        # K passes = 2K launches, no host sync in between
-    e1.record()
-    torch.cuda.synchronize()
+    events, total, reps = [], 0.0, 0
+    while True:
+        batch = []
+        for _ in range(1 if reps == 0 else min(max_reps - reps, max(1, int(0.25 * reps / max(total, 1e-6))))):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            g.sweep(W.BETA_C_2D, steps, tile, k)        # K passes = 2K launches, no host sync in between
+            e1.record()
+            batch.append((e0, e1))
+        torch.cuda.synchronize()
+        ms_batch = [a.elapsed_time(b) for a, b in batch]
+        events += ms_batch
+        total += sum(ms_batch) / 1e3
+        reps += len(batch)
+        if total >= min_seconds or reps >= max_reps:
+            break
     t1 = time.time()
-    ms = e0.elapsed_time(e1)
+    launches = (P.ising_kernel_launches() - n0) // reps
     clocks = sampler.stop(t0, t1) if sampler else None
-    launches = P.ising_kernel_launches() - n0
     path = g.sweep_path() + ("+jit" if g.last_sweep_specialized() else "")
     g.destroy()
     flips = steps * k * L * L
-    return {"ms": ms, "flips_per_ns": flips / (ms * 1e6), "launches": int(launches), "path": path, "clocks": clocks}
+    ms = float(np.median(events))
+    return {"ms": ms, "ms_min": float(min(events)), "ms_max": float(max(events)), "reps": reps, "gpu_seconds": total,
+            "flips_per_ns": flips / (ms * 1e6), "launches": int(launches), "path": path, "clocks": clocks}
 
 
 def time_e2e(P, torch, L, layout, tile, k, steps, rng="planes", packed=False):
@@ -420,6 +457,8 @@ def main() -> None:
     ap.add_argument("--k", type=int, default=1)
     ap.add_argument("--rng", default="planes", choices=["planes", "words"], help="RNG->site mapping (DESIGN.md R6)")
     ap.add_argument("--L", type=int, default=16384)
+    ap.add_argument("--min-seconds", type=float, default=1.0,
+                    help="repeat the timed K-step call back to back until this much GPU time has elapsed; value = median repetition")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the k/tile table")
     ap.add_argument("--jit", default="auto", choices=["auto", "on", "off"], help="run-time kernel specialisation (ising_set_jit)")
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5], help="time another BASELINE config (default 3 = the headline run)")
@@ -468,12 +507,15 @@ def main() -> None:
 
     barrier()
     sampler = ClockSampler(local) if rank == 0 else None
-    res = time_variant(P, torch, L, a.layout, a.tile, a.k, a.steps, a.warmup, sampler, a.rng)
+    res = time_variant(P, torch, L, a.layout, a.tile, a.k, a.steps, a.warmup, sampler, a.rng, min_seconds=a.min_seconds, max_reps=2000)
     barrier()
     ms, value = aggregate_replicas(res["ms"], world, a.steps, a.k, L, dist, "cuda")
 
     peak, peak_src, sm_max = measured_peaks()
     ncu = NCU.get((a.rng, a.layout, a.tile, a.k, res["path"].endswith("+jit"))) if L == 16384 else None
+    ncu_stale = ncu is not None and kernel_fingerprint() != NCU_FINGERPRINT
+    if ncu_stale:            # the kernel changed since the capture: quote nothing from it
+        ncu = None
     bpf = algorithmic_bytes_per_flip(a.tile, a.k, a.layout, L)
     launches_per_step = 2
     bytes_per_launch = bpf * a.k * L * L / launches_per_step
@@ -491,16 +533,22 @@ def main() -> None:
                              else f"lattice ({lat_bytes / 2 ** 20:g} MiB {a.layout}) fits L2: not an HBM claim",
                        "kernel_path": res["path"], "parallelism": "replicas only" if world > 1 else "single GPU"},
             "ns_per_flip": 1.0 / value, "gpu_launches": res["launches"], "clocks": res["clocks"],
+            "repetitions": {"n": res["reps"], "each": f"one ising_sweep({a.steps}) call = exactly {a.steps} steps, CUDA events around it",
+                            "reported": "median", "gpu_seconds": res["gpu_seconds"],
+                            "value_min": a.steps * a.k * L * L / (res["ms_max"] * 1e6) * world,
+                            "value_max": a.steps * a.k * L * L / (res["ms_min"] * 1e6) * world},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": ncu["traffic"] if ncu else None,
                          "traffic_source": ("ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, "
                                             + ncu.get("source", "profiles/r01d_tile_planes_jit_i8_t64.md")) if ncu else None,
+                         "traffic_stale": ncu_stale,
                          "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
                          "algorithmic_bytes_per_flip": bpf, "kernel": f"{res['path']}<{a.tile}>",
                          "avg_launch_ms": launch_ms,
                          "issue": ({"bound": "alu", "unit": "G warp-instr/s", "achieved": ncu["warp_instr"] / (launch_ms * 1e6),
                                     "peak": issue_peak_gips(sm_max), "frac": ncu["warp_instr"] / (launch_ms * 1e6) / issue_peak_gips(sm_max),
-                                    "note": "DESIGN.md 7.3: IMAD.WIDE and LOP3 do not overlap on sm_100a, 2 SMSP-cycles per warp-instruction"}
+                                    "kind": "model",
+                                    "note": "DESIGN.md 7.3 / profiles/r02_microbench.md: a cost model fitted to microbenchmarks, not a hardware limit"}
                                    if ncu else None)}}
     if rank == 0 and not a.no_extras and world == 1:
         table = {}
@@ -508,13 +556,13 @@ def main() -> None:
             for T in (32, 64):
                 for k in (1, 4, 16):
                     st = max(2, min(a.steps, 40 // k))
-                    r = time_variant(P, torch, L, lay, T, k, st, 3, None, rng)
-                    table[f"{rng}_{lay}_t{T}_k{k}"] = {"flips_per_ns": round(r["flips_per_ns"], 1), "steps": st,
+                    r = time_variant(P, torch, L, lay, T, k, st, 3, None, rng, min_seconds=0.25, max_reps=400)
+                    table[f"{rng}_{lay}_t{T}_k{k}"] = {"flips_per_ns": round(r["flips_per_ns"], 1), "steps": st, "reps": r["reps"],
                                                 "hbm_GBs": round(r["flips_per_ns"] * algorithmic_bytes_per_flip(T, k, lay), 1)}
         # the scheme the paper starts from (row a8): plain checkerboard, tile == L, a launch per half-sweep
         for lay in ("int8", "bits"):
             st = max(2, min(a.steps, 40))
-            r = time_variant(P, torch, L, lay, L, 1, st, 3, None, "planes")
+            r = time_variant(P, torch, L, lay, L, 1, st, 3, None, "planes", min_seconds=0.25, max_reps=400)
             table[f"planes_{lay}_plain"] = {"flips_per_ns": round(r["flips_per_ns"], 1), "steps": st, "kernel_path": r["path"],
                                             "hbm_GBs": round(r["flips_per_ns"] * algorithmic_bytes_per_flip(L, 1, lay, L), 1)}
         line["variants"] = table
