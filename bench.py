@@ -198,7 +198,7 @@ def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng=
     # the library's AUTO rule (specialise calls of >= 2^27 attempted flips), decided here for the timed call so that
     # the warm-up call, which is shorter, already compiles the kernel the timed call will use
     # (lattices small enough for the resident kernels stay on AUTO: they serve them)
-    resident = tile in (32, 64) and (L // tile) ** 2 // 2 // (64 // tile) <= 64 and steps >= 2
+    resident = tile in (32, 64) and (L // tile) ** 2 // 2 // (64 // tile) <= 64 and steps >= 2     # cluster-resident kernel: no specialised form
     if not resident:
         g.set_jit("on" if JIT == "on" or (JIT == "auto" and steps * k * L * L >= 2 ** 27) else "off")
     else:

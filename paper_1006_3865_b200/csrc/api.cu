@@ -214,6 +214,8 @@ void ising_destroy(ising_handle h) {
     dev_free(h->d_tiles);
     dev_free(h->d_Jtiles);
     dev_free(h->d_amsc_J);
+    dev_free(h->d_xedge);
+    dev_free(h->d_gacc);
     dev_free(h->d_obs);
     dev_free(h->d_flag);
     delete h;
@@ -481,6 +483,34 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
                 resident_done = true;
             } else {
                 cudaGetLastError();      // the cluster did not fit (shared or partitioned GPU): a launch per colour instead
+            }
+        }
+        // 2D lattices beyond the cluster (more than 64 jobs per colour) that still fit on chip: one cooperative launch, tiles in
+        // the shared memory / registers of all SMs, boundary words exchanged through L2 (k_grid_planes)
+        const bool use_grid = use_planes && !resident_done && n >= 2 && !h->no_resident &&
+                              !resident_planes_supported(h, T) && grid_planes_supported(h, T);
+        if (use_grid && !rc) {
+            const size_t xb = grid_planes_xedge_bytes(h, T), ab = want_series ? grid_planes_acc_bytes(h, n) : 0;
+            if (xb > h->xedge_bytes) {
+                cudaStreamSynchronize(st);
+                dev_free(h->d_xedge); h->xedge_bytes = 0;
+                h->d_xedge = dev_alloc(xb);
+                if (!h->d_xedge) rc = ISING_ENOMEM; else h->xedge_bytes = xb;
+            }
+            if (!rc && ab > h->gacc_bytes) {
+                cudaStreamSynchronize(st);
+                dev_free(h->d_gacc); h->gacc_bytes = 0;
+                h->d_gacc = dev_alloc(ab);
+                if (!h->d_gacc) rc = ISING_ENOMEM; else h->gacc_bytes = ab;
+            }
+            if (!rc) {
+                const int g = launch_grid_planes(h, acc, T, bits, n, k, h->t, h->d_xedge, h->d_gacc, d_E, d_M, use_jit);
+                if (g == 0) {
+                    h->last_path = bits ? "grid_planes_bits" : "grid_planes_i8";
+                    resident_done = true;
+                } else if (g != 1) {
+                    cudaGetLastError();      // the cooperative launch was refused (shared or partitioned GPU): a launch per colour instead
+                }
             }
         }
         for (int pass = 0; pass < n && !rc && !resident_done; ++pass) {

@@ -100,6 +100,10 @@ struct ising_ctx {
     void* d_tiles = nullptr;        // tile-record storage (TileI8 / PlaneI8 / PlaneBits)
     size_t tiles_bytes = 0;
     void* d_amsc_J = nullptr;       // JX, JY word lattices of a multi handle (2*N words), built on first use
+    void* d_xedge = nullptr;        // k_grid_planes: boundary-word exchange records (128 B per tile)
+    size_t xedge_bytes = 0;
+    void* d_gacc = nullptr;         // k_grid_planes: per-pass accumulators of a series call
+    size_t gacc_bytes = 0;
     void* d_Jtiles = nullptr;       // couplings in tile-record form for store_tile
     int Jtiles_tile = 0;
     int Jtiles_kind = -1;

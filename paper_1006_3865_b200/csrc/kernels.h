@@ -39,6 +39,12 @@ int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, in
                            long long* d_E, long long* d_M, bool plain, int Tc);   // d_E / d_M: optional series, n * R values each;
                                                                            // plain: the tile == L schedule, T = register tiling only
 
+bool grid_planes_supported(const ising_ctx* h, int T);          // 512 < L <= ~4096: the whole call in one launch, every tile in registers on all SMs
+size_t grid_planes_xedge_bytes(const ising_ctx* h, int T);
+size_t grid_planes_acc_bytes(const ising_ctx* h, int n);
+int launch_grid_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, void* d_xedge, void* d_acc,
+                       long long* d_E, long long* d_M, bool use_jit);     // returns 1 (nothing launched) if the lattice does not fit
+
 // ---- tile3d_planes.cu: 3D multi-spin tile kernel, 8x8x8 tiles (RNG mapping "planes") ----------
 bool tile3d_supported(const ising_ctx* h, int T);
 size_t tile3d_bytes(const ising_ctx* h, bool bits);
@@ -64,6 +70,7 @@ int launch_amsc_pass(ising_ctx* h, const Accept& acc, int T, int k, uint64_t t_f
 // ---- planes_jit.cu: run-time specialisation of k_tile_planes on the threshold head bits (NVRTC) ----
 cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R);
 cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3);   // nullptr: not available
+cudaKernel_t grid_jit_kernel(int T, bool bits, bool hasj, uint32_t hp);   // k_grid_planes specialised on the threshold heads
 uint64_t planes_jit_compiled();
 const char* planes_jit_last_log();
 

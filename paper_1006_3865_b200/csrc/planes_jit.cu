@@ -139,6 +139,13 @@ cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, 
     return cached(kJitSource, expr, {"-DISING_JIT_B=" + std::to_string(B) + "u", "-DISING_JIT_R=" + std::to_string(R) + "u"});
 }
 
+// The grid-resident 2D kernel (grid_planes_device.cuh) specialised for (T, BITS, HASJ, HP); geometry stays a run-time argument.
+cudaKernel_t grid_jit_kernel(int T, bool bits, bool hasj, uint32_t hp) {
+    char expr[160];
+    snprintf(expr, sizeof expr, "ising::jit::k_grid_planes<%d, %s, %s, %uu>", T, bits ? "true" : "false", hasj ? "true" : "false", hp);
+    return cached(kJitSource, expr, {});
+}
+
 // The 3D kernel specialised for (BITS, HP3 = the three threshold heads).
 cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3) {
     char expr[160];

@@ -25,6 +25,7 @@
 
 #include "kernels.h"
 #include "tile_planes_device.cuh"
+#include "grid_planes_device.cuh"
 
 namespace ising {
 
@@ -923,6 +924,115 @@ int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, in
     if (rc) return rc;
     ISING_CUDA_OK(cudaGetLastError());
     return 0;
+}
+
+// E[p][r] = 2 #unsat - 2N, M[p][r] = 2 #up - N from the slot copies of the accumulators
+__global__ void k_grid_series_finish(const long long* __restrict__ acc, long long* __restrict__ E, long long* __restrict__ Mo,
+                                     uint32_t count, long long nsites) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;          // pass * R + r
+    if (i >= count) return;
+    long long up = 0, unsat = 0;
+    for (int s = 0; s < kGridAccSlots; ++s) { up += acc[((size_t)i * kGridAccSlots + s) * 2]; unsat += acc[((size_t)i * kGridAccSlots + s) * 2 + 1]; }
+    if (Mo) Mo[i] = 2 * up - nsites;
+    if (E) E[i] = 2 * unsat - 2 * nsites;
+}
+
+namespace {
+constexpr uint32_t kGridMaxJobsPerWarp = 16;
+
+template <int T, bool BITS, bool HASJ>
+int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit) {
+    // specialised on the threshold head bits (planes_jit.cu) when asked for and available
+    cudaKernel_t spec = (use_jit && !R.P.force) ? grid_jit_kernel(T, BITS, HASJ, R.P.hp) : nullptr;
+    const void* fn = spec ? (const void*)spec : (const void*)k_grid_planes<T, BITS, HASJ>;
+    *used_jit = spec != nullptr;
+    int dev = 0, sms = 0;
+    ISING_CUDA_OK(cudaGetDevice(&dev));
+    ISING_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    if (spec) ISING_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    else if (int rc = set_max_dynamic_smem<k_grid_planes<T, BITS, HASJ>>(200 * 1024)) return rc;
+    *fits = false;
+    static const uint32_t warp_cap = getenv("ISING_GRID_WARPS") ? (uint32_t)atoi(getenv("ISING_GRID_WARPS")) : 0u;   // testing aid: several jobs per warp on small lattices
+    for (uint32_t M = 1; M <= kGridMaxJobsPerWarp; ++M) {
+        const uint32_t warps_needed = (R.jobs_total + M - 1) / M;
+        // few jobs: one warp per CTA, so that the CTAs (and the schedulers they land on) spread over all SMs
+        const int wpb = warps_needed <= (uint32_t)sms * 4u ? 1 : (warps_needed <= (uint32_t)sms * 8u ? 2 : 4);
+        const size_t smem = (size_t)wpb * 2u * M * (2u * PG<T>::NW) * 32u * sizeof(uint32_t);
+        if (smem > 200 * 1024) break;
+        int occ = 0;
+        ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, wpb * 32, smem));
+        const uint32_t grid = (warps_needed + wpb - 1) / wpb;
+        if (grid > (uint32_t)sms * (uint32_t)occ) continue;      // not co-resident: more jobs per warp
+        if (warp_cap && warps_needed > warp_cap && M < kGridMaxJobsPerWarp) continue;
+        R.jobs_per_warp = M;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(wpb * 32); cfg.dynamicSmemBytes = smem; cfg.stream = hooks().stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        void* args[] = {&R};
+        ISING_CUDA_OK(cudaLaunchKernelExC(&cfg, fn, args));
+        count_launch();
+        *fits = true;
+        return 0;
+    }
+    return 0;
+}
+}  // namespace
+
+size_t grid_planes_xedge_bytes(const ising_ctx* h, int T) { return (size_t)h->R * (size_t)(h->L / T) * (size_t)(h->L / T) * 128; }
+size_t grid_planes_acc_bytes(const ising_ctx* h, int n) { return (size_t)n * (size_t)h->R * kGridAccSlots * 2 * sizeof(long long); }
+
+// n passes in one cooperative launch; returns 1 if the lattice does not fit the register files of the GPU (nothing launched).
+// d_xedge: grid_planes_xedge_bytes; d_acc: grid_planes_acc_bytes(n) if a series is wanted, else nullptr.
+int launch_grid_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, void* d_xedge, void* d_acc,
+                       long long* d_E, long long* d_M, bool use_jit) {
+    GridArgs R;
+    PlaneArgs& A = R.P;
+    A.tiles = (uint8_t*)h->d_tiles;
+    A.seeds = h->d_sweep_seeds;
+    A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0;
+    A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
+    A.stream = 0;
+    A.njobs = 0;
+    A.magic_rep = fastdiv_magic((uint32_t)A.B * (uint32_t)A.B / 2u);
+    A.magic_hb = fastdiv_magic((uint32_t)A.B / 2u);
+    fill_accept(A, acc);
+    R.n = n;
+    R.jobs_per_warp = 1;
+    R.tiles_per_colour = (uint32_t)A.B * (uint32_t)A.B / 2u;
+    R.jobs_total = (uint32_t)h->R * R.tiles_per_colour / (uint32_t)(64 / T);
+    R.xedge = (unsigned long long*)d_xedge;
+    const bool series = (d_E || d_M) && n > 0;
+    R.acc = series ? (long long*)d_acc : nullptr;
+    cudaStream_t st = hooks().stream;
+    ISING_CUDA_OK(cudaMemsetAsync(d_xedge, 0, grid_planes_xedge_bytes(h, T), st));     // version 0 = nothing published
+    if (series) ISING_CUDA_OK(cudaMemsetAsync(d_acc, 0, grid_planes_acc_bytes(h, n), st));
+    bool fits = false, used = false;
+    int rc;
+    if (A.jrec) rc = T == 64 ? (bits ? launch_grid_one<64, true, true>(R, use_jit, &fits, &used) : launch_grid_one<64, false, true>(R, use_jit, &fits, &used))
+                             : (bits ? launch_grid_one<32, true, true>(R, use_jit, &fits, &used) : launch_grid_one<32, false, true>(R, use_jit, &fits, &used));
+    else rc = T == 64 ? (bits ? launch_grid_one<64, true, false>(R, use_jit, &fits, &used) : launch_grid_one<64, false, false>(R, use_jit, &fits, &used))
+                      : (bits ? launch_grid_one<32, true, false>(R, use_jit, &fits, &used) : launch_grid_one<32, false, false>(R, use_jit, &fits, &used));
+    if (rc) return rc;
+    if (!fits) return 1;
+    h->last_jit = used ? 1 : 0;
+    if (series) {
+        const uint32_t count = (uint32_t)n * (uint32_t)h->R;
+        k_grid_series_finish<<<(count + 255) / 256, 256, 0, st>>>((const long long*)d_acc, d_E, d_M, count, (long long)h->N);
+        count_launch();
+    }
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+bool grid_planes_supported(const ising_ctx* h, int T) {
+    if (!tile_planes_supported(h, T)) return false;
+    // the version counter is 32 bits wide: 2 n + 1 versions per call (n < 2^31) always fit; whether the state fits the shared
+    // memory of the resident warps is decided at launch (launch_grid_planes returns 1 if it does not)
+    const uint64_t jobs = (uint64_t)h->R * (uint64_t)(h->L / T) * (uint64_t)(h->L / T) / 2u / (uint64_t)(64 / T);
+    return jobs <= 148u * 32u * kGridMaxJobsPerWarp;
 }
 
 }  // namespace ising

@@ -94,7 +94,8 @@ def test_oracle_goldens_planes(P, orc, name, layout):
                 a, b = (int(v) for v in key.split(","))
                 assert g.overlap(a, b) == q
     if job["dim"] == 2 and job["tile"] in (32, 64) and job["L"] > 64:
-        assert g.sweep_path() in (f"tile_planes_{'i8' if layout == 'int8' else 'bits'}", f"resident_planes_{'i8' if layout == 'int8' else 'bits'}")
+        sfx = "i8" if layout == "int8" else "bits"
+        assert g.sweep_path() in (f"tile_planes_{sfx}", f"resident_planes_{sfx}", f"grid_planes_{sfx}")
     if job["tile"] == job["L"]:
         assert g.sweep_path() == ("tile_plain_" if job["dim"] == 2 else "tile3d_plain_") + ("i8" if layout == "int8" else "bits")
     elif job["dim"] == 3:

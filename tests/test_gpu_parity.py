@@ -430,7 +430,7 @@ def test_cluster_resident_kernel_matches_oracle(P, orc, L, tile, k, n, beta, see
     if L == 512 and tile == 32 and layout == "int8":                # larger lattices keep the per-pass kernels
         big = P.Ising(2, 1024, seed=1)
         big.sweep(beta, 2, 32, 1)
-        assert big.sweep_path() == "tile_planes_i8"
+        assert big.sweep_path() == "grid_planes_i8"             # ... of the grid-resident kernel (test_grid_resident_*)
     g.sweep(beta, 1, tile, k); o.sweep(beta, 1, tile, k)          # a single pass goes through the per-pass kernel and composes
     assert g.sweep_path().startswith("tile_planes")
     g.sweep(beta, 2, tile, k); o.sweep(beta, 2, tile, k)
@@ -673,3 +673,73 @@ def test_other_coarse_tiles_3d(P, orc, L, tile, k, n, beta, seeds, jseed, path, 
     Eo, Mo = o.sweep_series(beta, n, tile, k)
     assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
     _same_state(g, o)
+
+
+GRID = [
+    # L, tile, k, n, beta, seeds, jseed: more than 64 warp jobs per colour -> the grid-resident kernel (one cooperative launch)
+    (1024, 32, 4, 3, BC2, [2], None),          # config 2 shape
+    (1024, 64, 1, 4, BC2, [3], None),
+    (768, 32, 2, 3, 0.3, [5, 6], None),        # replicas; B = 24
+    (704, 32, 1, 5, BC2, [9], None),           # B = 22: 121 jobs per colour, ragged against every CTA size
+    (1152, 64, 2, 2, 0.6, [8], None),          # B = 18
+    (640, 32, 2, 3, 1.0, [100, 101], 5),       # +-J glass, replicas share the coupling records
+    (768, 64, 1, 3, 0.8, [7], 11),
+    (2048, 32, 1, 2, BC2, [3], None),          # 1024 jobs per colour
+    (1024, 32, 2, 2, 0.0, [2], None),          # beta = 0: every proposal accepted
+    (1024, 64, 2, 2, 30.0, [2], None),         # thresholds underflow to 0
+]
+
+
+@pytest.mark.parametrize("jit", ["off", "on"])
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,tile,k,n,beta,seeds,jseed", GRID)
+def test_grid_resident_kernel_matches_oracle(P, orc, L, tile, k, n, beta, seeds, jseed, layout, jit):
+    """512 < L <= 4096 (the paper's own sizes), n >= 2 passes: one cooperative launch, every tile on chip for the
+    whole call, boundary words exchanged through versioned 64-bit words in L2 (k_grid_planes).  Pre-compiled and run-time
+    specialised kernels; with and without the E/M series; composing with the per-pass kernels."""
+    J = W.couplings(2, L, jseed) if jseed is not None else None
+    g, o = _both(P, orc, 2, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.set_jit(jit)
+    sfx = "i8" if layout == "int8" else "bits"
+    g.sweep(beta, n, tile, k); o.sweep(beta, n, tile, k)
+    assert g.sweep_path() == f"grid_planes_{sfx}"
+    assert g.last_sweep_specialized() == (jit == "on" and beta > 0)
+    _same_state(g, o)
+    Eg, Mg = g.sweep_series(beta, n + 1, tile, k)                 # E and M after every pass, counted on the registers
+    assert g.sweep_path() == f"grid_planes_{sfx}"
+    Eo, Mo = o.sweep_series(beta, n + 1, tile, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    g.sweep(beta, 1, tile, k); o.sweep(beta, 1, tile, k)          # a single pass: the per-pass kernel, same trajectory
+    assert g.sweep_path() == f"tile_planes_{sfx}"
+    g.force_path(2)
+    g.sweep(beta, 2, tile, k); o.sweep(beta, 2, tile, k)
+    assert g.sweep_path() == f"tile_planes_{sfx}"
+    _same_state(g, o)
+    if len(seeds) > 1:
+        assert g.overlap(0, 1) == o.overlap(0, 1)
+
+
+def test_grid_resident_kernel_several_jobs_per_warp():
+    """The same kernel with the number of resident warps capped (ISING_GRID_WARPS, a testing aid): 2, 4, ... jobs of each colour
+    per warp, tile state parked in shared memory between phases; fresh process because the cap is read once."""
+    import os, subprocess, sys
+    code = (
+        "import numpy as np, paper_1006_3865_b200 as P\n"
+        "from oracle import oracle as O\n"
+        "P.use_torch()\n"
+        "for (L, T, k, n, seeds, bits) in ((1024, 32, 2, 3, [5], False), (768, 64, 1, 3, [6, 7], True), (704, 32, 1, 4, [8], False)):\n"
+        "    g = P.Ising(2, L, seeds=seeds); o = O.Oracle(2, L, seeds=seeds)\n"
+        "    if bits: g.set_layout(P.ISING_LAYOUT_BITS)\n"
+        "    Eg, Mg = g.sweep_series(0.44, n, T, k); Eo, Mo = o.sweep_series(0.44, n, T, k)\n"
+        "    assert g.sweep_path().startswith('grid_planes'), g.sweep_path()\n"
+        "    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)\n"
+        "    assert np.array_equal(np.asarray(g.copy_spins()).reshape(-1), np.asarray(o.spins()).reshape(-1))\n"
+        "print('capped ok')\n")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    for cap in ("40", "100"):
+        out = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, ISING_GRID_WARPS=cap),
+                             capture_output=True, text=True, timeout=900)
+        assert out.returncode == 0 and "capped ok" in out.stdout, out.stderr[-2000:]
