@@ -105,6 +105,12 @@ int ising_observables(ising_handle h, int64_t* E, int64_t* M);
 /* ising_overlap — replica overlap Q_ab = Σ_i s_i^a s_i^b (q = Q/N); S8c.7. */
 int ising_overlap(ising_handle h, int a, int b, int64_t* Q);
 
+/* ising_overlap_all — all pairwise overlaps of the R replicas of the handle in one call (BASELINE config 5: "per-replica E
+ * and pairwise overlap q"; replicas of the +-J glass; S8c.7): Q[a*R + b] = Σ_i s_i^a s_i^b for every a, b
+ * (symmetric, Q[a*R + a] = N), R·R int64 values to Q [host|device], caller-owned.  Computed where the spins currently live
+ * (XOR + popcount on the bit / byte tile records, no conversion to the canonical array).  Synchronises. */
+int ising_overlap_all(ising_handle h, int64_t* Q);
+
 /* ising_copy_spins — canonical int8 ±1 spins, R·N bytes, to dst [host|device]. Synchronises. */
 int ising_copy_spins(ising_handle h, int8_t* dst);
 

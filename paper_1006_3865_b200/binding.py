@@ -23,7 +23,7 @@ RNG_MODES = {"words": ISING_RNG_WORDS, "planes": ISING_RNG_PLANES}
 
 SYMBOLS = [
     "ising_create", "ising_create_batch", "ising_create_multi", "ising_destroy", "ising_sweep", "ising_sweep_series",
-    "ising_observables", "ising_overlap", "ising_copy_spins", "ising_set_spins", "ising_copy_spins_bits", "ising_set_spins_bits", "ising_set_layout", "ising_set_rng", "ising_set_jit", "ising_last_sweep_specialized",
+    "ising_observables", "ising_overlap", "ising_overlap_all", "ising_copy_spins", "ising_set_spins", "ising_copy_spins_bits", "ising_set_spins_bits", "ising_set_layout", "ising_set_rng", "ising_set_jit", "ising_last_sweep_specialized",
     "ising_get_counter", "ising_set_counter", "ising_thresholds", "ising_set_device_hooks",
     "ising_synchronize", "ising_kernel_launches", "ising_sweep_path", "ising_force_path",
     "ising_last_error",
@@ -67,6 +67,7 @@ def lib() -> C.CDLL:
     L.ising_sweep_series.argtypes = [vp, C.c_double, C.c_int, C.c_int, C.c_int, i64p, i64p]
     L.ising_observables.argtypes = [vp, i64p, i64p]
     L.ising_overlap.argtypes = [vp, C.c_int, C.c_int, i64p]
+    L.ising_overlap_all.argtypes = [vp, i64p]
     L.ising_copy_spins.argtypes = [vp, i8p]
     L.ising_set_spins.argtypes = [vp, i8p]
     L.ising_copy_spins_bits.argtypes = [vp, vp]
@@ -204,6 +205,13 @@ class Ising:
         q = np.zeros(1, dtype=np.int64)
         _check(lib().ising_overlap(self._h, int(a), int(b), _ptr(q)))
         return int(q[0])
+
+    def overlap_all(self, Q=None):
+        """(R, R) int64 matrix of all pairwise overlaps; Q: optional caller buffer (numpy or torch, host or device)."""
+        if Q is None:
+            Q = np.zeros((self.R, self.R), dtype=np.int64)
+        _check(lib().ising_overlap_all(self._h, _ptr(Q)))
+        return Q
 
     def copy_spins(self, dst=None):
         if dst is None:

@@ -100,7 +100,7 @@ static bool tile_valid(const ising_ctx* h, int T) {
 }
 
 // ---- storage bookkeeping --------------------------------------------------------------
-static int to_canon_scratch(ising_ctx* h) {   // tiles -> d_canon, store state unchanged
+static int to_canon_scratch_now(ising_ctx* h) {   // tiles -> d_canon, store state unchanged
     switch (h->store) {
         case Store::TileI8: return launch_tile_i8_to_canon(h, h->store_tile, h->d_tiles, h->d_canon);
         case Store::PlaneI8: return launch_planes_to_canon(h, h->store_tile, false, h->d_tiles, h->d_canon);
@@ -110,6 +110,20 @@ static int to_canon_scratch(ising_ctx* h) {   // tiles -> d_canon, store state u
         case Store::Amsc: return launch_amsc_to_canon(h, h->d_tiles, h->d_canon);
         default: return 0;
     }
+}
+
+// ... unless d_canon already holds the current state (read-only calls in a row convert once: ising_copy_spins,
+// ising_overlap, ising_copy_spins_bits; every writer of the tile records bumps state_version)
+static int to_canon_scratch(ising_ctx* h) {
+    if (h->store == Store::Canon) return 0;
+    if (h->sweeping) {                        // measuring between the passes of one call: the records change pass by pass
+        h->canon_version = 0;
+        return to_canon_scratch_now(h);
+    }
+    if (h->canon_version == h->state_version) return 0;
+    const int rc = to_canon_scratch_now(h);
+    h->canon_version = rc ? 0 : h->state_version;
+    return rc;
 }
 
 static int ensure_canon(ising_ctx* h) {
@@ -146,6 +160,7 @@ static int ensure_store(ising_ctx* h, Store kind, int T) {
     if (rc) return rc;
     h->store = kind;
     h->store_tile = T;
+    h->canon_version = h->state_version;         // d_canon still holds this very state
     return 0;
 }
 
@@ -217,6 +232,7 @@ void ising_destroy(ising_handle h) {
     dev_free(h->d_xedge);
     dev_free(h->d_gacc);
     dev_free(h->d_obs);
+    dev_free(h->d_pair);
     dev_free(h->d_flag);
     delete h;
 }
@@ -321,6 +337,11 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
     }
     const Accept acc = make_accept(beta, h->dim);
     cudaStream_t st = hooks().stream;
+    struct Sweeping {                         // while passes are being launched no cached canonical copy is valid
+        ising_ctx* h; bool on;
+        ~Sweeping() { h->sweeping = false; if (on) ++h->state_version; }
+    } sweeping{h, n > 0};
+    h->sweeping = n > 0;
     const bool want_series = (E != nullptr) || (M != nullptr);
     const size_t cnt = (size_t)n * h->R;
     long long *d_E = nullptr, *d_M = nullptr, *tmp = nullptr;
@@ -573,6 +594,40 @@ int ising_overlap(ising_handle h, int a, int b, int64_t* Q) {
     return copy_out(Q, d_Q, sizeof(long long), nullptr);
 }
 
+int ising_overlap_all(ising_handle h, int64_t* Q) {
+    if (!h || !Q) { set_error("ising_overlap_all: NULL argument"); return ISING_EINVAL; }
+    const size_t RR = (size_t)h->R * h->R;
+    if (!h->d_pair) {
+        h->d_pair = (long long*)dev_alloc(2 * RR * sizeof(long long));
+        if (!h->d_pair) return ISING_ENOMEM;
+    }
+    unsigned long long* d_D = (unsigned long long*)h->d_pair;
+    long long* d_Q = h->d_pair + RR;
+    int rc;
+    const uint64_t tiles_per_rep = h->store_tile ? (h->dim == 2 ? (uint64_t)(h->L / h->store_tile) * (h->L / h->store_tile)
+                                                                 : (uint64_t)(h->L / 8) * (h->L / 8) * (h->L / 8)) : 0;
+    switch (h->store) {                      // directly on the tile records where their spin bodies are contiguous
+        case Store::PlaneI8: case Store::PlaneBits: {
+            const uint32_t body = (uint32_t)(h->store == Store::PlaneBits ? h->store_tile * h->store_tile / 8 : h->store_tile * h->store_tile);
+            rc = launch_overlap_all(h, h->d_tiles, tiles_per_rep * (body + 64), tiles_per_rep, body + 64, body, 1, d_D, d_Q);
+            break;
+        }
+        case Store::Plane3I8: case Store::Plane3Bits: {
+            const bool bits = h->store == Store::Plane3Bits;
+            const uint32_t rec = (uint32_t)(tile3d_bytes(h, bits) / ((size_t)h->R * tiles_per_rep));
+            rc = launch_overlap_all(h, h->d_tiles, tiles_per_rep * rec, tiles_per_rep, rec, bits ? 64u : 512u, 1, d_D, d_Q);
+            break;
+        }
+        default: {                           // canonical +-1 bytes (0x01 ^ 0xff has 7 bits set); N is a multiple of 4 (L even)
+            const int8_t* s = canon_view(h, &rc);
+            if (!rc) rc = launch_overlap_all(h, s, h->N, 1, h->N, h->N, 7, d_D, d_Q);
+            break;
+        }
+    }
+    if (rc) return rc;
+    return copy_out(Q, d_Q, RR * sizeof(long long), nullptr);
+}
+
 int ising_copy_spins(ising_handle h, int8_t* dst) {
     if (!h || !dst) { set_error("ising_copy_spins: NULL argument"); return ISING_EINVAL; }
     int rc = 0;
@@ -590,6 +645,7 @@ int ising_set_spins(ising_handle h, const int8_t* src) {
     const bool scratch = h->store != Store::Canon;
     int8_t* land = scratch ? h->d_canon : (int8_t*)dev_alloc(bytes);
     if (!land) return ISING_ENOMEM;
+    if (scratch) h->canon_version = 0;            // the scratch copy is being overwritten
     const bool dev = is_device_ptr(src);
     cudaError_t e = cudaMemcpyAsync(land, src, bytes, dev ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st);
     int bad = 0;
@@ -600,7 +656,7 @@ int ising_set_spins(ising_handle h, const int8_t* src) {
         e = cudaMemcpyAsync(h->d_canon, land, bytes, cudaMemcpyDeviceToDevice, st);
         if (e != cudaSuccess) { set_error("ising_set_spins: %s", cudaGetErrorString(e)); rc = ISING_ECUDA; }
     }
-    if (!rc) { h->store = Store::Canon; h->store_tile = 0; }
+    if (!rc) { h->store = Store::Canon; h->store_tile = 0; ++h->state_version; }
     cudaStreamSynchronize(st);
     if (!scratch) dev_free(land);
     return rc;
@@ -632,8 +688,9 @@ int ising_set_spins_bits(ising_handle h, const uint32_t* src) {
     int rc = 0;
     cudaError_t e = cudaMemcpyAsync(stage, src, nwords * 4, is_device_ptr(src) ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, st);
     if (e != cudaSuccess) { set_error("ising_set_spins_bits: copy failed: %s", cudaGetErrorString(e)); rc = ISING_ECUDA; }
+    h->canon_version = 0;
     if (!rc) rc = launch_unpack_bits(stage, h->d_canon, nwords);      // every bit pattern is a valid state
-    if (!rc) { h->store = Store::Canon; h->store_tile = 0; }
+    if (!rc) { h->store = Store::Canon; h->store_tile = 0; ++h->state_version; }
     cudaStreamSynchronize(st);
     dev_free(stage);
     return rc;

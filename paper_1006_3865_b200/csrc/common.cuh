@@ -110,6 +110,10 @@ struct ising_ctx {
     size_t Jtiles_bytes = 0;
 
     long long* d_obs = nullptr;     // 2*R int64 accumulators (+1 for overlap)
+    long long* d_pair = nullptr;    // ising_overlap_all: R*R difference counts + R*R overlaps
+    uint64_t state_version = 1;     // bumped by everything that changes the spins
+    bool sweeping = false;          // inside ising_sweep / ising_sweep_series
+    uint64_t canon_version = 0;     // state_version d_canon was last converted from while the state lives in tile records (0: never)
     int* d_flag = nullptr;          // validation flag
     const char* last_path = "none";
     int force_generic = 0;

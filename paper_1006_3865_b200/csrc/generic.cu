@@ -6,6 +6,8 @@
 // (coarse colour C, inner sweep j, fine colour c): all sites of fine colour c inside tiles
 // of coarse colour C are independent, so one thread per site pair updates them in
 // place from the live array.  With tile == L this is the single checkerboard of P:62 (a8).
+#include <algorithm>
+
 #include "kernels.h"
 #include "philox.cuh"
 
@@ -301,6 +303,81 @@ int launch_overlap_canon(ising_ctx* h, const int8_t* d_spins, int a, int b, long
     ISING_CUDA_OK(cudaMemsetAsync(d_Q, 0, sizeof(long long), st));
     k_overlap<<<reduce_grid(h->N), kThreads, 0, st>>>(d_spins + (uint64_t)a * h->N,
                                                        d_spins + (uint64_t)b * h->N, h->N, d_Q);
+    count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+// ---- all pairwise overlaps Q_ab = sum_i s_i^a s_i^b (S8c.7; BASELINE config 5: "pairwise overlap q") in one pass
+// over the spins wherever they live.  A replica is a sequence of chunks (tile records, or the whole canonical array) of
+// which the first chunk_words 32-bit words hold spins: one bit per site, a 0/1 byte per site, or a +-1 byte per site; in
+// every encoding popc(word_a ^ word_b) = bits_per_diff x (number of sites of the word in which a and b differ), and
+// Q_ab = N - 2 #differing.  Block row a (blockIdx.y) compares replica a with the replicas b > a, eight at a time: D[a*R+b].
+constexpr int kPairChunk = 8;
+
+__global__ void __launch_bounds__(kThreads) k_overlap_all(const uint32_t* __restrict__ base, uint64_t rep_stride_words, uint64_t n_chunks,
+                                                          uint64_t chunk_stride_words, uint64_t chunk_words, int R,
+                                                          unsigned long long* __restrict__ D) {
+    const int a = blockIdx.y;
+    const uint64_t total = n_chunks * (uint64_t)chunk_words;
+    __shared__ unsigned long long sh[kThreads / 32][kPairChunk];
+    for (int b0 = a + 1; b0 < R; b0 += kPairChunk) {
+        unsigned long long acc[kPairChunk];
+#pragma unroll
+        for (int j = 0; j < kPairChunk; ++j) acc[j] = 0;
+        for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (uint64_t)gridDim.x * blockDim.x) {
+            uint64_t off = i;
+            if (n_chunks > 1) {                          // tile records: chunk sizes fit 32 bits
+                const uint32_t cw = (uint32_t)chunk_words;
+                const uint64_t ch = i / cw;
+                off = ch * chunk_stride_words + (i - ch * cw);
+            }
+            const uint32_t wa = __ldg(base + (uint64_t)a * rep_stride_words + off);
+#pragma unroll
+            for (int j = 0; j < kPairChunk; ++j)
+                if (b0 + j < R) acc[j] += (unsigned)__popc(wa ^ __ldg(base + (uint64_t)(b0 + j) * rep_stride_words + off));
+        }
+        const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+#pragma unroll
+        for (int j = 0; j < kPairChunk; ++j) {
+            unsigned long long v = acc[j];
+            for (int d = 16; d > 0; d >>= 1) v += __shfl_xor_sync(0xffffffffu, v, d);
+            if (lane == 0) sh[w][j] = v;
+        }
+        __syncthreads();
+        if (threadIdx.x < kPairChunk && b0 + (int)threadIdx.x < R) {
+            unsigned long long v = 0;
+            for (int ww = 0; ww < kThreads / 32; ++ww) v += sh[ww][threadIdx.x];
+            atomicAdd(D + (size_t)a * R + (b0 + threadIdx.x), v);
+        }
+        __syncthreads();
+    }
+}
+
+__global__ void k_overlap_finish(const unsigned long long* __restrict__ D, long long* __restrict__ Q, int R, long long nsites, int bits_per_diff) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= R * R) return;
+    const int a = i / R, b = i - a * R;
+    if (a == b) { Q[i] = nsites; return; }
+    const unsigned long long d = a < b ? D[(size_t)a * R + b] : D[(size_t)b * R + a];
+    Q[i] = nsites - 2ll * (long long)(d / (unsigned)bits_per_diff);
+}
+
+// d_D: R*R zeroed-by-us scratch words, d_Q: R*R results (both device)
+int launch_overlap_all(ising_ctx* h, const void* base, uint64_t rep_stride_bytes, uint64_t n_chunks, uint64_t chunk_stride_bytes,
+                       uint64_t chunk_bytes, int bits_per_diff, unsigned long long* d_D, long long* d_Q) {
+    cudaStream_t st = hooks().stream;
+    const int R = h->R;
+    ISING_CUDA_OK(cudaMemsetAsync(d_D, 0, sizeof(unsigned long long) * (size_t)R * R, st));
+    if (R > 1) {
+        const uint64_t total = n_chunks * (uint64_t)(chunk_bytes / 4);
+        unsigned gx = (unsigned)std::min<uint64_t>((total + kThreads - 1) / kThreads, 148u * 8u);
+        if (gx < 1) gx = 1;
+        k_overlap_all<<<dim3(gx, (unsigned)(R - 1)), kThreads, 0, st>>>((const uint32_t*)base, rep_stride_bytes / 4, n_chunks, chunk_stride_bytes / 4,
+                                                                       chunk_bytes / 4, R, d_D);
+        count_launch();
+    }
+    k_overlap_finish<<<(R * R + 255) / 256, 256, 0, st>>>(d_D, d_Q, R, (long long)h->N, bits_per_diff);
     count_launch();
     ISING_CUDA_OK(cudaGetLastError());
     return 0;

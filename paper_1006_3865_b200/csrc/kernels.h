@@ -11,6 +11,8 @@ int launch_generic_sweep(ising_ctx* h, const Accept& acc, int n, int T, int k,
 int launch_observables_canon(ising_ctx* h, const int8_t* d_spins, long long* d_E,
                              long long* d_M);                         // a10 (R values each)
 int launch_overlap_canon(ising_ctx* h, const int8_t* d_spins, int a, int b, long long* d_Q);
+int launch_overlap_all(ising_ctx* h, const void* base, uint64_t rep_stride_bytes, uint64_t n_chunks, uint64_t chunk_stride_bytes,
+                       uint64_t chunk_bytes, int bits_per_diff, unsigned long long* d_D, long long* d_Q);   // all R*R overlaps, any spin store
 int launch_validate_pm1(const int8_t* d, uint64_t n, int* d_flag, int* host_bad);
 int launch_pack_bits(const int8_t* d_canon, uint32_t* d_words, uint64_t nwords);     // +-1 bytes -> one bit per site
 int launch_unpack_bits(const uint32_t* d_words, int8_t* d_canon, uint64_t nwords);

@@ -953,7 +953,9 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit) {
     else if (int rc = set_max_dynamic_smem<k_grid_planes<T, BITS, HASJ>>(200 * 1024)) return rc;
     *fits = false;
     static const uint32_t warp_cap = getenv("ISING_GRID_WARPS") ? (uint32_t)atoi(getenv("ISING_GRID_WARPS")) : 0u;   // testing aid: several jobs per warp on small lattices
-    for (uint32_t M = 1; M <= kGridMaxJobsPerWarp; ++M) {
+    // measured: with more than two jobs of a colour per warp (L = 8192 and up) the per-pass kernels win
+    const uint32_t max_m = warp_cap ? kGridMaxJobsPerWarp : 2u;
+    for (uint32_t M = 1; M <= max_m; ++M) {
         const uint32_t warps_needed = (R.jobs_total + M - 1) / M;
         // few jobs: one warp per CTA, so that the CTAs (and the schedulers they land on) spread over all SMs
         const int wpb = warps_needed <= (uint32_t)sms * 4u ? 1 : (warps_needed <= (uint32_t)sms * 8u ? 2 : 4);

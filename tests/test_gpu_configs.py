@@ -89,10 +89,12 @@ def test_oracle_goldens_planes(P, orc, name, layout):
             assert "%016x" % orc.hash_bytes(np.ascontiguousarray(np.concatenate(Es)).astype("<i8")) == extra[0]
             assert "%016x" % orc.hash_bytes(np.ascontiguousarray(np.concatenate(Ms)).astype("<i8")) == extra[1]
             extra = extra[2:]
-        if job.get("overlaps") and p > 0:
+        if job.get("overlaps") and p > 0:                 # config 5's declared output: all 120 pairwise overlaps, one call
+            Q = g.overlap_all()
             for key, q in extra[0].items():
                 a, b = (int(v) for v in key.split(","))
-                assert g.overlap(a, b) == q
+                assert Q[a, b] == q and Q[b, a] == q
+            assert g.overlap(0, R - 1) == extra[0][f"0,{R - 1}"]
     if job["dim"] == 2 and job["tile"] in (32, 64) and job["L"] > 64:
         sfx = "i8" if layout == "int8" else "bits"
         assert g.sweep_path() in (f"tile_planes_{sfx}", f"resident_planes_{sfx}", f"grid_planes_{sfx}")

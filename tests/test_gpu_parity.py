@@ -743,3 +743,44 @@ def test_grid_resident_kernel_several_jobs_per_warp():
         out = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, ISING_GRID_WARPS=cap),
                              capture_output=True, text=True, timeout=900)
         assert out.returncode == 0 and "capped ok" in out.stdout, out.stderr[-2000:]
+
+
+@pytest.mark.parametrize("dim,L,tile,k,rng,layout,R,jseed", [
+    (2, 128, 32, 2, "planes", "int8", 5, 5),       # plane records, 0/1 bytes
+    (2, 128, 64, 1, "planes", "bits", 16, 7),      # bit records, two pair chunks per row (R - 1 > 8)
+    (2, 64, 32, 1, "planes", "int8", 2, None),
+    (3, 16, 8, 2, "planes", "int8", 4, 3),         # 3D records
+    (3, 32, 8, 1, "planes", "bits", 3, None),
+    (2, 128, 32, 1, "words", "int8", 4, None),     # row-major tile records: through the canonical array
+    (2, 36, 6, 1, "planes", "int8", 3, None),      # generic kernels: canonical array
+    (2, 64, 0, 2, "planes", "int8", 3, None),      # 64 x 64 plain checkerboard
+])
+def test_overlap_all_matches_oracle(P, orc, dim, L, tile, k, rng, layout, R, jseed):
+    """ising_overlap_all: every Q_ab in one call, computed where the spins live (XOR + popcount on the records), against the
+    oracle's pairwise definition; before the first sweep (canonical array), after sweeps, and again after a read-only call."""
+    J = W.couplings(dim, L, jseed) if jseed is not None else None
+    seeds = [300 + 7 * r for r in range(R)]
+    g, o = _both(P, orc, dim, L, seeds, J, rng)
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+
+    def want():
+        Q = np.zeros((R, R), dtype=np.int64)
+        for a in range(R):
+            for b in range(R):
+                Q[a, b] = o.overlap(a, b)
+        return Q
+    assert np.array_equal(g.overlap_all(), want())
+    g.sweep(0.7, 3, tile, k); o.sweep(0.7, 3, tile, k)
+    Q = want()
+    assert np.array_equal(np.diag(Q), np.full(R, L ** dim))
+    assert np.array_equal(g.overlap_all(), Q)
+    s = np.asarray(g.copy_spins()).reshape(R, -1)              # a read-only call converts the records once ...
+    assert np.array_equal(s, np.asarray(o.spins()).reshape(R, -1))
+    assert np.array_equal(g.overlap_all(), Q) and g.overlap(0, R - 1) == Q[0, R - 1]
+    g.sweep(0.7, 1, tile, k); o.sweep(0.7, 1, tile, k)         # ... and a sweep invalidates that copy
+    assert np.array_equal(np.asarray(g.copy_spins()).reshape(R, -1), np.asarray(o.spins()).reshape(R, -1))
+    import torch
+    Qd = torch.zeros((R, R), dtype=torch.int64, device="cuda")
+    g.overlap_all(Qd)
+    assert np.array_equal(Qd.cpu().numpy(), want())
