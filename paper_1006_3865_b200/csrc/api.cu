@@ -534,6 +534,31 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
                 }
             }
         }
+        const bool use_grid3 = use_3d && !resident_done && n >= 2 && !h->no_resident && !resident3d_supported(h, T) && grid3d_supported(h, T);
+        if (use_grid3 && !rc) {
+            const size_t xb = grid3d_xedge_bytes(h), ab = want_series ? grid3d_acc_bytes(h, n) : 0;
+            if (xb > h->xedge_bytes) {
+                cudaStreamSynchronize(st);
+                dev_free(h->d_xedge); h->xedge_bytes = 0;
+                h->d_xedge = dev_alloc(xb);
+                if (!h->d_xedge) rc = ISING_ENOMEM; else h->xedge_bytes = xb;
+            }
+            if (!rc && ab > h->gacc_bytes) {
+                cudaStreamSynchronize(st);
+                dev_free(h->d_gacc); h->gacc_bytes = 0;
+                h->d_gacc = dev_alloc(ab);
+                if (!h->d_gacc) rc = ISING_ENOMEM; else h->gacc_bytes = ab;
+            }
+            if (!rc) {
+                const int g = launch_grid3d(h, acc, bits, n, k, h->t, h->d_xedge, h->d_gacc, d_E, d_M, use_jit);
+                if (g == 0) {
+                    h->last_path = bits ? "grid3d_planes_bits" : "grid3d_planes_i8";
+                    resident_done = true;
+                } else if (g != 1) {
+                    cudaGetLastError();
+                }
+            }
+        }
         for (int pass = 0; pass < n && !rc && !resident_done; ++pass) {
             const uint64_t t0 = h->t + (uint64_t)pass * (uint64_t)k;
             rc = use_tile_i8 ? launch_tile_i8_pass(h, acc, T, k, t0)

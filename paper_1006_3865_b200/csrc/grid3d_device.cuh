@@ -1,0 +1,196 @@
+// grid3d_device.cuh — k_grid3d: the 3D lattice on chip across ALL SMs for a whole ising_sweep call (BASELINE config 4: 256^3;
+// VERDICT round 1 "next" 5).  The design of k_grid_planes (grid_planes_device.cuh) carried over to the 8^3 register tiling
+// of tile3d_planes_device.cuh: warp w owns the jobs w, w + W, ... (4 tiles each, lane = (tile, z-slice)) of both coarse
+// colours, parks the two words of every slice in shared memory between phases, and after every phase publishes the six
+// faces of its tiles in a 256-byte exchange record in global memory (L2) as self-validating 64-bit words
+// {value, version}; the six neighbours — all of the other coarse colour — poll exactly the words they need.
+// One cooperative launch (co-residency only), no grid barrier, HBM touched twice per call.
+#pragma once
+#include "tile3d_planes_device.cuh"
+
+namespace ising {
+
+namespace ISING_DEVICE_NS3 {
+
+constexpr int kGrid3AccSlots = 8;
+// exchange record of a tile, u64 = version << 32 | value:  X[lz] = {XL, XR} (16 words), Y[lz] = YL | YR << 8 (8), ZL[2], ZR[2], pad
+constexpr int kG3X = 0, kG3Y = 16, kG3ZL = 24, kG3ZR = 26, kG3Rec = 32;
+
+struct Grid3Args {
+    Plane3Args P;
+    int n;                                // outer passes
+    uint32_t jobs_total;                  // R * jobs per colour (4 tiles per job)
+    uint32_t jobs_per_warp;               // jobs of each colour a warp owns
+    unsigned long long* xedge;            // kG3Rec u64 per tile, replica-major, tile (tz, ty, tx) at (tz*B + ty)*B + tx
+    long long* acc;                       // optional series accumulators [n][R][kGrid3AccSlots][2] = {#up, #unsatisfied}, zeroed
+};
+
+__device__ __forceinline__ unsigned long long ld_x64(const unsigned long long* p) {
+    unsigned long long v;
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void ld_x64v2(const unsigned long long* p, unsigned long long& a, unsigned long long& b) {
+    asm volatile("ld.relaxed.gpu.global.v2.u64 {%0,%1}, [%2];" : "=l"(a), "=l"(b) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void st_x64(unsigned long long* p, unsigned long long a) {
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(a) : "memory");
+}
+__device__ __forceinline__ void st_x64v2(unsigned long long* p, unsigned long long a, unsigned long long b) {
+    asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1,%2};" ::"l"(p), "l"(a), "l"(b) : "memory");
+}
+
+template <bool BITS, bool HASJ, unsigned long long HP3 = kNoSpec3>
+__global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
+    extern __shared__ uint32_t grid3_smem[];                  // per warp: [colour][job][word][lane]
+    const Plane3Args& A = R.P;
+    const int lane = threadIdx.x & 31;
+    const uint32_t wg = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), W = gridDim.x * (blockDim.x >> 5);
+    const int sub = lane >> 3, lz = lane & 7;
+    const uint32_t B = (uint32_t)A.B, Mw = R.jobs_per_warp;
+    uint32_t* const ws = grid3_smem + (size_t)(threadIdx.x >> 5) * (2u * Mw * 2u * 32u) + lane;
+    const uint2* lut = kByteLutGlobal.e;
+    const bool series = R.acc != nullptr;
+
+    struct Job { Tile3 t; uint32_t self, xm, xp, ym, yp, zm, zp; };       // tile indices into xedge
+    auto decode = [&](uint32_t job, int C) {
+        const uint32_t q = job * 4u + (uint32_t)sub;
+        const uint32_t rr = fastdiv(q, A.per_rep, A.magic_rep);
+        uint32_t rem = q - rr * A.per_rep;
+        const uint32_t tz = fastdiv(rem, A.per_z, A.magic_z);
+        rem -= tz * A.per_z;
+        const uint32_t ty = fastdiv(rem, A.hb, A.magic_hb);
+        rem -= ty * A.hb;
+        const uint32_t tx = 2u * rem + ((ty + tz + (uint32_t)C) & 1u);
+        Job jb;
+        jb.t.r = (int)rr; jb.t.tx = (int)tx; jb.t.ty = (int)ty; jb.t.tz = (int)tz;
+        const uint32_t base = rr * B * B * B;
+        auto idx = [&](uint32_t x, uint32_t y, uint32_t z) { return base + (z * B + y) * B + x; };
+        jb.self = idx(tx, ty, tz);
+        jb.xm = idx(tx == 0 ? B - 1 : tx - 1, ty, tz); jb.xp = idx(tx == B - 1 ? 0 : tx + 1, ty, tz);
+        jb.ym = idx(tx, ty == 0 ? B - 1 : ty - 1, tz); jb.yp = idx(tx, ty == B - 1 ? 0 : ty + 1, tz);
+        jb.zm = idx(tx, ty, tz == 0 ? B - 1 : tz - 1); jb.zp = idx(tx, ty, tz == B - 1 ? 0 : tz + 1);
+        return jb;
+    };
+    auto publish = [&](const Slice& s, uint32_t me, uint32_t ver) {
+        uint32_t XL, XR, YL, YR;
+        face_words(s.S, lz, XL, XR, YL, YR);
+        const unsigned long long v = (unsigned long long)ver << 32;
+        unsigned long long* e = R.xedge + (size_t)me * kG3Rec;
+        st_x64v2(e + kG3X + 2 * lz, v | XL, v | XR);
+        st_x64(e + kG3Y + lz, v | (YL & 0xffu) | ((YR & 0xffu) << 8));
+        if (lz == 0) st_x64v2(e + kG3ZL, v | s.S[0], v | s.S[1]);
+        if (lz == 7) st_x64v2(e + kG3ZR, v | s.S[0], v | s.S[1]);
+    };
+    // wait until the six neighbours have published version `want`, and take the halos from their words
+    auto refresh = [&](Slice& s, const Job& jb, uint32_t want) {
+        const unsigned long long* pxm = R.xedge + (size_t)jb.xm * kG3Rec + kG3X + 2 * lz + 1;     // left tile's XR
+        const unsigned long long* pxp = R.xedge + (size_t)jb.xp * kG3Rec + kG3X + 2 * lz;         // right tile's XL
+        const unsigned long long* pym = R.xedge + (size_t)jb.ym * kG3Rec + kG3Y + lz;             // tile in front: its YR
+        const unsigned long long* pyp = R.xedge + (size_t)jb.yp * kG3Rec + kG3Y + lz;             // tile behind: its YL
+        const unsigned long long* pz = lz == 0 ? R.xedge + (size_t)jb.zm * kG3Rec + kG3ZR : R.xedge + (size_t)jb.zp * kG3Rec + kG3ZL;
+        const bool need_z = lz == 0 || lz == 7;
+        for (;;) {
+            const unsigned long long a = ld_x64(pxm), b = ld_x64(pxp), c = ld_x64(pym), d = ld_x64(pyp);
+            unsigned long long z0 = 0, z1 = 0;
+            bool ok = (uint32_t)(a >> 32) == want && (uint32_t)(b >> 32) == want && (uint32_t)(c >> 32) == want && (uint32_t)(d >> 32) == want;
+            if (need_z) {
+                ld_x64v2(pz, z0, z1);
+                ok = ok && (uint32_t)(z0 >> 32) == want && (uint32_t)(z1 >> 32) == want;
+            }
+            if (__all_sync(0xffffffffu, ok)) {
+                s.xl = (uint32_t)a; s.xr = (uint32_t)b;
+                s.ym = ((uint32_t)c >> 8) & 0xffu; s.yp = (uint32_t)d & 0xffu;
+                s.zm[0] = s.zm[1] = s.zp[0] = s.zp[1] = 0u;
+                if (lz == 0) { s.zm[0] = (uint32_t)z0; s.zm[1] = (uint32_t)z1; }
+                if (lz == 7) { s.zp[0] = (uint32_t)z0; s.zp[1] = (uint32_t)z1; }
+                return;
+            }
+        }
+    };
+    auto account = [&](const Slice& s, int r, int pass) {
+        int up = 0, unsat = 0;
+        count_slice<HASJ>(s, lz, up, unsat);
+#pragma unroll
+        for (int d = 4; d > 0; d >>= 1) {                          // the 8 slices of a tile
+            up += __shfl_xor_sync(0xffffffffu, up, d);
+            unsat += __shfl_xor_sync(0xffffffffu, unsat, d);
+        }
+        if (lz == 0) {
+            long long* a = R.acc + (((size_t)pass * A.R + r) * kGrid3AccSlots + ((wg + (uint32_t)sub) % kGrid3AccSlots)) * 2;
+            atomicAdd(reinterpret_cast<unsigned long long*>(a), (unsigned long long)up);
+            atomicAdd(reinterpret_cast<unsigned long long*>(a + 1), (unsigned long long)unsat);
+        }
+    };
+    auto sm_slot = [&](int C, uint32_t m) { return ws + (size_t)((uint32_t)C * Mw + m) * 64u; };
+
+    // records -> shared memory; the colour-1 tiles publish their initial faces (version 1 = what phase 0 waits for)
+    for (int C = 0; C < 2; ++C)
+        for (uint32_t m = 0; m < Mw; ++m) {
+            const uint32_t job = wg + m * W;
+            if (job >= R.jobs_total) break;                               // warp-uniform
+            const Job jb = decode(job, C);
+            Slice s;
+            load_slice<BITS>(A, jb.t, lz, s);
+            uint32_t* p = sm_slot(C, m);
+            p[0] = s.S[0]; p[32] = s.S[1];
+            if (C == 1) publish(s, jb.self, 1u);
+        }
+
+    for (int pass = 0; pass < R.n; ++pass) {
+        for (int C = 0; C < 2; ++C) {
+            const uint32_t ph = 2u * (uint32_t)pass + (uint32_t)C;       // waits for version ph + 1, publishes ph + 2
+#pragma unroll 1
+            for (uint32_t m = 0; m < Mw; ++m) {
+                const uint32_t job = wg + m * W;
+                if (job >= R.jobs_total) break;
+                const Job jb = decode(job, C);
+                Slice s;
+                uint32_t* p = sm_slot(C, m);
+                s.S[0] = p[0]; s.S[1] = p[32];
+                load_couplings<HASJ>(A, jb.t, lz, s);
+                refresh(s, jb, ph + 1u);
+                if (series && C == 0 && pass > 0) account(s, jb.t.r, pass - 1);
+                const uint64_t seed = A.seeds[jb.t.r];
+                const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+                const uint32_t z = (uint32_t)(jb.t.tz * kT3 + lz);
+                const uint32_t g = (z * B + (uint32_t)jb.t.ty) * B + (uint32_t)jb.t.tx;
+                const uint32_t p_base = (uint32_t)(jb.t.tx * 4) + (uint32_t)(A.L >> 1) * ((uint32_t)(jb.t.ty * kT3) + (uint32_t)A.L * z);
+                for (int j = 0; j < A.k; ++j) {
+                    const uint64_t tt = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
+                    half_sweep3<HP3, HASJ>(A, s, 0, lz, g, p_base, 2 * tt, k0, k1);
+                    half_sweep3<HP3, HASJ>(A, s, 1, lz, g, p_base, 2 * tt + 1, k0, k1);
+                }
+                publish(s, jb.self, ph + 2u);
+                if (series && C == 1) account(s, jb.t.r, pass);
+                p[0] = s.S[0]; p[32] = s.S[1];
+            }
+        }
+    }
+    if (series && R.n > 0)
+        for (uint32_t m = 0; m < Mw; ++m) {
+            const uint32_t job = wg + m * W;
+            if (job >= R.jobs_total) break;
+            const Job jb = decode(job, 0);
+            Slice s;
+            const uint32_t* p = sm_slot(0, m);
+            s.S[0] = p[0]; s.S[1] = p[32];
+            load_couplings<HASJ>(A, jb.t, lz, s);
+            refresh(s, jb, 2u * (uint32_t)R.n + 1u);
+            account(s, jb.t.r, R.n - 1);
+        }
+    for (int C = 0; C < 2; ++C)
+        for (uint32_t m = 0; m < Mw; ++m) {
+            const uint32_t job = wg + m * W;
+            if (job >= R.jobs_total) break;
+            const Job jb = decode(job, C);
+            Slice s;
+            const uint32_t* p = sm_slot(C, m);
+            s.S[0] = p[0]; s.S[1] = p[32];
+            store_slice<BITS>(A, jb.t, lz, s, lut);
+        }
+}
+
+}  // namespace
+
+}  // namespace ising

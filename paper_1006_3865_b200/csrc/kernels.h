@@ -58,6 +58,11 @@ int launch_convert_couplings3d(ising_ctx* h, void* d_jrec);
 bool resident3d_supported(const ising_ctx* h, int T);            // L <= 64: the whole call in one cluster launch
 int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, long long* d_E, long long* d_M,
                       bool plain, int Tc);                        // plain: the tile == L schedule; Tc: masked coarse tiles or 0
+bool grid3d_supported(const ising_ctx* h, int T);               // L > 64: the whole call in one cooperative launch (k_grid3d)
+size_t grid3d_xedge_bytes(const ising_ctx* h);
+size_t grid3d_acc_bytes(const ising_ctx* h, int n);
+int launch_grid3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, void* d_xedge, void* d_acc,
+                  long long* d_E, long long* d_M, bool use_jit);          // returns 1 (nothing launched) if the lattice does not fit
 int launch_tile3d_plain(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, int Tc);   // a8 in 3D, L > 64
 int launch_observables3d(ising_ctx* h, bool bits, long long* d_E, long long* d_M);   // a10 on 3D tile records
 
@@ -72,6 +77,7 @@ int launch_amsc_pass(ising_ctx* h, const Accept& acc, int T, int k, uint64_t t_f
 // ---- planes_jit.cu: run-time specialisation of k_tile_planes on the threshold head bits (NVRTC) ----
 cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R);
 cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3);   // nullptr: not available
+cudaKernel_t grid3d_jit_kernel(bool bits, unsigned long long hp3);      // k_grid3d specialised on the three threshold heads
 cudaKernel_t grid_jit_kernel(int T, bool bits, bool hasj, uint32_t hp);   // k_grid_planes specialised on the threshold heads
 uint64_t planes_jit_compiled();
 const char* planes_jit_last_log();

@@ -153,6 +153,12 @@ cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3) {
     return cached(kJitSource3d, expr, {});
 }
 
+cudaKernel_t grid3d_jit_kernel(bool bits, unsigned long long hp3) {
+    char expr[160];
+    snprintf(expr, sizeof expr, "ising::jit::k_grid3d<%s, false, %lluull>", bits ? "true" : "false", hp3);
+    return cached(kJitSource3d, expr, {});
+}
+
 uint64_t planes_jit_compiled() { return state().compiled; }
 const char* planes_jit_last_log() { return state().last_log.c_str(); }
 

@@ -23,6 +23,7 @@
 
 #include "kernels.h"
 #include "tile3d_planes_device.cuh"
+#include "grid3d_device.cuh"
 
 namespace ising {
 
@@ -619,6 +620,104 @@ int launch_resident3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, 
                           : (bits ? go(k_resident3d<true, false>) : go(k_resident3d<false, false>));
     if (rc) return rc;
     count_launch();
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
+}
+
+// ---- k_grid3d (grid3d_device.cuh): the whole call in one cooperative launch, slices on chip on all SMs ----
+__global__ void k_grid3d_series_finish(const long long* __restrict__ acc, long long* __restrict__ E, long long* __restrict__ Mo,
+                                       uint32_t count, long long nsites) {
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;          // pass * R + r
+    if (i >= count) return;
+    long long up = 0, unsat = 0;
+    for (int s = 0; s < kGrid3AccSlots; ++s) { up += acc[((size_t)i * kGrid3AccSlots + s) * 2]; unsat += acc[((size_t)i * kGrid3AccSlots + s) * 2 + 1]; }
+    if (Mo) Mo[i] = 2 * up - nsites;
+    if (E) E[i] = 2 * unsat - 3 * nsites;
+}
+
+size_t grid3d_xedge_bytes(const ising_ctx* h) {
+    const size_t B = (size_t)(h->L / kT3);
+    return (size_t)h->R * B * B * B * kG3Rec * sizeof(unsigned long long);
+}
+size_t grid3d_acc_bytes(const ising_ctx* h, int n) { return (size_t)n * (size_t)h->R * kGrid3AccSlots * 2 * sizeof(long long); }
+
+bool grid3d_supported(const ising_ctx* h, int T) {
+    if (!tile3d_supported(h, T)) return false;
+    const uint64_t B = (uint64_t)(h->L / kT3);
+    return (uint64_t)h->R * B * B * B / 8u <= 148u * 32u * 16u;
+}
+
+namespace {
+template <bool BITS, bool HASJ>
+int launch_grid3d_one(Grid3Args& R, cudaKernel_t spec, bool* fits) {
+    int dev = 0, sms = 0;
+    ISING_CUDA_OK(cudaGetDevice(&dev));
+    ISING_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const void* fn = spec ? (const void*)spec : (const void*)k_grid3d<BITS, HASJ>;
+    if (spec) ISING_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+    else if (int rc = set_max_dynamic_smem<k_grid3d<BITS, HASJ>>(200 * 1024)) return rc;
+    *fits = false;
+    static const uint32_t warp_cap = getenv("ISING_GRID_WARPS") ? (uint32_t)atoi(getenv("ISING_GRID_WARPS")) : 0u;   // testing aid
+    const uint32_t max_m = warp_cap ? 16u : 2u;              // as in launch_grid_planes: beyond two jobs per warp the per-pass kernels win
+    for (uint32_t M = 1; M <= max_m; ++M) {
+        const uint32_t warps_needed = (R.jobs_total + M - 1) / M;
+        const int wpb = warps_needed <= (uint32_t)sms * 4u ? 1 : (warps_needed <= (uint32_t)sms * 8u ? 2 : 4);
+        const size_t smem = (size_t)wpb * 2u * M * 2u * 32u * sizeof(uint32_t);
+        int occ = 0;
+        ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, wpb * 32, smem));
+        const uint32_t grid = (warps_needed + wpb - 1) / wpb;
+        if (grid > (uint32_t)sms * (uint32_t)occ) continue;      // not co-resident: more jobs per warp
+        if (warp_cap && warps_needed > warp_cap && M < 16u) continue;
+        R.jobs_per_warp = M;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(wpb * 32); cfg.dynamicSmemBytes = smem; cfg.stream = hooks().stream;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        void* args[] = {&R};
+        ISING_CUDA_OK(cudaLaunchKernelExC(&cfg, fn, args));
+        count_launch();
+        *fits = true;
+        return 0;
+    }
+    return 0;
+}
+}  // namespace
+
+// n passes in one cooperative launch; returns 1 (nothing launched) if the lattice does not fit on chip.
+int launch_grid3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, void* d_xedge, void* d_acc,
+                  long long* d_E, long long* d_M, bool use_jit) {
+    Grid3Args R;
+    Plane3Args& A = R.P;
+    A = Plane3Args{};
+    fill_geometry3(A, h);
+    fill_accept3(A, acc);
+    A.k = k; A.t_first = t_first; A.C = 0;
+    R.n = n;
+    R.jobs_total = A.njobs;
+    R.jobs_per_warp = 1;
+    R.xedge = (unsigned long long*)d_xedge;
+    const bool series = (d_E || d_M) && n > 0;
+    R.acc = series ? (long long*)d_acc : nullptr;
+    cudaStream_t st = hooks().stream;
+    ISING_CUDA_OK(cudaMemsetAsync(d_xedge, 0, grid3d_xedge_bytes(h), st));          // version 0 = nothing published
+    if (series) ISING_CUDA_OK(cudaMemsetAsync(d_acc, 0, grid3d_acc_bytes(h, n), st));
+    const unsigned long long hp3 = ((unsigned long long)(acc.thr[0] >> kTailBits) << 24) |
+                                   ((unsigned long long)(acc.thr[1] >> kTailBits) << 12) | (unsigned long long)(acc.thr[2] >> kTailBits);
+    cudaKernel_t spec = (use_jit && !A.force && !A.jrec) ? grid3d_jit_kernel(bits, hp3) : nullptr;
+    bool fits = false;
+    int rc;
+    if (A.jrec) rc = bits ? launch_grid3d_one<true, true>(R, nullptr, &fits) : launch_grid3d_one<false, true>(R, nullptr, &fits);
+    else rc = bits ? launch_grid3d_one<true, false>(R, spec, &fits) : launch_grid3d_one<false, false>(R, spec, &fits);
+    if (rc) return rc;
+    if (!fits) return 1;
+    h->last_jit = spec ? 1 : 0;
+    if (series) {
+        const uint32_t count = (uint32_t)n * (uint32_t)h->R;
+        k_grid3d_series_finish<<<(count + 255) / 256, 256, 0, st>>>((const long long*)d_acc, d_E, d_M, count, (long long)h->N);
+        count_launch();
+    }
     ISING_CUDA_OK(cudaGetLastError());
     return 0;
 }

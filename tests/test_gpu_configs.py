@@ -101,7 +101,8 @@ def test_oracle_goldens_planes(P, orc, name, layout):
     if job["tile"] == job["L"]:
         assert g.sweep_path() == ("tile_plain_" if job["dim"] == 2 else "tile3d_plain_") + ("i8" if layout == "int8" else "bits")
     elif job["dim"] == 3:
-        assert g.sweep_path() in (f"tile3d_planes_{'i8' if layout == 'int8' else 'bits'}", f"resident3d_planes_{'i8' if layout == 'int8' else 'bits'}")
+        sfx = "i8" if layout == "int8" else "bits"
+        assert g.sweep_path() in (f"tile3d_planes_{sfx}", f"resident3d_planes_{sfx}", f"grid3d_planes_{sfx}")
     g.destroy()
 
 

@@ -480,7 +480,7 @@ def test_cluster_resident_3d_kernel_matches_oracle(P, orc, L, k, n, beta, seeds,
     if L == 64 and layout == "int8":
         big = P.Ising(3, 128, seed=1)
         big.sweep(beta, 2, 8, 1)
-        assert big.sweep_path() == "tile3d_planes_i8"
+        assert big.sweep_path() == "grid3d_planes_i8"           # larger lattices: the grid-resident kernel (test_grid_resident_3d_*)
 
 
 @pytest.mark.parametrize("layout", ["int8", "bits"])
@@ -531,7 +531,7 @@ def test_tile3d_couplings_match_oracle(P, orc, L, k, n, beta, seeds, jseed, layo
     _same_state(g, o)
     g.force_path(0)
     g.sweep(beta, n, 8, k); o.sweep(beta, n, 8, k)
-    assert g.sweep_path().startswith("resident3d_planes" if L <= 64 else "tile3d_planes")
+    assert g.sweep_path().startswith("resident3d_planes" if L <= 64 else "grid3d_planes")
     _same_state(g, o)
     Eg, Mg = g.sweep_series(beta, n, 8, k)          # L <= 64: measured on the registers of the resident kernel
     Eo, Mo = o.sweep_series(beta, n, 8, k)
@@ -784,3 +784,62 @@ def test_overlap_all_matches_oracle(P, orc, dim, L, tile, k, rng, layout, R, jse
     Qd = torch.zeros((R, R), dtype=torch.int64, device="cuda")
     g.overlap_all(Qd)
     assert np.array_equal(Qd.cpu().numpy(), want())
+
+
+GRID3 = [
+    # L, k, n, beta, seeds, jseed: more than 64 warp jobs per colour -> k_grid3d (one cooperative launch)
+    (80, 1, 3, BC3, [4], None),              # B = 10
+    (96, 2, 2, BC3, [5], None),              # B = 12
+    (128, 1, 3, BC3, [9], None),             # 2^21 sites
+    (80, 1, 3, 0.3, [5, 6], None),           # replicas
+    (96, 1, 2, 0.9, [2], 10),                # 3D Edwards-Anderson glass
+    (80, 2, 2, 0.0, [2], None),
+    (80, 2, 2, 9.0, [2], None),
+]
+
+
+@pytest.mark.parametrize("jit", ["off", "on"])
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,k,n,beta,seeds,jseed", GRID3)
+def test_grid_resident_3d_kernel_matches_oracle(P, orc, L, k, n, beta, seeds, jseed, layout, jit):
+    """3D lattices beyond the cluster (L > 64; BASELINE config 4 is L = 256): the whole call in one cooperative launch,
+    slices on chip, the six faces of every tile exchanged as versioned 64-bit words in L2 (k_grid3d)."""
+    J = W.couplings(3, L, jseed) if jseed is not None else None
+    g, o = _both(P, orc, 3, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.set_jit(jit)
+    sfx = "i8" if layout == "int8" else "bits"
+    g.sweep(beta, n, 8, k); o.sweep(beta, n, 8, k)
+    assert g.sweep_path() == f"grid3d_planes_{sfx}"
+    assert g.last_sweep_specialized() == (jit == "on" and beta > 0 and jseed is None)
+    _same_state(g, o)
+    Eg, Mg = g.sweep_series(beta, n, 8, k)
+    assert g.sweep_path() == f"grid3d_planes_{sfx}"
+    Eo, Mo = o.sweep_series(beta, n, 8, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    g.sweep(beta, 1, 8, k); o.sweep(beta, 1, 8, k)                # a single pass: the per-pass kernel
+    assert g.sweep_path() == f"tile3d_planes_{sfx}"
+    _same_state(g, o)
+
+
+def test_grid_resident_3d_kernel_several_jobs_per_warp():
+    """k_grid3d with the number of resident warps capped (ISING_GRID_WARPS): several jobs of each colour per warp."""
+    import os, subprocess, sys
+    code = (
+        "import numpy as np, paper_1006_3865_b200 as P\n"
+        "from oracle import oracle as O\n"
+        "P.use_torch()\n"
+        "for (L, k, n, seeds, bits) in ((80, 2, 3, [5], False), (96, 1, 3, [6, 7], True)):\n"
+        "    g = P.Ising(3, L, seeds=seeds); o = O.Oracle(3, L, seeds=seeds)\n"
+        "    if bits: g.set_layout(P.ISING_LAYOUT_BITS)\n"
+        "    Eg, Mg = g.sweep_series(0.2216546, n, 8, k); Eo, Mo = o.sweep_series(0.2216546, n, 8, k)\n"
+        "    assert g.sweep_path().startswith('grid3d_planes'), g.sweep_path()\n"
+        "    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)\n"
+        "    assert np.array_equal(np.asarray(g.copy_spins()).reshape(-1), np.asarray(o.spins()).reshape(-1))\n"
+        "print('capped ok')\n")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, ISING_GRID_WARPS="50"),
+                         capture_output=True, text=True, timeout=900)
+    assert out.returncode == 0 and "capped ok" in out.stdout, out.stderr[-2000:]
