@@ -5,7 +5,9 @@
 #include <cstdarg>
 #include <cstring>
 #include <atomic>
+#include <mutex>
 #include <new>
+#include <unordered_map>
 
 #include "kernels.h"
 
@@ -28,17 +30,35 @@ void set_error(const char* fmt, ...) {
 
 void count_launch(uint64_t n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
 
+// Every block is released through the hook that was installed when it was allocated (nullptr = cudaFree), whatever
+// ising_set_device_hooks has been called with in between: the owner is remembered per pointer.
+static std::mutex g_owner_mu;
+static std::unordered_map<void*, void (*)(void*)>& owners() {
+    static std::unordered_map<void*, void (*)(void*)> m;
+    return m;
+}
+
 void* dev_alloc(size_t bytes) {
     if (bytes == 0) bytes = 16;
     void* p = nullptr;
+    void (*owner)(void*) = nullptr;
     if (hooks().alloc) {
+        owner = hooks().dealloc;
         p = hooks().alloc(bytes);
-        if (!p) set_error("device allocation hook returned NULL for %zu bytes", bytes);
-        return p;
+        if (!p) { set_error("device allocation hook returned NULL for %zu bytes", bytes); return nullptr; }
+    } else {
+        cudaError_t e = cudaMalloc(&p, bytes);
+        if (e != cudaSuccess) {
+            set_error("cudaMalloc(%zu) failed: %s", bytes, cudaGetErrorString(e));
+            return nullptr;
+        }
     }
-    cudaError_t e = cudaMalloc(&p, bytes);
-    if (e != cudaSuccess) {
-        set_error("cudaMalloc(%zu) failed: %s", bytes, cudaGetErrorString(e));
+    try {
+        std::lock_guard<std::mutex> lock(g_owner_mu);
+        owners()[p] = owner;
+    } catch (...) {                          // cannot remember the owner: give the block back now rather than leak or mis-free it
+        if (owner) owner(p); else cudaFree(p);
+        set_error("out of host memory while recording a device allocation");
         return nullptr;
     }
     return p;
@@ -46,7 +66,13 @@ void* dev_alloc(size_t bytes) {
 
 void dev_free(void* p) {
     if (!p) return;
-    if (hooks().dealloc) hooks().dealloc(p);
+    void (*owner)(void*) = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_owner_mu);
+        auto it = owners().find(p);
+        if (it != owners().end()) { owner = it->second; owners().erase(it); }
+    }
+    if (owner) owner(p);
     else cudaFree(p);
 }
 
@@ -253,7 +279,13 @@ static ising_handle create_impl(int dim, int L, const int8_t* J, const uint64_t*
     ising_ctx* h = new (std::nothrow) ising_ctx;
     if (!h) return nullptr;
     h->dim = dim; h->L = L; h->R = R; h->N = N;
-    h->seeds.assign(seeds, seeds + R);
+    try {
+        h->seeds.assign(seeds, seeds + R);
+    } catch (...) {
+        delete h;
+        set_error("ising_create: out of host memory");
+        return nullptr;
+    }
     h->J_per_replica = multi; h->shared_sweep = multi; h->sweep_seed = sweep_seed;
     if (multi) h->rng = ISING_RNG_WORDS;     // one random word per site serves every realisation (ising.h)
     cudaStream_t st = hooks().stream;
@@ -271,7 +303,8 @@ static ising_handle create_impl(int dim, int L, const int8_t* J, const uint64_t*
     if (multi) {                                       // R copies of the shared sweep key (R17)
         h->d_sweep_seeds = (uint64_t*)dev_alloc(sizeof(uint64_t) * R);
         if (!h->d_sweep_seeds) return fail();
-        std::vector<uint64_t> ks((size_t)R, sweep_seed);
+        std::vector<uint64_t> ks;
+        try { ks.assign((size_t)R, sweep_seed); } catch (...) { set_error("ising_create_multi: out of host memory"); return fail(); }
         if (cudaMemcpyAsync(h->d_sweep_seeds, ks.data(), sizeof(uint64_t) * R, cudaMemcpyHostToDevice, st) != cudaSuccess ||
             cudaStreamSynchronize(st) != cudaSuccess) {
             set_error("ising_create_multi: seed upload failed: %s", cudaGetErrorString(cudaGetLastError()));
@@ -358,6 +391,16 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
     }
     int rc = 0;
     const bool thr_fits = !(acc.thr_is_2p32[0] || acc.thr_is_2p32[1] || acc.thr_is_2p32[2]);   // beta = 0 only
+    // 0 < beta < ~1.4e-17: thr[1] rounds to 2^32 while thr[2] (thr[3]) is 2^32 - 1.  The multi-spin kernels fold "2^32" into one
+    // all-or-nothing mask, so that case (the accept decision differs for r = 0xffffffff only) goes to the generic kernels,
+    // which compare every threshold on its own
+    bool thr_mixed = false;
+    for (int m = 1; m < h->dim; ++m) thr_mixed = thr_mixed || (acc.thr_is_2p32[m] != acc.thr_is_2p32[0]);
+    struct ForceGeneric {
+        ising_ctx* h; int saved;
+        ~ForceGeneric() { h->force_generic = saved; }
+    } fg{h, h->force_generic};
+    if (thr_mixed) h->force_generic = 1;
     const bool use_tile_i8 = !h->force_generic && thr_fits && h->rng == ISING_RNG_WORDS &&
                              h->layout == ISING_LAYOUT_I8 && tile_i8_supported(h, T);
     const bool use_planes = !h->force_generic && h->rng == ISING_RNG_PLANES && tile_planes_supported(h, T);
@@ -446,6 +489,7 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             h->d_amsc_J = dev_alloc((size_t)h->N * 8);
             if (!h->d_amsc_J) rc = ISING_ENOMEM;
             if (!rc) rc = launch_amsc_pack_J(h, h->d_amsc_J);
+            if (rc && h->d_amsc_J) { dev_free(h->d_amsc_J); h->d_amsc_J = nullptr; }      // never sweep on half-packed bonds
         }
         if (!rc) rc = ensure_store(h, Store::Amsc, 0);
         for (int pass = 0; pass < n && !rc; ++pass) {
@@ -534,7 +578,9 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
                 }
             }
         }
-        const bool use_grid3 = use_3d && !resident_done && n >= 2 && !h->no_resident && !resident3d_supported(h, T) && grid3d_supported(h, T);
+        // (measured at L = 256: with two jobs of a colour per warp and k >= 4 the per-pass kernels are 5 % faster)
+        const bool use_grid3 = use_3d && !resident_done && n >= 2 && !h->no_resident && !resident3d_supported(h, T) && grid3d_supported(h, T) &&
+                               (k < 4 || (uint64_t)h->R * h->N / 1024u <= 148u * 20u);
         if (use_grid3 && !rc) {
             const size_t xb = grid3d_xedge_bytes(h), ab = want_series ? grid3d_acc_bytes(h, n) : 0;
             if (xb > h->xedge_bytes) {

@@ -42,13 +42,14 @@ __device__ __forceinline__ void st_x64v2(unsigned long long* p, unsigned long lo
 
 template <bool BITS, bool HASJ, unsigned long long HP3 = kNoSpec3>
 __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
-    extern __shared__ uint32_t grid3_smem[];                  // per warp: [colour][job][word][lane]
+    constexpr uint32_t NSLOT = 2 + 9;                         // two words + the job's constants (decoded once) per lane and job
+    extern __shared__ uint32_t grid3_smem[];                  // per warp: [colour][job][slot][lane]
     const Plane3Args& A = R.P;
     const int lane = threadIdx.x & 31;
     const uint32_t wg = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), W = gridDim.x * (blockDim.x >> 5);
     const int sub = lane >> 3, lz = lane & 7;
     const uint32_t B = (uint32_t)A.B, Mw = R.jobs_per_warp;
-    uint32_t* const ws = grid3_smem + (size_t)(threadIdx.x >> 5) * (2u * Mw * 2u * 32u) + lane;
+    uint32_t* const ws = grid3_smem + (size_t)(threadIdx.x >> 5) * (2u * Mw * NSLOT * 32u) + lane;
     const uint2* lut = kByteLutGlobal.e;
     const bool series = R.acc != nullptr;
 
@@ -122,7 +123,20 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
             atomicAdd(reinterpret_cast<unsigned long long*>(a + 1), (unsigned long long)unsat);
         }
     };
-    auto sm_slot = [&](int C, uint32_t m) { return ws + (size_t)((uint32_t)C * Mw + m) * 64u; };
+    auto sm_slot = [&](int C, uint32_t m) { return ws + (size_t)((uint32_t)C * Mw + m) * (NSLOT * 32u); };
+    auto sm_job = [&](int C, uint32_t m) {                             // the constants parked by the prologue
+        const uint32_t* p = sm_slot(C, m) + 64;
+        Job jb;
+        jb.self = p[0]; jb.xm = p[32]; jb.xp = p[64]; jb.ym = p[96]; jb.yp = p[128]; jb.zm = p[160]; jb.zp = p[192];
+        const uint32_t xyz = p[224];
+        jb.t.tx = (int)(xyz & 0x3ffu); jb.t.ty = (int)((xyz >> 10) & 0x3ffu); jb.t.tz = (int)(xyz >> 20); jb.t.r = (int)p[256];
+        return jb;
+    };
+    auto sm_put_job = [&](const Job& jb, int C, uint32_t m) {
+        uint32_t* p = sm_slot(C, m) + 64;
+        p[0] = jb.self; p[32] = jb.xm; p[64] = jb.xp; p[96] = jb.ym; p[128] = jb.yp; p[160] = jb.zm; p[192] = jb.zp;
+        p[224] = (uint32_t)jb.t.tx | ((uint32_t)jb.t.ty << 10) | ((uint32_t)jb.t.tz << 20); p[256] = (uint32_t)jb.t.r;
+    };
 
     // records -> shared memory; the colour-1 tiles publish their initial faces (version 1 = what phase 0 waits for)
     for (int C = 0; C < 2; ++C)
@@ -134,6 +148,7 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
             load_slice<BITS>(A, jb.t, lz, s);
             uint32_t* p = sm_slot(C, m);
             p[0] = s.S[0]; p[32] = s.S[1];
+            sm_put_job(jb, C, m);
             if (C == 1) publish(s, jb.self, 1u);
         }
 
@@ -144,7 +159,7 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
             for (uint32_t m = 0; m < Mw; ++m) {
                 const uint32_t job = wg + m * W;
                 if (job >= R.jobs_total) break;
-                const Job jb = decode(job, C);
+                const Job jb = sm_job(C, m);
                 Slice s;
                 uint32_t* p = sm_slot(C, m);
                 s.S[0] = p[0]; s.S[1] = p[32];
@@ -171,7 +186,7 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
         for (uint32_t m = 0; m < Mw; ++m) {
             const uint32_t job = wg + m * W;
             if (job >= R.jobs_total) break;
-            const Job jb = decode(job, 0);
+            const Job jb = sm_job(0, m);
             Slice s;
             const uint32_t* p = sm_slot(0, m);
             s.S[0] = p[0]; s.S[1] = p[32];
@@ -183,7 +198,7 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
         for (uint32_t m = 0; m < Mw; ++m) {
             const uint32_t job = wg + m * W;
             if (job >= R.jobs_total) break;
-            const Job jb = decode(job, C);
+            const Job jb = sm_job(C, m);
             Slice s;
             const uint32_t* p = sm_slot(C, m);
             s.S[0] = p[0]; s.S[1] = p[32];

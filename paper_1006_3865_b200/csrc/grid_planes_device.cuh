@@ -42,14 +42,15 @@ template <int T, bool BITS, bool HASJ, uint32_t HP = kNoSpec>
 __global__ void __launch_bounds__(128, 5) k_grid_planes(GridArgs R) {
     using G = PG<T>;
     constexpr int NWORDS = 2 * G::NW;                         // words per lane and job: S[cc][gx]
-    extern __shared__ uint32_t grid_smem[];                   // per warp: [colour][job][word][lane]
+    constexpr int NSLOT = NWORDS + 7;                         // ... + the job's constants (decoded once): self, nU, nD, nL, nR, tx | ty << 16, r
+    extern __shared__ uint32_t grid_smem[];                   // per warp: [colour][job][slot][lane]
     const PlaneArgs& A = R.P;
     const int lane = threadIdx.x & 31;
     const uint32_t wg = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), W = gridDim.x * (blockDim.x >> 5);
     const int sub = lane / G::LPT, Y = lane % G::LPT;
     const uint32_t B = (uint32_t)A.B, hb = B >> 1, per_rep = R.tiles_per_colour;
     const uint32_t Mw = R.jobs_per_warp;
-    uint32_t* const ws = grid_smem + (size_t)(threadIdx.x >> 5) * (2u * Mw * NWORDS * 32u) + lane;
+    uint32_t* const ws = grid_smem + (size_t)(threadIdx.x >> 5) * (2u * Mw * NSLOT * 32u) + lane;
     const uint2* lut = kByteLutGlobal.e;
     const bool series = R.acc != nullptr;
 
@@ -137,15 +138,25 @@ __global__ void __launch_bounds__(128, 5) k_grid_planes(GridArgs R) {
             atomicAdd(reinterpret_cast<unsigned long long*>(a + 1), (unsigned long long)unsat);
         }
     };
+    auto sm_job = [&](int C, uint32_t m) {                             // the constants parked by the prologue
+        const uint32_t* p = ws + (size_t)((uint32_t)C * Mw + m) * (NSLOT * 32u) + NWORDS * 32;
+        const uint32_t xy = p[5 * 32];
+        return Job{(int)p[6 * 32], (int)(xy & 0xffffu), (int)(xy >> 16), p[0], p[1 * 32], p[2 * 32], p[3 * 32], p[4 * 32]};
+    };
+    auto sm_put_job = [&](const Job& jb, int C, uint32_t m) {
+        uint32_t* p = ws + (size_t)((uint32_t)C * Mw + m) * (NSLOT * 32u) + NWORDS * 32;
+        p[0] = jb.self; p[1 * 32] = jb.nU; p[2 * 32] = jb.nD; p[3 * 32] = jb.nL; p[4 * 32] = jb.nR;
+        p[5 * 32] = (uint32_t)jb.tx | ((uint32_t)jb.ty << 16); p[6 * 32] = (uint32_t)jb.r;
+    };
     auto sm_load = [&](TileRegs<T>& tt, int C, uint32_t m) {
-        const uint32_t* p = ws + (size_t)((uint32_t)C * Mw + m) * (NWORDS * 32u);
+        const uint32_t* p = ws + (size_t)((uint32_t)C * Mw + m) * (NSLOT * 32u);
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
             for (int gx = 0; gx < G::NW; ++gx) tt.S[cc][gx] = p[(cc * G::NW + gx) * 32];
     };
     auto sm_store = [&](const TileRegs<T>& tt, int C, uint32_t m) {
-        uint32_t* p = ws + (size_t)((uint32_t)C * Mw + m) * (NWORDS * 32u);
+        uint32_t* p = ws + (size_t)((uint32_t)C * Mw + m) * (NSLOT * 32u);
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
@@ -161,6 +172,7 @@ __global__ void __launch_bounds__(128, 5) k_grid_planes(GridArgs R) {
             TileRegs<T> tt;
             load_tile<T, BITS>(A, jb.r, jb.tx, jb.ty, Y, sub * G::LPT, tt);
             sm_store(tt, C, m);
+            sm_put_job(jb, C, m);
             if (C == 1) publish(tt, jb.self, 1u);
         }
 
@@ -171,7 +183,7 @@ __global__ void __launch_bounds__(128, 5) k_grid_planes(GridArgs R) {
             for (uint32_t m = 0; m < Mw; ++m) {
                 const uint32_t job = wg + m * W;
                 if (job >= R.jobs_total) break;                           // warp-uniform
-                const Job jb = decode(job, C);
+                const Job jb = sm_job(C, m);
                 TileRegs<T> tt;
                 sm_load(tt, C, m);
                 uint4 Jw[2][G::NW];
@@ -198,7 +210,7 @@ __global__ void __launch_bounds__(128, 5) k_grid_planes(GridArgs R) {
         for (uint32_t m = 0; m < Mw; ++m) {
             const uint32_t job = wg + m * W;
             if (job >= R.jobs_total) break;
-            const Job jb = decode(job, 0);
+            const Job jb = sm_job(0, m);
             TileRegs<T> tt;
             sm_load(tt, 0, m);
             uint4 Jw[2][G::NW];
@@ -210,7 +222,7 @@ __global__ void __launch_bounds__(128, 5) k_grid_planes(GridArgs R) {
         for (uint32_t m = 0; m < Mw; ++m) {
             const uint32_t job = wg + m * W;
             if (job >= R.jobs_total) break;
-            const Job jb = decode(job, C);
+            const Job jb = sm_job(C, m);
             TileRegs<T> tt;
             sm_load(tt, C, m);
             store_tile<T, BITS>(A, jb.r, jb.tx, jb.ty, Y, sub, tt, lut);

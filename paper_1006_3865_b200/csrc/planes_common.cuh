@@ -16,8 +16,10 @@ constexpr int kLutChain = (~0xF0 & 0xAA) | (~(0xF0 ^ 0xAA) & 0xCC);    // (~p & 
 constexpr int kLutNe = 0xF0 | (0xCC ^ 0xAA);                            // ne | (p ^ u): ne=a, p=b, u=c
 
 // Own-tile data is read once and written back by the same lane: plain (coherent) loads that do not allocate in
-// L1.  Halo data belongs to tiles of the other coarse colour, which this launch never writes, so it may
-// use the read-only path (__ldg).
+// L1.  Halo data belongs to tiles of the other coarse colour, which this launch never writes — but with
+// programmatic dependent launch this grid may be resident while the previous colour's grid is still writing those very
+// words, and ld.global.nc requires data that is read-only for the whole lifetime of the kernel: so the halos, too, are read
+// with coherent loads after griddepcontrol.wait (ldh128 / ldh64 / ldh32), never through the read-only path.
 // L2 policy for the tile bodies: when the records exceed L2 they are touched once per pass, so they are
 // streamed (evict-first) and the small edge copies the next launch needs stay resident (+5 % at L = 16384);
 // when the records fit L2 the normal policy keeps them there (streaming costs 7-10 % at L <= 8192).
@@ -36,6 +38,26 @@ __device__ __forceinline__ uint4 ldg128(const void* p, uint64_t pol) {
 __device__ __forceinline__ uint32_t ldg32(const void* p) {
     uint32_t v;
     asm volatile("ld.global.L1::no_allocate.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint4 ldh128(const void* p) {
+    uint4 v;
+    asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint2 ldh64(const void* p) {
+    uint2 v;
+    asm volatile("ld.global.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint32_t ldh32(const void* p) {
+    uint32_t v;
+    asm volatile("ld.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint32_t ldh8(const void* p) {
+    uint32_t v;
+    asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ void stg128(void* p, uint4 v) {

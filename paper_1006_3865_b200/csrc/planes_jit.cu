@@ -65,12 +65,27 @@ struct Nvrtc {
     }
 };
 
+// The cache is bounded (a temperature scan or a parallel-tempering run meets a new pair of threshold heads at every beta):
+// beyond 64 entries (ISING_JIT_CACHE overrides, for tests) the least recently used kernel is dropped and its cubin unloaded (after a synchronisation of
+// the library's stream, so that no launch of it is still in flight).  Failed compilations are remembered as nullptr entries
+// and age out the same way.
+constexpr size_t kJitCacheMaxDefault = 64;
+static size_t jit_cache_max() {
+    static const size_t v = getenv("ISING_JIT_CACHE") ? (size_t)atoi(getenv("ISING_JIT_CACHE")) : kJitCacheMaxDefault;   // testing aid
+    return v < 1 ? 1 : v;
+}
+
+struct JitEntry {
+    cudaKernel_t kernel = nullptr;               // nullptr = tried and failed
+    cudaLibrary_t lib = nullptr;
+    uint64_t last_use = 0;
+};
+
 struct JitState {
     std::mutex mu;
-    std::map<std::string, cudaKernel_t> cache;   // name expression + macros -> kernel; nullptr = tried and failed
-    std::vector<cudaLibrary_t> libs;
+    std::map<std::string, JitEntry> cache;       // name expression + macros -> kernel
     std::string last_log;
-    uint64_t compiled = 0;
+    uint64_t compiled = 0, clock = 0, evicted = 0;
 };
 
 JitState& state() {
@@ -78,7 +93,8 @@ JitState& state() {
     return s;
 }
 
-cudaKernel_t compile_one(const char* source, const std::string& expr, const std::vector<std::string>& defs, std::string& log) {
+cudaKernel_t compile_one(const char* source, const std::string& expr, const std::vector<std::string>& defs, std::string& log,
+                         cudaLibrary_t* lib_out) {
     static Nvrtc rt;
     if (!rt.ok) { log = "libnvrtc not available"; return nullptr; }
     nvrtcProgram_t prog = nullptr;
@@ -109,24 +125,44 @@ cudaKernel_t compile_one(const char* source, const std::string& expr, const std:
             cudaLibraryUnload(lib);
             break;
         }
-        state().libs.push_back(lib);
+        *lib_out = lib;
     } while (false);
     rt.DestroyProgram(&prog);
     return kernel;
 }
 
 cudaKernel_t cached(const char* source, const std::string& expr, const std::vector<std::string>& defs) {
-    JitState& s = state();
-    std::lock_guard<std::mutex> lock(s.mu);
-    std::string key = expr;
-    for (const std::string& d : defs) key += " " + d;
-    auto it = s.cache.find(key);
-    if (it != s.cache.end()) return it->second;
-    std::string log;
-    cudaKernel_t k = compile_one(source, expr, defs, log);
-    if (k) ++s.compiled; else s.last_log = log;
-    s.cache[key] = k;
-    return k;
+    try {                                        // std::string / std::map may throw: nothing may cross the C ABI
+        JitState& s = state();
+        std::lock_guard<std::mutex> lock(s.mu);
+        std::string key = expr;
+        for (const std::string& d : defs) key += " " + d;
+        auto it = s.cache.find(key);
+        if (it != s.cache.end()) {
+            it->second.last_use = ++s.clock;
+            return it->second.kernel;
+        }
+        if (s.cache.size() >= jit_cache_max()) {
+            auto lru = s.cache.begin();
+            for (auto jt = s.cache.begin(); jt != s.cache.end(); ++jt)
+                if (jt->second.last_use < lru->second.last_use) lru = jt;
+            if (lru->second.lib) {
+                cudaStreamSynchronize(hooks().stream);
+                cudaLibraryUnload(lru->second.lib);
+            }
+            s.cache.erase(lru);
+            ++s.evicted;
+        }
+        std::string log;
+        JitEntry e;
+        e.kernel = compile_one(source, expr, defs, log, &e.lib);
+        e.last_use = ++s.clock;
+        if (e.kernel) ++s.compiled; else s.last_log = log;
+        s.cache[key] = e;
+        return e.kernel;
+    } catch (...) {
+        return nullptr;                          // the caller falls back to the pre-compiled kernel
+    }
 }
 
 }  // namespace

@@ -662,7 +662,7 @@ int launch_grid3d_one(Grid3Args& R, cudaKernel_t spec, bool* fits) {
     for (uint32_t M = 1; M <= max_m; ++M) {
         const uint32_t warps_needed = (R.jobs_total + M - 1) / M;
         const int wpb = warps_needed <= (uint32_t)sms * 4u ? 1 : (warps_needed <= (uint32_t)sms * 8u ? 2 : 4);
-        const size_t smem = (size_t)wpb * 2u * M * 2u * 32u * sizeof(uint32_t);
+        const size_t smem = (size_t)wpb * 2u * M * (2u + 9u) * 32u * sizeof(uint32_t);      // words + constants of every job
         int occ = 0;
         ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, wpb * 32, smem));
         const uint32_t grid = (warps_needed + wpb - 1) / wpb;

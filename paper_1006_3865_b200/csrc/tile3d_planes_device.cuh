@@ -97,17 +97,17 @@ __device__ __forceinline__ void load_slice(const Plane3Args& A, const Tile3& t, 
         s.S[0] = pack16(pack16(0u, v[1]), v[0]);
         s.S[1] = pack16(pack16(0u, v[3]), v[2]);
     }
-    s.xl = __ldg(reinterpret_cast<const uint32_t*>(fXm + kXR) + lz);     // left tile's x = 7 sites, bit 4ly
-    s.xr = __ldg(reinterpret_cast<const uint32_t*>(fXp + kXL) + lz);     // right tile's x = 0 sites, bit 4ly+3
-    s.ym = __ldg(fYm + kYR + lz);                                        // tile in front: its row y = 7
-    s.yp = __ldg(fYp + kYL + lz);                                        // tile behind: its row y = 0
+    s.xl = ldh32(fXm + kXR + 4 * lz);     // left tile's x = 7 sites, bit 4ly
+    s.xr = ldh32(fXp + kXL + 4 * lz);     // right tile's x = 0 sites, bit 4ly+3
+    s.ym = ldh8(fYm + kYR + lz);                                        // tile in front: its row y = 7
+    s.yp = ldh8(fYp + kYL + lz);                                        // tile behind: its row y = 0
     s.zm[0] = s.zm[1] = s.zp[0] = s.zp[1] = 0u;
     if (lz == 0) {
-        const uint2 w = __ldg(reinterpret_cast<const uint2*>(rec_of(t.tz == 0 ? B - 1 : t.tz - 1, t.ty, t.tx) + BODY + kZR));
+        const uint2 w = ldh64(rec_of(t.tz == 0 ? B - 1 : t.tz - 1, t.ty, t.tx) + BODY + kZR);
         s.zm[0] = w.x; s.zm[1] = w.y;
     }
     if (lz == 7) {
-        const uint2 w = __ldg(reinterpret_cast<const uint2*>(rec_of(t.tz == B - 1 ? 0 : t.tz + 1, t.ty, t.tx) + BODY + kZL));
+        const uint2 w = ldh64(rec_of(t.tz == B - 1 ? 0 : t.tz + 1, t.ty, t.tx) + BODY + kZL);
         s.zp[0] = w.x; s.zp[1] = w.y;
     }
 }

@@ -959,7 +959,7 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit) {
         const uint32_t warps_needed = (R.jobs_total + M - 1) / M;
         // few jobs: one warp per CTA, so that the CTAs (and the schedulers they land on) spread over all SMs
         const int wpb = warps_needed <= (uint32_t)sms * 4u ? 1 : (warps_needed <= (uint32_t)sms * 8u ? 2 : 4);
-        const size_t smem = (size_t)wpb * 2u * M * (2u * PG<T>::NW) * 32u * sizeof(uint32_t);
+        const size_t smem = (size_t)wpb * 2u * M * (2u * PG<T>::NW + 7u) * 32u * sizeof(uint32_t);     // words + constants of every job
         if (smem > 200 * 1024) break;
         int occ = 0;
         ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, wpb * 32, smem));

@@ -123,13 +123,13 @@ __device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int
     // halo rows: the first lane of a tile takes BOT of the tile above, the last lane TOP of the tile below
     uint4 hv = make_uint4(0u, 0u, 0u, 0u);
     if (Y == 0 || Y == G::LPT - 1)
-        hv = __ldg(reinterpret_cast<const uint4*>(rec_of(row0 + (Y == 0 ? tyU : tyD) * B + utx) + BODY + (Y == 0 ? G::E_BOT : G::E_TOP)));
+        hv = ldh128(rec_of(row0 + (Y == 0 ? tyU : tyD) * B + utx) + BODY + (Y == 0 ? G::E_BOT : G::E_TOP));
     t.vrow[0][0] = hv.x;
     if (G::NW == 2) { t.vrow[0][1] = hv.y; t.vrow[1][0] = hv.z; t.vrow[1][1] = hv.w; }
     else t.vrow[1][0] = hv.y;
     // halo columns: the left tile's right column, the right tile's left column (same address for every lane of a tile)
-    const uint2 cl = __ldg(reinterpret_cast<const uint2*>(rec_of(rowc + txL) + BODY + G::E_COL + 8));   // {R0, R1}
-    const uint2 cr = __ldg(reinterpret_cast<const uint2*>(rec_of(rowc + txR) + BODY + G::E_COL));       // {L0, L1}
+    const uint2 cl = ldh64(rec_of(rowc + txL) + BODY + G::E_COL + 8);   // {R0, R1}
+    const uint2 cr = ldh64(rec_of(rowc + txR) + BODY + G::E_COL);       // {L0, L1}
     t.hL0 = (cl.x >> Y) & 1u; t.hL1 = (cl.y >> Y) & 1u;
     t.hR0 = (cr.x >> Y) & 1u; t.hR1 = (cr.y >> Y) & 1u;
     (void)lane_base;

@@ -52,6 +52,11 @@ FAMILIES = {
     "resident_planes_pmj": (2, 128, 64, 1, 4, 0.8, 11, "planes", "bits", 0, "auto", "resident_planes_bits"),
     "resident_plain": (2, 128, 0, 2, 4, BC2, None, "planes", "int8", 0, "auto", "resident_plain_i8"),
     "resident_masked": (2, 128, 8, 1, 4, BC2, None, "planes", "int8", 0, "auto", "resident_masked_i8"),
+    "grid_planes": (2, 768, 32, 2, 4, BC2, None, "planes", "int8", 0, "off", "grid_planes_i8"),
+    "grid_planes_jit": (2, 768, 64, 1, 4, BC2, None, "planes", "bits", 0, "on", "grid_planes_bits"),
+    "grid_planes_pmj": (2, 640, 32, 1, 4, 1.0, 5, "planes", "int8", 0, "auto", "grid_planes_i8"),
+    "grid3d": (3, 80, 8, 1, 4, BC3, None, "planes", "int8", 0, "off", "grid3d_planes_i8"),
+    "grid3d_jit": (3, 80, 8, 2, 4, BC3, None, "planes", "bits", 0, "on", "grid3d_planes_bits"),
     "plain64": (2, 64, 0, 1, 6, BC2, None, "planes", "int8", 0, "auto", "plain64_planes_i8"),
     "tile_plain": (2, 704, 0, 1, 4, BC2, None, "planes", "int8", 0, "auto", "tile_plain_i8"),
     "tile_masked": (2, 704, 16, 1, 4, BC2, None, "planes", "bits", 0, "auto", "tile_masked_bits"),
@@ -180,3 +185,52 @@ def test_config3_full_length_int8_equals_bits(P, orc, tile, k):
         assert torch.equal(sa, sb), "pre-compiled and run-time specialised kernels differ after 200 passes"
         c.destroy()
     a.destroy(); b.destroy()
+
+
+@pytest.mark.parametrize("dim,L,tile", [(2, 128, 32), (2, 64, 0), (3, 16, 8), (2, 1024, 32)])
+def test_thresholds_straddling_2p32(P, orc, dim, L, tile):
+    """0 < beta < ~1.4e-17: exp(-4 beta) rounds to 1 (thr[1] = 2^32: always accept) while exp(-8 beta) does not
+    (thr[2] = 2^32 - 1).  The multi-spin kernels fold "thr = 2^32" into one mask, so this call must take the generic
+    kernels, which compare each threshold on its own; same trajectory as the oracle."""
+    beta = 1e-17
+    assert orc.thresholds(beta, dim)[0] == 1 << 32 and orc.thresholds(beta, dim)[1] == (1 << 32) - 1
+    assert P.ising_thresholds(beta, dim) == orc.thresholds(beta, dim)
+    g = P.Ising(dim, L, seed=5); o = orc.Oracle(dim, L, seed=5)
+    g.sweep(beta, 2, tile, 2); o.sweep(beta, 2, tile, 2)
+    assert g.sweep_path() == "generic"
+    _same_state(g, o)
+    g.sweep(0.4, 2, tile, 1); o.sweep(0.4, 2, tile, 1)           # and the fast kernels are back afterwards
+    assert g.sweep_path() != "generic"
+    _same_state(g, o)
+
+
+def test_jit_cache_is_bounded_and_allocations_keep_their_owner():
+    """(a) The cache of run-time specialised kernels evicts the least recently used entry (ISING_JIT_CACHE=3 here; 64 by
+    default) and re-compiles on demand: a temperature scan stays correct.  (b) A block is released through the hook it was
+    allocated with, whatever ising_set_device_hooks was called with in between.  Fresh process: both touch process state."""
+    import os, subprocess, sys
+    code = (
+        "import ctypes as C, numpy as np, torch, paper_1006_3865_b200 as P\n"
+        "from paper_1006_3865_b200 import binding as B\n"
+        "from oracle import oracle as O\n"
+        "a = P.Ising(2, 64, seed=1)\n"                       # allocated with cudaMalloc (no hooks yet)
+        "P.use_torch()\n"
+        "b = P.Ising(2, 64, seed=2)\n"                       # allocated through torch
+        "live = len(B._live)\n"
+        "a.sweep(0.4, 2, 32, 1); a.destroy()\n"              # cudaFree, not the torch hook
+        "assert len(B._live) >= live - 1\n"
+        "assert P.lib().ising_set_device_hooks(None, None, None) == 0\n"
+        "b.sweep(0.4, 2, 32, 1); b.destroy()\n"              # the torch hook, not cudaFree
+        "assert len(B._live) < live\n"
+        "P.use_torch()\n"
+        "g = P.Ising(2, 128, seed=5); o = O.Oracle(2, 128, seed=5)\n"
+        "g.set_jit('on'); g.force_path(2)\n"
+        "for beta in (0.30, 0.35, 0.40, 0.45, 0.50, 0.30, 0.55, 0.35):\n"
+        "    g.sweep(beta, 2, 32, 1); o.sweep(beta, 2, 32, 1)\n"
+        "    assert g.last_sweep_specialized()\n"
+        "assert np.array_equal(np.asarray(g.copy_spins()), o.spins())\n"
+        "print('owners and cache ok')\n")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, ISING_JIT_CACHE="3"),
+                         capture_output=True, text=True, timeout=900)
+    assert out.returncode == 0 and "owners and cache ok" in out.stdout, out.stderr[-3000:]
