@@ -269,7 +269,8 @@ class Ising:
         return lib().ising_sweep_path(self._h).decode()
 
     def force_path(self, mode) -> None:
-        """0 / False: automatic; 1 / True: generic kernels only; 2: automatic but never the cluster-resident kernel."""
+        """0 / False: automatic; 1 / True: generic kernels only; 2: a launch per colour (no cluster / grid / data-flow kernel);
+        3: no data-flow kernel; 4: no cluster / grid resident kernels (the data-flow kernel may run at any size and k)."""
         _check(lib().ising_force_path(self._h, int(mode)))
 
 

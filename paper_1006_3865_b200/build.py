@@ -31,7 +31,7 @@ def _stale() -> bool:
 
 
 JIT_SOURCES = {   # generated file -> device headers in inclusion order
-    "jit_source.inc": ["philox.cuh", "planes_common.cuh", "tile_planes_device.cuh", "grid_planes_device.cuh"],
+    "jit_source.inc": ["philox.cuh", "planes_common.cuh", "tile_planes_device.cuh", "grid_planes_device.cuh", "flow_planes_device.cuh"],
     "jit_source3d.inc": ["philox.cuh", "planes_common.cuh", "tile3d_planes_device.cuh", "grid3d_device.cuh"],
 }
 

@@ -415,7 +415,7 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
     // (and tiles of 128, 256, ...: whole register tiles switched on and off)
     const int Tc = (T >= 2 && (T & (T - 1)) == 0 && T != 32 && T != 64 && T != h->L) ? T : 0;
     if (!h->force_generic && !use_plain64 && !use_amsc && h->rng == ISING_RNG_PLANES && (T == h->L || Tc) && h->dim == 2 && n > 0) {
-        if (!h->no_resident) Tp = resident_planes_supported(h, 32) ? 32 : (resident_planes_supported(h, 64) ? 64 : 0);
+        if (!h->no_resident && !h->no_onchip) Tp = resident_planes_supported(h, 32) ? 32 : (resident_planes_supported(h, 64) ? 64 : 0);
         Tp_resident = Tp != 0;
         if (!Tp) Tp = tile_planes_supported(h, 64) ? 64 : (tile_planes_supported(h, 32) ? 32 : 0);   // large L: a launch per half-sweep
     }
@@ -463,7 +463,7 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             if (!rc) rc = launch_convert_couplings3d(h, h->d_Jtiles);
             if (!rc) h->Jtiles_tile = 8;
         }
-        if (!rc && !h->no_resident && resident3d_supported(h, 8)) {
+        if (!rc && !h->no_resident && !h->no_onchip && resident3d_supported(h, 8)) {
             if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M, true, Tc3) == 0) {
                 h->last_path = Tc3 ? (bits ? "resident3d_masked_bits" : "resident3d_masked_i8") : (bits ? "resident3d_plain_bits" : "resident3d_plain_i8");
                 plain_done = true;
@@ -529,10 +529,10 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
                              (h->jit_mode == ISING_JIT_AUTO && (double)n * k * (double)h->N * h->R >= 134217728.0));
         h->last_jit = 0;
         // small lattices, several passes, nothing to measure in between: the whole call in one cluster launch
-        const bool use_resident = use_planes && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident &&
+        const bool use_resident = use_planes && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident && !h->no_onchip &&
                                   resident_planes_supported(h, T);
         bool resident_done = false;
-        const bool use_resident3 = use_3d && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident &&
+        const bool use_resident3 = use_3d && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident && !h->no_onchip &&
                                    resident3d_supported(h, T);
         if (use_resident3 && !rc) {
             if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M, false, 0) == 0) {
@@ -552,7 +552,7 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         }
         // 2D lattices beyond the cluster (more than 64 jobs per colour) that still fit on chip: one cooperative launch, tiles in
         // the shared memory / registers of all SMs, boundary words exchanged through L2 (k_grid_planes)
-        const bool use_grid = use_planes && !resident_done && n >= 2 && !h->no_resident &&
+        const bool use_grid = use_planes && !resident_done && n >= 2 && !h->no_resident && !h->no_onchip &&
                               !resident_planes_supported(h, T) && grid_planes_supported(h, T);
         if (use_grid && !rc) {
             const size_t xb = grid_planes_xedge_bytes(h, T), ab = want_series ? grid_planes_acc_bytes(h, n) : 0;
@@ -579,7 +579,27 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
             }
         }
         // (measured at L = 256: with two jobs of a colour per warp and k >= 4 the per-pass kernels are 5 % faster)
-        const bool use_grid3 = use_3d && !resident_done && n >= 2 && !h->no_resident && !resident3d_supported(h, T) && grid3d_supported(h, T) &&
+        // HBM-resident 2D lattices, several passes, nothing to measure in between, k = 1 (the HBM-bound case): one persistent
+        // launch, colours ordered by data flow (k_flow_planes: +2.5 % at L = 16384, +5 % at L = 8192; for k >= 2 the register
+        // budget of the persistent loop costs more than the idle launch tails it removes: a launch per colour)
+        const bool use_flow = use_planes && !resident_done && !want_series && !h->no_resident && !h->no_flow && (k == 1 || h->no_onchip) &&
+                              flow_planes_supported(h, T, n);
+        if (use_flow && !rc) {
+            const size_t sb = flow_planes_scratch_bytes(h, T);
+            if (sb > h->xedge_bytes) {
+                cudaStreamSynchronize(st);
+                dev_free(h->d_xedge); h->xedge_bytes = 0;
+                h->d_xedge = dev_alloc(sb);
+                if (!h->d_xedge) rc = ISING_ENOMEM; else h->xedge_bytes = sb;
+            }
+            if (!rc && launch_flow_planes(h, acc, T, bits, n, k, h->t, h->d_xedge, use_jit) == 0) {
+                h->last_path = bits ? "flow_planes_bits" : "flow_planes_i8";
+                resident_done = true;
+            } else if (!rc) {
+                cudaGetLastError();
+            }
+        }
+        const bool use_grid3 = use_3d && !resident_done && n >= 2 && !h->no_resident && !h->no_onchip && !resident3d_supported(h, T) && grid3d_supported(h, T) &&
                                (k < 4 || (uint64_t)h->R * h->N / 1024u <= 148u * 20u);
         if (use_grid3 && !rc) {
             const size_t xb = grid3d_xedge_bytes(h), ab = want_series ? grid3d_acc_bytes(h, n) : 0;
@@ -823,6 +843,8 @@ int ising_force_path(ising_handle h, int generic_only) {
     if (!h) { set_error("ising_force_path: NULL handle"); return ISING_EINVAL; }
     h->force_generic = generic_only == 1 ? 1 : 0;
     h->no_resident = generic_only == 2 ? 1 : 0;
+    h->no_flow = generic_only == 3 ? 1 : 0;
+    h->no_onchip = generic_only == 4 ? 1 : 0;
     return 0;
 }
 

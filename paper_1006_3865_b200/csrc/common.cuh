@@ -118,6 +118,8 @@ struct ising_ctx {
     const char* last_path = "none";
     int force_generic = 0;
     int no_resident = 0;            // ising_force_path(h, 2): per-pass launches even where the cluster-resident kernel applies
+    int no_flow = 0;                // ising_force_path(h, 3): a launch per colour also where the persistent data-flow kernel applies
+    int no_onchip = 0;              // ising_force_path(h, 4): never the cluster / grid resident kernels (the data-flow kernel may run)
     int jit_mode = 0;               // ISING_JIT_AUTO / OFF / ON (ising_set_jit)
     int last_jit = 0;               // 1 if the last tile launch used a run-time specialised kernel
 };

@@ -47,6 +47,10 @@ size_t grid_planes_acc_bytes(const ising_ctx* h, int n);
 int launch_grid_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, void* d_xedge, void* d_acc,
                        long long* d_E, long long* d_M, bool use_jit);     // returns 1 (nothing launched) if the lattice does not fit
 
+bool flow_planes_supported(const ising_ctx* h, int T, int n);   // HBM-resident lattices, n >= 2 passes: one persistent launch, colours ordered by data flow
+size_t flow_planes_scratch_bytes(const ising_ctx* h, int T);
+int launch_flow_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, void* d_scratch, bool use_jit);
+
 // ---- tile3d_planes.cu: 3D multi-spin tile kernel, 8x8x8 tiles (RNG mapping "planes") ----------
 bool tile3d_supported(const ising_ctx* h, int T);
 size_t tile3d_bytes(const ising_ctx* h, bool bits);
@@ -75,9 +79,10 @@ int launch_amsc_to_canon(ising_ctx* h, const void* d_words, int8_t* d_canon);
 int launch_amsc_pass(ising_ctx* h, const Accept& acc, int T, int k, uint64_t t_first, const void* d_jwords);
 
 // ---- planes_jit.cu: run-time specialisation of k_tile_planes on the threshold head bits (NVRTC) ----
-cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R);
+cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R, int NS);   // NS: tiles per lane
 cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3);   // nullptr: not available
 cudaKernel_t grid3d_jit_kernel(bool bits, unsigned long long hp3);      // k_grid3d specialised on the three threshold heads
+cudaKernel_t flow_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R, int NS);   // k_flow_planes, specialised like k_tile_planes
 cudaKernel_t grid_jit_kernel(int T, bool bits, bool hasj, uint32_t hp);   // k_grid_planes specialised on the threshold heads
 uint64_t planes_jit_compiled();
 const char* planes_jit_last_log();

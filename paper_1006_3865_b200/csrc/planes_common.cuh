@@ -19,7 +19,8 @@ constexpr int kLutNe = 0xF0 | (0xCC ^ 0xAA);                            // ne | 
 // L1.  Halo data belongs to tiles of the other coarse colour, which this launch never writes — but with
 // programmatic dependent launch this grid may be resident while the previous colour's grid is still writing those very
 // words, and ld.global.nc requires data that is read-only for the whole lifetime of the kernel: so the halos, too, are read
-// with coherent loads after griddepcontrol.wait (ldh128 / ldh64 / ldh32), never through the read-only path.
+// with coherent loads after griddepcontrol.wait (ldh128 / ldh64 / ldh32), never through the read-only path;
+// and they are cached in L2 only (.cg), so that a persistent kernel (k_flow_planes) can never meet a stale copy in L1.
 // L2 policy for the tile bodies: when the records exceed L2 they are touched once per pass, so they are
 // streamed (evict-first) and the small edge copies the next launch needs stay resident (+5 % at L = 16384);
 // when the records fit L2 the normal policy keeps them there (streaming costs 7-10 % at L <= 8192).
@@ -42,22 +43,27 @@ __device__ __forceinline__ uint32_t ldg32(const void* p) {
 }
 __device__ __forceinline__ uint4 ldh128(const void* p) {
     uint4 v;
-    asm volatile("ld.global.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
+    asm volatile("ld.global.cg.v4.u32 {%0,%1,%2,%3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ uint2 ldh64(const void* p) {
     uint2 v;
-    asm volatile("ld.global.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p) : "memory");
+    asm volatile("ld.global.cg.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ uint32_t ldh32(const void* p) {
     uint32_t v;
-    asm volatile("ld.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    asm volatile("ld.global.cg.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
 __device__ __forceinline__ uint32_t ldh8(const void* p) {
     uint32_t v;
-    asm volatile("ld.global.u8 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    asm volatile("ld.global.cg.u8 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ uint2 lds64(uint32_t saddr) {
+    uint2 v;
+    asm volatile("ld.shared.v2.u32 {%0,%1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(saddr));
     return v;
 }
 __device__ __forceinline__ void stg128(void* p, uint4 v) {

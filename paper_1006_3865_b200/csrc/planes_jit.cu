@@ -169,9 +169,15 @@ cudaKernel_t cached(const char* source, const std::string& expr, const std::vect
 
 // The 2D kernel specialised for (T, BITS, HASJ, HP) and the geometry (B tiles per side, R replicas), compiled on
 // first use; nullptr if it cannot be had.
-cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R) {
+cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R, int NS) {
     char expr[160];
-    snprintf(expr, sizeof expr, "ising::jit::k_tile_planes<%d, %s, %s, %uu>", T, bits ? "true" : "false", hasj ? "true" : "false", hp);
+    snprintf(expr, sizeof expr, "ising::jit::k_tile_planes<%d, %s, %s, %uu, %d>", T, bits ? "true" : "false", hasj ? "true" : "false", hp, NS);
+    return cached(kJitSource, expr, {"-DISING_JIT_B=" + std::to_string(B) + "u", "-DISING_JIT_R=" + std::to_string(R) + "u"});
+}
+
+cudaKernel_t flow_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R, int NS) {
+    char expr[160];
+    snprintf(expr, sizeof expr, "ising::jit::k_flow_planes<%d, %s, %s, %uu, %d>", T, bits ? "true" : "false", hasj ? "true" : "false", hp, NS);
     return cached(kJitSource, expr, {"-DISING_JIT_B=" + std::to_string(B) + "u", "-DISING_JIT_R=" + std::to_string(R) + "u"});
 }
 

@@ -21,11 +21,13 @@
 //   bits  record = T*T/8 body + 64 edge bytes: word (cc, Y, gx) at ((cc*NW+gx)*LPT + Y)*4.
 //   edge  = bit-packed copies of the tile's own first / last block row and first / last column, written by
 //         the tile, so that every halo is one 16-byte run of ready-made words in the neighbour's record.
+#include <algorithm>
 #include <cooperative_groups.h>
 
 #include "kernels.h"
 #include "tile_planes_device.cuh"
 #include "grid_planes_device.cuh"
+#include "flow_planes_device.cuh"
 
 namespace ising {
 
@@ -310,9 +312,20 @@ __global__ void k_convert_couplings(const int8_t* __restrict__ J, uint32_t* __re
     if (h2) atomicOr(w + 3, bit);
 }
 
-template <int T, bool BITS>
-int launch_colour_planes(const PlaneArgs& A, bool use_jit, bool* used_jit) {
+// tiles per lane (k_tile_planes NS): two for tile 32 where the tile rows allow it, so that a warp job is 4096 sites at either
+// tile edge; ISING_SLOTS overrides (testing / tuning aid)
+static int plane_slots(int T, int B) {
+    static const int forced = getenv("ISING_SLOTS") ? atoi(getenv("ISING_SLOTS")) : 0;
+    int ns = forced ? forced : (T == 32 ? 2 : 1);
+    if (ns != 1 && ns != 2) ns = 1;
+    if ((B / 2) % ns) ns = 1;
+    return ns;
+}
+
+template <int T, bool BITS, int NS>
+int launch_colour_planes(PlaneArgs A, bool use_jit, bool* used_jit) {
     const int warps = kPlaneThreads / 32;
+    A.njobs /= (uint32_t)NS;
     const uint32_t grid = (A.njobs + warps - 1) / warps;
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(grid); cfg.blockDim = dim3(warps * 32); cfg.dynamicSmemBytes = 0; cfg.stream = hooks().stream;
@@ -322,18 +335,23 @@ int launch_colour_planes(const PlaneArgs& A, bool use_jit, bool* used_jit) {
     attr[0].val.programmaticStreamSerializationAllowed = pdl;
     cfg.attrs = attr; cfg.numAttrs = 1;
     // specialised on the threshold head bits (planes_jit.cu) when asked for and available, else run-time operands
-    cudaKernel_t spec = (use_jit && !A.force) ? planes_jit_kernel(T, BITS, A.jrec != nullptr, A.hp, A.B, A.R) : nullptr;
+    cudaKernel_t spec = (use_jit && !A.force) ? planes_jit_kernel(T, BITS, A.jrec != nullptr, A.hp, A.B, A.R, NS) : nullptr;
     if (spec) {
-        void* args[] = {const_cast<PlaneArgs*>(&A)};
+        void* args[] = {&A};
         ISING_CUDA_OK(cudaLaunchKernelExC(&cfg, (const void*)spec, args));
     } else if (A.jrec) {
-        ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes<T, BITS, true>, A));
+        ISING_CUDA_OK((cudaLaunchKernelEx(&cfg, k_tile_planes<T, BITS, true, kNoSpec, NS>, A)));
     } else {
-        ISING_CUDA_OK(cudaLaunchKernelEx(&cfg, k_tile_planes<T, BITS, false>, A));
+        ISING_CUDA_OK((cudaLaunchKernelEx(&cfg, k_tile_planes<T, BITS, false, kNoSpec, NS>, A)));
     }
     if (used_jit) *used_jit = spec != nullptr;
     count_launch();
     return 0;
+}
+
+template <int T, bool BITS>
+int launch_colour_planes(const PlaneArgs& A, bool use_jit, bool* used_jit) {
+    return plane_slots(T, A.B) == 2 ? launch_colour_planes<T, BITS, 2>(A, use_jit, used_jit) : launch_colour_planes<T, BITS, 1>(A, use_jit, used_jit);
 }
 
 }  // namespace
@@ -423,6 +441,7 @@ int launch_plain64(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uin
     PlaneArgs A;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;
+    A.seed0 = h->shared_sweep ? h->sweep_seed : h->seeds[0];
     A.L = 64; A.B = 1; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0; A.njobs = (uint32_t)h->R;
     A.magic_rep = A.magic_hb = 0;
     A.stream = 0;
@@ -449,6 +468,7 @@ int launch_observables_planes(ising_ctx* h, int T, bool bits, long long* d_E, lo
     PlaneArgs A = {};
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;
+    A.seed0 = h->shared_sweep ? h->sweep_seed : h->seeds[0];
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = 0; A.t_first = 0;
     A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
     const uint32_t tiles_per_colour = (uint32_t)((size_t)h->R * A.B * A.B / 2);
@@ -478,6 +498,7 @@ int launch_tile_planes_pass(ising_ctx* h, const Accept& acc, int T, bool bits, i
     PlaneArgs A;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;
+    A.seed0 = h->shared_sweep ? h->sweep_seed : h->seeds[0];
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first;
     A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
     A.stream = tile_planes_bytes(h, T, bits) > kL2StreamBytes ? 1u : 0u;
@@ -610,6 +631,7 @@ int launch_tile_planes_plain(ising_ctx* h, const Accept& acc, int T, bool bits, 
     PlaneArgs A;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;
+    A.seed0 = h->shared_sweep ? h->sweep_seed : h->seeds[0];
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0;
     A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
     A.stream = tile_planes_bytes(h, T, bits) > kL2StreamBytes ? 1u : 0u;
@@ -909,6 +931,7 @@ int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, in
     PlaneArgs& A = R.P;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;
+    A.seed0 = h->shared_sweep ? h->sweep_seed : h->seeds[0];
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0;
     A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;        // shared by the replicas
     A.stream = 0;
@@ -994,6 +1017,7 @@ int launch_grid_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n,
     PlaneArgs& A = R.P;
     A.tiles = (uint8_t*)h->d_tiles;
     A.seeds = h->d_sweep_seeds;
+    A.seed0 = h->shared_sweep ? h->sweep_seed : h->seeds[0];
     A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0;
     A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
     A.stream = 0;
@@ -1035,6 +1059,80 @@ bool grid_planes_supported(const ising_ctx* h, int T) {
     // memory of the resident warps is decided at launch (launch_grid_planes returns 1 if it does not)
     const uint64_t jobs = (uint64_t)h->R * (uint64_t)(h->L / T) * (uint64_t)(h->L / T) / 2u / (uint64_t)(64 / T);
     return jobs <= 148u * 32u * kGridMaxJobsPerWarp;
+}
+
+// ---- k_flow_planes (flow_planes_device.cuh): all n passes of an HBM-resident lattice in one persistent launch ----
+namespace {
+template <int T, bool BITS, int NS>
+int launch_flow_one(FlowArgs& F, bool use_jit, bool* used_jit) {
+    const PlaneArgs& A = F.P;
+    int dev = 0, sms = 0;
+    ISING_CUDA_OK(cudaGetDevice(&dev));
+    ISING_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    cudaKernel_t spec = (use_jit && !A.force) ? flow_jit_kernel(T, BITS, A.jrec != nullptr, A.hp, A.B, A.R, NS) : nullptr;
+    const void* fn = spec ? (const void*)spec
+                          : (A.jrec ? (const void*)k_flow_planes<T, BITS, true, kNoSpec, NS> : (const void*)k_flow_planes<T, BITS, false, kNoSpec, NS>);
+    int occ = 0;
+    ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kPlaneThreads, 0));
+    if (occ < 1) { set_error("k_flow_planes does not fit an SM"); return ISING_ECUDA; }
+    const uint32_t warps = kPlaneThreads / 32;
+    uint32_t grid = (uint32_t)sms * (uint32_t)occ;
+    grid = std::min<uint32_t>(grid, (F.jobs_per_phase + warps - 1) / warps);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kPlaneThreads); cfg.dynamicSmemBytes = 0; cfg.stream = hooks().stream;
+    void* args[] = {&F};
+    ISING_CUDA_OK(cudaLaunchKernelExC(&cfg, fn, args));
+    count_launch();
+    *used_jit = spec != nullptr;
+    return 0;
+}
+}  // namespace
+
+size_t flow_planes_scratch_bytes(const ising_ctx* h, int T) { return 256 + (size_t)h->R * (size_t)(h->L / T) * (size_t)(h->L / T) * sizeof(uint32_t); }
+
+bool flow_planes_supported(const ising_ctx* h, int T, int n) {
+    if (!tile_planes_supported(h, T)) return false;
+    // tickets are 32 bits wide: 2 n phases x jobs per phase (at most R * tiles / 2) must stay below 2^32
+    const uint64_t jobs = (uint64_t)h->R * (uint64_t)(h->L / T) * (uint64_t)(h->L / T) / 2u;
+    return n >= 2 && 2ull * (uint64_t)n * jobs < 0xffffffffull;
+}
+
+// n passes in one persistent launch.  d_scratch: flow_planes_scratch_bytes (ticket counter + one progress word per tile).
+int launch_flow_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, void* d_scratch, bool use_jit) {
+    FlowArgs F;
+    PlaneArgs& A = F.P;
+    A.tiles = (uint8_t*)h->d_tiles;
+    A.seeds = h->d_sweep_seeds;
+    A.seed0 = h->shared_sweep ? h->sweep_seed : h->seeds[0];
+    A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0;
+    A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
+    A.stream = tile_planes_bytes(h, T, bits) > kL2StreamBytes ? 1u : 0u;
+    A.magic_rep = fastdiv_magic((uint32_t)A.B * (uint32_t)A.B / 2u);
+    A.magic_hb = fastdiv_magic((uint32_t)A.B / 2u);
+    fill_accept(A, acc);
+    const int ns = plane_slots(T, A.B);
+    const uint32_t tiles_per_colour = (uint32_t)((size_t)h->R * A.B * A.B / 2);
+    const uint32_t per_job = (uint32_t)(64 / T) * (uint32_t)ns;
+    A.njobs = tiles_per_colour / per_job;
+    F.jobs_per_phase = A.njobs;
+    F.n_phases = 2u * (uint32_t)n;
+    F.phase_shift = (2u * (uint32_t)(A.B / 2) + per_job - 1) / per_job;      // two tile rows of jobs
+    if (F.phase_shift >= F.jobs_per_phase) F.phase_shift = 0;
+    F.magic_jp = fastdiv_magic(F.jobs_per_phase);
+    F.total = F.n_phases * F.jobs_per_phase;
+    F.ticket = (unsigned int*)d_scratch;
+    F.prog = (uint32_t*)((char*)d_scratch + 256);
+    ISING_CUDA_OK(cudaMemsetAsync(d_scratch, 0, flow_planes_scratch_bytes(h, T), hooks().stream));
+    bool used = false;
+    int rc;
+    if (ns == 2) rc = T == 64 ? (bits ? launch_flow_one<64, true, 2>(F, use_jit, &used) : launch_flow_one<64, false, 2>(F, use_jit, &used))
+                              : (bits ? launch_flow_one<32, true, 2>(F, use_jit, &used) : launch_flow_one<32, false, 2>(F, use_jit, &used));
+    else rc = T == 64 ? (bits ? launch_flow_one<64, true, 1>(F, use_jit, &used) : launch_flow_one<64, false, 1>(F, use_jit, &used))
+                      : (bits ? launch_flow_one<32, true, 1>(F, use_jit, &used) : launch_flow_one<32, false, 1>(F, use_jit, &used));
+    if (rc) return rc;
+    h->last_jit = used ? 1 : 0;
+    ISING_CUDA_OK(cudaGetLastError());
+    return 0;
 }
 
 }  // namespace ising

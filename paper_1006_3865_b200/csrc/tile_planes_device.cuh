@@ -37,6 +37,8 @@ struct PG {
 struct PlaneArgs {
     uint8_t* tiles;              // records, replica-major
     const uint64_t* seeds;
+    uint64_t seed0;              // seeds[0]: with one replica (known when the kernel is specialised at run time) the Philox key is a
+                                 // kernel parameter, i.e. uniform: its ten-round schedule lives in uniform registers, not in 20 per lane
     int L, B, R;
     int C;                       // coarse colour of this launch
     int k;
@@ -64,11 +66,12 @@ __device__ __forceinline__ uint32_t geom_B(const PlaneArgs& A) { return (uint32_
 __device__ __forceinline__ uint32_t geom_R(const PlaneArgs& A) { return (uint32_t)A.R; }
 #endif
 
-template <int T>
-__device__ __forceinline__ void job_tile(const PlaneArgs& A, uint32_t job, int sub, int& r, int& tx, int& ty) {
-    // colour-C tiles enumerated row by row: q -> ty = q / (B/2), tx = 2*(q % (B/2)) + ((ty + C) & 1)
+template <int T, int NS = 1>
+__device__ __forceinline__ void job_tile(const PlaneArgs& A, uint32_t job, int sub, int& r, int& tx, int& ty, int C = -1) {
+    // colour-C tiles enumerated row by row: q -> ty = q / (B/2), tx = 2*(q % (B/2)) + ((ty + C) & 1); a lane with NS slots
+    // owns the tiles q, q + 1, ..., q + NS - 1 (same row: (B/2) % NS == 0)
     const uint32_t B = geom_B(A), per_rep = B * B / 2u, hb = B >> 1;
-    const uint32_t q = job * PG<T>::TPW + (uint32_t)sub;
+    const uint32_t q = (job * PG<T>::TPW + (uint32_t)sub) * (uint32_t)NS;
 #ifdef ISING_JIT_B
     const uint32_t rr = ISING_JIT_R == 1 ? 0u : q / per_rep;      // divisions by constants
     const uint32_t qq = q - rr * per_rep;
@@ -80,7 +83,7 @@ __device__ __forceinline__ void job_tile(const PlaneArgs& A, uint32_t job, int s
 #endif
     r = (int)rr;
     ty = (int)yy;
-    tx = (int)(2u * (qq - yy * hb)) + ((ty + A.C) & 1);
+    tx = (int)(2u * (qq - yy * hb)) + ((ty + (C < 0 ? A.C : C)) & 1);
 }
 
 // Everything a lane keeps of its job between load and store.
@@ -136,9 +139,10 @@ __device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int
 }
 
 // a7: write the lane's block row back, and the bit-packed copies of the tile's boundary (see PG).
-template <int T, bool BITS>
+// SLUT: the table is a copy in shared memory, lut_smem = its 32-bit shared address (persistent kernels build it once per CTA)
+template <int T, bool BITS, bool SLUT = false>
 __device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, int ty, int Y, int sub, const TileRegs<T>& t,
-                                           const uint2* lut) {
+                                           const uint2* lut, uint32_t lut_smem = 0) {
     using G = PG<T>;
     constexpr uint32_t REC = BITS ? G::REC_BITS : G::REC_I8;
     constexpr uint32_t BODY = REC - G::EDGE;
@@ -158,8 +162,14 @@ __device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, in
                 const uint32_t w = t.S[cc][gx];
 #pragma unroll
                 for (int rp = 0; rp < 2; ++rp) {
-                    const uint2 a = __ldg(lut + ((w >> (16 * rp)) & 0xffu));          // bits 0..7  -> bytes 0..7
-                    const uint2 b = __ldg(lut + ((w >> (16 * rp + 8)) & 0xffu));      // bits 8..15 -> bytes 8..15
+                    uint2 a, b;                                                       // bits 0..7 -> bytes 0..7, bits 8..15 -> bytes 8..15
+                    if (SLUT) {
+                        a = lds64(lut_smem + (((w >> (16 * rp)) & 0xffu) << 3));
+                        b = lds64(lut_smem + (((w >> (16 * rp + 8)) & 0xffu) << 3));
+                    } else {
+                        a = __ldg(lut + ((w >> (16 * rp)) & 0xffu));
+                        b = __ldg(lut + ((w >> (16 * rp + 8)) & 0xffu));
+                    }
                     stg128(rec + ((((rp * 2 + cc) * G::NW + gx) * G::LPT) + Y) * 16, make_uint4(a.x, a.y, b.x, b.y), pol);
                 }
             }
@@ -223,23 +233,74 @@ __host__ __device__ constexpr int lut_ne_sel(int u1, int u2) {           // inpu
     return l;
 }
 template <uint32_t HP, int Q>
-__device__ __forceinline__ void sel_step(uint32_t p, uint32_t sel, uint32_t& bw, uint32_t& ne) {
-    constexpr int u1 = (HP >> (12 + 11 - Q)) & 1, u2 = (HP >> (11 - Q)) & 1;
-    constexpr int LC = lut_chain_sel(u1, u2), LN = lut_ne_sel(u1, u2);
-    bw = lop3<LC>(p, bw, sel);
-    ne = lop3<LN>(ne, p, sel);
+struct HeadBit {                                   // head bit of plane Q (0 = most significant) of thr[1] / thr[2]
+    static constexpr int u1 = (HP >> (12 + 11 - Q)) & 1, u2 = (HP >> (11 - Q)) & 1;
+    static constexpr bool same = u1 == u2;         // the site's choice of threshold does not matter for this plane
+};
+// Two adjacent planes whose head bits do not depend on the choice: one LOP3 advances the borrow chain by both
+// (inputs a = p_Q, the less significant plane, b = p_(Q-1), c = bw), and one LOP3 accumulates both "differs" bits.
+__host__ __device__ constexpr int lut_chain_pair(int uq, int uq1) {
+    int l = 0;
+    for (int i = 0; i < 8; ++i) {
+        const int pq = (i >> 2) & 1, pq1 = (i >> 1) & 1, bw = i & 1;
+        const int b1 = ((!pq) && uq) || ((pq == uq) && bw);            // after plane Q
+        const int b2 = ((!pq1) && uq1) || ((pq1 == uq1) && b1);        // after plane Q-1
+        l |= b2 << i;
+    }
+    return l;
+}
+__host__ __device__ constexpr int lut_ne_pair(int ua, int ub) {          // inputs a = ne, b = p_a, c = p_b
+    int l = 0;
+    for (int i = 0; i < 8; ++i) {
+        const int ne = (i >> 2) & 1, pa = (i >> 1) & 1, pb = i & 1;
+        l |= (ne || (pa != ua) || (pb != ub)) << i;
+    }
+    return l;
+}
+// borrow chain from plane Q down to plane 0 (least significant plane first: Q = 11)
+template <uint32_t HP, int Q>
+__device__ __forceinline__ void chain_from(const uint32_t (&p)[kHeadBits], uint32_t sel, uint32_t& bw) {
+    if constexpr (Q >= 0) {
+        if constexpr (Q >= 1 && HeadBit<HP, Q>::same && HeadBit<HP, (Q >= 1 ? Q - 1 : 0)>::same) {
+            bw = lop3<lut_chain_pair(HeadBit<HP, Q>::u1, HeadBit<HP, Q - 1>::u1)>(p[Q], p[Q - 1], bw);
+            chain_from<HP, Q - 2>(p, sel, bw);
+        } else {
+            bw = lop3<lut_chain_sel(HeadBit<HP, Q>::u1, HeadBit<HP, Q>::u2)>(p[Q], bw, sel);
+            chain_from<HP, Q - 1>(p, sel, bw);
+        }
+    }
+}
+// "some head bit differs from the threshold's": planes whose bit depends on the choice one by one, the others two at a
+// time (PEND = a choice-independent plane waiting for a partner, or -1)
+template <uint32_t HP, int Q, int PEND>
+__device__ __forceinline__ void ne_from(const uint32_t (&p)[kHeadBits], uint32_t sel, uint32_t& ne) {
+    if constexpr (Q >= 0) {
+        if constexpr (!HeadBit<HP, Q>::same) {
+            ne = lop3<lut_ne_sel(HeadBit<HP, Q>::u1, HeadBit<HP, Q>::u2)>(ne, p[Q], sel);
+            ne_from<HP, Q - 1, PEND>(p, sel, ne);
+        } else if constexpr (PEND < 0) {
+            ne_from<HP, Q - 1, Q>(p, sel, ne);
+        } else {
+            ne = lop3<lut_ne_pair(HeadBit<HP, (PEND >= 0 ? PEND : 0)>::u1, HeadBit<HP, Q>::u1)>(ne, p[PEND >= 0 ? PEND : 0], p[Q]);
+            ne_from<HP, Q - 1, -1>(p, sel, ne);
+        }
+    } else if constexpr (PEND >= 0) {
+        ne = lop3<lut_ne_pair(HeadBit<HP, (PEND >= 0 ? PEND : 0)>::u1, HeadBit<HP, (PEND >= 0 ? PEND : 0)>::u1)>(ne, p[PEND >= 0 ? PEND : 0], p[PEND >= 0 ? PEND : 0]);
+    }
 }
 template <uint32_t HP>
 __device__ __forceinline__ void head_masks_sel(uint32_t g, uint32_t Hlo, uint32_t Hhi, uint32_t k0, uint32_t k1, uint32_t sel,
                                                uint32_t& R, uint32_t& eq) {
     static_assert(kHeadBits == 12, "three Philox calls");
+    uint32_t p[kHeadBits];
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+        const u32x4 o = philox4x32_10(g, kTagPlanes + 256u * n, Hlo, Hhi, k0, k1);
+        p[4 * n] = o.x; p[4 * n + 1] = o.y; p[4 * n + 2] = o.z; p[4 * n + 3] = o.w;
+    }
     uint32_t bw = 0, ne = 0;
-    u32x4 o = philox4x32_10(g, kTagPlanes + 512u, Hlo, Hhi, k0, k1);       // least significant planes first
-    sel_step<HP, 11>(o.w, sel, bw, ne); sel_step<HP, 10>(o.z, sel, bw, ne); sel_step<HP, 9>(o.y, sel, bw, ne); sel_step<HP, 8>(o.x, sel, bw, ne);
-    o = philox4x32_10(g, kTagPlanes + 256u, Hlo, Hhi, k0, k1);
-    sel_step<HP, 7>(o.w, sel, bw, ne); sel_step<HP, 6>(o.z, sel, bw, ne); sel_step<HP, 5>(o.y, sel, bw, ne); sel_step<HP, 4>(o.x, sel, bw, ne);
-    o = philox4x32_10(g, kTagPlanes, Hlo, Hhi, k0, k1);
-    sel_step<HP, 3>(o.w, sel, bw, ne); sel_step<HP, 2>(o.z, sel, bw, ne); sel_step<HP, 1>(o.y, sel, bw, ne); sel_step<HP, 0>(o.x, sel, bw, ne);
+    chain_from<HP, kHeadBits - 1>(p, sel, bw);
+    ne_from<HP, kHeadBits - 1, -1>(p, sel, ne);
     R = bw; eq = ~ne;
 }
 
@@ -254,7 +315,8 @@ __device__ __forceinline__ uint32_t update_block(const PlaneArgs& A, uint32_t S,
     const uint32_t c = S ^ H1 ^ (HASJ ? Jw.z : 0u), d = S ^ H2 ^ (HASJ ? Jw.w : 0u);
     const uint32_t p1 = a | b, q1 = a & b, p2 = c | d, q2 = c & d;
     const uint32_t ge1 = p1 | p2;                                     // n_dis >= 1
-    const uint32_t ge2 = (p1 & p2) | q1 | q2 | A.force;               // n_dis >= 2  <=>  dE <= 0: always flip (eq. (2))
+    // n_dis >= 2  <=>  dE <= 0: always flip (eq. (2)); beta = 0 (force) never meets a specialised kernel
+    const uint32_t ge2 = (p1 & p2) | q1 | q2 | (HP == kNoSpec ? A.force : 0u);
     if (HP != kNoSpec) {
         const uint32_t sel = ~ge1;                                    // n_dis == 0: the site is compared with thr[2]
         uint32_t R, eq;
@@ -309,16 +371,23 @@ __device__ __forceinline__ void neighbour_words(const TileRegs<T>& t, int c, int
     V1 = __byte_perm(O, O, 0x1032);               // the other row of the same block
     V2 = __byte_perm(Oup, Odn, 0x5432);           // row above the block | row below the block
     H1 = O;
-    // pair-shifted word: colour 0: even rows look at pair j-1 (carry from the left), odd rows at j+1;
-    // colour 1: even rows j+1, odd rows j-1.
+    // pair-shifted word: colour 0: even rows (low half) look at pair j-1, odd rows (high half) at pair j+1; colour 1 the
+    // other way round.  A half shifted by one pair with the carry from the adjacent word (or the halo column) is 16
+    // consecutive bits of a 32-bit word glued from the two halves involved: one byte permute + one shift each.
+    //   "pair j-1" of half X with left neighbour half Lh:  bits [30:15] of (X << 16 | Lh)
+    //   "pair j+1" of half X with right neighbour half Rh: bits [16:1]  of (Rh << 16 | X)
     if (c == 0) {
-        const uint32_t cl = (gx == 0 && !PERIODIC) ? t.hL0 : ((Ol >> 15) & 1u);
-        const uint32_t cr = (gx == G::NW - 1 && !PERIODIC) ? t.hR1 : ((Or >> 16) & 1u);
-        H2 = ((O << 1) & 0x0000fffeu) | cl | ((O >> 1) & 0x7fff0000u) | (cr << 31);
+        const uint32_t lf = (gx == 0 && !PERIODIC) ? (t.hL0 << 15) : Ol;                 // low half: its bit 15 is the carry in
+        const uint32_t rt = (gx == G::NW - 1 && !PERIODIC) ? (t.hR1 << 16) : Or;         // high half: its bit 16 is the carry in
+        const uint32_t lo = __byte_perm(lf, O, 0x5410) >> 15;                            // (O.lo16 << 16 | lf.lo16) >> 15: result in bits [15:0]
+        const uint32_t hi = __byte_perm(O, rt, 0x7632) << 15;                            // (rt.hi16 << 16 | O.hi16) << 15: result in bits [31:16]
+        H2 = (lo & 0x0000ffffu) | (hi & 0xffff0000u);
     } else {
-        const uint32_t cr = (gx == G::NW - 1 && !PERIODIC) ? t.hR0 : (Or & 1u);
-        const uint32_t cl = (gx == 0 && !PERIODIC) ? t.hL1 : (Ol >> 31);
-        H2 = ((O >> 1) & 0x00007fffu) | (cr << 15) | ((O << 1) & 0xfffe0000u) | (cl << 16);
+        const uint32_t rt = (gx == G::NW - 1 && !PERIODIC) ? t.hR0 : Or;                 // low half looks right: carry = bit 0 of the right word's low half
+        const uint32_t lf = (gx == 0 && !PERIODIC) ? (t.hL1 << 31) : Ol;                 // high half looks left: carry = bit 31 of the left word
+        const uint32_t lo = __byte_perm(O, rt, 0x5410) >> 1;                             // (rt.lo16 << 16 | O.lo16) >> 1
+        const uint32_t hi = __byte_perm(lf, O, 0x7632) << 1;                             // (O.hi16 << 16 | lf.hi16) << 1
+        H2 = (lo & 0x0000ffffu) | (hi & 0xffff0000u);
     }
 }
 
@@ -358,7 +427,10 @@ __device__ __forceinline__ void count_row(const TileRegs<T>& t, const uint4 (&Jw
 
 constexpr int kPlaneThreads = 128;      // 4 warps = 4 jobs per CTA
 
-template <int T, bool BITS, bool HASJ, uint32_t HP = kNoSpec>
+// NS = tiles per lane ("slots"): the lane's tiles are NS consecutive tiles of the colour in one tile row, (tx + 2s, ty), so
+// the job's set-up (tile coordinates, record addresses, key schedule, the ballots of the boundary columns) is paid once per
+// NS tiles — what makes tile 32 as cheap per site as tile 64 ("missing" 1).  Needs (B/2) % NS == 0.
+template <int T, bool BITS, bool HASJ, uint32_t HP = kNoSpec, int NS = 1>
 __global__ void __launch_bounds__(kPlaneThreads) k_tile_planes(PlaneArgs A) {
     using G = PG<T>;
     // int8 write-back table (8 bits -> 8 bytes of 0/1): a constant array in global memory read through the
@@ -372,28 +444,40 @@ __global__ void __launch_bounds__(kPlaneThreads) k_tile_planes(PlaneArgs A) {
     const uint32_t job = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     if (job >= A.njobs) return;
     const int sub = lane / G::LPT, Y = lane % G::LPT;
-    int r, tx, ty;
-    job_tile<T>(A, job, sub, r, tx, ty);
-    TileRegs<T> t;
-    load_tile<T, BITS>(A, r, tx, ty, Y, sub * G::LPT, t);
-    uint4 Jw[2][G::NW];
+    int r, tx0, ty;
+    job_tile<T, NS>(A, job, sub, r, tx0, ty);
+    TileRegs<T> t[NS];
+    uint4 Jw[NS][2][G::NW];
 #pragma unroll
-    for (int cc = 0; cc < 2; ++cc)
+    for (int s = 0; s < NS; ++s) {
+        const int tx = tx0 + 2 * s;
+        load_tile<T, BITS>(A, r, tx, ty, Y, sub * G::LPT, t[s]);
 #pragma unroll
-        for (int gx = 0; gx < G::NW; ++gx)
-            Jw[cc][gx] = HASJ ? __ldg(A.jrec + ((size_t)ty * geom_B(A) + tx) * (2 * G::NW * G::LPT) + (cc * G::NW + gx) * G::LPT + Y)
-                              : make_uint4(0u, 0u, 0u, 0u);
+        for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+            for (int gx = 0; gx < G::NW; ++gx)
+                Jw[s][cc][gx] = HASJ ? __ldg(A.jrec + ((size_t)ty * geom_B(A) + tx) * (2 * G::NW * G::LPT) + (cc * G::NW + gx) * G::LPT + Y)
+                                     : make_uint4(0u, 0u, 0u, 0u);
+    }
+#if defined(ISING_JIT_R) && ISING_JIT_R == 1
+    const uint64_t seed = A.seed0;
+#else
     const uint64_t seed = A.seeds[r];
+#endif
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     const uint32_t Yg = (uint32_t)(ty * G::LPT + Y);                         // global block row
-    const uint32_t g0 = Yg * (geom_B(A) * G::NW) + (uint32_t)(tx * G::NW);   // RNG block of gx = 0 (L / 32 blocks per row)
-    const uint32_t p0 = 2u * Yg * (geom_B(A) * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx * G::NW);   // pair index of its bit 0
+    const uint32_t g0 = Yg * (geom_B(A) * G::NW) + (uint32_t)(tx0 * G::NW);  // RNG block of gx = 0 (L / 32 blocks per row)
+    const uint32_t p0 = 2u * Yg * (geom_B(A) * (uint32_t)(T / 2)) + 16u * (uint32_t)(tx0 * G::NW);   // pair index of its bit 0
     for (int j = 0; j < A.k; ++j) {
         const uint64_t tt = A.t_first + (uint64_t)j;
-        half_sweep<T, HASJ, false, HP>(A, t, Jw, 0, Y, g0, p0, 2 * tt, k0, k1);
-        half_sweep<T, HASJ, false, HP>(A, t, Jw, 1, Y, g0, p0, 2 * tt + 1, k0, k1);
+#pragma unroll
+        for (int c = 0; c < 2; ++c)
+#pragma unroll
+            for (int s = 0; s < NS; ++s)
+                half_sweep<T, HASJ, false, HP>(A, t[s], Jw[s], c, Y, g0 + (uint32_t)(2 * s * G::NW), p0 + 32u * (uint32_t)(s * G::NW), 2 * tt + (uint64_t)c, k0, k1);
     }
-    store_tile<T, BITS>(A, r, tx, ty, Y, sub, t, lut);
+#pragma unroll
+    for (int s = 0; s < NS; ++s) store_tile<T, BITS>(A, r, tx0 + 2 * s, ty, Y, sub, t[s], lut);
 }
 
 

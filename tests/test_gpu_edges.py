@@ -167,7 +167,8 @@ def test_config3_full_length_int8_equals_bits(P, orc, tile, k):
     for p in (2, 50, n):
         a.sweep(BC2, p - done, tile, k); b.sweep(BC2, p - done, tile, k)
         done = p
-        assert a.sweep_path() == "tile_planes_i8" and b.sweep_path() == "tile_planes_bits"
+        kind = "flow_planes" if k == 1 else "tile_planes"       # k = 1: the persistent data-flow kernel, else a launch per colour
+        assert a.sweep_path() == f"{kind}_i8" and b.sweep_path() == f"{kind}_bits"
         assert a.last_sweep_specialized() and b.last_sweep_specialized()
         a.copy_spins(sa); b.copy_spins(sb)
         assert torch.equal(sa, sb), f"int8 and bit records differ after pass {p}"
@@ -184,6 +185,13 @@ def test_config3_full_length_int8_equals_bits(P, orc, tile, k):
         c.copy_spins(sb)
         assert torch.equal(sa, sb), "pre-compiled and run-time specialised kernels differ after 200 passes"
         c.destroy()
+        d = P.Ising(2, L, seed=3)                           # ... and so does a launch per colour (no data-flow kernel)
+        d.force_path(3)
+        d.sweep(BC2, n, tile, k)
+        assert d.sweep_path() == "tile_planes_i8"
+        d.copy_spins(sb)
+        assert torch.equal(sa, sb), "data-flow kernel and per-colour launches differ after 200 passes"
+        d.destroy()
     a.destroy(); b.destroy()
 
 

@@ -843,3 +843,43 @@ def test_grid_resident_3d_kernel_several_jobs_per_warp():
     out = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, ISING_GRID_WARPS="50"),
                          capture_output=True, text=True, timeout=900)
     assert out.returncode == 0 and "capped ok" in out.stdout, out.stderr[-2000:]
+
+
+FLOW = [
+    # L, tile, k, n, beta, seeds, jseed
+    (256, 32, 1, 3, BC2, [3], None),
+    (256, 64, 2, 3, BC2, [4], None),
+    (384, 32, 1, 5, 0.3, [5, 6], None),        # replicas; B = 12: tile rows of 3 two-slot jobs
+    (192, 32, 2, 4, 1.0, [7], 5),              # B = 6: one slot per lane (B/2 odd); +-J
+    (320, 64, 1, 6, BC2, [8], None),           # B = 5 is odd: not a valid double checkerboard -> skipped below
+    (1024, 64, 1, 4, BC2, [8], None),
+    (2048, 32, 1, 3, BC2, [9], None),
+    (256, 32, 1, 2, 0.0, [2], None),
+    (256, 64, 1, 2, 30.0, [2], None),
+]
+
+
+@pytest.mark.parametrize("jit", ["off", "on"])
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,tile,k,n,beta,seeds,jseed", [c for c in FLOW if (c[0] // c[1]) % 2 == 0])
+def test_data_flow_kernel_matches_oracle(P, orc, L, tile, k, n, beta, seeds, jseed, layout, jit):
+    """k_flow_planes: all passes of a call in ONE persistent launch, the coarse colours ordered by per-tile progress counters
+    instead of kernel boundaries (the path bench.py times at L = 16384, k = 1).  force_path(4) keeps the on-chip kernels
+    out of the way so that small lattices reach it; then the per-pass kernels continue the same trajectory."""
+    J = W.couplings(2, L, jseed) if jseed is not None else None
+    g, o = _both(P, orc, 2, L, seeds, J, rng="planes")
+    if layout == "bits":
+        g.set_layout(P.ISING_LAYOUT_BITS)
+    g.set_jit(jit)
+    g.force_path(4)
+    sfx = "i8" if layout == "int8" else "bits"
+    g.sweep(beta, n, tile, k); o.sweep(beta, n, tile, k)
+    assert g.sweep_path() == f"flow_planes_{sfx}"
+    assert g.last_sweep_specialized() == (jit == "on" and beta > 0)
+    _same_state(g, o)
+    g.sweep(beta, n + 1, tile, k); o.sweep(beta, n + 1, tile, k)      # again: scratch counters are reset per call
+    _same_state(g, o)
+    g.force_path(3)                                                   # no data-flow kernel: a launch per colour
+    g.sweep(beta, 2, tile, k); o.sweep(beta, 2, tile, k)
+    assert g.sweep_path() in (f"tile_planes_{sfx}", f"resident_planes_{sfx}", f"grid_planes_{sfx}")
+    _same_state(g, o)
