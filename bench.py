@@ -184,6 +184,7 @@ def selftest_ranks(rank: int, world: int) -> None:
 
 
 JIT = "auto"     # --jit: run-time specialisation of the planes kernel (ising_set_jit)
+FORCE = 0        # --force-path: ising_force_path (0 automatic, 2 a launch per colour, 3 no data-flow kernel, 4 no on-chip kernels)
 
 
 def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng="planes", min_seconds=0.0, max_reps=1):
@@ -205,6 +206,8 @@ def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng=
         g.set_jit(JIT)
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
+    if FORCE:
+        g.force_path(FORCE)
     if sampler:
         sampler.start()
     g.sweep(W.BETA_C_2D, warmup, tile, k)
@@ -472,6 +475,8 @@ def main() -> None:
                     help="repeat the timed K-step call back to back until this much GPU time has elapsed; value = median repetition")
     ap.add_argument("--no-extras", action="store_true", help="skip e2e, cpu_baseline and the k/tile table")
     ap.add_argument("--jit", default="auto", choices=["auto", "on", "off"], help="run-time kernel specialisation (ising_set_jit)")
+    ap.add_argument("--force-path", type=int, default=0, choices=[0, 2, 3, 4],
+                    help="ising_force_path: 2 = a launch per coarse colour, 3 = no data-flow kernel, 4 = no on-chip (cluster / grid) kernels")
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5], help="time another BASELINE config (default 3 = the headline run)")
     ap.add_argument("--amsc", action="store_true", help="study: asynchronous multi-spin coding throughput (SURVEY 8(f)-1)")
     ap.add_argument("--heisenberg", action="store_true", help="study: the continuous-spin (Heisenberg) sweep, include/heisenberg.h (SURVEY 8(f)-4)")
@@ -480,8 +485,9 @@ def main() -> None:
     ap.add_argument("--autocorr", action="store_true", help="study: autocorrelation time against k (SURVEY 8(f)-2)")
     ap.add_argument("--selftest-ranks", action="store_true", help="CPU/gloo check of the multi-rank aggregation, no GPU")
     a = ap.parse_args()
-    global JIT
+    global JIT, FORCE
     JIT = a.jit
+    FORCE = a.force_path
     a.warmup = max(a.warmup, 3) if a.impl == "ours" else a.warmup
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

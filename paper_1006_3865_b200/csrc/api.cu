@@ -582,8 +582,8 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         // HBM-resident 2D lattices, several passes, nothing to measure in between, k = 1 (the HBM-bound case): one persistent
         // launch, colours ordered by data flow (k_flow_planes: +2.5 % at L = 16384, +5 % at L = 8192; for k >= 2 the register
         // budget of the persistent loop costs more than the idle launch tails it removes: a launch per colour)
-        const bool use_flow = use_planes && !resident_done && !want_series && !h->no_resident && !h->no_flow && (k == 1 || h->no_onchip) &&
-                              flow_planes_supported(h, T, n);
+        const bool use_flow = use_planes && !resident_done && !want_series && !h->no_resident && !h->no_flow && ((k == 1 && !bits) || h->no_onchip) &&
+                              flow_planes_supported(h, T, n);      // (bit records: 2854 against 2886 flips/ns, no gain)
         if (use_flow && !rc) {
             const size_t sb = flow_planes_scratch_bytes(h, T);
             if (sb > h->xedge_bytes) {

@@ -175,9 +175,10 @@ cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, 
     return cached(kJitSource, expr, {"-DISING_JIT_B=" + std::to_string(B) + "u", "-DISING_JIT_R=" + std::to_string(R) + "u"});
 }
 
-cudaKernel_t flow_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R, int NS) {
+cudaKernel_t flow_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R, int NS, bool staged) {
     char expr[160];
-    snprintf(expr, sizeof expr, "ising::jit::k_flow_planes<%d, %s, %s, %uu, %d>", T, bits ? "true" : "false", hasj ? "true" : "false", hp, NS);
+    snprintf(expr, sizeof expr, "ising::jit::k_flow_planes%s<%d, %s, %s, %uu, %d>", staged ? "_staged" : "", T, bits ? "true" : "false",
+             hasj ? "true" : "false", hp, NS);
     return cached(kJitSource, expr, {"-DISING_JIT_B=" + std::to_string(B) + "u", "-DISING_JIT_R=" + std::to_string(R) + "u"});
 }
 

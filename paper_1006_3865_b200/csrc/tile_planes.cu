@@ -1064,22 +1064,29 @@ bool grid_planes_supported(const ising_ctx* h, int T) {
 // ---- k_flow_planes (flow_planes_device.cuh): all n passes of an HBM-resident lattice in one persistent launch ----
 namespace {
 template <int T, bool BITS, int NS>
-int launch_flow_one(FlowArgs& F, bool use_jit, bool* used_jit) {
+int launch_flow_one(FlowArgs& F, bool use_jit, bool* used_jit, int stage_mode) {
     const PlaneArgs& A = F.P;
     int dev = 0, sms = 0;
     ISING_CUDA_OK(cudaGetDevice(&dev));
     ISING_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    cudaKernel_t spec = (use_jit && !A.force) ? flow_jit_kernel(T, BITS, A.jrec != nullptr, A.hp, A.B, A.R, NS) : nullptr;
-    const void* fn = spec ? (const void*)spec
-                          : (A.jrec ? (const void*)k_flow_planes<T, BITS, true, kNoSpec, NS> : (const void*)k_flow_planes<T, BITS, false, kNoSpec, NS>);
-    int occ = 0;
-    ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kPlaneThreads, 0));
-    if (occ < 1) { set_error("k_flow_planes does not fit an SM"); return ISING_ECUDA; }
     const uint32_t warps = kPlaneThreads / 32;
+    // TMA staging of the next job's bodies: only where a tile's previous write-back is certainly older than anything this
+    // grid still has in flight (a phase of more than 2 x the resident warps), and never with coupling records (kept simple)
+    const uint32_t resident_max = (uint32_t)sms * 16u * warps;
+    bool staged = stage_mode == 1 || (stage_mode == 0 && false);
+    if (F.jobs_per_phase <= 2u * resident_max || A.jrec) staged = false;
+    const size_t smem = staged ? (size_t)warps * (64 / T) * NS * (BITS ? T * T / 8 : T * T) : 0;
+    cudaKernel_t spec = (use_jit && !A.force) ? flow_jit_kernel(T, BITS, A.jrec != nullptr, A.hp, A.B, A.R, NS, staged) : nullptr;
+    const void* fn = spec ? (const void*)spec
+                   : staged ? (const void*)k_flow_planes_staged<T, BITS, false, kNoSpec, NS>
+                   : (A.jrec ? (const void*)k_flow_planes<T, BITS, true, kNoSpec, NS> : (const void*)k_flow_planes<T, BITS, false, kNoSpec, NS>);
+    int occ = 0;
+    ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kPlaneThreads, smem));
+    if (occ < 1) { set_error("k_flow_planes does not fit an SM"); return ISING_ECUDA; }
     uint32_t grid = (uint32_t)sms * (uint32_t)occ;
     grid = std::min<uint32_t>(grid, (F.jobs_per_phase + warps - 1) / warps);
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kPlaneThreads); cfg.dynamicSmemBytes = 0; cfg.stream = hooks().stream;
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kPlaneThreads); cfg.dynamicSmemBytes = smem; cfg.stream = hooks().stream;
     void* args[] = {&F};
     ISING_CUDA_OK(cudaLaunchKernelExC(&cfg, fn, args));
     count_launch();
@@ -1099,6 +1106,7 @@ bool flow_planes_supported(const ising_ctx* h, int T, int n) {
 
 // n passes in one persistent launch.  d_scratch: flow_planes_scratch_bytes (ticket counter + one progress word per tile).
 int launch_flow_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, void* d_scratch, bool use_jit) {
+    static const int stage_mode = getenv("ISING_FLOW_STAGE") ? atoi(getenv("ISING_FLOW_STAGE")) : 0;     // 1: TMA staging of the next job (profiles/r02: measured, not faster), default off
     FlowArgs F;
     PlaneArgs& A = F.P;
     A.tiles = (uint8_t*)h->d_tiles;
@@ -1125,10 +1133,10 @@ int launch_flow_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n,
     ISING_CUDA_OK(cudaMemsetAsync(d_scratch, 0, flow_planes_scratch_bytes(h, T), hooks().stream));
     bool used = false;
     int rc;
-    if (ns == 2) rc = T == 64 ? (bits ? launch_flow_one<64, true, 2>(F, use_jit, &used) : launch_flow_one<64, false, 2>(F, use_jit, &used))
-                              : (bits ? launch_flow_one<32, true, 2>(F, use_jit, &used) : launch_flow_one<32, false, 2>(F, use_jit, &used));
-    else rc = T == 64 ? (bits ? launch_flow_one<64, true, 1>(F, use_jit, &used) : launch_flow_one<64, false, 1>(F, use_jit, &used))
-                      : (bits ? launch_flow_one<32, true, 1>(F, use_jit, &used) : launch_flow_one<32, false, 1>(F, use_jit, &used));
+    if (ns == 2) rc = T == 64 ? (bits ? launch_flow_one<64, true, 2>(F, use_jit, &used, stage_mode) : launch_flow_one<64, false, 2>(F, use_jit, &used, stage_mode))
+                              : (bits ? launch_flow_one<32, true, 2>(F, use_jit, &used, stage_mode) : launch_flow_one<32, false, 2>(F, use_jit, &used, stage_mode));
+    else rc = T == 64 ? (bits ? launch_flow_one<64, true, 1>(F, use_jit, &used, stage_mode) : launch_flow_one<64, false, 1>(F, use_jit, &used, stage_mode))
+                      : (bits ? launch_flow_one<32, true, 1>(F, use_jit, &used, stage_mode) : launch_flow_one<32, false, 1>(F, use_jit, &used, stage_mode));
     if (rc) return rc;
     h->last_jit = used ? 1 : 0;
     ISING_CUDA_OK(cudaGetLastError());

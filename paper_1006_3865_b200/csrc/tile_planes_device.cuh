@@ -95,8 +95,10 @@ struct TileRegs {
     uint32_t hL0, hL1, hR0, hR1;  // halo column bits: x = -1 / x = T of rows 2Y (0) and 2Y+1 (1)
 };
 
+// body_smem != 0: the record body has been staged in shared memory (32-bit shared address of its first byte, same layout)
 template <int T, bool BITS>
-__device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int ty, int Y, int lane_base, TileRegs<T>& t) {
+__device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int ty, int Y, int lane_base, TileRegs<T>& t,
+                                          uint32_t body_smem = 0) {
     using G = PG<T>;
     constexpr uint32_t REC = BITS ? G::REC_BITS : G::REC_I8;
     constexpr uint32_t BODY = REC - G::EDGE;
@@ -112,11 +114,13 @@ __device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
 #pragma unroll
-            for (int gx = 0; gx < G::NW; ++gx) t.S[cc][gx] = ldg32(rec + ((cc * G::NW + gx) * G::LPT + Y) * 4);
+            for (int gx = 0; gx < G::NW; ++gx)
+                t.S[cc][gx] = body_smem ? lds32(body_smem + ((cc * G::NW + gx) * G::LPT + Y) * 4) : ldg32(rec + ((cc * G::NW + gx) * G::LPT + Y) * 4);
     } else {
         uint4 v[G::NCH];
 #pragma unroll
-        for (int ch = 0; ch < G::NCH; ++ch) v[ch] = ldg128(rec + (ch * G::LPT + Y) * 16, pol);
+        for (int ch = 0; ch < G::NCH; ++ch)
+            v[ch] = body_smem ? lds128(body_smem + (ch * G::LPT + Y) * 16) : ldg128(rec + (ch * G::LPT + Y) * 16, pol);
 #pragma unroll
         for (int cc = 0; cc < 2; ++cc)
 #pragma unroll

@@ -167,8 +167,8 @@ def test_config3_full_length_int8_equals_bits(P, orc, tile, k):
     for p in (2, 50, n):
         a.sweep(BC2, p - done, tile, k); b.sweep(BC2, p - done, tile, k)
         done = p
-        kind = "flow_planes" if k == 1 else "tile_planes"       # k = 1: the persistent data-flow kernel, else a launch per colour
-        assert a.sweep_path() == f"{kind}_i8" and b.sweep_path() == f"{kind}_bits"
+        # int8 records at k = 1: the persistent data-flow kernel, else a launch per colour
+        assert a.sweep_path() == ("flow_planes_i8" if k == 1 else "tile_planes_i8") and b.sweep_path() == "tile_planes_bits"
         assert a.last_sweep_specialized() and b.last_sweep_specialized()
         a.copy_spins(sa); b.copy_spins(sb)
         assert torch.equal(sa, sb), f"int8 and bit records differ after pass {p}"
