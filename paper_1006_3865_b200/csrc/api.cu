@@ -569,7 +569,7 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
                 if (!h->d_gacc) rc = ISING_ENOMEM; else h->gacc_bytes = ab;
             }
             if (!rc) {
-                const int g = launch_grid_planes(h, acc, T, bits, n, k, h->t, h->d_xedge, h->d_gacc, d_E, d_M, use_jit);
+                const int g = launch_grid_planes(h, acc, T, bits, n, k, h->t, h->d_xedge, h->d_gacc, d_E, d_M, use_jit, h->jit_mode != ISING_JIT_ON);
                 if (g == 0) {
                     h->last_path = bits ? "grid_planes_bits" : "grid_planes_i8";
                     resident_done = true;

@@ -27,6 +27,7 @@ struct GridArgs {
     uint32_t jobs_per_warp;               // M: jobs of each colour a warp owns (state in shared memory between phases)
     unsigned long long* xedge;            // per tile 16 x u64: TOP[4] | COL[4] = {L0, L1, R0, R1} | BOT[4] | pad; u64 = version << 32 | word
     long long* acc;                       // optional series accumulators [n][R][kGridAccSlots][2] = {#up, #unsatisfied}, zeroed
+    uint32_t magic_k;                     // PC kernels: fastdiv magic of k
 };
 
 __device__ __forceinline__ ulonglong2 ld_xedge2(const unsigned long long* p) {
@@ -38,19 +39,64 @@ __device__ __forceinline__ void st_xedge2(unsigned long long* p, unsigned long l
     asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1,%2};" ::"l"(p), "l"(a), "l"(b) : "memory");
 }
 
-template <int T, bool BITS, bool HASJ, uint32_t HP = kNoSpec>
-__global__ void __launch_bounds__(128, 5) k_grid_planes(GridArgs R) {
+// ---- PC = true: producer / consumer form for lattices so small that every warp would be alone on its scheduler (one job
+// per colour for fewer warps than the GPU has schedulers: L = 1024 at tile 32).  There a warp's k inner sweeps are a serial
+// chain of ~800 cycles per block update, 85 % of it random numbers and compares that do not depend on the spins.  A CTA is
+// then one consumer warp (warp 0: the grid worker described above) and 3 or 7 producer warps on the schedulers of the SM
+// (two warps per scheduler overlap their ALU and multiplier work, a single warp cannot): the producers compute R_m = [r < thr[m]] (head planes, borrow chains, ties resolved for every site whose head
+// equals a threshold head) for the consumer's coming half-sweeps, round robin, into a ring in shared memory; the consumer
+// only does the spin-dependent part (neighbour words, bit adder, flip = [n>=2] | [n>=1] & R1 | R2: ~40 instructions).
+constexpr int kPcRing = 16;               // half-sweeps of masks in flight per consumer
+
+__device__ __forceinline__ uint32_t lds_acquire(uint32_t saddr) {
+    uint32_t v;
+    asm volatile("ld.acquire.cta.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr) : "memory");
+    return v;
+}
+__device__ __forceinline__ void sts_release(uint32_t saddr, uint32_t v) {
+    asm volatile("st.release.cta.shared.u32 [%0], %1;" ::"r"(saddr), "r"(v) : "memory");
+}
+
+// the spin-dependent part of update_block for all blocks of the lane, R1 / R2 given
+template <int T, bool HASJ>
+__device__ __forceinline__ void half_sweep_masks(const PlaneArgs& A, TileRegs<T>& t, const uint4 (&Jw)[2][PG<T>::NW], int c, int Y,
+                                                 const uint32_t (&R1)[PG<T>::NW], const uint32_t (&R2)[PG<T>::NW]) {
+    using G = PG<T>;
+    uint32_t Snew[G::NW];
+#pragma unroll
+    for (int gx = 0; gx < G::NW; ++gx) {
+        uint32_t V1, V2, H1, H2;
+        neighbour_words<T, false>(t, c, gx, Y, V1, V2, H1, H2);
+        const uint32_t S = t.S[c][gx];
+        const uint4& J = Jw[c][gx];
+        const uint32_t a = S ^ V1 ^ (HASJ ? J.x : 0u), b = S ^ V2 ^ (HASJ ? J.y : 0u);
+        const uint32_t e = S ^ H1 ^ (HASJ ? J.z : 0u), d = S ^ H2 ^ (HASJ ? J.w : 0u);
+        const uint32_t p1 = a | b, q1 = a & b, p2 = e | d, q2 = e & d;
+        const uint32_t ge1 = p1 | p2, ge2 = (p1 & p2) | q1 | q2 | A.force;
+        Snew[gx] = S ^ (ge2 | (ge1 & R1[gx]) | R2[gx]);
+    }
+#pragma unroll
+    for (int gx = 0; gx < G::NW; ++gx) t.S[c][gx] = Snew[gx];
+}
+
+template <int T, bool BITS, bool HASJ, uint32_t HP = kNoSpec, bool PC = false>
+__global__ void __launch_bounds__(PC ? 256 : 128, PC ? 2 : 5) k_grid_planes(GridArgs R) {
     using G = PG<T>;
     constexpr int NWORDS = 2 * G::NW;                         // words per lane and job: S[cc][gx]
     constexpr int NSLOT = NWORDS + 7;                         // ... + the job's constants (decoded once): self, nU, nD, nL, nR, tx | ty << 16, r
     extern __shared__ uint32_t grid_smem[];                   // per warp: [colour][job][slot][lane]
     const PlaneArgs& A = R.P;
     const int lane = threadIdx.x & 31;
-    const uint32_t wg = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5), W = gridDim.x * (blockDim.x >> 5);
+    const int wic = threadIdx.x >> 5;
+    const uint32_t wg = PC ? blockIdx.x : blockIdx.x * (blockDim.x >> 5) + (uint32_t)wic, W = PC ? gridDim.x : gridDim.x * (blockDim.x >> 5);
     const int sub = lane / G::LPT, Y = lane % G::LPT;
     const uint32_t B = (uint32_t)A.B, hb = B >> 1, per_rep = R.tiles_per_colour;
-    const uint32_t Mw = R.jobs_per_warp;
-    uint32_t* const ws = grid_smem + (size_t)(threadIdx.x >> 5) * (2u * Mw * NSLOT * 32u) + lane;
+    const uint32_t Mw = PC ? 1u : R.jobs_per_warp;
+    uint32_t* const ws = grid_smem + (PC ? 0u : (size_t)wic * (2u * Mw * NSLOT * 32u)) + lane;
+    // PC: behind the consumer's area, the ring [slot][R1 | R2][gx][lane], its "full" words and the consumed counter
+    uint32_t* const ring = grid_smem + 2u * NSLOT * 32u;
+    const uint32_t flags = (uint32_t)__cvta_generic_to_shared(ring + kPcRing * 2 * G::NW * 32);
+    const uint32_t total_hs = PC ? (uint32_t)R.n * 4u * (uint32_t)A.k : 0u;
     const uint2* lut = kByteLutGlobal.e;
     const bool series = R.acc != nullptr;
 
@@ -163,8 +209,9 @@ __global__ void __launch_bounds__(128, 5) k_grid_planes(GridArgs R) {
             for (int gx = 0; gx < G::NW; ++gx) p[(cc * G::NW + gx) * 32] = tt.S[cc][gx];
     };
 
+    if (PC && threadIdx.x < kPcRing + 1) ring[kPcRing * 2 * G::NW * 32 + threadIdx.x] = 0u;      // full[] and the consumed counter
     // records -> shared memory; the colour-1 tiles publish their initial boundary (version 1 = what phase 0 waits for)
-    for (int C = 0; C < 2; ++C)
+    for (int C = 0; C < 2 && (!PC || wic == 0); ++C)
         for (uint32_t m = 0; m < Mw; ++m) {
             const uint32_t job = wg + m * W;
             if (job >= R.jobs_total) break;                               // warp-uniform
@@ -176,6 +223,58 @@ __global__ void __launch_bounds__(128, 5) k_grid_planes(GridArgs R) {
             if (C == 1) publish(tt, jb.self, 1u);
         }
 
+    if (PC) {
+        __syncthreads();                                   // the consumer's job constants and the ring flags are in place
+        if (wic > 0) {                                     // ---- producers: masks of the half-sweeps wic - 1, wic - 1 + 3, ...
+            if (wg < R.jobs_total) {
+                const uint32_t NP = (blockDim.x >> 5) - 1u;              // producer warps of the CTA
+                for (uint32_t hs = (uint32_t)wic - 1u; hs < total_hs; hs += NP) {
+                    const uint32_t c = hs & 1u, q = hs >> 1;
+                    const uint32_t phq = fastdiv(q, (uint32_t)A.k, R.magic_k), j = q - phq * (uint32_t)A.k;
+                    const int C = (int)(phq & 1u);
+                    const Job jb = sm_job(C, 0);
+                    const uint64_t seed = A.seeds[jb.r];
+                    const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+                    const uint32_t Yg = (uint32_t)(jb.ty * G::LPT + Y);
+                    const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(jb.tx * G::NW);
+                    const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(jb.tx * G::NW);
+                    const uint64_t H = 2 * (A.t_first + (uint64_t)(phq >> 1) * (uint64_t)A.k + (uint64_t)j) + (uint64_t)c;
+                    uint32_t R1[G::NW], R2[G::NW], e1[G::NW], e2[G::NW], any = 0;
+#pragma unroll
+                    for (int gx = 0; gx < G::NW; ++gx) {
+                        head_masks(A, g0 + (uint32_t)gx, (uint32_t)H, (uint32_t)(H >> 32), k0, k1, R1[gx], R2[gx], e1[gx], e2[gx]);
+                        any |= e1[gx] | e2[gx];
+                    }
+                    if (any) {                             // ties: 2^-11 per site, whether or not the site will need that threshold
+                        const uint32_t prow = B * (uint32_t)(T / 2);
+#pragma unroll
+                        for (int gx = 0; gx < G::NW; ++gx) {
+                            uint32_t und = e1[gx] | e2[gx];
+                            while (und) {
+                                const int jj = __ffs(und) - 1;
+                                und &= und - 1;
+                                const uint32_t p = p0 + 16u * (uint32_t)gx + (uint32_t)(jj >> 4) * prow + (uint32_t)(jj & 15);
+                                const u32x4 o = philox4x32_10(p, kTagTail, (uint32_t)H, (uint32_t)(H >> 32), k0, k1);
+                                const uint32_t tail = o.x >> kHeadBits;
+                                if ((e1[gx] >> jj) & 1u) R1[gx] |= (uint32_t)(tail < A.t1_tail) << jj;
+                                if ((e2[gx] >> jj) & 1u) R2[gx] |= (uint32_t)(tail < A.t2_tail) << jj;
+                            }
+                        }
+                    }
+                    const uint32_t slot = hs % kPcRing;
+                    if (hs >= kPcRing)                     // the consumer must be done with the slot's previous content
+                        while ((int)(lds_acquire(flags + 4u * kPcRing) - (hs - kPcRing + 1u)) < 0) {}
+                    uint32_t* dst = ring + (size_t)slot * (2 * G::NW * 32) + lane;
+#pragma unroll
+                    for (int gx = 0; gx < G::NW; ++gx) { dst[gx * 32] = R1[gx]; dst[(G::NW + gx) * 32] = R2[gx]; }
+                    __syncwarp();
+                    if (lane == 0) sts_release(flags + 4u * slot, hs + 1u);
+                }
+            }
+            return;
+        }
+    }
+    uint32_t hs_next = 0;                                  // PC: the consumer's running half-sweep index
     for (int pass = 0; pass < R.n; ++pass) {
         for (int C = 0; C < 2; ++C) {
             const uint32_t ph = 2u * (uint32_t)pass + (uint32_t)C;       // this phase waits for version ph + 1 and publishes ph + 2
@@ -197,8 +296,23 @@ __global__ void __launch_bounds__(128, 5) k_grid_planes(GridArgs R) {
                 const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(jb.tx * G::NW);
                 for (int j = 0; j < A.k; ++j) {
                     const uint64_t t64 = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
-                    half_sweep<T, HASJ, false, HP>(A, tt, Jw, 0, Y, g0, p0, 2 * t64, k0, k1);
-                    half_sweep<T, HASJ, false, HP>(A, tt, Jw, 1, Y, g0, p0, 2 * t64 + 1, k0, k1);
+                    if (PC) {
+#pragma unroll
+                        for (int c = 0; c < 2; ++c) {
+                            const uint32_t hs = hs_next++, slot = hs % kPcRing;
+                            while (lds_acquire(flags + 4u * slot) != hs + 1u) {}
+                            const uint32_t* src = ring + (size_t)slot * (2 * G::NW * 32) + lane;
+                            uint32_t R1[G::NW], R2[G::NW];
+#pragma unroll
+                            for (int gx = 0; gx < G::NW; ++gx) { R1[gx] = src[gx * 32]; R2[gx] = src[(G::NW + gx) * 32]; }
+                            __syncwarp();
+                            if (lane == 0) sts_release(flags + 4u * kPcRing, hs + 1u);      // the slot may be refilled
+                            half_sweep_masks<T, HASJ>(A, tt, Jw, c, Y, R1, R2);
+                        }
+                    } else {
+                        half_sweep<T, HASJ, false, HP>(A, tt, Jw, 0, Y, g0, p0, 2 * t64, k0, k1);
+                        half_sweep<T, HASJ, false, HP>(A, tt, Jw, 1, Y, g0, p0, 2 * t64 + 1, k0, k1);
+                    }
                 }
                 publish(tt, jb.self, ph + 2u);
                 if (series && C == 1) account(tt, Jw, jb.r, pass);       // colour-1 tiles: their halos (colour 0) are final for this pass

@@ -45,7 +45,8 @@ bool grid_planes_supported(const ising_ctx* h, int T);          // 512 < L <= ~4
 size_t grid_planes_xedge_bytes(const ising_ctx* h, int T);
 size_t grid_planes_acc_bytes(const ising_ctx* h, int n);
 int launch_grid_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, void* d_xedge, void* d_acc,
-                       long long* d_E, long long* d_M, bool use_jit);     // returns 1 (nothing launched) if the lattice does not fit
+                       long long* d_E, long long* d_M, bool use_jit, bool allow_pc);   // returns 1 (nothing launched) if the lattice does not fit;
+                                                                                       // allow_pc: the producer / consumer form where it applies
 
 bool flow_planes_supported(const ising_ctx* h, int T, int n);   // HBM-resident lattices, n >= 2 passes: one persistent launch, colours ordered by data flow
 size_t flow_planes_scratch_bytes(const ising_ctx* h, int T);

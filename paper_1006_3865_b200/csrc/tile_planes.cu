@@ -964,14 +964,43 @@ namespace {
 constexpr uint32_t kGridMaxJobsPerWarp = 16;
 
 template <int T, bool BITS, bool HASJ>
-int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit) {
+int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit, bool allow_pc) {
+    int dev = 0, sms = 0;
+    ISING_CUDA_OK(cudaGetDevice(&dev));
+    ISING_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    // producer / consumer form (one consumer + three producer warps per job pair): where a warp would be alone on its scheduler
+    // anyway, i.e. at most four jobs of a colour per SM (L = 1024, and L = 2048 at tile 64: measured);
+    // ISING_GRID_PC = 0 / 1 overrides (tuning aid); not when the caller insists on the run-time specialised kernel
+    static const int pc_mode = getenv("ISING_GRID_PC") ? atoi(getenv("ISING_GRID_PC")) : -1;
+    const uint64_t total_hs = (uint64_t)R.n * 4u * (uint64_t)R.P.k;
+    if (allow_pc && (pc_mode == 1 || (pc_mode < 0 && R.jobs_total <= (uint32_t)sms * 4u)) && total_hs < 0x7fffffffull) {
+        const void* fn = (const void*)k_grid_planes<T, BITS, HASJ, kNoSpec, true>;
+        const size_t smem = (2u * (2u * PG<T>::NW + 7u) * 32u + kPcRing * 2u * PG<T>::NW * 32u + kPcRing + 1u) * sizeof(uint32_t);
+        int occ = 0;
+        static const int pc_warps = getenv("ISING_GRID_PC_WARPS") ? atoi(getenv("ISING_GRID_PC_WARPS")) : 4;      // consumer + producers: 4 (default) or 8 (no faster)
+        const int pc_threads = pc_warps == 4 ? 128 : 256;
+        ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, pc_threads, smem));
+        if (R.jobs_total <= (uint32_t)sms * (uint32_t)occ) {
+            R.jobs_per_warp = 1;
+            R.magic_k = fastdiv_magic((uint32_t)R.P.k);
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3(R.jobs_total); cfg.blockDim = dim3(pc_threads); cfg.dynamicSmemBytes = smem; cfg.stream = hooks().stream;
+            cudaLaunchAttribute attr[1];
+            attr[0].id = cudaLaunchAttributeCooperative;
+            attr[0].val.cooperative = 1;
+            cfg.attrs = attr; cfg.numAttrs = 1;
+            void* args[] = {&R};
+            ISING_CUDA_OK(cudaLaunchKernelExC(&cfg, fn, args));
+            count_launch();
+            *fits = true;
+            *used_jit = false;
+            return 0;
+        }
+    }
     // specialised on the threshold head bits (planes_jit.cu) when asked for and available
     cudaKernel_t spec = (use_jit && !R.P.force) ? grid_jit_kernel(T, BITS, HASJ, R.P.hp) : nullptr;
     const void* fn = spec ? (const void*)spec : (const void*)k_grid_planes<T, BITS, HASJ>;
     *used_jit = spec != nullptr;
-    int dev = 0, sms = 0;
-    ISING_CUDA_OK(cudaGetDevice(&dev));
-    ISING_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     if (spec) ISING_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
     else if (int rc = set_max_dynamic_smem<k_grid_planes<T, BITS, HASJ>>(200 * 1024)) return rc;
     *fits = false;
@@ -1012,7 +1041,7 @@ size_t grid_planes_acc_bytes(const ising_ctx* h, int n) { return (size_t)n * (si
 // n passes in one cooperative launch; returns 1 if the lattice does not fit the register files of the GPU (nothing launched).
 // d_xedge: grid_planes_xedge_bytes; d_acc: grid_planes_acc_bytes(n) if a series is wanted, else nullptr.
 int launch_grid_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, void* d_xedge, void* d_acc,
-                       long long* d_E, long long* d_M, bool use_jit) {
+                       long long* d_E, long long* d_M, bool use_jit, bool allow_pc) {
     GridArgs R;
     PlaneArgs& A = R.P;
     A.tiles = (uint8_t*)h->d_tiles;
@@ -1027,6 +1056,7 @@ int launch_grid_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n,
     fill_accept(A, acc);
     R.n = n;
     R.jobs_per_warp = 1;
+    R.magic_k = 0;
     R.tiles_per_colour = (uint32_t)A.B * (uint32_t)A.B / 2u;
     R.jobs_total = (uint32_t)h->R * R.tiles_per_colour / (uint32_t)(64 / T);
     R.xedge = (unsigned long long*)d_xedge;
@@ -1037,10 +1067,10 @@ int launch_grid_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n,
     if (series) ISING_CUDA_OK(cudaMemsetAsync(d_acc, 0, grid_planes_acc_bytes(h, n), st));
     bool fits = false, used = false;
     int rc;
-    if (A.jrec) rc = T == 64 ? (bits ? launch_grid_one<64, true, true>(R, use_jit, &fits, &used) : launch_grid_one<64, false, true>(R, use_jit, &fits, &used))
-                             : (bits ? launch_grid_one<32, true, true>(R, use_jit, &fits, &used) : launch_grid_one<32, false, true>(R, use_jit, &fits, &used));
-    else rc = T == 64 ? (bits ? launch_grid_one<64, true, false>(R, use_jit, &fits, &used) : launch_grid_one<64, false, false>(R, use_jit, &fits, &used))
-                      : (bits ? launch_grid_one<32, true, false>(R, use_jit, &fits, &used) : launch_grid_one<32, false, false>(R, use_jit, &fits, &used));
+    if (A.jrec) rc = T == 64 ? (bits ? launch_grid_one<64, true, true>(R, use_jit, &fits, &used, allow_pc) : launch_grid_one<64, false, true>(R, use_jit, &fits, &used, allow_pc))
+                             : (bits ? launch_grid_one<32, true, true>(R, use_jit, &fits, &used, allow_pc) : launch_grid_one<32, false, true>(R, use_jit, &fits, &used, allow_pc));
+    else rc = T == 64 ? (bits ? launch_grid_one<64, true, false>(R, use_jit, &fits, &used, allow_pc) : launch_grid_one<64, false, false>(R, use_jit, &fits, &used, allow_pc))
+                      : (bits ? launch_grid_one<32, true, false>(R, use_jit, &fits, &used, allow_pc) : launch_grid_one<32, false, false>(R, use_jit, &fits, &used, allow_pc));
     if (rc) return rc;
     if (!fits) return 1;
     h->last_jit = used ? 1 : 0;

@@ -695,8 +695,9 @@ GRID = [
 @pytest.mark.parametrize("L,tile,k,n,beta,seeds,jseed", GRID)
 def test_grid_resident_kernel_matches_oracle(P, orc, L, tile, k, n, beta, seeds, jseed, layout, jit):
     """512 < L <= 4096 (the paper's own sizes), n >= 2 passes: one cooperative launch, every tile on chip for the
-    whole call, boundary words exchanged through versioned 64-bit words in L2 (k_grid_planes).  Pre-compiled and run-time
-    specialised kernels; with and without the E/M series; composing with the per-pass kernels."""
+    whole call, boundary words exchanged through versioned 64-bit words in L2 (k_grid_planes).  jit "off": at these sizes the
+    producer / consumer form (one consumer warp + three producer warps per pair of jobs); jit "on": the run-time specialised
+    kernel, every warp on its own.  With and without the E/M series; composing with the per-pass kernels."""
     J = W.couplings(2, L, jseed) if jseed is not None else None
     g, o = _both(P, orc, 2, L, seeds, J, rng="planes")
     if layout == "bits":
