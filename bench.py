@@ -55,20 +55,21 @@ def kernel_fingerprint() -> str:
     kernel it was captured from is the kernel being timed."""
     import hashlib
     h = hashlib.sha1()
-    for n in ("philox.cuh", "planes_common.cuh", "tile_planes_device.cuh", "tile_planes.cu"):
+    for n in ("philox.cuh", "planes_common.cuh", "tile_planes_device.cuh", "flow_planes_device.cuh"):
         h.update(open(os.path.join(ROOT, "paper_1006_3865_b200", "csrc", n), "rb").read())
     return h.hexdigest()[:12]
 
 
-# From the committed ncu captures, per launch of the kernel: DRAM bytes read + written, and executed warp-instructions.
-# Keyed by (rng, layout, tile, k, jit); "fingerprint" = kernel_fingerprint() of the sources the capture was taken from.
-NCU_FINGERPRINT = "335e7167c47f"
+# From the committed ncu captures, per PHASE (one coarse colour of one pass = one launch of k_tile_planes, or a sixth of
+# the captured 3-pass launch of the persistent k_flow_planes): DRAM bytes read + written, and executed warp-instructions.
+# Keyed by (rng, layout, tile, k, kernel family); NCU_FINGERPRINT = kernel_fingerprint() of the sources they were captured from.
+NCU_FINGERPRINT = "91027744a042"
 NCU = {
-    ("planes", "int8", 64, 1, True): {"traffic": 138.44e6 + 79.40e6, "warp_instr": 33.78e6},
-    ("planes", "int8", 64, 16, True): {"traffic": 138.44e6 + 79.33e6, "warp_instr": 391.3e6},
-    # plain checkerboard, one launch = one half-sweep of the whole lattice (profiles/r01g_tile_planes_plain_i8.md)
-    ("planes", "int8", 16384, 1, False): {"traffic": 272.66e6 + 97.58e6, "warp_instr": 52.12e6,
-                                          "source": "profiles/r01g_tile_planes_plain_i8.md"},
+    ("planes", "int8", 64, 1, "flow"): {"traffic": (803.30e6 + 758.07e6) / 6, "warp_instr": 219.99e6 / 6, "source": "profiles/r02c_flow_planes_i8.md"},
+    ("planes", "int8", 32, 1, "flow"): {"traffic": (803.04e6 + 798.70e6) / 6, "warp_instr": 248.68e6 / 6, "source": "profiles/r02c_flow_planes_i8.md"},
+    ("planes", "int8", 64, 1, "tile"): {"traffic": 138.46e6 + 80.11e6, "warp_instr": 33.83e6, "source": "profiles/r02c_flow_planes_i8.md"},
+    # plain checkerboard, one launch = one half-sweep of the whole lattice (round-1 capture; the fingerprint check drops it
+    # when the kernel has changed since)
 }
 # Issue ceiling of the path (DESIGN.md §7.3): 148 SMs x 4 SMSPs, one warp-instruction per 2 cycles at sm_max_mhz.
 def issue_peak_gips(sm_mhz: float) -> float:
@@ -529,7 +530,8 @@ def main() -> None:
     ms, value = aggregate_replicas(res["ms"], world, a.steps, a.k, L, dist, "cuda")
 
     peak, peak_src, sm_max = measured_peaks()
-    ncu = NCU.get((a.rng, a.layout, a.tile, a.k, res["path"].endswith("+jit"))) if L == 16384 else None
+    family = "flow" if res["path"].startswith("flow") else "tile" if res["path"].startswith("tile_planes") else res["path"]
+    ncu = NCU.get((a.rng, a.layout, a.tile, a.k, family)) if L == 16384 and res["path"].endswith("+jit") else None
     ncu_stale = ncu is not None and kernel_fingerprint() != NCU_FINGERPRINT
     if ncu_stale:            # the kernel changed since the capture: quote nothing from it
         ncu = None
@@ -545,7 +547,7 @@ def main() -> None:
             "dtype": "u8" if a.layout == "int8" else "u32 bit-planes", "data": "synthetic",
             "config": {"workload": f"{'BASELINE config 3' if L == 16384 else 'config 3 at another size'}: 2D Ising L={L} hot start seed 3 "
                                    f"beta=0.4406868 layout={a.layout} rng={a.rng} tile={a.tile} k={a.k}; one step = one outer pass "
-                                   + ("(2 launches)" if not res["path"].startswith("resident") else "(all steps in one cluster launch)"),
+                                   + ("(2 launches)" if res["path"].startswith("tile") else "(all steps of a call in one persistent launch)"),
                        "l2": f"lattice ({lat_bytes / 2 ** 20:g} MiB {a.layout}) exceeds the 126 MB L2; no explicit flush" if lat_bytes > 126e6
                              else f"lattice ({lat_bytes / 2 ** 20:g} MiB {a.layout}) fits L2: not an HBM claim",
                        "kernel_path": res["path"], "parallelism": "replicas only" if world > 1 else "single GPU"},
@@ -556,12 +558,14 @@ def main() -> None:
                             "value_max": a.steps * a.k * L * L / (res["ms_min"] * 1e6) * world},
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": ncu["traffic"] if ncu else None,
-                         "traffic_source": ("ncu dram__bytes_read.sum + dram__bytes_write.sum per launch, "
-                                            + ncu.get("source", "profiles/r01d_tile_planes_jit_i8_t64.md")) if ncu else None,
+                         "traffic_source": ("ncu dram__bytes_read.sum + dram__bytes_write.sum per phase, "
+                                            + ncu.get("source", "profiles/")) if ncu else None,
                          "traffic_stale": ncu_stale,
                          "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
                          "algorithmic_bytes_per_flip": bpf, "kernel": f"{res['path']}<{a.tile}>",
                          "avg_launch_ms": launch_ms,
+                         "launch_unit": "one launch of k_tile_planes = one coarse colour of one pass" if res["path"].startswith("tile") else
+                                        "one phase (coarse colour of a pass) of the persistent launch: CUDA-event time of the call / (2 * steps)",
                          "issue": ({"bound": "alu", "unit": "G warp-instr/s", "achieved": ncu["warp_instr"] / (launch_ms * 1e6),
                                     "peak": issue_peak_gips(sm_max), "frac": ncu["warp_instr"] / (launch_ms * 1e6) / issue_peak_gips(sm_max),
                                     "kind": "model",
