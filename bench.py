@@ -71,9 +71,9 @@ NCU = {
     # plain checkerboard, one launch = one half-sweep of the whole lattice (round-1 capture; the fingerprint check drops it
     # when the kernel has changed since)
 }
-# Issue ceiling of the path: 148 SMs x 4 SMSPs, one warp-instruction per 2 cycles at sm_max_mhz.
+# Issue slots of the GPU: 148 SMs x 4 schedulers, one warp-instruction per cycle at sm_max_mhz.
 def issue_peak_gips(sm_mhz: float) -> float:
-    return 148 * 4 * sm_mhz * 1e6 / 2 / 1e9
+    return 148 * 4 * sm_mhz * 1e6 / 1e9
 
 
 class ClockSampler:
@@ -200,11 +200,14 @@ def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng=
     # the library's AUTO rule (specialise calls of >= 2^27 attempted flips), decided here for the timed call so that
     # the warm-up call, which is shorter, already compiles the kernel the timed call will use
     # (lattices small enough for the resident kernels stay on AUTO: they serve them)
-    resident = tile in (32, 64) and (L // tile) ** 2 // 2 // (64 // tile) <= 64 and steps >= 2     # cluster-resident kernel: no specialised form
-    if not resident:
+    # Lattices that live on chip for a whole call (cluster / grid resident kernels: at most two jobs of a colour per warp of the
+    # GPU) stay on the library's AUTO rule: it chooses between the producer / consumer form and the specialised kernel.
+    onchip = tile in (32, 64) and (L // tile) ** 2 // 2 // (64 // tile) <= 148 * 20 * 2 and steps >= 2
+    if not onchip:
         g.set_jit("on" if JIT == "on" or (JIT == "auto" and steps * k * L * L >= 2 ** 27) else "off")
     else:
         g.set_jit(JIT)
+        warmup = max(warmup, steps)          # the same call once before: whatever AUTO compiles is compiled outside the timed region
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
     if FORCE:
@@ -568,8 +571,9 @@ def main() -> None:
                                         "one phase (coarse colour of a pass) of the persistent launch: CUDA-event time of the call / (2 * steps)",
                          "issue": ({"bound": "alu", "unit": "G warp-instr/s", "achieved": ncu["warp_instr"] / (launch_ms * 1e6),
                                     "peak": issue_peak_gips(sm_max), "frac": ncu["warp_instr"] / (launch_ms * 1e6) / issue_peak_gips(sm_max),
-                                    "kind": "model",
-                                    "note": "DESIGN.md 7.3 / profiles/r02_microbench.md: a cost model fitted to microbenchmarks, not a hardware limit"}
+                                    "kind": "issue slots (one warp-instruction per scheduler cycle, 592 schedulers)",
+                                    "note": "what binds is not the slot count but the dispatch model of DESIGN.md 7.3 / profiles/r02_microbench.md "
+                                            "(a 16-lane ALU instruction holds the scheduler 2 cycles, a wide multiply 2.25): a model, not a hardware counter"}
                                    if ncu else None)}}
     if rank == 0 and not a.no_extras and world == 1:
         table = {}
