@@ -354,12 +354,12 @@ def run_amsc(P, torch, a) -> None:
 
 def heis_alu_peak(dim: int, sm_mhz: float = 1965.0) -> dict:
     """Issue ceiling of one Heisenberg update on B200: the operations H2-H6 state, costed with the
-    pipe rates measured in profiles/r01_microbench.md.  Per warp-update, in SMSP-cycles: half a Philox4x32-10 call
-    (84.6 measured per call, one call serves two updates), every stated float / convert / bit-field / select operation
+    pipe rates measured in profiles/r02_microbench.md.  Per warp-update, in SMSP-cycles: half a Philox4x32-10 call
+    (109 measured per call, profiles/r02_microbench.md; one call serves two updates), every stated float / convert / bit-field / select operation
     and every shared-memory access one issue slot."""
     fp = 35 + (3 + 6 * (dim - 1)) + 3 + 3 + 3 + 16 + 3       # direction, field adds, d, e, u, P(beta*e), decision
     lsu = 3 * (2 * dim + 1) + 3                              # neighbour + own loads, store of an accepted spin
-    cycles = 84.6 / 2 + fp + lsu
+    cycles = 109.0 / 2 + fp + lsu
     return {"cycles_per_warp_update": cycles, "peak": 148 * 4 * sm_mhz * 1e6 / cycles * 32 / 1e9}
 
 

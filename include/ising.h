@@ -86,9 +86,17 @@ void ising_destroy(ising_handle h);
  * tile visit runs k_inner ≥ 1 times (even sites, then odd sites) with its halo frozen.
  * tile = edge T: T even, T | L, and L/T even or T == L; 0 means T = L (the single
  * checkerboard of P:62).  beta finite, ≥ 0.  Acceptance is the integer test
- * r < floor(exp(-β ΔE)·2^32), table built in double on the host (S8c.4).  Half-sweep
- * H = 2t + colour uses r = Philox(ctr={p>>2,0,lo32 H,hi32 H}, key=seed)[p&3], p = i>>1.
- * Advances t by n_sweeps·k_inner.  Asynchronous. */
+ * r < floor(exp(-β ΔE)·2^32), table built in double on the host (S8c.4).  The 32-bit uniform r of site i in
+ * half-sweep H = 2t + colour comes from Philox4x32-10 keyed by the seed, under the handle's RNG mapping (ising_set_rng):
+ *   ISING_RNG_PLANES (default): the 12 leading bits of r are bit j of the planes
+ *     Philox(ctr={g, 3 + 256 (q>>2), lo32 H, hi32 H})[q&3], q = 0..11, of the site's 32-site block g (bit j = the site's place in
+ *     the block), the 20 trailing bits are Philox(ctr={i>>1, 4, lo32 H, hi32 H})[0] >> 12;
+ *   ISING_RNG_WORDS: r = Philox(ctr={p>>2, 0, lo32 H, hi32 H})[p&3], p = i>>1.
+ * Both give every (site, half-sweep) its own uniform r; the trajectories differ.  Advances t by n_sweeps·k_inner.
+ * Asynchronous.  Which kernel runs (a launch per coarse colour, one persistent launch per call for HBM-resident
+ * lattices, one cooperative launch with the lattice on chip for smaller ones, ...) never changes the result:
+ * ising_sweep_path.  A change of `tile` between calls re-lays the spins out in HBM (through the canonical array,
+ * one extra pass over the lattice in each direction). */
 int ising_sweep(ising_handle h, double beta, int n_sweeps, int tile, int k_inner);
 
 /* ising_sweep_series — same as ising_sweep, and after every outer pass writes
@@ -195,13 +203,18 @@ uint64_t ising_kernel_launches(void);
  *   resident_masked_*, tile_masked_*, resident3d_masked_*, tile3d_masked_*
  *                           double checkerboard with power-of-two tiles other than the register tiles (2D: 2, 4, 8, 16 —
  *                           the paper's sizes, P:86 — and 128, 256, ...; 3D: 2, 4, 16, 32, ...) as masked half-sweeps
+ *   grid_planes_{i8,bits}, grid3d_planes_{i8,bits}   lattices beyond the cluster that fit on chip (2D 512 < L <= 4096, 3D 64 < L): the
+ *                           whole call in one cooperative launch, boundary words exchanged through L2
+ *   flow_planes_{i8,bits}   HBM-resident 2D lattices: all passes in one persistent launch, coarse colours ordered by per-tile
+ *                           progress counters
  *   amsc                    asynchronous multi-spin coding of a multi-realisation batch (ising_create_multi)
  * The fast 2D families need L % 32 == 0 (L % 64 for tile 64) and an even number of register tiles per side, the 3D ones
  * L % 8 == 0 and L / 8 even. */
 const char* ising_sweep_path(ising_handle h);
 
-/* ising_force_path — testing aid: 0 = automatic kernel choice, 1 = always the generic
- * global-memory kernels, 2 = automatic but never the cluster-resident kernel. */
+/* ising_force_path — testing / measuring aid: 0 = automatic kernel choice, 1 = always the generic global-memory kernels,
+ * 2 = a launch per coarse colour (never a cluster-resident, grid-resident or data-flow kernel), 3 = never the persistent
+ * data-flow kernel, 4 = never the cluster / grid resident kernels (the data-flow kernel may then run at any size and k). */
 int ising_force_path(ising_handle h, int generic_only);
 
 const char* ising_last_error(void); /* thread-local, never NULL */
