@@ -7,6 +7,7 @@
 #include <atomic>
 #include <mutex>
 #include <new>
+#include <string>
 #include <unordered_map>
 
 #include "kernels.h"
@@ -355,7 +356,258 @@ ising_handle ising_create(int dim, int L, const int8_t* J, uint64_t seed) {
 }  // extern "C"
 
 // ---- sweeps ---------------------------------------------------------------------------
-static bool thr_fits_or_zero(const Accept&) { return true; }   // amsc.cu handles thr = 2^32 with all-ones masks
+// One ising_sweep / ising_sweep_series call.  Kernel families are tried in the order of kPaths: each entry either does not
+// apply (kSkip: the next one is asked), or runs the whole call (kDone), or fails (a negative ISING_E* code).
+namespace {
+
+struct SweepCall {
+    ising_ctx* h;
+    Accept acc;
+    int n, T, k;
+    long long *d_E, *d_M;          // series outputs on the device (or nullptr)
+    bool want_series, bits, thr_fits;
+    cudaStream_t st;
+    int Tc2, Tc3;                  // coarse tile edge of a masked double checkerboard on the 2D / 3D register tiling, or 0
+    const char* sfx() const { return bits ? "bits" : "i8"; }
+};
+constexpr int kSkip = 1, kDone = 0;
+
+// last_path strings live for the life of the process: "<family>_<i8|bits>"
+const char* path_name(const char* family, bool bits) {
+    static std::mutex mu;
+    static std::unordered_map<std::string, std::string>* names = new std::unordered_map<std::string, std::string>();
+    try {
+        std::lock_guard<std::mutex> lock(mu);
+        std::string key = std::string(family) + (bits ? "_bits" : "_i8");
+        return names->emplace(key, key).first->second.c_str();
+    } catch (...) {
+        return family;
+    }
+}
+
+// coupling records (a9) in the form of the tile records in use: built once per (kind, tile edge)
+int ensure_couplings(ising_ctx* h, bool three_d, int T) {
+    if (!h->has_J || (h->Jtiles_tile == T && h->Jtiles_kind == (three_d ? 3 : 2))) return 0;
+    const size_t need = three_d ? coupling_record3d_bytes(h) : coupling_record_bytes(h);
+    if (need > h->Jtiles_bytes) {
+        cudaStreamSynchronize(hooks().stream);
+        dev_free(h->d_Jtiles); h->d_Jtiles = nullptr; h->Jtiles_bytes = 0; h->Jtiles_tile = 0;
+        h->d_Jtiles = dev_alloc(need);
+        if (!h->d_Jtiles) return ISING_ENOMEM;
+        h->Jtiles_bytes = need;
+    }
+    h->Jtiles_tile = 0;
+    const int rc = three_d ? launch_convert_couplings3d(h, h->d_Jtiles) : launch_convert_couplings(h, T, h->d_Jtiles);
+    if (rc) return rc;
+    h->Jtiles_tile = T; h->Jtiles_kind = three_d ? 3 : 2;
+    return 0;
+}
+
+int ensure_scratch(void** p, size_t* have, size_t need) {
+    if (need <= *have) return 0;
+    cudaStreamSynchronize(hooks().stream);
+    dev_free(*p); *p = nullptr; *have = 0;
+    *p = dev_alloc(need);
+    if (!*p) return ISING_ENOMEM;
+    *have = need;
+    return 0;
+}
+
+// n passes, one launcher call per pass, E and M measured on the records after each pass if a series is wanted
+template <class Launch>
+int per_pass(const SweepCall& c, Launch launch) {
+    ising_ctx* h = c.h;
+    int rc = 0;
+    for (int pass = 0; pass < c.n && !rc; ++pass) {
+        rc = launch(h->t + (uint64_t)pass * (uint64_t)c.k);
+        if (!rc && c.want_series)
+            rc = observables_now(h, c.d_E ? c.d_E + (size_t)pass * h->R : nullptr, c.d_M ? c.d_M + (size_t)pass * h->R : nullptr);
+    }
+    return rc;
+}
+
+bool planes_rng(const SweepCall& c) { return !c.h->force_generic && c.h->rng == ISING_RNG_PLANES; }
+bool onchip_ok(const ising_ctx* h) { return !h->no_resident && !h->no_onchip; }
+
+// f1: asynchronous multi-spin coding, 32 realisations per word, one random number per site
+int path_amsc(SweepCall& c) {
+    ising_ctx* h = c.h;
+    if (h->force_generic || !amsc_supported(h, c.T)) return kSkip;
+    h->last_path = "amsc";
+    int rc = 0;
+    if (!h->d_amsc_J) {
+        h->d_amsc_J = dev_alloc((size_t)h->N * 8);
+        if (!h->d_amsc_J) return ISING_ENOMEM;
+        rc = launch_amsc_pack_J(h, h->d_amsc_J);
+        if (rc) { dev_free(h->d_amsc_J); h->d_amsc_J = nullptr; return rc; }      // never sweep on half-packed bonds
+    }
+    rc = ensure_store(h, Store::Amsc, 0);
+    if (rc) return rc;
+    return per_pass(c, [&](uint64_t t0) { return launch_amsc_pass(h, c.acc, c.T, c.k, t0, h->d_amsc_J); });
+}
+
+// a8, config 1: the 64 x 64 plain checkerboard, the whole run in one launch, E / M measured in the kernel
+int path_plain64(SweepCall& c) {
+    ising_ctx* h = c.h;
+    if (!planes_rng(c) || !plain64_supported(h, c.T)) return kSkip;
+    h->last_path = path_name("plain64_planes", c.bits);
+    int rc = ensure_store(h, c.bits ? Store::PlaneBits : Store::PlaneI8, c.T);
+    if (!rc) rc = ensure_couplings(h, false, c.T);
+    if (!rc && c.n > 0) rc = launch_plain64(h, c.acc, c.bits, c.n, c.k, h->t, c.d_E, c.d_M);
+    return rc;
+}
+
+// a8 beyond L = 64 (tile == L) and the double checkerboard of coarse tiles other than the register tiles (the paper's
+// T = 2 ... 16; 128, 256, ...) as masked half-sweeps, 2D: cluster-resident if the lattice is small, else a launch
+// per half-sweep.  The register tiling Tp is invisible in the result.
+int path_plain2d(SweepCall& c) {
+    ising_ctx* h = c.h;
+    if (!planes_rng(c) || h->dim != 2 || c.n <= 0 || !(c.T == h->L || c.Tc2)) return kSkip;
+    int Tp = 0;
+    if (onchip_ok(h)) Tp = resident_planes_supported(h, 32) ? 32 : (resident_planes_supported(h, 64) ? 64 : 0);
+    const bool resident = Tp != 0;
+    if (!Tp) Tp = tile_planes_supported(h, 64) ? 64 : (tile_planes_supported(h, 32) ? 32 : 0);
+    if (!Tp) return kSkip;
+    int rc = ensure_store(h, c.bits ? Store::PlaneBits : Store::PlaneI8, Tp);
+    if (!rc) rc = ensure_couplings(h, false, Tp);
+    if (rc) return rc;
+    if (resident) {
+        if (launch_resident_planes(h, c.acc, Tp, c.bits, c.n, c.k, h->t, c.d_E, c.d_M, true, c.Tc2) == 0) {
+            h->last_path = path_name(c.Tc2 ? "resident_masked" : "resident_plain", c.bits);
+            return kDone;
+        }
+        cudaGetLastError();          // the cluster did not fit: a launch per half-sweep
+    }
+    h->last_path = path_name(c.Tc2 ? "tile_masked" : "tile_plain", c.bits);
+    return per_pass(c, [&](uint64_t t0) { return launch_tile_planes_plain(h, c.acc, Tp, c.bits, 1, c.k, t0, c.Tc2); });
+}
+
+// the same in 3D: 8^3 register tiles, cluster-resident up to L = 64, else a launch per half-sweep
+int path_plain3d(SweepCall& c) {
+    ising_ctx* h = c.h;
+    if (!planes_rng(c) || h->dim != 3 || c.n <= 0 || !(c.T == h->L || c.Tc3) || !tile3d_supported(h, 8)) return kSkip;
+    int rc = ensure_store(h, c.bits ? Store::Plane3Bits : Store::Plane3I8, 8);
+    if (!rc) rc = ensure_couplings(h, true, 8);
+    if (rc) return rc;
+    if (onchip_ok(h) && resident3d_supported(h, 8)) {
+        if (launch_resident3d(h, c.acc, c.bits, c.n, c.k, h->t, c.d_E, c.d_M, true, c.Tc3) == 0) {
+            h->last_path = path_name(c.Tc3 ? "resident3d_masked" : "resident3d_plain", c.bits);
+            return kDone;
+        }
+        cudaGetLastError();
+    }
+    h->last_path = path_name(c.Tc3 ? "tile3d_masked" : "tile3d_plain", c.bits);
+    return per_pass(c, [&](uint64_t t0) { return launch_tile3d_plain(h, c.acc, c.bits, 1, c.k, t0, c.Tc3); });
+}
+
+// a1-a7 on the 2D register tiles 32 / 64 (planes mapping): one launch per call where that pays — cluster-resident (small
+// lattices), grid-resident (lattices that fit on chip), data-flow (HBM-resident, k = 1) — else a launch per coarse colour
+int path_tiled2d(SweepCall& c) {
+    ising_ctx* h = c.h;
+    if (!planes_rng(c) || !tile_planes_supported(h, c.T)) return kSkip;
+    const int T = c.T, n = c.n, k = c.k;
+    int rc = ensure_store(h, c.bits ? Store::PlaneBits : Store::PlaneI8, T);
+    if (!rc) rc = ensure_couplings(h, false, T);
+    if (rc) return rc;
+    // run-time specialisation pays for its ~1 s of compilation only on big calls (AUTO: >= 2^27 attempted flips)
+    const bool use_jit = h->jit_mode == ISING_JIT_ON || (h->jit_mode == ISING_JIT_AUTO && (double)n * k * (double)h->N * h->R >= 134217728.0);
+    h->last_jit = 0;
+    if (n >= 2 && onchip_ok(h)) {
+        if (resident_planes_supported(h, T)) {
+            // small lattices: one thread-block cluster per replica (no specialised form: not when the caller insists on one)
+            if (h->jit_mode != ISING_JIT_ON) {
+                if (launch_resident_planes(h, c.acc, T, c.bits, n, k, h->t, c.d_E, c.d_M, false, 0) == 0) {
+                    h->last_path = path_name("resident_planes", c.bits);
+                    return kDone;
+                }
+                cudaGetLastError();      // the cluster did not fit (shared or partitioned GPU): a launch per colour instead
+            }
+        } else if (grid_planes_supported(h, T)) {
+            // beyond the cluster, still on chip: one cooperative launch on all SMs, boundary words through L2 (k_grid_planes)
+            rc = ensure_scratch(&h->d_xedge, &h->xedge_bytes, grid_planes_xedge_bytes(h, T));
+            if (!rc && c.want_series) rc = ensure_scratch(&h->d_gacc, &h->gacc_bytes, grid_planes_acc_bytes(h, n));
+            if (rc) return rc;
+            const int g = launch_grid_planes(h, c.acc, T, c.bits, n, k, h->t, h->d_xedge, h->d_gacc, c.d_E, c.d_M, use_jit, h->jit_mode != ISING_JIT_ON);
+            if (g == 0) { h->last_path = path_name("grid_planes", c.bits); return kDone; }
+            if (g != 1) cudaGetLastError();      // the cooperative launch was refused (shared or partitioned GPU)
+        }
+    }
+    // HBM-resident lattices, several passes, nothing to measure in between, int8 records at k = 1 (the HBM-bound case): one
+    // persistent launch, colours ordered by data flow (k_flow_planes: +2.5 % at L = 16384, +5 % at L = 8192; for k >= 2 the
+    // register budget of the persistent loop costs more than the idle launch tails it removes, and bit records gain nothing)
+    if (!c.want_series && !h->no_resident && !h->no_flow && ((k == 1 && !c.bits) || h->no_onchip) && flow_planes_supported(h, T, n)) {
+        rc = ensure_scratch(&h->d_xedge, &h->xedge_bytes, flow_planes_scratch_bytes(h, T));
+        if (rc) return rc;
+        if (launch_flow_planes(h, c.acc, T, c.bits, n, k, h->t, h->d_xedge, use_jit) == 0) {
+            h->last_path = path_name("flow_planes", c.bits);
+            return kDone;
+        }
+        cudaGetLastError();
+    }
+    h->last_path = path_name("tile_planes", c.bits);
+    return per_pass(c, [&](uint64_t t0) { return launch_tile_planes_pass(h, c.acc, T, c.bits, k, t0, use_jit); });
+}
+
+// the same on the 3D 8^3 register tiles
+int path_tiled3d(SweepCall& c) {
+    ising_ctx* h = c.h;
+    if (!planes_rng(c) || !tile3d_supported(h, c.T)) return kSkip;
+    const int T = c.T, n = c.n, k = c.k;
+    int rc = ensure_store(h, c.bits ? Store::Plane3Bits : Store::Plane3I8, T);
+    if (!rc) rc = ensure_couplings(h, true, T);
+    if (rc) return rc;
+    const bool use_jit = h->jit_mode == ISING_JIT_ON || (h->jit_mode == ISING_JIT_AUTO && (double)n * k * (double)h->N * h->R >= 134217728.0);
+    h->last_jit = 0;
+    if (n >= 2 && onchip_ok(h)) {
+        if (resident3d_supported(h, T)) {
+            if (h->jit_mode != ISING_JIT_ON) {
+                if (launch_resident3d(h, c.acc, c.bits, n, k, h->t, c.d_E, c.d_M, false, 0) == 0) {
+                    h->last_path = path_name("resident3d_planes", c.bits);
+                    return kDone;
+                }
+                cudaGetLastError();
+            }
+        } else if (grid3d_supported(h, T) && (k < 4 || (uint64_t)h->R * h->N / 1024u <= 148u * 20u)) {
+            // (measured at L = 256: with two jobs of a colour per warp and k >= 4 the per-pass kernels are 5 % faster)
+            rc = ensure_scratch(&h->d_xedge, &h->xedge_bytes, grid3d_xedge_bytes(h));
+            if (!rc && c.want_series) rc = ensure_scratch(&h->d_gacc, &h->gacc_bytes, grid3d_acc_bytes(h, n));
+            if (rc) return rc;
+            const int g = launch_grid3d(h, c.acc, c.bits, n, k, h->t, h->d_xedge, h->d_gacc, c.d_E, c.d_M, use_jit);
+            if (g == 0) { h->last_path = path_name("grid3d_planes", c.bits); return kDone; }
+            if (g != 1) cudaGetLastError();
+        }
+    }
+    h->last_path = path_name("tile3d_planes", c.bits);
+    return per_pass(c, [&](uint64_t t0) { return launch_tile3d_pass(h, c.acc, c.bits, k, t0, use_jit); });
+}
+
+// words mapping, int8 row-major tile records (SURVEY's normative mapping)
+int path_tile_i8(SweepCall& c) {
+    ising_ctx* h = c.h;
+    if (h->force_generic || !c.thr_fits || h->rng != ISING_RNG_WORDS || h->layout != ISING_LAYOUT_I8 || !tile_i8_supported(h, c.T)) return kSkip;
+    h->last_path = "tile_i8";
+    const int rc = ensure_store(h, Store::TileI8, c.T);
+    if (rc) return rc;
+    return per_pass(c, [&](uint64_t t0) { return launch_tile_i8_pass(h, c.acc, c.T, c.k, t0); });
+}
+
+// everything else: global-memory kernels on the canonical array (correct, not fast; never a CPU path)
+int path_generic(SweepCall& c) {
+    ising_ctx* h = c.h;
+    if (h->layout != ISING_LAYOUT_I8 && !h->force_generic) {
+        set_error("ising_sweep: no bit-packed kernel for dim=%d L=%d tile=%d rng=%d", h->dim, h->L, c.T, h->rng);
+        return ISING_EUNSUPPORTED;
+    }
+    h->last_path = "generic";
+    const int rc = ensure_canon(h);
+    if (rc) return rc;
+    return launch_generic_sweep(h, c.acc, c.n, c.T, c.k, c.d_E, c.d_M);
+}
+
+typedef int (*SweepPath)(SweepCall&);
+const SweepPath kPaths[] = {path_amsc, path_plain64, path_plain2d, path_plain3d, path_tiled2d, path_tiled3d, path_tile_i8, path_generic};
+
+}  // namespace
 
 static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64_t* E, int64_t* M) {
     if (!h) { set_error("ising_sweep: NULL handle"); return ISING_EINVAL; }
@@ -368,29 +620,32 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         set_error("ising_sweep: need k_inner >= 1, n_sweeps >= 0, finite beta >= 0");
         return ISING_EINVAL;
     }
-    const Accept acc = make_accept(beta, h->dim);
-    cudaStream_t st = hooks().stream;
+    SweepCall c;
+    c.h = h; c.acc = make_accept(beta, h->dim); c.n = n; c.T = T; c.k = k;
+    c.st = hooks().stream;
+    c.bits = h->layout == ISING_LAYOUT_BITS;
+    c.want_series = (E != nullptr) || (M != nullptr);
+    c.d_E = c.d_M = nullptr;
     struct Sweeping {                         // while passes are being launched no cached canonical copy is valid
         ising_ctx* h; bool on;
         ~Sweeping() { h->sweeping = false; if (on) ++h->state_version; }
     } sweeping{h, n > 0};
     h->sweeping = n > 0;
-    const bool want_series = (E != nullptr) || (M != nullptr);
     const size_t cnt = (size_t)n * h->R;
-    long long *d_E = nullptr, *d_M = nullptr, *tmp = nullptr;
+    long long* tmp = nullptr;
     const bool E_dev = E && is_device_ptr(E), M_dev = M && is_device_ptr(M);
-    if (want_series && cnt) {
+    if (c.want_series && cnt) {
         const size_t need = ((E && !E_dev) ? cnt : 0) + ((M && !M_dev) ? cnt : 0);
         if (need) {
             tmp = (long long*)dev_alloc(need * sizeof(long long));
             if (!tmp) return ISING_ENOMEM;
         }
         long long* q = tmp;
-        if (E) { d_E = E_dev ? (long long*)E : q; if (!E_dev) q += cnt; }
-        if (M) { d_M = M_dev ? (long long*)M : q; }
+        if (E) { c.d_E = E_dev ? (long long*)E : q; if (!E_dev) q += cnt; }
+        if (M) { c.d_M = M_dev ? (long long*)M : q; }
     }
-    int rc = 0;
-    const bool thr_fits = !(acc.thr_is_2p32[0] || acc.thr_is_2p32[1] || acc.thr_is_2p32[2]);   // beta = 0 only
+    const Accept& acc = c.acc;
+    c.thr_fits = !(acc.thr_is_2p32[0] || acc.thr_is_2p32[1] || acc.thr_is_2p32[2]);   // beta = 0 only
     // 0 < beta < ~1.4e-17: thr[1] rounds to 2^32 while thr[2] (thr[3]) is 2^32 - 1.  The multi-spin kernels fold "2^32" into one
     // all-or-nothing mask, so that case (the accept decision differs for r = 0xffffffff only) goes to the generic kernels,
     // which compare every threshold on its own
@@ -401,245 +656,13 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         ~ForceGeneric() { h->force_generic = saved; }
     } fg{h, h->force_generic};
     if (thr_mixed) h->force_generic = 1;
-    const bool use_tile_i8 = !h->force_generic && thr_fits && h->rng == ISING_RNG_WORDS &&
-                             h->layout == ISING_LAYOUT_I8 && tile_i8_supported(h, T);
-    const bool use_planes = !h->force_generic && h->rng == ISING_RNG_PLANES && tile_planes_supported(h, T);
-    const bool use_plain64 = !h->force_generic && h->rng == ISING_RNG_PLANES && plain64_supported(h, T);
-    const bool use_3d = !h->force_generic && h->rng == ISING_RNG_PLANES && tile3d_supported(h, T);
-    const bool use_amsc = !h->force_generic && thr_fits_or_zero(acc) && amsc_supported(h, T);
-    // a8 beyond L = 64: the plain checkerboard (tile == L) on the cluster-resident kernel; the register tiling Tp is
-    // invisible in the result
-    int Tp = 0;
-    bool Tp_resident = false;
-    // ... and the double checkerboard of the paper's small tiles (T = 2, 4, 8, 16 < 32) as masked half-sweeps on the same tiling
-    // (and tiles of 128, 256, ...: whole register tiles switched on and off)
-    const int Tc = (T >= 2 && (T & (T - 1)) == 0 && T != 32 && T != 64 && T != h->L) ? T : 0;
-    if (!h->force_generic && !use_plain64 && !use_amsc && h->rng == ISING_RNG_PLANES && (T == h->L || Tc) && h->dim == 2 && n > 0) {
-        if (!h->no_resident && !h->no_onchip) Tp = resident_planes_supported(h, 32) ? 32 : (resident_planes_supported(h, 64) ? 64 : 0);
-        Tp_resident = Tp != 0;
-        if (!Tp) Tp = tile_planes_supported(h, 64) ? 64 : (tile_planes_supported(h, 32) ? 32 : 0);   // large L: a launch per half-sweep
-    }
-    bool plain_done = false;
-    if (Tp) {
-        const bool bits = h->layout == ISING_LAYOUT_BITS;
-        rc = ensure_store(h, bits ? Store::PlaneBits : Store::PlaneI8, Tp);
-        if (!rc && h->has_J && h->Jtiles_tile != Tp) {
-            if (!h->d_Jtiles) {
-                h->d_Jtiles = dev_alloc(coupling_record_bytes(h));
-                if (!h->d_Jtiles) rc = ISING_ENOMEM;
-            }
-            if (!rc) rc = launch_convert_couplings(h, Tp, h->d_Jtiles);
-            if (!rc) h->Jtiles_tile = Tp;
-        }
-        if (!rc && Tp_resident) {
-            if (launch_resident_planes(h, acc, Tp, bits, n, k, h->t, d_E, d_M, true, Tc) == 0) {
-                h->last_path = Tc ? (bits ? "resident_masked_bits" : "resident_masked_i8") : (bits ? "resident_plain_bits" : "resident_plain_i8");
-                plain_done = true;
-            } else {
-                cudaGetLastError();          // the cluster did not fit: a launch per half-sweep
-            }
-        }
-        if (!rc && !plain_done) {
-            h->last_path = Tc ? (bits ? "tile_masked_bits" : "tile_masked_i8") : (bits ? "tile_plain_bits" : "tile_plain_i8");
-            for (int pass = 0; pass < n && !rc; ++pass) {
-                rc = launch_tile_planes_plain(h, acc, Tp, bits, 1, k, h->t + (uint64_t)pass * (uint64_t)k, Tc);
-                if (!rc && want_series)
-                    rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);
-            }
-            plain_done = !rc;
-        }
-    }
-    // the same in 3D: 8^3 register tiles, cluster-resident up to L = 64, else a launch per half-sweep
-    const int Tc3 = (h->dim == 3 && T >= 2 && (T & (T - 1)) == 0 && T != 8 && T != h->L) ? T : 0;      // masked coarse tiles in 3D
-    if (!Tp && !rc && !h->force_generic && !use_amsc && h->rng == ISING_RNG_PLANES && (T == h->L || Tc3) && h->dim == 3 && n > 0 &&
-        tile3d_supported(h, 8)) {
-        const bool bits = h->layout == ISING_LAYOUT_BITS;
-        rc = ensure_store(h, bits ? Store::Plane3Bits : Store::Plane3I8, 8);
-        if (!rc && h->has_J && h->Jtiles_tile != 8) {
-            if (!h->d_Jtiles) {
-                h->d_Jtiles = dev_alloc(coupling_record3d_bytes(h));
-                if (!h->d_Jtiles) rc = ISING_ENOMEM;
-            }
-            if (!rc) rc = launch_convert_couplings3d(h, h->d_Jtiles);
-            if (!rc) h->Jtiles_tile = 8;
-        }
-        if (!rc && !h->no_resident && !h->no_onchip && resident3d_supported(h, 8)) {
-            if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M, true, Tc3) == 0) {
-                h->last_path = Tc3 ? (bits ? "resident3d_masked_bits" : "resident3d_masked_i8") : (bits ? "resident3d_plain_bits" : "resident3d_plain_i8");
-                plain_done = true;
-            } else {
-                cudaGetLastError();
-            }
-        }
-        if (!rc && !plain_done) {
-            h->last_path = Tc3 ? (bits ? "tile3d_masked_bits" : "tile3d_masked_i8") : (bits ? "tile3d_plain_bits" : "tile3d_plain_i8");
-            for (int pass = 0; pass < n && !rc; ++pass) {
-                rc = launch_tile3d_plain(h, acc, bits, 1, k, h->t + (uint64_t)pass * (uint64_t)k, Tc3);
-                if (!rc && want_series)
-                    rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);
-            }
-            plain_done = !rc;
-        }
-    }
-    if (plain_done || rc) {
-        // nothing more to launch
-    } else if (use_amsc) {                          // f1: 32 realisations per word, one random number per site
-        h->last_path = "amsc";
-        if (!h->d_amsc_J) {
-            h->d_amsc_J = dev_alloc((size_t)h->N * 8);
-            if (!h->d_amsc_J) rc = ISING_ENOMEM;
-            if (!rc) rc = launch_amsc_pack_J(h, h->d_amsc_J);
-            if (rc && h->d_amsc_J) { dev_free(h->d_amsc_J); h->d_amsc_J = nullptr; }      // never sweep on half-packed bonds
-        }
-        if (!rc) rc = ensure_store(h, Store::Amsc, 0);
-        for (int pass = 0; pass < n && !rc; ++pass) {
-            rc = launch_amsc_pass(h, acc, T, k, h->t + (uint64_t)pass * (uint64_t)k, h->d_amsc_J);
-            if (!rc && want_series)
-                rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);
-        }
-    } else if (use_plain64) {                // a8: whole run in one launch, E/M measured in the kernel
-        const bool bits = h->layout == ISING_LAYOUT_BITS;
-        h->last_path = bits ? "plain64_planes_bits" : "plain64_planes_i8";
-        rc = ensure_store(h, bits ? Store::PlaneBits : Store::PlaneI8, T);
-        if (!rc && h->has_J && h->Jtiles_tile != T) {
-            if (!h->d_Jtiles) {
-                h->d_Jtiles = dev_alloc(coupling_record_bytes(h));
-                if (!h->d_Jtiles) rc = ISING_ENOMEM;
-            }
-            if (!rc) rc = launch_convert_couplings(h, T, h->d_Jtiles);
-            if (!rc) h->Jtiles_tile = T;
-        }
-        if (!rc && n > 0) rc = launch_plain64(h, acc, bits, n, k, h->t, d_E, d_M);
-    } else if (use_tile_i8 || use_planes || use_3d) {
-        const bool bits = h->layout == ISING_LAYOUT_BITS;
-        h->last_path = use_tile_i8 ? "tile_i8" : use_3d ? (bits ? "tile3d_planes_bits" : "tile3d_planes_i8")
-                                                        : (bits ? "tile_planes_bits" : "tile_planes_i8");
-        rc = ensure_store(h, use_tile_i8 ? Store::TileI8 : use_3d ? (bits ? Store::Plane3Bits : Store::Plane3I8)
-                                                                  : (bits ? Store::PlaneBits : Store::PlaneI8), T);
-        if (!rc && (use_planes || use_3d) && h->has_J && h->Jtiles_tile != T) {      // coupling records for this tile edge
-            if (!h->d_Jtiles) {
-                h->d_Jtiles = dev_alloc(use_3d ? coupling_record3d_bytes(h) : coupling_record_bytes(h));
-                if (!h->d_Jtiles) rc = ISING_ENOMEM;
-            }
-            if (!rc) rc = use_3d ? launch_convert_couplings3d(h, h->d_Jtiles) : launch_convert_couplings(h, T, h->d_Jtiles);
-            if (!rc) h->Jtiles_tile = T;
-        }
-        // run-time specialisation pays for its ~1 s of compilation only on big calls (AUTO: >= 2^27 attempted flips)
-        const bool use_jit = (use_planes || use_3d) && (h->jit_mode == ISING_JIT_ON ||
-                             (h->jit_mode == ISING_JIT_AUTO && (double)n * k * (double)h->N * h->R >= 134217728.0));
-        h->last_jit = 0;
-        // small lattices, several passes, nothing to measure in between: the whole call in one cluster launch
-        const bool use_resident = use_planes && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident && !h->no_onchip &&
-                                  resident_planes_supported(h, T);
-        bool resident_done = false;
-        const bool use_resident3 = use_3d && n >= 2 && h->jit_mode != ISING_JIT_ON && !h->no_resident && !h->no_onchip &&
-                                   resident3d_supported(h, T);
-        if (use_resident3 && !rc) {
-            if (launch_resident3d(h, acc, bits, n, k, h->t, d_E, d_M, false, 0) == 0) {
-                h->last_path = bits ? "resident3d_planes_bits" : "resident3d_planes_i8";
-                resident_done = true;
-            } else {
-                cudaGetLastError();
-            }
-        }
-        if (use_resident && !rc) {
-            if (launch_resident_planes(h, acc, T, bits, n, k, h->t, d_E, d_M, false, 0) == 0) {
-                h->last_path = bits ? "resident_planes_bits" : "resident_planes_i8";
-                resident_done = true;
-            } else {
-                cudaGetLastError();      // the cluster did not fit (shared or partitioned GPU): a launch per colour instead
-            }
-        }
-        // 2D lattices beyond the cluster (more than 64 jobs per colour) that still fit on chip: one cooperative launch, tiles in
-        // the shared memory / registers of all SMs, boundary words exchanged through L2 (k_grid_planes)
-        const bool use_grid = use_planes && !resident_done && n >= 2 && !h->no_resident && !h->no_onchip &&
-                              !resident_planes_supported(h, T) && grid_planes_supported(h, T);
-        if (use_grid && !rc) {
-            const size_t xb = grid_planes_xedge_bytes(h, T), ab = want_series ? grid_planes_acc_bytes(h, n) : 0;
-            if (xb > h->xedge_bytes) {
-                cudaStreamSynchronize(st);
-                dev_free(h->d_xedge); h->xedge_bytes = 0;
-                h->d_xedge = dev_alloc(xb);
-                if (!h->d_xedge) rc = ISING_ENOMEM; else h->xedge_bytes = xb;
-            }
-            if (!rc && ab > h->gacc_bytes) {
-                cudaStreamSynchronize(st);
-                dev_free(h->d_gacc); h->gacc_bytes = 0;
-                h->d_gacc = dev_alloc(ab);
-                if (!h->d_gacc) rc = ISING_ENOMEM; else h->gacc_bytes = ab;
-            }
-            if (!rc) {
-                const int g = launch_grid_planes(h, acc, T, bits, n, k, h->t, h->d_xedge, h->d_gacc, d_E, d_M, use_jit, h->jit_mode != ISING_JIT_ON);
-                if (g == 0) {
-                    h->last_path = bits ? "grid_planes_bits" : "grid_planes_i8";
-                    resident_done = true;
-                } else if (g != 1) {
-                    cudaGetLastError();      // the cooperative launch was refused (shared or partitioned GPU): a launch per colour instead
-                }
-            }
-        }
-        // (measured at L = 256: with two jobs of a colour per warp and k >= 4 the per-pass kernels are 5 % faster)
-        // HBM-resident 2D lattices, several passes, nothing to measure in between, k = 1 (the HBM-bound case): one persistent
-        // launch, colours ordered by data flow (k_flow_planes: +2.5 % at L = 16384, +5 % at L = 8192; for k >= 2 the register
-        // budget of the persistent loop costs more than the idle launch tails it removes: a launch per colour)
-        const bool use_flow = use_planes && !resident_done && !want_series && !h->no_resident && !h->no_flow && ((k == 1 && !bits) || h->no_onchip) &&
-                              flow_planes_supported(h, T, n);      // (bit records: 2854 against 2886 flips/ns, no gain)
-        if (use_flow && !rc) {
-            const size_t sb = flow_planes_scratch_bytes(h, T);
-            if (sb > h->xedge_bytes) {
-                cudaStreamSynchronize(st);
-                dev_free(h->d_xedge); h->xedge_bytes = 0;
-                h->d_xedge = dev_alloc(sb);
-                if (!h->d_xedge) rc = ISING_ENOMEM; else h->xedge_bytes = sb;
-            }
-            if (!rc && launch_flow_planes(h, acc, T, bits, n, k, h->t, h->d_xedge, use_jit) == 0) {
-                h->last_path = bits ? "flow_planes_bits" : "flow_planes_i8";
-                resident_done = true;
-            } else if (!rc) {
-                cudaGetLastError();
-            }
-        }
-        const bool use_grid3 = use_3d && !resident_done && n >= 2 && !h->no_resident && !h->no_onchip && !resident3d_supported(h, T) && grid3d_supported(h, T) &&
-                               (k < 4 || (uint64_t)h->R * h->N / 1024u <= 148u * 20u);
-        if (use_grid3 && !rc) {
-            const size_t xb = grid3d_xedge_bytes(h), ab = want_series ? grid3d_acc_bytes(h, n) : 0;
-            if (xb > h->xedge_bytes) {
-                cudaStreamSynchronize(st);
-                dev_free(h->d_xedge); h->xedge_bytes = 0;
-                h->d_xedge = dev_alloc(xb);
-                if (!h->d_xedge) rc = ISING_ENOMEM; else h->xedge_bytes = xb;
-            }
-            if (!rc && ab > h->gacc_bytes) {
-                cudaStreamSynchronize(st);
-                dev_free(h->d_gacc); h->gacc_bytes = 0;
-                h->d_gacc = dev_alloc(ab);
-                if (!h->d_gacc) rc = ISING_ENOMEM; else h->gacc_bytes = ab;
-            }
-            if (!rc) {
-                const int g = launch_grid3d(h, acc, bits, n, k, h->t, h->d_xedge, h->d_gacc, d_E, d_M, use_jit);
-                if (g == 0) {
-                    h->last_path = bits ? "grid3d_planes_bits" : "grid3d_planes_i8";
-                    resident_done = true;
-                } else if (g != 1) {
-                    cudaGetLastError();
-                }
-            }
-        }
-        for (int pass = 0; pass < n && !rc && !resident_done; ++pass) {
-            const uint64_t t0 = h->t + (uint64_t)pass * (uint64_t)k;
-            rc = use_tile_i8 ? launch_tile_i8_pass(h, acc, T, k, t0)
-                 : use_3d ? launch_tile3d_pass(h, acc, bits, k, t0, use_jit)
-                          : launch_tile_planes_pass(h, acc, T, bits, k, t0, use_jit);
-            if (!rc && want_series)
-                rc = observables_now(h, d_E ? d_E + (size_t)pass * h->R : nullptr, d_M ? d_M + (size_t)pass * h->R : nullptr);
-        }
-    } else if (h->layout == ISING_LAYOUT_I8 || h->force_generic) {
-        h->last_path = "generic";
-        rc = ensure_canon(h);
-        if (!rc) rc = launch_generic_sweep(h, acc, n, T, k, d_E, d_M);
-    } else {
-        set_error("ising_sweep: no bit-packed kernel for dim=%d L=%d tile=%d rng=%d", h->dim, h->L, T, h->rng);
-        rc = ISING_EUNSUPPORTED;
+    const bool pow2 = T >= 2 && (T & (T - 1)) == 0 && T != h->L;
+    c.Tc2 = (pow2 && T != 32 && T != 64) ? T : 0;
+    c.Tc3 = (h->dim == 3 && pow2 && T != 8) ? T : 0;
+    int rc = kSkip;
+    for (SweepPath path : kPaths) {
+        rc = path(c);
+        if (rc != kSkip) break;
     }
     if (!rc) h->t += (uint64_t)n * (uint64_t)k;
     if (!rc && tmp) {
@@ -647,7 +670,7 @@ static int sweep_impl(ising_handle h, double beta, int n, int tile, int k, int64
         if (E && !E_dev) { rc = copy_out(E, q, cnt * sizeof(long long), nullptr); q += cnt; }
         if (!rc && M && !M_dev) rc = copy_out(M, q, cnt * sizeof(long long), nullptr);
     }
-    if (tmp) { cudaStreamSynchronize(st); dev_free(tmp); }
+    if (tmp) { cudaStreamSynchronize(c.st); dev_free(tmp); }
     return rc;
 }
 
