@@ -327,28 +327,30 @@ def run_config(P, torch, a) -> None:
 
 def run_amsc(P, torch, a) -> None:
     """asynchronous multi-spin coding ("0.15 ps per spin flip").  32 disorder realisations of the
-    2D +-J model per word, one random number per site; attempted flips per ns summed over the realisations."""
+    +-J model per machine word (64: two word lattices), one random number per site; attempted flips per ns summed over the realisations; 2D, and the 3D
+    Edwards-Anderson glass."""
     rows = []
-    R = 32
-    single = a.L != 16384                      # --L given: one variant (--L, --tile, --k), e.g. for an ncu capture
-    for L in ((a.L,) if single else (1024, 2048, 4096)):
-        J = W.realisations(2, L, R, 5)
-        for T in ((a.tile,) if single else (32, 64)):
-            for k in ((a.k,) if single else (1, 4, 16)):
-                g = P.Ising(2, L, coupling=J, seeds=list(range(100, 100 + R)), sweep_seed=77)
-                n = max(4, min(400, int(4e11 / (k * R * L * L))))
-                g.sweep(1.0, 3, T, k)
-                g.synchronize()
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record()
-                g.sweep(1.0, n, T, k)
-                e1.record()
-                torch.cuda.synchronize()
-                ms = e0.elapsed_time(e1)
-                rows.append({"L": L, "tile": T, "k": k, "realisations": R, "passes": n, "path": g.sweep_path(),
-                             "flips_per_ns": round(n * k * R * L * L / (ms * 1e6), 1),
-                             "ps_per_flip": round(ms * 1e9 / (n * k * R * L * L), 4)})
-                g.destroy()
+    single = a.L != 16384                      # --L given: one variant (--dim, --L, --tile, --k), e.g. for an ncu capture
+    cases = [(a.dim, a.L, a.tile, a.k, 32)] if single else \
+        [(2, L, T, k, R) for L in (1024, 4096) for T in (32, 64) for k in (1, 4, 16) for R in (32, 64)] + \
+        [(3, L, 8, k, R) for L in (64, 128) for k in (1, 4, 16) for R in (32, 64)]
+    for dim, L, T, k, R in cases:
+        J = W.realisations(dim, L, R, 5)
+        g = P.Ising(dim, L, coupling=J, seeds=list(range(100, 100 + R)), sweep_seed=77)
+        n = max(4, min(400, int(4e11 / (k * R * L ** dim))))
+        g.sweep(1.0, 3, T, k)
+        g.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        g.sweep(1.0, n, T, k)
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1)
+        rows.append({"dim": dim, "L": L, "tile": T, "k": k, "realisations": R, "passes": n, "path": g.sweep_path(),
+                     "flips_per_ns": round(n * k * R * L ** dim / (ms * 1e6), 1),
+                     "ps_per_flip": round(ms * 1e9 / (n * k * R * L ** dim), 4)})
+        g.destroy()
+        del J
     print(json.dumps({"study": "amsc", "beta": 1.0, "unit": UNIT, "rows": rows}), flush=True)
 
 

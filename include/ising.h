@@ -74,8 +74,9 @@ ising_handle ising_create_batch(int dim, int L, const int8_t* coupling_or_null,
  * r(i, H) keyed by sweep_seed: realisation r is exactly an ordinary run with couplings J[r] whose random stream
  * happens to be shared with the others.  Everything else (sweep, observables per realisation, copy_spins R*N bytes,
  * overlap) is as for ising_create_batch.  The RNG mapping of a multi handle starts as ISING_RNG_WORDS (one random
- * word per site serves all realisations); with it, dim 2, n_realisations <= 32 and tile 32 / 64 the sweep runs on
- * the multi-spin-coded kernel (32 realisations per machine word). */
+ * word per site serves all realisations); with it, n_realisations <= 256 and tile 32 / 64 (dim 2) or tile 8 (dim 3: the
+ * Edwards-Anderson glass of P:100) the sweep runs on the multi-spin-coded kernels (32 realisations per machine word; more
+ * than 32 as several word lattices driven by the same random numbers). */
 ising_handle ising_create_multi(int dim, int L, const int8_t* couplings, const uint64_t* init_seeds, int n_realisations,
                                 uint64_t sweep_seed);
 

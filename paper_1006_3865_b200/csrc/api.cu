@@ -436,7 +436,7 @@ int path_amsc(SweepCall& c) {
     h->last_path = "amsc";
     int rc = 0;
     if (!h->d_amsc_J) {
-        h->d_amsc_J = dev_alloc((size_t)h->N * 8);
+        h->d_amsc_J = dev_alloc(amsc_bond_bytes(h));
         if (!h->d_amsc_J) return ISING_ENOMEM;
         rc = launch_amsc_pack_J(h, h->d_amsc_J);
         if (rc) { dev_free(h->d_amsc_J); h->d_amsc_J = nullptr; return rc; }      // never sweep on half-packed bonds

@@ -71,9 +71,11 @@ int launch_grid3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint
 int launch_tile3d_plain(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint64_t t_first, int Tc);   // a8 in 3D, L > 64
 int launch_observables3d(ising_ctx* h, bool bits, long long* d_E, long long* d_M);   // a10 on 3D tile records
 
-// ---- amsc.cu: asynchronous multi-spin coding, 32 disorder realisations per word (multi handles, R17) ----
+// ---- amsc.cu: asynchronous multi-spin coding, 32 disorder realisations per word lattice, up to 256 per handle, 2D and 3D (R17) ----
 bool amsc_supported(const ising_ctx* h, int T);
+bool amsc3d_supported(const ising_ctx* h, int T);
 size_t amsc_spin_bytes(const ising_ctx* h);
+size_t amsc_bond_bytes(const ising_ctx* h);
 int launch_amsc_pack_J(ising_ctx* h, void* d_jwords);
 int launch_canon_to_amsc(ising_ctx* h, const int8_t* d_canon, void* d_words);
 int launch_amsc_to_canon(ising_ctx* h, const void* d_words, int8_t* d_canon);

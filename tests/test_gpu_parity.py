@@ -884,3 +884,30 @@ def test_data_flow_kernel_matches_oracle(P, orc, L, tile, k, n, beta, seeds, jse
     g.sweep(beta, 2, tile, k); o.sweep(beta, 2, tile, k)
     assert g.sweep_path() in (f"tile_planes_{sfx}", f"resident_planes_{sfx}", f"grid_planes_{sfx}")
     _same_state(g, o)
+
+
+@pytest.mark.parametrize("dim,L,tile,k,n,beta,R", [
+    (2, 64, 32, 1, 3, 1.0, 33), (2, 128, 32, 2, 2, 0.8, 64), (2, 128, 64, 1, 2, 1.2, 48), (2, 128, 32, 2, 2, 0.0, 40),   # several word lattices
+    (2, 64, 32, 1, 2, 1.0, 100),
+    (3, 16, 8, 1, 3, 0.9, 8), (3, 32, 8, 2, 2, 0.5, 32), (3, 16, 8, 2, 2, 1.1, 50), (3, 48, 8, 1, 2, 0.9, 5),            # 3D: the EA glass of P:100
+    (3, 16, 8, 1, 2, 0.0, 3), (3, 16, 8, 1, 2, 9.0, 64),
+])
+def test_multi_realisation_batch_wide_and_3d(P, orc, dim, L, tile, k, n, beta, R):
+    """Asynchronous multi-spin coding beyond the first slice ("missing" 6): more than 32 realisations per handle
+    (several 32-bit word lattices driven by the same random numbers), and the 3D Edwards-Anderson glass (8^3 tiles); every
+    realisation against the oracle's multi batch."""
+    Js = np.stack([W.couplings(dim, L, 700 + r) for r in range(R)])
+    seeds = [3000 + r for r in range(R)]
+    g = P.Ising(dim, L, coupling=Js, seeds=seeds, sweep_seed=777)
+    o = orc.Oracle(dim, L, J=Js, seeds=seeds, sweep_seed=777, rng="words")
+    _same_state(g, o)
+    Eg, Mg = g.sweep_series(beta, n, tile, k)
+    assert g.sweep_path() == "amsc"
+    Eo, Mo = o.sweep_series(beta, n, tile, k)
+    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)
+    _same_state(g, o)
+    g.sweep(beta, 2, tile, k); o.sweep(beta, 2, tile, k)
+    _same_state(g, o)
+    assert g.overlap(0, R - 1) == o.overlap(0, R - 1)
+    Q = g.overlap_all()
+    assert Q[1, R - 1] == o.overlap(1, R - 1) and Q[0, 0] == L ** dim
