@@ -166,7 +166,11 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
                 load_couplings<HASJ>(A, jb.t, lz, s);
                 refresh(s, jb, ph + 1u);
                 if (series && C == 0 && pass > 0) account(s, jb.t.r, pass - 1);
+#if defined(ISING_JIT_R) && ISING_JIT_R == 1
+                const uint64_t seed = A.seed0;
+#else
                 const uint64_t seed = A.seeds[jb.t.r];
+#endif
                 const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
                 const uint32_t z = (uint32_t)(jb.t.tz * kT3 + lz);
                 const uint32_t g = (z * B + (uint32_t)jb.t.ty) * B + (uint32_t)jb.t.tx;

@@ -190,16 +190,16 @@ cudaKernel_t grid_jit_kernel(int T, bool bits, bool hasj, uint32_t hp) {
 }
 
 // The 3D kernel specialised for (BITS, HP3 = the three threshold heads).
-cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3) {
+cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3, int R) {
     char expr[160];
     snprintf(expr, sizeof expr, "ising::jit::k_tile3d_planes<%s, %lluull>", bits ? "true" : "false", hp3);
-    return cached(kJitSource3d, expr, {});
+    return cached(kJitSource3d, expr, {R == 1 ? "-DISING_JIT_R=1" : "-DISING_JIT_R=0"});
 }
 
-cudaKernel_t grid3d_jit_kernel(bool bits, unsigned long long hp3) {
+cudaKernel_t grid3d_jit_kernel(bool bits, unsigned long long hp3, int R) {
     char expr[160];
     snprintf(expr, sizeof expr, "ising::jit::k_grid3d<%s, false, %lluull>", bits ? "true" : "false", hp3);
-    return cached(kJitSource3d, expr, {});
+    return cached(kJitSource3d, expr, {R == 1 ? "-DISING_JIT_R=1" : "-DISING_JIT_R=0"});
 }
 
 uint64_t planes_jit_compiled() { return state().compiled; }

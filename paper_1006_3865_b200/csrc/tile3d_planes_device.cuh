@@ -22,6 +22,7 @@ constexpr int kXL = 0, kXR = 32, kYL = 64, kYR = 72, kZL = 80, kZR = 88;   // of
 struct Plane3Args {
     uint8_t* tiles;              // records, replica-major; tile (tz, ty, tx) at ((tz*B + ty)*B + tx)
     const uint64_t* seeds;
+    uint64_t seed0;              // seeds[0]: the (uniform) key of a single-replica handle, used by kernels compiled with ISING_JIT_R == 1
     int L, B, R;
     int C;                       // coarse colour of this launch
     int k;
@@ -178,35 +179,98 @@ __device__ __forceinline__ void head_masks3(const Plane3Args& A, uint32_t g, uin
 // ---- the same compare specialised on the head bits of the three thresholds (HP3 = head(thr[1]) << 24 |
 // head(thr[2]) << 12 | head(thr[3]); tile_planes_device.cuh explains the idea).  A site needs one threshold:
 // thr[3] if s0 (no unsatisfied bond), thr[2] if s1 (one), else thr[1].  Per plane the threshold bit of every site is a
-// compile-time function of (s0, s1): a constant, or one LOP3; then one borrow chain and one tie accumulator.
+// compile-time function of (s0, s1); then one borrow chain and one tie accumulator.
 constexpr unsigned long long kNoSpec3 = ~0ull;
-__host__ __device__ constexpr int lut_usel3(int u1, int u2, int u3) {        // inputs a = s0, b = s1, c unused
+// Of three binary head bits that are not all equal exactly one differs from the other two, so the site's threshold bit depends on
+// ONE mask: s0 (thr[3] differs), s1 (thr[2] differs) or s0 | s1 (thr[1] differs) — the third LOP3 input of the chain and tie steps.
+// Planes whose bit is the same for all three thresholds need no mask, and two of them share one LOP3 (as in 2D).
+template <unsigned long long HP3, int Q>
+struct HeadBit3 {
+    static constexpr int u1 = (int)((HP3 >> (24 + 11 - Q)) & 1), u2 = (int)((HP3 >> (12 + 11 - Q)) & 1), u3 = (int)((HP3 >> (11 - Q)) & 1);
+    static constexpr bool same = u1 == u2 && u2 == u3;
+    static constexpr int which = same ? -1 : (u1 == u2 ? 0 : (u1 == u3 ? 1 : 2));     // mask: 0 = s0, 1 = s1, 2 = s0 | s1
+    static constexpr int u_clear = u1;                         // the site's threshold bit where the mask is 0 (thr[1] applies, or agrees) ...
+    static constexpr int u_set = u1 == u2 ? u3 : u2;           // ... and where it is 1
+};
+__host__ __device__ constexpr int lut_chain_mask(int u_clear, int u_set) {            // inputs a = p, b = bw, c = mask
     int l = 0;
     for (int i = 0; i < 8; ++i) {
-        const int s0 = (i >> 2) & 1, s1 = (i >> 1) & 1;
-        l |= (s0 ? u3 : (s1 ? u2 : u1)) << i;
+        const int p = (i >> 2) & 1, bw = (i >> 1) & 1, m = i & 1, u = m ? u_set : u_clear;
+        l |= (((!p) && u) || ((p == u) && bw)) << i;
+    }
+    return l;
+}
+__host__ __device__ constexpr int lut_ne_mask(int u_clear, int u_set) {               // inputs a = ne, b = p, c = mask
+    int l = 0;
+    for (int i = 0; i < 8; ++i) {
+        const int ne = (i >> 2) & 1, p = (i >> 1) & 1, m = i & 1, u = m ? u_set : u_clear;
+        l |= (ne || (p != u)) << i;
+    }
+    return l;
+}
+__host__ __device__ constexpr int lut_chain_pair3(int uq, int uq1) {                   // inputs a = p_Q, b = p_(Q-1), c = bw
+    int l = 0;
+    for (int i = 0; i < 8; ++i) {
+        const int pq = (i >> 2) & 1, pq1 = (i >> 1) & 1, bw = i & 1;
+        const int b1 = ((!pq) && uq) || ((pq == uq) && bw);
+        const int b2 = ((!pq1) && uq1) || ((pq1 == uq1) && b1);
+        l |= b2 << i;
+    }
+    return l;
+}
+__host__ __device__ constexpr int lut_ne_pair3(int ua, int ub) {                       // inputs a = ne, b = p_a, c = p_b
+    int l = 0;
+    for (int i = 0; i < 8; ++i) {
+        const int ne = (i >> 2) & 1, pa = (i >> 1) & 1, pb = i & 1;
+        l |= (ne || (pa != ua) || (pb != ub)) << i;
     }
     return l;
 }
 template <unsigned long long HP3, int Q>
-__device__ __forceinline__ void sel_step3(uint32_t p, uint32_t s0, uint32_t s1, uint32_t& bw, uint32_t& ne) {
-    constexpr int u1 = (int)((HP3 >> (24 + 11 - Q)) & 1), u2 = (int)((HP3 >> (12 + 11 - Q)) & 1), u3 = (int)((HP3 >> (11 - Q)) & 1);
-    constexpr int LU = lut_usel3(u1, u2, u3);
-    const uint32_t usel = (u1 == u2 && u2 == u3) ? (u1 ? 0xffffffffu : 0u) : lop3<LU>(s0, s1, 0u);
-    bw = lop3<kLutChain>(p, bw, usel);
-    ne = lop3<kLutNe>(ne, p, usel);
+__device__ __forceinline__ void chain3_from(const uint32_t (&p)[kHeadBits], const uint32_t (&mask)[3], uint32_t& bw) {
+    if constexpr (Q >= 0) {
+        using H = HeadBit3<HP3, Q>;
+        if constexpr (Q >= 1 && H::same && HeadBit3<HP3, (Q >= 1 ? Q - 1 : 0)>::same) {
+            bw = lop3<lut_chain_pair3(H::u1, HeadBit3<HP3, Q - 1>::u1)>(p[Q], p[Q - 1], bw);
+            chain3_from<HP3, Q - 2>(p, mask, bw);
+        } else {
+            bw = lop3<lut_chain_mask(H::same ? H::u1 : H::u_clear, H::same ? H::u1 : H::u_set)>(p[Q], bw, mask[H::same ? 0 : H::which]);
+            chain3_from<HP3, Q - 1>(p, mask, bw);
+        }
+    }
+}
+template <unsigned long long HP3, int Q, int PEND>
+__device__ __forceinline__ void ne3_from(const uint32_t (&p)[kHeadBits], const uint32_t (&mask)[3], uint32_t& ne) {
+    if constexpr (Q >= 0) {
+        using H = HeadBit3<HP3, Q>;
+        if constexpr (!H::same) {
+            ne = lop3<lut_ne_mask(H::u_clear, H::u_set)>(ne, p[Q], mask[H::which]);
+            ne3_from<HP3, Q - 1, PEND>(p, mask, ne);
+        } else if constexpr (PEND < 0) {
+            ne3_from<HP3, Q - 1, Q>(p, mask, ne);
+        } else {
+            ne = lop3<lut_ne_pair3(HeadBit3<HP3, (PEND >= 0 ? PEND : 0)>::u1, H::u1)>(ne, p[PEND >= 0 ? PEND : 0], p[Q]);
+            ne3_from<HP3, Q - 1, -1>(p, mask, ne);
+        }
+    } else if constexpr (PEND >= 0) {
+        constexpr int u = HeadBit3<HP3, (PEND >= 0 ? PEND : 0)>::u1;
+        ne = lop3<lut_ne_pair3(u, u)>(ne, p[PEND >= 0 ? PEND : 0], p[PEND >= 0 ? PEND : 0]);
+    }
 }
 template <unsigned long long HP3>
 __device__ __forceinline__ void head_masks3_sel(uint32_t g, uint32_t Hlo, uint32_t Hhi, uint32_t k0, uint32_t k1, uint32_t s0,
                                                 uint32_t s1, uint32_t& R, uint32_t& eq) {
     static_assert(kHeadBits == 12, "three Philox calls");
+    uint32_t p[kHeadBits];
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+        const u32x4 o = philox4x32_10(g, kTagPlanes + 256u * n, Hlo, Hhi, k0, k1);
+        p[4 * n] = o.x; p[4 * n + 1] = o.y; p[4 * n + 2] = o.z; p[4 * n + 3] = o.w;
+    }
+    const uint32_t mask[3] = {s0, s1, s0 | s1};
     uint32_t bw = 0, ne = 0;
-    u32x4 o = philox4x32_10(g, kTagPlanes + 512u, Hlo, Hhi, k0, k1);       // least significant planes first
-    sel_step3<HP3, 11>(o.w, s0, s1, bw, ne); sel_step3<HP3, 10>(o.z, s0, s1, bw, ne); sel_step3<HP3, 9>(o.y, s0, s1, bw, ne); sel_step3<HP3, 8>(o.x, s0, s1, bw, ne);
-    o = philox4x32_10(g, kTagPlanes + 256u, Hlo, Hhi, k0, k1);
-    sel_step3<HP3, 7>(o.w, s0, s1, bw, ne); sel_step3<HP3, 6>(o.z, s0, s1, bw, ne); sel_step3<HP3, 5>(o.y, s0, s1, bw, ne); sel_step3<HP3, 4>(o.x, s0, s1, bw, ne);
-    o = philox4x32_10(g, kTagPlanes, Hlo, Hhi, k0, k1);
-    sel_step3<HP3, 3>(o.w, s0, s1, bw, ne); sel_step3<HP3, 2>(o.z, s0, s1, bw, ne); sel_step3<HP3, 1>(o.y, s0, s1, bw, ne); sel_step3<HP3, 0>(o.x, s0, s1, bw, ne);
+    chain3_from<HP3, kHeadBits - 1>(p, mask, bw);
+    ne3_from<HP3, kHeadBits - 1, -1>(p, mask, ne);
     R = bw; eq = ~ne;
 }
 
@@ -307,7 +371,11 @@ __global__ void __launch_bounds__(kThreads3) k_tile3d_planes(Plane3Args A) {
     Slice s;
     load_slice<BITS>(A, t, lz, s);
     load_couplings<HASJ>(A, t, lz, s);
+#if defined(ISING_JIT_R) && ISING_JIT_R == 1
+    const uint64_t seed = A.seed0;
+#else
     const uint64_t seed = A.seeds[t.r];
+#endif
     const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
     const uint32_t z = (uint32_t)(t.tz * kT3 + lz);
     const uint32_t g = (z * (uint32_t)A.B + (uint32_t)t.ty) * (uint32_t)A.B + (uint32_t)t.tx;     // RNG block (S3.4)

@@ -137,8 +137,10 @@ __device__ __forceinline__ void load_tile(const PlaneArgs& A, int r, int tx, int
     // halo columns: the left tile's right column, the right tile's left column (same address for every lane of a tile)
     const uint2 cl = ldh64(rec_of(rowc + txL) + BODY + G::E_COL + 8);   // {R0, R1}
     const uint2 cr = ldh64(rec_of(rowc + txR) + BODY + G::E_COL);       // {L0, L1}
-    t.hL0 = (cl.x >> Y) & 1u; t.hL1 = (cl.y >> Y) & 1u;
-    t.hR0 = (cr.x >> Y) & 1u; t.hR1 = (cr.y >> Y) & 1u;
+    // bit 0 = the halo site of this lane's row; the bits above it (other rows) are never looked at: neighbour_words moves bit 0
+    // to the edge of a half-word and everything else out of it
+    t.hL0 = cl.x >> Y; t.hL1 = cl.y >> Y;
+    t.hR0 = cr.x >> Y; t.hR1 = cr.y >> Y;
     (void)lane_base;
 }
 
@@ -180,11 +182,13 @@ __device__ __forceinline__ void store_tile(const PlaneArgs& A, int r, int tx, in
     }
     // boundary columns: x = 0 is colour 0 on even rows (bit 0) and colour 1 on odd rows (bit 16); x = T-1 is
     // colour 1 / colour 0, last pair.  One ballot each; a warp holds 64 / T tiles, LPT bits per tile.
-    const uint32_t sh = (uint32_t)sub * G::LPT, m = G::LPT == 32 ? 0xffffffffu : ((1u << G::LPT) - 1u);
-    const uint32_t L0 = (__ballot_sync(0xffffffffu, t.S[0][0] & 1u) >> sh) & m;
-    const uint32_t L1 = (__ballot_sync(0xffffffffu, (t.S[1][0] >> 16) & 1u) >> sh) & m;
-    const uint32_t R0 = (__ballot_sync(0xffffffffu, (t.S[1][G::NW - 1] >> 15) & 1u) >> sh) & m;
-    const uint32_t R1 = (__ballot_sync(0xffffffffu, t.S[0][G::NW - 1] >> 31) >> sh) & m;
+    // (tile 32: the tile's 16 lanes are one half of the ballot: one byte permute picks it)
+    const uint32_t half = sub ? 0x4432u : 0x4410u;
+    auto mine = [&](uint32_t ballot) { return G::LPT == 32 ? ballot : __byte_perm(ballot, 0u, half); };
+    const uint32_t L0 = mine(__ballot_sync(0xffffffffu, t.S[0][0] & 1u));
+    const uint32_t L1 = mine(__ballot_sync(0xffffffffu, (t.S[1][0] >> 16) & 1u));
+    const uint32_t R0 = mine(__ballot_sync(0xffffffffu, (t.S[1][G::NW - 1] >> 15) & 1u));
+    const uint32_t R1 = mine(__ballot_sync(0xffffffffu, t.S[0][G::NW - 1] >> 31));
     // first lane: TOP + COL (one sector), last lane: BOT + padding (the other sector)
     if (Y == 0 || Y == G::LPT - 1) {
         const uint4 w = G::NW == 2 ? make_uint4(t.S[0][0], t.S[0][1], t.S[1][0], t.S[1][1]) : make_uint4(t.S[0][0], t.S[1][0], 0u, 0u);
