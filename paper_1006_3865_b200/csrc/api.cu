@@ -368,7 +368,6 @@ struct SweepCall {
     bool want_series, bits, thr_fits;
     cudaStream_t st;
     int Tc2, Tc3;                  // coarse tile edge of a masked double checkerboard on the 2D / 3D register tiling, or 0
-    const char* sfx() const { return bits ? "bits" : "i8"; }
 };
 constexpr int kSkip = 1, kDone = 0;
 
