@@ -566,8 +566,10 @@ int path_tiled3d(SweepCall& c) {
                 }
                 cudaGetLastError();
             }
-        } else if (grid3d_supported(h, T) && (k < 4 || (uint64_t)h->R * h->N / 1024u <= 148u * 20u)) {
-            // (measured at L = 256: with two jobs of a colour per warp and k >= 4 the per-pass kernels are 5 % faster)
+        } else if (grid3d_supported(h, T) && ((use_jit && !h->has_J) || k < 4 || (uint64_t)h->R * h->N / 1024u <= 148u * 20u)) {
+            // The run-time build of k_grid3d takes the CTA shape the lattice wants and wins at every k (config 4, k = 16:
+            // 3030 against 2720 flips/ns); the pre-compiled one with two jobs of a colour per warp loses 5 % to the
+            // per-pass kernels at k >= 4.
             rc = ensure_scratch(&h->d_xedge, &h->xedge_bytes, grid3d_xedge_bytes(h));
             if (!rc && c.want_series) rc = ensure_scratch(&h->d_gacc, &h->gacc_bytes, grid3d_acc_bytes(h, n));
             if (rc) return rc;

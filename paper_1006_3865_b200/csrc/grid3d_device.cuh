@@ -15,6 +15,7 @@ namespace ISING_DEVICE_NS3 {
 constexpr int kGrid3AccSlots = 8;
 // exchange record of a tile, u64 = version << 32 | value:  X[lz] = {XL, XR} (16 words), Y[lz] = YL | YR << 8 (8), ZL[2], ZR[2], pad
 constexpr int kG3X = 0, kG3Y = 16, kG3ZL = 24, kG3ZR = 26, kG3Rec = 32;
+constexpr int kG3Slots = 2 + 10;        // shared-memory words per lane and job: the slice and the job's constants
 
 struct Grid3Args {
     Plane3Args P;
@@ -40,9 +41,15 @@ __device__ __forceinline__ void st_x64v2(unsigned long long* p, unsigned long lo
     asm volatile("st.relaxed.gpu.global.v2.u64 [%0], {%1,%2};" ::"l"(p), "l"(a), "l"(b) : "memory");
 }
 
+// CTA shape: the pre-compiled kernels take up to 128 threads, 5 CTAs per SM; the run-time build names its own (launch_grid3d_one)
+#ifndef ISING_G3_THREADS
+#define ISING_G3_THREADS 128
+#define ISING_G3_BLOCKS 5
+#endif
+
 template <bool BITS, bool HASJ, unsigned long long HP3 = kNoSpec3>
-__global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
-    constexpr uint32_t NSLOT = 2 + 9;                         // two words + the job's constants (decoded once) per lane and job
+__global__ void __launch_bounds__(ISING_G3_THREADS, ISING_G3_BLOCKS) k_grid3d(Grid3Args R) {
+    constexpr uint32_t NSLOT = kG3Slots;                      // two words + the job's constants (decoded once) per lane and job
     extern __shared__ uint32_t grid3_smem[];                  // per warp: [colour][job][slot][lane]
     const Plane3Args& A = R.P;
     const int lane = threadIdx.x & 31;
@@ -53,7 +60,8 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
     const uint2* lut = kByteLutGlobal.e;
     const bool series = R.acc != nullptr;
 
-    struct Job { Tile3 t; uint32_t self, xm, xp, ym, yp, zm, zp; };       // tile indices into xedge
+    // what a lane keeps of a job: its tile, and the u64 offsets into xedge of its own record and of the words it polls
+    struct Job { Tile3 t; uint32_t self, oxm, oxp, oym, oyp, oz, g, p_base; };
     auto decode = [&](uint32_t job, int C) {
         const uint32_t q = job * 4u + (uint32_t)sub;
         const uint32_t rr = fastdiv(q, A.per_rep, A.magic_rep);
@@ -66,18 +74,24 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
         Job jb;
         jb.t.r = (int)rr; jb.t.tx = (int)tx; jb.t.ty = (int)ty; jb.t.tz = (int)tz;
         const uint32_t base = rr * B * B * B;
-        auto idx = [&](uint32_t x, uint32_t y, uint32_t z) { return base + (z * B + y) * B + x; };
-        jb.self = idx(tx, ty, tz);
-        jb.xm = idx(tx == 0 ? B - 1 : tx - 1, ty, tz); jb.xp = idx(tx == B - 1 ? 0 : tx + 1, ty, tz);
-        jb.ym = idx(tx, ty == 0 ? B - 1 : ty - 1, tz); jb.yp = idx(tx, ty == B - 1 ? 0 : ty + 1, tz);
-        jb.zm = idx(tx, ty, tz == 0 ? B - 1 : tz - 1); jb.zp = idx(tx, ty, tz == B - 1 ? 0 : tz + 1);
+        auto rec = [&](uint32_t x, uint32_t y, uint32_t z) { return (base + (z * B + y) * B + x) * (uint32_t)kG3Rec; };
+        const uint32_t ulz = (uint32_t)lz;
+        jb.self = rec(tx, ty, tz);
+        jb.oxm = rec(tx == 0 ? B - 1 : tx - 1, ty, tz) + kG3X + 2u * ulz + 1u;     // left tile's XR
+        jb.oxp = rec(tx == B - 1 ? 0 : tx + 1, ty, tz) + kG3X + 2u * ulz;          // right tile's XL
+        jb.oym = rec(tx, ty == 0 ? B - 1 : ty - 1, tz) + kG3Y + ulz;               // tile in front: its YR
+        jb.oyp = rec(tx, ty == B - 1 ? 0 : ty + 1, tz) + kG3Y + ulz;               // tile behind: its YL
+        jb.oz = lz == 0 ? rec(tx, ty, tz == 0 ? B - 1 : tz - 1) + kG3ZR : rec(tx, ty, tz == B - 1 ? 0 : tz + 1) + kG3ZL;
+        const uint32_t z = tz * (uint32_t)kT3 + ulz;
+        jb.g = (z * B + ty) * B + tx;                                              // RNG block (S3.4)
+        jb.p_base = tx * 4u + (uint32_t)(A.L >> 1) * (ty * (uint32_t)kT3 + (uint32_t)A.L * z);
         return jb;
     };
     auto publish = [&](const Slice& s, uint32_t me, uint32_t ver) {
         uint32_t XL, XR, YL, YR;
         face_words(s.S, lz, XL, XR, YL, YR);
         const unsigned long long v = (unsigned long long)ver << 32;
-        unsigned long long* e = R.xedge + (size_t)me * kG3Rec;
+        unsigned long long* e = R.xedge + me;
         st_x64v2(e + kG3X + 2 * lz, v | XL, v | XR);
         st_x64(e + kG3Y + lz, v | (YL & 0xffu) | ((YR & 0xffu) << 8));
         if (lz == 0) st_x64v2(e + kG3ZL, v | s.S[0], v | s.S[1]);
@@ -85,11 +99,8 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
     };
     // wait until the six neighbours have published version `want`, and take the halos from their words
     auto refresh = [&](Slice& s, const Job& jb, uint32_t want) {
-        const unsigned long long* pxm = R.xedge + (size_t)jb.xm * kG3Rec + kG3X + 2 * lz + 1;     // left tile's XR
-        const unsigned long long* pxp = R.xedge + (size_t)jb.xp * kG3Rec + kG3X + 2 * lz;         // right tile's XL
-        const unsigned long long* pym = R.xedge + (size_t)jb.ym * kG3Rec + kG3Y + lz;             // tile in front: its YR
-        const unsigned long long* pyp = R.xedge + (size_t)jb.yp * kG3Rec + kG3Y + lz;             // tile behind: its YL
-        const unsigned long long* pz = lz == 0 ? R.xedge + (size_t)jb.zm * kG3Rec + kG3ZR : R.xedge + (size_t)jb.zp * kG3Rec + kG3ZL;
+        const unsigned long long *pxm = R.xedge + jb.oxm, *pxp = R.xedge + jb.oxp, *pym = R.xedge + jb.oym, *pyp = R.xedge + jb.oyp;
+        const unsigned long long* pz = R.xedge + jb.oz;
         const bool need_z = lz == 0 || lz == 7;
         for (;;) {
             const unsigned long long a = ld_x64(pxm), b = ld_x64(pxp), c = ld_x64(pym), d = ld_x64(pyp);
@@ -100,11 +111,9 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
                 ok = ok && (uint32_t)(z0 >> 32) == want && (uint32_t)(z1 >> 32) == want;
             }
             if (__all_sync(0xffffffffu, ok)) {
-                s.xl = (uint32_t)a; s.xr = (uint32_t)b;
-                s.ym = ((uint32_t)c >> 8) & 0xffu; s.yp = (uint32_t)d & 0xffu;
-                s.zm[0] = s.zm[1] = s.zp[0] = s.zp[1] = 0u;
-                if (lz == 0) { s.zm[0] = (uint32_t)z0; s.zm[1] = (uint32_t)z1; }
-                if (lz == 7) { s.zp[0] = (uint32_t)z0; s.zp[1] = (uint32_t)z1; }
+                s.x = (uint32_t)a | (uint32_t)b;
+                s.y = (((uint32_t)c >> 8) & 0xffu) | (((uint32_t)d & 0xffu) << 8);
+                s.zq[0] = (uint32_t)z0; s.zq[1] = (uint32_t)z1;          // zero unless lz is 0 or 7
                 return;
             }
         }
@@ -124,20 +133,23 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
         }
     };
     auto sm_slot = [&](int C, uint32_t m) { return ws + (size_t)((uint32_t)C * Mw + m) * (NSLOT * 32u); };
-    auto sm_job = [&](int C, uint32_t m) {                             // the constants parked by the prologue
+    // the constants parked by the prologue; the tile itself only where it is needed (couplings, series, write-back)
+    auto sm_job = [&](int C, uint32_t m, bool with_tile) {
         const uint32_t* p = sm_slot(C, m) + 64;
         Job jb;
-        jb.self = p[0]; jb.xm = p[32]; jb.xp = p[64]; jb.ym = p[96]; jb.yp = p[128]; jb.zm = p[160]; jb.zp = p[192];
-        const uint32_t xyz = p[224];
-        jb.t.tx = (int)(xyz & 0x3ffu); jb.t.ty = (int)((xyz >> 10) & 0x3ffu); jb.t.tz = (int)(xyz >> 20); jb.t.r = (int)p[256];
+        jb.self = p[0]; jb.oxm = p[32]; jb.oxp = p[64]; jb.oym = p[96]; jb.oyp = p[128]; jb.oz = p[160]; jb.g = p[192]; jb.p_base = p[224];
+        jb.t = Tile3{0, 0, 0, 0};
+        if (with_tile) {
+            const uint32_t xyz = p[256];
+            jb.t.tx = (int)(xyz & 0x3ffu); jb.t.ty = (int)((xyz >> 10) & 0x3ffu); jb.t.tz = (int)(xyz >> 20); jb.t.r = (int)p[288];
+        }
         return jb;
     };
     auto sm_put_job = [&](const Job& jb, int C, uint32_t m) {
         uint32_t* p = sm_slot(C, m) + 64;
-        p[0] = jb.self; p[32] = jb.xm; p[64] = jb.xp; p[96] = jb.ym; p[128] = jb.yp; p[160] = jb.zm; p[192] = jb.zp;
-        p[224] = (uint32_t)jb.t.tx | ((uint32_t)jb.t.ty << 10) | ((uint32_t)jb.t.tz << 20); p[256] = (uint32_t)jb.t.r;
+        p[0] = jb.self; p[32] = jb.oxm; p[64] = jb.oxp; p[96] = jb.oym; p[128] = jb.oyp; p[160] = jb.oz; p[192] = jb.g; p[224] = jb.p_base;
+        p[256] = (uint32_t)jb.t.tx | ((uint32_t)jb.t.ty << 10) | ((uint32_t)jb.t.tz << 20); p[288] = (uint32_t)jb.t.r;
     };
-
     // records -> shared memory; the colour-1 tiles publish their initial faces (version 1 = what phase 0 waits for)
     for (int C = 0; C < 2; ++C)
         for (uint32_t m = 0; m < Mw; ++m) {
@@ -159,24 +171,31 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
             for (uint32_t m = 0; m < Mw; ++m) {
                 const uint32_t job = wg + m * W;
                 if (job >= R.jobs_total) break;
-                const Job jb = sm_job(C, m);
+#if defined(ISING_JIT_R) && ISING_JIT_R == 1
+                const Job jb = sm_job(C, m, HASJ || series);
+                const uint64_t seed = A.seed0;
+#else
+                const Job jb = sm_job(C, m, true);
+                const uint64_t seed = A.seeds[jb.t.r];
+#endif
                 Slice s;
                 uint32_t* p = sm_slot(C, m);
                 s.S[0] = p[0]; s.S[1] = p[32];
                 load_couplings<HASJ>(A, jb.t, lz, s);
+                const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+                const uint32_t g = jb.g, p_base = jb.p_base;
+                const uint64_t t0 = A.t_first + (uint64_t)pass * (uint64_t)A.k;
+                // the random planes of the first half-sweep are drawn before the wait: the faces published a moment ago by
+                // the neighbours need about a microsecond to arrive, and all warps of an SM reach this point together
+                uint32_t drawn[kHeadBits];
+                if (HP3 != kNoSpec3) head_planes3(g, (uint32_t)(2 * t0), (uint32_t)((2 * t0) >> 32), k0, k1, drawn);
                 refresh(s, jb, ph + 1u);
                 if (series && C == 0 && pass > 0) account(s, jb.t.r, pass - 1);
-#if defined(ISING_JIT_R) && ISING_JIT_R == 1
-                const uint64_t seed = A.seed0;
-#else
-                const uint64_t seed = A.seeds[jb.t.r];
-#endif
-                const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
-                const uint32_t z = (uint32_t)(jb.t.tz * kT3 + lz);
-                const uint32_t g = (z * B + (uint32_t)jb.t.ty) * B + (uint32_t)jb.t.tx;
-                const uint32_t p_base = (uint32_t)(jb.t.tx * 4) + (uint32_t)(A.L >> 1) * ((uint32_t)(jb.t.ty * kT3) + (uint32_t)A.L * z);
-                for (int j = 0; j < A.k; ++j) {
-                    const uint64_t tt = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
+                half_sweep3<HP3, HASJ, HP3 != kNoSpec3>(A, s, 0, lz, g, p_base, 2 * t0, k0, k1, drawn);
+                half_sweep3<HP3, HASJ>(A, s, 1, lz, g, p_base, 2 * t0 + 1, k0, k1);
+#pragma unroll 1
+                for (int j = 1; j < A.k; ++j) {
+                    const uint64_t tt = t0 + (uint64_t)j;
                     half_sweep3<HP3, HASJ>(A, s, 0, lz, g, p_base, 2 * tt, k0, k1);
                     half_sweep3<HP3, HASJ>(A, s, 1, lz, g, p_base, 2 * tt + 1, k0, k1);
                 }
@@ -190,7 +209,7 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
         for (uint32_t m = 0; m < Mw; ++m) {
             const uint32_t job = wg + m * W;
             if (job >= R.jobs_total) break;
-            const Job jb = sm_job(0, m);
+            const Job jb = sm_job(0, m, true);
             Slice s;
             const uint32_t* p = sm_slot(0, m);
             s.S[0] = p[0]; s.S[1] = p[32];
@@ -202,7 +221,7 @@ __global__ void __launch_bounds__(128, 5) k_grid3d(Grid3Args R) {
         for (uint32_t m = 0; m < Mw; ++m) {
             const uint32_t job = wg + m * W;
             if (job >= R.jobs_total) break;
-            const Job jb = sm_job(C, m);
+            const Job jb = sm_job(C, m, true);
             Slice s;
             const uint32_t* p = sm_slot(C, m);
             s.S[0] = p[0]; s.S[1] = p[32];

@@ -196,10 +196,11 @@ cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3, int R) {
     return cached(kJitSource3d, expr, {R == 1 ? "-DISING_JIT_R=1" : "-DISING_JIT_R=0"});
 }
 
-cudaKernel_t grid3d_jit_kernel(bool bits, unsigned long long hp3, int R) {
+cudaKernel_t grid3d_jit_kernel(bool bits, unsigned long long hp3, int R, int threads, int blocks) {
     char expr[160];
     snprintf(expr, sizeof expr, "ising::jit::k_grid3d<%s, false, %lluull>", bits ? "true" : "false", hp3);
-    return cached(kJitSource3d, expr, {R == 1 ? "-DISING_JIT_R=1" : "-DISING_JIT_R=0"});
+    return cached(kJitSource3d, expr, {R == 1 ? "-DISING_JIT_R=1" : "-DISING_JIT_R=0", "-DISING_G3_THREADS=" + std::to_string(threads),
+                                       "-DISING_G3_BLOCKS=" + std::to_string(blocks)});
 }
 
 uint64_t planes_jit_compiled() { return state().compiled; }

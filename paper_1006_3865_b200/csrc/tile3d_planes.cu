@@ -468,12 +468,10 @@ __global__ void __launch_bounds__(kRes3Warps * 32) k_resident3d(Res3Args R) {
         if (lz == 7) *reinterpret_cast<uint2*>(f + kZR) = make_uint2(s.S[0], s.S[1]);
     };
     auto refresh = [&](const Nb& nb, Slice& s) {
-        s.xl = reinterpret_cast<const uint32_t*>(nb.xm + kXR)[lz];
-        s.xr = reinterpret_cast<const uint32_t*>(nb.xp + kXL)[lz];
-        s.ym = nb.ym[kYR + lz];
-        s.yp = nb.yp[kYL + lz];
-        if (lz == 0) { const uint2 w = *reinterpret_cast<const uint2*>(nb.zm + kZR); s.zm[0] = w.x; s.zm[1] = w.y; }
-        if (lz == 7) { const uint2 w = *reinterpret_cast<const uint2*>(nb.zp + kZL); s.zp[0] = w.x; s.zp[1] = w.y; }
+        s.x = reinterpret_cast<const uint32_t*>(nb.xm + kXR)[lz] | reinterpret_cast<const uint32_t*>(nb.xp + kXL)[lz];
+        s.y = (uint32_t)nb.ym[kYR + lz] | ((uint32_t)nb.yp[kYL + lz] << 8);
+        if (lz == 0) { const uint2 w = *reinterpret_cast<const uint2*>(nb.zm + kZR); s.zq[0] = w.x; s.zq[1] = w.y; }
+        if (lz == 7) { const uint2 w = *reinterpret_cast<const uint2*>(nb.zp + kZL); s.zq[0] = w.x; s.zq[1] = w.y; }
     };
 
     const bool mine = wg < JC;
@@ -651,26 +649,43 @@ bool grid3d_supported(const ising_ctx* h, int T) {
 }
 
 namespace {
+// One cooperative launch with M = 1 or 2 jobs of each colour per warp.  The run-time build (bits/hp3 given) is compiled
+// for the CTA shape the lattice wants: ONE CTA per SM with ceil(warps / SMs) warps, rounded up to a multiple of four, so
+// that every SM and every scheduler carries the same number of jobs (config 4: 4096 jobs per colour = 28 warps on each
+// SM, one job per warp, 72 registers).  Measured on config 4, k = 1 / 4 / 16: 5 CTAs of 4 warps with two jobs per warp
+// 1684 / - / -; 4 CTAs of 7 warps 1917 / 2338 / 2382; 7 CTAs of 4 warps 1855 / 2201 / 2269; one CTA of 28 warps
+// 1967 / 2713 / 3030 flips/ns.  The pre-compiled kernels keep their fixed shape (CTAs of up to 4 warps, 5 per SM).
 template <bool BITS, bool HASJ>
-int launch_grid3d_one(Grid3Args& R, cudaKernel_t spec, bool* fits) {
+int launch_grid3d_one(Grid3Args& R, bool want_jit, unsigned long long hp3, int reps, bool* fits, bool* used_jit) {
     int dev = 0, sms = 0;
     ISING_CUDA_OK(cudaGetDevice(&dev));
     ISING_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    const void* fn = spec ? (const void*)spec : (const void*)k_grid3d<BITS, HASJ>;
-    if (spec) ISING_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    else if (int rc = set_max_dynamic_smem<k_grid3d<BITS, HASJ>>(200 * 1024)) return rc;
-    *fits = false;
+    *fits = false; *used_jit = false;
     static const uint32_t warp_cap = getenv("ISING_GRID_WARPS") ? (uint32_t)atoi(getenv("ISING_GRID_WARPS")) : 0u;   // testing aid
+    static const uint32_t wsm_cap = getenv("ISING_G3_WSM") ? (uint32_t)atoi(getenv("ISING_G3_WSM")) : 28u;   // 28 warps: 72 registers each
     const uint32_t max_m = warp_cap ? 16u : 2u;              // as in launch_grid_planes: beyond two jobs per warp the per-pass kernels win
     for (uint32_t M = 1; M <= max_m; ++M) {
         const uint32_t warps_needed = (R.jobs_total + M - 1) / M;
-        const int wpb = warps_needed <= (uint32_t)sms * 4u ? 1 : (warps_needed <= (uint32_t)sms * 8u ? 2 : 4);
-        const size_t smem = (size_t)wpb * 2u * M * (2u + 9u) * 32u * sizeof(uint32_t);      // words + constants of every job
+        if (warp_cap && warps_needed > warp_cap && M < 16u) continue;
+        const uint32_t w_sm = (warps_needed + (uint32_t)sms - 1) / (uint32_t)sms;
+        int wpb, bps;
+        const void* fn = nullptr;
+        if (want_jit && !HASJ && w_sm <= wsm_cap) {
+            wpb = (int)((w_sm + 3u) / 4u * 4u); bps = 1;         // one CTA per SM, the same number of warps on every scheduler
+            fn = (const void*)grid3d_jit_kernel(BITS, hp3, reps, wpb * 32, bps);
+        }
+        if (fn) *used_jit = true;
+        else {
+            fn = (const void*)k_grid3d<BITS, HASJ>;
+            wpb = warps_needed <= (uint32_t)sms * 4u ? 1 : (warps_needed <= (uint32_t)sms * 8u ? 2 : 4);
+            *used_jit = false;
+        }
+        ISING_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        const size_t smem = (size_t)wpb * 2u * M * (size_t)kG3Slots * 32u * sizeof(uint32_t);    // words + constants of every job
         int occ = 0;
         ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, wpb * 32, smem));
         const uint32_t grid = (warps_needed + wpb - 1) / wpb;
         if (grid > (uint32_t)sms * (uint32_t)occ) continue;      // not co-resident: more jobs per warp
-        if (warp_cap && warps_needed > warp_cap && M < 16u) continue;
         R.jobs_per_warp = M;
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(grid); cfg.blockDim = dim3(wpb * 32); cfg.dynamicSmemBytes = smem; cfg.stream = hooks().stream;
@@ -708,14 +723,14 @@ int launch_grid3d(ising_ctx* h, const Accept& acc, bool bits, int n, int k, uint
     if (series) ISING_CUDA_OK(cudaMemsetAsync(d_acc, 0, grid3d_acc_bytes(h, n), st));
     const unsigned long long hp3 = ((unsigned long long)(acc.thr[0] >> kTailBits) << 24) |
                                    ((unsigned long long)(acc.thr[1] >> kTailBits) << 12) | (unsigned long long)(acc.thr[2] >> kTailBits);
-    cudaKernel_t spec = (use_jit && !A.force && !A.jrec) ? grid3d_jit_kernel(bits, hp3, h->R) : nullptr;
-    bool fits = false;
+    const bool want_jit = use_jit && !A.force && !A.jrec;
+    bool fits = false, used_jit = false;
     int rc;
-    if (A.jrec) rc = bits ? launch_grid3d_one<true, true>(R, nullptr, &fits) : launch_grid3d_one<false, true>(R, nullptr, &fits);
-    else rc = bits ? launch_grid3d_one<true, false>(R, spec, &fits) : launch_grid3d_one<false, false>(R, spec, &fits);
+    if (A.jrec) rc = bits ? launch_grid3d_one<true, true>(R, false, hp3, h->R, &fits, &used_jit) : launch_grid3d_one<false, true>(R, false, hp3, h->R, &fits, &used_jit);
+    else rc = bits ? launch_grid3d_one<true, false>(R, want_jit, hp3, h->R, &fits, &used_jit) : launch_grid3d_one<false, false>(R, want_jit, hp3, h->R, &fits, &used_jit);
     if (rc) return rc;
     if (!fits) return 1;
-    h->last_jit = spec ? 1 : 0;
+    h->last_jit = used_jit ? 1 : 0;
     if (series) {
         const uint32_t count = (uint32_t)n * (uint32_t)h->R;
         k_grid3d_series_finish<<<(count + 255) / 256, 256, 0, st>>>((const long long*)d_acc, d_E, d_M, count, (long long)h->N);

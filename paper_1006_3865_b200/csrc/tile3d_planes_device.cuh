@@ -59,9 +59,9 @@ __device__ __forceinline__ Tile3 job_tile3(const Plane3Args& A, uint32_t q) {
 // What a lane keeps of its slice.
 struct Slice {
     uint32_t S[2];        // the slice's two colour words
-    uint32_t xl, xr;      // halo bits x = -1 (at 4ly) and x = 8 (at 4ly+3), every row, either colour
-    uint32_t ym, yp;      // halo row y = -1 and y = 8: colour 0 pairs in bits 0-3, colour 1 in bits 4-7
-    uint32_t zm[2], zp[2];// lanes lz = 0 / 7: the slice below / above, by colour
+    uint32_t x;           // halo bits x = -1 (at 4ly) and x = 8 (at 4ly+3), every row, either colour
+    uint32_t y;           // halo rows y = -1 (bits 0-7) and y = 8 (bits 8-15): colour 0 pairs in the low nibble, colour 1 in the high
+    uint32_t zq[2];       // lanes lz = 0 / 7: the slice below / above, by colour (no lane is both)
     uint32_t J[2][6];     // coupling words of the slice's two colours (kernels with HASJ only)
 };
 
@@ -98,18 +98,18 @@ __device__ __forceinline__ void load_slice(const Plane3Args& A, const Tile3& t, 
         s.S[0] = pack16(pack16(0u, v[1]), v[0]);
         s.S[1] = pack16(pack16(0u, v[3]), v[2]);
     }
-    s.xl = ldh32(fXm + kXR + 4 * lz);     // left tile's x = 7 sites, bit 4ly
-    s.xr = ldh32(fXp + kXL + 4 * lz);     // right tile's x = 0 sites, bit 4ly+3
-    s.ym = ldh8(fYm + kYR + lz);                                        // tile in front: its row y = 7
-    s.yp = ldh8(fYp + kYL + lz);                                        // tile behind: its row y = 0
-    s.zm[0] = s.zm[1] = s.zp[0] = s.zp[1] = 0u;
+    s.x = ldh32(fXm + kXR + 4 * lz) |     // left tile's x = 7 sites, bit 4ly
+          ldh32(fXp + kXL + 4 * lz);      // right tile's x = 0 sites, bit 4ly+3
+    s.y = ldh8(fYm + kYR + lz) |                                        // tile in front: its row y = 7
+          (ldh8(fYp + kYL + lz) << 8);                                  // tile behind: its row y = 0
+    s.zq[0] = s.zq[1] = 0u;
     if (lz == 0) {
         const uint2 w = ldh64(rec_of(t.tz == 0 ? B - 1 : t.tz - 1, t.ty, t.tx) + BODY + kZR);
-        s.zm[0] = w.x; s.zm[1] = w.y;
+        s.zq[0] = w.x; s.zq[1] = w.y;
     }
     if (lz == 7) {
         const uint2 w = ldh64(rec_of(t.tz == B - 1 ? 0 : t.tz + 1, t.ty, t.tx) + BODY + kZL);
-        s.zp[0] = w.x; s.zp[1] = w.y;
+        s.zq[0] = w.x; s.zq[1] = w.y;
     }
 }
 
@@ -257,16 +257,18 @@ __device__ __forceinline__ void ne3_from(const uint32_t (&p)[kHeadBits], const u
         ne = lop3<lut_ne_pair3(u, u)>(ne, p[PEND >= 0 ? PEND : 0], p[PEND >= 0 ? PEND : 0]);
     }
 }
-template <unsigned long long HP3>
-__device__ __forceinline__ void head_masks3_sel(uint32_t g, uint32_t Hlo, uint32_t Hhi, uint32_t k0, uint32_t k1, uint32_t s0,
-                                                uint32_t s1, uint32_t& R, uint32_t& eq) {
+// the twelve head planes of block g at half-sweep H (S3.4): they do not depend on the spins, so k_grid3d draws those of a
+// job's first half-sweep while the neighbours' faces are still on their way
+__device__ __forceinline__ void head_planes3(uint32_t g, uint32_t Hlo, uint32_t Hhi, uint32_t k0, uint32_t k1, uint32_t (&p)[kHeadBits]) {
     static_assert(kHeadBits == 12, "three Philox calls");
-    uint32_t p[kHeadBits];
 #pragma unroll
     for (int n = 0; n < 3; ++n) {
         const u32x4 o = philox4x32_10(g, kTagPlanes + 256u * n, Hlo, Hhi, k0, k1);
         p[4 * n] = o.x; p[4 * n + 1] = o.y; p[4 * n + 2] = o.z; p[4 * n + 3] = o.w;
     }
+}
+template <unsigned long long HP3>
+__device__ __forceinline__ void head_masks3_sel(const uint32_t (&p)[kHeadBits], uint32_t s0, uint32_t s1, uint32_t& R, uint32_t& eq) {
     const uint32_t mask[3] = {s0, s1, s0 | s1};
     uint32_t bw = 0, ne = 0;
     chain3_from<HP3, kHeadBits - 1>(p, mask, bw);
@@ -282,14 +284,14 @@ __device__ __forceinline__ void neighbour_words3(const Slice& s, int c, int lz, 
     O = s.S[o];
     Zm = __shfl_up_sync(0xffffffffu, O, 1);
     Zp = __shfl_down_sync(0xffffffffu, O, 1);
-    if (lz == 0) Zm = s.zm[o];
-    if (lz == 7) Zp = s.zp[o];
-    Ym = (O << 4) | ((s.ym >> (4 * o)) & 0xfu);
-    Yp = (O >> 4) | (((s.yp >> (4 * o)) & 0xfu) << 28);
+    if (lz == 0) Zm = s.zq[o];
+    if (lz == 7) Zp = s.zq[o];
+    Ym = (O << 4) | ((s.y >> (4 * o)) & 0xfu);
+    Yp = (O >> 4) | (((s.y >> (8 + 4 * o)) & 0xfu) << 28);
     // rows where the active site is the left one of its pair (x = 2 p_x): ly = lz + c (mod 2); their second
     // x-neighbour is pair p_x - 1, the other rows' is pair p_x + 1
     const uint32_t m = ((lz + c) & 1) ? 0xf0f0f0f0u : 0x0f0f0f0fu;
-    X2 = ((((O << 1) & 0xeeeeeeeeu) | s.xl) & m) | ((((O >> 1) & 0x77777777u) | s.xr) & ~m);
+    X2 = ((((O << 1) & 0xeeeeeeeeu) | (s.x & 0x11111111u)) & m) | ((((O >> 1) & 0x77777777u) | (s.x & 0x88888888u)) & ~m);
 }
 
 // a10 on a slice held in registers: #up spins of both colours and #unsatisfied bonds seen from the colour-0 sites (every
@@ -305,9 +307,10 @@ __device__ __forceinline__ void count_slice(const Slice& s, int lz, int& up, int
 }
 
 // One half-sweep of colour c on the lane's slice (a4-a5, 6 neighbours).
-template <unsigned long long HP3 = kNoSpec3, bool HASJ = false>
+// DRAWN: p holds the head planes of (g, H) already (specialised kernels only); otherwise p is scratch.
+template <unsigned long long HP3, bool HASJ, bool DRAWN>
 __device__ __forceinline__ void half_sweep3(const Plane3Args& A, Slice& s, int c, int lz, uint32_t g, uint32_t p_base,
-                                            uint64_t H, uint32_t k0, uint32_t k1) {
+                                            uint64_t H, uint32_t k0, uint32_t k1, uint32_t (&p)[kHeadBits]) {
     const uint32_t Hlo = (uint32_t)H, Hhi = (uint32_t)(H >> 32);
     const uint32_t S = s.S[c];
     uint32_t Zm, Zp, Ym, Yp, O, X2;
@@ -324,7 +327,8 @@ __device__ __forceinline__ void half_sweep3(const Plane3Args& A, Slice& s, int c
     if (HP3 != kNoSpec3) {
         const uint32_t s0 = ~ge1, s1 = ge1 & ~ge2;                  // no / exactly one unsatisfied bond
         uint32_t R, eq;
-        head_masks3_sel<HP3>(g, Hlo, Hhi, k0, k1, s0, s1, R, eq);
+        if (!DRAWN) head_planes3(g, Hlo, Hhi, k0, k1, p);
+        head_masks3_sel<HP3>(p, s0, s1, R, eq);
         uint32_t und = eq & ~ge3;
         while (und) {                                               // probability 2^-12 per site
             const int j = __ffs(und) - 1;
@@ -354,7 +358,14 @@ __device__ __forceinline__ void half_sweep3(const Plane3Args& A, Slice& s, int c
     s.S[c] = S ^ flip;
 }
 
-constexpr int kThreads3 = 64;        // 2 warps = 8 tiles per CTA: small CTAs so that config 4 (4096 warp jobs) fits one wave
+template <unsigned long long HP3 = kNoSpec3, bool HASJ = false>
+__device__ __forceinline__ void half_sweep3(const Plane3Args& A, Slice& s, int c, int lz, uint32_t g, uint32_t p_base,
+                                            uint64_t H, uint32_t k0, uint32_t k1) {
+    uint32_t p[kHeadBits];
+    half_sweep3<HP3, HASJ, false>(A, s, c, lz, g, p_base, H, k0, k1, p);
+}
+
+constexpr int kThreads3 = 64;        // 2 warps = 8 tiles per CTA (measured at L = 256 .. 512, k = 1 .. 16: 64 = 128 > 256 > 512 threads)
 
 template <bool BITS, unsigned long long HP3 = kNoSpec3, bool HASJ = false>
 __global__ void __launch_bounds__(kThreads3) k_tile3d_planes(Plane3Args A) {
