@@ -79,18 +79,31 @@ __device__ __forceinline__ void half_sweep_masks(const PlaneArgs& A, TileRegs<T>
     for (int gx = 0; gx < G::NW; ++gx) t.S[c][gx] = Snew[gx];
 }
 
+// CTA shape: the pre-compiled kernels take up to 128 threads, 5 CTAs per SM; the run-time build names its own (launch_grid_one)
+#ifndef ISING_G2_THREADS
+#define ISING_G2_THREADS 128
+#define ISING_G2_BLOCKS 5
+#endif
+// ISING_G2_PARK = 0 (run-time build only): the jobs' constants are not parked beside their words but decoded again in every
+// phase (a dozen instructions with the geometry known at compile time), so that shared memory holds nothing but spins:
+// 28 warps x 16 jobs x 512 bytes = 229376 of the 232448 bytes of an SM hold a 16384^2 lattice on the 148 SMs of a B200.
+#ifndef ISING_G2_PARK
+#define ISING_G2_PARK 1
+#endif
+
 template <int T, bool BITS, bool HASJ, uint32_t HP = kNoSpec, bool PC = false>
-__global__ void __launch_bounds__(PC ? 256 : 128, PC ? 2 : 5) k_grid_planes(GridArgs R) {
+__global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2_BLOCKS) k_grid_planes(GridArgs R) {
     using G = PG<T>;
     constexpr int NWORDS = 2 * G::NW;                         // words per lane and job: S[cc][gx]
-    constexpr int NSLOT = NWORDS + 7;                         // ... + the job's constants (decoded once): self, nU, nD, nL, nR, tx | ty << 16, r
+    constexpr bool PARK = PC || ISING_G2_PARK;
+    constexpr int NSLOT = NWORDS + (PARK ? 7 : 0);            // ... + the job's constants (decoded once): self, nU, nD, nL, nR, tx | ty << 16, r
     extern __shared__ uint32_t grid_smem[];                   // per warp: [colour][job][slot][lane]
     const PlaneArgs& A = R.P;
     const int lane = threadIdx.x & 31;
     const int wic = threadIdx.x >> 5;
     const uint32_t wg = PC ? blockIdx.x : blockIdx.x * (blockDim.x >> 5) + (uint32_t)wic, W = PC ? gridDim.x : gridDim.x * (blockDim.x >> 5);
     const int sub = lane / G::LPT, Y = lane % G::LPT;
-    const uint32_t B = (uint32_t)A.B, hb = B >> 1, per_rep = R.tiles_per_colour;
+    const uint32_t B = geom_B(A);
     const uint32_t Mw = PC ? 1u : R.jobs_per_warp;
     uint32_t* const ws = grid_smem + (PC ? 0u : (size_t)wic * (2u * Mw * NSLOT * 32u)) + lane;
     // PC: behind the consumer's area, the ring [slot][R1 | R2][gx][lane], its "full" words and the consumed counter
@@ -102,9 +115,9 @@ __global__ void __launch_bounds__(PC ? 256 : 128, PC ? 2 : 5) k_grid_planes(Grid
 
     struct Job { int r, tx, ty; uint32_t self, nU, nD, nL, nR; };
     auto decode = [&](uint32_t job, int C) {
-        const uint32_t q = job * G::TPW + (uint32_t)sub;
-        const uint32_t r = fastdiv(q, per_rep, A.magic_rep), qq = q - r * per_rep;
-        const uint32_t ty = fastdiv(qq, hb, A.magic_hb), tx = 2u * (qq - ty * hb) + ((ty + (uint32_t)C) & 1u);
+        int ri, txi, tyi;
+        job_tile<T>(A, job, sub, ri, txi, tyi, C);
+        const uint32_t r = (uint32_t)ri, tx = (uint32_t)txi, ty = (uint32_t)tyi;
         const uint32_t base = r * B * B, row = base + ty * B;
         const uint32_t tyU = ty == 0 ? B - 1 : ty - 1, tyD = ty == B - 1 ? 0 : ty + 1;
         const uint32_t txL = tx == 0 ? B - 1 : tx - 1, txR = tx == B - 1 ? 0 : tx + 1;
@@ -185,11 +198,13 @@ __global__ void __launch_bounds__(PC ? 256 : 128, PC ? 2 : 5) k_grid_planes(Grid
         }
     };
     auto sm_job = [&](int C, uint32_t m) {                             // the constants parked by the prologue
+        if (!PARK) return decode(wg + m * W, C);
         const uint32_t* p = ws + (size_t)((uint32_t)C * Mw + m) * (NSLOT * 32u) + NWORDS * 32;
         const uint32_t xy = p[5 * 32];
         return Job{(int)p[6 * 32], (int)(xy & 0xffffu), (int)(xy >> 16), p[0], p[1 * 32], p[2 * 32], p[3 * 32], p[4 * 32]};
     };
     auto sm_put_job = [&](const Job& jb, int C, uint32_t m) {
+        if (!PARK) return;
         uint32_t* p = ws + (size_t)((uint32_t)C * Mw + m) * (NSLOT * 32u) + NWORDS * 32;
         p[0] = jb.self; p[1 * 32] = jb.nU; p[2 * 32] = jb.nD; p[3 * 32] = jb.nL; p[4 * 32] = jb.nR;
         p[5 * 32] = (uint32_t)jb.tx | ((uint32_t)jb.ty << 16); p[6 * 32] = (uint32_t)jb.r;
@@ -278,6 +293,8 @@ __global__ void __launch_bounds__(PC ? 256 : 128, PC ? 2 : 5) k_grid_planes(Grid
     for (int pass = 0; pass < R.n; ++pass) {
         for (int C = 0; C < 2; ++C) {
             const uint32_t ph = 2u * (uint32_t)pass + (uint32_t)C;       // this phase waits for version ph + 1 and publishes ph + 2
+            // (Starting each phase one band of jobs later, so that no job waits for the end of the phase before, was
+            // measured: no gain at tile 32, -8 % at tile 64 where the extra state spills.)
 #pragma unroll 1
             for (uint32_t m = 0; m < Mw; ++m) {
                 const uint32_t job = wg + m * W;
@@ -289,7 +306,11 @@ __global__ void __launch_bounds__(PC ? 256 : 128, PC ? 2 : 5) k_grid_planes(Grid
                 jwords(jb, Jw);
                 refresh(tt, jb, ph + 1u);
                 if (series && C == 0 && pass > 0) account(tt, Jw, jb.r, pass - 1);     // colour-0 tiles: the halos of the finished pass just arrived
+#if defined(ISING_JIT_R) && ISING_JIT_R == 1
+                const uint64_t seed = A.seed0;
+#else
                 const uint64_t seed = A.seeds[jb.r];
+#endif
                 const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
                 const uint32_t Yg = (uint32_t)(jb.ty * G::LPT + Y);
                 const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(jb.tx * G::NW);

@@ -680,7 +680,7 @@ int launch_grid3d_one(Grid3Args& R, bool want_jit, unsigned long long hp3, int r
             wpb = warps_needed <= (uint32_t)sms * 4u ? 1 : (warps_needed <= (uint32_t)sms * 8u ? 2 : 4);
             *used_jit = false;
         }
-        ISING_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        ISING_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         const size_t smem = (size_t)wpb * 2u * M * (size_t)kG3Slots * 32u * sizeof(uint32_t);    // words + constants of every job
         int occ = 0;
         ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, wpb * 32, smem));

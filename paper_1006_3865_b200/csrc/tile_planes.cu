@@ -997,27 +997,55 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit, bool 
             return 0;
         }
     }
-    // specialised on the threshold head bits (planes_jit.cu) when asked for and available
-    cudaKernel_t spec = (use_jit && !R.P.force) ? grid_jit_kernel(T, BITS, HASJ, R.P.hp) : nullptr;
-    const void* fn = spec ? (const void*)spec : (const void*)k_grid_planes<T, BITS, HASJ>;
-    *used_jit = spec != nullptr;
-    if (spec) ISING_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-    else if (int rc = set_max_dynamic_smem<k_grid_planes<T, BITS, HASJ>>(200 * 1024)) return rc;
-    *fits = false;
+    // Specialised on the threshold head bits (planes_jit.cu) when asked for and available; that build also takes the CTA
+    // shape the lattice wants: ONE CTA per SM with ceil(warps / SMs) warps, rounded up to a multiple of four, so that every
+    // SM and every scheduler carries the same number of jobs (as launch_grid3d_one, measured there).
+    *fits = false; *used_jit = false;
     static const uint32_t warp_cap = getenv("ISING_GRID_WARPS") ? (uint32_t)atoi(getenv("ISING_GRID_WARPS")) : 0u;   // testing aid: several jobs per warp on small lattices
-    // measured: with more than two jobs of a colour per warp (L = 8192 and up) the per-pass kernels win
-    const uint32_t max_m = warp_cap ? kGridMaxJobsPerWarp : 2u;
+    static const uint32_t wsm_cap = getenv("ISING_G2_WSM") ? (uint32_t)atoi(getenv("ISING_G2_WSM")) : 28u;        // 28 warps: 72 registers each
+    static const int park_mode = getenv("ISING_G2_PARK") ? atoi(getenv("ISING_G2_PARK")) : -1;                  // testing aid: 0 = never park the constants
+    bool shaped = use_jit && !R.P.force;
+    // The pre-compiled kernel (fixed shape) loses to the per-pass kernels beyond two jobs of a colour per warp (BASELINE.md
+    // 5.1, round 2); the shaped run-time build keeps winning (L = 8192, tile 64, k = 1 / 4 / 16: 2895 / 3303 / 3455 against
+    // 2313 / 3019 / 3334 flips/ns), but a call must be long enough to pay for loading and storing the lattice once (n k >= 8
+    // beyond two jobs per warp), and with 8 or 16 jobs per warp (L = 16384: all of the shared memory of the GPU holds spins)
+    // its 28 warps per SM lose to the 40 of the per-pass kernels where those are not HBM-bound: int8 records at k = 1 only
+    // (2776 against 2486 flips/ns at tile 64, 2416 against 2100 at tile 32; bits 2925 against 2942; k = 4: 3150 against 3233).
+    const uint32_t max_m = kGridMaxJobsPerWarp;
+    constexpr size_t kSmemMax = 227 * 1024;
     for (uint32_t M = 1; M <= max_m; ++M) {
         const uint32_t warps_needed = (R.jobs_total + M - 1) / M;
-        // few jobs: one warp per CTA, so that the CTAs (and the schedulers they land on) spread over all SMs
-        const int wpb = warps_needed <= (uint32_t)sms * 4u ? 1 : (warps_needed <= (uint32_t)sms * 8u ? 2 : 4);
-        const size_t smem = (size_t)wpb * 2u * M * (2u * PG<T>::NW + 7u) * 32u * sizeof(uint32_t);     // words + constants of every job
-        if (smem > 200 * 1024) break;
+        if (warp_cap && warps_needed > warp_cap && M < kGridMaxJobsPerWarp) continue;
+        if (M > 2 && !warp_cap) {
+            if ((uint64_t)R.n * (uint64_t)R.P.k < 8u) break;
+            if (M > 4 && (R.P.k != 1 || BITS)) break;             // measured at L = 16384: only int8 at k = 1 gains
+        }
+        const uint32_t w_sm = (warps_needed + (uint32_t)sms - 1) / (uint32_t)sms;
+        int wpb = 0;
+        bool park = true;
+        const void* fn = nullptr;
+        const size_t lane_bytes = 32u * sizeof(uint32_t);
+        if (shaped) {
+            if (w_sm > wsm_cap) continue;                         // more jobs per warp
+            wpb = (int)((w_sm + 3u) / 4u * 4u);
+            park = park_mode != 0 && (size_t)wpb * 2u * M * (2u * PG<T>::NW + 7u) * lane_bytes <= kSmemMax;
+            if (!park && (size_t)wpb * 2u * M * (2u * PG<T>::NW) * lane_bytes > kSmemMax) break;      // the lattice does not fit on chip
+            fn = (const void*)grid_jit_kernel(T, BITS, HASJ, R.P.hp, R.P.B, R.P.R, wpb * 32, 1, park);
+            if (!fn) { shaped = false; M = 0; continue; }         // no run-time compiler: again with the pre-compiled kernel
+            *used_jit = true;
+        } else {
+            if (M > 2 && !warp_cap) break;
+            fn = (const void*)k_grid_planes<T, BITS, HASJ>;
+            // few jobs: one warp per CTA, so that the CTAs (and the schedulers they land on) spread over all SMs
+            wpb = warps_needed <= (uint32_t)sms * 4u ? 1 : (warps_needed <= (uint32_t)sms * 8u ? 2 : 4);
+        }
+        const size_t smem = (size_t)wpb * 2u * M * (2u * PG<T>::NW + (park ? 7u : 0u)) * lane_bytes;     // words (+ constants) of every job
+        if (smem > kSmemMax) break;
+        ISING_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax));
         int occ = 0;
         ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, wpb * 32, smem));
         const uint32_t grid = (warps_needed + wpb - 1) / wpb;
         if (grid > (uint32_t)sms * (uint32_t)occ) continue;      // not co-resident: more jobs per warp
-        if (warp_cap && warps_needed > warp_cap && M < kGridMaxJobsPerWarp) continue;
         R.jobs_per_warp = M;
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(grid); cfg.blockDim = dim3(wpb * 32); cfg.dynamicSmemBytes = smem; cfg.stream = hooks().stream;
@@ -1099,7 +1127,8 @@ int launch_flow_one(FlowArgs& F, bool use_jit, bool* used_jit, int stage_mode) {
     int dev = 0, sms = 0;
     ISING_CUDA_OK(cudaGetDevice(&dev));
     ISING_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-    const uint32_t warps = kPlaneThreads / 32;
+    const int threads = kPlaneThreads;       // measured on config 3: 128 x 10 CTAs per SM 2485 / 2100 flips/ns (tile 64 / 32); 256 x 5 2463 / 2092; 320 x 4 2450 / 2088; 640 x 2 2416 / 2057; 1024 x 1 2340 / 1788
+    const uint32_t warps = threads / 32;
     // TMA staging of the next job's bodies: only where a tile's previous write-back is certainly older than anything this
     // grid still has in flight (a phase of more than 2 x the resident warps), and never with coupling records (kept simple)
     const uint32_t resident_max = (uint32_t)sms * 16u * warps;
@@ -1111,12 +1140,12 @@ int launch_flow_one(FlowArgs& F, bool use_jit, bool* used_jit, int stage_mode) {
                    : staged ? (const void*)k_flow_planes_staged<T, BITS, false, kNoSpec, NS>
                    : (A.jrec ? (const void*)k_flow_planes<T, BITS, true, kNoSpec, NS> : (const void*)k_flow_planes<T, BITS, false, kNoSpec, NS>);
     int occ = 0;
-    ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, kPlaneThreads, smem));
+    ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, threads, smem));
     if (occ < 1) { set_error("k_flow_planes does not fit an SM"); return ISING_ECUDA; }
     uint32_t grid = (uint32_t)sms * (uint32_t)occ;
     grid = std::min<uint32_t>(grid, (F.jobs_per_phase + warps - 1) / warps);
     cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(kPlaneThreads); cfg.dynamicSmemBytes = smem; cfg.stream = hooks().stream;
+    cfg.gridDim = dim3(grid); cfg.blockDim = dim3(threads); cfg.dynamicSmemBytes = smem; cfg.stream = hooks().stream;
     void* args[] = {&F};
     ISING_CUDA_OK(cudaLaunchKernelExC(&cfg, fn, args));
     count_launch();

@@ -165,10 +165,13 @@ def test_config3_full_length_int8_equals_bits(P, orc, tile, k):
     sb = torch.empty(L * L, dtype=torch.int8, device="cuda")
     done = 0
     for p in (2, 50, n):
-        a.sweep(BC2, p - done, tile, k); b.sweep(BC2, p - done, tile, k)
+        n_call = p - done
+        a.sweep(BC2, n_call, tile, k); b.sweep(BC2, n_call, tile, k)
         done = p
-        # int8 records at k = 1: the persistent data-flow kernel, else a launch per colour
-        assert a.sweep_path() == ("flow_planes_i8" if k == 1 else "tile_planes_i8") and b.sweep_path() == "tile_planes_bits"
+        # int8 records at k = 1: the whole lattice on chip (a call of 8 passes or more), else the persistent data-flow
+        # kernel; k > 1 and bit records: a launch per colour
+        want = "tile_planes_i8" if k > 1 else ("grid_planes_i8" if n_call >= 8 else "flow_planes_i8")
+        assert a.sweep_path() == want and b.sweep_path() == "tile_planes_bits"
         assert a.last_sweep_specialized() and b.last_sweep_specialized()
         a.copy_spins(sa); b.copy_spins(sb)
         assert torch.equal(sa, sb), f"int8 and bit records differ after pass {p}"
@@ -185,13 +188,20 @@ def test_config3_full_length_int8_equals_bits(P, orc, tile, k):
         c.copy_spins(sb)
         assert torch.equal(sa, sb), "pre-compiled and run-time specialised kernels differ after 200 passes"
         c.destroy()
-        d = P.Ising(2, L, seed=3)                           # ... and so does a launch per colour (no data-flow kernel)
-        d.force_path(3)
+        d = P.Ising(2, L, seed=3)                           # ... and so do a launch per colour
+        d.force_path(2)
         d.sweep(BC2, n, tile, k)
         assert d.sweep_path() == "tile_planes_i8"
         d.copy_spins(sb)
-        assert torch.equal(sa, sb), "data-flow kernel and per-colour launches differ after 200 passes"
+        assert torch.equal(sa, sb), "on-chip kernel and per-colour launches differ after 200 passes"
         d.destroy()
+        e = P.Ising(2, L, seed=3)                           # ... and the data-flow kernel
+        e.force_path(4)
+        e.sweep(BC2, n, tile, k)
+        assert e.sweep_path() == "flow_planes_i8"
+        e.copy_spins(sb)
+        assert torch.equal(sa, sb), "on-chip and data-flow kernels differ after 200 passes"
+        e.destroy()
     a.destroy(); b.destroy()
 
 
