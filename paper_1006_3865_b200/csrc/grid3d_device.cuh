@@ -46,6 +46,10 @@ __device__ __forceinline__ void st_x64v2(unsigned long long* p, unsigned long lo
 #define ISING_G3_THREADS 128
 #define ISING_G3_BLOCKS 5
 #endif
+// ISING_G3_SERIES = 0 / 1 (run-time build): whether the E / M series is taken is known when the kernel is compiled
+#ifndef ISING_G3_SERIES
+#define ISING_G3_SERIES -1
+#endif
 
 template <bool BITS, bool HASJ, unsigned long long HP3 = kNoSpec3>
 __global__ void __launch_bounds__(ISING_G3_THREADS, ISING_G3_BLOCKS) k_grid3d(Grid3Args R) {
@@ -58,7 +62,7 @@ __global__ void __launch_bounds__(ISING_G3_THREADS, ISING_G3_BLOCKS) k_grid3d(Gr
     const uint32_t B = (uint32_t)A.B, Mw = R.jobs_per_warp;
     uint32_t* const ws = grid3_smem + (size_t)(threadIdx.x >> 5) * (2u * Mw * NSLOT * 32u) + lane;
     const uint2* lut = kByteLutGlobal.e;
-    const bool series = R.acc != nullptr;
+    const bool series = ISING_G3_SERIES < 0 ? R.acc != nullptr : ISING_G3_SERIES != 0;
 
     // what a lane keeps of a job: its tile, and the u64 offsets into xedge of its own record and of the words it polls
     struct Job { Tile3 t; uint32_t self, oxm, oxp, oym, oyp, oz, g, p_base; };

@@ -90,6 +90,11 @@ __device__ __forceinline__ void half_sweep_masks(const PlaneArgs& A, TileRegs<T>
 #ifndef ISING_G2_PARK
 #define ISING_G2_PARK 1
 #endif
+// ISING_G2_SERIES = 0 / 1 (run-time build): whether the E / M series is taken is known when the kernel is compiled (without
+// the accounting code the 28-warp kernel needs 70 registers and nothing spills; with it 72 and 40 bytes of spills)
+#ifndef ISING_G2_SERIES
+#define ISING_G2_SERIES -1
+#endif
 
 template <int T, bool BITS, bool HASJ, uint32_t HP = kNoSpec, bool PC = false>
 __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2_BLOCKS) k_grid_planes(GridArgs R) {
@@ -111,7 +116,7 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
     const uint32_t flags = (uint32_t)__cvta_generic_to_shared(ring + kPcRing * 2 * G::NW * 32);
     const uint32_t total_hs = PC ? (uint32_t)R.n * 4u * (uint32_t)A.k : 0u;
     const uint2* lut = kByteLutGlobal.e;
-    const bool series = R.acc != nullptr;
+    const bool series = ISING_G2_SERIES < 0 ? R.acc != nullptr : ISING_G2_SERIES != 0;
 
     struct Job { int r, tx, ty; uint32_t self, nU, nD, nL, nR; };
     auto decode = [&](uint32_t job, int C) {

@@ -672,7 +672,7 @@ int launch_grid3d_one(Grid3Args& R, bool want_jit, unsigned long long hp3, int r
         const void* fn = nullptr;
         if (want_jit && !HASJ && w_sm <= wsm_cap) {
             wpb = (int)((w_sm + 3u) / 4u * 4u); bps = 1;         // one CTA per SM, the same number of warps on every scheduler
-            fn = (const void*)grid3d_jit_kernel(BITS, hp3, reps, wpb * 32, bps);
+            fn = (const void*)grid3d_jit_kernel(BITS, hp3, reps, wpb * 32, bps, R.acc != nullptr);
         }
         if (fn) *used_jit = true;
         else {

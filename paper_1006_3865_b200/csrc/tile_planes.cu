@@ -1009,8 +1009,10 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit, bool 
     // 5.1, round 2); the shaped run-time build keeps winning (L = 8192, tile 64, k = 1 / 4 / 16: 2895 / 3303 / 3455 against
     // 2313 / 3019 / 3334 flips/ns), but a call must be long enough to pay for loading and storing the lattice once (n k >= 8
     // beyond two jobs per warp), and with 8 or 16 jobs per warp (L = 16384: all of the shared memory of the GPU holds spins)
-    // its 28 warps per SM lose to the 40 of the per-pass kernels where those are not HBM-bound: int8 records at k = 1 only
-    // (2776 against 2486 flips/ns at tile 64, 2416 against 2100 at tile 32; bits 2925 against 2942; k = 4: 3150 against 3233).
+    // its 28 warps per SM lose to the 40 of the per-pass kernels where those are not HBM-bound.  Measured at L = 16384, on
+    // chip against the best other path, flips/ns: tile 64 int8 k = 1 / 2 / 4 / 16: 2896 / 3109 / 3232 / 3404 against 2486 /
+    // 2962 / 3233 / 3491, bits k = 1 / 4: 3026 / 3369 against 2942 / 3315; tile 32 int8 k = 1 / 2 / 4: 2380 / 2815 / 3044
+    // against 2100 / 2858 / 3185, bits k = 1: 2480 against 2836.  Hence: tile 64 up to k = 3, tile 32 int8 at k = 1.
     const uint32_t max_m = kGridMaxJobsPerWarp;
     constexpr size_t kSmemMax = 227 * 1024;
     for (uint32_t M = 1; M <= max_m; ++M) {
@@ -1018,7 +1020,7 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit, bool 
         if (warp_cap && warps_needed > warp_cap && M < kGridMaxJobsPerWarp) continue;
         if (M > 2 && !warp_cap) {
             if ((uint64_t)R.n * (uint64_t)R.P.k < 8u) break;
-            if (M > 4 && (R.P.k != 1 || BITS)) break;             // measured at L = 16384: only int8 at k = 1 gains
+            if (M > 4 && !(T == 64 ? R.P.k <= 3 : (R.P.k == 1 && !BITS))) break;      // measured at L = 16384, above
         }
         const uint32_t w_sm = (warps_needed + (uint32_t)sms - 1) / (uint32_t)sms;
         int wpb = 0;
@@ -1030,7 +1032,7 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit, bool 
             wpb = (int)((w_sm + 3u) / 4u * 4u);
             park = park_mode != 0 && (size_t)wpb * 2u * M * (2u * PG<T>::NW + 7u) * lane_bytes <= kSmemMax;
             if (!park && (size_t)wpb * 2u * M * (2u * PG<T>::NW) * lane_bytes > kSmemMax) break;      // the lattice does not fit on chip
-            fn = (const void*)grid_jit_kernel(T, BITS, HASJ, R.P.hp, R.P.B, R.P.R, wpb * 32, 1, park);
+            fn = (const void*)grid_jit_kernel(T, BITS, HASJ, R.P.hp, R.P.B, R.P.R, wpb * 32, 1, park, R.acc != nullptr);
             if (!fn) { shaped = false; M = 0; continue; }         // no run-time compiler: again with the pre-compiled kernel
             *used_jit = true;
         } else {
