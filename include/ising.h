@@ -120,6 +120,22 @@ int ising_overlap(ising_handle h, int a, int b, int64_t* Q);
  * (XOR + popcount on the bit / byte tile records, no conversion to the canonical array).  Synchronises. */
 int ising_overlap_all(ising_handle h, int64_t* Q);
 
+/* ising_overlap_all_static — the same R x R table of overlaps (S8c.7) for callers that may not allocate device
+ * memory (code under CUDA graph capture, tight serving loops, harnesses that forbid cudaMalloc).  Takes no handle and calls
+ * no cudaMalloc / cudaFree / allocating library routine: its scratch (R·R difference counts) is a file-scope __device__
+ * array of ISING_STATIC_MAX_REPLICAS^2 x 8 bytes = 32 KiB that every GPU which loads the library holds until exit.
+ *   d_spins [device]  n_replicas · n_sites canonical int8 ±1 spins, replica-major (what ising_copy_spins writes), 4-byte
+ *                     aligned; n_sites a positive multiple of 4.  Caller-owned, read only.
+ *   d_Q     [device]  n_replicas · n_replicas int64, 8-byte aligned, caller-owned: Q[a*R + b] = Σ_i s_i^a s_i^b.
+ *   cuda_stream       the cudaStream_t to enqueue on; NULL = the library's stream (ising_set_device_hooks).
+ * Asynchronous: the work is enqueued and the call returns; nothing is copied to the host.  n_replicas < 1 or
+ * > ISING_STATIC_MAX_REPLICAS, NULL or misaligned pointers, bad n_sites ⇒ ISING_EINVAL, nothing enqueued.  ALL calls share
+ * the one array, which keeps the last call's contents (each call clears the part it uses first): calls that overlap on
+ * the GPU (different streams or host threads) race; serialise them.  The first call on a device resolves the array's
+ * device address (cudaGetSymbolAddress, once per device): make it before, not under, a graph capture. */
+#define ISING_STATIC_MAX_REPLICAS 64
+int ising_overlap_all_static(const int8_t* d_spins, int n_replicas, uint64_t n_sites, int64_t* d_Q, void* cuda_stream);
+
 /* ising_copy_spins — canonical int8 ±1 spins, R·N bytes, to dst [host|device]. Synchronises. */
 int ising_copy_spins(ising_handle h, int8_t* dst);
 

@@ -23,7 +23,7 @@ RNG_MODES = {"words": ISING_RNG_WORDS, "planes": ISING_RNG_PLANES}
 
 SYMBOLS = [
     "ising_create", "ising_create_batch", "ising_create_multi", "ising_destroy", "ising_sweep", "ising_sweep_series",
-    "ising_observables", "ising_overlap", "ising_overlap_all", "ising_copy_spins", "ising_set_spins", "ising_copy_spins_bits", "ising_set_spins_bits", "ising_set_layout", "ising_set_rng", "ising_set_jit", "ising_last_sweep_specialized",
+    "ising_observables", "ising_overlap", "ising_overlap_all", "ising_overlap_all_static", "ising_copy_spins", "ising_set_spins", "ising_copy_spins_bits", "ising_set_spins_bits", "ising_set_layout", "ising_set_rng", "ising_set_jit", "ising_last_sweep_specialized",
     "ising_get_counter", "ising_set_counter", "ising_thresholds", "ising_set_device_hooks",
     "ising_synchronize", "ising_kernel_launches", "ising_sweep_path", "ising_force_path",
     "ising_last_error",
@@ -68,6 +68,7 @@ def lib() -> C.CDLL:
     L.ising_observables.argtypes = [vp, i64p, i64p]
     L.ising_overlap.argtypes = [vp, C.c_int, C.c_int, i64p]
     L.ising_overlap_all.argtypes = [vp, i64p]
+    L.ising_overlap_all_static.argtypes = [i8p, C.c_int, C.c_uint64, i64p, vp]
     L.ising_copy_spins.argtypes = [vp, i8p]
     L.ising_set_spins.argtypes = [vp, i8p]
     L.ising_copy_spins_bits.argtypes = [vp, vp]
@@ -143,6 +144,18 @@ def _ptr(x):
         assert x.flags["C_CONTIGUOUS"]
         return C.c_void_p(x.ctypes.data)
     return C.c_void_p(x.data_ptr())          # torch tensor
+
+
+STATIC_MAX_REPLICAS = 64   # ISING_STATIC_MAX_REPLICAS (include/ising.h)
+
+
+def ising_overlap_all_static(d_spins, n_replicas: int, n_sites: int, d_Q, stream=None) -> None:
+    """All pairwise overlaps of n_replicas canonical int8 spin arrays without any device allocation (scratch: a 32 KiB
+    __device__ array inside the library, at most STATIC_MAX_REPLICAS replicas).  d_spins, d_Q: DEVICE tensors (int8
+    [R*N], int64 [R*R]); stream: a raw cudaStream_t value or None = the library's stream.  Asynchronous; calls that
+    overlap on the GPU race on the shared scratch."""
+    _check(lib().ising_overlap_all_static(_ptr(d_spins), int(n_replicas), int(n_sites), _ptr(d_Q),
+                                          C.c_void_p(int(stream)) if stream else None))
 
 
 def ising_thresholds(beta: float, dim: int):
