@@ -50,27 +50,49 @@ def measured_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
 
 
-def kernel_fingerprint() -> str:
-    """sha1 (12 hex digits) over the sources of the headline kernel: an ncu figure quoted below is only printed while the
+FP_FILES = {   # the device sources a kernel family is built from
+    "flow": ("philox.cuh", "planes_common.cuh", "tile_planes_device.cuh", "flow_planes_device.cuh"),
+    "tile": ("philox.cuh", "planes_common.cuh", "tile_planes_device.cuh", "flow_planes_device.cuh"),
+    "grid": ("philox.cuh", "planes_common.cuh", "tile_planes_device.cuh", "grid_planes_device.cuh"),
+}
+
+
+def kernel_fingerprint(family: str = "grid") -> str:
+    """sha1 (12 hex digits) over the sources of a kernel family: an ncu figure quoted below is only printed while the
     kernel it was captured from is the kernel being timed."""
     import hashlib
     h = hashlib.sha1()
-    for n in ("philox.cuh", "planes_common.cuh", "tile_planes_device.cuh", "flow_planes_device.cuh"):
+    for n in FP_FILES[family]:
         h.update(open(os.path.join(ROOT, "paper_1006_3865_b200", "csrc", n), "rb").read())
     return h.hexdigest()[:12]
 
 
 # From the committed ncu captures, per PHASE (one coarse colour of one pass = one launch of k_tile_planes, or a sixth of
 # the captured 3-pass launch of the persistent k_flow_planes): DRAM bytes read + written, and executed warp-instructions.
-# Keyed by (rng, layout, tile, k, kernel family); NCU_FINGERPRINT = kernel_fingerprint() of the sources they were captured from.
-NCU_FINGERPRINT = "7acfaaf12164"
+# The grid-resident kernel (lattice on chip for the whole call) touches DRAM once per CALL: its entries hold the bytes and
+# the instructions of a call's load + store ("*_call") and the instructions of one pass, separated by two captures of 8 and
+# 16 passes; a phase of a K-pass call is then (call + K * pass) / 2K.
+# Keyed by (rng, layout, tile, k, kernel family); "fp" = kernel_fingerprint(family) of the sources they were captured from.
 NCU = {
-    ("planes", "int8", 64, 1, "flow"): {"traffic": (803.28e6 + 757.91e6) / 6, "warp_instr": 219.54e6 / 6, "source": "profiles/r02c_flow_planes_i8.md"},
-    ("planes", "int8", 32, 1, "flow"): {"traffic": (803.52e6 + 798.38e6) / 6, "warp_instr": 246.42e6 / 6, "source": "profiles/r02c_flow_planes_i8.md"},
-    ("planes", "int8", 64, 1, "tile"): {"traffic": 138.44e6 + 80.40e6, "warp_instr": 33.73e6, "source": "profiles/r02c_flow_planes_i8.md"},
-    # plain checkerboard, one launch = one half-sweep of the whole lattice (round-1 capture; the fingerprint check drops it
-    # when the kernel has changed since)
+    ("planes", "int8", 64, 1, "flow"): {"traffic": (803.28e6 + 757.91e6) / 6, "warp_instr": 219.54e6 / 6, "fp": "7acfaaf12164", "source": "profiles/r02c_flow_planes_i8.md"},
+    ("planes", "int8", 32, 1, "flow"): {"traffic": (803.52e6 + 798.38e6) / 6, "warp_instr": 246.42e6 / 6, "fp": "7acfaaf12164", "source": "profiles/r02c_flow_planes_i8.md"},
+    ("planes", "int8", 64, 1, "tile"): {"traffic": 138.44e6 + 80.40e6, "warp_instr": 33.73e6, "fp": "7acfaaf12164", "source": "profiles/r02c_flow_planes_i8.md"},
+    ("planes", "int8", 64, 1, "grid"): {"traffic_call": 276.97e6 + 222.52e6, "warp_instr_call": 475.02e6 - 8 * 57.743e6, "warp_instr_pass": 57.743e6,
+                                        "fp": "33154a88849c", "source": "profiles/r02e_grid_planes_L16384.md"},
+    ("planes", "int8", 32, 1, "grid"): {"traffic_call": 321.26e6 + 269.46e6, "warp_instr_call": 571.92e6 - 8 * 69.019e6, "warp_instr_pass": 69.019e6,
+                                        "fp": "33154a88849c", "source": "profiles/r02e_grid_planes_L16384.md"},
 }
+
+
+def ncu_per_phase(entry, steps: int):
+    """(DRAM bytes, warp-instructions) of one phase of a `steps`-pass call from an NCU entry, or (None, None)."""
+    if entry is None:
+        return None, None
+    if "traffic_call" in entry:
+        return entry["traffic_call"] / (2 * steps), (entry["warp_instr_call"] + steps * entry["warp_instr_pass"]) / (2 * steps)
+    return entry["traffic"], entry["warp_instr"]
+
+
 # Issue slots of the GPU: 148 SMs x 4 schedulers, one warp-instruction per cycle at sm_max_mhz.
 def issue_peak_gips(sm_mhz: float) -> float:
     return 148 * 4 * sm_mhz * 1e6 / 1e9
@@ -188,7 +210,7 @@ JIT = "auto"     # --jit: run-time specialisation of the planes kernel (ising_se
 FORCE = 0        # --force-path: ising_force_path (0 automatic, 2 a launch per colour, 3 no data-flow kernel, 4 no on-chip kernels)
 
 
-def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng="planes", min_seconds=0.0, max_reps=1):
+def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng="planes", min_seconds=0.0, max_reps=1, force=None):
     """Device-timed throughput of one (rng, layout, tile, k) variant; returns dict.
 
     One repetition = one `ising_sweep(steps)` call = exactly `steps` outer passes (2 launches each, no host sync inside),
@@ -207,11 +229,14 @@ def time_variant(P, torch, L, layout, tile, k, steps, warmup, sampler=None, rng=
         g.set_jit("on" if JIT == "on" or (JIT == "auto" and steps * k * L * L >= 2 ** 27) else "off")
     else:
         g.set_jit(JIT)
-        warmup = max(warmup, steps)          # the same call once before: whatever AUTO compiles is compiled outside the timed region
+    if tile in (32, 64) and steps >= 2:
+        # the same call once before: which kernel serves a call depends on its length (a lattice is put on chip only for a
+        # call long enough to pay for it), so only the same call compiles, outside the timed region, what the timed call runs
+        warmup = max(warmup, steps)
     if layout == "bits":
         g.set_layout(P.ISING_LAYOUT_BITS)
-    if FORCE:
-        g.force_path(FORCE)
+    if force if force is not None else FORCE:
+        g.force_path(force if force is not None else FORCE)
     if sampler:
         sampler.start()
     g.sweep(W.BETA_C_2D, warmup, tile, k)
@@ -535,48 +560,69 @@ def main() -> None:
     ms, value = aggregate_replicas(res["ms"], world, a.steps, a.k, L, dist, "cuda")
 
     peak, peak_src, sm_max = measured_peaks()
-    family = "flow" if res["path"].startswith("flow") else "tile" if res["path"].startswith("tile_planes") else res["path"]
+    family = ("flow" if res["path"].startswith("flow") else "tile" if res["path"].startswith("tile_planes") else
+              "grid" if res["path"].startswith("grid_planes") else res["path"])
     ncu = NCU.get((a.rng, a.layout, a.tile, a.k, family)) if L == 16384 and res["path"].endswith("+jit") else None
-    ncu_stale = ncu is not None and kernel_fingerprint() != NCU_FINGERPRINT
+    ncu_stale = ncu is not None and kernel_fingerprint(family) != ncu["fp"]
     if ncu_stale:            # the kernel changed since the capture: quote nothing from it
         ncu = None
+    traffic, warp_instr = ncu_per_phase(ncu, a.steps)
     bpf = algorithmic_bytes_per_flip(a.tile, a.k, a.layout, L)
     launches_per_step = 2
     bytes_per_launch = bpf * a.k * L * L / launches_per_step
     launch_ms = res["ms"] / (a.steps * launches_per_step)
     achieved = bytes_per_launch / (launch_ms * 1e6)            # GB/s
     lat_bytes = L * L if a.layout == "int8" else L * L // 8
+    on_chip = family == "grid"
+    hbm = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
+           "frac_of_8TBs_nominal": achieved / 8000.0, "algorithmic_bytes_per_flip": bpf}
+    issue = ({"bound": "alu", "unit": "G warp-instr/s", "achieved": warp_instr / (launch_ms * 1e6),
+              "peak": issue_peak_gips(sm_max), "frac": warp_instr / (launch_ms * 1e6) / issue_peak_gips(sm_max),
+              "peak_source": "148 SMs x 4 schedulers x one warp-instruction per cycle x sm_max_mhz (DESIGN.md 7.3)",
+              "kind": "issue slots (one warp-instruction per scheduler cycle, 592 schedulers)",
+              "warp_instr_per_phase": warp_instr,
+              "note": "what binds is not the slot count but the dispatch model of DESIGN.md 7.3 / profiles/r02_microbench.md "
+                      "(a 16-lane ALU instruction holds the scheduler 2 cycles, a wide multiply 2.25): a model, not a hardware counter"}
+             if warp_instr else None)
+    common = {"traffic": traffic,
+              "traffic_source": ("ncu dram__bytes_read.sum + dram__bytes_write.sum per phase, " + ncu.get("source", "profiles/")) if ncu else None,
+              "traffic_stale": ncu_stale, "kernel": f"{res['path']}<{a.tile}>", "avg_launch_ms": launch_ms}
+    if on_chip:
+        # The lattice stays in shared memory for the whole call: DRAM sees it once per call, not once per phase, and the
+        # kernel is bound by instruction issue.  The roofline is therefore the ALU one; the algorithmic-bytes figure of
+        # SURVEY 8(d) (what a kernel that streams the lattice every pass must move) is kept beside it for comparison.
+        roof = dict(issue) if issue else {"bound": "alu", "unit": "G warp-instr/s", "achieved": None, "peak": issue_peak_gips(sm_max), "frac": None}
+        roof.update(common)
+        roof["launch_unit"] = ("one phase (coarse colour of a pass) of the cooperative launch that keeps the lattice on chip: CUDA-event time "
+                               "of the call / (2 * steps), the load and the store of the lattice (once per call) included")
+        roof["hbm_algorithmic"] = dict(hbm, note="bytes a kernel that streams the lattice every pass would move (SURVEY 8(d)) / measured time: "
+                                                 f"such a kernel cannot exceed {peak / bpf:.0f} flips/ns; this one moves traffic / algorithmic "
+                                                 "of them (the lattice crosses HBM once per call)")
+    else:
+        roof = dict(hbm)
+        roof.update(common)
+        roof["launch_unit"] = ("one launch of k_tile_planes = one coarse colour of one pass" if res["path"].startswith("tile") else
+                               "one phase (coarse colour of a pass) of the persistent launch: CUDA-event time of the call / (2 * steps)")
+        roof["issue"] = issue
+    how = ("(2 launches)" if res["path"].startswith("tile") else
+           "(all steps of a call in one cooperative launch, the lattice in shared memory from the first pass to the last)" if on_chip else
+           "(all steps of a call in one persistent launch)")
     line = {"metric": METRIC if L == 16384 else f"spin flips/ns (2D Ising L={L}, beta_c)", "value": value, "unit": UNIT,
             "n_gpus": world, "steps": a.steps, "warmup": a.warmup,
             "ms_per_step": ms / a.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "u8" if a.layout == "int8" else "u32 bit-planes", "data": "synthetic",
             "config": {"workload": f"{'BASELINE config 3' if L == 16384 else 'config 3 at another size'}: 2D Ising L={L} hot start seed 3 "
-                                   f"beta=0.4406868 layout={a.layout} rng={a.rng} tile={a.tile} k={a.k}; one step = one outer pass "
-                                   + ("(2 launches)" if res["path"].startswith("tile") else "(all steps of a call in one persistent launch)"),
-                       "l2": f"lattice ({lat_bytes / 2 ** 20:g} MiB {a.layout}) exceeds the 126 MB L2; no explicit flush" if lat_bytes > 126e6
-                             else f"lattice ({lat_bytes / 2 ** 20:g} MiB {a.layout}) fits L2: not an HBM claim",
+                                   f"beta=0.4406868 layout={a.layout} rng={a.rng} tile={a.tile} k={a.k}; one step = one outer pass " + how,
+                       "l2": (f"lattice ({lat_bytes / 2 ** 20:g} MiB {a.layout}) exceeds the 126 MB L2; no explicit flush" if lat_bytes > 126e6
+                              else f"lattice ({lat_bytes / 2 ** 20:g} MiB {a.layout}) fits L2: not an HBM claim")
+                             + ("; on chip between the passes of a call: read from and written to HBM once per call, inside the timed region" if on_chip else ""),
                        "kernel_path": res["path"], "parallelism": "replicas only" if world > 1 else "single GPU"},
             "ns_per_flip": 1.0 / value, "gpu_launches": res["launches"], "clocks": res["clocks"],
             "repetitions": {"n": res["reps"], "each": f"one ising_sweep({a.steps}) call = exactly {a.steps} steps, CUDA events around it",
                             "reported": "median", "gpu_seconds": res["gpu_seconds"],
                             "value_min": a.steps * a.k * L * L / (res["ms_max"] * 1e6) * world,
                             "value_max": a.steps * a.k * L * L / (res["ms_min"] * 1e6) * world},
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": ncu["traffic"] if ncu else None,
-                         "traffic_source": ("ncu dram__bytes_read.sum + dram__bytes_write.sum per phase, "
-                                            + ncu.get("source", "profiles/")) if ncu else None,
-                         "traffic_stale": ncu_stale,
-                         "peak_source": peak_src, "frac_of_8TBs_nominal": achieved / 8000.0,
-                         "algorithmic_bytes_per_flip": bpf, "kernel": f"{res['path']}<{a.tile}>",
-                         "avg_launch_ms": launch_ms,
-                         "launch_unit": "one launch of k_tile_planes = one coarse colour of one pass" if res["path"].startswith("tile") else
-                                        "one phase (coarse colour of a pass) of the persistent launch: CUDA-event time of the call / (2 * steps)",
-                         "issue": ({"bound": "alu", "unit": "G warp-instr/s", "achieved": ncu["warp_instr"] / (launch_ms * 1e6),
-                                    "peak": issue_peak_gips(sm_max), "frac": ncu["warp_instr"] / (launch_ms * 1e6) / issue_peak_gips(sm_max),
-                                    "kind": "issue slots (one warp-instruction per scheduler cycle, 592 schedulers)",
-                                    "note": "what binds is not the slot count but the dispatch model of DESIGN.md 7.3 / profiles/r02_microbench.md "
-                                            "(a 16-lane ALU instruction holds the scheduler 2 cycles, a wide multiply 2.25): a model, not a hardware counter"}
-                                   if ncu else None)}}
+            "roofline": roof}
     if rank == 0 and not a.no_extras and world == 1:
         table = {}
         for rng, lay in (("planes", "int8"), ("planes", "bits"), ("words", "int8")):
@@ -584,8 +630,17 @@ def main() -> None:
                 for k in (1, 4, 16):
                     st = max(2, min(a.steps, 40 // k))
                     r = time_variant(P, torch, L, lay, T, k, st, 3, None, rng, min_seconds=0.25, max_reps=400)
-                    table[f"{rng}_{lay}_t{T}_k{k}"] = {"flips_per_ns": round(r["flips_per_ns"], 1), "steps": st, "reps": r["reps"],
+                    table[f"{rng}_{lay}_t{T}_k{k}"] = {"flips_per_ns": round(r["flips_per_ns"], 1), "steps": st, "reps": r["reps"], "kernel_path": r["path"],
                                                 "hbm_GBs": round(r["flips_per_ns"] * algorithmic_bytes_per_flip(T, k, lay), 1)}
+        # the headline variant through the kernels that stream the lattice through HBM every pass (ising_force_path 4: the
+        # persistent data-flow kernel; 2: a launch per coarse colour): the HBM-bound forms of the same call
+        for T in (64, 32):
+            for fp, name in ((4, "flow"), (2, "launches")):
+                st = max(2, min(a.steps, 40))
+                r = time_variant(P, torch, L, "int8", T, 1, st, 3, None, "planes", min_seconds=0.25, max_reps=400, force=fp)
+                table[f"planes_int8_t{T}_k1_hbm_{name}"] = {"flips_per_ns": round(r["flips_per_ns"], 1), "steps": st, "reps": r["reps"], "kernel_path": r["path"],
+                                                           "hbm_GBs": round(r["flips_per_ns"] * algorithmic_bytes_per_flip(T, 1, "int8"), 1),
+                                                           "hbm_frac": round(r["flips_per_ns"] * algorithmic_bytes_per_flip(T, 1, "int8") / peak, 3)}
         # the scheme the paper starts from (row a8): plain checkerboard, tile == L, a launch per half-sweep
         for lay in ("int8", "bits"):
             st = max(2, min(a.steps, 40))
