@@ -746,6 +746,38 @@ def test_grid_resident_kernel_several_jobs_per_warp():
         assert out.returncode == 0 and "capped ok" in out.stdout, out.stderr[-2000:]
 
 
+def test_grid_resident_kernel_run_time_build_without_parked_constants():
+    """The run-time build of the same kernel in the form that holds BASELINE config 3 on chip (one CTA per SM, geometry and
+    threshold heads compiled in, up to 16 jobs of a colour per warp, the jobs' constants decoded in every phase instead of
+    parked in shared memory: ISING_G2_PARK=0, a testing aid, forces that form on lattices the oracle finishes in seconds),
+    with and without the E / M series (two different builds), replicas (per-replica Philox keys) and +-J couplings."""
+    import os, subprocess, sys
+    code = (
+        "import numpy as np, paper_1006_3865_b200 as P\n"
+        "from oracle import oracle as O\n"
+        "import ising_workloads as W\n"
+        "P.use_torch()\n"
+        "for (L, T, k, n, seeds, bits, jseed, beta) in ((1024, 32, 1, 4, [5], False, None, 0.4406868), (768, 64, 2, 3, [6, 7], True, None, 0.44),\n"
+        "                                              (640, 32, 1, 3, [8], False, 5, 1.0), (1024, 64, 1, 5, [9], False, None, 0.4406868)):\n"
+        "    J = W.couplings(2, L, jseed) if jseed is not None else None\n"
+        "    g = P.Ising(2, L, coupling=J, seeds=seeds); o = O.Oracle(2, L, seeds=seeds, J=J)\n"
+        "    g.set_jit('on')\n"
+        "    if bits: g.set_layout(P.ISING_LAYOUT_BITS)\n"
+        "    g.sweep(beta, n, T, k); o.sweep(beta, n, T, k)\n"
+        "    assert g.sweep_path().startswith('grid_planes') and g.last_sweep_specialized(), g.sweep_path()\n"
+        "    assert np.array_equal(np.asarray(g.copy_spins()).reshape(-1), np.asarray(o.spins()).reshape(-1))\n"
+        "    Eg, Mg = g.sweep_series(beta, n, T, k); Eo, Mo = o.sweep_series(beta, n, T, k)\n"
+        "    assert g.sweep_path().startswith('grid_planes') and g.last_sweep_specialized(), g.sweep_path()\n"
+        "    assert np.array_equal(Eg, Eo) and np.array_equal(Mg, Mo)\n"
+        "    assert np.array_equal(np.asarray(g.copy_spins()).reshape(-1), np.asarray(o.spins()).reshape(-1))\n"
+        "print('unparked ok')\n")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    for cap in ("24", "100"):
+        out = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, ISING_GRID_WARPS=cap, ISING_G2_PARK="0"),
+                             capture_output=True, text=True, timeout=900)
+        assert out.returncode == 0 and "unparked ok" in out.stdout, out.stderr[-2000:]
+
+
 @pytest.mark.parametrize("dim,L,tile,k,rng,layout,R,jseed", [
     (2, 128, 32, 2, "planes", "int8", 5, 5),       # plane records, 0/1 bytes
     (2, 128, 64, 1, "planes", "bits", 16, 7),      # bit records, two pair chunks per row (R - 1 > 8)
