@@ -220,10 +220,12 @@ uint64_t ising_kernel_launches(void);
  *   resident_masked_*, tile_masked_*, resident3d_masked_*, tile3d_masked_*
  *                           double checkerboard with power-of-two tiles other than the register tiles (2D: 2, 4, 8, 16 —
  *                           the paper's sizes, P:86 — and 128, 256, ...; 3D: 2, 4, 16, 32, ...) as masked half-sweeps
- *   grid_planes_{i8,bits}, grid3d_planes_{i8,bits}   lattices beyond the cluster that fit on chip (2D 512 < L <= 4096, 3D 64 < L): the
- *                           whole call in one cooperative launch, boundary words exchanged through L2
- *   flow_planes_{i8,bits}   HBM-resident 2D lattices: all passes in one persistent launch, coarse colours ordered by per-tile
- *                           progress counters
+ *   grid_planes_{i8,bits}, grid3d_planes_{i8,bits}   lattices beyond the cluster that fit in the shared memory of the GPU (2D
+ *                           512 < L, up to 2^28 sites on a B200 where measured to pay: DESIGN.md §6.1g; 3D 64 < L): the whole
+ *                           call in one cooperative launch, the lattice read from and written to HBM once per call, boundary
+ *                           words exchanged through L2
+ *   flow_planes_{i8,bits}   HBM-resident 2D lattices (and calls too short to pay for putting the lattice on chip): all passes in
+ *                           one persistent launch, coarse colours ordered by per-tile progress counters
  *   amsc                    asynchronous multi-spin coding of a multi-realisation batch (ising_create_multi)
  * The fast 2D families need L % 32 == 0 (L % 64 for tile 64) and an even number of register tiles per side, the 3D ones
  * L % 8 == 0 and L / 8 even. */
