@@ -95,6 +95,24 @@ __device__ __forceinline__ void half_sweep_masks(const PlaneArgs& A, TileRegs<T>
 #ifndef ISING_G2_SERIES
 #define ISING_G2_SERIES -1
 #endif
+// ISING_G2_STRIP = M > 0 (run-time build, several jobs per warp): warp w owns the M CONSECUTIVE jobs w M ... w M + M - 1 of
+// each colour, i.e. a strip of 2 M (tile 64) or 4 M (tile 32) adjacent tiles of one tile row (M divides the jobs of a row),
+// instead of the jobs w, w + W, ...  The left and right neighbours of a tile (other colour, same row) are then the warp's
+// own jobs, except at the two ends of the strip: their boundary columns are read from the words the warp has parked in shared
+// memory (same block row = same lane, or the other half-warp at tile 32) instead of being published to and polled from L2;
+// only the tile rows above and below, and the strip ends, go through the exchange records.  With the colour-C tiles of a row at
+// tx = 2 q + p, p = (ty + C) & 1, and the other colour's at 2 q' + 1 - p: p = 0: right neighbour q' = q, left q' = q - 1;
+// p = 1: left q' = q, right q' = q + 1 (tile 32: q = 2 job + sub).
+#ifndef ISING_G2_STRIP
+#define ISING_G2_STRIP 0
+#endif
+
+// tile row (its parity is all that is used) of the strip that starts at job j0: jobs of a colour are enumerated row by row
+template <int T>
+__device__ __forceinline__ uint32_t geom_strip_row(const PlaneArgs& A, uint32_t j0) {
+    const uint32_t jobs_per_row = geom_B(A) / 2u / (uint32_t)PG<T>::TPW;
+    return (j0 / jobs_per_row) % geom_B(A);
+}
 
 template <int T, bool BITS, bool HASJ, uint32_t HP = kNoSpec, bool PC = false>
 __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2_BLOCKS) k_grid_planes(GridArgs R) {
@@ -109,7 +127,9 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
     const uint32_t wg = PC ? blockIdx.x : blockIdx.x * (blockDim.x >> 5) + (uint32_t)wic, W = PC ? gridDim.x : gridDim.x * (blockDim.x >> 5);
     const int sub = lane / G::LPT, Y = lane % G::LPT;
     const uint32_t B = geom_B(A);
-    const uint32_t Mw = PC ? 1u : R.jobs_per_warp;
+    constexpr uint32_t STRIP = PC ? 0u : (uint32_t)ISING_G2_STRIP;
+    const uint32_t Mw = PC ? 1u : (STRIP ? STRIP : R.jobs_per_warp);
+    auto job_of = [&](uint32_t m) { return STRIP ? wg * Mw + m : wg + m * W; };
     uint32_t* const ws = grid_smem + (PC ? 0u : (size_t)wic * (2u * Mw * NSLOT * 32u)) + lane;
     // PC: behind the consumer's area, the ring [slot][R1 | R2][gx][lane], its "full" words and the consumed counter
     uint32_t* const ring = grid_smem + 2u * NSLOT * 32u;
@@ -125,6 +145,7 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
         const uint32_t r = (uint32_t)ri, tx = (uint32_t)txi, ty = (uint32_t)tyi;
         const uint32_t base = r * B * B, row = base + ty * B;
         const uint32_t tyU = ty == 0 ? B - 1 : ty - 1, tyD = ty == B - 1 ? 0 : ty + 1;
+        if (STRIP) return Job{(int)r, (int)tx, (int)ty, row + tx, base + tyU * B + tx, base + tyD * B + tx, 0u, 0u};      // nL / nR: refresh, strip ends only
         const uint32_t txL = tx == 0 ? B - 1 : tx - 1, txR = tx == B - 1 ? 0 : tx + 1;
         return Job{(int)r, (int)tx, (int)ty, row + tx, base + tyU * B + tx, base + tyD * B + tx, row + txL, row + txR};
     };
@@ -137,14 +158,23 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
                                   : make_uint4(0u, 0u, 0u, 0u);
     };
     // the tile's boundary words, version ver, into its exchange record
-    auto publish = [&](const TileRegs<T>& tt, uint32_t me, uint32_t ver) {
+    auto publish = [&](const TileRegs<T>& tt, const Job& jb, uint32_t ver, int C, uint32_t m) {
         const uint32_t sh = (uint32_t)sub * G::LPT, msk = G::LPT == 32 ? 0xffffffffu : ((1u << G::LPT) - 1u);
-        const uint32_t L0 = (__ballot_sync(0xffffffffu, tt.S[0][0] & 1u) >> sh) & msk;
-        const uint32_t L1 = (__ballot_sync(0xffffffffu, (tt.S[1][0] >> 16) & 1u) >> sh) & msk;
-        const uint32_t R0 = (__ballot_sync(0xffffffffu, (tt.S[1][G::NW - 1] >> 15) & 1u) >> sh) & msk;
-        const uint32_t R1 = (__ballot_sync(0xffffffffu, tt.S[0][G::NW - 1] >> 31) >> sh) & msk;
         const unsigned long long v = (unsigned long long)ver << 32;
-        unsigned long long* e = R.xedge + (size_t)me * 16;
+        unsigned long long* e = R.xedge + (size_t)jb.self * 16;
+        // STRIP: only the tiles at the two ends of the warp's strip have a left / right neighbour in another warp (warp-uniform)
+        const uint32_t par = ((uint32_t)jb.ty + (uint32_t)C) & 1u;
+        const bool pubL = !STRIP || (par == 0u && m == 0u), pubR = !STRIP || (par == 1u && m + 1u == Mw);
+        if (pubL) {
+            const uint32_t L0 = (__ballot_sync(0xffffffffu, tt.S[0][0] & 1u) >> sh) & msk;
+            const uint32_t L1 = (__ballot_sync(0xffffffffu, (tt.S[1][0] >> 16) & 1u) >> sh) & msk;
+            if (Y == 0 && (!STRIP || sub == 0)) st_xedge2(e + 4, v | L0, v | L1);      // (T = 32: Y = 0 of each of the two tiles)
+        }
+        if (pubR) {
+            const uint32_t R0 = (__ballot_sync(0xffffffffu, (tt.S[1][G::NW - 1] >> 15) & 1u) >> sh) & msk;
+            const uint32_t R1 = (__ballot_sync(0xffffffffu, tt.S[0][G::NW - 1] >> 31) >> sh) & msk;
+            if (Y == 0 && (!STRIP || sub == G::TPW - 1)) st_xedge2(e + 6, v | R0, v | R1);
+        }
         if (Y == 0 || Y == G::LPT - 1) {
             unsigned long long* rw = e + (Y == 0 ? 0 : 8);          // TOP : BOT
             if (G::NW == 2) {
@@ -154,21 +184,68 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
                 st_xedge2(rw, v | tt.S[0][0], v | tt.S[1][0]);
             }
         }
-        if (Y == 0) {                                               // (T = 32: Y = 0 of each of the two tiles)
-            st_xedge2(e + 4, v | L0, v | L1);
-            st_xedge2(e + 6, v | R0, v | R1);
-        }
     };
     // wait until the four neighbours have published version `want`, and take the halos from their words
-    auto refresh = [&](TileRegs<T>& tt, const Job& jb, uint32_t want) {
+    auto refresh = [&](TileRegs<T>& tt, const Job& jb, uint32_t want, int C, uint32_t m) {
         const unsigned long long* rowp = R.xedge + (size_t)(Y == 0 ? jb.nU : jb.nD) * 16 + (Y == 0 ? 8 : 0);   // BOT of the tile above : TOP of the tile below
-        const unsigned long long* lf = R.xedge + (size_t)jb.nL * 16 + 6;                                       // {R0, R1}
-        const unsigned long long* rt = R.xedge + (size_t)jb.nR * 16 + 4;                                       // {L0, L1}
+        auto left_of = [&]() { return STRIP ? jb.self - (uint32_t)jb.tx + (jb.tx == 0 ? B - 1u : (uint32_t)jb.tx - 1u) : jb.nL; };
+        auto right_of = [&]() { return STRIP ? jb.self - (uint32_t)jb.tx + ((uint32_t)jb.tx == B - 1u ? 0u : (uint32_t)jb.tx + 1u) : jb.nR; };
         const bool need_row = Y == 0 || Y == G::LPT - 1;
+        bool extL = true, extR = true;                        // (per lane) the neighbour lives in another warp: through the exchange record
+        bool edge = true;                                     // (per warp) some lane has such a neighbour
+        if (STRIP) {
+            if (G::TPW == 2) __syncwarp();                    // the other half-warp's parked words: written by other lanes
+            // slot (of the other colour) and lane of the tiles to the left and to the right (header comment)
+            const uint32_t par = ((uint32_t)jb.ty + (uint32_t)C) & 1u;
+            edge = par == 0u ? m == 0u : m + 1u == Mw;
+            constexpr int S = NSLOT * 32;
+            const uint32_t* same = ws + (size_t)((uint32_t)(1 - C) * Mw + m) * (uint32_t)S;      // the other colour's job of the same index
+            const uint32_t *ql, *qr;
+            if (G::TPW == 1) {
+                ql = same - (par ? 0 : S); qr = ql + S;
+            } else {
+                const int flip = (lane & 16) ? -16 : 16;
+                if (par == 0u) { qr = same; ql = same + flip - (sub == 0 ? S : 0); }
+                else { ql = same; qr = same + flip + (sub == 1 ? S : 0); }
+            }
+            extL = par == 0u && m == 0u && (G::TPW == 1 || sub == 0);
+            extR = par == 1u && m + 1u == Mw && (G::TPW == 1 || sub == 1);
+            if (!extL) { tt.hL0 = (ql[(2 * G::NW - 1) * 32] >> 15) & 1u; tt.hL1 = ql[(G::NW - 1) * 32] >> 31; }      // its R0, R1
+            if (!extR) { tt.hR0 = qr[0] & 1u; tt.hR1 = (qr[G::NW * 32] >> 16) & 1u; }                               // its L0, L1
+        }
+        if (STRIP && !edge) {                                 // all but one job of a phase: only the tile rows above and below
+            for (;;) {
+                ulonglong2 r0 = make_ulonglong2(0, 0), r1 = r0;
+                bool ok = true;
+                if (need_row) {
+                    r0 = ld_xedge2(rowp);
+                    ok = (uint32_t)(r0.x >> 32) == want && (uint32_t)(r0.y >> 32) == want;
+                    if (G::NW == 2) {
+                        r1 = ld_xedge2(rowp + 2);
+                        ok = ok && (uint32_t)(r1.x >> 32) == want && (uint32_t)(r1.y >> 32) == want;
+                    }
+                }
+                if (__all_sync(0xffffffffu, ok)) {
+                    tt.vrow[0][0] = (uint32_t)r0.x;
+                    if (G::NW == 2) { tt.vrow[0][1] = (uint32_t)r0.y; tt.vrow[1][0] = (uint32_t)r1.x; tt.vrow[1][1] = (uint32_t)r1.y; }
+                    else tt.vrow[1][0] = (uint32_t)r0.y;
+                    return;
+                }
+            }
+        }
+        const unsigned long long* lf = R.xedge + (size_t)left_of() * 16 + 6;                                    // {R0, R1}
+        const unsigned long long* rt = R.xedge + (size_t)right_of() * 16 + 4;                                   // {L0, L1}
         for (;;) {
-            ulonglong2 r0 = make_ulonglong2(0, 0), r1 = r0;
-            const ulonglong2 a = ld_xedge2(lf), b = ld_xedge2(rt);
-            bool ok = (uint32_t)(a.x >> 32) == want && (uint32_t)(a.y >> 32) == want && (uint32_t)(b.x >> 32) == want && (uint32_t)(b.y >> 32) == want;
+            ulonglong2 r0 = make_ulonglong2(0, 0), r1 = r0, a = r0, b = r0;
+            bool ok = true;
+            if (extL) {
+                a = ld_xedge2(lf);
+                ok = ok && (uint32_t)(a.x >> 32) == want && (uint32_t)(a.y >> 32) == want;
+            }
+            if (extR) {
+                b = ld_xedge2(rt);
+                ok = ok && (uint32_t)(b.x >> 32) == want && (uint32_t)(b.y >> 32) == want;
+            }
             if (need_row) {
                 r0 = ld_xedge2(rowp);
                 ok = ok && (uint32_t)(r0.x >> 32) == want && (uint32_t)(r0.y >> 32) == want;
@@ -181,8 +258,8 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
                 tt.vrow[0][0] = (uint32_t)r0.x;
                 if (G::NW == 2) { tt.vrow[0][1] = (uint32_t)r0.y; tt.vrow[1][0] = (uint32_t)r1.x; tt.vrow[1][1] = (uint32_t)r1.y; }
                 else tt.vrow[1][0] = (uint32_t)r0.y;
-                tt.hL0 = ((uint32_t)a.x >> Y) & 1u; tt.hL1 = ((uint32_t)a.y >> Y) & 1u;
-                tt.hR0 = ((uint32_t)b.x >> Y) & 1u; tt.hR1 = ((uint32_t)b.y >> Y) & 1u;
+                if (extL) { tt.hL0 = ((uint32_t)a.x >> Y) & 1u; tt.hL1 = ((uint32_t)a.y >> Y) & 1u; }
+                if (extR) { tt.hR0 = ((uint32_t)b.x >> Y) & 1u; tt.hR1 = ((uint32_t)b.y >> Y) & 1u; }
                 return;
             }
         }
@@ -203,7 +280,7 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
         }
     };
     auto sm_job = [&](int C, uint32_t m) {                             // the constants parked by the prologue
-        if (!PARK) return decode(wg + m * W, C);
+        if (!PARK) return decode(job_of(m), C);
         const uint32_t* p = ws + (size_t)((uint32_t)C * Mw + m) * (NSLOT * 32u) + NWORDS * 32;
         const uint32_t xy = p[5 * 32];
         return Job{(int)p[6 * 32], (int)(xy & 0xffffu), (int)(xy >> 16), p[0], p[1 * 32], p[2 * 32], p[3 * 32], p[4 * 32]};
@@ -233,14 +310,14 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
     // records -> shared memory; the colour-1 tiles publish their initial boundary (version 1 = what phase 0 waits for)
     for (int C = 0; C < 2 && (!PC || wic == 0); ++C)
         for (uint32_t m = 0; m < Mw; ++m) {
-            const uint32_t job = wg + m * W;
+            const uint32_t job = job_of(m);
             if (job >= R.jobs_total) break;                               // warp-uniform
             const Job jb = decode(job, C);
             TileRegs<T> tt;
             load_tile<T, BITS>(A, jb.r, jb.tx, jb.ty, Y, sub * G::LPT, tt);
             sm_store(tt, C, m);
             sm_put_job(jb, C, m);
-            if (C == 1) publish(tt, jb.self, 1u);
+            if (C == 1) publish(tt, jb, 1u, C, m);
         }
 
     if (PC) {
@@ -300,16 +377,22 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
             const uint32_t ph = 2u * (uint32_t)pass + (uint32_t)C;       // this phase waits for version ph + 1 and publishes ph + 2
             // (Starting each phase one band of jobs later, so that no job waits for the end of the phase before, was
             // measured: no gain at tile 32, -8 % at tile 64 where the extra state spills.)
+            // STRIP: the two tiles at the ends of a strip wait for a tile of the neighbouring warp, and that one for them.  Where the
+            // colour's tiles sit at even tx (p = 0) the dependent tile is m = 0, else m = M - 1: a warp walks its strip from that
+            // end, so that both are the first job of their phases and each has had M - 1 jobs of time to arrive (walking always
+            // from m = 0 made the first job of every phase wait for the last job of the phase before: -4 % at tile 64).
+            const bool backwards = STRIP && (((geom_strip_row<T>(A, wg * Mw) + (uint32_t)C) & 1u) != 0u);
 #pragma unroll 1
-            for (uint32_t m = 0; m < Mw; ++m) {
-                const uint32_t job = wg + m * W;
+            for (uint32_t mi = 0; mi < Mw; ++mi) {
+                const uint32_t m = backwards ? Mw - 1u - mi : mi;
+                const uint32_t job = job_of(m);
                 if (job >= R.jobs_total) break;                           // warp-uniform
                 const Job jb = sm_job(C, m);
                 TileRegs<T> tt;
                 sm_load(tt, C, m);
                 uint4 Jw[2][G::NW];
                 jwords(jb, Jw);
-                refresh(tt, jb, ph + 1u);
+                refresh(tt, jb, ph + 1u, C, m);
                 if (series && C == 0 && pass > 0) account(tt, Jw, jb.r, pass - 1);     // colour-0 tiles: the halos of the finished pass just arrived
 #if defined(ISING_JIT_R) && ISING_JIT_R == 1
                 const uint64_t seed = A.seed0;
@@ -340,7 +423,7 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
                         half_sweep<T, HASJ, false, HP>(A, tt, Jw, 1, Y, g0, p0, 2 * t64 + 1, k0, k1);
                     }
                 }
-                publish(tt, jb.self, ph + 2u);
+                publish(tt, jb, ph + 2u, C, m);
                 if (series && C == 1) account(tt, Jw, jb.r, pass);       // colour-1 tiles: their halos (colour 0) are final for this pass
                 sm_store(tt, C, m);
             }
@@ -348,19 +431,19 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
     }
     if (series && R.n > 0)
         for (uint32_t m = 0; m < Mw; ++m) {
-            const uint32_t job = wg + m * W;
+            const uint32_t job = job_of(m);
             if (job >= R.jobs_total) break;
             const Job jb = sm_job(0, m);
             TileRegs<T> tt;
             sm_load(tt, 0, m);
             uint4 Jw[2][G::NW];
             jwords(jb, Jw);
-            refresh(tt, jb, 2u * (uint32_t)R.n + 1u);
+            refresh(tt, jb, 2u * (uint32_t)R.n + 1u, 0, m);
             account(tt, Jw, jb.r, R.n - 1);
         }
     for (int C = 0; C < 2; ++C)
         for (uint32_t m = 0; m < Mw; ++m) {
-            const uint32_t job = wg + m * W;
+            const uint32_t job = job_of(m);
             if (job >= R.jobs_total) break;
             const Job jb = sm_job(C, m);
             TileRegs<T> tt;

@@ -86,7 +86,7 @@ cudaKernel_t planes_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, 
 cudaKernel_t planes3d_jit_kernel(bool bits, unsigned long long hp3, int R);   // nullptr: not available
 cudaKernel_t grid3d_jit_kernel(bool bits, unsigned long long hp3, int R, int threads, int blocks, bool series);   // k_grid3d specialised on the three threshold heads and the CTA shape
 cudaKernel_t flow_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R, int NS, bool staged);   // k_flow_planes, specialised like k_tile_planes
-cudaKernel_t grid_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R, int threads, int blocks, bool park, bool series);   // k_grid_planes specialised on the threshold heads and the CTA shape
+cudaKernel_t grid_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R, int threads, int blocks, bool park, bool series, int strip);   // k_grid_planes specialised on the threshold heads and the CTA shape
 uint64_t planes_jit_compiled();
 const char* planes_jit_last_log();
 

@@ -184,12 +184,12 @@ cudaKernel_t flow_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, in
 
 // The grid-resident 2D kernel (grid_planes_device.cuh) specialised for (T, BITS, HASJ, HP), the geometry, the CTA shape and
 // whether the jobs' constants are parked in shared memory.
-cudaKernel_t grid_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R, int threads, int blocks, bool park, bool series) {
+cudaKernel_t grid_jit_kernel(int T, bool bits, bool hasj, uint32_t hp, int B, int R, int threads, int blocks, bool park, bool series, int strip) {
     char expr[160];
     snprintf(expr, sizeof expr, "ising::jit::k_grid_planes<%d, %s, %s, %uu>", T, bits ? "true" : "false", hasj ? "true" : "false", hp);
     return cached(kJitSource, expr, {"-DISING_JIT_B=" + std::to_string(B) + "u", "-DISING_JIT_R=" + std::to_string(R) + "u",
                                      "-DISING_G2_THREADS=" + std::to_string(threads), "-DISING_G2_BLOCKS=" + std::to_string(blocks),
-                                     park ? "-DISING_G2_PARK=1" : "-DISING_G2_PARK=0", series ? "-DISING_G2_SERIES=1" : "-DISING_G2_SERIES=0"});
+                                     park ? "-DISING_G2_PARK=1" : "-DISING_G2_PARK=0", series ? "-DISING_G2_SERIES=1" : "-DISING_G2_SERIES=0", "-DISING_G2_STRIP=" + std::to_string(strip)});
 }
 
 // The 3D kernel specialised for (BITS, HP3 = the three threshold heads).

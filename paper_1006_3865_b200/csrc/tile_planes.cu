@@ -1012,7 +1012,9 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit, bool 
     // its 28 warps per SM lose to the 40 of the per-pass kernels where those are not HBM-bound.  Measured at L = 16384, on
     // chip against the best other path, flips/ns: tile 64 int8 k = 1 / 2 / 4 / 16: 2896 / 3109 / 3232 / 3404 against 2486 /
     // 2962 / 3233 / 3491, bits k = 1 / 4: 3026 / 3369 against 2942 / 3315; tile 32 int8 k = 1 / 2 / 4: 2380 / 2815 / 3044
-    // against 2100 / 2858 / 3185, bits k = 1: 2480 against 2836.  Hence: tile 64 up to k = 3, tile 32 int8 at k = 1.
+    // against 2100 / 2858 / 3185, bits k = 1: 2480 against 2836; tile 32 as strips (below), int8 k = 1 / 2 / 3 / 4: 2645 / 2983 /
+    // 3107 / 3175 against 2100 / 2867 / 3083 / 3194, bits k = 1 / 2: 2685 / 3033 against 2842 / 3186.  Hence: up to k = 3; at tile 32
+    // int8 records only.
     const uint32_t max_m = kGridMaxJobsPerWarp;
     constexpr size_t kSmemMax = 227 * 1024;
     for (uint32_t M = 1; M <= max_m; ++M) {
@@ -1020,7 +1022,8 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit, bool 
         if (warp_cap && warps_needed > warp_cap && M < kGridMaxJobsPerWarp) continue;
         if (M > 2 && !warp_cap) {
             if ((uint64_t)R.n * (uint64_t)R.P.k < 8u) break;
-            if (M > 4 && !(T == 64 ? R.P.k <= 3 : (R.P.k == 1 && !BITS))) break;      // measured at L = 16384, above
+            static const bool any = getenv("ISING_GRID_ANY") != nullptr;                   // tuning aid: on chip whatever k and layout
+            if (M > 4 && !(R.P.k <= 3 && (T == 64 || !BITS)) && !any) break;               // measured at L = 16384, above
         }
         const uint32_t w_sm = (warps_needed + (uint32_t)sms - 1) / (uint32_t)sms;
         int wpb = 0;
@@ -1032,7 +1035,13 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit, bool 
             wpb = (int)((w_sm + 3u) / 4u * 4u);
             park = park_mode != 0 && (size_t)wpb * 2u * M * (2u * PG<T>::NW + 7u) * lane_bytes <= kSmemMax;
             if (!park && (size_t)wpb * 2u * M * (2u * PG<T>::NW) * lane_bytes > kSmemMax) break;      // the lattice does not fit on chip
-            fn = (const void*)grid_jit_kernel(T, BITS, HASJ, R.P.hp, R.P.B, R.P.R, wpb * 32, 1, park, R.acc != nullptr);
+            // several jobs per warp: as a strip of adjacent tiles of one tile row where M divides the jobs of a row (ISING_G2_STRIP in
+            // grid_planes_device.cuh: left / right neighbours from the warp's own shared memory); ISING_G2_STRIP=0: testing aid
+            static const bool strip_ok = !(getenv("ISING_G2_STRIP") && atoi(getenv("ISING_G2_STRIP")) == 0);
+            const uint32_t jobs_per_row = (uint32_t)R.P.B / 2u / (uint32_t)(64 / T);
+            // tile 32 only: at tile 64 (twice the state per lane, half the exchanges per site) the extra code spills and loses 4 %
+            const int strip = (strip_ok && T == 32 && M >= 2 && jobs_per_row % M == 0) ? (int)M : 0;
+            fn = (const void*)grid_jit_kernel(T, BITS, HASJ, R.P.hp, R.P.B, R.P.R, wpb * 32, 1, park, R.acc != nullptr, strip);
             if (!fn) { shaped = false; M = 0; continue; }         // no run-time compiler: again with the pre-compiled kernel
             *used_jit = true;
         } else {

@@ -170,7 +170,7 @@ def test_config3_full_length_int8_equals_bits(P, orc, tile, k):
         done = p
         # int8 records at k = 1: the whole lattice on chip (a call of 8 passes or more), else the persistent data-flow
         # kernel; k > 1 and bit records: a launch per colour
-        # (launch_grid_one's rule, measured: on chip at tile 64 up to k = 3, at tile 32 for int8 records at k = 1)
+        # (launch_grid_one's rule, measured: on chip up to k = 3, at tile 32 for int8 records only)
         want = "tile_planes_i8" if k > 1 else ("grid_planes_i8" if n_call >= 8 else "flow_planes_i8")
         want_b = "grid_planes_bits" if (k == 1 and tile == 64 and n_call >= 8) else "tile_planes_bits"
         assert a.sweep_path() == want and b.sweep_path() == want_b

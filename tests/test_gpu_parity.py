@@ -750,7 +750,10 @@ def test_grid_resident_kernel_run_time_build_without_parked_constants():
     """The run-time build of the same kernel in the form that holds BASELINE config 3 on chip (one CTA per SM, geometry and
     threshold heads compiled in, up to 16 jobs of a colour per warp, the jobs' constants decoded in every phase instead of
     parked in shared memory: ISING_G2_PARK=0, a testing aid, forces that form on lattices the oracle finishes in seconds),
-    with and without the E / M series (two different builds), replicas (per-replica Philox keys) and +-J couplings."""
+    with and without the E / M series (two different builds), replicas (per-replica Philox keys) and +-J couplings.  Where the
+    jobs per warp divide the jobs of a tile row, tile 32 runs as strips (left / right neighbours from the warp's own shared
+    memory, ISING_G2_STRIP in grid_planes_device.cuh): caps 64 and 128 at L = 1024 (4 and 2 jobs per warp; 8 and 4 with two
+    replicas), cap 24 at L = 640 (a whole tile row per warp: the strip's ends are each other's neighbours)."""
     import os, subprocess, sys
     code = (
         "import numpy as np, paper_1006_3865_b200 as P\n"
@@ -758,7 +761,8 @@ def test_grid_resident_kernel_run_time_build_without_parked_constants():
         "import ising_workloads as W\n"
         "P.use_torch()\n"
         "for (L, T, k, n, seeds, bits, jseed, beta) in ((1024, 32, 1, 4, [5], False, None, 0.4406868), (768, 64, 2, 3, [6, 7], True, None, 0.44),\n"
-        "                                              (640, 32, 1, 3, [8], False, 5, 1.0), (1024, 64, 1, 5, [9], False, None, 0.4406868)):\n"
+        "                                              (640, 32, 1, 3, [8], False, 5, 1.0), (1024, 64, 1, 5, [9], False, None, 0.4406868),\n"
+        "                                              (1024, 32, 2, 3, [10, 11], True, None, 0.5)):\n"
         "    J = W.couplings(2, L, jseed) if jseed is not None else None\n"
         "    g = P.Ising(2, L, coupling=J, seeds=seeds); o = O.Oracle(2, L, seeds=seeds, J=J)\n"
         "    g.set_jit('on')\n"
@@ -772,7 +776,7 @@ def test_grid_resident_kernel_run_time_build_without_parked_constants():
         "    assert np.array_equal(np.asarray(g.copy_spins()).reshape(-1), np.asarray(o.spins()).reshape(-1))\n"
         "print('unparked ok')\n")
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
-    for cap in ("24", "100"):
+    for cap in ("24", "64", "128"):
         out = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, ISING_GRID_WARPS=cap, ISING_G2_PARK="0"),
                              capture_output=True, text=True, timeout=900)
         assert out.returncode == 0 and "unparked ok" in out.stdout, out.stderr[-2000:]
