@@ -103,6 +103,9 @@ __device__ __forceinline__ void half_sweep_masks(const PlaneArgs& A, TileRegs<T>
 // only the tile rows above and below, and the strip ends, go through the exchange records.  With the colour-C tiles of a row at
 // tx = 2 q + p, p = (ty + C) & 1, and the other colour's at 2 q' + 1 - p: p = 0: right neighbour q' = q, left q' = q - 1;
 // p = 1: left q' = q, right q' = q + 1 (tile 32: q = 2 job + sub).
+// (Tried without strips, any mapping: the other colour's job of the SAME index is always the warp's own neighbour, to the right
+// where p = 0, to the left where p = 1, so one of the two columns could always come from shared memory, halving the column
+// exchange.  Measured: config 3 tile 64 k = 1 2990 -> 2894 flips/ns, L = 4096 and 8192 unchanged or -1 %: dropped.)
 #ifndef ISING_G2_STRIP
 #define ISING_G2_STRIP 0
 #endif
