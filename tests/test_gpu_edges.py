@@ -207,6 +207,39 @@ def test_config3_full_length_int8_equals_bits(P, orc, tile, k):
     a.destroy(); b.destroy()
 
 
+@pytest.mark.parametrize("layout", ["int8", "bits"])
+@pytest.mark.parametrize("L,tile,k,jobs", [(4096, 32, 1, 1), (4096, 64, 2, 1), (8192, 32, 1, 4), (8192, 32, 3, 4), (8192, 64, 1, 2), (8192, 64, 3, 2)])
+def test_on_chip_kernel_equals_a_launch_per_colour_at_full_size(P, L, tile, k, jobs, layout):
+    """Lattices of 2^24 and 2^26 sites in the launch configurations the library chooses for them (run-time build of
+    k_grid_planes: `jobs` jobs of a colour per warp, at L = 8192 without parked constants and, at tile 32, as strips): the whole
+    call on chip against a launch per coarse colour (ising_force_path 2) — canonical spins compared on the device, E, M and the
+    series of the on-chip call against observables of the other.  Both paths are pinned to the oracle on small lattices
+    (test_gpu_parity.py); this checks the full-size geometry (147 CTAs, 28 warps each)."""
+    import torch
+    n = 9
+    a = P.Ising(2, L, seed=12); b = P.Ising(2, L, seed=12)
+    if layout == "bits":
+        a.set_layout(P.ISING_LAYOUT_BITS); b.set_layout(P.ISING_LAYOUT_BITS)
+    b.force_path(2)
+    sfx = "i8" if layout == "int8" else "bits"
+    a.sweep(BC2, n, tile, k); b.sweep(BC2, n, tile, k)
+    assert a.sweep_path() == f"grid_planes_{sfx}" and a.last_sweep_specialized() and b.sweep_path() == f"tile_planes_{sfx}"
+    sa = torch.empty(L * L, dtype=torch.int8, device="cuda"); sb = torch.empty_like(sa)
+    a.copy_spins(sa); b.copy_spins(sb)
+    assert torch.equal(sa, sb), "on-chip kernel and per-colour launches differ"
+    E, M = a.sweep_series(BC2, n, tile, k)                  # the series build of the same kernel
+    assert a.sweep_path() == f"grid_planes_{sfx}"
+    b.sweep(BC2, n - 1, tile, k)
+    Eb, Mb = b.observables()
+    assert (int(E[n - 2][0]), int(M[n - 2][0])) == (int(Eb[0]), int(Mb[0]))
+    b.sweep(BC2, 1, tile, k)
+    a.copy_spins(sa); b.copy_spins(sb)
+    assert torch.equal(sa, sb)
+    Ea, Ma = a.observables(); Eb, Mb = b.observables()
+    assert (int(Ea[0]), int(Ma[0])) == (int(Eb[0]), int(Mb[0])) == (int(E[n - 1][0]), int(M[n - 1][0]))
+    a.destroy(); b.destroy()
+
+
 @pytest.mark.parametrize("dim,L,tile", [(2, 128, 32), (2, 64, 0), (3, 16, 8), (2, 1024, 32)])
 def test_thresholds_straddling_2p32(P, orc, dim, L, tile):
     """0 < beta < ~1.4e-17: exp(-4 beta) rounds to 1 (thr[1] = 2^32: always accept) while exp(-8 beta) does not
