@@ -650,7 +650,7 @@ bool grid3d_supported(const ising_ctx* h, int T) {
 
 namespace {
 // One cooperative launch with M = 1 or 2 jobs of each colour per warp.  The run-time build (bits/hp3 given) is compiled
-// for the CTA shape the lattice wants: ONE CTA per SM with ceil(warps / SMs) warps, rounded up to a multiple of four, so
+// for the CTA shape the lattice wants: ONE CTA per SM with ceil(warps / SMs) warps (rounding them up to a multiple of four gains nothing, measured), so
 // that every SM and every scheduler carries the same number of jobs (config 4: 4096 jobs per colour = 28 warps on each
 // SM, one job per warp, 72 registers).  Measured on config 4, k = 1 / 4 / 16: 5 CTAs of 4 warps with two jobs per warp
 // 1684 / - / -; 4 CTAs of 7 warps 1917 / 2338 / 2382; 7 CTAs of 4 warps 1855 / 2201 / 2269; one CTA of 28 warps
@@ -671,7 +671,7 @@ int launch_grid3d_one(Grid3Args& R, bool want_jit, unsigned long long hp3, int r
         int wpb, bps;
         const void* fn = nullptr;
         if (want_jit && !HASJ && w_sm <= wsm_cap) {
-            wpb = (int)((w_sm + 3u) / 4u * 4u); bps = 1;         // one CTA per SM, the same number of warps on every scheduler
+            wpb = (int)w_sm; bps = 1;         // one CTA per SM
             fn = (const void*)grid3d_jit_kernel(BITS, hp3, reps, wpb * 32, bps, R.acc != nullptr);
         }
         if (fn) *used_jit = true;

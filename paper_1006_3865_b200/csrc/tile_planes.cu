@@ -998,7 +998,7 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit, bool 
         }
     }
     // Specialised on the threshold head bits (planes_jit.cu) when asked for and available; that build also takes the CTA
-    // shape the lattice wants: ONE CTA per SM with ceil(warps / SMs) warps, rounded up to a multiple of four, so that every
+    // shape the lattice wants: ONE CTA per SM with ceil(warps / SMs) warps (rounding them up to a multiple of four loses SMs: -2 % at L = 4096, tile 64), so that every
     // SM and every scheduler carries the same number of jobs (as launch_grid3d_one, measured there).
     *fits = false; *used_jit = false;
     static const uint32_t warp_cap = getenv("ISING_GRID_WARPS") ? (uint32_t)atoi(getenv("ISING_GRID_WARPS")) : 0u;   // testing aid: several jobs per warp on small lattices
@@ -1032,7 +1032,7 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit, bool 
         const size_t lane_bytes = 32u * sizeof(uint32_t);
         if (shaped) {
             if (w_sm > wsm_cap) continue;                         // more jobs per warp
-            wpb = (int)((w_sm + 3u) / 4u * 4u);
+            wpb = (int)w_sm;
             park = park_mode != 0 && (size_t)wpb * 2u * M * (2u * PG<T>::NW + 7u) * lane_bytes <= kSmemMax;
             if (!park && (size_t)wpb * 2u * M * (2u * PG<T>::NW) * lane_bytes > kSmemMax) break;      // the lattice does not fit on chip
             // several jobs per warp: as a strip of adjacent tiles of one tile row where M divides the jobs of a row (ISING_G2_STRIP in
