@@ -244,22 +244,26 @@ __global__ void __launch_bounds__(256) k_canon_to_planes_i8(const int8_t* __rest
     }
 }
 
+// Records -> canonical rows.  A lane owns a block row (two tile rows), so a direct store would scatter every 16-byte store
+// instruction over 32 different rows (round 1: 3.4 TB/s, LG throttle 19.5 per issue); the tile is therefore staged in shared
+// memory (per warp, 128-byte blocks of 8 swizzled 16-byte chunks: conflict-free both ways) and written out as whole rows.
 template <int T>
 __global__ void __launch_bounds__(256) k_planes_i8_to_canon(int8_t* __restrict__ canon, const uint8_t* __restrict__ tiles,
                                                             int L, int B, uint32_t ntiles) {
     using G = PG<T>;
+    __shared__ __align__(16) uint8_t stage_all[8][4096];
     const int lane = threadIdx.x & 31;
     const uint32_t warp = (uint32_t)((blockIdx.x * blockDim.x + threadIdx.x) >> 5);
     const uint32_t tile = warp * G::TPW + (uint32_t)(lane / G::LPT);
     const int Y = lane % G::LPT;
-    if (tile >= ntiles) return;
-    const uint32_t per_rep = (uint32_t)B * B;
-    const uint32_t r = tile / per_rep, t2 = tile - r * per_rep;
-    const int ty = (int)(t2 / B), tx = (int)(t2 - (uint32_t)ty * B);
+    if (tile >= ntiles) return;                              // whole warps only: ntiles is even
+    uint8_t* stage = stage_all[threadIdx.x >> 5];
     const uint8_t* rec = tiles + (size_t)tile * G::REC_I8;
+    // where chunk c (16 bytes) of row 2Y + rp of this lane's tile goes
+    const int blk = T == 64 ? Y : lane >> 1;
+    auto slot = [&](int rp, int c) { return blk * 128 + ((((T == 64 ? rp * 4 : (lane & 1) * 4 + rp * 2) + c) ^ (blk & 7)) << 4); };
 #pragma unroll
     for (int rp = 0; rp < 2; ++rp) {
-        int8_t* rowp = canon + (size_t)r * L * L + (size_t)(ty * T + 2 * Y + rp) * L + (size_t)tx * T;
 #pragma unroll
         for (int gx = 0; gx < G::NW; ++gx) {
             // even bytes of the run = colour rp, odd bytes = colour 1 - rp
@@ -281,9 +285,24 @@ __global__ void __launch_bounds__(256) k_planes_i8_to_canon(int8_t* __restrict__
             }
 #pragma unroll
             for (int i = 0; i < 8; ++i) w[i] = ((w[i] ^ 0x01010101u) * 255u) | w[i];   // 1 -> 0x01, 0 -> 0xff
-            *reinterpret_cast<uint4*>(rowp + 32 * gx) = make_uint4(w[0], w[1], w[2], w[3]);
-            *reinterpret_cast<uint4*>(rowp + 32 * gx + 16) = make_uint4(w[4], w[5], w[6], w[7]);
+            *reinterpret_cast<uint4*>(stage + slot(rp, 2 * gx)) = make_uint4(w[0], w[1], w[2], w[3]);
+            *reinterpret_cast<uint4*>(stage + slot(rp, 2 * gx + 1)) = make_uint4(w[4], w[5], w[6], w[7]);
         }
+    }
+    __syncwarp();
+    // out: instruction i writes bytes [512 i, 512 i + 512) of the warp's tiles in row-major order, 16 bytes per lane
+    const uint32_t per_rep = (uint32_t)B * B;
+#pragma unroll
+    for (int i = 0; i < G::TPW * T * T / 512; ++i) {
+        const int s = (512 * i) / (T * T), o = (512 * i) % (T * T) + 16 * lane;
+        const int row = o / T, c = (o % T) >> 4, y = row >> 1, rp = row & 1;
+        const int lsrc = s * G::LPT + y, bsrc = T == 64 ? y : lsrc >> 1;
+        const int src = bsrc * 128 + ((((T == 64 ? rp * 4 : (lsrc & 1) * 4 + rp * 2) + c) ^ (bsrc & 7)) << 4);
+        const uint32_t tl = warp * G::TPW + (uint32_t)s;
+        const uint32_t r = tl / per_rep, t2 = tl - r * per_rep;
+        const int ty = (int)(t2 / B), tx = (int)(t2 - (uint32_t)ty * B);
+        int8_t* dst = canon + (size_t)r * L * L + (size_t)(ty * T + row) * L + (size_t)tx * T + 16 * c;
+        *reinterpret_cast<uint4*>(dst) = *reinterpret_cast<const uint4*>(stage + src);
     }
 }
 
