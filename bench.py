@@ -78,8 +78,10 @@ NCU = {
     ("planes", "int8", 32, 1, "flow"): {"traffic": (803.52e6 + 798.38e6) / 6, "warp_instr": 246.42e6 / 6, "fp": "7acfaaf12164", "source": "profiles/r02c_flow_planes_i8.md"},
     ("planes", "int8", 64, 1, "tile"): {"traffic": 138.44e6 + 80.40e6, "warp_instr": 33.73e6, "fp": "7acfaaf12164", "source": "profiles/r02c_flow_planes_i8.md"},
     ("planes", "int8", 64, 1, "grid"): {"traffic_call": 277.03e6 + 222.71e6, "warp_instr_call": 480.83e6 - 8 * 58.560e6, "warp_instr_pass": 58.560e6,
+                                        "pipes_16_passes": {"alu": 0.617, "fmaheavy": 0.598, "issue_active": 0.549},
                                         "fp": "3fbc907deeb1", "source": "profiles/r02e_grid_planes_L16384.md"},
     ("planes", "int8", 32, 1, "grid"): {"traffic_call": 321.08e6 + 255.54e6, "warp_instr_call": 581.98e6 - 8 * 70.146e6, "warp_instr_pass": 70.146e6,
+                                        "pipes_16_passes": {"alu": 0.615, "fmaheavy": 0.610, "issue_active": 0.585},
                                         "fp": "3fbc907deeb1", "source": "profiles/r02e_grid_planes_L16384.md"},
 }
 
@@ -593,6 +595,9 @@ def main() -> None:
         # SURVEY 8(d) (what a kernel that streams the lattice every pass must move) is kept beside it for comparison.
         roof = dict(issue) if issue else {"bound": "alu", "unit": "G warp-instr/s", "achieved": None, "peak": issue_peak_gips(sm_max), "frac": None}
         roof.update(common)
+        if ncu and "pipes_16_passes" in ncu:        # hardware counters of the committed 16-pass capture (not of this run)
+            roof["ncu_pipe_utilisation"] = dict(ncu["pipes_16_passes"], source=ncu["source"] + ": sm__pipe_alu_cycles_active, "
+                                                "sm__pipe_fmaheavy_cycles_active, sm__issue_active (.avg.pct_of_peak_sustained_elapsed / 100)")
         roof["launch_unit"] = ("one phase (coarse colour of a pass) of the cooperative launch that keeps the lattice on chip: CUDA-event time "
                                "of the call / (2 * steps), the load and the store of the lattice (once per call) included")
         roof["hbm_algorithmic"] = dict(hbm, note="bytes a kernel that streams the lattice every pass would move (SURVEY 8(d)) / measured time: "
