@@ -220,6 +220,9 @@ uint64_t ising_kernel_launches(void);
  *   resident_masked_*, tile_masked_*, resident3d_masked_*, tile3d_masked_*
  *                           double checkerboard with power-of-two tiles other than the register tiles (2D: 2, 4, 8, 16 —
  *                           the paper's sizes, P:86 — and 128, 256, ...; 3D: 2, 4, 16, 32, ...) as masked half-sweeps
+ *   grid_plain_*, grid_masked_*   the same two schemes for 2D lattices beyond the cluster, up to 2^24 sites, in calls of four
+ *                           sweeps or more: every half-sweep of the call in one cooperative launch, the lattice on chip on all
+ *                           SMs, every tile exchanging its boundary after every half-sweep (k_grid_plain)
  *   grid_planes_{i8,bits}, grid3d_planes_{i8,bits}   lattices beyond the cluster that fit in the shared memory of the GPU (2D
  *                           512 < L, up to 2^28 sites on a B200 where measured to pay: DESIGN.md §6.1g; 3D 64 < L): the whole
  *                           call in one cooperative launch, the lattice read from and written to HBM once per call, boundary

@@ -467,6 +467,14 @@ int path_plain2d(SweepCall& c) {
     const bool resident = Tp != 0;
     if (!Tp) Tp = tile_planes_supported(h, 64) ? 64 : (tile_planes_supported(h, 32) ? 32 : 0);
     if (!Tp) return kSkip;
+    // k_grid_plain (below) wants the 32 x 32 register tiling: at 64 x 64 its unspecialised compare spills under the 72 registers of
+    // 28 warps per SM
+    // (measured: with every tile exchanging its boundary after every half-sweep the on-chip form wins up to
+    // 2^24 sites — 1.3 ... 2.3 x — and loses to the launch per half-sweep from 2^26 on, where that one is HBM-bound at 70 %)
+    const bool grid_ok = !resident && !c.want_series && onchip_ok(h) && (uint64_t)c.n * (uint64_t)c.k * (c.Tc2 ? 2u : 1u) >= 4u &&
+                         (uint64_t)h->R * h->N <= (1ull << 24);
+    static const int plain_T = getenv("ISING_GRID_PLAIN_T") ? atoi(getenv("ISING_GRID_PLAIN_T")) : 32;       // tuning aid
+    if (grid_ok && tile_planes_supported(h, plain_T) && grid_planes_supported(h, plain_T)) Tp = plain_T;
     int rc = ensure_store(h, c.bits ? Store::PlaneBits : Store::PlaneI8, Tp);
     if (!rc) rc = ensure_couplings(h, false, Tp);
     if (rc) return rc;
@@ -476,6 +484,15 @@ int path_plain2d(SweepCall& c) {
             return kDone;
         }
         cudaGetLastError();          // the cluster did not fit: a launch per half-sweep
+    }
+    // beyond the cluster, while the lattice fits the shared memory of the GPU: every half-sweep of the call in one cooperative
+    // launch (k_grid_plain); a call of a few half-sweeps does not pay for loading and storing the lattice once
+    if (grid_ok && grid_planes_supported(h, Tp)) {
+        rc = ensure_scratch(&h->d_xedge, &h->xedge_bytes, grid_plain_xedge_bytes(h, Tp));
+        if (rc) return rc;
+        const int g = launch_grid_plain(h, c.acc, Tp, c.bits, c.n, c.k, h->t, c.Tc2, h->d_xedge);
+        if (g == 0) { h->last_path = path_name(c.Tc2 ? "grid_masked" : "grid_plain", c.bits); return kDone; }
+        if (g != 1) return g;
     }
     h->last_path = path_name(c.Tc2 ? "tile_masked" : "tile_plain", c.bits);
     return per_pass(c, [&](uint64_t t0) { return launch_tile_planes_plain(h, c.acc, Tp, c.bits, 1, c.k, t0, c.Tc2); });

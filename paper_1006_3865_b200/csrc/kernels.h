@@ -43,6 +43,9 @@ int launch_resident_planes(ising_ctx* h, const Accept& acc, int T, bool bits, in
 
 bool grid_planes_supported(const ising_ctx* h, int T);          // 512 < L <= ~4096: the whole call in one launch, every tile in registers on all SMs
 size_t grid_planes_xedge_bytes(const ising_ctx* h, int T);
+size_t grid_plain_xedge_bytes(const ising_ctx* h, int T);      // k_grid_plain: two exchange records per tile
+// a8 / coarse tiles on chip on all SMs (k_grid_plain): 0 = done, 1 = does not fit or refused (nothing launched)
+int launch_grid_plain(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, int Tc, void* d_xedge);
 size_t grid_planes_acc_bytes(const ising_ctx* h, int n);
 int launch_grid_planes(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, void* d_xedge, void* d_acc,
                        long long* d_E, long long* d_M, bool use_jit, bool allow_pc);   // returns 1 (nothing launched) if the lattice does not fit;

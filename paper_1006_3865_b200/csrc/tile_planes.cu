@@ -1149,6 +1149,229 @@ bool grid_planes_supported(const ising_ctx* h, int T) {
     return jobs <= 148u * 32u * kGridMaxJobsPerWarp;
 }
 
+// ---- k_grid_plain: the plain checkerboard (a8, tile == L) and the double checkerboard of coarse tiles other than the
+// register tiles (the paper's own T = 2 ... 16; 128, ...) on chip on all SMs, beyond the cluster-resident kernel.
+// With a launch per half-sweep the whole lattice crosses HBM twice per half-sweep and small lattices pay a launch
+// latency per half-sweep (L = 1024: 125 flips/ns).  Here, as in k_grid_planes, one cooperative launch keeps every register
+// tile in shared memory for the whole call; but EVERY tile takes part in every phase (a phase = one half-sweep of fine
+// colour c of the whole lattice, masked to the coarse colour Cc where there are coarse tiles), so a tile's neighbours are
+// being updated while it is.  A tile therefore keeps TWO exchange records, used in turn: phase p reads the neighbours'
+// version p + 1 from record (p + 1) & 1 and writes its own version p + 2 into record p & 1, which held version p — read
+// by the neighbours in their phase p - 1, which they had finished before they published the version p + 1 this tile has
+// just waited for.  No grid barrier.
+template <int T, bool BITS, bool HASJ>
+__global__ void __launch_bounds__(896, 1) k_grid_plain(GridArgs R, int Tc, int split) {
+    using G = PG<T>;
+    constexpr int NWORDS = 2 * G::NW;                         // words per lane and job, nothing else is parked
+    extern __shared__ uint32_t grid_plain_smem[];             // per warp: [colour][job][word][lane]
+    const PlaneArgs& A = R.P;
+    const int lane = threadIdx.x & 31, wic = threadIdx.x >> 5;
+    // split (small lattices): a warp owns jobs of ONE colour of register tiles (the parity of its index), so that twice as many
+    // warps share a phase; else warp w owns the jobs w, w + W, ... of both
+    const uint32_t wg_all = blockIdx.x * (blockDim.x >> 5) + (uint32_t)wic, W_all = gridDim.x * (blockDim.x >> 5);
+    const uint32_t wg = split ? wg_all >> 1 : wg_all, W = split ? W_all >> 1 : W_all;
+    const int C0 = split ? (int)(wg_all & 1u) : 0, C1 = split ? C0 + 1 : 2;
+    const int sub = lane / G::LPT, Y = lane % G::LPT;
+    const uint32_t B = (uint32_t)A.B, Mw = R.jobs_per_warp;
+    uint32_t* const ws = grid_plain_smem + (size_t)wic * (2u * Mw * NWORDS * 32u) + lane;
+    const uint2* lut = kByteLutGlobal.e;
+
+    struct Job { int r, tx, ty; uint32_t self, nU, nD, nL, nR; };
+    auto decode = [&](uint32_t job, int C) {
+        int ri, txi, tyi;
+        job_tile<T>(A, job, sub, ri, txi, tyi, C);
+        const uint32_t r = (uint32_t)ri, tx = (uint32_t)txi, ty = (uint32_t)tyi;
+        const uint32_t base = r * B * B, row = base + ty * B;
+        const uint32_t tyU = ty == 0 ? B - 1 : ty - 1, tyD = ty == B - 1 ? 0 : ty + 1;
+        const uint32_t txL = tx == 0 ? B - 1 : tx - 1, txR = tx == B - 1 ? 0 : tx + 1;
+        return Job{(int)r, (int)tx, (int)ty, row + tx, base + tyU * B + tx, base + tyD * B + tx, row + txL, row + txR};
+    };
+    // record of tile i for version v: 16 u64 = TOP[4] | {L0, L1, R0, R1} | BOT[4] | pad, u64 = version << 32 | word
+    auto rec = [&](uint32_t i, uint32_t v) { return R.xedge + ((size_t)i * 2u + (v & 1u)) * 16u; };
+    auto publish = [&](const TileRegs<T>& tt, const Job& jb, uint32_t ver) {
+        const uint32_t sh = (uint32_t)sub * G::LPT, msk = G::LPT == 32 ? 0xffffffffu : ((1u << G::LPT) - 1u);
+        const uint32_t L0 = (__ballot_sync(0xffffffffu, tt.S[0][0] & 1u) >> sh) & msk;
+        const uint32_t L1 = (__ballot_sync(0xffffffffu, (tt.S[1][0] >> 16) & 1u) >> sh) & msk;
+        const uint32_t R0 = (__ballot_sync(0xffffffffu, (tt.S[1][G::NW - 1] >> 15) & 1u) >> sh) & msk;
+        const uint32_t R1 = (__ballot_sync(0xffffffffu, tt.S[0][G::NW - 1] >> 31) >> sh) & msk;
+        const unsigned long long v = (unsigned long long)ver << 32;
+        unsigned long long* e = rec(jb.self, ver);
+        if (Y == 0 || Y == G::LPT - 1) {
+            unsigned long long* rw = e + (Y == 0 ? 0 : 8);          // TOP : BOT
+            if (G::NW == 2) {
+                st_xedge2(rw, v | tt.S[0][0], v | tt.S[0][1]);
+                st_xedge2(rw + 2, v | tt.S[1][0], v | tt.S[1][1]);
+            } else {
+                st_xedge2(rw, v | tt.S[0][0], v | tt.S[1][0]);
+            }
+        }
+        if (Y == 0) {
+            st_xedge2(e + 4, v | L0, v | L1);
+            st_xedge2(e + 6, v | R0, v | R1);
+        }
+    };
+    auto refresh = [&](TileRegs<T>& tt, const Job& jb, uint32_t want) {
+        const unsigned long long* rowp = rec(Y == 0 ? jb.nU : jb.nD, want) + (Y == 0 ? 8 : 0);     // BOT of the tile above : TOP of the tile below
+        const unsigned long long* lf = rec(jb.nL, want) + 6;                                       // {R0, R1}
+        const unsigned long long* rt = rec(jb.nR, want) + 4;                                       // {L0, L1}
+        const bool need_row = Y == 0 || Y == G::LPT - 1;
+        for (;;) {
+            ulonglong2 r0 = make_ulonglong2(0, 0), r1 = r0;
+            const ulonglong2 a = ld_xedge2(lf), b = ld_xedge2(rt);
+            bool ok = (uint32_t)(a.x >> 32) == want && (uint32_t)(a.y >> 32) == want && (uint32_t)(b.x >> 32) == want && (uint32_t)(b.y >> 32) == want;
+            if (need_row) {
+                r0 = ld_xedge2(rowp);
+                ok = ok && (uint32_t)(r0.x >> 32) == want && (uint32_t)(r0.y >> 32) == want;
+                if (G::NW == 2) {
+                    r1 = ld_xedge2(rowp + 2);
+                    ok = ok && (uint32_t)(r1.x >> 32) == want && (uint32_t)(r1.y >> 32) == want;
+                }
+            }
+            if (__all_sync(0xffffffffu, ok)) {
+                tt.vrow[0][0] = (uint32_t)r0.x;
+                if (G::NW == 2) { tt.vrow[0][1] = (uint32_t)r0.y; tt.vrow[1][0] = (uint32_t)r1.x; tt.vrow[1][1] = (uint32_t)r1.y; }
+                else tt.vrow[1][0] = (uint32_t)r0.y;
+                tt.hL0 = ((uint32_t)a.x >> Y) & 1u; tt.hL1 = ((uint32_t)a.y >> Y) & 1u;
+                tt.hR0 = ((uint32_t)b.x >> Y) & 1u; tt.hR1 = ((uint32_t)b.y >> Y) & 1u;
+                return;
+            }
+        }
+    };
+    auto slot = [&](int C, uint32_t m) { return ws + (size_t)((uint32_t)C * Mw + m) * (NWORDS * 32u); };
+    auto sm_load = [&](TileRegs<T>& tt, int C, uint32_t m) {
+        const uint32_t* p = slot(C, m);
+#pragma unroll
+        for (int i = 0; i < NWORDS; ++i) tt.S[i / G::NW][i % G::NW] = p[i * 32];
+    };
+    auto sm_store = [&](const TileRegs<T>& tt, int C, uint32_t m) {
+        uint32_t* p = slot(C, m);
+#pragma unroll
+        for (int i = 0; i < NWORDS; ++i) p[i * 32] = tt.S[i / G::NW][i % G::NW];
+    };
+
+    // records -> shared memory; every tile publishes its boundary as version 1 (what phase 0 waits for)
+    for (int C = C0; C < C1; ++C)
+        for (uint32_t m = 0; m < Mw; ++m) {
+            const uint32_t job = wg + m * W;
+            if (job >= R.jobs_total) break;                               // warp-uniform
+            const Job jb = decode(job, C);
+            TileRegs<T> tt;
+            load_tile<T, BITS>(A, jb.r, jb.tx, jb.ty, Y, sub * G::LPT, tt);
+            sm_store(tt, C, m);
+            publish(tt, jb, 1u);
+        }
+    uint32_t ph = 0;                                                      // phases done: waits for version ph + 1, publishes ph + 2
+    for (int pass = 0; pass < R.n; ++pass)
+        for (int Cc = 0; Cc < (Tc ? 2 : 1); ++Cc)                         // (coarse tiles: both coarse colours in turn)
+            for (int j = 0; j < A.k; ++j) {
+                const uint64_t t64 = A.t_first + (uint64_t)pass * (uint64_t)A.k + (uint64_t)j;
+                for (int c = 0; c < 2; ++c, ++ph)
+                    for (int C = C0; C < C1; ++C)
+#pragma unroll 1
+                        for (uint32_t m = 0; m < Mw; ++m) {
+                            const uint32_t job = wg + m * W;
+                            if (job >= R.jobs_total) break;
+                            const Job jb = decode(job, C);
+                            TileRegs<T> tt;
+                            sm_load(tt, C, m);
+                            uint4 Jw[2][G::NW];
+#pragma unroll
+                            for (int cc = 0; cc < 2; ++cc)
+#pragma unroll
+                                for (int gx = 0; gx < G::NW; ++gx)
+                                    Jw[cc][gx] = HASJ ? __ldg(A.jrec + ((size_t)jb.ty * B + jb.tx) * (2 * G::NW * G::LPT) + (cc * G::NW + gx) * G::LPT + Y)
+                                                      : make_uint4(0u, 0u, 0u, 0u);
+                            refresh(tt, jb, ph + 1u);
+                            const uint64_t seed = A.seeds[jb.r];
+                            const uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+                            const uint32_t Yg = (uint32_t)(jb.ty * G::LPT + Y);
+                            const uint32_t g0 = Yg * (B * G::NW) + (uint32_t)(jb.tx * G::NW);
+                            const uint32_t p0 = 2u * Yg * (B * (uint32_t)(T / 2)) + 16u * (uint32_t)(jb.tx * G::NW);
+                            half_sweep_masked<T, HASJ>(A, tt, Jw, c, Y, g0, p0, 2 * t64 + (uint64_t)c, k0, k1, Tc, Yg, (uint32_t)(jb.tx * G::NW), Cc);
+                            publish(tt, jb, ph + 2u);
+                            sm_store(tt, C, m);
+                        }
+            }
+    for (int C = C0; C < C1; ++C)
+        for (uint32_t m = 0; m < Mw; ++m) {
+            const uint32_t job = wg + m * W;
+            if (job >= R.jobs_total) break;
+            const Job jb = decode(job, C);
+            TileRegs<T> tt;
+            sm_load(tt, C, m);
+            store_tile<T, BITS>(A, jb.r, jb.tx, jb.ty, Y, sub, tt, lut);
+        }
+}
+
+size_t grid_plain_xedge_bytes(const ising_ctx* h, int T) { return 2 * grid_planes_xedge_bytes(h, T); }
+
+// n passes (of k sweeps each) of the plain checkerboard (Tc = 0) or of the double checkerboard of coarse tiles Tc in one
+// cooperative launch; returns 1 (nothing launched) if the lattice does not fit the shared memory of the GPU or the launch
+// is refused.  d_xedge: grid_plain_xedge_bytes.
+int launch_grid_plain(ising_ctx* h, const Accept& acc, int T, bool bits, int n, int k, uint64_t t_first, int Tc, void* d_xedge) {
+    GridArgs R;
+    PlaneArgs& A = R.P;
+    A.tiles = (uint8_t*)h->d_tiles;
+    A.seeds = h->d_sweep_seeds;
+    A.seed0 = h->shared_sweep ? h->sweep_seed : h->seeds[0];
+    A.L = h->L; A.B = h->L / T; A.R = h->R; A.k = k; A.t_first = t_first; A.C = 0;
+    A.jrec = h->has_J ? (const uint4*)h->d_Jtiles : nullptr;
+    A.stream = 0;
+    A.njobs = 0;
+    A.magic_rep = fastdiv_magic((uint32_t)A.B * (uint32_t)A.B / 2u);
+    A.magic_hb = fastdiv_magic((uint32_t)A.B / 2u);
+    fill_accept(A, acc);
+    R.n = n;
+    R.magic_k = 0;
+    R.tiles_per_colour = (uint32_t)A.B * (uint32_t)A.B / 2u;
+    R.jobs_total = (uint32_t)h->R * R.tiles_per_colour / (uint32_t)(64 / T);
+    R.xedge = (unsigned long long*)d_xedge;
+    R.acc = nullptr;
+    // versions are 32 bits wide: two per phase
+    if ((uint64_t)n * (uint64_t)(Tc ? 2 : 1) * (uint64_t)k * 2u + 2u >= 0xffffffffull) return 1;
+    int dev = 0, sms = 0;
+    ISING_CUDA_OK(cudaGetDevice(&dev));
+    ISING_CUDA_OK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const void* fn = T == 64 ? (bits ? (A.jrec ? (const void*)k_grid_plain<64, true, true> : (const void*)k_grid_plain<64, true, false>)
+                                     : (A.jrec ? (const void*)k_grid_plain<64, false, true> : (const void*)k_grid_plain<64, false, false>))
+                             : (bits ? (A.jrec ? (const void*)k_grid_plain<32, true, true> : (const void*)k_grid_plain<32, true, false>)
+                                     : (A.jrec ? (const void*)k_grid_plain<32, false, true> : (const void*)k_grid_plain<32, false, false>));
+    constexpr size_t kSmemMax = 227 * 1024;
+    ISING_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax));
+    static const uint32_t warp_cap = getenv("ISING_GRID_WARPS") ? (uint32_t)atoi(getenv("ISING_GRID_WARPS")) : 0u;   // testing aid, as in launch_grid_one
+    const uint32_t nwords = 2u * (uint32_t)(T / 32);
+    // one job per warp and phase where the GPU holds a warp for every register-tile job of either colour
+    int split = (!warp_cap && 2u * R.jobs_total <= (uint32_t)sms * 28u) ? 1 : 0;
+    for (uint32_t M = 1; M <= kGridMaxJobsPerWarp; ++M) {
+        if (split && M > 1) split = 0, M = 1;
+        const uint32_t warps_needed = (split ? 2u : 1u) * ((R.jobs_total + M - 1) / M);
+        if (warp_cap && warps_needed > warp_cap && M < kGridMaxJobsPerWarp) continue;
+        const uint32_t w_sm = (warps_needed + (uint32_t)sms - 1) / (uint32_t)sms;
+        if (w_sm > 28u) continue;                                 // more jobs per warp
+        const int wpb = (int)((w_sm + 1u) & ~1u);                 // even: with split, the two colours alternate over the warp index
+        const size_t smem = (size_t)wpb * 2u * M * nwords * 32u * sizeof(uint32_t);
+        if (smem > kSmemMax) break;                               // the lattice does not fit on chip
+        int occ = 0;
+        ISING_CUDA_OK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, fn, wpb * 32, smem));
+        const uint32_t grid = (warps_needed + wpb - 1) / wpb;
+        if (grid > (uint32_t)sms * (uint32_t)occ) continue;
+        R.jobs_per_warp = M;
+        cudaStream_t st = hooks().stream;
+        ISING_CUDA_OK(cudaMemsetAsync(d_xedge, 0, grid_plain_xedge_bytes(h, T), st));      // version 0 = nothing published
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3(grid); cfg.blockDim = dim3(wpb * 32); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cudaLaunchAttribute attr[1];
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+        cfg.attrs = attr; cfg.numAttrs = 1;
+        void* args[] = {&R, &Tc, &split};
+        if (cudaLaunchKernelExC(&cfg, fn, args) != cudaSuccess) { cudaGetLastError(); return 1; }      // refused (shared or partitioned GPU)
+        count_launch();
+        return 0;
+    }
+    return 1;
+}
+
 // ---- k_flow_planes (flow_planes_device.cuh): all n passes of an HBM-resident lattice in one persistent launch ----
 namespace {
 template <int T, bool BITS, int NS>

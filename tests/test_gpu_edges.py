@@ -58,8 +58,11 @@ FAMILIES = {
     "grid3d": (3, 80, 8, 1, 4, BC3, None, "planes", "int8", 0, "off", "grid3d_planes_i8"),
     "grid3d_jit": (3, 80, 8, 2, 4, BC3, None, "planes", "bits", 0, "on", "grid3d_planes_bits"),
     "plain64": (2, 64, 0, 1, 6, BC2, None, "planes", "int8", 0, "auto", "plain64_planes_i8"),
-    "tile_plain": (2, 704, 0, 1, 4, BC2, None, "planes", "int8", 0, "auto", "tile_plain_i8"),
-    "tile_masked": (2, 704, 16, 1, 4, BC2, None, "planes", "bits", 0, "auto", "tile_masked_bits"),
+    "tile_plain": (2, 704, 0, 1, 4, BC2, None, "planes", "int8", 2, "auto", "tile_plain_i8"),
+    "tile_masked": (2, 704, 16, 1, 4, BC2, None, "planes", "bits", 2, "auto", "tile_masked_bits"),
+    "grid_plain": (2, 704, 0, 1, 4, BC2, None, "planes", "int8", 0, "auto", "grid_plain_i8"),
+    "grid_masked": (2, 704, 16, 1, 4, BC2, None, "planes", "bits", 0, "auto", "grid_masked_bits"),
+    "grid_masked_pmj": (2, 704, 8, 2, 2, 1.0, 5, "planes", "int8", 0, "auto", "grid_masked_i8"),
     "tile3d": (3, 32, 8, 2, 4, BC3, None, "planes", "int8", 2, "off", "tile3d_planes_i8"),
     "tile3d_jit": (3, 32, 8, 1, 4, BC3, None, "planes", "bits", 2, "on", "tile3d_planes_bits"),
     "tile3d_pmj": (3, 32, 8, 1, 4, 0.9, 7, "planes", "int8", 2, "off", "tile3d_planes_i8"),

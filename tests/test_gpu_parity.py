@@ -593,6 +593,41 @@ def test_plain_checkerboard_large_lattices(P, orc, L, k, n, beta, seeds, jseed, 
     _same_state(g, o)
     g.sweep(beta, 2, L, 1); o.sweep(beta, 2, L, 1)
     _same_state(g, o)
+    # a call of four sweeps or more: every half-sweep in one cooperative launch, the lattice on chip (k_grid_plain: every tile
+    # active in every phase, two exchange records per tile used in turn)
+    sfx = "i8" if layout == "int8" else "bits"
+    g.sweep(beta, 5, 0, k); o.sweep(beta, 5, 0, k)
+    assert g.sweep_path() == f"grid_plain_{sfx}"
+    _same_state(g, o)
+    g.sweep(beta, 4, L, 1); o.sweep(beta, 4, L, 1)              # again: the exchange records are reset per call
+    assert g.sweep_path() == f"grid_plain_{sfx}"
+    _same_state(g, o)
+
+
+def test_grid_plain_kernel_several_jobs_per_warp():
+    """k_grid_plain with the number of resident warps capped (ISING_GRID_WARPS, a testing aid): several register-tile jobs of
+    each colour per warp, as on lattices of 2^24 sites; fresh process because the cap is read once."""
+    import os, subprocess, sys
+    code = (
+        "import numpy as np, paper_1006_3865_b200 as P\n"
+        "from oracle import oracle as O\n"
+        "import ising_workloads as W\n"
+        "P.use_torch()\n"
+        "for (L, T, k, n, seeds, bits, jseed) in ((1024, 0, 1, 4, [5], False, None), (768, 16, 2, 2, [6, 7], True, None), (704, 8, 1, 3, [8], False, 5), (1024, 128, 1, 2, [9], True, None)):\n"
+        "    J = W.couplings(2, L, jseed) if jseed is not None else None\n"
+        "    g = P.Ising(2, L, coupling=J, seeds=seeds); o = O.Oracle(2, L, seeds=seeds, J=J)\n"
+        "    if bits: g.set_layout(P.ISING_LAYOUT_BITS)\n"
+        "    g.sweep(0.44, n, T, k); o.sweep(0.44, n, T, k)\n"
+        "    assert g.sweep_path().startswith('grid_plain' if T == 0 else 'grid_masked'), g.sweep_path()\n"
+        "    assert np.array_equal(np.asarray(g.copy_spins()).reshape(-1), np.asarray(o.spins()).reshape(-1))\n"
+        "    Eg, Mg = g.observables(); Eo, Mo = o.observables()\n"
+        "    assert list(Eg) == list(Eo) and list(Mg) == list(Mo)\n"
+        "print('capped ok')\n")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    for cap in ("24", "100"):
+        out = subprocess.run([sys.executable, "-c", code], cwd=root, env=dict(os.environ, ISING_GRID_WARPS=cap),
+                             capture_output=True, text=True, timeout=900)
+        assert out.returncode == 0 and "capped ok" in out.stdout, out.stderr[-2000:]
 
 
 @pytest.mark.parametrize("layout", ["int8", "bits"])
@@ -629,13 +664,16 @@ def test_plain_checkerboard_3d(P, orc, L, k, n, beta, seeds, jseed, path, layout
     (64, 2, 3, 2, 0.3, [8], None, "resident_masked"),
     (256, 16, 4, 2, 1.0, [100, 101], 5, "resident_masked"),  # +-J
     (512, 128, 2, 2, BC2, [11], None, "resident_masked"),    # tiles above 64: whole register tiles switched on and off
-    (1024, 256, 1, 2, 0.5, [12], None, "tile_masked"),
-    (1024, 128, 2, 1, BC2, [13], None, "tile_masked"),
-    (1024, 16, 1, 2, BC2, [9], None, "tile_masked"),
-    (704, 8, 2, 1, 0.5, [10], None, "tile_masked"),
+    (1024, 256, 1, 2, 0.5, [12], None, "grid_masked"),       # beyond the cluster: on chip on all SMs (k_grid_plain) ...
+    (1024, 128, 2, 1, BC2, [13], None, "grid_masked"),
+    (1024, 16, 1, 2, BC2, [9], None, "grid_masked"),
+    (704, 8, 2, 1, 0.5, [10, 11], None, "grid_masked"),
+    (704, 4, 1, 3, 1.0, [100], 5, "grid_masked"),            # +-J
+    (1024, 16, 1, 1, BC2, [9], None, "tile_masked"),         # ... unless the call is too short to pay for it: a launch per half-sweep
 ])
 def test_small_coarse_tiles_on_the_fast_kernels(P, orc, L, tile, k, n, beta, seeds, jseed, path, layout):
-    """Double checkerboard with coarse tiles smaller than a register tile: masked half-sweeps, same trajectory as the oracle's."""
+    """Double checkerboard with coarse tiles smaller than a register tile: masked half-sweeps, same trajectory as the oracle's
+    (the series call that follows takes a launch per half-sweep at the sizes beyond the cluster)."""
     J = W.couplings(2, L, jseed) if jseed is not None else None
     g, o = _both(P, orc, 2, L, seeds, J, rng="planes")
     if layout == "bits":
