@@ -1162,7 +1162,8 @@ bool grid_planes_supported(const ising_ctx* h, int T) {
 template <int T, bool BITS, bool HASJ>
 __global__ void __launch_bounds__(896, 1) k_grid_plain(GridArgs R, int Tc, int split) {
     using G = PG<T>;
-    constexpr int NWORDS = 2 * G::NW;                         // words per lane and job, nothing else is parked
+    constexpr int NWORDS = 2 * G::NW;                         // words per lane and job: S[cc][gx]
+    constexpr int NSLOT = NWORDS + 7;                         // ... + the job's constants (decoded once): self, nU, nD, nL, nR, tx | ty << 16, r
     extern __shared__ uint32_t grid_plain_smem[];             // per warp: [colour][job][word][lane]
     const PlaneArgs& A = R.P;
     const int lane = threadIdx.x & 31, wic = threadIdx.x >> 5;
@@ -1173,7 +1174,7 @@ __global__ void __launch_bounds__(896, 1) k_grid_plain(GridArgs R, int Tc, int s
     const int C0 = split ? (int)(wg_all & 1u) : 0, C1 = split ? C0 + 1 : 2;
     const int sub = lane / G::LPT, Y = lane % G::LPT;
     const uint32_t B = (uint32_t)A.B, Mw = R.jobs_per_warp;
-    uint32_t* const ws = grid_plain_smem + (size_t)wic * (2u * Mw * NWORDS * 32u) + lane;
+    uint32_t* const ws = grid_plain_smem + (size_t)wic * (2u * Mw * NSLOT * 32u) + lane;
     const uint2* lut = kByteLutGlobal.e;
 
     struct Job { int r, tx, ty; uint32_t self, nU, nD, nL, nR; };
@@ -1237,7 +1238,17 @@ __global__ void __launch_bounds__(896, 1) k_grid_plain(GridArgs R, int Tc, int s
             }
         }
     };
-    auto slot = [&](int C, uint32_t m) { return ws + (size_t)((uint32_t)C * Mw + m) * (NWORDS * 32u); };
+    auto slot = [&](int C, uint32_t m) { return ws + (size_t)((uint32_t)C * Mw + m) * (NSLOT * 32u); };
+    auto sm_job = [&](int C, uint32_t m) {                             // the constants parked by the prologue
+        const uint32_t* p = slot(C, m) + NWORDS * 32;
+        const uint32_t xy = p[5 * 32];
+        return Job{(int)p[6 * 32], (int)(xy & 0xffffu), (int)(xy >> 16), p[0], p[1 * 32], p[2 * 32], p[3 * 32], p[4 * 32]};
+    };
+    auto sm_put_job = [&](const Job& jb, int C, uint32_t m) {
+        uint32_t* p = slot(C, m) + NWORDS * 32;
+        p[0] = jb.self; p[1 * 32] = jb.nU; p[2 * 32] = jb.nD; p[3 * 32] = jb.nL; p[4 * 32] = jb.nR;
+        p[5 * 32] = (uint32_t)jb.tx | ((uint32_t)jb.ty << 16); p[6 * 32] = (uint32_t)jb.r;
+    };
     auto sm_load = [&](TileRegs<T>& tt, int C, uint32_t m) {
         const uint32_t* p = slot(C, m);
 #pragma unroll
@@ -1258,6 +1269,7 @@ __global__ void __launch_bounds__(896, 1) k_grid_plain(GridArgs R, int Tc, int s
             TileRegs<T> tt;
             load_tile<T, BITS>(A, jb.r, jb.tx, jb.ty, Y, sub * G::LPT, tt);
             sm_store(tt, C, m);
+            sm_put_job(jb, C, m);
             publish(tt, jb, 1u);
         }
     uint32_t ph = 0;                                                      // phases done: waits for version ph + 1, publishes ph + 2
@@ -1271,7 +1283,7 @@ __global__ void __launch_bounds__(896, 1) k_grid_plain(GridArgs R, int Tc, int s
                         for (uint32_t m = 0; m < Mw; ++m) {
                             const uint32_t job = wg + m * W;
                             if (job >= R.jobs_total) break;
-                            const Job jb = decode(job, C);
+                            const Job jb = sm_job(C, m);
                             TileRegs<T> tt;
                             sm_load(tt, C, m);
                             uint4 Jw[2][G::NW];
@@ -1296,7 +1308,7 @@ __global__ void __launch_bounds__(896, 1) k_grid_plain(GridArgs R, int Tc, int s
         for (uint32_t m = 0; m < Mw; ++m) {
             const uint32_t job = wg + m * W;
             if (job >= R.jobs_total) break;
-            const Job jb = decode(job, C);
+            const Job jb = sm_job(C, m);
             TileRegs<T> tt;
             sm_load(tt, C, m);
             store_tile<T, BITS>(A, jb.r, jb.tx, jb.ty, Y, sub, tt, lut);
@@ -1339,7 +1351,7 @@ int launch_grid_plain(ising_ctx* h, const Accept& acc, int T, bool bits, int n, 
     constexpr size_t kSmemMax = 227 * 1024;
     ISING_CUDA_OK(cudaFuncSetAttribute(fn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemMax));
     static const uint32_t warp_cap = getenv("ISING_GRID_WARPS") ? (uint32_t)atoi(getenv("ISING_GRID_WARPS")) : 0u;   // testing aid, as in launch_grid_one
-    const uint32_t nwords = 2u * (uint32_t)(T / 32);
+    const uint32_t nwords = 2u * (uint32_t)(T / 32) + 7u;      // spin words + the job's parked constants
     // one job per warp and phase where the GPU holds a warp for every register-tile job of either colour
     int split = (!warp_cap && 2u * R.jobs_total <= (uint32_t)sms * 28u) ? 1 : 0;
     for (uint32_t M = 1; M <= kGridMaxJobsPerWarp; ++M) {
