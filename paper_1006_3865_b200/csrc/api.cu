@@ -475,6 +475,9 @@ int path_plain2d(SweepCall& c) {
                          (uint64_t)h->R * h->N <= (1ull << 24);
     static const int plain_T = getenv("ISING_GRID_PLAIN_T") ? atoi(getenv("ISING_GRID_PLAIN_T")) : 32;       // tuning aid
     if (grid_ok && tile_planes_supported(h, plain_T) && grid_planes_supported(h, plain_T)) Tp = plain_T;
+    else if (!resident && (h->store == Store::PlaneI8 || h->store == Store::PlaneBits) && (h->store_tile == 32 || h->store_tile == 64) &&
+             tile_planes_supported(h, h->store_tile))
+        Tp = h->store_tile;          // short calls and series between long ones: keep the register tiling the records are in
     int rc = ensure_store(h, c.bits ? Store::PlaneBits : Store::PlaneI8, Tp);
     if (!rc) rc = ensure_couplings(h, false, Tp);
     if (rc) return rc;
