@@ -79,10 +79,10 @@ NCU = {
     ("planes", "int8", 64, 1, "tile"): {"traffic": 138.44e6 + 80.40e6, "warp_instr": 33.73e6, "fp": "7acfaaf12164", "source": "profiles/r02c_flow_planes_i8.md"},
     ("planes", "int8", 64, 1, "grid"): {"traffic_call": 277.03e6 + 222.71e6, "warp_instr_call": 480.83e6 - 8 * 58.560e6, "warp_instr_pass": 58.560e6,
                                         "pipes_16_passes": {"alu": 0.617, "fmaheavy": 0.598, "issue_active": 0.549},
-                                        "fp": "3fbc907deeb1", "source": "profiles/r02e_grid_planes_L16384.md"},
+                                        "fp": "c1c009a23ee4", "source": "profiles/r02e_grid_planes_L16384.md"},
     ("planes", "int8", 32, 1, "grid"): {"traffic_call": 321.08e6 + 255.54e6, "warp_instr_call": 581.98e6 - 8 * 70.146e6, "warp_instr_pass": 70.146e6,
                                         "pipes_16_passes": {"alu": 0.615, "fmaheavy": 0.610, "issue_active": 0.585},
-                                        "fp": "3fbc907deeb1", "source": "profiles/r02e_grid_planes_L16384.md"},
+                                        "fp": "c1c009a23ee4", "source": "profiles/r02e_grid_planes_L16384.md"},
 }
 
 

@@ -323,7 +323,7 @@ __global__ void __launch_bounds__(PC ? 256 : ISING_G2_THREADS, PC ? 2 : ISING_G2
             if (C == 1) publish(tt, jb, 1u, C, m);
         }
 
-    if (PC) {
+    if constexpr (PC) {
         __syncthreads();                                   // the consumer's job constants and the ring flags are in place
         if (wic > 0) {                                     // ---- producers: masks of the half-sweeps wic - 1, wic - 1 + 3, ...
             if (wg < R.jobs_total) {
