@@ -1059,7 +1059,8 @@ int launch_grid_one(GridArgs& R, bool use_jit, bool* fits, bool* used_jit, bool 
             static const bool strip_ok = !(getenv("ISING_G2_STRIP") && atoi(getenv("ISING_G2_STRIP")) == 0);
             const uint32_t jobs_per_row = (uint32_t)R.P.B / 2u / (uint32_t)(64 / T);
             // tile 32 only: at tile 64 (twice the state per lane, half the exchanges per site) the extra code spills and loses 4 %
-            const int strip = (strip_ok && T == 32 && M >= 2 && jobs_per_row % M == 0) ? (int)M : 0;
+            // (and a job of two 32 x 32 tiles must not straddle tile rows: the B / 2 tiles of a colour in a row must be an even number)
+            const int strip = (strip_ok && T == 32 && M >= 2 && ((uint32_t)R.P.B / 2u) % (uint32_t)(64 / T) == 0 && jobs_per_row % M == 0) ? (int)M : 0;
             fn = (const void*)grid_jit_kernel(T, BITS, HASJ, R.P.hp, R.P.B, R.P.R, wpb * 32, 1, park, R.acc != nullptr, strip);
             if (!fn) { shaped = false; M = 0; continue; }         // no run-time compiler: again with the pre-compiled kernel
             *used_jit = true;

@@ -213,7 +213,8 @@ def test_config3_full_length_int8_equals_bits(P, orc, tile, k):
 @pytest.mark.parametrize("L,tile,k,jobs,layout",
                          [(L, T, k, j, lay) for (L, T, k, j) in [(4096, 32, 1, 1), (4096, 64, 2, 1), (8192, 32, 1, 4), (8192, 32, 3, 4), (8192, 64, 1, 2), (8192, 64, 3, 2)]
                           for lay in ("int8", "bits")]
-                         + [(16384, 64, 1, 8, "int8"), (16384, 64, 2, 8, "bits"), (16384, 32, 1, 16, "int8"), (16384, 32, 3, 16, "int8")])
+                         + [(5184, 32, 1, 2, "int8"),      # 81 tiles of a colour per row: a job of two tiles may straddle rows (no strips)
+                            (16384, 64, 1, 8, "int8"), (16384, 64, 2, 8, "bits"), (16384, 32, 1, 16, "int8"), (16384, 32, 3, 16, "int8")])
 def test_on_chip_kernel_equals_a_launch_per_colour_at_full_size(P, L, tile, k, jobs, layout):
     """Lattices of 2^24, 2^26 and 2^28 sites (BASELINE config 3: all of the GPU's shared memory) in the launch configurations the
     library chooses for them (run-time build of k_grid_planes: `jobs` jobs of a colour per warp, from L = 8192 on without parked constants and, at tile 32, as strips): the whole

@@ -800,7 +800,8 @@ def test_grid_resident_kernel_run_time_build_without_parked_constants():
         "P.use_torch()\n"
         "for (L, T, k, n, seeds, bits, jseed, beta) in ((1024, 32, 1, 4, [5], False, None, 0.4406868), (768, 64, 2, 3, [6, 7], True, None, 0.44),\n"
         "                                              (640, 32, 1, 3, [8], False, 5, 1.0), (1024, 64, 1, 5, [9], False, None, 0.4406868),\n"
-        "                                              (1024, 32, 2, 3, [10, 11], True, None, 0.5)):\n"
+        "                                              (1024, 32, 2, 3, [10, 11], True, None, 0.5),\n"
+        "                                              (832, 32, 1, 3, [12], True, 5, 1.0)):\n"     # 13 tiles of a colour per row: jobs straddle rows, no strips
         "    J = W.couplings(2, L, jseed) if jseed is not None else None\n"
         "    g = P.Ising(2, L, coupling=J, seeds=seeds); o = O.Oracle(2, L, seeds=seeds, J=J)\n"
         "    g.set_jit('on')\n"
