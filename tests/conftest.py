@@ -12,6 +12,16 @@ def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box with -m gpu)")
 
 
+def pytest_collection_modifyitems(config, items):
+    """Every GPU test gets a time limit (pytest-timeout, if it is installed): the one-launch-per-call kernels wait for their
+    neighbours' data, and a kernel that waits for ever must fail its test, not hold the GPU box until somebody kills the job."""
+    if not config.pluginmanager.hasplugin("timeout"):
+        return
+    for item in items:
+        if "gpu" in item.keywords and item.get_closest_marker("timeout") is None:
+            item.add_marker(pytest.mark.timeout(1500, method="thread"))
+
+
 @pytest.fixture(scope="session")
 def orc():
     """The sequential CPU oracle (test infrastructure)."""
