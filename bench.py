@@ -575,7 +575,7 @@ def main() -> None:
     launch_ms = res["ms"] / (a.steps * launches_per_step)
     achieved = bytes_per_launch / (launch_ms * 1e6)            # GB/s
     lat_bytes = L * L if a.layout == "int8" else L * L // 8
-    on_chip = family == "grid"
+    on_chip = res["path"].startswith("grid_")          # k_grid_planes, and k_grid_plain for the plain / masked schemes
     hbm = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "peak_source": peak_src,
            "frac_of_8TBs_nominal": achieved / 8000.0, "algorithmic_bytes_per_flip": bpf}
     issue = ({"bound": "alu", "unit": "G warp-instr/s", "achieved": warp_instr / (launch_ms * 1e6),
